@@ -1,0 +1,191 @@
+/* optcc.h -- C ABI of liboptcc: planning, costing, executing and verifying OPTCC AllReduce schedules
+ * on one B200 (arxiv/paper_2606_01680, "Don't Let a Few Network Failures Slow the Entire AllReduce").
+ *
+ * Citations are PAPER.md:<line> (+ section / equation) and docs/PLAN_SPEC.md, which freezes the canonical
+ * plan tables.  p virtual ranks' buffers live in ONE GPU's HBM; every "flow" of the paper (a section moved
+ * between two ranks and either reduced into or copied over the destination) becomes a range
+ * reduce / copy between two rank buffers.  No torch types, no exceptions, no CPU fallback: every entry point
+ * returns an integer code; out-parameters are untouched on error.
+ *
+ * Pointer kinds are stated per argument: [host] = ordinary host memory, [device] = CUDA device memory of the
+ * current device, [pinned] = page-locked host memory.
+ */
+#ifndef OPTCC_H_
+#define OPTCC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define OPTCC_ABI_VERSION 1
+#if defined(__GNUC__)
+#define OPTCC_API __attribute__((visibility("default")))
+#else
+#define OPTCC_API
+#endif
+
+/* element types of the rank buffers */
+enum { OPTCC_F32 = 0, OPTCC_BF16 = 1 };
+
+/* return codes */
+enum {
+  OPTCC_OK = 0,
+  OPTCC_EINVAL = 1,       /* arguments violate PLAN_SPEC 1 (p<3 PAPER.md:68, g does not divide p, ell<1, ...) */
+  OPTCC_EUNSUPPORTED = 2, /* g>1 with m!=1 (PAPER.md:943 gives no construction); p>128 for masks */
+  OPTCC_ENOMEM = 3,
+  OPTCC_ECUDA = 4,        /* a CUDA runtime call failed; optcc_last_cuda_error() has the code */
+  OPTCC_EVERIFY = 5       /* contributor-mask verification found a wrong element */
+};
+
+/* PLAN_SPEC 3 enumerations */
+enum { OPTCC_OP_REDUCE = 0, OPTCC_OP_COPY = 1 };
+enum { OPTCC_S1 = 0, OPTCC_S2, OPTCC_S3, OPTCC_S4, OPTCC_BUB_UP, OPTCC_BUB_DOWN, OPTCC_N_COLLECT, OPTCC_N_DISTRIBUTE };
+enum { OPTCC_LINK_NIC = 0, OPTCC_LINK_NVLINK = 1 };
+/* constructions (PLAN_SPEC 4): C0 plain ring, C1 one straggler (4.1-4.2, App. C),
+ * C2 m>=2 stragglers (App. D), C3 g>1 with one straggler server (App. E) */
+enum { OPTCC_C0 = 0, OPTCC_C1 = 1, OPTCC_C2 = 2, OPTCC_C3 = 3 };
+/* executor modes */
+enum {
+  OPTCC_EXEC_PERSISTENT = 0, /* one cooperative kernel for the whole schedule, grid barrier between steps */
+  OPTCC_EXEC_PER_STEP = 1    /* one kernel launch per step (stream order is the step barrier) */
+};
+
+typedef struct optcc_plan optcc_plan_t; /* opaque; immutable after creation except for cached device state */
+
+/* One flow (PLAN_SPEC 3): 40 bytes, little endian, natural alignment.  off/len in ELEMENTS. */
+typedef struct optcc_flow {
+  uint64_t off;      /* first element of the range (same in src and dst: a flow never moves data along n) */
+  uint64_t len;      /* > 0 */
+  uint32_t step;     /* steps execute in order; flows of one step are independent (PLAN_SPEC 5.1) */
+  uint32_t seg;      /* segment b */
+  uint32_t sec;      /* section c of the segment; 0 for bubble flows */
+  uint16_t src;      /* sending rank */
+  uint16_t dst;      /* receiving rank */
+  uint8_t  op;       /* OPTCC_OP_* */
+  uint8_t  stage;    /* OPTCC_S1.. */
+  uint8_t  link;     /* OPTCC_LINK_* (cost model only) */
+  uint8_t  part;     /* lambda, the leading-GPU index for g>1 */
+  uint32_t reserved; /* 0 */
+} optcc_flow_t;
+
+typedef struct optcc_opts {
+  uint32_t k;         /* segments; 0 = auto (PLAN_SPEC 2 "k"); else a multiple of 4 */
+  uint32_t exec_mode; /* OPTCC_EXEC_* */
+  uint32_t grid_ctas; /* 0 = auto (SM count x resident CTAs per SM); else CTAs of the executor grid */
+  uint32_t copy_path; /* 0 = auto, 1 = LDG/STG vector copy, 2 = cp.async.bulk (TMA 1-D) copy */
+} optcc_opts_t;
+
+typedef struct optcc_plan_info {
+  uint32_t p, g, q, m, H, k;   /* ranks, GPUs/server, servers, straggler servers, healthy servers, segments */
+  uint32_t construction;       /* OPTCC_C* */
+  uint32_t dtype;              /* OPTCC_F32 | OPTCC_BF16 */
+  uint32_t unit_elems;         /* A = 16/sizeof(dtype) (PLAN_SPEC 2) */
+  uint32_t mask_words;         /* 64-bit words per contributor mask: 1 (p<=64) or 2 (p<=128); 0 if p>128 */
+  uint64_t n, n_ring, n_p2p;   /* elements per rank; on the ring path; on the P2P (bubble) path */
+  uint64_t U, U_ring, U_p2p;   /* the same in 16-byte units */
+  uint32_t n_steps;
+  uint32_t n_flows;
+  uint32_t max_flows_per_step;
+  uint32_t n_sec_bounds;       /* entries of sec_bounds */
+  uint32_t n_p2p_bounds;       /* entries of p2p_bounds (0 if no P2P path) */
+  uint32_t reserved;
+  uint64_t reduce_elems;       /* sum of len over reduce flows  = (p-1) n  (Lemma 4) */
+  uint64_t copy_elems;         /* sum of len over copy flows    = (p-1) n */
+  uint64_t workspace_bytes;    /* device workspace optcc_execute needs (tables, barrier, bf16 fp32 partials) */
+  uint64_t verify_workspace_bytes; /* device workspace optcc_verify needs (>= workspace_bytes) */
+  uint64_t mask_offset_bytes;  /* after optcc_verify: masks of (rank r, element e, word w) at
+                                  workspace + mask_offset_bytes + ((r*padded_n + e)*mask_words + w)*8 */
+  uint64_t padded_n;           /* n rounded up to a multiple of 8: per-rank stride of masks and fp32 partials */
+  double   plan_build_seconds; /* wall time optcc_plan spent ("< 1 ms at p=1024") */
+} optcc_plan_info_t;
+
+typedef struct optcc_cost_params {
+  double alpha; /* fixed cost per flow (PAPER.md:68 excludes it: default 0; :201 reports a 14% fixed share) */
+  double beta;  /* time per element on a healthy NIC (default 1) */
+} optcc_cost_params_t;
+
+typedef struct optcc_cost {
+  double T;             /* completion time of the plan under the port model (PLAN_SPEC 6) */
+  double T0;            /* 2(p-1)n/(g p), fault-free optimum */
+  double T_over_T0;
+  double T_closed_form; /* the paper's finite-k form: Eq.(1) :173 / Eq.(2) :185 (exact for C1); (k+4)T_body :809
+                           and Eq.(21)/(22) :920-926 (upper bounds for C2 / C3); T0 for C0 */
+  double T_limit;       /* its k -> infinity limit (:173, :185, :831, :920) */
+  double lb_table1;     /* Theorem 1 (:76) / 2 (:82) / 3 (:112): the Table-1 lower bound */
+  double lb_tight;      /* Theorem 6 (:413) / 13 (:664); NaN for m>1 (Remark 9, :519) */
+  double T0_server;     /* 2(q-1)n/(q g): the base the Theorem-3 series are relative to */
+  double bodies;        /* T / (body duration): the "(k+c)" of the finite-k factor */
+  double straggler_sent;/* NIC elements sent by the slowest straggler's first GPU (z* n at the optimum, :455) */
+  double straggler_recv;
+  int32_t lb_table1_thm;/* 1, 2 or 3; 0 for no straggler */
+  int32_t lb_tight_thm; /* 6 or 13; 0 if none */
+  int32_t regime;       /* 0 no straggler, 1 ring-bound (ell<2 resp. first max-term), 2 straggler-bound */
+  int32_t reserved;
+} optcc_cost_t;
+
+typedef struct optcc_verify_result {
+  uint64_t bad_elements;   /* (rank, element) pairs whose final mask is not "every rank exactly once" */
+  uint64_t overlap_elements; /* (flow, element) pairs where a reduce joined overlapping contributor sets */
+  uint64_t first_bad;      /* smallest r*n+e that is bad; UINT64_MAX if none */
+  uint64_t checked;        /* p*n */
+} optcc_verify_result_t;
+
+/* ---- planning (host only; needs no GPU) ------------------------------------------------------------------ */
+
+/* Build the ell-weighted stage/chunk/step plan of PAPER.md 3 (problem statement :68) and 4.1-4.4 as frozen
+ * in docs/PLAN_SPEC.md.  ell [host, p doubles]: slowdown factor of every rank, >= 1; ranks of one server
+ * (floor(i/g)) must share ell (PXN pooling, :274, :850).  n: elements per rank.  *out receives a new plan
+ * owned by the library (optcc_plan_destroy).  Same as optcc_plan_ex with opts = NULL (k auto). */
+OPTCC_API int optcc_plan(int p, int g, const double* ell, uint64_t n, int dtype, optcc_plan_t** out);
+OPTCC_API int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dtype, const optcc_opts_t* opts,
+                  optcc_plan_t** out);
+/* Frees the plan's host tables.  Device state cached in a caller workspace is simply forgotten. NULL is ok. */
+OPTCC_API void optcc_plan_destroy(optcc_plan_t* plan);
+OPTCC_API int optcc_plan_info(const optcc_plan_t* plan, optcc_plan_info_t* out);
+/* Borrowed [host] pointers, valid until optcc_plan_destroy.  Any out-pointer may be NULL.
+ * flows[n_flows] sorted by (step, link, stage, src, dst, off); step_begin[n_steps+1] CSR index into it;
+ * sec_bounds / p2p_bounds: section and P2P-piece boundaries in elements (PLAN_SPEC 2). */
+OPTCC_API int optcc_plan_tables(const optcc_plan_t* plan, const optcc_flow_t** flows, const uint32_t** step_begin,
+                      const uint64_t** sec_bounds, const uint64_t** p2p_bounds);
+
+/* ---- alpha-beta cost model (host only) --------------------------------------------------------------------
+ * Event-simulates the plan under the paper's port model (one send + one receive port per NIC, PAPER.md:124,
+ * :134; ell time units per element on straggler-incident flows, :68, :356; NVLink at (g-1)x, :847, :908) and
+ * reports T/T0 beside the lower bounds of Table 1 (:17-26).  params NULL = {alpha 0, beta 1}. */
+OPTCC_API int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* params, optcc_cost_t* out);
+
+/* ---- execution (current CUDA device) -----------------------------------------------------------------------
+ * optcc_execute: in-place AllReduce.  bufs [host array of p DEVICE pointers], each n elements of the plan's
+ * dtype, 16-byte aligned, pairwise disjoint.  On entry bufs[i] holds x_i; when the stream reaches the end of
+ * the enqueued work every bufs[i] holds sum_j x_j and all p outputs are bitwise identical (PAPER.md:68 (ii)).
+ * The reduce-scatter and all-gather steps are carried out exactly as the plan lists them, step by step.
+ * workspace [device, >= workspace_bytes, 256-byte aligned] owned by the caller; the first call with a given
+ * workspace uploads the tables into it (optcc_prepare does this ahead of time).  stream: a cudaStream_t
+ * (NULL = default stream).  Asynchronous: never synchronises the device or the stream.
+ * Errors: EINVAL (NULL / misaligned pointers), ECUDA. */
+OPTCC_API int optcc_prepare(optcc_plan_t* plan, void* workspace, void* stream);
+OPTCC_API int optcc_execute(optcc_plan_t* plan, void* const* bufs, void* workspace, void* stream);
+/* End-to-end variant: host_in [host array of p PINNED host pointers] are copied to bufs (device, as above),
+ * the plan is executed, and every result is copied to host_out[i] (pinned; may equal host_in[i]).  All on
+ * `stream`, asynchronous. */
+OPTCC_API int optcc_execute_host(optcc_plan_t* plan, const void* const* host_in, void* const* host_out,
+                       void* const* bufs, void* workspace, void* stream);
+
+/* ---- verification --------------------------------------------------------------------------------------------
+ * Runs the SAME step tables through the executor with contributor bitmasks as elements (rank r starts as
+ * {r}; reduce = disjoint OR, copy = assign) and checks that every rank's every element ends as "all p ranks,
+ * each once" (PAPER.md:68 correctness (ii)).  workspace [device, >= verify_workspace_bytes].  Synchronises
+ * `stream` once to read the counters.  Returns OPTCC_EVERIFY if any element is wrong (out is still filled).
+ * The masks stay in the workspace at mask_offset_bytes (see optcc_plan_info_t). */
+OPTCC_API int optcc_verify(optcc_plan_t* plan, void* workspace, void* stream, optcc_verify_result_t* out);
+
+OPTCC_API const char* optcc_strerror(int code);
+OPTCC_API int optcc_last_cuda_error(void);   /* cudaError_t of the last failing CUDA call on this thread, 0 if none */
+OPTCC_API int optcc_abi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OPTCC_H_ */

@@ -1,0 +1,122 @@
+// alpha-beta cost model of liboptcc: modeled completion time T/T0 of a plan next to the paper's lower bounds.
+//
+// Event simulation under the paper's port model, as frozen in docs/PLAN_SPEC.md 6:
+//   * a healthy NIC moves one element per time unit, a straggler's NIC needs ell;
+//   * a NIC handles one incoming flow at a time (:124) and is full duplex: one send + one receive (:134);
+//   * a transfer incident to a straggler costs ell per element (:356, :432);
+//   * an NVLink lane runs at (g-1)x NIC speed per GPU and direction (:847-848, :908).
+// Closed forms: T0 (:70-72), Theorems 1/2/3 (:76, :82, :112) = Table 1 (:17-26), Theorems 6/13 (:413, :664),
+// Eq.(1) :173, Eq.(2) :185, D.3 :805-831, Eq.(21)/(22) :920-926.  Host only, double precision.
+#include <algorithm>
+#include <cmath>
+#include <limits>
+
+#include "optcc_internal.h"
+
+extern "C" int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* params, optcc_cost_t* out) {
+  if (!plan || !out) return OPTCC_EINVAL;
+  const optcc_plan_info_t& in = plan->info;
+  const double alpha = params ? params->alpha : 0.0, beta = params ? params->beta : 1.0;
+  if (!(alpha >= 0.0) || !(beta > 0.0) || !std::isfinite(alpha) || !std::isfinite(beta)) return OPTCC_EINVAL;
+  const uint32_t p = in.p, g = in.g, q = in.q, m = in.m, k = in.k;
+  const double n = double(in.n);
+
+  // ---- event simulation (PLAN_SPEC 6) ----
+  std::vector<uint64_t> offs;
+  offs.reserve(plan->flows.size());
+  for (const auto& f : plan->flows) offs.push_back(f.off);
+  std::sort(offs.begin(), offs.end());
+  offs.erase(std::unique(offs.begin(), offs.end()), offs.end());
+  const size_t nr = offs.size();
+  std::vector<double> wfin, rfin, send_free, recv_free;
+  try {
+    wfin.assign(size_t(p) * nr, 0.0);
+    rfin.assign(size_t(p) * nr, 0.0);
+    send_free.assign(size_t(p) * 2, 0.0);
+    recv_free.assign(size_t(p) * 2, 0.0);
+  } catch (const std::bad_alloc&) {
+    return OPTCC_ENOMEM;
+  }
+  double T = 0.0;
+  const uint32_t r_str = m ? plan->stragglers[0] * g : 0;
+  double sent = 0.0, recvd = 0.0;
+  for (const auto& f : plan->flows) {
+    size_t reg = size_t(std::lower_bound(offs.begin(), offs.end(), f.off) - offs.begin());
+    double dur;
+    if (f.link == OPTCC_LINK_NIC)
+      dur = alpha + beta * double(f.len) * std::max(plan->ell[f.src], plan->ell[f.dst]);
+    else
+      dur = alpha + beta * double(f.len) / double(g - 1);
+    double& sf = send_free[size_t(f.src) * 2 + f.link];
+    double& rf = recv_free[size_t(f.dst) * 2 + f.link];
+    double& ws = wfin[size_t(f.src) * nr + reg];
+    double& wd = wfin[size_t(f.dst) * nr + reg];
+    double& rd = rfin[size_t(f.dst) * nr + reg];
+    double& rs = rfin[size_t(f.src) * nr + reg];
+    double start = std::max(std::max(sf, rf), std::max(ws, std::max(wd, rd)));
+    double fin = start + dur;
+    sf = fin;
+    rf = fin;
+    rs = std::max(rs, fin);
+    wd = fin;
+    T = std::max(T, fin);
+    if (m && f.link == OPTCC_LINK_NIC) {
+      if (f.src == r_str) sent += double(f.len);
+      if (f.dst == r_str) recvd += double(f.len);
+    }
+  }
+
+  // ---- closed forms ----
+  optcc_cost_t c;
+  c.T = T;
+  c.T0 = beta * 2.0 * double(p - 1) * n / (double(g) * double(p));                 // :70-72 (R6: the printed q is g)
+  c.T0_server = beta * 2.0 * double(q - 1) * n / (double(q) * double(g));          // base of Thm 3's series (:112, R6)
+  c.T_over_T0 = T / c.T0;
+  c.straggler_sent = sent;
+  c.straggler_recv = recvd;
+  c.reserved = 0;
+  const double nan = std::numeric_limits<double>::quiet_NaN();
+  if (m == 0) {
+    c.lb_table1 = c.lb_tight = c.T_closed_form = c.T_limit = c.T0;
+    c.lb_table1_thm = 0; c.lb_tight_thm = 0; c.regime = 0;
+  } else {
+    const double l1 = plan->ell[r_str];
+    if (in.construction == OPTCC_C3) {
+      const double Q = double(q);
+      c.lb_table1 = beta * (n / g) * std::max(2.0 * l1 * (Q - 1.0) / (1.0 + l1 * (Q - 1.0)), l1);   // Thm 3 (:112, :538)
+      c.lb_tight = beta * (n / g) * std::max(2.0 * l1 * (Q - 1.0) / (l1 * (Q - 2.0) + 2.0), l1);     // Thm 13 (:664)
+      c.lb_table1_thm = 3; c.lb_tight_thm = 13;
+      c.T_limit = beta * std::max(l1, 2.0) * n / g;                                                  // Eq.(21)/(22) limits
+      c.T_closed_form = c.T_limit * (double(k) + 5.5) / double(k);                                   // <= (k+5.5) bodies (:916-926)
+      c.regime = l1 >= 2.0 ? 2 : 1;
+    } else if (m == 1) {
+      const double P = double(p);
+      c.lb_table1 = beta * std::max(2.0 * l1 * (P - 1.0) / (l1 * (P - 1.0) + 1.0), l1) * n;          // Thm 1 (:76)
+      c.lb_tight = beta * std::max(2.0 * l1 * (P - 1.0) / (l1 * (P - 2.0) + 2.0), l1) * n;           // Thm 6 (:413)
+      c.lb_table1_thm = 1; c.lb_tight_thm = 6;
+      if (l1 < 2.0) {  // Eq.(2) (:185, :752): 2(p-1) l n / ((p-2) l + 2) * (k + l - 1)/k
+        c.T_limit = beta * 2.0 * (P - 1.0) * l1 * n / ((P - 2.0) * l1 + 2.0);
+        c.T_closed_form = c.T_limit * (double(k) + l1 - 1.0) / double(k);
+        c.regime = 1;
+      } else {         // Eq.(1) (:173): l n (k+1)/k
+        c.T_limit = beta * l1 * n;
+        c.T_closed_form = c.T_limit * (double(k) + 1.0) / double(k);
+        c.regime = 2;
+      }
+    } else {
+      double inv = 0.0;
+      for (uint32_t v : plan->stragglers) inv += 1.0 / plan->ell[v * g];
+      const double P = double(p), M = double(m);
+      c.lb_table1 = beta * std::max(2.0 * (P - 1.0) / (P - M + inv), l1) * n;                        // Thm 2 (:82)
+      c.lb_tight = nan;                                                                               // Remark 9 (:519)
+      c.lb_table1_thm = 2; c.lb_tight_thm = 0;
+      const double ring_body = 2.0 * (P - 1.0), str_body = l1 * (P - M) + 2.0 * (M - 1.0);            // D.3 (:805), x s
+      c.T_limit = beta * std::max(ring_body, str_body) / (P - M) * n;                                 // (:831)
+      c.T_closed_form = c.T_limit * (double(k) + 4.0) / double(k);                                    // (k+4) T_body (:809)
+      c.regime = str_body > ring_body ? 2 : 1;
+    }
+  }
+  c.bodies = T * double(k) / c.T_limit;
+  *out = c;
+  return OPTCC_OK;
+}

@@ -1,0 +1,474 @@
+// Executor and verifier of liboptcc (sm_100a): carries out an OPTCC plan step by step over p virtual ranks'
+// buffers held in one GPU's HBM.  Reduce flows (Stage 1 hops PAPER.md:126, Stage 3 fold-in :132, bubble-up :165,
+// NVLink collect :862-875) are range additions dst[R] += src[R]; copy flows (Stage 4 :136, Stage 2 :130,
+// bubble-down :165, NVLink distribute :863-876) are range copies.  Flows of step t+1 see all writes of steps
+// <= t (:138 data dependencies).  No tensor cores: nothing here is a dense contraction.
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "optcc_internal.h"
+#include "optcc_kernels.cuh"
+
+using namespace optcc_dev;
+
+static_assert(sizeof(DFlow) == OPTCC_DFLOW_BYTES, "layout constant out of date");
+static_assert(sizeof(Slice) == OPTCC_SLICE_BYTES, "layout constant out of date");
+static_assert(sizeof(Ctrl) <= OPTCC_CTRL_BYTES, "control block too large");
+
+namespace {
+
+thread_local int g_last_cuda_error = 0;
+
+#define CU_TRY(call)                          \
+  do {                                        \
+    cudaError_t e_ = (call);                  \
+    if (e_ != cudaSuccess) {                  \
+      g_last_cuda_error = (int)e_;            \
+      (void)cudaGetLastError();               \
+      return OPTCC_ECUDA;                     \
+    }                                         \
+  } while (0)
+
+template <int MODE> struct ModeTraits;
+template <> struct ModeTraits<MODE_F32>   { static constexpr int ESIZE = 4,  VE = 4; };
+template <> struct ModeTraits<MODE_BF16>  { static constexpr int ESIZE = 2,  VE = 8; };
+template <> struct ModeTraits<MODE_MASK1> { static constexpr int ESIZE = 8,  VE = 2; };
+template <> struct ModeTraits<MODE_MASK2> { static constexpr int ESIZE = 16, VE = 1; };
+
+__device__ __forceinline__ char* rank_ptr(const ExecParams& P, unsigned int r) {
+  return reinterpret_cast<char*>(P.ptr_table ? P.ptr_table[r] : P.bufs[r]);
+}
+
+// One piece of one flow: 16-byte units [ubeg, uend) of the flow, executed by the whole CTA.
+template <int MODE>
+__device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& f, unsigned long long ubeg,
+                                              unsigned long long uend, unsigned int& overlaps) {
+  using MT = ModeTraits<MODE>;
+  const unsigned long long A = P.unit_elems;
+  const unsigned long long e0 = ubeg * A;
+  unsigned long long e1 = uend * A;
+  if (e1 > f.len) e1 = f.len;
+  if (e0 >= e1) return;
+  const unsigned long long vbeg = e0 / MT::VE, vend = e1 / MT::VE;  // full 16-byte vectors
+  const unsigned int tail = (unsigned int)(e1 % MT::VE);            // ragged end of the buffer (n not a multiple of A)
+
+  if (MODE == MODE_F32) {
+    const char* s = rank_ptr(P, f.src) + f.off * 4;
+    char* d = rank_ptr(P, f.dst) + f.off * 4;
+    if (f.op == 0) range_add_f32<4>(s, d, vbeg, vend); else range_copy16<4>(s, d, vbeg, vend);
+    if (threadIdx.x < tail) {
+      unsigned long long e = vend * 4 + threadIdx.x;
+      const float* sf = reinterpret_cast<const float*>(s);
+      float* df = reinterpret_cast<float*>(d);
+      float x = __ldcg(sf + e);
+      if (f.op == 0) x = __fadd_rn(__ldcg(df + e), x);
+      __stcg(df + e, x);
+    }
+  } else if (MODE == MODE_MASK1 || MODE == MODE_MASK2) {
+    constexpr int W = MODE == MODE_MASK1 ? 1 : 2;
+    const char* s = rank_ptr(P, f.src) + f.off * (8 * W);
+    char* d = rank_ptr(P, f.dst) + f.off * (8 * W);
+    if (f.op == 0) range_or_mask<4, W>(s, d, vbeg, vend, overlaps); else range_copy16<4>(s, d, vbeg, vend);
+    if (threadIdx.x < tail) {  // MASK1 only: one odd element
+      unsigned long long e = vend * 2;
+      const unsigned long long* sm = reinterpret_cast<const unsigned long long*>(s);
+      unsigned long long* dm = reinterpret_cast<unsigned long long*>(d);
+      unsigned long long x = __ldcg(sm + e);
+      if (f.op == 0) {
+        unsigned long long y = __ldcg(dm + e);
+        overlaps += (x & y) != 0ull;
+        x |= y;
+      }
+      __stcg(dm + e, x);
+    }
+  } else {  // MODE_BF16
+    const char* s = f.ksrc ? reinterpret_cast<const char*>(P.shadow + (unsigned long long)f.src * P.padded_n + f.off)
+                           : rank_ptr(P, f.src) + f.off * 2;
+    const char* di = f.kdin ? reinterpret_cast<const char*>(P.shadow + (unsigned long long)f.dst * P.padded_n + f.off)
+                            : rank_ptr(P, f.dst) + f.off * 2;
+    char* dout = f.kdout ? reinterpret_cast<char*>(P.shadow + (unsigned long long)f.dst * P.padded_n + f.off)
+                         : rank_ptr(P, f.dst) + f.off * 2;
+    if (f.op == 0) {
+      switch ((f.ksrc << 2) | (f.kdin << 1) | f.kdout) {
+        case 0: range_add_bf16<0, 0, 0>(s, di, dout, vbeg, vend); break;
+        case 1: range_add_bf16<0, 0, 1>(s, di, dout, vbeg, vend); break;
+        case 2: range_add_bf16<0, 1, 0>(s, di, dout, vbeg, vend); break;
+        case 3: range_add_bf16<0, 1, 1>(s, di, dout, vbeg, vend); break;
+        case 4: range_add_bf16<1, 0, 0>(s, di, dout, vbeg, vend); break;
+        case 5: range_add_bf16<1, 0, 1>(s, di, dout, vbeg, vend); break;
+        case 6: range_add_bf16<1, 1, 0>(s, di, dout, vbeg, vend); break;
+        default: range_add_bf16<1, 1, 1>(s, di, dout, vbeg, vend); break;
+      }
+    } else if (f.ksrc == 0) {
+      range_copy16<4>(s, dout, vbeg, vend);                 // bf16 -> bf16: one vector per unit
+    } else {
+      range_copy16<4>(s, dout, vbeg * 2, vend * 2);         // fp32 partial -> fp32 partial: two vectors per unit
+    }
+    if (threadIdx.x < tail) {
+      unsigned long long e = vend * 8 + threadIdx.x;
+      float x = f.ksrc ? __ldcg(reinterpret_cast<const float*>(s) + e)
+                       : bf16_to_f32(__ldcg(reinterpret_cast<const unsigned short*>(s) + e));
+      if (f.op == 0) {
+        float y = f.kdin ? __ldcg(reinterpret_cast<const float*>(di) + e)
+                         : bf16_to_f32(__ldcg(reinterpret_cast<const unsigned short*>(di) + e));
+        x = __fadd_rn(y, x);
+      }
+      if (f.kdout) __stcg(reinterpret_cast<float*>(dout) + e, x);
+      else __stcg(reinterpret_cast<unsigned short*>(dout) + e, (unsigned short)f32_to_bf16_rne(x));
+    }
+  }
+}
+
+// The executor kernel.  gridDim.x CTAs; CTA c executes slice c of every step in [step_lo, step_hi).
+template <int MODE>
+__global__ void __launch_bounds__(THREADS, CTAS_PER_SM) optcc_exec_kernel(const __grid_constant__ ExecParams P) {
+  __shared__ DFlow s_flow[2][STAGE];             // the CTA's part of the step table, staged one step ahead
+  __shared__ unsigned long long s_ubeg[2], s_uend[2];
+  __shared__ unsigned int s_f0[2], s_nf[2];
+
+  const unsigned int G = gridDim.x, cta = blockIdx.x;
+  unsigned int overlaps = 0;
+
+  auto stage = [&](unsigned int step, int buf, unsigned int lane) {
+    // called by one warp: fetch the slice bounds and up to STAGE flow records of `step`
+    const Slice* sl = P.slices + (unsigned long long)step * (G + 1) + cta;
+    const uint4 ra = __ldg(reinterpret_cast<const uint4*>(sl)), rb = __ldg(reinterpret_cast<const uint4*>(sl + 1));
+    const unsigned int a_flow = ra.x, b_flow = rb.x;
+    const unsigned long long a_unit = ra.z | ((unsigned long long)ra.w << 32), b_unit = rb.z | ((unsigned long long)rb.w << 32);
+    unsigned int nf = b_flow - a_flow + (b_unit > 0 ? 1u : 0u);
+    if (lane == 0) { s_f0[buf] = a_flow; s_nf[buf] = nf; s_ubeg[buf] = a_unit; s_uend[buf] = b_unit; }
+    if (lane < nf && lane < STAGE) {
+      const uint4* src = reinterpret_cast<const uint4*>(P.flows + a_flow + lane);
+      uint4* dst = reinterpret_cast<uint4*>(&s_flow[buf][lane]);
+      dst[0] = __ldg(src);
+      dst[1] = __ldg(src + 1);
+    }
+  };
+
+  if (threadIdx.x < 32) stage(P.step_lo, P.step_lo & 1, threadIdx.x);
+  __syncthreads();
+
+  for (unsigned int step = P.step_lo; step < P.step_hi; ++step) {
+    const int buf = step & 1;
+    if (step + 1 < P.step_hi && threadIdx.x >= THREADS - 32) stage(step + 1, buf ^ 1, threadIdx.x - (THREADS - 32));
+    const unsigned int f0 = s_f0[buf], nf = s_nf[buf];
+    const unsigned long long ub = s_ubeg[buf], ue = s_uend[buf];
+    for (unsigned int i = 0; i < nf; ++i) {
+      DFlow f;
+      if (i < STAGE) {
+        f = s_flow[buf][i];
+      } else {  // more flows in one slice than staged: read the record from the table directly
+        const uint4* src = reinterpret_cast<const uint4*>(P.flows + f0 + i);
+        uint4 lo = __ldg(src), hi = __ldg(src + 1);
+        memcpy(&f, &lo, 16);
+        memcpy(reinterpret_cast<char*>(&f) + 16, &hi, 16);
+      }
+      const unsigned long long A = P.unit_elems;
+      const unsigned long long nunits = (f.len + A - 1) / A;
+      const unsigned long long ubeg = i == 0 ? ub : 0ull;
+      const unsigned long long uend = (i + 1 == nf && ue > 0) ? ue : nunits;
+      process_piece<MODE>(P, f, ubeg, uend, overlaps);
+    }
+    if (step + 1 < P.step_hi) {
+      if (P.use_barrier) grid_barrier(&P.ctrl->barrier, (unsigned long long)(step - P.step_lo + 1) * G);
+      else __syncthreads();
+    }
+  }
+
+  if (MODE == MODE_MASK1 || MODE == MODE_MASK2) {
+    // warp-shuffle reduction of the per-thread overlap counts, one atomic per warp
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) overlaps += __shfl_xor_sync(0xFFFFFFFFu, overlaps, o);
+    if ((threadIdx.x & 31) == 0 && overlaps) atomicAdd(&P.ctrl->overlap, (unsigned long long)overlaps);
+  }
+}
+
+// masks[r][e][w] = {r}
+__global__ void __launch_bounds__(256) optcc_mask_init_kernel(unsigned long long* masks, unsigned int p,
+                                                              unsigned long long n, unsigned long long padded_n,
+                                                              unsigned int W) {
+  const unsigned long long total = (unsigned long long)p * n;
+  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < total;
+       i += (unsigned long long)gridDim.x * blockDim.x) {
+    unsigned int r = (unsigned int)(i / n);
+    unsigned long long e = i - (unsigned long long)r * n;
+    unsigned long long* m = masks + ((unsigned long long)r * padded_n + e) * W;
+    if (W == 1) {
+      m[0] = 1ull << r;
+    } else {
+      m[0] = r < 64 ? 1ull << r : 0ull;
+      m[1] = r >= 64 ? 1ull << (r - 64) : 0ull;
+    }
+  }
+}
+
+// every (rank, element) must hold every rank exactly once: mask == all p bits (PAPER.md:68 (ii))
+__global__ void __launch_bounds__(256) optcc_mask_check_kernel(const unsigned long long* masks, unsigned int p,
+                                                               unsigned long long n, unsigned long long padded_n,
+                                                               unsigned int W, Ctrl* ctrl) {
+  const unsigned long long total = (unsigned long long)p * n;
+  const unsigned long long full0 = p >= 64 ? ~0ull : ((1ull << p) - 1ull);
+  const unsigned long long full1 = p > 64 ? (p >= 128 ? ~0ull : ((1ull << (p - 64)) - 1ull)) : 0ull;
+  unsigned long long bad = 0, first = ~0ull;
+  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < total;
+       i += (unsigned long long)gridDim.x * blockDim.x) {
+    unsigned int r = (unsigned int)(i / n);
+    unsigned long long e = i - (unsigned long long)r * n;
+    const unsigned long long* m = masks + ((unsigned long long)r * padded_n + e) * W;
+    bool ok = __ldcg(m) == full0 && (W == 1 || __ldcg(m + 1) == full1);
+    if (!ok) { ++bad; first = first < i ? first : i; }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    bad += __shfl_xor_sync(0xFFFFFFFFu, bad, o);
+    unsigned long long other = __shfl_xor_sync(0xFFFFFFFFu, first, o);
+    first = first < other ? first : other;
+  }
+  if ((threadIdx.x & 31) == 0 && bad) {
+    atomicAdd(&ctrl->bad, bad);
+    atomicMin(&ctrl->first_bad, first);
+  }
+}
+
+}  // namespace
+
+// =====================================================================================================
+// Host side
+// =====================================================================================================
+
+struct optcc_exec_state {
+  int device = -1;
+  int sm_count = 0;
+  int coop = 0;
+  uint32_t G = 0;                 // executor grid (CTAs)
+  void* prepared_ws = nullptr;    // workspace that currently holds the device tables
+  std::vector<DFlow> dflows;
+  std::vector<Slice> slices;      // [n_steps][G + 1]
+};
+
+void optcc_exec_state_free(optcc_exec_state* s) { delete s; }
+
+namespace {
+
+template <int MODE>
+int kernel_occupancy(int* out) {
+  CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, optcc_exec_kernel<MODE>, THREADS, 0));
+  return OPTCC_OK;
+}
+
+// bytes one 16-byte unit of a flow moves through HBM (what the slices are balanced on)
+inline uint64_t unit_cost(const optcc_plan_t* pl, size_t i) {
+  const optcc_flow_t& f = pl->flows[i];
+  auto sz = [](uint8_t kind) -> uint64_t { return kind == OPTCC_KIND_F32 ? 32 : 16; };
+  uint64_t c = sz(pl->kind_src[i]) + sz(pl->kind_dst_out[i]);
+  if (f.op == OPTCC_OP_REDUCE) c += sz(pl->kind_dst_in[i]);
+  return c;
+}
+
+int build_state(optcc_plan_t* pl) {
+  optcc_exec_state* st = pl->exec;
+  if (!st) {
+    st = new (std::nothrow) optcc_exec_state();
+    if (!st) return OPTCC_ENOMEM;
+    pl->exec = st;
+  }
+  int dev = 0;
+  CU_TRY(cudaGetDevice(&dev));
+  if (st->device == dev && st->G != 0) return OPTCC_OK;
+  st->prepared_ws = nullptr;
+  st->device = dev;
+  CU_TRY(cudaDeviceGetAttribute(&st->sm_count, cudaDevAttrMultiProcessorCount, dev));
+  CU_TRY(cudaDeviceGetAttribute(&st->coop, cudaDevAttrCooperativeLaunch, dev));
+  int occ = 0, o = 0, rc;
+  if ((rc = kernel_occupancy<MODE_F32>(&o)) != OPTCC_OK) return rc;
+  occ = o;
+  if ((rc = kernel_occupancy<MODE_BF16>(&o)) != OPTCC_OK) return rc;
+  occ = std::min(occ, o);
+  if ((rc = kernel_occupancy<MODE_MASK1>(&o)) != OPTCC_OK) return rc;
+  occ = std::min(occ, o);
+  if ((rc = kernel_occupancy<MODE_MASK2>(&o)) != OPTCC_OK) return rc;
+  occ = std::min(occ, o);
+  if (occ < 1) { g_last_cuda_error = (int)cudaErrorLaunchOutOfResources; return OPTCC_ECUDA; }
+  occ = std::min(occ, CTAS_PER_SM);
+  uint32_t maxG = std::min<uint32_t>(uint32_t(st->sm_count) * uint32_t(occ), OPTCC_MAX_GRID);
+  uint32_t G = pl->opts.grid_ctas ? std::min(pl->opts.grid_ctas, maxG) : maxG;
+  st->G = G;
+
+  const optcc_plan_info_t& in = pl->info;
+  const uint64_t A = in.unit_elems;
+  try {
+    st->dflows.resize(in.n_flows);
+    for (size_t i = 0; i < in.n_flows; ++i) {
+      const optcc_flow_t& f = pl->flows[i];
+      DFlow d;
+      std::memset(&d, 0, sizeof d);
+      d.off = f.off; d.len = f.len; d.src = f.src; d.dst = f.dst; d.op = f.op;
+      d.ksrc = pl->kind_src[i]; d.kdin = pl->kind_dst_in[i]; d.kdout = pl->kind_dst_out[i];
+      st->dflows[i] = d;
+    }
+    // slice table: cut every step into G slices of equal HBM bytes
+    st->slices.assign(size_t(in.n_steps) * (G + 1), Slice{0, 0, 0});
+    for (uint32_t t = 0; t < in.n_steps; ++t) {
+      const uint32_t lo = pl->step_begin[t], hi = pl->step_begin[t + 1];
+      uint64_t Wtot = 0;
+      for (uint32_t i = lo; i < hi; ++i) Wtot += ((pl->flows[i].len + A - 1) / A) * unit_cost(pl, i);
+      Slice* row = st->slices.data() + size_t(t) * (G + 1);
+      uint32_t i = lo;
+      uint64_t prefix = 0;  // cost of flows [lo, i)
+      for (uint32_t c = 0; c <= G; ++c) {
+        const uint64_t Bc = (unsigned __int128)Wtot * c / G;
+        while (i < hi) {
+          uint64_t w = ((pl->flows[i].len + A - 1) / A) * unit_cost(pl, i);
+          if (prefix + w > Bc) break;
+          prefix += w;
+          ++i;
+        }
+        row[c].flow = i;
+        row[c].pad = 0;
+        row[c].unit = i < hi ? (Bc - prefix) / unit_cost(pl, i) : 0;
+      }
+    }
+  } catch (const std::bad_alloc&) {
+    return OPTCC_ENOMEM;
+  }
+  return OPTCC_OK;
+}
+
+int upload_tables(optcc_plan_t* pl, void* workspace, cudaStream_t stream) {
+  optcc_exec_state* st = pl->exec;
+  if (st->prepared_ws == workspace) return OPTCC_OK;
+  const optcc_ws_layout L = optcc_layout(pl->info);
+  char* ws = static_cast<char*>(workspace);
+  CU_TRY(cudaMemsetAsync(ws + L.ctrl, 0, OPTCC_CTRL_BYTES, stream));
+  if (!st->dflows.empty())
+    CU_TRY(cudaMemcpyAsync(ws + L.dflows, st->dflows.data(), st->dflows.size() * sizeof(DFlow), cudaMemcpyHostToDevice, stream));
+  if (!st->slices.empty())
+    CU_TRY(cudaMemcpyAsync(ws + L.slices, st->slices.data(), st->slices.size() * sizeof(Slice), cudaMemcpyHostToDevice, stream));
+  st->prepared_ws = workspace;
+  return OPTCC_OK;
+}
+
+template <int MODE>
+int launch_plan(optcc_plan_t* pl, ExecParams& P, cudaStream_t stream) {
+  optcc_exec_state* st = pl->exec;
+  const optcc_plan_info_t& in = pl->info;
+  if (in.n_steps == 0) return OPTCC_OK;
+  const bool persistent = pl->opts.exec_mode == OPTCC_EXEC_PERSISTENT && st->coop;
+  if (persistent) {
+    CU_TRY(cudaMemsetAsync(&P.ctrl->barrier, 0, sizeof(unsigned long long), stream));
+    P.step_lo = 0;
+    P.step_hi = in.n_steps;
+    P.use_barrier = 1;
+    void* args[] = {&P};
+    CU_TRY(cudaLaunchCooperativeKernel((const void*)optcc_exec_kernel<MODE>, dim3(st->G), dim3(THREADS), args, 0, stream));
+  } else {
+    P.use_barrier = 0;
+    for (uint32_t t = 0; t < in.n_steps; ++t) {
+      if (pl->step_begin[t] == pl->step_begin[t + 1]) continue;
+      P.step_lo = t;
+      P.step_hi = t + 1;
+      optcc_exec_kernel<MODE><<<st->G, THREADS, 0, stream>>>(P);
+    }
+    CU_TRY(cudaGetLastError());
+  }
+  return OPTCC_OK;
+}
+
+void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
+  const optcc_ws_layout L = optcc_layout(pl->info);
+  char* ws = static_cast<char*>(workspace);
+  std::memset(&P, 0, sizeof P);
+  P.flows = reinterpret_cast<const DFlow*>(ws + L.dflows);
+  P.slices = reinterpret_cast<const Slice*>(ws + L.slices);
+  P.ctrl = reinterpret_cast<Ctrl*>(ws + L.ctrl);
+  P.shadow = reinterpret_cast<float*>(ws + L.shadow);
+  P.padded_n = pl->info.padded_n;
+  P.unit_elems = pl->info.unit_elems;
+}
+
+}  // namespace
+
+extern "C" int optcc_last_cuda_error(void) { return g_last_cuda_error; }
+
+extern "C" int optcc_prepare(optcc_plan_t* plan, void* workspace, void* stream) {
+  if (!plan || !workspace || (reinterpret_cast<uintptr_t>(workspace) & 255)) return OPTCC_EINVAL;
+  int rc = build_state(plan);
+  if (rc != OPTCC_OK) return rc;
+  return upload_tables(plan, workspace, static_cast<cudaStream_t>(stream));
+}
+
+extern "C" int optcc_execute(optcc_plan_t* plan, void* const* bufs, void* workspace, void* stream_) {
+  if (!plan || !bufs || !workspace) return OPTCC_EINVAL;
+  const optcc_plan_info_t& in = plan->info;
+  for (uint32_t r = 0; r < in.p; ++r)
+    if (!bufs[r] || (reinterpret_cast<uintptr_t>(bufs[r]) & 15)) return OPTCC_EINVAL;
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  int rc = optcc_prepare(plan, workspace, stream_);
+  if (rc != OPTCC_OK) return rc;
+  ExecParams P;
+  fill_common(plan, workspace, P);
+  if (in.p <= (uint32_t)MAX_PARAM_PTRS) {
+    for (uint32_t r = 0; r < in.p; ++r) P.bufs[r] = bufs[r];
+  } else {
+    const optcc_ws_layout L = optcc_layout(in);
+    char* ws = static_cast<char*>(workspace);
+    CU_TRY(cudaMemcpyAsync(ws + L.ptrs, bufs, size_t(in.p) * sizeof(void*), cudaMemcpyHostToDevice, stream));
+    P.ptr_table = reinterpret_cast<void* const*>(ws + L.ptrs);
+  }
+  return in.dtype == OPTCC_F32 ? launch_plan<MODE_F32>(plan, P, stream) : launch_plan<MODE_BF16>(plan, P, stream);
+}
+
+extern "C" int optcc_execute_host(optcc_plan_t* plan, const void* const* host_in, void* const* host_out,
+                                  void* const* bufs, void* workspace, void* stream_) {
+  if (!plan || !host_in || !host_out || !bufs) return OPTCC_EINVAL;
+  const optcc_plan_info_t& in = plan->info;
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  const size_t bytes = size_t(in.n) * (in.dtype == OPTCC_F32 ? 4 : 2);
+  for (uint32_t r = 0; r < in.p; ++r) {
+    if (!host_in[r] || !host_out[r] || !bufs[r]) return OPTCC_EINVAL;
+    CU_TRY(cudaMemcpyAsync(bufs[r], host_in[r], bytes, cudaMemcpyHostToDevice, stream));
+  }
+  int rc = optcc_execute(plan, bufs, workspace, stream_);
+  if (rc != OPTCC_OK) return rc;
+  for (uint32_t r = 0; r < in.p; ++r) CU_TRY(cudaMemcpyAsync(host_out[r], bufs[r], bytes, cudaMemcpyDeviceToHost, stream));
+  return OPTCC_OK;
+}
+
+extern "C" int optcc_verify(optcc_plan_t* plan, void* workspace, void* stream_, optcc_verify_result_t* out) {
+  if (!plan || !workspace || !out) return OPTCC_EINVAL;
+  const optcc_plan_info_t& in = plan->info;
+  if (in.mask_words == 0) return OPTCC_EUNSUPPORTED;
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  int rc = optcc_prepare(plan, workspace, stream_);
+  if (rc != OPTCC_OK) return rc;
+  const optcc_ws_layout L = optcc_layout(in);
+  char* ws = static_cast<char*>(workspace);
+  unsigned long long* masks = reinterpret_cast<unsigned long long*>(ws + L.masks);
+  ExecParams P;
+  fill_common(plan, workspace, P);
+  for (uint32_t r = 0; r < in.p; ++r) P.bufs[r] = masks + uint64_t(r) * in.padded_n * in.mask_words;
+  Ctrl init;
+  std::memset(&init, 0, sizeof init);
+  init.first_bad = ~0ull;
+  CU_TRY(cudaMemcpyAsync(P.ctrl, &init, sizeof init, cudaMemcpyHostToDevice, stream));
+  const int blocks = plan->exec->sm_count * 8;
+  optcc_mask_init_kernel<<<blocks, 256, 0, stream>>>(masks, in.p, in.n, in.padded_n, in.mask_words);
+  CU_TRY(cudaGetLastError());
+  rc = in.mask_words == 1 ? launch_plan<MODE_MASK1>(plan, P, stream) : launch_plan<MODE_MASK2>(plan, P, stream);
+  if (rc != OPTCC_OK) return rc;
+  optcc_mask_check_kernel<<<blocks, 256, 0, stream>>>(masks, in.p, in.n, in.padded_n, in.mask_words, P.ctrl);
+  CU_TRY(cudaGetLastError());
+  Ctrl res;
+  CU_TRY(cudaMemcpyAsync(&res, P.ctrl, sizeof res, cudaMemcpyDeviceToHost, stream));
+  CU_TRY(cudaStreamSynchronize(stream));
+  optcc_verify_result_t r;
+  r.bad_elements = res.bad;
+  r.overlap_elements = res.overlap;
+  r.first_bad = res.first_bad;
+  r.checked = uint64_t(in.p) * in.n;
+  *out = r;
+  return (r.bad_elements || r.overlap_elements) ? OPTCC_EVERIFY : OPTCC_OK;
+}

@@ -1,0 +1,220 @@
+// Device code of the OPTCC executor (sm_100a).  Included only by optcc_exec.cu.
+//
+// One kernel template walks the plan's step tables for all element types:
+//   MODE_F32    rank buffers of float; reduce = one IEEE fp32 add per element ("adds its own section")
+//   MODE_BF16   rank buffers of bf16, fp32 partial sums in a shadow array, one RNE rounding when a sum completes (R12)
+//   MODE_MASK1  contributor bitmasks, one 64-bit word per element  (p <= 64)   reduce = disjoint OR, copy = assign
+//   MODE_MASK2  contributor bitmasks, two 64-bit words per element (p <= 128)
+// so the verifier (PAPER.md:68 correctness (ii)) runs exactly the tables the executor runs.
+//
+// Work distribution: a step's flows are concatenated in table order and cut into gridDim.x slices of equal
+// HBM bytes (host-built slice table); CTA c streams slice c with 16-byte vector loads/stores, fully coalesced,
+// UNROLL independent vectors in flight per thread.  The CTA's part of the step table is staged in shared memory
+// one step ahead.  Steps are separated by a grid-wide barrier (persistent mode) or by kernel boundaries.
+#ifndef OPTCC_KERNELS_CUH_
+#define OPTCC_KERNELS_CUH_
+
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace optcc_dev {
+
+enum { MODE_F32 = 0, MODE_BF16 = 1, MODE_MASK1 = 2, MODE_MASK2 = 3 };
+
+constexpr int THREADS = 512;      // threads per CTA
+constexpr int CTAS_PER_SM = 2;    // resident CTAs per SM the kernels are tuned for (<= 64 registers/thread)
+constexpr int STAGE = 16;         // flow records staged in shared memory per CTA and step
+constexpr int MAX_PARAM_PTRS = 128;
+
+struct __align__(16) DFlow {      // 32 bytes: what the device needs of an optcc_flow_t
+  unsigned long long off;         // elements
+  unsigned long long len;         // elements
+  unsigned short src, dst;
+  unsigned char op, ksrc, kdin, kdout;  // op: 0 reduce, 1 copy; k*: 0 rank buffer, 1 fp32 shadow (bf16 plans)
+  unsigned int pad0, pad1;
+};
+static_assert(sizeof(DFlow) == 32, "DFlow must be 32 bytes");
+
+struct __align__(16) Slice {      // start of a CTA's slice of a step: flow index and 16-byte unit inside it
+  unsigned int flow;
+  unsigned int pad;
+  unsigned long long unit;
+};
+static_assert(sizeof(Slice) == 16, "Slice must be 16 bytes");
+
+struct Ctrl {                     // control block at the start of the workspace
+  unsigned long long barrier;     // monotone arrival counter of the grid barrier
+  unsigned long long bad;         // verify: wrong final masks
+  unsigned long long overlap;     // verify: reduce over overlapping contributor sets
+  unsigned long long first_bad;   // verify: smallest bad r*n+e
+};
+
+struct ExecParams {
+  void* bufs[MAX_PARAM_PTRS];     // rank buffers (p <= 128); masks: per-rank mask arrays
+  void* const* ptr_table;         // rank buffers when p > 128 (device array), else nullptr
+  const DFlow* flows;
+  const Slice* slices;            // [n_steps][gridDim.x + 1]
+  Ctrl* ctrl;
+  float* shadow;                  // bf16 plans: fp32 partials, [p][padded_n]
+  unsigned long long padded_n;
+  unsigned int step_lo, step_hi;  // steps [lo, hi) are executed by this launch
+  unsigned int unit_elems;        // A (PLAN_SPEC 2)
+  unsigned int use_barrier;       // 1: grid barrier between steps (cooperative launch)
+};
+
+// ---- memory access helpers: L2-only loads (data written by other SMs in the previous step), streaming stores ----
+__device__ __forceinline__ uint4 ld16(const void* p) { return __ldcg(reinterpret_cast<const uint4*>(p)); }
+__device__ __forceinline__ void st16(void* p, uint4 v) { __stcg(reinterpret_cast<uint4*>(p), v); }
+
+__device__ __forceinline__ float bf16_to_f32(unsigned int h) { return __uint_as_float(h << 16); }
+// float -> bf16 bits, round to nearest even; NaN stays a quiet NaN
+__device__ __forceinline__ unsigned int f32_to_bf16_rne(float f) {
+  unsigned int u = __float_as_uint(f);
+  if ((u & 0x7FFFFFFFu) > 0x7F800000u) return (u >> 16) | 0x40u;
+  return (u + 0x7FFFu + ((u >> 16) & 1u)) >> 16;
+}
+
+__device__ __forceinline__ uint4 add_f32x4(uint4 a, uint4 b) {
+  uint4 r;
+  r.x = __float_as_uint(__fadd_rn(__uint_as_float(a.x), __uint_as_float(b.x)));
+  r.y = __float_as_uint(__fadd_rn(__uint_as_float(a.y), __uint_as_float(b.y)));
+  r.z = __float_as_uint(__fadd_rn(__uint_as_float(a.z), __uint_as_float(b.z)));
+  r.w = __float_as_uint(__fadd_rn(__uint_as_float(a.w), __uint_as_float(b.w)));
+  return r;
+}
+
+// ---- grid-wide barrier: every CTA arrives once per step; counter is monotone, target = arrivals expected so far ----
+__device__ __forceinline__ void grid_barrier(unsigned long long* ctr, unsigned long long target) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned long long seen;
+    asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(ctr) : "memory");
+    do {
+      asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(ctr) : "memory");
+    } while (seen < target);
+    __threadfence();
+  }
+  __syncthreads();
+}
+
+// =====================================================================================================
+// Range operations.  All ranges are given in 16-byte vectors [vbeg, vend) relative to the flow's start.
+// =====================================================================================================
+
+template <int UNROLL>
+__device__ __forceinline__ void range_copy16(const char* __restrict__ s, char* __restrict__ d,
+                                             unsigned long long vbeg, unsigned long long vend) {
+  unsigned long long v = vbeg + threadIdx.x;
+  for (; v + (UNROLL - 1) * (unsigned long long)THREADS < vend; v += UNROLL * (unsigned long long)THREADS) {
+    uint4 x[UNROLL];
+#pragma unroll
+    for (int j = 0; j < UNROLL; ++j) x[j] = ld16(s + (v + j * (unsigned long long)THREADS) * 16);
+#pragma unroll
+    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)THREADS) * 16, x[j]);
+  }
+  for (; v < vend; v += THREADS) st16(d + v * 16, ld16(s + v * 16));
+}
+
+template <int UNROLL>
+__device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* __restrict__ d,
+                                              unsigned long long vbeg, unsigned long long vend) {
+  unsigned long long v = vbeg + threadIdx.x;
+  for (; v + (UNROLL - 1) * (unsigned long long)THREADS < vend; v += UNROLL * (unsigned long long)THREADS) {
+    uint4 a[UNROLL], b[UNROLL];
+#pragma unroll
+    for (int j = 0; j < UNROLL; ++j) {
+      a[j] = ld16(s + (v + j * (unsigned long long)THREADS) * 16);
+      b[j] = ld16(d + (v + j * (unsigned long long)THREADS) * 16);
+    }
+#pragma unroll
+    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)THREADS) * 16, add_f32x4(b[j], a[j]));
+  }
+  for (; v < vend; v += THREADS) st16(d + v * 16, add_f32x4(ld16(d + v * 16), ld16(s + v * 16)));
+}
+
+// masks: OR with overlap detection.  WORDS = 64-bit words per element (1 or 2); a 16-byte vector holds 2/WORDS elements
+template <int UNROLL, int WORDS>
+__device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* __restrict__ d,
+                                              unsigned long long vbeg, unsigned long long vend,
+                                              unsigned int& overlaps) {
+  unsigned long long v = vbeg + threadIdx.x;
+  auto join = [&](uint4 a, uint4 b) {
+    unsigned int lo = ((a.x & b.x) | (a.y & b.y)) != 0u, hi = ((a.z & b.z) | (a.w & b.w)) != 0u;
+    overlaps += (WORDS == 1) ? (lo + hi) : ((lo | hi) ? 1u : 0u);
+    return make_uint4(a.x | b.x, a.y | b.y, a.z | b.z, a.w | b.w);
+  };
+  for (; v + (UNROLL - 1) * (unsigned long long)THREADS < vend; v += UNROLL * (unsigned long long)THREADS) {
+    uint4 a[UNROLL], b[UNROLL];
+#pragma unroll
+    for (int j = 0; j < UNROLL; ++j) {
+      a[j] = ld16(s + (v + j * (unsigned long long)THREADS) * 16);
+      b[j] = ld16(d + (v + j * (unsigned long long)THREADS) * 16);
+    }
+#pragma unroll
+    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)THREADS) * 16, join(a[j], b[j]));
+  }
+  for (; v < vend; v += THREADS) st16(d + v * 16, join(ld16(s + v * 16), ld16(d + v * 16)));
+}
+
+// bf16 plans: a unit is 8 elements = 16 bytes in a rank buffer or 32 bytes in the fp32 shadow.
+template <int KIND>
+__device__ __forceinline__ void load8(const char* base, unsigned long long unit, float (&x)[8]) {
+  if (KIND == 0) {
+    uint4 r = ld16(base + unit * 16);
+    x[0] = bf16_to_f32(r.x & 0xFFFFu); x[1] = bf16_to_f32(r.x >> 16);
+    x[2] = bf16_to_f32(r.y & 0xFFFFu); x[3] = bf16_to_f32(r.y >> 16);
+    x[4] = bf16_to_f32(r.z & 0xFFFFu); x[5] = bf16_to_f32(r.z >> 16);
+    x[6] = bf16_to_f32(r.w & 0xFFFFu); x[7] = bf16_to_f32(r.w >> 16);
+  } else {
+    uint4 r0 = ld16(base + unit * 32), r1 = ld16(base + unit * 32 + 16);
+    x[0] = __uint_as_float(r0.x); x[1] = __uint_as_float(r0.y); x[2] = __uint_as_float(r0.z); x[3] = __uint_as_float(r0.w);
+    x[4] = __uint_as_float(r1.x); x[5] = __uint_as_float(r1.y); x[6] = __uint_as_float(r1.z); x[7] = __uint_as_float(r1.w);
+  }
+}
+template <int KIND>
+__device__ __forceinline__ void store8(char* base, unsigned long long unit, const float (&x)[8]) {
+  if (KIND == 0) {
+    uint4 r;
+    r.x = f32_to_bf16_rne(x[0]) | (f32_to_bf16_rne(x[1]) << 16);
+    r.y = f32_to_bf16_rne(x[2]) | (f32_to_bf16_rne(x[3]) << 16);
+    r.z = f32_to_bf16_rne(x[4]) | (f32_to_bf16_rne(x[5]) << 16);
+    r.w = f32_to_bf16_rne(x[6]) | (f32_to_bf16_rne(x[7]) << 16);
+    st16(base + unit * 16, r);
+  } else {
+    st16(base + unit * 32, make_uint4(__float_as_uint(x[0]), __float_as_uint(x[1]), __float_as_uint(x[2]), __float_as_uint(x[3])));
+    st16(base + unit * 32 + 16, make_uint4(__float_as_uint(x[4]), __float_as_uint(x[5]), __float_as_uint(x[6]), __float_as_uint(x[7])));
+  }
+}
+
+template <int KS, int KD, int KO>
+__device__ __forceinline__ void range_add_bf16(const char* __restrict__ s, const char* __restrict__ din,
+                                               char* __restrict__ dout, unsigned long long ubeg,
+                                               unsigned long long uend) {
+  constexpr int UNROLL = 2;
+  unsigned long long u = ubeg + threadIdx.x;
+  for (; u + (UNROLL - 1) * (unsigned long long)THREADS < uend; u += UNROLL * (unsigned long long)THREADS) {
+    float a[UNROLL][8], b[UNROLL][8];
+#pragma unroll
+    for (int j = 0; j < UNROLL; ++j) {
+      load8<KS>(s, u + j * (unsigned long long)THREADS, a[j]);
+      load8<KD>(din, u + j * (unsigned long long)THREADS, b[j]);
+    }
+#pragma unroll
+    for (int j = 0; j < UNROLL; ++j) {
+#pragma unroll
+      for (int e = 0; e < 8; ++e) b[j][e] = __fadd_rn(b[j][e], a[j][e]);
+      store8<KO>(dout, u + j * (unsigned long long)THREADS, b[j]);
+    }
+  }
+  for (; u < uend; u += THREADS) {
+    float a[8], b[8];
+    load8<KS>(s, u, a);
+    load8<KD>(din, u, b);
+#pragma unroll
+    for (int e = 0; e < 8; ++e) b[e] = __fadd_rn(b[e], a[e]);
+    store8<KO>(dout, u, b);
+  }
+}
+
+}  // namespace optcc_dev
+#endif
