@@ -75,6 +75,9 @@ typedef struct optcc_opts {
   uint32_t exec_mode; /* OPTCC_EXEC_* */
   uint32_t grid_ctas; /* 0 = auto (SM count x resident CTAs per SM); else CTAs of the executor grid */
   uint32_t copy_path; /* 0 = auto, 1 = LDG/STG vector copy, 2 = cp.async.bulk (TMA 1-D) copy */
+  uint32_t step_limit;/* 0 = all steps; else execute / verify only the first step_limit steps (debugging and
+                         profiling: a truncated schedule must FAIL verification) */
+  uint32_t reserved;  /* 0 */
 } optcc_opts_t;
 
 typedef struct optcc_plan_info {

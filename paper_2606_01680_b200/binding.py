@@ -28,7 +28,8 @@ FLOW_DTYPE = np.dtype([
 
 
 class optcc_opts_t(C.Structure):
-    _fields_ = [("k", C.c_uint32), ("exec_mode", C.c_uint32), ("grid_ctas", C.c_uint32), ("copy_path", C.c_uint32)]
+    _fields_ = [("k", C.c_uint32), ("exec_mode", C.c_uint32), ("grid_ctas", C.c_uint32), ("copy_path", C.c_uint32),
+                ("step_limit", C.c_uint32), ("reserved", C.c_uint32)]
 
 
 class optcc_plan_info_t(C.Structure):
@@ -146,11 +147,11 @@ class Plan:
             pass
 
 
-def optcc_plan(p, g, ell, n, dtype, k=0, exec_mode=0, grid_ctas=0, copy_path=0):
+def optcc_plan(p, g, ell, n, dtype, k=0, exec_mode=0, grid_ctas=0, copy_path=0, step_limit=0):
     """optcc_plan_ex: returns a Plan.  ell: sequence of p floats."""
     lib = load()
     ell_arr = (C.c_double * len(ell))(*[float(x) for x in ell])
-    opts = optcc_opts_t(k, exec_mode, grid_ctas, copy_path)
+    opts = optcc_opts_t(k, exec_mode, grid_ctas, copy_path, step_limit, 0)
     h = C.c_void_p()
     rc = lib.optcc_plan_ex(int(p), int(g), ell_arr, int(n), int(dtype), C.byref(opts), C.byref(h))
     if rc:

@@ -351,22 +351,28 @@ int upload_tables(optcc_plan_t* pl, void* workspace, cudaStream_t stream) {
   return OPTCC_OK;
 }
 
+inline uint32_t plan_steps(const optcc_plan_t* pl) {
+  const uint32_t lim = pl->opts.step_limit;
+  return lim ? std::min(lim, pl->info.n_steps) : pl->info.n_steps;
+}
+
 template <int MODE>
 int launch_plan(optcc_plan_t* pl, ExecParams& P, cudaStream_t stream) {
   optcc_exec_state* st = pl->exec;
   const optcc_plan_info_t& in = pl->info;
-  if (in.n_steps == 0) return OPTCC_OK;
+  const uint32_t n_steps = plan_steps(pl);
+  if (n_steps == 0) return OPTCC_OK;
   const bool persistent = pl->opts.exec_mode == OPTCC_EXEC_PERSISTENT && st->coop;
   if (persistent) {
     CU_TRY(cudaMemsetAsync(&P.ctrl->barrier, 0, sizeof(unsigned long long), stream));
     P.step_lo = 0;
-    P.step_hi = in.n_steps;
+    P.step_hi = n_steps;
     P.use_barrier = 1;
     void* args[] = {&P};
     CU_TRY(cudaLaunchCooperativeKernel((const void*)optcc_exec_kernel<MODE>, dim3(st->G), dim3(THREADS), args, 0, stream));
   } else {
     P.use_barrier = 0;
-    for (uint32_t t = 0; t < in.n_steps; ++t) {
+    for (uint32_t t = 0; t < n_steps; ++t) {
       if (pl->step_begin[t] == pl->step_begin[t + 1]) continue;
       P.step_lo = t;
       P.step_hi = t + 1;

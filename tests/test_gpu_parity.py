@@ -1,0 +1,188 @@
+"""GPU parity tests (run on the B200 box: pytest -m gpu).  Every call goes through the C-ABI (binding -> liboptcc).
+
+Bars (BASELINE.json north_star):
+  * contributor masks equal the oracle's element by element, bit-exactly; plan tables too (CPU test file);
+  * fp32 outputs: |y - y_ref| <= p 2^-23 sum_i |x_i| per element against the fp64 reference sum, AND bit-identical
+    to the oracle's plan-order fp32 emulation (each reduce flow is one IEEE add per element in a plan-fixed order);
+  * bf16 outputs: within 2^-7 relative (+ fp32 accumulation floor, R12) of the fp64 reference, AND bit-identical to
+    the oracle's fp32-partials / one-final-RNE emulation;
+  * all p outputs bitwise identical (PAPER.md:68 (ii)).
+"""
+import numpy as np
+import pytest
+
+from paper_2606_01680_b200 import binding as B
+from paper_2606_01680_b200 import workloads as W
+from oracle import planner as OP
+from oracle import interpreter as OI
+from oracle import reference as OR
+
+pytestmark = pytest.mark.gpu
+
+
+def _session(plan, verify=False):
+    from paper_2606_01680_b200.device import Session
+    return Session(plan, verify=verify)
+
+
+def _wl(p, g, st, n, dtype, seed, dist="normal"):
+    ell = tuple(float(st.get(i, 1.0)) for i in range(p))
+    return W.Workload(f"t{p}x{n}", p, g, ell, n, dtype, dist, 1.0, seed)
+
+
+def _run_and_check(w, k, exec_mode, grid_ctas=0):
+    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=k, exec_mode=exec_mode, grid_ctas=grid_ctas)
+    oplan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=k)
+    x = W.all_inputs(w)
+    s = _session(plan)
+    s.upload(x)
+    s.execute()
+    y = s.download()
+    assert OR.all_ranks_identical(y)
+    if w.dtype == W.F32:
+        assert OR.check_f32(y[0], x).all()                       # north_star fp32 bound vs the fp64 sum
+        y_or = OI.run_f32(oplan, x)
+        assert y.view(np.uint32).tobytes() == y_or.view(np.uint32).tobytes()   # plan-order bit parity
+    else:
+        xf = OI.bf16_bits_to_f32(x)
+        assert OR.check_bf16(OI.bf16_bits_to_f32(y[0]), xf).all()
+        y_or = OI.run_bf16(oplan, x)
+        assert y.tobytes() == y_or.tobytes()
+    return plan, s
+
+
+# sizes: a few hundred KB per rank so that slices, unrolled bodies, remainders and ragged tails are all exercised
+F32_CASES = [
+    # p, g, stragglers, n, k
+    (4, 1, {0: 2.0}, 2 ** 16, 8),                       # C1 shape, scaled n
+    (4, 1, {0: 2.0}, 100003, 4),                        # ragged: n % 4 = 3
+    (5, 1, {2: 1.5}, 50001, 4),                         # bubble filling (l < 2), ragged n % 4 = 1
+    (16, 1, {0: 8.0 / 7.0}, 2 ** 17 + 2, 8),            # C2 shape
+    (6, 1, {}, 77777, 0),                               # C0 plain ring
+    (7, 1, {0: 2.0, 1: 4.0 / 3.0}, 65539, 4),           # C2 construction, m = 2
+    (16, 4, {r: 2.0 for r in range(4)}, 40001, 4),      # C3 construction, g = 4
+    (32, 1, {0: 2.0 - 1.0 / 31.0}, 2 ** 15, 12),        # C5 shape at the Thm-1 switch
+    (3, 1, {1: 3.0}, 5, 4),                             # fewer units than sections: most flows dropped
+    (3, 1, {0: 2.0}, 1, 4),                             # one element
+]
+
+
+@pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_PERSISTENT, B.OPTCC_EXEC_PER_STEP])
+@pytest.mark.parametrize("p,g,st,n,k", F32_CASES)
+def test_f32_parity(p, g, st, n, k, exec_mode):
+    _run_and_check(_wl(p, g, st, n, W.F32, seed=100 + p), k, exec_mode)
+
+
+BF16_CASES = [
+    (4, 1, {0: 2.0}, 2 ** 16, 8),
+    (5, 1, {2: 1.5}, 50003, 4),                         # ragged: n % 8 = 3
+    (64, 1, {5: 8.0 / 7.0, 17: 4.0 / 3.0, 40: 2.0}, 70001, 4),   # C3 shape (config 3), ragged
+    (6, 1, {}, 33333, 0),
+    (12, 2, {0: 1.5, 1: 1.5}, 4097, 12),
+    (3, 1, {0: 2.0}, 1, 4),
+]
+
+
+@pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_PERSISTENT, B.OPTCC_EXEC_PER_STEP])
+@pytest.mark.parametrize("p,g,st,n,k", BF16_CASES)
+def test_bf16_parity(p, g, st, n, k, exec_mode):
+    _run_and_check(_wl(p, g, st, n, W.BF16, seed=200 + p), k, exec_mode)
+
+
+@pytest.mark.parametrize("grid_ctas", [1, 7, 148])
+def test_f32_parity_any_grid(grid_ctas):
+    """Slices are cut per CTA: the result must not depend on the grid."""
+    _run_and_check(_wl(16, 1, {3: 4.0 / 3.0}, 2 ** 16 + 13, W.F32, seed=7), 8, B.OPTCC_EXEC_PERSISTENT, grid_ctas)
+
+
+MASK_CASES = [
+    (4, 1, {0: 2.0}, 4099, W.F32, 8), (5, 1, {2: 1.5}, 50001, W.F32, 4), (6, 1, {}, 7777, W.F32, 0),
+    (64, 1, {5: 8.0 / 7.0, 17: 4.0 / 3.0, 40: 2.0}, 9001, W.BF16, 4),
+    (128, 8, {r: 2.0 for r in range(8)}, 6007, W.F32, 4),               # two mask words (p = 128)
+    (72, 1, {1: 2.0}, 3001, W.BF16, 4),                                   # two mask words, p not a multiple of 64
+    (16, 4, {r: 2.0 for r in range(4)}, 40001, W.F32, 4),
+]
+
+
+@pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_PERSISTENT, B.OPTCC_EXEC_PER_STEP])
+@pytest.mark.parametrize("p,g,st,n,dtype,k", MASK_CASES)
+def test_verifier_masks_equal_oracle(p, g, st, n, dtype, k, exec_mode):
+    ell = [float(st.get(i, 1.0)) for i in range(p)]
+    plan = B.optcc_plan(p, g, ell, n, dtype, k=k, exec_mode=exec_mode)
+    oplan = OP.build_plan(p, g, ell, n, dtype, k=k)
+    s = _session(plan, verify=True)
+    res = s.verify()
+    assert res["bad_elements"] == 0 and res["overlap_elements"] == 0
+    assert res["checked"] == p * n and res["first_bad"] == 2 ** 64 - 1
+    m_or, overlaps = OI.element_masks(oplan)
+    assert overlaps == 0
+    m = s.masks()
+    assert m.shape == m_or.shape and m.tobytes() == m_or.tobytes()
+    assert (m == OI.full_mask_words(p)[None, None, :]).all()
+
+
+@pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_PERSISTENT, B.OPTCC_EXEC_PER_STEP])
+@pytest.mark.parametrize("limit", [1, 9, 19])
+def test_verifier_detects_a_truncated_schedule(limit, exec_mode):
+    """The verifier is not vacuous: a schedule cut after `limit` steps must fail, with exactly the masks and
+    the number of wrong elements the oracle's interpreter finds for the same truncated table."""
+    import dataclasses
+    p, n, k = 5, 4099, 4
+    ell = [1.0, 1.0, 1.5, 1.0, 1.0]
+    plan = B.optcc_plan(p, 1, ell, n, W.F32, k=k, exec_mode=exec_mode, step_limit=limit)
+    oplan = OP.build_plan(p, 1, ell, n, W.F32, k=k)
+    assert limit < oplan.n_steps
+    s = _session(plan, verify=True)
+    res = s.verify(raise_on_fail=False)
+    m_or, _ = OI.element_masks(dataclasses.replace(oplan, n_steps=limit))
+    m = s.masks()
+    assert m.tobytes() == m_or.tobytes()
+    bad = (m_or != OI.full_mask_words(p)[None, None, :]).any(axis=2)
+    assert res["bad_elements"] == int(bad.sum()) > 0
+    assert res["first_bad"] == int(np.flatnonzero(bad.reshape(-1))[0])
+    with pytest.raises(B.OptccError) as e:
+        s.verify()
+    assert e.value.name == "EVERIFY"
+
+
+def test_execute_rejects_bad_arguments():
+    import torch
+    plan = B.optcc_plan(4, 1, [2.0, 1.0, 1.0, 1.0], 4096, W.F32, k=4)
+    s = _session(plan)
+    bufs = list(s.bufs)
+    with pytest.raises(B.OptccError) as e:
+        B.optcc_execute(plan, [bufs[0].data_ptr() + 4] + bufs[1:], s.ws_ptr, torch.cuda.current_stream().cuda_stream)
+    assert e.value.name == "EINVAL"               # misaligned rank buffer
+    with pytest.raises(B.OptccError) as e:
+        B.optcc_execute(plan, [0] + bufs[1:], s.ws_ptr, torch.cuda.current_stream().cuda_stream)
+    assert e.value.name == "EINVAL"
+
+
+def test_execute_host_roundtrip():
+    import torch
+    w = _wl(8, 1, {0: 2.0}, 2 ** 15 + 5, W.F32, seed=31)
+    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=4)
+    s = _session(plan)
+    x = W.all_inputs(w)
+    hin = [torch.from_numpy(x[r].copy()).pin_memory() for r in range(w.p)]
+    hout = [torch.empty(w.n, dtype=torch.float32).pin_memory() for r in range(w.p)]
+    s.execute_host(hin, hout)
+    torch.cuda.synchronize()
+    y = np.stack([t.numpy() for t in hout])
+    assert OR.all_ranks_identical(y)
+    assert OR.check_f32(y[0], x).all()
+    oplan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=4)
+    assert y.tobytes() == OI.run_f32(oplan, x).tobytes()
+
+
+def test_repeated_execute_on_same_session_is_deterministic():
+    w = _wl(16, 1, {0: 8.0 / 7.0}, 2 ** 16, W.F32, seed=5)
+    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=8)
+    s = _session(plan)
+    x = W.all_inputs(w)
+    outs = []
+    for _ in range(3):
+        s.upload(x)
+        s.execute()
+        outs.append(s.download([0, w.p - 1]).tobytes())
+    assert outs[0] == outs[1] == outs[2]

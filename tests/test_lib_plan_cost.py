@@ -1,0 +1,167 @@
+"""CPU tests of liboptcc's host side (no GPU): the library loads and exports every symbol of include/optcc.h;
+the C++ planner's integer tables equal the oracle's byte for byte (north_star: "integer plan/step tables match
+bit-exactly"); optcc_cost agrees with the oracle's exact-rational simulation and closed forms to 1e-12 relative.
+"""
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2606_01680_b200 import binding as B
+from paper_2606_01680_b200 import build as optcc_build
+from paper_2606_01680_b200 import workloads as W
+from oracle import planner as OP
+from oracle import cost_sim, closed_forms as cf
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    optcc_build.build()
+
+
+def _ell(p, d):
+    return [float(d.get(i, 1.0)) for i in range(p)]
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "optcc.h")).read()
+    declared = set(re.findall(r"OPTCC_API\s+[\w\s\*]+?\b(optcc_\w+)\s*\(", header))
+    assert declared == set(B.EXPORTS)
+    lib = B.load()
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert lib.optcc_abi_version() == 1
+    assert B.FLOW_DTYPE.itemsize == 40
+
+
+def _compare(p, g, ell, n, dtype, k):
+    pl = B.optcc_plan(p, g, ell, n, dtype, k=k)
+    op = OP.build_plan(p, g, list(ell), n, dtype, k=k)
+    fl, sb, sec, p2p = B.optcc_plan_tables(pl)
+    i = pl.info
+    assert fl.tobytes() == op.flows.tobytes()
+    assert np.array_equal(sb, op.step_begin)
+    assert np.array_equal(sec, op.sec_bounds)
+    assert np.array_equal(p2p, op.p2p_bounds)
+    for key, val in (("p", op.p), ("g", op.g), ("q", op.q), ("m", op.m), ("H", op.H), ("k", op.k),
+                     ("construction", op.construction), ("unit_elems", op.A), ("n", op.n), ("n_ring", op.n_ring),
+                     ("n_p2p", op.n_p2p), ("U", op.U), ("U_ring", op.U_ring), ("U_p2p", op.U_p2p),
+                     ("n_steps", op.n_steps), ("n_flows", len(op.flows))):
+        assert i[key] == val, key
+    assert i["reduce_elems"] == (p - 1) * n and i["copy_elems"] == (p - 1) * n   # Lemma 4 with equality (:340)
+    return pl, op
+
+
+@pytest.mark.parametrize("ci", range(5))
+@pytest.mark.parametrize("k", [0, 8])
+def test_tables_equal_oracle_on_baseline_configs(ci, k):
+    w = W.config(ci)
+    _compare(w.p, w.g, w.ell, w.n, w.dtype, k)
+
+
+@pytest.mark.parametrize("ell", W.C5_ELLS)
+def test_tables_equal_oracle_on_c5_sweep(ell):
+    w = W.config(4, ell)
+    _compare(w.p, w.g, w.ell, w.n, w.dtype, 0)
+
+
+GRID = [
+    # p, g, stragglers, n, dtype, k
+    (3, 1, {0: 2.0}, 1, 0, 4), (3, 1, {1: 1.5}, 7, 0, 4), (4, 1, {}, 1001, 0, 0), (5, 1, {0: 2.0}, 4803, 0, 4),
+    (5, 1, {2: 1.5}, 4803, 1, 4), (7, 1, {0: 2.0, 1: 4.0 / 3.0}, 10007, 0, 4), (7, 1, {3: 1.25, 6: 1.25}, 99991, 1, 8),
+    (16, 1, {9: 8.0 / 7.0}, 123457, 0, 8), (12, 4, {4: 2.0, 5: 2.0, 6: 2.0, 7: 2.0}, 65537, 0, 4),
+    (12, 2, {0: 1.5, 1: 1.5}, 4097, 1, 12), (32, 1, {0: 2.0 - 1.0 / 31.0}, 1 << 20, 0, 20), (32, 1, {31: 3.0}, 999983, 1, 0),
+    (9, 3, {3: 8.0 / 7.0, 4: 8.0 / 7.0, 5: 8.0 / 7.0}, 30011, 0, 8), (6, 1, {1: 1.0 + 2 ** -40}, 5000, 0, 4),
+    (64, 1, {5: 8.0 / 7.0, 17: 4.0 / 3.0, 40: 2.0}, 70001, 1, 4), (40, 8, {r: 2.0 for r in range(8, 16)}, 262147, 0, 8),
+]
+
+
+@pytest.mark.parametrize("p,g,st,n,dtype,k", GRID)
+def test_tables_equal_oracle_on_grid(p, g, st, n, dtype, k):
+    _compare(p, g, _ell(p, st), n, dtype, k)
+
+
+@pytest.mark.parametrize("args,code", [
+    ((2, 1, [1.0, 2.0], 10, 0, 0), "EINVAL"),                 # p >= 3 (:68)
+    ((4, 3, [1.0] * 4, 10, 0, 0), "EINVAL"),                  # g | p
+    ((4, 1, [1.0, 0.5, 1.0, 1.0], 10, 0, 0), "EINVAL"),       # ell >= 1
+    ((4, 1, [1.0, float("nan"), 1.0, 1.0], 10, 0, 0), "EINVAL"),
+    ((4, 2, [1.0, 2.0, 1.0, 1.0], 10, 0, 0), "EINVAL"),       # one ell per server (:274)
+    ((4, 1, [2.0, 2.0, 2.0, 1.0], 10, 0, 0), "EINVAL"),       # two healthy servers needed
+    ((4, 1, [2.0, 1.0, 1.0, 1.0], 0, 0, 0), "EINVAL"),        # n > 0
+    ((4, 1, [2.0, 1.0, 1.0, 1.0], 10, 0, 6), "EINVAL"),       # k multiple of 4 (:155)
+    ((4, 1, [2.0, 1.0, 1.0, 1.0], 10, 7, 0), "EINVAL"),       # dtype
+    ((8, 2, [2.0, 2.0, 1.5, 1.5, 1.0, 1.0, 1.0, 1.0], 10, 0, 0), "EUNSUPPORTED"),  # g>1, m>1 (:943)
+    ((8, 2, [1.0] * 8, 10, 0, 0), "EUNSUPPORTED"),
+])
+def test_error_codes_match_oracle(args, code):
+    p, g, ell, n, dtype, k = args
+    with pytest.raises(OP.PlanError) as eo:
+        OP.build_plan(p, g, ell, n, dtype, k=k)
+    assert eo.value.code == code
+    with pytest.raises(B.OptccError) as el:
+        B.optcc_plan(p, g, ell, n, dtype, k=k)
+    assert el.value.name == code
+
+
+COST_CASES = [
+    (4, 1, {0: 2.0}, 4 * 3 * 8 * 16, 0, 8), (5, 1, {0: 1.5}, 4 * 4 * 4 * 50, 0, 4), (16, 1, {0: 8.0 / 7.0}, 1 << 16, 0, 8),
+    (7, 1, {0: 2.0, 1: 4.0 / 3.0}, 4 * 5 * 8 * 9, 0, 8), (64, 1, {5: 8.0 / 7.0, 17: 4.0 / 3.0, 40: 2.0}, 8 * 61 * 8 * 3, 1, 8),
+    (16, 4, {r: 2.0 for r in range(4)}, 4 * 4 * 3 * 8 * 5, 0, 8), (32, 1, {0: 3.0}, 4 * 31 * 12 * 7, 0, 12),
+    (6, 1, {}, 6000, 0, 0), (12, 2, {0: 1.5, 1: 1.5}, 4097, 1, 12),
+]
+
+
+@pytest.mark.parametrize("p,g,st,n,dtype,k", COST_CASES)
+def test_cost_matches_oracle_simulation_and_closed_forms(p, g, st, n, dtype, k):
+    ell = _ell(p, st)
+    pl, op = _compare(p, g, ell, n, dtype, k)
+    c = B.optcc_cost(pl)
+    sim = cost_sim.simulate(op)
+    lbs = cost_sim.lower_bounds(op)
+    rel = lambda a, b: abs(a - float(b)) <= 1e-12 * abs(float(b))
+    assert rel(c["T"], sim["T"])
+    assert rel(c["T0"], sim["T0"])
+    assert rel(c["T_over_T0"], sim["ratio"])
+    assert rel(c["lb_table1"], lbs["table1"])
+    if lbs["tight"] is None:
+        assert math.isnan(c["lb_tight"])
+    else:
+        assert rel(c["lb_tight"], lbs["tight"])
+    assert rel(c["T_closed_form"], cost_sim.paper_closed_form(op))
+    assert rel(c["T0_server"], cf.T0_server(p, n, g))
+    assert c["T"] >= c["lb_table1"] * (1 - 1e-12)
+    if op.m:
+        r = op.stragglers[0] * g
+        assert c["straggler_sent"] == sim["nic_sent"][r] and c["straggler_recv"] == sim["nic_recvd"][r]
+    # alpha-beta: a fixed cost per flow and a scaled element time
+    c2 = B.optcc_cost(pl, alpha=0.25, beta=3.0)
+    sim2 = cost_sim.simulate(op, alpha=cf.Fr(1, 4), beta=3)
+    assert rel(c2["T"], sim2["T"])
+
+
+def test_cost_reports_paper_numbers_for_baseline_configs(golden):
+    """Modeled T/T0 lies on or above the Table-1 bound and within the paper's reported gap (north_star)."""
+    w = W.config(1)                       # C2: Eq.(2) exact for the canonical plan (:185)
+    pl = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=20)
+    c = B.optcc_cost(pl)
+    assert c["lb_table1"] <= c["T"]
+    assert abs(c["T"] / c["T_closed_form"] - 1) < 1e-5       # n not divisible by k(p-1): unit rounding only
+    assert c["T_over_T0"] < 1.06                               # "within 2-6 %" (:7, :217)
+    w = W.config(0)                       # C1: l = 2, T/T0 -> 4/3 (k+1)/k
+    c = B.optcc_cost(B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=8))
+    assert abs(c["T_over_T0"] - (4.0 / 3.0) * 9 / 8) < 1e-4       # 2^20 is not divisible by 3k: unit rounding
+    assert c["regime"] == 2 and c["lb_table1_thm"] == 1 and c["lb_tight_thm"] == 6
+
+
+def test_plan_build_time_is_submillisecond_scale_at_p1024():
+    """schedule generation '< 1 ms at p=1024' is for closed-form rules; ours also materialises and
+    sorts every flow, so only a loose bound is asserted, the measured value is reported by bench.py."""
+    p = 1024
+    pl = B.optcc_plan(p, 1, _ell(p, {0: 2.0}), 1 << 26, 0, k=4)
+    assert pl.info["n_flows"] > 0
+    assert pl.info["plan_build_seconds"] < 5.0
