@@ -1,0 +1,384 @@
+#!/usr/bin/env python
+"""bench.py -- OPTCC-schedule AllReduce on B200: algbw GB/s, schedule bytes vs the HBM roofline, modeled T/T0.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--k 0] [--impl reference]
+
+One "step" = one pass of the whole hot path over one batch of seeded synthetic input:
+optcc_plan (classify, bandwidth-weighted chunking, flow/step tables) -> optcc_cost (alpha-beta model) ->
+optcc_execute (reduce + copy steps with step barriers) -> optcc_verify (contributor masks), all through the C-ABI.
+`value` = n*sizeof(dtype) / step time (algorithm bandwidth, BASELINE.json metric) summed over ranks; the
+`execute_only` object gives the same metric for the AllReduce proper (optcc_execute alone), and `roofline` is the
+executor kernel's schedule bytes (5 (p-1) n sizeof) over its measured duration against the measured
+HBM copy peak.  Inputs are restored from a pristine device copy between steps, outside the timed events (the
+AllReduce is in place); that restore also flushes L2 (footprint >> 126 MB).
+
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+Multi-GPU (torchrun): every rank runs the same workload on its own GPU -- the path shards along the element axis
+with no data-path collective; scaling is "weak".
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "OPTCC-schedule AllReduce algbw"
+UNIT = "GB/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="native", choices=["native", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1 = C2, the metric's config)")
+    ap.add_argument("--ell", type=float, default=1.6, help="ell for config 4 (the C5 sweep)")
+    ap.add_argument("--k", type=int, default=0, help="segments; 0 = planner's auto rule")
+    ap.add_argument("--exec-mode", type=int, default=0, help="0 persistent cooperative kernel, 1 one launch per step")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-sample-log2", type=int, default=0,
+                    help="log2 of n per rank for the CPU-oracle sample (0 = 24 for the cpu_baseline leg, 22 per --impl reference step)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def workload_name(w, k):
+    return f"{w.name}: {w.note}; k={k}"
+
+
+# ------------------------------------------------------------------------------------------------------------
+# CPU oracle legs (the only place bench.py executes oracle/)
+# ------------------------------------------------------------------------------------------------------------
+def oracle_step(w, k):
+    """One pass of the whole path by the oracle as it stands, on workload w (a bounded sample of the config):
+    plan, cost simulation, plan-order execution, masks, fp64 reference sum.  Returns seconds."""
+    import numpy as np
+    from paper_2606_01680_b200 import workloads as W
+    from oracle import planner as OP, interpreter as OI, cost_sim, reference as OR
+    x = W.all_inputs(w)
+    t0 = time.perf_counter()
+    plan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=k)
+    cost_sim.simulate(plan)
+    if w.dtype == W.F32:
+        y = OI.run_f32(plan, x)
+        ok = OR.check_f32(y[0], x).all()
+    else:
+        y = OI.run_bf16(plan, x)
+        ok = OR.check_bf16(OI.bf16_bits_to_f32(y[0]), OI.bf16_bits_to_f32(x)).all()
+    masks, overlaps = OI.element_masks(plan)
+    ok = ok and overlaps == 0 and bool((masks == OI.full_mask_words(w.p)[None, None, :]).all())
+    dt = time.perf_counter() - t0
+    if not ok:
+        raise RuntimeError("oracle self-check failed")
+    return dt
+
+
+def cpu_threads_used():
+    """Threads the oracle actually uses: its numpy work is elementwise slicing/adding (no BLAS), one thread."""
+    return 1
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric / config, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2606_01680_b200 import workloads as W
+    w_full = W.config(args.config, args.ell) if args.config == 4 else W.config(args.config)
+    lg = args.cpu_sample_log2 or 22
+    w = w_full.scaled(min(w_full.n, 2 ** lg))
+    from oracle import planner as OP
+    k = OP.build_plan(w_full.p, w_full.g, list(w_full.ell), w_full.n, w_full.dtype, k=args.k).k
+    for _ in range(min(args.warmup, 1)):
+        oracle_step(w, k)
+    ts = [oracle_step(w, k) for _ in range(args.steps)]
+    t = sum(ts) / len(ts)
+    value = w.n * w.elem_bytes / t / 1e9
+    sample = f"n={w.n} elements per rank (2^{lg}) of the config's n={w_full.n}, all p={w.p} ranks, every flow of the plan"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": min(args.warmup, 1), "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32" if w.dtype == W.F32 else "bf16", "data": "synthetic",
+        "config": {"workload": workload_name(w_full, k), "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cpu_threads_used(), "kind": "oracle", "sample": sample,
+                         "host_cores": os.cpu_count()},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------------------
+# native arm
+# ------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons of one GPU while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.thread.join(timeout=2)
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = float(r[1])
+            except Exception:
+                continue
+            for name, val in zip(names, r[4:8]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, device copy)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def ncu_traffic(workload, kernel):
+    """dram bytes per launch of `kernel` from the committed ncu --set full capture, or None."""
+    path = os.path.join(ROOT, "profiles", "exec_kernel_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    for line in open(path):
+        parts = [s.strip() for s in line.split(",")]
+        if len(parts) >= 3 and parts[0] == workload and parts[1] == kernel:
+            try:
+                return float(parts[2])
+            except ValueError:
+                return None
+    return None
+
+
+def run_native(args):
+    import numpy as np
+    import torch
+    from paper_2606_01680_b200 import binding as B, workloads as W
+    from paper_2606_01680_b200 import build as optcc_build
+    from paper_2606_01680_b200.device import Session
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: liboptcc has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    if rank == 0:
+        optcc_build.build()
+    if dist:
+        dist.barrier()
+    B.load()
+
+    w = W.config(args.config, args.ell) if args.config == 4 else W.config(args.config)
+    if world > 1:   # every rank draws its own slice of a world x n job: same shape, different seed stream
+        w = W.Workload(w.name, w.p, w.g, w.ell, w.n, w.dtype, w.dist, w.sigma, w.seed + 1000 * rank, w.note)
+    esize = w.elem_bytes
+    mk = lambda: B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=args.k, exec_mode=args.exec_mode)
+    plan0 = mk()
+    k = plan0.info["k"]
+    cost0 = B.optcc_cost(plan0)
+    sched_bytes = 5 * (w.p - 1) * w.n * esize            # 3 sizeof per reduce element + 2 per copy element
+    sess = Session(plan0, device=dev, verify=True)
+
+    # seeded synthetic inputs -> pristine device copy (restored between steps, untimed)
+    x = W.all_inputs(w)
+    sess.upload(x)
+    pristine = [b.clone() for b in sess.bufs]
+    restore = lambda: [b.copy_(s) for b, s in zip(sess.bufs, pristine)]
+    stream = torch.cuda.current_stream(dev)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    launches_per_step = (1 if args.exec_mode == 0 else plan0.info["n_steps"]) * 2 + 2   # execute + verify(init, exec, check)
+
+    def full_step(timed):
+        """a1-a3 optcc_plan, a4 optcc_cost, a5-a7 optcc_execute, a8 optcc_verify; returns event pairs + host times."""
+        e = [ev() for _ in range(4)]
+        e[0].record(stream)
+        t0 = time.perf_counter()
+        plan = mk()
+        t1 = time.perf_counter()
+        cost = B.optcc_cost(plan)
+        t2 = time.perf_counter()
+        sess.plan = plan
+        sess.prepare()
+        e[1].record(stream)
+        sess.execute()
+        e[2].record(stream)
+        res = sess.verify()          # synchronises the stream once to read the counters
+        e[3].record(stream)
+        torch.cuda.synchronize(dev)
+        if res["bad_elements"] or res["overlap_elements"]:
+            raise RuntimeError(f"verification failed: {res}")
+        return {"total": e[0].elapsed_time(e[3]), "plan_host": (t1 - t0) * 1e3, "cost_host": (t2 - t1) * 1e3,
+                "plan_to_launch": e[0].elapsed_time(e[1]), "execute": e[1].elapsed_time(e[2]),
+                "verify": e[2].elapsed_time(e[3]), "T_over_T0": cost["T_over_T0"]}
+
+    for _ in range(max(args.warmup, 3)):
+        restore()
+        full_step(False)
+    sampler = ClockSampler(local)
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize(dev)
+    sampler.start()
+    recs = []
+    wall0 = time.perf_counter()
+    for _ in range(args.steps):
+        restore()
+        torch.cuda.synchronize(dev)
+        recs.append(full_step(True))
+    torch.cuda.synchronize(dev)
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop()
+    if dist:
+        dist.barrier()
+    mean = lambda key: sum(r[key] for r in recs) / len(recs)
+    t_step, t_exec, t_ver = mean("total"), mean("execute"), mean("verify")
+    if dist:
+        tt = torch.tensor([t_step, t_exec, t_ver], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_step, t_exec, t_ver = [float(v) for v in tt]
+
+    # parity spot-check of the last timed step against the fp64 sum on sampled elements (cheap, outside timing)
+    idx = W.sample_indices(w, 4096)
+    y0 = sess.bufs[0][torch.from_numpy(idx).to(dev)].float().cpu().numpy().astype(np.float64)
+    if w.dtype == W.F32:
+        xs = x[:, idx].astype(np.float64)
+        tol = w.p * 2.0 ** -23 * np.abs(xs).sum(0)
+    else:
+        xs = (x[:, idx].astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+        tol = 2.0 ** -7 * np.abs(xs.sum(0)) + w.p * 2.0 ** -23 * np.abs(xs).sum(0)
+    parity_ok = bool((np.abs(y0 - xs.sum(0)) <= tol).all())
+
+    # e2e: the same step through the C-ABI call with HOST buffers, H2D + D2H inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        hin = [torch.from_numpy(x[r]).pin_memory() if w.dtype == W.F32 else
+               torch.from_numpy(x[r].view(np.int16)).pin_memory() for r in range(w.p)]
+        hout = [torch.empty_like(t).pin_memory() for t in hin]
+        ts = []
+        for i in range(1 + args.e2e_steps):
+            a, b_ = ev(), ev()
+            torch.cuda.synchronize(dev)
+            a.record(stream)
+            plan = mk()
+            B.optcc_cost(plan)
+            sess.plan = plan
+            sess.execute_host(hin, hout)
+            res = sess.verify()
+            b_.record(stream)
+            torch.cuda.synchronize(dev)
+            if i:
+                ts.append(a.elapsed_time(b_))
+        t_e2e = sum(ts) / len(ts)
+        if dist:
+            tt = torch.tensor([t_e2e], device=dev, dtype=torch.float64)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            t_e2e = float(tt[0])
+        ok = all(torch.equal(hout[0], h) for h in hout[1:])
+        e2e = {"value": world * w.n * esize / t_e2e / 1e6, "unit": UNIT, "h2d_bytes_per_step": w.p * w.n * esize,
+               "d2h_bytes_per_step": w.p * w.n * esize, "ms_per_step": t_e2e, "steps": len(ts),
+               "all_ranks_identical": bool(ok)}
+        del hin, hout
+
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return 0
+
+    peak, peak_src = measured_peak()
+    kern = "optcc_exec_kernel<MODE_F32>" if w.dtype == W.F32 else "optcc_exec_kernel<MODE_BF16>"
+    achieved = sched_bytes / t_exec / 1e6
+    mask_bytes = 5 * (w.p - 1) * w.n * 8 * plan0.info["mask_words"]
+    line = {
+        "metric": METRIC, "value": world * w.n * esize / t_step / 1e6, "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": t_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32" if w.dtype == W.F32 else "bf16(f32 accumulate)",
+        "data": "synthetic",
+        "config": {"workload": workload_name(w, k), "step": "optcc_plan + optcc_cost + optcc_execute + optcc_verify (SURVEY 8(a) a1-a8)",
+                   "exec_mode": "persistent cooperative kernel, grid barrier per step" if args.exec_mode == 0 else "one launch per step",
+                   "plan_steps": plan0.info["n_steps"], "plan_flows": plan0.info["n_flows"], "parallelism": f"replicas x{world} (element-axis shards, no collective)",
+                   "l2": "inputs larger than L2 (footprint %.2f GB) and restored from a pristine copy between steps, untimed" % (w.p * w.n * esize / 1e9)},
+        "execute_only": {"algbw": world * w.n * esize / t_exec / 1e6, "unit": UNIT, "ms": t_exec,
+                         "schedule_GBs": achieved, "pct_of_8TBs_nominal": achieved / 8000 * 100,
+                         "pct_of_measured_peak": achieved / peak * 100},
+        "breakdown_ms": {"plan_host": mean("plan_host"), "cost_host": mean("cost_host"), "plan_to_launch": mean("plan_to_launch"),
+                         "execute": t_exec, "verify": t_ver},
+        "model": {"T_over_T0": cost0["T_over_T0"], "lb_table1_over_T0": cost0["lb_table1"] / cost0["T0"],
+                  "lb_tight_over_T0": (cost0["lb_tight"] / cost0["T0"]) if cost0["lb_tight"] == cost0["lb_tight"] else None,
+                  "paper_closed_form_over_T0": cost0["T_closed_form"] / cost0["T0"], "limit_over_T0": cost0["T_limit"] / cost0["T0"],
+                  "bodies": cost0["bodies"], "k": k,
+                  "paper_context": "SimAI: OPTCC within 2-6% of fault-free NCCL ring at <=50% bandwidth loss; prior work up to 57% (PAPER.md:7)"},
+        "roofline": {"bound": "hbm", "kernel": kern, "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": ncu_traffic(w.name.split("[")[0], kern),
+                     "algorithmic_bytes_per_launch": sched_bytes, "share_of_step": t_exec / t_step},
+        "roofline_verify": {"bound": "hbm", "kernel": "optcc_exec_kernel<MODE_MASK%d> (+init, check)" % plan0.info["mask_words"],
+                            "achieved": mask_bytes / t_ver / 1e6, "peak": peak, "unit": "GB/s", "frac": mask_bytes / t_ver / 1e6 / peak,
+                            "share_of_step": t_ver / t_step},
+        "parity_spot_check": {"sampled_elements": int(len(idx)), "within_tolerance": parity_ok},
+        "clocks": clocks, "gpu_launches": launches_per_step * args.steps, "wall_s_timed_region": wall,
+    }
+    if e2e:
+        line["e2e"] = e2e
+    if world == 1 and not args.no_cpu_baseline:
+        ws = w.scaled(min(w.n, 2 ** (args.cpu_sample_log2 or 24)))
+        t = oracle_step(ws, k)
+        line["cpu_baseline"] = {"value": ws.n * esize / t / 1e9, "unit": UNIT, "cores": cpu_threads_used(), "kind": "oracle",
+                                "sample": f"n={ws.n} elements per rank of the config's n={w.n}, all p={w.p} ranks, every flow; {t:.1f} s",
+                                "host_cores": os.cpu_count()}
+    if not parity_ok:
+        line["error"] = "parity spot check failed"
+    print(json.dumps(line), flush=True)
+    if dist:
+        dist.destroy_process_group()
+    return 0 if parity_ok else 1
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    sys.exit(run_reference(a) if a.impl == "reference" else run_native(a))
