@@ -49,7 +49,10 @@ enum { OPTCC_C0 = 0, OPTCC_C1 = 1, OPTCC_C2 = 2, OPTCC_C3 = 3 };
 /* executor modes */
 enum {
   OPTCC_EXEC_PERSISTENT = 0, /* one cooperative kernel for the whole schedule, grid barrier between steps */
-  OPTCC_EXEC_PER_STEP = 1    /* one kernel launch per step (stream order is the step barrier) */
+  OPTCC_EXEC_PER_STEP = 1,   /* one kernel launch per step (stream order is the step barrier) */
+  OPTCC_EXEC_DATAFLOW = 2    /* one cooperative kernel, no grid barrier: every flow is cut into tiles, tile-ops are
+                                claimed in table order and wait on per-(rank, range) completion counters, so a
+                                tile-op starts as soon as the flows it depends on have finished there */
 };
 
 typedef struct optcc_plan optcc_plan_t; /* opaque; immutable after creation except for cached device state */
@@ -77,7 +80,7 @@ typedef struct optcc_opts {
   uint32_t copy_path; /* 0 = auto, 1 = LDG/STG vector copy, 2 = cp.async.bulk (TMA 1-D) copy */
   uint32_t step_limit;/* 0 = all steps; else execute / verify only the first step_limit steps (debugging and
                          profiling: a truncated schedule must FAIL verification) */
-  uint32_t reserved;  /* 0 */
+  uint32_t tile_units;/* dataflow executor: 16-byte units per tile-op; 0 = auto (2048 = 32 KB of f32/bf16) */
 } optcc_opts_t;
 
 typedef struct optcc_plan_info {

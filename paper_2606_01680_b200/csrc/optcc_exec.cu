@@ -43,7 +43,7 @@ __device__ __forceinline__ char* rank_ptr(const ExecParams& P, unsigned int r) {
 }
 
 // One piece of one flow: 16-byte units [ubeg, uend) of the flow, executed by the whole CTA.
-template <int MODE>
+template <int MODE, int NT>
 __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& f, unsigned long long ubeg,
                                               unsigned long long uend, unsigned int& overlaps) {
   using MT = ModeTraits<MODE>;
@@ -58,7 +58,7 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
   if (MODE == MODE_F32) {
     const char* s = rank_ptr(P, f.src) + f.off * 4;
     char* d = rank_ptr(P, f.dst) + f.off * 4;
-    if (f.op == 0) range_add_f32<4>(s, d, vbeg, vend); else range_copy16<4>(s, d, vbeg, vend);
+    if (f.op == 0) range_add_f32<4, NT>(s, d, vbeg, vend); else range_copy16<4, NT>(s, d, vbeg, vend);
     if (threadIdx.x < tail) {
       unsigned long long e = vend * 4 + threadIdx.x;
       const float* sf = reinterpret_cast<const float*>(s);
@@ -71,7 +71,7 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
     constexpr int W = MODE == MODE_MASK1 ? 1 : 2;
     const char* s = rank_ptr(P, f.src) + f.off * (8 * W);
     char* d = rank_ptr(P, f.dst) + f.off * (8 * W);
-    if (f.op == 0) range_or_mask<4, W>(s, d, vbeg, vend, overlaps); else range_copy16<4>(s, d, vbeg, vend);
+    if (f.op == 0) range_or_mask<4, W, NT>(s, d, vbeg, vend, overlaps); else range_copy16<4, NT>(s, d, vbeg, vend);
     if (threadIdx.x < tail) {  // MASK1 only: one odd element
       unsigned long long e = vend * 2;
       const unsigned long long* sm = reinterpret_cast<const unsigned long long*>(s);
@@ -93,19 +93,19 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
                          : rank_ptr(P, f.dst) + f.off * 2;
     if (f.op == 0) {
       switch ((f.ksrc << 2) | (f.kdin << 1) | f.kdout) {
-        case 0: range_add_bf16<0, 0, 0>(s, di, dout, vbeg, vend); break;
-        case 1: range_add_bf16<0, 0, 1>(s, di, dout, vbeg, vend); break;
-        case 2: range_add_bf16<0, 1, 0>(s, di, dout, vbeg, vend); break;
-        case 3: range_add_bf16<0, 1, 1>(s, di, dout, vbeg, vend); break;
-        case 4: range_add_bf16<1, 0, 0>(s, di, dout, vbeg, vend); break;
-        case 5: range_add_bf16<1, 0, 1>(s, di, dout, vbeg, vend); break;
-        case 6: range_add_bf16<1, 1, 0>(s, di, dout, vbeg, vend); break;
-        default: range_add_bf16<1, 1, 1>(s, di, dout, vbeg, vend); break;
+        case 0: range_add_bf16<0, 0, 0, NT>(s, di, dout, vbeg, vend); break;
+        case 1: range_add_bf16<0, 0, 1, NT>(s, di, dout, vbeg, vend); break;
+        case 2: range_add_bf16<0, 1, 0, NT>(s, di, dout, vbeg, vend); break;
+        case 3: range_add_bf16<0, 1, 1, NT>(s, di, dout, vbeg, vend); break;
+        case 4: range_add_bf16<1, 0, 0, NT>(s, di, dout, vbeg, vend); break;
+        case 5: range_add_bf16<1, 0, 1, NT>(s, di, dout, vbeg, vend); break;
+        case 6: range_add_bf16<1, 1, 0, NT>(s, di, dout, vbeg, vend); break;
+        default: range_add_bf16<1, 1, 1, NT>(s, di, dout, vbeg, vend); break;
       }
     } else if (f.ksrc == 0) {
-      range_copy16<4>(s, dout, vbeg, vend);                 // bf16 -> bf16: one vector per unit
+      range_copy16<4, NT>(s, dout, vbeg, vend);                 // bf16 -> bf16: one vector per unit
     } else {
-      range_copy16<4>(s, dout, vbeg * 2, vend * 2);         // fp32 partial -> fp32 partial: two vectors per unit
+      range_copy16<4, NT>(s, dout, vbeg * 2, vend * 2);         // fp32 partial -> fp32 partial: two vectors per unit
     }
     if (threadIdx.x < tail) {
       unsigned long long e = vend * 8 + threadIdx.x;
@@ -170,7 +170,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) optcc_exec_kernel(const 
       const unsigned long long nunits = (f.len + A - 1) / A;
       const unsigned long long ubeg = i == 0 ? ub : 0ull;
       const unsigned long long uend = (i + 1 == nf && ue > 0) ? ue : nunits;
-      process_piece<MODE>(P, f, ubeg, uend, overlaps);
+      process_piece<MODE, THREADS>(P, f, ubeg, uend, overlaps);
     }
     if (step + 1 < P.step_hi) {
       if (P.use_barrier) grid_barrier(&P.ctrl->barrier, (unsigned long long)(step - P.step_lo + 1) * G);
@@ -183,6 +183,118 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) optcc_exec_kernel(const 
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) overlaps += __shfl_xor_sync(0xFFFFFFFFu, overlaps, o);
     if ((threadIdx.x & 31) == 0 && overlaps) atomicAdd(&P.ctrl->overlap, (unsigned long long)overlaps);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Dataflow executor: no grid barrier.  15 streaming warps + 1 scheduler warp per CTA.  The scheduler claims the
+// next tile-op (global ticket, table order), fetches its flow record into a shared-memory slot (the "segment
+// table" of this CTA: two slots, one being streamed, one being prepared), waits until the accesses it depends on
+// have completed (per-(rank, region, tile) counters, ld.acquire.gpu), and publishes the slot.  Streaming warps
+// never synchronise with each other: each polls the slot's sequence number, streams its share, and bumps a
+// shared done-counter; the scheduler then fences and bumps the global counters of the ranges the op touched.
+// Claims are made in table order and an op only waits on ops with smaller tickets, each held by a resident CTA
+// (cooperative launch), so progress is guaranteed.
+// ---------------------------------------------------------------------------------------------------------
+struct DfSlot {
+  DFlow f;
+  unsigned long long ubeg, uend;
+  unsigned int valid;
+  unsigned int pad[3];
+};
+
+__device__ __forceinline__ unsigned int ld_acquire_gpu_u32(const unsigned int* p) {
+  unsigned int v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ unsigned int ld_acquire_cta_shared_u32(const unsigned int* p) {
+  unsigned int v;
+  asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(v) : "r"((unsigned int)__cvta_generic_to_shared(p)) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_cta_shared_u32(unsigned int* p, unsigned int v) {
+  asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"((unsigned int)__cvta_generic_to_shared(p)), "r"(v) : "memory");
+}
+__device__ __forceinline__ void red_release_cta_shared_add(unsigned int* p, unsigned int v) {
+  asm volatile("red.release.cta.shared.add.u32 [%0], %1;" ::"r"((unsigned int)__cvta_generic_to_shared(p)), "r"(v) : "memory");
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel(const __grid_constant__ ExecParams P) {
+  constexpr unsigned int NW = DF_COMPUTE_THREADS / 32;   // streaming warps
+  __shared__ DfSlot s_slot[2];
+  __shared__ unsigned int s_full[2];    // sequence number of the op published in the slot (j + 1)
+  __shared__ unsigned int s_done[2];    // streaming warps that finished the slot's op (monotone)
+  if (threadIdx.x < 2) { s_full[threadIdx.x] = 0; s_done[threadIdx.x] = 0; }
+  __syncthreads();
+  unsigned int overlaps = 0;
+
+  if (threadIdx.x >= DF_COMPUTE_THREADS) {
+    // ---------------- scheduler warp (lane 0 works) ----------------
+    if (threadIdx.x == DF_COMPUTE_THREADS) {
+      unsigned int c_src[2] = {0u, 0u}, c_dst[2] = {0u, 0u};   // counters to bump when the slot's op completes
+      unsigned int completed = 0;               // ops completed (in order)
+      auto try_complete = [&](unsigned int j) -> bool {   // op j (0-based) sits in slot j & 1
+        const unsigned int s = j & 1;
+        if (ld_acquire_cta_shared_u32(&s_done[s]) < NW * (j / 2 + 1)) return false;
+        __threadfence();
+        atomicAdd(P.counters + c_src[s], 1u);
+        atomicAdd(P.counters + c_dst[s], 1u);
+        return true;
+      };
+      unsigned int j = 0;
+      for (;; ++j) {
+        const unsigned int s = j & 1;
+        while (completed + 2 <= j) { if (try_complete(completed)) ++completed; }   // slot s must be free
+        const unsigned long long t = atomicAdd(&P.ctrl->ticket, 1ull);
+        if (t >= P.n_ops) break;
+        const unsigned long long opw = __ldg(reinterpret_cast<const unsigned long long*>(P.ops + t));
+        TileOp op;
+        op.flow = (unsigned int)opw;
+        op.tile = (unsigned int)(opw >> 32);
+        const uint4* fr = reinterpret_cast<const uint4*>(P.flows + op.flow);
+        const uint4 f0 = __ldg(fr), f1 = __ldg(fr + 1);
+        const uint4 dp = __ldg(reinterpret_cast<const uint4*>(P.deps + op.flow));
+        DfSlot& sl = s_slot[s];
+        memcpy(&sl.f, &f0, 16);
+        memcpy(reinterpret_cast<char*>(&sl.f) + 16, &f1, 16);
+        const unsigned long long A = P.unit_elems, nunits = (sl.f.len + A - 1) / A;
+        sl.ubeg = (unsigned long long)op.tile * P.tile_units;
+        sl.uend = sl.ubeg + P.tile_units < nunits ? sl.ubeg + P.tile_units : nunits;
+        sl.valid = 1;
+        c_src[s] = dp.x + op.tile;
+        c_dst[s] = dp.y + op.tile;
+        // wait for the accesses this op depends on; keep completing our own earlier op meanwhile
+        for (;;) {
+          const bool ok = ld_acquire_gpu_u32(P.counters + c_src[s]) >= dp.z && ld_acquire_gpu_u32(P.counters + c_dst[s]) >= dp.w;
+          if (ok) break;
+          if (completed < j && try_complete(completed)) ++completed;
+        }
+        st_release_cta_shared_u32(&s_full[s], j + 1);
+      }
+      // drain: complete what is still streaming, then tell the streaming warps to stop
+      while (completed < j) { if (try_complete(completed)) ++completed; }
+      s_slot[j & 1].valid = 0;
+      st_release_cta_shared_u32(&s_full[j & 1], j + 1);
+    }
+  } else {
+    // ---------------- streaming warps ----------------
+    for (unsigned int j = 0;; ++j) {
+      const unsigned int s = j & 1;
+      while (ld_acquire_cta_shared_u32(&s_full[s]) < j + 1) { }
+      if (!s_slot[s].valid) break;
+      const DFlow f = s_slot[s].f;
+      const unsigned long long ubeg = s_slot[s].ubeg, uend = s_slot[s].uend;
+      process_piece<MODE, DF_COMPUTE_THREADS>(P, f, ubeg, uend, overlaps);
+      __syncwarp();
+      if ((threadIdx.x & 31) == 0) red_release_cta_shared_add(&s_done[s], 1u);
+    }
+    if (MODE == MODE_MASK1 || MODE == MODE_MASK2) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) overlaps += __shfl_xor_sync(0xFFFFFFFFu, overlaps, o);
+      if ((threadIdx.x & 31) == 0 && overlaps) atomicAdd(&P.ctrl->overlap, (unsigned long long)overlaps);
+    }
   }
 }
 
@@ -247,11 +359,56 @@ struct optcc_exec_state {
   void* prepared_ws = nullptr;    // workspace that currently holds the device tables
   std::vector<DFlow> dflows;
   std::vector<Slice> slices;      // [n_steps][G + 1]
+  // dataflow executor
+  uint32_t G_df = 0;              // grid of the dataflow kernel
+  bool df_ok = false;             // counters fit 32-bit indices
+  std::vector<DDep> deps;         // [n_flows]
+  std::vector<TileOp> ops;        // [n_tile_ops], table order
+  std::vector<uint64_t> step_op_begin;   // [n_steps + 1]
 };
 
 void optcc_exec_state_free(optcc_exec_state* s) { delete s; }
 
 namespace {
+
+template <int MODE>
+int df_kernel_occupancy(int* out) {
+  CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, optcc_dataflow_kernel<MODE>, DF_THREADS, 0));
+  return OPTCC_OK;
+}
+
+// Dataflow tables: tile-ops in table order and, per flow, the completion counts its ranges must have reached.
+// Per (rank, region) the accesses are ordered as in the table; a read waits for the last write before it, a write
+// for every earlier access (see optcc_dataflow_kernel).
+void build_dataflow_tables(optcc_plan_t* pl, optcc_exec_state* st) {
+  const optcc_plan_info_t& in = pl->info;
+  const uint64_t A = in.unit_elems, TU = pl->tile_units, nr = pl->region_offs.size();
+  st->df_ok = uint64_t(in.p) * pl->tiles_per_rank < (uint64_t(1) << 32) && pl->n_tile_ops < (uint64_t(1) << 40);
+  if (!st->df_ok) return;
+  std::vector<uint32_t> count(size_t(in.p) * nr, 0), lastw(size_t(in.p) * nr, 0);
+  st->deps.resize(in.n_flows);
+  st->ops.clear();
+  st->ops.reserve(pl->n_tile_ops);
+  st->step_op_begin.assign(in.n_steps + 1, 0);
+  uint32_t step = 0;
+  for (uint32_t i = 0; i < in.n_flows; ++i) {
+    const optcc_flow_t& f = pl->flows[i];
+    while (step < f.step) st->step_op_begin[++step] = st->ops.size();
+    const size_t reg = size_t(std::lower_bound(pl->region_offs.begin(), pl->region_offs.end(), f.off) - pl->region_offs.begin());
+    const size_t ls = size_t(f.src) * nr + reg, ld = size_t(f.dst) * nr + reg;
+    DDep d;
+    d.csrc = uint32_t(uint64_t(f.src) * pl->tiles_per_rank + pl->region_tile0[reg]);
+    d.cdst = uint32_t(uint64_t(f.dst) * pl->tiles_per_rank + pl->region_tile0[reg]);
+    d.need_src = lastw[ls];
+    count[ls]++;
+    d.need_dst = count[ld];
+    lastw[ld] = ++count[ld];
+    st->deps[i] = d;
+    const uint64_t ntiles = ((f.len + A - 1) / A + TU - 1) / TU;
+    for (uint64_t t = 0; t < ntiles; ++t) st->ops.push_back(TileOp{i, uint32_t(t)});
+  }
+  while (step < in.n_steps) st->step_op_begin[++step] = st->ops.size();
+}
 
 template <int MODE>
 int kernel_occupancy(int* out) {
@@ -296,6 +453,19 @@ int build_state(optcc_plan_t* pl) {
   uint32_t maxG = std::min<uint32_t>(uint32_t(st->sm_count) * uint32_t(occ), OPTCC_MAX_GRID);
   uint32_t G = pl->opts.grid_ctas ? std::min(pl->opts.grid_ctas, maxG) : maxG;
   st->G = G;
+  {
+    int od = 0, o2 = 0;
+    if ((rc = df_kernel_occupancy<MODE_F32>(&o2)) != OPTCC_OK) return rc;
+    od = o2;
+    if ((rc = df_kernel_occupancy<MODE_BF16>(&o2)) != OPTCC_OK) return rc;
+    od = std::min(od, o2);
+    if ((rc = df_kernel_occupancy<MODE_MASK1>(&o2)) != OPTCC_OK) return rc;
+    od = std::min(od, o2);
+    if ((rc = df_kernel_occupancy<MODE_MASK2>(&o2)) != OPTCC_OK) return rc;
+    od = std::min(std::min(od, o2), CTAS_PER_SM);
+    uint32_t maxGd = std::min<uint32_t>(uint32_t(st->sm_count) * uint32_t(std::max(od, 0)), OPTCC_MAX_GRID);
+    st->G_df = pl->opts.grid_ctas ? std::min(pl->opts.grid_ctas, maxGd) : maxGd;
+  }
 
   const optcc_plan_info_t& in = pl->info;
   const uint64_t A = in.unit_elems;
@@ -331,6 +501,7 @@ int build_state(optcc_plan_t* pl) {
         row[c].unit = i < hi ? (Bc - prefix) / unit_cost(pl, i) : 0;
       }
     }
+    build_dataflow_tables(pl, st);
   } catch (const std::bad_alloc&) {
     return OPTCC_ENOMEM;
   }
@@ -340,13 +511,17 @@ int build_state(optcc_plan_t* pl) {
 int upload_tables(optcc_plan_t* pl, void* workspace, cudaStream_t stream) {
   optcc_exec_state* st = pl->exec;
   if (st->prepared_ws == workspace) return OPTCC_OK;
-  const optcc_ws_layout L = optcc_layout(pl->info);
+  const optcc_ws_layout L = optcc_layout(pl);
   char* ws = static_cast<char*>(workspace);
   CU_TRY(cudaMemsetAsync(ws + L.ctrl, 0, OPTCC_CTRL_BYTES, stream));
   if (!st->dflows.empty())
     CU_TRY(cudaMemcpyAsync(ws + L.dflows, st->dflows.data(), st->dflows.size() * sizeof(DFlow), cudaMemcpyHostToDevice, stream));
   if (!st->slices.empty())
     CU_TRY(cudaMemcpyAsync(ws + L.slices, st->slices.data(), st->slices.size() * sizeof(Slice), cudaMemcpyHostToDevice, stream));
+  if (st->df_ok && !st->ops.empty()) {
+    CU_TRY(cudaMemcpyAsync(ws + L.deps, st->deps.data(), st->deps.size() * sizeof(DDep), cudaMemcpyHostToDevice, stream));
+    CU_TRY(cudaMemcpyAsync(ws + L.ops, st->ops.data(), st->ops.size() * sizeof(TileOp), cudaMemcpyHostToDevice, stream));
+  }
   st->prepared_ws = workspace;
   return OPTCC_OK;
 }
@@ -363,7 +538,15 @@ int launch_plan(optcc_plan_t* pl, ExecParams& P, cudaStream_t stream) {
   const uint32_t n_steps = plan_steps(pl);
   if (n_steps == 0) return OPTCC_OK;
   const bool persistent = pl->opts.exec_mode == OPTCC_EXEC_PERSISTENT && st->coop;
-  if (persistent) {
+  const bool dataflow = pl->opts.exec_mode == OPTCC_EXEC_DATAFLOW && st->coop && st->df_ok && st->G_df > 0;
+  if (dataflow) {
+    P.n_ops = st->step_op_begin[n_steps];
+    if (P.n_ops == 0) return OPTCC_OK;
+    CU_TRY(cudaMemsetAsync(P.counters, 0, size_t(in.p) * pl->tiles_per_rank * sizeof(unsigned int), stream));
+    CU_TRY(cudaMemsetAsync(&P.ctrl->ticket, 0, sizeof(unsigned long long), stream));
+    void* args[] = {&P};
+    CU_TRY(cudaLaunchCooperativeKernel((const void*)optcc_dataflow_kernel<MODE>, dim3(st->G_df), dim3(DF_THREADS), args, 0, stream));
+  } else if (persistent) {
     CU_TRY(cudaMemsetAsync(&P.ctrl->barrier, 0, sizeof(unsigned long long), stream));
     P.step_lo = 0;
     P.step_hi = n_steps;
@@ -384,7 +567,7 @@ int launch_plan(optcc_plan_t* pl, ExecParams& P, cudaStream_t stream) {
 }
 
 void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
-  const optcc_ws_layout L = optcc_layout(pl->info);
+  const optcc_ws_layout L = optcc_layout(pl);
   char* ws = static_cast<char*>(workspace);
   std::memset(&P, 0, sizeof P);
   P.flows = reinterpret_cast<const DFlow*>(ws + L.dflows);
@@ -393,6 +576,10 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   P.shadow = reinterpret_cast<float*>(ws + L.shadow);
   P.padded_n = pl->info.padded_n;
   P.unit_elems = pl->info.unit_elems;
+  P.deps = reinterpret_cast<const DDep*>(ws + L.deps);
+  P.ops = reinterpret_cast<const TileOp*>(ws + L.ops);
+  P.counters = reinterpret_cast<unsigned int*>(ws + L.counters);
+  P.tile_units = pl->tile_units;
 }
 
 }  // namespace
@@ -419,7 +606,7 @@ extern "C" int optcc_execute(optcc_plan_t* plan, void* const* bufs, void* worksp
   if (in.p <= (uint32_t)MAX_PARAM_PTRS) {
     for (uint32_t r = 0; r < in.p; ++r) P.bufs[r] = bufs[r];
   } else {
-    const optcc_ws_layout L = optcc_layout(in);
+    const optcc_ws_layout L = optcc_layout(plan);
     char* ws = static_cast<char*>(workspace);
     CU_TRY(cudaMemcpyAsync(ws + L.ptrs, bufs, size_t(in.p) * sizeof(void*), cudaMemcpyHostToDevice, stream));
     P.ptr_table = reinterpret_cast<void* const*>(ws + L.ptrs);
@@ -450,7 +637,7 @@ extern "C" int optcc_verify(optcc_plan_t* plan, void* workspace, void* stream_, 
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   int rc = optcc_prepare(plan, workspace, stream_);
   if (rc != OPTCC_OK) return rc;
-  const optcc_ws_layout L = optcc_layout(in);
+  const optcc_ws_layout L = optcc_layout(plan);
   char* ws = static_cast<char*>(workspace);
   unsigned long long* masks = reinterpret_cast<unsigned long long*>(ws + L.masks);
   ExecParams P;

@@ -26,6 +26,13 @@ struct optcc_plan {
   std::vector<uint64_t> p2p_bounds;
   // per flow, bf16 plans only: storage kinds of src, dst before, dst after (host walk over contributor counts)
   std::vector<uint8_t> kind_src, kind_dst_in, kind_dst_out;
+  // dataflow executor (exec_mode 2): every flow is cut into tiles of `tile_units` 16-byte units; tile-ops are
+  // claimed in table order and wait on per-(rank, region, tile) completion counters instead of a grid barrier
+  uint32_t tile_units = 0;
+  uint64_t n_tile_ops = 0;              // sum over flows of ceil(units / tile_units)
+  uint64_t tiles_per_rank = 0;          // sum over regions of ceil(units / tile_units): counters per rank
+  std::vector<uint64_t> region_offs;    // sorted unique flow offsets (regions tile [0, n), PLAN_SPEC 5.4)
+  std::vector<uint64_t> region_tile0;   // first tile counter of every region (prefix sum)
   optcc_exec_state* exec;               // created lazily by the executor; freed by optcc_plan_destroy
 };
 
@@ -33,25 +40,33 @@ struct optcc_plan {
 void optcc_exec_state_free(optcc_exec_state*);
 
 // ---- device workspace layout (bytes from the workspace base; every region 256-byte aligned) -----------------
-//   control block | rank pointers | device flow records | per-(step, CTA) slice table | fp32 shadow (bf16 plans) | masks (verify)
+//   control block | rank pointers | device flow records | per-(step, CTA) slice table | dataflow deps, tile-ops, counters | fp32 shadow (bf16 plans) | masks (verify)
 constexpr uint32_t OPTCC_MAX_GRID = 1024;       // upper bound on executor CTAs (sizes the slice table)
 constexpr uint64_t OPTCC_CTRL_BYTES = 256;
 constexpr uint64_t OPTCC_DFLOW_BYTES = 32;      // sizeof(DFlow) in optcc_exec.cu
 constexpr uint64_t OPTCC_SLICE_BYTES = 16;      // sizeof(Slice)
 
 struct optcc_ws_layout {
-  uint64_t ctrl, ptrs, dflows, slices, shadow, masks, end_exec, end_verify;
+  uint64_t ctrl, ptrs, dflows, slices, deps, ops, counters, shadow, masks, end_exec, end_verify;
 };
 
 static inline uint64_t optcc_align256(uint64_t x) { return (x + 255) & ~uint64_t(255); }
 
-static inline optcc_ws_layout optcc_layout(const optcc_plan_info_t& in) {
+constexpr uint32_t OPTCC_TILE_UNITS_DEFAULT = 2048;  // 32 KB of f32 / bf16 per tile-op
+constexpr uint64_t OPTCC_DEP_BYTES = 16;             // sizeof(DDep)
+constexpr uint64_t OPTCC_OP_BYTES = 8;               // sizeof(TileOp)
+
+static inline optcc_ws_layout optcc_layout(const optcc_plan_t* pl) {
+  const optcc_plan_info_t& in = pl->info;
   optcc_ws_layout L;
   L.ctrl = 0;
   L.ptrs = OPTCC_CTRL_BYTES;                                   // rank pointer table (used when p > 128)
   L.dflows = optcc_align256(L.ptrs + uint64_t(in.p) * 8);
   L.slices = optcc_align256(L.dflows + uint64_t(in.n_flows) * OPTCC_DFLOW_BYTES);
-  L.shadow = optcc_align256(L.slices + uint64_t(in.n_steps) * (OPTCC_MAX_GRID + 1) * OPTCC_SLICE_BYTES);
+  L.deps = optcc_align256(L.slices + uint64_t(in.n_steps) * (OPTCC_MAX_GRID + 1) * OPTCC_SLICE_BYTES);
+  L.ops = optcc_align256(L.deps + uint64_t(in.n_flows) * OPTCC_DEP_BYTES);
+  L.counters = optcc_align256(L.ops + pl->n_tile_ops * OPTCC_OP_BYTES);
+  L.shadow = optcc_align256(L.counters + uint64_t(in.p) * pl->tiles_per_rank * 4);
   uint64_t n_pad = (in.n + 7) & ~uint64_t(7);
   L.end_exec = optcc_align256(L.shadow + (in.dtype == OPTCC_BF16 ? uint64_t(in.p) * n_pad * 4 : 0));
   L.masks = L.end_exec;

@@ -42,11 +42,24 @@ struct __align__(16) Slice {      // start of a CTA's slice of a step: flow inde
 };
 static_assert(sizeof(Slice) == 16, "Slice must be 16 bytes");
 
+struct __align__(16) DDep {       // dataflow dependencies of a flow (same for all its tiles)
+  unsigned int csrc, cdst;        // first tile counter of (src rank, region) / (dst rank, region)
+  unsigned int need_src;          // accesses of the src range that must be complete before it is read
+  unsigned int need_dst;          // accesses of the dst range that must be complete before it is written
+};
+static_assert(sizeof(DDep) == 16, "DDep must be 16 bytes");
+
+struct TileOp { unsigned int flow, tile; };   // one unit of work of the dataflow executor
+
+constexpr int DF_COMPUTE_THREADS = 480;   // 15 streaming warps
+constexpr int DF_THREADS = DF_COMPUTE_THREADS + 32;   // + 1 scheduler warp
+
 struct Ctrl {                     // control block at the start of the workspace
   unsigned long long barrier;     // monotone arrival counter of the grid barrier
   unsigned long long bad;         // verify: wrong final masks
   unsigned long long overlap;     // verify: reduce over overlapping contributor sets
   unsigned long long first_bad;   // verify: smallest bad r*n+e
+  unsigned long long ticket;      // dataflow: next tile-op to claim
 };
 
 struct ExecParams {
@@ -60,6 +73,12 @@ struct ExecParams {
   unsigned int step_lo, step_hi;  // steps [lo, hi) are executed by this launch
   unsigned int unit_elems;        // A (PLAN_SPEC 2)
   unsigned int use_barrier;       // 1: grid barrier between steps (cooperative launch)
+  // dataflow executor
+  const DDep* deps;               // [n_flows]
+  const TileOp* ops;              // [n_ops], table order
+  unsigned int* counters;         // [p * tiles_per_rank] completed accesses per (rank, region, tile)
+  unsigned long long n_ops;
+  unsigned int tile_units;
 };
 
 // ---- memory access helpers: L2-only loads (data written by other SMs in the previous step), streaming stores ----
@@ -101,39 +120,39 @@ __device__ __forceinline__ void grid_barrier(unsigned long long* ctr, unsigned l
 // Range operations.  All ranges are given in 16-byte vectors [vbeg, vend) relative to the flow's start.
 // =====================================================================================================
 
-template <int UNROLL>
+template <int UNROLL, int NT>
 __device__ __forceinline__ void range_copy16(const char* __restrict__ s, char* __restrict__ d,
                                              unsigned long long vbeg, unsigned long long vend) {
   unsigned long long v = vbeg + threadIdx.x;
-  for (; v + (UNROLL - 1) * (unsigned long long)THREADS < vend; v += UNROLL * (unsigned long long)THREADS) {
+  for (; v + (UNROLL - 1) * (unsigned long long)NT < vend; v += UNROLL * (unsigned long long)NT) {
     uint4 x[UNROLL];
 #pragma unroll
-    for (int j = 0; j < UNROLL; ++j) x[j] = ld16(s + (v + j * (unsigned long long)THREADS) * 16);
+    for (int j = 0; j < UNROLL; ++j) x[j] = ld16(s + (v + j * (unsigned long long)NT) * 16);
 #pragma unroll
-    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)THREADS) * 16, x[j]);
+    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, x[j]);
   }
-  for (; v < vend; v += THREADS) st16(d + v * 16, ld16(s + v * 16));
+  for (; v < vend; v += NT) st16(d + v * 16, ld16(s + v * 16));
 }
 
-template <int UNROLL>
+template <int UNROLL, int NT>
 __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* __restrict__ d,
                                               unsigned long long vbeg, unsigned long long vend) {
   unsigned long long v = vbeg + threadIdx.x;
-  for (; v + (UNROLL - 1) * (unsigned long long)THREADS < vend; v += UNROLL * (unsigned long long)THREADS) {
+  for (; v + (UNROLL - 1) * (unsigned long long)NT < vend; v += UNROLL * (unsigned long long)NT) {
     uint4 a[UNROLL], b[UNROLL];
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) {
-      a[j] = ld16(s + (v + j * (unsigned long long)THREADS) * 16);
-      b[j] = ld16(d + (v + j * (unsigned long long)THREADS) * 16);
+      a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16);
+      b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16);
     }
 #pragma unroll
-    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)THREADS) * 16, add_f32x4(b[j], a[j]));
+    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, add_f32x4(b[j], a[j]));
   }
-  for (; v < vend; v += THREADS) st16(d + v * 16, add_f32x4(ld16(d + v * 16), ld16(s + v * 16)));
+  for (; v < vend; v += NT) st16(d + v * 16, add_f32x4(ld16(d + v * 16), ld16(s + v * 16)));
 }
 
 // masks: OR with overlap detection.  WORDS = 64-bit words per element (1 or 2); a 16-byte vector holds 2/WORDS elements
-template <int UNROLL, int WORDS>
+template <int UNROLL, int WORDS, int NT>
 __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* __restrict__ d,
                                               unsigned long long vbeg, unsigned long long vend,
                                               unsigned int& overlaps) {
@@ -143,17 +162,17 @@ __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* 
     overlaps += (WORDS == 1) ? (lo + hi) : ((lo | hi) ? 1u : 0u);
     return make_uint4(a.x | b.x, a.y | b.y, a.z | b.z, a.w | b.w);
   };
-  for (; v + (UNROLL - 1) * (unsigned long long)THREADS < vend; v += UNROLL * (unsigned long long)THREADS) {
+  for (; v + (UNROLL - 1) * (unsigned long long)NT < vend; v += UNROLL * (unsigned long long)NT) {
     uint4 a[UNROLL], b[UNROLL];
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) {
-      a[j] = ld16(s + (v + j * (unsigned long long)THREADS) * 16);
-      b[j] = ld16(d + (v + j * (unsigned long long)THREADS) * 16);
+      a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16);
+      b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16);
     }
 #pragma unroll
-    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)THREADS) * 16, join(a[j], b[j]));
+    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, join(a[j], b[j]));
   }
-  for (; v < vend; v += THREADS) st16(d + v * 16, join(ld16(s + v * 16), ld16(d + v * 16)));
+  for (; v < vend; v += NT) st16(d + v * 16, join(ld16(s + v * 16), ld16(d + v * 16)));
 }
 
 // bf16 plans: a unit is 8 elements = 16 bytes in a rank buffer or 32 bytes in the fp32 shadow.
@@ -186,27 +205,27 @@ __device__ __forceinline__ void store8(char* base, unsigned long long unit, cons
   }
 }
 
-template <int KS, int KD, int KO>
+template <int KS, int KD, int KO, int NT>
 __device__ __forceinline__ void range_add_bf16(const char* __restrict__ s, const char* __restrict__ din,
                                                char* __restrict__ dout, unsigned long long ubeg,
                                                unsigned long long uend) {
   constexpr int UNROLL = 2;
   unsigned long long u = ubeg + threadIdx.x;
-  for (; u + (UNROLL - 1) * (unsigned long long)THREADS < uend; u += UNROLL * (unsigned long long)THREADS) {
+  for (; u + (UNROLL - 1) * (unsigned long long)NT < uend; u += UNROLL * (unsigned long long)NT) {
     float a[UNROLL][8], b[UNROLL][8];
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) {
-      load8<KS>(s, u + j * (unsigned long long)THREADS, a[j]);
-      load8<KD>(din, u + j * (unsigned long long)THREADS, b[j]);
+      load8<KS>(s, u + j * (unsigned long long)NT, a[j]);
+      load8<KD>(din, u + j * (unsigned long long)NT, b[j]);
     }
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) {
 #pragma unroll
       for (int e = 0; e < 8; ++e) b[j][e] = __fadd_rn(b[j][e], a[j][e]);
-      store8<KO>(dout, u + j * (unsigned long long)THREADS, b[j]);
+      store8<KO>(dout, u + j * (unsigned long long)NT, b[j]);
     }
   }
-  for (; u < uend; u += THREADS) {
+  for (; u < uend; u += NT) {
     float a[8], b[8];
     load8<KS>(s, u, a);
     load8<KD>(din, u, b);

@@ -286,7 +286,27 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     delete pl;
     return OPTCC_ENOMEM;
   }
-  optcc_ws_layout L = optcc_layout(in);
+  // dataflow tiling: regions (unique offsets; all flows over one offset share a length, PLAN_SPEC 5.4) and tile counts
+  try {
+    pl->tile_units = pl->opts.tile_units ? pl->opts.tile_units : OPTCC_TILE_UNITS_DEFAULT;
+    std::vector<std::pair<uint64_t, uint64_t>> regs;
+    regs.reserve(pl->flows.size());
+    for (const auto& f : pl->flows) regs.push_back({f.off, f.len});
+    std::sort(regs.begin(), regs.end());
+    regs.erase(std::unique(regs.begin(), regs.end()), regs.end());
+    uint64_t tiles = 0;
+    for (const auto& r : regs) {
+      pl->region_offs.push_back(r.first);
+      pl->region_tile0.push_back(tiles);
+      tiles += ((r.second + B.A - 1) / B.A + pl->tile_units - 1) / pl->tile_units;
+    }
+    pl->tiles_per_rank = tiles;
+    for (const auto& f : pl->flows) pl->n_tile_ops += ((f.len + B.A - 1) / B.A + pl->tile_units - 1) / pl->tile_units;
+  } catch (const std::bad_alloc&) {
+    delete pl;
+    return OPTCC_ENOMEM;
+  }
+  optcc_ws_layout L = optcc_layout(pl);
   in.workspace_bytes = L.end_exec;
   in.verify_workspace_bytes = L.end_verify;
   in.mask_offset_bytes = L.masks;

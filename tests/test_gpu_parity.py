@@ -19,6 +19,8 @@ from oracle import reference as OR
 
 pytestmark = pytest.mark.gpu
 
+MODES = [B.OPTCC_EXEC_PERSISTENT, B.OPTCC_EXEC_PER_STEP, B.OPTCC_EXEC_DATAFLOW]
+
 
 def _session(plan, verify=False):
     from paper_2606_01680_b200.device import Session
@@ -67,7 +69,7 @@ F32_CASES = [
 ]
 
 
-@pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_PERSISTENT, B.OPTCC_EXEC_PER_STEP])
+@pytest.mark.parametrize("exec_mode", MODES)
 @pytest.mark.parametrize("p,g,st,n,k", F32_CASES)
 def test_f32_parity(p, g, st, n, k, exec_mode):
     _run_and_check(_wl(p, g, st, n, W.F32, seed=100 + p), k, exec_mode)
@@ -83,16 +85,30 @@ BF16_CASES = [
 ]
 
 
-@pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_PERSISTENT, B.OPTCC_EXEC_PER_STEP])
+@pytest.mark.parametrize("exec_mode", MODES)
 @pytest.mark.parametrize("p,g,st,n,k", BF16_CASES)
 def test_bf16_parity(p, g, st, n, k, exec_mode):
     _run_and_check(_wl(p, g, st, n, W.BF16, seed=200 + p), k, exec_mode)
 
 
+@pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_PERSISTENT, B.OPTCC_EXEC_DATAFLOW])
 @pytest.mark.parametrize("grid_ctas", [1, 7, 148])
-def test_f32_parity_any_grid(grid_ctas):
-    """Slices are cut per CTA: the result must not depend on the grid."""
-    _run_and_check(_wl(16, 1, {3: 4.0 / 3.0}, 2 ** 16 + 13, W.F32, seed=7), 8, B.OPTCC_EXEC_PERSISTENT, grid_ctas)
+def test_f32_parity_any_grid(grid_ctas, exec_mode):
+    """Work is cut per CTA (slices) or claimed dynamically (tile-ops): the result must not depend on the grid."""
+    _run_and_check(_wl(16, 1, {3: 4.0 / 3.0}, 2 ** 16 + 13, W.F32, seed=7), 8, exec_mode, grid_ctas)
+
+
+@pytest.mark.parametrize("tile_units", [1, 64, 4096])
+def test_dataflow_parity_any_tile_size(tile_units):
+    w = _wl(7, 1, {0: 2.0, 1: 4.0 / 3.0}, 20011, W.F32, seed=11)
+    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=4, exec_mode=B.OPTCC_EXEC_DATAFLOW, tile_units=tile_units)
+    oplan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=4)
+    x = W.all_inputs(w)
+    s = _session(plan)
+    s.upload(x)
+    s.execute()
+    y = s.download()
+    assert y.tobytes() == OI.run_f32(oplan, x).tobytes()
 
 
 MASK_CASES = [
@@ -104,7 +120,7 @@ MASK_CASES = [
 ]
 
 
-@pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_PERSISTENT, B.OPTCC_EXEC_PER_STEP])
+@pytest.mark.parametrize("exec_mode", MODES)
 @pytest.mark.parametrize("p,g,st,n,dtype,k", MASK_CASES)
 def test_verifier_masks_equal_oracle(p, g, st, n, dtype, k, exec_mode):
     ell = [float(st.get(i, 1.0)) for i in range(p)]
@@ -121,7 +137,7 @@ def test_verifier_masks_equal_oracle(p, g, st, n, dtype, k, exec_mode):
     assert (m == OI.full_mask_words(p)[None, None, :]).all()
 
 
-@pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_PERSISTENT, B.OPTCC_EXEC_PER_STEP])
+@pytest.mark.parametrize("exec_mode", MODES)
 @pytest.mark.parametrize("limit", [1, 9, 19])
 def test_verifier_detects_a_truncated_schedule(limit, exec_mode):
     """The verifier is not vacuous: a schedule cut after `limit` steps must fail, with exactly the masks and
