@@ -80,7 +80,7 @@ typedef struct optcc_opts {
   uint32_t copy_path; /* 0 = auto, 1 = LDG/STG vector copy, 2 = cp.async.bulk (TMA 1-D) copy */
   uint32_t step_limit;/* 0 = all steps; else execute / verify only the first step_limit steps (debugging and
                          profiling: a truncated schedule must FAIL verification) */
-  uint32_t tile_units;/* dataflow executor: 16-byte units per tile-op; 0 = auto (2048 = 32 KB of f32/bf16) */
+  uint32_t tile_units;/* dataflow executor: 16-byte units per tile-op; 0 = auto (a power of two in [256, 4096]: about two tile-ops per CTA and step) */
 } optcc_opts_t;
 
 typedef struct optcc_plan_info {
@@ -143,7 +143,7 @@ typedef struct optcc_verify_result {
 /* Build the ell-weighted stage/chunk/step plan of PAPER.md 3 (problem statement :68) and 4.1-4.4 as frozen
  * in docs/PLAN_SPEC.md.  ell [host, p doubles]: slowdown factor of every rank, >= 1; ranks of one server
  * (floor(i/g)) must share ell (PXN pooling, :274, :850).  n: elements per rank.  *out receives a new plan
- * owned by the library (optcc_plan_destroy).  Same as optcc_plan_ex with opts = NULL (k auto). */
+ * owned by the library (optcc_plan_destroy).  Same as optcc_plan_ex with opts = NULL (k auto, dataflow executor). */
 OPTCC_API int optcc_plan(int p, int g, const double* ell, uint64_t n, int dtype, optcc_plan_t** out);
 OPTCC_API int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dtype, const optcc_opts_t* opts,
                   optcc_plan_t** out);

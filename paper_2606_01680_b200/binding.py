@@ -147,7 +147,7 @@ class Plan:
             pass
 
 
-def optcc_plan(p, g, ell, n, dtype, k=0, exec_mode=0, grid_ctas=0, copy_path=0, step_limit=0, tile_units=0):
+def optcc_plan(p, g, ell, n, dtype, k=0, exec_mode=OPTCC_EXEC_DATAFLOW, grid_ctas=0, copy_path=0, step_limit=0, tile_units=0):
     """optcc_plan_ex: returns a Plan.  ell: sequence of p floats."""
     lib = load()
     ell_arr = (C.c_double * len(ell))(*[float(x) for x in ell])

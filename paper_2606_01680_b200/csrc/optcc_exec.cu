@@ -5,6 +5,7 @@
 // <= t (:138 data dependencies).  No tensor cores: nothing here is a dense contraction.
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -45,7 +46,7 @@ __device__ __forceinline__ char* rank_ptr(const ExecParams& P, unsigned int r) {
 // One piece of one flow: 16-byte units [ubeg, uend) of the flow, executed by the whole CTA.
 template <int MODE, int NT>
 __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& f, unsigned long long ubeg,
-                                              unsigned long long uend, unsigned int& overlaps) {
+                                              unsigned long long uend, unsigned int& overlaps, const Pol& pol) {
   using MT = ModeTraits<MODE>;
   const unsigned long long A = P.unit_elems;
   const unsigned long long e0 = ubeg * A;
@@ -58,7 +59,7 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
   if (MODE == MODE_F32) {
     const char* s = rank_ptr(P, f.src) + f.off * 4;
     char* d = rank_ptr(P, f.dst) + f.off * 4;
-    if (f.op == 0) range_add_f32<4, NT>(s, d, vbeg, vend); else range_copy16<4, NT>(s, d, vbeg, vend);
+    if (f.op == 0) range_add_f32<4, NT>(s, d, vbeg, vend, pol); else range_copy16<4, NT>(s, d, vbeg, vend, pol);
     if (threadIdx.x < tail) {
       unsigned long long e = vend * 4 + threadIdx.x;
       const float* sf = reinterpret_cast<const float*>(s);
@@ -71,7 +72,7 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
     constexpr int W = MODE == MODE_MASK1 ? 1 : 2;
     const char* s = rank_ptr(P, f.src) + f.off * (8 * W);
     char* d = rank_ptr(P, f.dst) + f.off * (8 * W);
-    if (f.op == 0) range_or_mask<4, W, NT>(s, d, vbeg, vend, overlaps); else range_copy16<4, NT>(s, d, vbeg, vend);
+    if (f.op == 0) range_or_mask<4, W, NT>(s, d, vbeg, vend, overlaps, pol); else range_copy16<4, NT>(s, d, vbeg, vend, pol);
     if (threadIdx.x < tail) {  // MASK1 only: one odd element
       unsigned long long e = vend * 2;
       const unsigned long long* sm = reinterpret_cast<const unsigned long long*>(s);
@@ -93,19 +94,19 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
                          : rank_ptr(P, f.dst) + f.off * 2;
     if (f.op == 0) {
       switch ((f.ksrc << 2) | (f.kdin << 1) | f.kdout) {
-        case 0: range_add_bf16<0, 0, 0, NT>(s, di, dout, vbeg, vend); break;
-        case 1: range_add_bf16<0, 0, 1, NT>(s, di, dout, vbeg, vend); break;
-        case 2: range_add_bf16<0, 1, 0, NT>(s, di, dout, vbeg, vend); break;
-        case 3: range_add_bf16<0, 1, 1, NT>(s, di, dout, vbeg, vend); break;
-        case 4: range_add_bf16<1, 0, 0, NT>(s, di, dout, vbeg, vend); break;
-        case 5: range_add_bf16<1, 0, 1, NT>(s, di, dout, vbeg, vend); break;
-        case 6: range_add_bf16<1, 1, 0, NT>(s, di, dout, vbeg, vend); break;
-        default: range_add_bf16<1, 1, 1, NT>(s, di, dout, vbeg, vend); break;
+        case 0: range_add_bf16<0, 0, 0, NT>(s, di, dout, vbeg, vend, pol); break;
+        case 1: range_add_bf16<0, 0, 1, NT>(s, di, dout, vbeg, vend, pol); break;
+        case 2: range_add_bf16<0, 1, 0, NT>(s, di, dout, vbeg, vend, pol); break;
+        case 3: range_add_bf16<0, 1, 1, NT>(s, di, dout, vbeg, vend, pol); break;
+        case 4: range_add_bf16<1, 0, 0, NT>(s, di, dout, vbeg, vend, pol); break;
+        case 5: range_add_bf16<1, 0, 1, NT>(s, di, dout, vbeg, vend, pol); break;
+        case 6: range_add_bf16<1, 1, 0, NT>(s, di, dout, vbeg, vend, pol); break;
+        default: range_add_bf16<1, 1, 1, NT>(s, di, dout, vbeg, vend, pol); break;
       }
     } else if (f.ksrc == 0) {
-      range_copy16<4, NT>(s, dout, vbeg, vend);                 // bf16 -> bf16: one vector per unit
+      range_copy16<4, NT>(s, dout, vbeg, vend, pol);                 // bf16 -> bf16: one vector per unit
     } else {
-      range_copy16<4, NT>(s, dout, vbeg * 2, vend * 2);         // fp32 partial -> fp32 partial: two vectors per unit
+      range_copy16<4, NT>(s, dout, vbeg * 2, vend * 2, pol);         // fp32 partial -> fp32 partial: two vectors per unit
     }
     if (threadIdx.x < tail) {
       unsigned long long e = vend * 8 + threadIdx.x;
@@ -131,6 +132,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) optcc_exec_kernel(const 
 
   const unsigned int G = gridDim.x, cta = blockIdx.x;
   unsigned int overlaps = 0;
+  const Pol pol = make_policies(P.l2_hints);
 
   auto stage = [&](unsigned int step, int buf, unsigned int lane) {
     // called by one warp: fetch the slice bounds and up to STAGE flow records of `step`
@@ -170,7 +172,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) optcc_exec_kernel(const 
       const unsigned long long nunits = (f.len + A - 1) / A;
       const unsigned long long ubeg = i == 0 ? ub : 0ull;
       const unsigned long long uend = (i + 1 == nf && ue > 0) ? ue : nunits;
-      process_piece<MODE, THREADS>(P, f, ubeg, uend, overlaps);
+      process_piece<MODE, THREADS>(P, f, ubeg, uend, overlaps, pol);
     }
     if (step + 1 < P.step_hi) {
       if (P.use_barrier) grid_barrier(&P.ctrl->barrier, (unsigned long long)(step - P.step_lo + 1) * G);
@@ -187,14 +189,15 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) optcc_exec_kernel(const 
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Dataflow executor: no grid barrier.  15 streaming warps + 1 scheduler warp per CTA.  The scheduler claims the
-// next tile-op (global ticket, table order), fetches its flow record into a shared-memory slot (the "segment
-// table" of this CTA: two slots, one being streamed, one being prepared), waits until the accesses it depends on
-// have completed (per-(rank, region, tile) counters, ld.acquire.gpu), and publishes the slot.  Streaming warps
-// never synchronise with each other: each polls the slot's sequence number, streams its share, and bumps a
-// shared done-counter; the scheduler then fences and bumps the global counters of the ranges the op touched.
-// Claims are made in table order and an op only waits on ops with smaller tickets, each held by a resident CTA
-// (cooperative launch), so progress is guaranteed.
+// Dataflow executor: no grid barrier.  12 streaming warps + up to 4 scheduler agents (one lane each) per CTA.
+// Agent w owns slot w of a small ring in shared memory (this CTA's staged part of the segment table): it claims the
+// next tile-op (global ticket, table order), fetches its flow record into the slot, waits until the accesses the op
+// depends on have completed (per-(rank, region, tile) counters, ld.acquire.gpu), publishes the slot, waits for the
+// streaming warps to finish it, then fences and bumps the counters of the two ranges the op touched.  Streaming
+// warps never synchronise with each other: each polls the slot's sequence number, streams its share and bumps a
+// shared done-counter.  Tickets are claimed in local order (s_turn), so inside a CTA the local order is the table
+// order; an op only waits on ops with smaller tickets, each held by a resident CTA (cooperative launch), whose
+// streaming warps reach them in order -- progress is guaranteed.
 // ---------------------------------------------------------------------------------------------------------
 struct DfSlot {
   DFlow f;
@@ -223,70 +226,65 @@ __device__ __forceinline__ void red_release_cta_shared_add(unsigned int* p, unsi
 template <int MODE>
 __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel(const __grid_constant__ ExecParams P) {
   constexpr unsigned int NW = DF_COMPUTE_THREADS / 32;   // streaming warps
-  __shared__ DfSlot s_slot[2];
-  __shared__ unsigned int s_full[2];    // sequence number of the op published in the slot (j + 1)
-  __shared__ unsigned int s_done[2];    // streaming warps that finished the slot's op (monotone)
-  if (threadIdx.x < 2) { s_full[threadIdx.x] = 0; s_done[threadIdx.x] = 0; }
+  const unsigned int NS = P.df_slots;                    // slots in the ring = scheduler agents in use (<= DF_SLOTS)
+  __shared__ DfSlot s_slot[DF_SLOTS];
+  __shared__ unsigned int s_full[DF_SLOTS];   // sequence number of the op published in the slot (j + 1)
+  __shared__ unsigned int s_done[DF_SLOTS];   // streaming warps that finished ops of the slot (monotone)
+  __shared__ unsigned int s_turn;             // local sequence number whose ticket is claimed next
+  if (threadIdx.x < DF_SLOTS) { s_full[threadIdx.x] = 0; s_done[threadIdx.x] = 0; }
+  if (threadIdx.x == 0) s_turn = 0;
   __syncthreads();
   unsigned int overlaps = 0;
+  const Pol pol = make_policies(P.l2_hints);
 
   if (threadIdx.x >= DF_COMPUTE_THREADS) {
-    // ---------------- scheduler warp (lane 0 works) ----------------
-    if (threadIdx.x == DF_COMPUTE_THREADS) {
-      unsigned int c_src[2] = {0u, 0u}, c_dst[2] = {0u, 0u};   // counters to bump when the slot's op completes
-      unsigned int completed = 0;               // ops completed (in order)
-      auto try_complete = [&](unsigned int j) -> bool {   // op j (0-based) sits in slot j & 1
-        const unsigned int s = j & 1;
-        if (ld_acquire_cta_shared_u32(&s_done[s]) < NW * (j / 2 + 1)) return false;
-        __threadfence();
-        atomicAdd(P.counters + c_src[s], 1u);
-        atomicAdd(P.counters + c_dst[s], 1u);
-        return true;
-      };
-      unsigned int j = 0;
-      for (;; ++j) {
-        const unsigned int s = j & 1;
-        while (completed + 2 <= j) { if (try_complete(completed)) ++completed; }   // slot s must be free
-        const unsigned long long t = atomicAdd(&P.ctrl->ticket, 1ull);
-        if (t >= P.n_ops) break;
-        const unsigned long long opw = __ldg(reinterpret_cast<const unsigned long long*>(P.ops + t));
-        TileOp op;
-        op.flow = (unsigned int)opw;
-        op.tile = (unsigned int)(opw >> 32);
-        const uint4* fr = reinterpret_cast<const uint4*>(P.flows + op.flow);
-        const uint4 f0 = __ldg(fr), f1 = __ldg(fr + 1);
-        const uint4 dp = __ldg(reinterpret_cast<const uint4*>(P.deps + op.flow));
-        DfSlot& sl = s_slot[s];
-        memcpy(&sl.f, &f0, 16);
-        memcpy(reinterpret_cast<char*>(&sl.f) + 16, &f1, 16);
-        const unsigned long long A = P.unit_elems, nunits = (sl.f.len + A - 1) / A;
-        sl.ubeg = (unsigned long long)op.tile * P.tile_units;
-        sl.uend = sl.ubeg + P.tile_units < nunits ? sl.ubeg + P.tile_units : nunits;
-        sl.valid = 1;
-        c_src[s] = dp.x + op.tile;
-        c_dst[s] = dp.y + op.tile;
-        // wait for the accesses this op depends on; keep completing our own earlier op meanwhile
-        for (;;) {
-          const bool ok = ld_acquire_gpu_u32(P.counters + c_src[s]) >= dp.z && ld_acquire_gpu_u32(P.counters + c_dst[s]) >= dp.w;
-          if (ok) break;
-          if (completed < j && try_complete(completed)) ++completed;
-        }
-        st_release_cta_shared_u32(&s_full[s], j + 1);
+    // ---------------- scheduler agents: warp w (lane 0) owns slot w and the ops j = w, w + NS, ... ----------------
+    const unsigned int w = (threadIdx.x - DF_COMPUTE_THREADS) >> 5;
+    if ((threadIdx.x & 31) != 0 || w >= NS) return;
+    DfSlot& sl = s_slot[w];
+    for (unsigned int j = w;; j += NS) {
+      // tickets are claimed in local order, so that local order == table order inside the CTA
+      while (ld_acquire_cta_shared_u32(&s_turn) != j) { }
+      const unsigned long long t = atomicAdd(&P.ctrl->ticket, 1ull);
+      st_release_cta_shared_u32(&s_turn, j + 1);
+      if (t >= P.n_ops) {              // nothing left: stop marker (the streaming warps stop at the first one)
+        sl.valid = 0;
+        st_release_cta_shared_u32(&s_full[w], j + 1);
+        return;
       }
-      // drain: complete what is still streaming, then tell the streaming warps to stop
-      while (completed < j) { if (try_complete(completed)) ++completed; }
-      s_slot[j & 1].valid = 0;
-      st_release_cta_shared_u32(&s_full[j & 1], j + 1);
+      const unsigned long long opw = __ldg(reinterpret_cast<const unsigned long long*>(P.ops + t));
+      const unsigned int flow = (unsigned int)opw, tile = (unsigned int)(opw >> 32);
+      const uint4* fr = reinterpret_cast<const uint4*>(P.flows + flow);
+      const uint4 f0 = __ldg(fr), f1 = __ldg(fr + 1);
+      const uint4 dp = __ldg(reinterpret_cast<const uint4*>(P.deps + flow));
+      memcpy(&sl.f, &f0, 16);
+      memcpy(reinterpret_cast<char*>(&sl.f) + 16, &f1, 16);
+      const unsigned long long A = P.unit_elems, nunits = (sl.f.len + A - 1) / A;
+      sl.ubeg = (unsigned long long)tile * P.tile_units;
+      sl.uend = sl.ubeg + P.tile_units < nunits ? sl.ubeg + P.tile_units : nunits;
+      sl.valid = 1;
+      unsigned int* c_src = P.counters + dp.x + tile;
+      unsigned int* c_dst = P.counters + dp.y + tile;
+      // the accesses this op depends on (PAPER.md:138 data dependencies), per (rank, region, tile)
+      while (ld_acquire_gpu_u32(c_src) < dp.z) { }
+      while (ld_acquire_gpu_u32(c_dst) < dp.w) { }
+      st_release_cta_shared_u32(&s_full[w], j + 1);
+      // completion: every streaming warp is done with it -> make the writes visible, bump the range counters
+      const unsigned int target = NW * (j / NS + 1);
+      while (ld_acquire_cta_shared_u32(&s_done[w]) < target) { }
+      __threadfence();
+      atomicAdd(c_src, 1u);
+      atomicAdd(c_dst, 1u);
     }
   } else {
     // ---------------- streaming warps ----------------
     for (unsigned int j = 0;; ++j) {
-      const unsigned int s = j & 1;
+      const unsigned int s = j % NS;
       while (ld_acquire_cta_shared_u32(&s_full[s]) < j + 1) { }
       if (!s_slot[s].valid) break;
       const DFlow f = s_slot[s].f;
       const unsigned long long ubeg = s_slot[s].ubeg, uend = s_slot[s].uend;
-      process_piece<MODE, DF_COMPUTE_THREADS>(P, f, ubeg, uend, overlaps);
+      process_piece<MODE, DF_COMPUTE_THREADS>(P, f, ubeg, uend, overlaps, pol);
       __syncwarp();
       if ((threadIdx.x & 31) == 0) red_release_cta_shared_add(&s_done[s], 1u);
     }
@@ -580,6 +578,12 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   P.ops = reinterpret_cast<const TileOp*>(ws + L.ops);
   P.counters = reinterpret_cast<unsigned int*>(ws + L.counters);
   P.tile_units = pl->tile_units;
+  P.l2_hints = 1;
+  if (const char* e = std::getenv("OPTCC_L2_HINTS")) P.l2_hints = (unsigned int)std::atoi(e);
+  P.df_slots = pl->tile_units >= 2048 ? 2 : 4;   // big tiles: short look-ahead keeps the L2 reuse distance small
+  P.df_batch = 1;
+  if (const char* e = std::getenv("OPTCC_DF_SLOTS")) P.df_slots = std::max(1, std::min(DF_SLOTS, std::atoi(e)));
+  if (const char* e = std::getenv("OPTCC_DF_BATCH")) P.df_batch = std::max(1, std::min((int)P.df_slots, std::atoi(e)));
 }
 
 }  // namespace

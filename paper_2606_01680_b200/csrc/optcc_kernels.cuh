@@ -51,8 +51,9 @@ static_assert(sizeof(DDep) == 16, "DDep must be 16 bytes");
 
 struct TileOp { unsigned int flow, tile; };   // one unit of work of the dataflow executor
 
-constexpr int DF_COMPUTE_THREADS = 480;   // 15 streaming warps
-constexpr int DF_THREADS = DF_COMPUTE_THREADS + 32;   // + 1 scheduler warp
+constexpr int DF_COMPUTE_THREADS = 448;   // 14 streaming warps
+constexpr int DF_SLOTS = 4;               // scheduler agents = tile-ops a CTA can hold (claimed, waiting or streaming)
+constexpr int DF_THREADS = DF_COMPUTE_THREADS + 32 * DF_SLOTS;
 
 struct Ctrl {                     // control block at the start of the workspace
   unsigned long long barrier;     // monotone arrival counter of the grid barrier
@@ -79,11 +80,40 @@ struct ExecParams {
   unsigned int* counters;         // [p * tiles_per_rank] completed accesses per (rank, region, tile)
   unsigned long long n_ops;
   unsigned int tile_units;
+  unsigned int df_slots;          // ring depth: tile-ops a CTA holds (claimed, waiting or streaming), <= DF_SLOTS
+  unsigned int df_batch;          // tickets claimed per scheduler iteration
+  unsigned int l2_hints;          // 0 none, 1 loads evict_first, 2 + stores evict_last
 };
 
 // ---- memory access helpers: L2-only loads (data written by other SMs in the previous step), streaming stores ----
-__device__ __forceinline__ uint4 ld16(const void* p) { return __ldcg(reinterpret_cast<const uint4*>(p)); }
-__device__ __forceinline__ void st16(void* p, uint4 v) { __stcg(reinterpret_cast<uint4*>(p), v); }
+// L2 eviction policies (createpolicy): loads of the streams are evict_first -- a section is dead once the next hop has
+// read it, raw destination data is dead once summed -- so that what was just written (the next step's source) stays.
+struct Pol { unsigned long long lds, ldd, st; };   // source loads, destination loads, stores
+__device__ __forceinline__ unsigned long long make_policy(unsigned int kind) {   // 0 normal, 1 evict_first, 2 evict_last
+  unsigned long long p;
+  if (kind == 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  else if (kind == 2) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+// mode = kind(src loads) + 4 * kind(dst loads) + 16 * kind(stores)
+__device__ __forceinline__ Pol make_policies(unsigned int mode) {
+  Pol p;
+  p.lds = make_policy(mode & 3u);
+  p.ldd = make_policy((mode >> 2) & 3u);
+  p.st = make_policy((mode >> 4) & 3u);
+  return p;
+}
+__device__ __forceinline__ uint4 ld16(const void* p, unsigned long long policy) {
+  uint4 v;
+  asm volatile("ld.global.cg.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
+               : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p), "l"(policy) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st16(void* p, uint4 v, const Pol& pol) {
+  asm volatile("st.global.cg.L2::cache_hint.v4.u32 [%0], {%1,%2,%3,%4}, %5;"
+               ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(pol.st) : "memory");
+}
 
 __device__ __forceinline__ float bf16_to_f32(unsigned int h) { return __uint_as_float(h << 16); }
 // float -> bf16 bits, round to nearest even; NaN stays a quiet NaN
@@ -122,40 +152,40 @@ __device__ __forceinline__ void grid_barrier(unsigned long long* ctr, unsigned l
 
 template <int UNROLL, int NT>
 __device__ __forceinline__ void range_copy16(const char* __restrict__ s, char* __restrict__ d,
-                                             unsigned long long vbeg, unsigned long long vend) {
+                                             unsigned long long vbeg, unsigned long long vend, const Pol& pol) {
   unsigned long long v = vbeg + threadIdx.x;
   for (; v + (UNROLL - 1) * (unsigned long long)NT < vend; v += UNROLL * (unsigned long long)NT) {
     uint4 x[UNROLL];
 #pragma unroll
-    for (int j = 0; j < UNROLL; ++j) x[j] = ld16(s + (v + j * (unsigned long long)NT) * 16);
+    for (int j = 0; j < UNROLL; ++j) x[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds);
 #pragma unroll
-    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, x[j]);
+    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, x[j], pol);
   }
-  for (; v < vend; v += NT) st16(d + v * 16, ld16(s + v * 16));
+  for (; v < vend; v += NT) st16(d + v * 16, ld16(s + v * 16, pol.lds), pol);
 }
 
 template <int UNROLL, int NT>
 __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* __restrict__ d,
-                                              unsigned long long vbeg, unsigned long long vend) {
+                                              unsigned long long vbeg, unsigned long long vend, const Pol& pol) {
   unsigned long long v = vbeg + threadIdx.x;
   for (; v + (UNROLL - 1) * (unsigned long long)NT < vend; v += UNROLL * (unsigned long long)NT) {
     uint4 a[UNROLL], b[UNROLL];
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) {
-      a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16);
-      b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16);
+      a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds);
+      b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd);
     }
 #pragma unroll
-    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, add_f32x4(b[j], a[j]));
+    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, add_f32x4(b[j], a[j]), pol);
   }
-  for (; v < vend; v += NT) st16(d + v * 16, add_f32x4(ld16(d + v * 16), ld16(s + v * 16)));
+  for (; v < vend; v += NT) st16(d + v * 16, add_f32x4(ld16(d + v * 16, pol.ldd), ld16(s + v * 16, pol.lds)), pol);
 }
 
 // masks: OR with overlap detection.  WORDS = 64-bit words per element (1 or 2); a 16-byte vector holds 2/WORDS elements
 template <int UNROLL, int WORDS, int NT>
 __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* __restrict__ d,
                                               unsigned long long vbeg, unsigned long long vend,
-                                              unsigned int& overlaps) {
+                                              unsigned int& overlaps, const Pol& pol) {
   unsigned long long v = vbeg + threadIdx.x;
   auto join = [&](uint4 a, uint4 b) {
     unsigned int lo = ((a.x & b.x) | (a.y & b.y)) != 0u, hi = ((a.z & b.z) | (a.w & b.w)) != 0u;
@@ -166,72 +196,72 @@ __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* 
     uint4 a[UNROLL], b[UNROLL];
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) {
-      a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16);
-      b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16);
+      a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds);
+      b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd);
     }
 #pragma unroll
-    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, join(a[j], b[j]));
+    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, join(a[j], b[j]), pol);
   }
-  for (; v < vend; v += NT) st16(d + v * 16, join(ld16(s + v * 16), ld16(d + v * 16)));
+  for (; v < vend; v += NT) st16(d + v * 16, join(ld16(s + v * 16, pol.lds), ld16(d + v * 16, pol.ldd)), pol);
 }
 
 // bf16 plans: a unit is 8 elements = 16 bytes in a rank buffer or 32 bytes in the fp32 shadow.
 template <int KIND>
-__device__ __forceinline__ void load8(const char* base, unsigned long long unit, float (&x)[8]) {
+__device__ __forceinline__ void load8(const char* base, unsigned long long unit, float (&x)[8], unsigned long long pol) {
   if (KIND == 0) {
-    uint4 r = ld16(base + unit * 16);
+    uint4 r = ld16(base + unit * 16, pol);
     x[0] = bf16_to_f32(r.x & 0xFFFFu); x[1] = bf16_to_f32(r.x >> 16);
     x[2] = bf16_to_f32(r.y & 0xFFFFu); x[3] = bf16_to_f32(r.y >> 16);
     x[4] = bf16_to_f32(r.z & 0xFFFFu); x[5] = bf16_to_f32(r.z >> 16);
     x[6] = bf16_to_f32(r.w & 0xFFFFu); x[7] = bf16_to_f32(r.w >> 16);
   } else {
-    uint4 r0 = ld16(base + unit * 32), r1 = ld16(base + unit * 32 + 16);
+    uint4 r0 = ld16(base + unit * 32, pol), r1 = ld16(base + unit * 32 + 16, pol);
     x[0] = __uint_as_float(r0.x); x[1] = __uint_as_float(r0.y); x[2] = __uint_as_float(r0.z); x[3] = __uint_as_float(r0.w);
     x[4] = __uint_as_float(r1.x); x[5] = __uint_as_float(r1.y); x[6] = __uint_as_float(r1.z); x[7] = __uint_as_float(r1.w);
   }
 }
 template <int KIND>
-__device__ __forceinline__ void store8(char* base, unsigned long long unit, const float (&x)[8]) {
+__device__ __forceinline__ void store8(char* base, unsigned long long unit, const float (&x)[8], const Pol& pol) {
   if (KIND == 0) {
     uint4 r;
     r.x = f32_to_bf16_rne(x[0]) | (f32_to_bf16_rne(x[1]) << 16);
     r.y = f32_to_bf16_rne(x[2]) | (f32_to_bf16_rne(x[3]) << 16);
     r.z = f32_to_bf16_rne(x[4]) | (f32_to_bf16_rne(x[5]) << 16);
     r.w = f32_to_bf16_rne(x[6]) | (f32_to_bf16_rne(x[7]) << 16);
-    st16(base + unit * 16, r);
+    st16(base + unit * 16, r, pol);
   } else {
-    st16(base + unit * 32, make_uint4(__float_as_uint(x[0]), __float_as_uint(x[1]), __float_as_uint(x[2]), __float_as_uint(x[3])));
-    st16(base + unit * 32 + 16, make_uint4(__float_as_uint(x[4]), __float_as_uint(x[5]), __float_as_uint(x[6]), __float_as_uint(x[7])));
+    st16(base + unit * 32, make_uint4(__float_as_uint(x[0]), __float_as_uint(x[1]), __float_as_uint(x[2]), __float_as_uint(x[3])), pol);
+    st16(base + unit * 32 + 16, make_uint4(__float_as_uint(x[4]), __float_as_uint(x[5]), __float_as_uint(x[6]), __float_as_uint(x[7])), pol);
   }
 }
 
 template <int KS, int KD, int KO, int NT>
 __device__ __forceinline__ void range_add_bf16(const char* __restrict__ s, const char* __restrict__ din,
                                                char* __restrict__ dout, unsigned long long ubeg,
-                                               unsigned long long uend) {
+                                               unsigned long long uend, const Pol& pol) {
   constexpr int UNROLL = 2;
   unsigned long long u = ubeg + threadIdx.x;
   for (; u + (UNROLL - 1) * (unsigned long long)NT < uend; u += UNROLL * (unsigned long long)NT) {
     float a[UNROLL][8], b[UNROLL][8];
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) {
-      load8<KS>(s, u + j * (unsigned long long)NT, a[j]);
-      load8<KD>(din, u + j * (unsigned long long)NT, b[j]);
+      load8<KS>(s, u + j * (unsigned long long)NT, a[j], pol.lds);
+      load8<KD>(din, u + j * (unsigned long long)NT, b[j], pol.ldd);
     }
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) {
 #pragma unroll
       for (int e = 0; e < 8; ++e) b[j][e] = __fadd_rn(b[j][e], a[j][e]);
-      store8<KO>(dout, u + j * (unsigned long long)NT, b[j]);
+      store8<KO>(dout, u + j * (unsigned long long)NT, b[j], pol);
     }
   }
   for (; u < uend; u += NT) {
     float a[8], b[8];
-    load8<KS>(s, u, a);
-    load8<KD>(din, u, b);
+    load8<KS>(s, u, a, pol.lds);
+    load8<KD>(din, u, b, pol.ldd);
 #pragma unroll
     for (int e = 0; e < 8; ++e) b[e] = __fadd_rn(b[e], a[e]);
-    store8<KO>(dout, u, b);
+    store8<KO>(dout, u, b, pol);
   }
 }
 

@@ -129,6 +129,7 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
   std::memset(&pl->info, 0, sizeof pl->info);
   std::memset(&pl->opts, 0, sizeof pl->opts);
   if (opts) pl->opts = *opts;
+  else pl->opts.exec_mode = OPTCC_EXEC_DATAFLOW;   // the default executor
   pl->ell.assign(ell, ell + p);
   pl->stragglers = stragglers;
   pl->healthy = healthy;
@@ -288,7 +289,18 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
   }
   // dataflow tiling: regions (unique offsets; all flows over one offset share a length, PLAN_SPEC 5.4) and tile counts
   try {
-    pl->tile_units = pl->opts.tile_units ? pl->opts.tile_units : OPTCC_TILE_UNITS_DEFAULT;
+    if (pl->opts.tile_units) {
+      pl->tile_units = pl->opts.tile_units;
+    } else {
+      // auto: about two tile-ops per CTA and step (592 = 2 x 296 CTAs on a B200), as a power of two in [256, 4096]:
+      // big steps get 64 KB tiles (bandwidth-bound), small steps get short tiles (more parallel dependency chains)
+      uint64_t units = 0;
+      for (const auto& f : pl->flows) units += (f.len + B.A - 1) / B.A;
+      const uint64_t per = n_steps ? units / n_steps / 592 : 0;
+      uint32_t tu = 256;
+      while (tu < OPTCC_TILE_UNITS_DEFAULT && uint64_t(tu) * 3 / 2 < per) tu *= 2;
+      pl->tile_units = tu;
+    }
     std::vector<std::pair<uint64_t, uint64_t>> regs;
     regs.reserve(pl->flows.size());
     for (const auto& f : pl->flows) regs.push_back({f.off, f.len});
