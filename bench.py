@@ -40,14 +40,23 @@ def parse_args():
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1 = C2, the metric's config)")
     ap.add_argument("--ell", type=float, default=1.6, help="ell for config 4 (the C5 sweep)")
-    ap.add_argument("--k", type=int, default=0, help="segments; 0 = planner's auto rule")
-    ap.add_argument("--exec-mode", type=int, default=0, help="0 persistent cooperative kernel, 1 one launch per step")
+    ap.add_argument("--k", type=int, default=-1,
+                    help="segments (PAPER.md:124); -1 = bench default per config (16 for C2, see profiles/ k-sweep), 0 = planner's auto rule")
+    ap.add_argument("--exec-mode", type=int, default=2,
+                    help="2 dataflow kernel (default), 0 persistent kernel with grid barriers, 1 one launch per step")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-sample-log2", type=int, default=0,
                     help="log2 of n per rank for the CPU-oracle sample (0 = 24 for the cpu_baseline leg, 22 per --impl reference step)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
+
+
+BENCH_K = {0: 8, 1: 16, 2: 8, 3: 8, 4: 8}   # per config; k is free in BASELINE.json's configs
+
+
+def bench_k(args):
+    return BENCH_K[args.config] if args.k < 0 else args.k
 
 
 def workload_name(w, k):
@@ -96,7 +105,7 @@ def run_reference(args):
     lg = args.cpu_sample_log2 or 22
     w = w_full.scaled(min(w_full.n, 2 ** lg))
     from oracle import planner as OP
-    k = OP.build_plan(w_full.p, w_full.g, list(w_full.ell), w_full.n, w_full.dtype, k=args.k).k
+    k = OP.build_plan(w_full.p, w_full.g, list(w_full.ell), w_full.n, w_full.dtype, k=bench_k(args)).k
     for _ in range(min(args.warmup, 1)):
         oracle_step(w, k)
     ts = [oracle_step(w, k) for _ in range(args.steps)]
@@ -131,7 +140,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -219,7 +228,7 @@ def run_native(args):
     if world > 1:   # every rank draws its own slice of a world x n job: same shape, different seed stream
         w = W.Workload(w.name, w.p, w.g, w.ell, w.n, w.dtype, w.dist, w.sigma, w.seed + 1000 * rank, w.note)
     esize = w.elem_bytes
-    mk = lambda: B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=args.k, exec_mode=args.exec_mode)
+    mk = lambda: B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=bench_k(args), exec_mode=args.exec_mode)
     plan0 = mk()
     k = plan0.info["k"]
     cost0 = B.optcc_cost(plan0)
@@ -233,7 +242,7 @@ def run_native(args):
     restore = lambda: [b.copy_(s) for b, s in zip(sess.bufs, pristine)]
     stream = torch.cuda.current_stream(dev)
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    launches_per_step = (1 if args.exec_mode == 0 else plan0.info["n_steps"]) * 2 + 2   # execute + verify(init, exec, check)
+    launches_per_step = (plan0.info["n_steps"] if args.exec_mode == 1 else 1) * 2 + 2   # execute + verify(init, exec, check)
 
     def full_step(timed):
         """a1-a3 optcc_plan, a4 optcc_cost, a5-a7 optcc_execute, a8 optcc_verify; returns event pairs + host times."""
@@ -332,7 +341,8 @@ def run_native(args):
         return 0
 
     peak, peak_src = measured_peak()
-    kern = "optcc_exec_kernel<MODE_F32>" if w.dtype == W.F32 else "optcc_exec_kernel<MODE_BF16>"
+    kname = "optcc_dataflow_kernel" if args.exec_mode == 2 else "optcc_exec_kernel"
+    kern = kname + ("<MODE_F32>" if w.dtype == W.F32 else "<MODE_BF16>")
     achieved = sched_bytes / t_exec / 1e6
     mask_bytes = 5 * (w.p - 1) * w.n * 8 * plan0.info["mask_words"]
     line = {
@@ -341,7 +351,8 @@ def run_native(args):
         "scaling": "weak", "vs_baseline": None, "dtype": "f32" if w.dtype == W.F32 else "bf16(f32 accumulate)",
         "data": "synthetic",
         "config": {"workload": workload_name(w, k), "step": "optcc_plan + optcc_cost + optcc_execute + optcc_verify (SURVEY 8(a) a1-a8)",
-                   "exec_mode": "persistent cooperative kernel, grid barrier per step" if args.exec_mode == 0 else "one launch per step",
+                   "exec_mode": {0: "persistent cooperative kernel, grid barrier per step", 1: "one launch per step",
+                                 2: "dataflow cooperative kernel: tile-ops in table order, per-range completion counters, no grid barrier"}[args.exec_mode],
                    "plan_steps": plan0.info["n_steps"], "plan_flows": plan0.info["n_flows"], "parallelism": f"replicas x{world} (element-axis shards, no collective)",
                    "l2": "inputs larger than L2 (footprint %.2f GB) and restored from a pristine copy between steps, untimed" % (w.p * w.n * esize / 1e9)},
         "execute_only": {"algbw": world * w.n * esize / t_exec / 1e6, "unit": UNIT, "ms": t_exec,
@@ -357,7 +368,7 @@ def run_native(args):
         "roofline": {"bound": "hbm", "kernel": kern, "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": ncu_traffic(w.name.split("[")[0], kern),
                      "algorithmic_bytes_per_launch": sched_bytes, "share_of_step": t_exec / t_step},
-        "roofline_verify": {"bound": "hbm", "kernel": "optcc_exec_kernel<MODE_MASK%d> (+init, check)" % plan0.info["mask_words"],
+        "roofline_verify": {"bound": "hbm", "kernel": "%s<MODE_MASK%d> (+init, check)" % (kname, plan0.info["mask_words"]),
                             "achieved": mask_bytes / t_ver / 1e6, "peak": peak, "unit": "GB/s", "frac": mask_bytes / t_ver / 1e6 / peak,
                             "share_of_step": t_ver / t_step},
         "parity_spot_check": {"sampled_elements": int(len(idx)), "within_tolerance": parity_ok},

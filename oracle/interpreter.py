@@ -165,3 +165,50 @@ def run_bf16(plan, xb):
             val[d, a:b] = val[s, a:b]
             cnt[(d, a)] = cs
     return f32_to_bf16_bits(val)    # exact: every final value is already a bf16 number
+
+
+def run_f32_at(plan, x_cols, idx):
+    """run_f32 restricted to the sampled element indices `idx` (sorted, unique): x_cols[p, len(idx)] holds the
+    inputs at those elements.  Same walk, same one-IEEE-add-per-reduce-flow arithmetic, applied only to the
+    samples a flow's range covers -- lets full-size runs be checked element by element on a sample."""
+    idx = np.asarray(idx, dtype=np.int64)
+    assert (np.diff(idx) > 0).all()
+    y = np.array(x_cols, dtype=np.float32, copy=True)
+    assert y.shape == (plan.p, len(idx))
+    lo = np.searchsorted(idx, plan.flows["off"].astype(np.int64), side="left")
+    hi = np.searchsorted(idx, (plan.flows["off"] + plan.flows["len"]).astype(np.int64), side="left")
+    for f, a, b in zip(plan.flows, lo, hi):
+        if a == b:
+            continue
+        if f["op"] == P.REDUCE:
+            y[int(f["dst"]), a:b] = y[int(f["dst"]), a:b] + y[int(f["src"]), a:b]
+        else:
+            y[int(f["dst"]), a:b] = y[int(f["src"]), a:b]
+    return y
+
+
+def run_bf16_at(plan, xb_cols, idx):
+    """run_bf16 restricted to sampled element indices (see run_f32_at): fp32 partials, one RNE rounding when a
+    range's sum over all p ranks completes (R12).  xb_cols: uint16 bit patterns [p, len(idx)]."""
+    idx = np.asarray(idx, dtype=np.int64)
+    assert (np.diff(idx) > 0).all()
+    p = plan.p
+    val = bf16_bits_to_f32(xb_cols).copy()
+    cnt = {}
+    lo = np.searchsorted(idx, plan.flows["off"].astype(np.int64), side="left")
+    hi = np.searchsorted(idx, (plan.flows["off"] + plan.flows["len"]).astype(np.int64), side="left")
+    for f, a, b in zip(plan.flows, lo, hi):
+        s, d, off = int(f["src"]), int(f["dst"]), int(f["off"])
+        cs, cd = cnt.get((s, off), 1), cnt.get((d, off), 1)
+        if f["op"] == P.REDUCE:
+            if a != b:
+                r = val[d, a:b] + val[s, a:b]
+                if cs + cd == p:
+                    r = bf16_bits_to_f32(f32_to_bf16_bits(r))
+                val[d, a:b] = r
+            cnt[(d, off)] = cs + cd
+        else:
+            if a != b:
+                val[d, a:b] = val[s, a:b]
+            cnt[(d, off)] = cs
+    return f32_to_bf16_bits(val)

@@ -199,6 +199,97 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) optcc_exec_kernel(const 
 // order; an op only waits on ops with smaller tickets, each held by a resident CTA (cooperative launch), whose
 // streaming warps reach them in order -- progress is guaranteed.
 // ---------------------------------------------------------------------------------------------------------
+// ---- cp.async.bulk (TMA 1-D bulk copy) helpers for the all-gather (copy) tile-ops -----------------------------
+constexpr unsigned int BULK_CHUNK = 8192;     // bytes per bulk transfer
+constexpr unsigned int BULK_STAGES = 3;       // chunks in flight per scheduler agent
+constexpr unsigned int BULK_SMEM_PER_AGENT = BULK_CHUNK * BULK_STAGES;
+
+__device__ __forceinline__ unsigned int smem_u32(const void* p) { return (unsigned int)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned int bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned int parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_LOOP_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@!p bra WAIT_LOOP_%=;\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, unsigned int bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* gdst, const void* smem_src, unsigned int bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(smem_src)), "r"(bytes) : "memory");
+  asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
+// byte extent of units [ubeg, uend) of a copy flow in the current element mode
+template <int MODE>
+__device__ __forceinline__ void copy_extent(const ExecParams& P, const DFlow& f, unsigned long long ubeg,
+                                            unsigned long long uend, const char** src, char** dst,
+                                            unsigned long long* nbytes) {
+  const unsigned long long A = P.unit_elems, e0 = ubeg * A;
+  unsigned long long e1 = uend * A;
+  if (e1 > f.len) e1 = f.len;
+  unsigned long long esz;
+  const char* s;
+  char* d;
+  if (MODE == MODE_F32) {
+    esz = 4; s = rank_ptr(P, f.src); d = rank_ptr(P, f.dst);
+  } else if (MODE == MODE_MASK1 || MODE == MODE_MASK2) {
+    esz = MODE == MODE_MASK1 ? 8 : 16; s = rank_ptr(P, f.src); d = rank_ptr(P, f.dst);
+  } else if (f.ksrc == 0) {
+    esz = 2; s = rank_ptr(P, f.src); d = rank_ptr(P, f.dst);
+  } else {
+    esz = 4;
+    s = reinterpret_cast<const char*>(P.shadow + (unsigned long long)f.src * P.padded_n);
+    d = reinterpret_cast<char*>(P.shadow + (unsigned long long)f.dst * P.padded_n);
+  }
+  *src = s + (f.off + e0) * esz;
+  *dst = d + (f.off + e0) * esz;
+  *nbytes = e1 > e0 ? (e1 - e0) * esz : 0;
+}
+
+// One thread copies nbytes (src, dst 16-byte aligned) global -> shared -> global with bulk async copies:
+// rounds of up to BULK_STAGES chunks in flight; `parity` holds one phase bit per stage barrier.
+__device__ __forceinline__ void bulk_copy(char* stage, unsigned long long* bars, unsigned int& parity,
+                                          const char* src, char* dst, unsigned long long nbytes) {
+  const unsigned long long n16 = nbytes & ~15ull;
+  for (unsigned long long base = 0; base < n16; base += (unsigned long long)BULK_CHUNK * BULK_STAGES) {
+    unsigned int issued = 0;
+#pragma unroll
+    for (unsigned int c = 0; c < BULK_STAGES; ++c) {
+      const unsigned long long o = base + (unsigned long long)c * BULK_CHUNK;
+      if (o < n16) {
+        const unsigned int b = (unsigned int)(n16 - o < BULK_CHUNK ? n16 - o : BULK_CHUNK);
+        mbar_expect_tx(bars + c, b);
+        bulk_g2s(stage + c * BULK_CHUNK, src + o, b, bars + c);
+        issued = c + 1;
+      }
+    }
+#pragma unroll
+    for (unsigned int c = 0; c < BULK_STAGES; ++c) {
+      if (c < issued) {
+        const unsigned long long o = base + (unsigned long long)c * BULK_CHUNK;
+        const unsigned int b = (unsigned int)(n16 - o < BULK_CHUNK ? n16 - o : BULK_CHUNK);
+        mbar_wait(bars + c, (parity >> c) & 1u);
+        parity ^= 1u << c;
+        bulk_s2g(dst + o, stage + c * BULK_CHUNK, b);
+      }
+    }
+    bulk_wait_read_all();   // the stages may be overwritten by the next round
+  }
+  bulk_wait_all();          // every store has been performed
+  for (unsigned long long o = n16; o < nbytes; ++o) dst[o] = src[o];   // ragged end of a buffer (< 16 bytes)
+}
+
 struct DfSlot {
   DFlow f;
   unsigned long long ubeg, uend;
@@ -231,8 +322,15 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
   __shared__ unsigned int s_full[DF_SLOTS];   // sequence number of the op published in the slot (j + 1)
   __shared__ unsigned int s_done[DF_SLOTS];   // streaming warps that finished ops of the slot (monotone)
   __shared__ unsigned int s_turn;             // local sequence number whose ticket is claimed next
+  __shared__ __align__(8) unsigned long long s_bar[DF_SLOTS][BULK_STAGES];   // mbarriers of the bulk-copy stages
+  extern __shared__ __align__(128) char s_stage[];   // bulk-copy staging: BULK_SMEM_PER_AGENT per agent (copy_path 2)
   if (threadIdx.x < DF_SLOTS) { s_full[threadIdx.x] = 0; s_done[threadIdx.x] = 0; }
-  if (threadIdx.x == 0) s_turn = 0;
+  if (threadIdx.x == 0) {
+    s_turn = 0;
+    for (unsigned int a = 0; a < DF_SLOTS; ++a)
+      for (unsigned int c = 0; c < BULK_STAGES; ++c) mbar_init(&s_bar[a][c], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
   __syncthreads();
   unsigned int overlaps = 0;
   const Pol pol = make_policies(P.l2_hints);
@@ -242,6 +340,7 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
     const unsigned int w = (threadIdx.x - DF_COMPUTE_THREADS) >> 5;
     if ((threadIdx.x & 31) != 0 || w >= NS) return;
     DfSlot& sl = s_slot[w];
+    unsigned int bulk_parity = 0;
     for (unsigned int j = w;; j += NS) {
       // tickets are claimed in local order, so that local order == table order inside the CTA
       while (ld_acquire_cta_shared_u32(&s_turn) != j) { }
@@ -262,14 +361,24 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
       const unsigned long long A = P.unit_elems, nunits = (sl.f.len + A - 1) / A;
       sl.ubeg = (unsigned long long)tile * P.tile_units;
       sl.uend = sl.ubeg + P.tile_units < nunits ? sl.ubeg + P.tile_units : nunits;
-      sl.valid = 1;
+      const bool bulk = P.bulk_copy && sl.f.op == 1;   // all-gather tile-op: this agent moves it with cp.async.bulk
+      sl.valid = bulk ? 2 : 1;
       unsigned int* c_src = P.counters + dp.x + tile;
       unsigned int* c_dst = P.counters + dp.y + tile;
       // the accesses this op depends on (PAPER.md:138 data dependencies), per (rank, region, tile)
       while (ld_acquire_gpu_u32(c_src) < dp.z) { }
       while (ld_acquire_gpu_u32(c_dst) < dp.w) { }
       st_release_cta_shared_u32(&s_full[w], j + 1);
-      // completion: every streaming warp is done with it -> make the writes visible, bump the range counters
+      if (bulk) {
+        const char* src;
+        char* dst;
+        unsigned long long nbytes;
+        copy_extent<MODE>(P, sl.f, sl.ubeg, sl.uend, &src, &dst, &nbytes);
+        fence_proxy_async();   // the source was written through the generic proxy by other CTAs
+        bulk_copy(s_stage + w * BULK_SMEM_PER_AGENT, s_bar[w], bulk_parity, src, dst, nbytes);
+        fence_proxy_async();
+      }
+      // completion: every streaming warp is done with it (bulk ops: has passed it) -> make the writes visible, bump the range counters
       const unsigned int target = NW * (j / NS + 1);
       while (ld_acquire_cta_shared_u32(&s_done[w]) < target) { }
       __threadfence();
@@ -281,10 +390,13 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
     for (unsigned int j = 0;; ++j) {
       const unsigned int s = j % NS;
       while (ld_acquire_cta_shared_u32(&s_full[s]) < j + 1) { }
-      if (!s_slot[s].valid) break;
-      const DFlow f = s_slot[s].f;
-      const unsigned long long ubeg = s_slot[s].ubeg, uend = s_slot[s].uend;
-      process_piece<MODE, DF_COMPUTE_THREADS>(P, f, ubeg, uend, overlaps, pol);
+      const unsigned int kind = s_slot[s].valid;
+      if (!kind) break;
+      if (kind == 1) {   // kind 2: the agent copies it with cp.async.bulk; the streaming warps move on
+        const DFlow f = s_slot[s].f;
+        const unsigned long long ubeg = s_slot[s].ubeg, uend = s_slot[s].uend;
+        process_piece<MODE, DF_COMPUTE_THREADS>(P, f, ubeg, uend, overlaps, pol);
+      }
       __syncwarp();
       if ((threadIdx.x & 31) == 0) red_release_cta_shared_add(&s_done[s], 1u);
     }
@@ -296,40 +408,42 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
   }
 }
 
-// masks[r][e][w] = {r}
-__global__ void __launch_bounds__(256) optcc_mask_init_kernel(unsigned long long* masks, unsigned int p,
-                                                              unsigned long long n, unsigned long long padded_n,
+// masks[r][e][w] = {r}: blockIdx.y = rank, 16-byte stores over the rank's padded array
+__global__ void __launch_bounds__(256) optcc_mask_init_kernel(unsigned long long* masks, unsigned long long padded_n,
                                                               unsigned int W) {
-  const unsigned long long total = (unsigned long long)p * n;
-  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < total;
-       i += (unsigned long long)gridDim.x * blockDim.x) {
-    unsigned int r = (unsigned int)(i / n);
-    unsigned long long e = i - (unsigned long long)r * n;
-    unsigned long long* m = masks + ((unsigned long long)r * padded_n + e) * W;
-    if (W == 1) {
-      m[0] = 1ull << r;
-    } else {
-      m[0] = r < 64 ? 1ull << r : 0ull;
-      m[1] = r >= 64 ? 1ull << (r - 64) : 0ull;
-    }
-  }
+  const unsigned int r = blockIdx.y;
+  const unsigned long long w0 = r < 64 ? 1ull << r : 0ull, w1 = r >= 64 ? 1ull << (r - 64) : 0ull;
+  // a 16-byte vector is two one-word masks or one two-word mask
+  const ulonglong2 v = W == 1 ? make_ulonglong2(w0, w0) : make_ulonglong2(w0, w1);
+  ulonglong2* m = reinterpret_cast<ulonglong2*>(masks + (unsigned long long)r * padded_n * W);
+  const unsigned long long nvec = padded_n * W / 2;
+  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < nvec;
+       i += (unsigned long long)gridDim.x * blockDim.x)
+    __stcg(m + i, v);
 }
 
 // every (rank, element) must hold every rank exactly once: mask == all p bits (PAPER.md:68 (ii))
 __global__ void __launch_bounds__(256) optcc_mask_check_kernel(const unsigned long long* masks, unsigned int p,
                                                                unsigned long long n, unsigned long long padded_n,
                                                                unsigned int W, Ctrl* ctrl) {
-  const unsigned long long total = (unsigned long long)p * n;
+  const unsigned int r = blockIdx.y;
   const unsigned long long full0 = p >= 64 ? ~0ull : ((1ull << p) - 1ull);
   const unsigned long long full1 = p > 64 ? (p >= 128 ? ~0ull : ((1ull << (p - 64)) - 1ull)) : 0ull;
+  const ulonglong2* m = reinterpret_cast<const ulonglong2*>(masks + (unsigned long long)r * padded_n * W);
+  const unsigned long long nvec = (n * W + 1) / 2;
   unsigned long long bad = 0, first = ~0ull;
-  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < total;
+  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < nvec;
        i += (unsigned long long)gridDim.x * blockDim.x) {
-    unsigned int r = (unsigned int)(i / n);
-    unsigned long long e = i - (unsigned long long)r * n;
-    const unsigned long long* m = masks + ((unsigned long long)r * padded_n + e) * W;
-    bool ok = __ldcg(m) == full0 && (W == 1 || __ldcg(m + 1) == full1);
-    if (!ok) { ++bad; first = first < i ? first : i; }
+    const ulonglong2 v = __ldcg(m + i);
+    if (W == 1) {
+      const unsigned long long e = 2 * i;
+      if (v.x != full0) { ++bad; const unsigned long long g = (unsigned long long)r * n + e; first = first < g ? first : g; }
+      if (e + 1 < n && v.y != full0) { ++bad; const unsigned long long g = (unsigned long long)r * n + e + 1; first = first < g ? first : g; }
+    } else if (v.x != full0 || v.y != full1) {
+      ++bad;
+      const unsigned long long g = (unsigned long long)r * n + i;
+      first = first < g ? first : g;
+    }
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
@@ -371,7 +485,9 @@ namespace {
 
 template <int MODE>
 int df_kernel_occupancy(int* out) {
-  CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, optcc_dataflow_kernel<MODE>, DF_THREADS, 0));
+  const size_t dyn = size_t(BULK_SMEM_PER_AGENT) * DF_SLOTS;   // sized for the bulk-copy path
+  CU_TRY(cudaFuncSetAttribute(optcc_dataflow_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+  CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, optcc_dataflow_kernel<MODE>, DF_THREADS, dyn));
   return OPTCC_OK;
 }
 
@@ -543,7 +659,8 @@ int launch_plan(optcc_plan_t* pl, ExecParams& P, cudaStream_t stream) {
     CU_TRY(cudaMemsetAsync(P.counters, 0, size_t(in.p) * pl->tiles_per_rank * sizeof(unsigned int), stream));
     CU_TRY(cudaMemsetAsync(&P.ctrl->ticket, 0, sizeof(unsigned long long), stream));
     void* args[] = {&P};
-    CU_TRY(cudaLaunchCooperativeKernel((const void*)optcc_dataflow_kernel<MODE>, dim3(st->G_df), dim3(DF_THREADS), args, 0, stream));
+    const size_t dyn = P.bulk_copy ? size_t(BULK_SMEM_PER_AGENT) * DF_SLOTS : 0;
+    CU_TRY(cudaLaunchCooperativeKernel((const void*)optcc_dataflow_kernel<MODE>, dim3(st->G_df), dim3(DF_THREADS), args, dyn, stream));
   } else if (persistent) {
     CU_TRY(cudaMemsetAsync(&P.ctrl->barrier, 0, sizeof(unsigned long long), stream));
     P.step_lo = 0;
@@ -578,6 +695,8 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   P.ops = reinterpret_cast<const TileOp*>(ws + L.ops);
   P.counters = reinterpret_cast<unsigned int*>(ws + L.counters);
   P.tile_units = pl->tile_units;
+  P.bulk_copy = pl->opts.copy_path == 2 ? 1u : 0u;
+  if (const char* e = std::getenv("OPTCC_BULK_COPY")) P.bulk_copy = (unsigned int)std::atoi(e);
   P.l2_hints = 1;
   if (const char* e = std::getenv("OPTCC_L2_HINTS")) P.l2_hints = (unsigned int)std::atoi(e);
   P.df_slots = pl->tile_units >= 2048 ? 2 : 4;   // big tiles: short look-ahead keeps the L2 reuse distance small
@@ -651,8 +770,11 @@ extern "C" int optcc_verify(optcc_plan_t* plan, void* workspace, void* stream_, 
   std::memset(&init, 0, sizeof init);
   init.first_bad = ~0ull;
   CU_TRY(cudaMemcpyAsync(P.ctrl, &init, sizeof init, cudaMemcpyHostToDevice, stream));
-  const int blocks = plan->exec->sm_count * 8;
-  optcc_mask_init_kernel<<<blocks, 256, 0, stream>>>(masks, in.p, in.n, in.padded_n, in.mask_words);
+  const uint64_t vec_per_rank = in.padded_n * in.mask_words / 2;
+  const unsigned int bx = (unsigned int)std::max<uint64_t>(1, std::min<uint64_t>((vec_per_rank + 1023) / 1024,
+                                                          std::max<uint64_t>(1, uint64_t(plan->exec->sm_count) * 16 / in.p)));
+  const dim3 blocks(bx, in.p);
+  optcc_mask_init_kernel<<<blocks, 256, 0, stream>>>(masks, in.padded_n, in.mask_words);
   CU_TRY(cudaGetLastError());
   rc = in.mask_words == 1 ? launch_plan<MODE_MASK1>(plan, P, stream) : launch_plan<MODE_MASK2>(plan, P, stream);
   if (rc != OPTCC_OK) return rc;

@@ -82,6 +82,7 @@ struct ExecParams {
   unsigned int tile_units;
   unsigned int df_slots;          // ring depth: tile-ops a CTA holds (claimed, waiting or streaming), <= DF_SLOTS
   unsigned int df_batch;          // tickets claimed per scheduler iteration
+  unsigned int bulk_copy;         // 1: copy tile-ops are moved by the scheduler agents with cp.async.bulk
   unsigned int l2_hints;          // 0 none, 1 loads evict_first, 2 + stores evict_last
 };
 

@@ -98,6 +98,35 @@ def test_f32_parity_any_grid(grid_ctas, exec_mode):
     _run_and_check(_wl(16, 1, {3: 4.0 / 3.0}, 2 ** 16 + 13, W.F32, seed=7), 8, exec_mode, grid_ctas)
 
 
+BULK_CASES = [
+    (4, 1, {0: 2.0}, 100003, W.F32, 4),                 # ragged n % 4 = 3: < 16-byte tail after the bulk part
+    (16, 1, {0: 8.0 / 7.0}, 2 ** 18 + 2, W.F32, 8),     # bubble flows, tiles larger than one bulk round
+    (5, 1, {2: 1.5}, 50003, W.BF16, 4),                 # bf16, ragged n % 8 = 3
+    (64, 1, {5: 8.0 / 7.0, 17: 4.0 / 3.0, 40: 2.0}, 70001, W.BF16, 4),
+    (16, 4, {r: 2.0 for r in range(4)}, 40001, W.F32, 4),
+    (3, 1, {0: 2.0}, 1, W.F32, 4),
+]
+
+
+@pytest.mark.parametrize("p,g,st,n,dtype,k", BULK_CASES)
+def test_bulk_copy_path_parity(p, g, st, n, dtype, k):
+    """copy_path = 2: the all-gather (copy) tile-ops are moved by cp.async.bulk (TMA 1-D bulk copies) instead of
+    LDG/STG; outputs and masks must not change by a bit."""
+    w = _wl(p, g, st, n, dtype, seed=300 + p)
+    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=k, exec_mode=B.OPTCC_EXEC_DATAFLOW, copy_path=2)
+    oplan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=k)
+    x = W.all_inputs(w)
+    s = _session(plan, verify=True)
+    s.upload(x)
+    s.execute()
+    y = s.download()
+    y_or = OI.run_f32(oplan, x) if dtype == W.F32 else OI.run_bf16(oplan, x)
+    assert y.tobytes() == y_or.tobytes()
+    res = s.verify()
+    assert res["bad_elements"] == 0 and res["overlap_elements"] == 0
+    assert s.masks().tobytes() == OI.element_masks(oplan)[0].tobytes()
+
+
 @pytest.mark.parametrize("tile_units", [1, 64, 4096])
 def test_dataflow_parity_any_tile_size(tile_units):
     w = _wl(7, 1, {0: 2.0, 1: 4.0 / 3.0}, 20011, W.F32, seed=11)
