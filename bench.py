@@ -207,26 +207,20 @@ def run_native(args):
     from paper_2606_01680_b200 import build as optcc_build
     from paper_2606_01680_b200.device import Session
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2606_01680_b200.replicas import Replicas
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: liboptcc has no CPU fallback (use --impl reference for the oracle)")
+    local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
+    rep = Replicas(backend="nccl", device=dev)
+    rank, world = rep.rank, rep.world
     if rank == 0:
         optcc_build.build()
-    if dist:
-        dist.barrier()
+    rep.barrier()
     B.load()
 
-    w = W.config(args.config, args.ell) if args.config == 4 else W.config(args.config)
-    if world > 1:   # every rank draws its own slice of a world x n job: same shape, different seed stream
-        w = W.Workload(w.name, w.p, w.g, w.ell, w.n, w.dtype, w.dist, w.sigma, w.seed + 1000 * rank, w.note)
+    w = rep.shard(W.config(args.config, args.ell) if args.config == 4 else W.config(args.config))
     esize = w.elem_bytes
     mk = lambda: B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=bench_k(args), exec_mode=args.exec_mode)
     plan0 = mk()
@@ -271,8 +265,7 @@ def run_native(args):
         restore()
         full_step(False)
     sampler = ClockSampler(local)
-    if dist:
-        dist.barrier()
+    rep.barrier()
     torch.cuda.synchronize(dev)
     sampler.start()
     recs = []
@@ -284,14 +277,10 @@ def run_native(args):
     torch.cuda.synchronize(dev)
     wall = time.perf_counter() - wall0
     clocks = sampler.stop()
-    if dist:
-        dist.barrier()
+    rep.barrier()
     mean = lambda key: sum(r[key] for r in recs) / len(recs)
     t_step, t_exec, t_ver = mean("total"), mean("execute"), mean("verify")
-    if dist:
-        tt = torch.tensor([t_step, t_exec, t_ver], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_step, t_exec, t_ver = [float(v) for v in tt]
+    t_step, t_exec, t_ver = rep.max_over_ranks([t_step, t_exec, t_ver])
 
     # parity spot-check of the last timed step against the fp64 sum on sampled elements (cheap, outside timing)
     idx = W.sample_indices(w, 4096)
@@ -325,19 +314,16 @@ def run_native(args):
             if i:
                 ts.append(a.elapsed_time(b_))
         t_e2e = sum(ts) / len(ts)
-        if dist:
-            tt = torch.tensor([t_e2e], device=dev, dtype=torch.float64)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            t_e2e = float(tt[0])
+        t_e2e = rep.max_over_ranks([t_e2e])[0]
         ok = all(torch.equal(hout[0], h) for h in hout[1:])
         e2e = {"value": world * w.n * esize / t_e2e / 1e6, "unit": UNIT, "h2d_bytes_per_step": w.p * w.n * esize,
                "d2h_bytes_per_step": w.p * w.n * esize, "ms_per_step": t_e2e, "steps": len(ts),
                "all_ranks_identical": bool(ok)}
         del hin, hout
 
+    parity_ok = rep.all_true(parity_ok)
     if rank != 0:
-        if dist:
-            dist.destroy_process_group()
+        rep.close()
         return 0
 
     peak, peak_src = measured_peak()
@@ -385,8 +371,7 @@ def run_native(args):
     if not parity_ok:
         line["error"] = "parity spot check failed"
     print(json.dumps(line), flush=True)
-    if dist:
-        dist.destroy_process_group()
+    rep.close()
     return 0 if parity_ok else 1
 
 

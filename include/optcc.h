@@ -80,7 +80,7 @@ typedef struct optcc_opts {
   uint32_t copy_path; /* 0 = auto, 1 = LDG/STG vector copy, 2 = cp.async.bulk (TMA 1-D) copy */
   uint32_t step_limit;/* 0 = all steps; else execute / verify only the first step_limit steps (debugging and
                          profiling: a truncated schedule must FAIL verification) */
-  uint32_t tile_units;/* dataflow executor: 16-byte units per tile-op; 0 = auto (a power of two in [256, 4096]: about two tile-ops per CTA and step) */
+  uint32_t tile_units;/* dataflow executor: 16-byte units per tile-op; 0 = auto (224..3584: about two tile-ops per CTA and step, whole streaming rounds) */
 } optcc_opts_t;
 
 typedef struct optcc_plan_info {

@@ -52,7 +52,7 @@ struct optcc_ws_layout {
 
 static inline uint64_t optcc_align256(uint64_t x) { return (x + 255) & ~uint64_t(255); }
 
-constexpr uint32_t OPTCC_TILE_UNITS_DEFAULT = 4096;  // 64 KB of f32 / bf16 per tile-op
+constexpr uint32_t OPTCC_TILE_UNITS_DEFAULT = 3584;  // largest auto tile: 56 KB of f32 / bf16 = two streaming rounds
 constexpr uint64_t OPTCC_DEP_BYTES = 16;             // sizeof(DDep)
 constexpr uint64_t OPTCC_OP_BYTES = 8;               // sizeof(TileOp)
 

@@ -292,12 +292,13 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     if (pl->opts.tile_units) {
       pl->tile_units = pl->opts.tile_units;
     } else {
-      // auto: about two tile-ops per CTA and step (592 = 2 x 296 CTAs on a B200), as a power of two in [256, 4096]:
-      // big steps get 64 KB tiles (bandwidth-bound), small steps get short tiles (more parallel dependency chains)
+      // auto: about two tile-ops per CTA and step (592 = 2 x 296 CTAs on a B200), from {224, 448, 896, 1792, 3584}
+      // -- multiples / fractions of one streaming round of the dataflow kernel (448 threads x 4 vectors), so a tile is
+      // whole rounds; big steps get 56 KB tiles (bandwidth-bound), small steps short tiles (more parallel chains)
       uint64_t units = 0;
       for (const auto& f : pl->flows) units += (f.len + B.A - 1) / B.A;
       const uint64_t per = n_steps ? units / n_steps / 592 : 0;
-      uint32_t tu = 256;
+      uint32_t tu = 224;
       while (tu < OPTCC_TILE_UNITS_DEFAULT && uint64_t(tu) * 3 / 2 < per) tu *= 2;
       pl->tile_units = tu;
     }
