@@ -46,6 +46,12 @@ enum { OPTCC_LINK_NIC = 0, OPTCC_LINK_NVLINK = 1 };
 /* constructions (PLAN_SPEC 4): C0 plain ring, C1 one straggler (4.1-4.2, App. C),
  * C2 m>=2 stragglers (App. D), C3 g>1 with one straggler server (App. E) */
 enum { OPTCC_C0 = 0, OPTCC_C1 = 1, OPTCC_C2 = 2, OPTCC_C3 = 3 };
+/* schedules (PLAN_SPEC 1 option `schedule`): the baseline runs in the same executor and cost model */
+enum {
+  OPTCC_SCHED_OPTCC = 0,
+  OPTCC_SCHED_RING_DEGRADED = 1 /* NCCL-style ring over all p ranks whatever ell is: the paper's ICCL comparison
+                                   point under the bandwidth model; g must be 1 */
+};
 /* executor modes */
 enum {
   OPTCC_EXEC_PERSISTENT = 0, /* one cooperative kernel for the whole schedule, grid barrier between steps */
@@ -81,6 +87,8 @@ typedef struct optcc_opts {
   uint32_t step_limit;/* 0 = all steps; else execute / verify only the first step_limit steps (debugging and
                          profiling: a truncated schedule must FAIL verification) */
   uint32_t tile_units;/* dataflow executor: 16-byte units per tile-op; 0 = auto (224..3584: about two tile-ops per CTA and step, whole streaming rounds) */
+  uint32_t schedule;  /* OPTCC_SCHED_*: 0 = OPTCC (default), 1 = plain ring on the degraded topology (baseline) */
+  uint32_t reserved;  /* 0 */
 } optcc_opts_t;
 
 typedef struct optcc_plan_info {
@@ -125,6 +133,9 @@ typedef struct optcc_cost {
   double bodies;        /* T / (body duration): the "(k+c)" of the finite-k factor */
   double straggler_sent;/* NIC elements sent by the slowest straggler's first GPU (z* n at the optimum, :455) */
   double straggler_recv;
+  double T_ring_degraded; /* context: max(ell) * T0, the plain ring on the degraded topology (ICCL model, :199, :217) */
+  double T_r2ccl;       /* context: T0 (1 + p(ell-1)/(2(p-1))), the closed form the paper plots for R2CCL (:963);
+                           NaN unless g = 1 and m = 1 */
   int32_t lb_table1_thm;/* 1, 2 or 3; 0 for no straggler */
   int32_t lb_tight_thm; /* 6 or 13; 0 if none */
   int32_t regime;       /* 0 no straggler, 1 ring-bound (ell<2 resp. first max-term), 2 straggler-bound */

@@ -188,3 +188,9 @@ def T_r2ccl(p, ell, n=1):
     """R2CCL closed form used by the paper for plotting (:963): T_NCCL (1 + p(l-1)/(2(p-1)))."""
     l = _fr(ell)
     return T0(p, n) * (1 + p * (l - 1) / (2 * (p - 1)))
+
+
+def T_ring_degraded(p, ells, n=1):
+    """Plain ring on the degraded topology (the ICCL comparison point, :199, :217) under the bandwidth model: every
+    one of the 2(p-1) ring steps moves n/p elements over every link and waits for the slowest one: max(l) T0."""
+    return max([_fr(l) for l in ells] + [Fr(1)]) * T0(p, n)

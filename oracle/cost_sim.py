@@ -70,6 +70,8 @@ def paper_closed_form(plan):
     (k+4) T_body (:809) and Eq.(21)/(22) (:920-926) as upper bounds."""
     p, g, n, k = plan.p, plan.g, plan.n, plan.k
     ells = [plan.ell[v * g] for v in plan.stragglers]
+    if getattr(plan, "schedule", 0) == P.RING_DEGRADED:
+        return cf.T_ring_degraded(p, ells, n)
     if plan.m == 0:
         return cf.T0(p, n, g)
     if g > 1:

@@ -14,6 +14,7 @@ S1, S2, S3, S4, BUB_UP, BUB_DOWN, N_COLLECT, N_DISTRIBUTE = range(8)
 NIC, NVLINK = 0, 1
 F32, BF16 = 0, 1
 C0, C1, C2, C3 = 0, 1, 2, 3
+OPTCC, RING_DEGRADED = 0, 1   # PLAN_SPEC §1 option `schedule`
 
 FLOW_DTYPE = np.dtype([
     ("off", "<u8"), ("len", "<u8"), ("step", "<u4"), ("seg", "<u4"), ("sec", "<u4"),
@@ -54,6 +55,7 @@ class Plan:
     step_begin: np.ndarray = field(repr=False, default=None)  # u32 [n_steps+1]
     sec_bounds: np.ndarray = field(repr=False, default=None)  # u64, elements
     p2p_bounds: np.ndarray = field(repr=False, default=None)  # u64, elements
+    schedule: int = 0
 
 
 def _split(lo, hi, parts, i):
@@ -109,9 +111,14 @@ def auto_k(construction, ell1, H, ring_units):
     return max(4, min(k_t, k_c))
 
 
-def build_plan(p, g, ell, n, dtype, k=0, _u_p2p_override=None):
+def build_plan(p, g, ell, n, dtype, k=0, _u_p2p_override=None, schedule=OPTCC):
     """optcc_plan of the oracle.  `_u_p2p_override` (brute-force search only) replaces U_p2p."""
     ell = [float(x) for x in ell]
+    if schedule not in (OPTCC, RING_DEGRADED):
+        raise PlanError("EINVAL", "schedule")
+    if schedule == RING_DEGRADED and g != 1:
+        if p >= 3 and g >= 1 and p % g == 0:
+            raise PlanError("EUNSUPPORTED", "the ring baseline is defined for g = 1")
     q, stragglers, healthy = classify(p, g, ell)
     if n <= 0 or n > 2 ** 40:
         raise PlanError("EINVAL", "0 < n <= 2^40 required")
@@ -120,7 +127,7 @@ def build_plan(p, g, ell, n, dtype, k=0, _u_p2p_override=None):
     if k != 0 and (k % 4 != 0 or k < 0 or k > 65536):
         raise PlanError("EINVAL", "k must be a multiple of 4 (:155), <= 65536")
     m, H = len(stragglers), len(healthy)
-    construction = C0 if m == 0 else (C3 if g > 1 else (C1 if m == 1 else C2))
+    construction = C0 if (m == 0 or schedule == RING_DEGRADED) else (C3 if g > 1 else (C1 if m == 1 else C2))
     A = 4 if dtype == F32 else 8
     U = -(-n // A)
     E = lambda u: min(u * A, n)
@@ -232,4 +239,4 @@ def build_plan(p, g, ell, n, dtype, k=0, _u_p2p_override=None):
     return Plan(p=p, g=g, q=q, m=m, H=H, k=k, n=n, dtype=dtype, construction=construction, A=A, U=U,
                 U_ring=U_ring, U_p2p=U_p2p, n_ring=E(U_ring), n_p2p=n - E(U_ring), n_steps=n_steps,
                 ell=ell, stragglers=stragglers, healthy=healthy, flows=arr, step_begin=step_begin,
-                sec_bounds=np.array(sb, dtype=np.uint64), p2p_bounds=np.array(pb, dtype=np.uint64))
+                sec_bounds=np.array(sb, dtype=np.uint64), p2p_bounds=np.array(pb, dtype=np.uint64), schedule=schedule)

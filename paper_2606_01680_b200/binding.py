@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(HERE, "liboptcc.so")
 OPTCC_F32, OPTCC_BF16 = 0, 1
 OPTCC_OK, OPTCC_EINVAL, OPTCC_EUNSUPPORTED, OPTCC_ENOMEM, OPTCC_ECUDA, OPTCC_EVERIFY = range(6)
 OPTCC_EXEC_PERSISTENT, OPTCC_EXEC_PER_STEP, OPTCC_EXEC_DATAFLOW = 0, 1, 2
+OPTCC_SCHED_OPTCC, OPTCC_SCHED_RING_DEGRADED = 0, 1
 ERROR_NAMES = {1: "EINVAL", 2: "EUNSUPPORTED", 3: "ENOMEM", 4: "ECUDA", 5: "EVERIFY"}
 
 # optcc_flow_t (PLAN_SPEC 3): 40 bytes
@@ -29,7 +30,7 @@ FLOW_DTYPE = np.dtype([
 
 class optcc_opts_t(C.Structure):
     _fields_ = [("k", C.c_uint32), ("exec_mode", C.c_uint32), ("grid_ctas", C.c_uint32), ("copy_path", C.c_uint32),
-                ("step_limit", C.c_uint32), ("tile_units", C.c_uint32)]
+                ("step_limit", C.c_uint32), ("tile_units", C.c_uint32), ("schedule", C.c_uint32), ("reserved", C.c_uint32)]
 
 
 class optcc_plan_info_t(C.Structure):
@@ -47,7 +48,7 @@ class optcc_cost_params_t(C.Structure):
 
 class optcc_cost_t(C.Structure):
     _fields_ = [(n, C.c_double) for n in ("T", "T0", "T_over_T0", "T_closed_form", "T_limit", "lb_table1", "lb_tight",
-                                          "T0_server", "bodies", "straggler_sent", "straggler_recv")] + \
+                                          "T0_server", "bodies", "straggler_sent", "straggler_recv", "T_ring_degraded", "T_r2ccl")] + \
                [(n, C.c_int32) for n in ("lb_table1_thm", "lb_tight_thm", "regime", "reserved")]
 
 
@@ -147,11 +148,11 @@ class Plan:
             pass
 
 
-def optcc_plan(p, g, ell, n, dtype, k=0, exec_mode=OPTCC_EXEC_DATAFLOW, grid_ctas=0, copy_path=0, step_limit=0, tile_units=0):
+def optcc_plan(p, g, ell, n, dtype, k=0, exec_mode=OPTCC_EXEC_DATAFLOW, grid_ctas=0, copy_path=0, step_limit=0, tile_units=0, schedule=0):
     """optcc_plan_ex: returns a Plan.  ell: sequence of p floats."""
     lib = load()
     ell_arr = (C.c_double * len(ell))(*[float(x) for x in ell])
-    opts = optcc_opts_t(k, exec_mode, grid_ctas, copy_path, step_limit, tile_units)
+    opts = optcc_opts_t(k, exec_mode, grid_ctas, copy_path, step_limit, tile_units, schedule, 0)
     h = C.c_void_p()
     rc = lib.optcc_plan_ex(int(p), int(g), ell_arr, int(n), int(dtype), C.byref(opts), C.byref(h))
     if rc:

@@ -76,6 +76,10 @@ extern "C" int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* p
   c.straggler_recv = recvd;
   c.reserved = 0;
   const double nan = std::numeric_limits<double>::quiet_NaN();
+  double lmax = 1.0;
+  for (double l : plan->ell) lmax = std::max(lmax, l);
+  c.T_ring_degraded = lmax * c.T0;   // every ring step waits for the slowest link (ICCL model, :199, :217)
+  c.T_r2ccl = (g == 1 && m == 1) ? c.T0 * (1.0 + double(p) * (lmax - 1.0) / (2.0 * double(p - 1))) : nan;   // :963
   if (m == 0) {
     c.lb_table1 = c.lb_tight = c.T_closed_form = c.T_limit = c.T0;
     c.lb_table1_thm = 0; c.lb_tight_thm = 0; c.regime = 0;
@@ -115,6 +119,9 @@ extern "C" int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* p
       c.T_closed_form = c.T_limit * (double(k) + 4.0) / double(k);                                    // (k+4) T_body (:809)
       c.regime = str_body > ring_body ? 2 : 1;
     }
+  }
+  if (plan->opts.schedule == OPTCC_SCHED_RING_DEGRADED) {   // the baseline's own closed form; bounds stay those of the failure
+    c.T_closed_form = c.T_limit = c.T_ring_degraded;
   }
   c.bodies = T * double(k) / c.T_limit;
   *out = c;

@@ -432,9 +432,16 @@ __global__ void __launch_bounds__(256) optcc_mask_check_kernel(const unsigned lo
   const ulonglong2* m = reinterpret_cast<const ulonglong2*>(masks + (unsigned long long)r * padded_n * W);
   const unsigned long long nvec = (n * W + 1) / 2;
   unsigned long long bad = 0, first = ~0ull;
-  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < nvec;
-       i += (unsigned long long)gridDim.x * blockDim.x) {
-    const ulonglong2 v = __ldcg(m + i);
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long i0 = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i0 < nvec; i0 += 4 * stride) {
+    ulonglong2 vv[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) vv[q] = i0 + q * stride < nvec ? __ldcg(m + i0 + q * stride) : make_ulonglong2(full0, W == 1 ? full0 : full1);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+    const unsigned long long i = i0 + q * stride;
+    if (i >= nvec) break;
+    const ulonglong2 v = vv[q];
     if (W == 1) {
       const unsigned long long e = 2 * i;
       if (v.x != full0) { ++bad; const unsigned long long g = (unsigned long long)r * n + e; first = first < g ? first : g; }
@@ -443,6 +450,7 @@ __global__ void __launch_bounds__(256) optcc_mask_check_kernel(const unsigned lo
       ++bad;
       const unsigned long long g = (unsigned long long)r * n + i;
       first = first < g ? first : g;
+    }
     }
   }
 #pragma unroll
@@ -593,9 +601,13 @@ int build_state(optcc_plan_t* pl) {
       d.ksrc = pl->kind_src[i]; d.kdin = pl->kind_dst_in[i]; d.kdout = pl->kind_dst_out[i];
       st->dflows[i] = d;
     }
+    // dataflow tables when that executor will run; otherwise the slice table of the barrier executors
+    st->df_ok = false;
+    if (pl->opts.exec_mode == OPTCC_EXEC_DATAFLOW && st->coop && st->G_df > 0) build_dataflow_tables(pl, st);
     // slice table: cut every step into G slices of equal HBM bytes
-    st->slices.assign(size_t(in.n_steps) * (G + 1), Slice{0, 0, 0});
-    for (uint32_t t = 0; t < in.n_steps; ++t) {
+    st->slices.clear();
+    if (!st->df_ok) st->slices.assign(size_t(in.n_steps) * (G + 1), Slice{0, 0, 0});
+    for (uint32_t t = 0; t < in.n_steps && !st->df_ok; ++t) {
       const uint32_t lo = pl->step_begin[t], hi = pl->step_begin[t + 1];
       uint64_t Wtot = 0;
       for (uint32_t i = lo; i < hi; ++i) Wtot += ((pl->flows[i].len + A - 1) / A) * unit_cost(pl, i);
@@ -615,7 +627,6 @@ int build_state(optcc_plan_t* pl) {
         row[c].unit = i < hi ? (Bc - prefix) / unit_cost(pl, i) : 0;
       }
     }
-    build_dataflow_tables(pl, st);
   } catch (const std::bad_alloc&) {
     return OPTCC_ENOMEM;
   }

@@ -105,6 +105,9 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
   if (!out || !ell) return OPTCC_EINVAL;
   // ---- PLAN_SPEC 1: validation and classification (PAPER.md:68 "p >= 3", :78, :274, :850) ----
   if (p < 3 || p > 65535 || g < 1 || p % g != 0) return OPTCC_EINVAL;
+  const uint32_t schedule = opts ? opts->schedule : OPTCC_SCHED_OPTCC;
+  if (schedule != OPTCC_SCHED_OPTCC && schedule != OPTCC_SCHED_RING_DEGRADED) return OPTCC_EINVAL;
+  if (schedule == OPTCC_SCHED_RING_DEGRADED && g != 1) return OPTCC_EUNSUPPORTED;   // PLAN_SPEC 1: ring baseline, g = 1
   for (int i = 0; i < p; ++i)
     if (!std::isfinite(ell[i]) || ell[i] < 1.0) return OPTCC_EINVAL;
   const uint32_t q = uint32_t(p / g);
@@ -134,7 +137,8 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
   pl->stragglers = stragglers;
   pl->healthy = healthy;
   const uint32_t m = (uint32_t)stragglers.size(), H = (uint32_t)healthy.size();
-  const uint32_t construction = m == 0 ? OPTCC_C0 : (g > 1 ? OPTCC_C3 : (m == 1 ? OPTCC_C1 : OPTCC_C2));
+  const uint32_t construction = (m == 0 || schedule == OPTCC_SCHED_RING_DEGRADED)
+                                    ? OPTCC_C0 : (g > 1 ? OPTCC_C3 : (m == 1 ? OPTCC_C1 : OPTCC_C2));
   const double ell1 = m ? ell[stragglers[0] * g] : 1.0;
 
   Builder B;
