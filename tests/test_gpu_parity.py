@@ -231,3 +231,40 @@ def test_repeated_execute_on_same_session_is_deterministic():
         s.execute()
         outs.append(s.download([0, w.p - 1]).tobytes())
     assert outs[0] == outs[1] == outs[2]
+
+
+@pytest.mark.parametrize("exec_mode", MODES)
+@pytest.mark.parametrize("dtype,n", [(W.F32, 100003), (W.BF16, 50003)])
+def test_no_write_outside_the_rank_buffers(dtype, n, exec_mode):
+    """compute-sanitizer is closed on this pool, so out-of-bounds writes are caught with guard bands: every rank
+    buffer sits between two 4 KB canaries inside one allocation; after execute (ragged n, every executor) the
+    canaries and the slack after element n-1 must be untouched and the result still bit-equal to the oracle."""
+    import torch
+    p, k = 6, 4
+    w = _wl(p, 1, {2: 1.5}, n, dtype, seed=41)
+    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=k, exec_mode=exec_mode)
+    oplan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=k)
+    esz = 4 if dtype == W.F32 else 2
+    guard = 4096
+    stride = ((n * esz + 255) // 256) * 256 + 2 * guard
+    from paper_2606_01680_b200.device import Session
+    s = Session(plan, alloc_bufs=False)
+    arena = torch.full((p * stride,), 0xA5, dtype=torch.uint8, device=s.device)
+    base = arena.data_ptr()
+    assert base % 256 == 0
+    x = W.all_inputs(w)
+    ptrs = []
+    for r in range(p):
+        off = r * stride + guard
+        arena[off:off + n * esz] = torch.from_numpy(x[r].view(np.uint8).copy()).to(s.device)
+        ptrs.append(base + off)
+    B.optcc_execute(plan, ptrs, s.ws_ptr, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    host = arena.cpu().numpy()
+    y = np.stack([host[r * stride + guard: r * stride + guard + n * esz].view(x.dtype) for r in range(p)])
+    y_or = OI.run_f32(oplan, x) if dtype == W.F32 else OI.run_bf16(oplan, x)
+    assert y.tobytes() == y_or.tobytes()
+    for r in range(p):
+        lo, hi = r * stride, r * stride + guard + n * esz
+        assert (host[lo:lo + guard] == 0xA5).all(), f"rank {r}: write before the buffer"
+        assert (host[hi:(r + 1) * stride] == 0xA5).all(), f"rank {r}: write past element n-1"
