@@ -707,13 +707,8 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   P.counters = reinterpret_cast<unsigned int*>(ws + L.counters);
   P.tile_units = pl->tile_units;
   P.bulk_copy = pl->opts.copy_path == 2 ? 1u : 0u;
-  if (const char* e = std::getenv("OPTCC_BULK_COPY")) P.bulk_copy = (unsigned int)std::atoi(e);
-  P.l2_hints = 1;
-  if (const char* e = std::getenv("OPTCC_L2_HINTS")) P.l2_hints = (unsigned int)std::atoi(e);
+  P.l2_hints = 1;   // source loads evict_first, destination loads and stores evict_normal (measured best)
   P.df_slots = pl->tile_units >= 1792 ? 2 : 4;   // big tiles: short look-ahead keeps the L2 reuse distance small
-  P.df_batch = 1;
-  if (const char* e = std::getenv("OPTCC_DF_SLOTS")) P.df_slots = std::max(1, std::min(DF_SLOTS, std::atoi(e)));
-  if (const char* e = std::getenv("OPTCC_DF_BATCH")) P.df_batch = std::max(1, std::min((int)P.df_slots, std::atoi(e)));
 }
 
 }  // namespace

@@ -81,9 +81,8 @@ struct ExecParams {
   unsigned long long n_ops;
   unsigned int tile_units;
   unsigned int df_slots;          // ring depth: tile-ops a CTA holds (claimed, waiting or streaming), <= DF_SLOTS
-  unsigned int df_batch;          // tickets claimed per scheduler iteration
   unsigned int bulk_copy;         // 1: copy tile-ops are moved by the scheduler agents with cp.async.bulk
-  unsigned int l2_hints;          // 0 none, 1 loads evict_first, 2 + stores evict_last
+  unsigned int l2_hints;          // kind(src loads) + 4 kind(dst loads) + 16 kind(stores); kind: 0 normal, 1 evict_first, 2 evict_last
 };
 
 // ---- memory access helpers: L2-only loads (data written by other SMs in the previous step), streaming stores ----
