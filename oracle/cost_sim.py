@@ -76,6 +76,8 @@ def paper_closed_form(plan):
         return cf.T0(p, n, g)
     if g > 1:
         return cf.T_multigpu_bound(p, g, ells[0], k, n)
+    if plan.m == 1 and getattr(plan, "ordering", 2) == 1:
+        return cf.T_single_limit(p, ells[0], n) * cf.Fr(k + 3, k)    # one stage per body: k + 3 bodies (PLAN_SPEC C1')
     if plan.m == 1:
         return cf.T_single(p, ells[0], k, n)
     return cf.T_multi_paper(p, ells, k, n)

@@ -56,6 +56,7 @@ class Plan:
     sec_bounds: np.ndarray = field(repr=False, default=None)  # u64, elements
     p2p_bounds: np.ndarray = field(repr=False, default=None)  # u64, elements
     schedule: int = 0
+    ordering: int = 2
 
 
 def _split(lo, hi, parts, i):
@@ -111,7 +112,7 @@ def auto_k(construction, ell1, H, ring_units):
     return max(4, min(k_t, k_c))
 
 
-def build_plan(p, g, ell, n, dtype, k=0, _u_p2p_override=None, schedule=OPTCC):
+def build_plan(p, g, ell, n, dtype, k=0, _u_p2p_override=None, schedule=OPTCC, ordering=2):
     """optcc_plan of the oracle.  `_u_p2p_override` (brute-force search only) replaces U_p2p."""
     ell = [float(x) for x in ell]
     if schedule not in (OPTCC, RING_DEGRADED):
@@ -120,6 +121,10 @@ def build_plan(p, g, ell, n, dtype, k=0, _u_p2p_override=None, schedule=OPTCC):
         if p >= 3 and g >= 1 and p % g == 0:
             raise PlanError("EUNSUPPORTED", "the ring baseline is defined for g = 1")
     q, stragglers, healthy = classify(p, g, ell)
+    if ordering not in (1, 2):
+        raise PlanError("EINVAL", "ordering is 1 or 2 (:138)")
+    if ordering == 1 and not (g == 1 and len(stragglers) == 1 and schedule == OPTCC):
+        raise PlanError("EUNSUPPORTED", "ordering (1) is constructed for one straggler, g = 1 (PLAN_SPEC C1')")
     if n <= 0 or n > 2 ** 40:
         raise PlanError("EINVAL", "0 < n <= 2^40 required")
     if dtype not in (F32, BF16):
@@ -161,7 +166,38 @@ def build_plan(p, g, ell, n, dtype, k=0, _u_p2p_override=None, schedule=OPTCC):
         if ln > 0:
             flows.append((off, ln, step, seg, sec, src, dst, op, stage, link, part, 0))
 
-    if construction == C0:
+    if construction == C1 and ordering == 1:
+        # C1': ordering (1) of :138, S1 -> S2 -> S3 -> S4, one stage per body (PLAN_SPEC §4 C1')
+        n_steps = (k + 3) * H
+        sg = stragglers[0]
+        hr = list(healthy)
+        bubbles = ell1 < 2.0
+        W = lambda j, t: t if t < j else t + 1          # ring link j idle in window j
+        for B in range(k + 3):
+            base = B * H
+            for j in range(H):
+                src, dst = hr[j], hr[(j + 1) % H]
+                for t in range(H - 1):
+                    step = base + W(j, t)
+                    if B < k:            # Stage 1 hop t of segment B: healthy-only partial sums (:126)
+                        c = (j - t) % H
+                        emit(step, REDUCE, S1, NIC, 0, src, dst, B, c, sec_units(0, B, c))
+                    if 3 <= B:           # Stage 4 hop t of segment B-3: global sum of section j starts at healthy j (:136)
+                        c = (j - t) % H
+                        emit(step, COPY, S4, NIC, 0, src, dst, B - 3, c, sec_units(0, B - 3, c))
+            for a in range(H):
+                d = (a + 1) % H
+                step = base + a
+                if 1 <= B <= k:          # Stage 2: owner a uploads its partial sum, the straggler adds its own (:130-132)
+                    c = (a + 1) % H
+                    emit(step, REDUCE, S2, NIC, 0, hr[a], sg, B - 1, c, sec_units(0, B - 1, c))
+                if 2 <= B <= k + 1:      # Stage 3: the straggler returns the global sum to the uploader's successor (:132, R11)
+                    emit(step, COPY, S3, NIC, 0, sg, hr[d], B - 2, d, sec_units(0, B - 2, d))
+                if bubbles and B < k:    # bubble-up / bubble-down as in C1 (:165)
+                    emit(step, REDUCE, BUB_UP, NIC, 0, hr[a], sg, B, 0, p2p_piece(B))
+                if bubbles and 1 <= B <= k:
+                    emit(step, COPY, BUB_DOWN, NIC, 0, sg, hr[d], B - 1, 0, p2p_piece(B - 1))
+    elif construction == C0:
         # plain ring reduce-scatter + allgather over all p ranks (:52, :72)
         n_steps = 2 * (p - 1)
         for t in range(p - 1):
@@ -239,4 +275,4 @@ def build_plan(p, g, ell, n, dtype, k=0, _u_p2p_override=None, schedule=OPTCC):
     return Plan(p=p, g=g, q=q, m=m, H=H, k=k, n=n, dtype=dtype, construction=construction, A=A, U=U,
                 U_ring=U_ring, U_p2p=U_p2p, n_ring=E(U_ring), n_p2p=n - E(U_ring), n_steps=n_steps,
                 ell=ell, stragglers=stragglers, healthy=healthy, flows=arr, step_begin=step_begin,
-                sec_bounds=np.array(sb, dtype=np.uint64), p2p_bounds=np.array(pb, dtype=np.uint64), schedule=schedule)
+                sec_bounds=np.array(sb, dtype=np.uint64), p2p_bounds=np.array(pb, dtype=np.uint64), schedule=schedule, ordering=ordering)

@@ -120,6 +120,8 @@ extern "C" int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* p
       c.regime = str_body > ring_body ? 2 : 1;
     }
   }
+  if (plan->opts.ordering == 1 && in.construction == OPTCC_C1)   // one stage per body: k + 3 bodies (PLAN_SPEC C1')
+    c.T_closed_form = c.T_limit * (double(k) + 3.0) / double(k);
   if (plan->opts.schedule == OPTCC_SCHED_RING_DEGRADED) {   // the baseline's own closed form; bounds stay those of the failure
     c.T_closed_form = c.T_limit = c.T_ring_degraded;
   }

@@ -121,6 +121,9 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
   if (healthy.size() < 2) return OPTCC_EINVAL;
   if (g > 1 && stragglers.size() != 1) return OPTCC_EUNSUPPORTED;  // E.5 (:943); all-healthy g>1 is NCCL's ring (:88)
   if (g > 255) return OPTCC_EUNSUPPORTED;                           // `part` is a byte
+  const uint32_t ordering = (opts && opts->ordering) ? opts->ordering : 2;   // 0 = default = ordering (2)
+  if (ordering != 1 && ordering != 2) return OPTCC_EINVAL;                   // the two valid orderings of :138
+  if (ordering == 1 && !(g == 1 && stragglers.size() == 1 && schedule == OPTCC_SCHED_OPTCC)) return OPTCC_EUNSUPPORTED;
   if (n == 0 || n > (uint64_t(1) << 40)) return OPTCC_EINVAL;
   if (dtype != OPTCC_F32 && dtype != OPTCC_BF16) return OPTCC_EINVAL;
   uint32_t k = opts ? opts->k : 0;
@@ -182,7 +185,36 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
   // ---- PLAN_SPEC 4: constructions ----
   uint32_t n_steps = 0;
   try {
-    if (construction == OPTCC_C0) {
+    if (construction == OPTCC_C1 && ordering == 1) {
+      // C1': ordering (1) of :138, S1 -> S2 -> S3 -> S4, one stage per body (PLAN_SPEC 4 C1')
+      n_steps = (k + 3) * H;
+      const uint32_t sg = stragglers[0];
+      for (uint32_t Bd = 0; Bd < k + 3; ++Bd) {
+        const uint32_t base = Bd * H;
+        for (uint32_t j = 0; j < H; ++j) {
+          const uint32_t src = healthy[j], dst = healthy[(j + 1) % H];
+          for (uint32_t t = 0; t + 1 < H; ++t) {
+            const uint32_t step = base + (t < j ? t : t + 1);
+            const uint32_t c = modH(int64_t(j) - t, H);
+            if (Bd < k)    // Stage 1: partial sums of the healthy servers (:126)
+              B.emit_sec(step, OPTCC_OP_REDUCE, OPTCC_S1, OPTCC_LINK_NIC, 0, src, dst, Bd, c);
+            if (Bd >= 3)   // Stage 4: the all-gather of section c starts at healthy c (:136)
+              B.emit_sec(step, OPTCC_OP_COPY, OPTCC_S4, OPTCC_LINK_NIC, 0, src, dst, Bd - 3, c);
+          }
+        }
+        for (uint32_t a = 0; a < H; ++a) {
+          const uint32_t d = (a + 1) % H, step = base + a;
+          if (Bd >= 1 && Bd <= k)       // Stage 2: the straggler adds its own data to the uploaded partial sum (:130-132)
+            B.emit_sec(step, OPTCC_OP_REDUCE, OPTCC_S2, OPTCC_LINK_NIC, 0, healthy[a], sg, Bd - 1, (a + 1) % H);
+          if (Bd >= 2 && Bd <= k + 1)   // Stage 3: the global sum returns to the uploader's ring successor (:132, R11)
+            B.emit_sec(step, OPTCC_OP_COPY, OPTCC_S3, OPTCC_LINK_NIC, 0, sg, healthy[d], Bd - 2, d);
+          if (bubbles && Bd < k)
+            B.emit_units(step, OPTCC_OP_REDUCE, OPTCC_BUB_UP, OPTCC_LINK_NIC, 0, healthy[a], sg, Bd, 0, p2p_lo(Bd), p2p_lo(Bd + 1));
+          if (bubbles && Bd >= 1 && Bd <= k)
+            B.emit_units(step, OPTCC_OP_COPY, OPTCC_BUB_DOWN, OPTCC_LINK_NIC, 0, sg, healthy[d], Bd - 1, 0, p2p_lo(Bd - 1), p2p_lo(Bd));
+        }
+      }
+    } else if (construction == OPTCC_C0) {
       // plain ring: reduce-scatter p-1 hops then all-gather p-1 hops (:52, :72)
       n_steps = 2 * (p - 1);
       for (int t = 0; t < p - 1; ++t)
