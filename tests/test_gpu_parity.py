@@ -268,3 +268,16 @@ def test_no_write_outside_the_rank_buffers(dtype, n, exec_mode):
         lo, hi = r * stride, r * stride + guard + n * esz
         assert (host[lo:lo + guard] == 0xA5).all(), f"rank {r}: write before the buffer"
         assert (host[hi:(r + 1) * stride] == 0xA5).all(), f"rank {r}: write past element n-1"
+
+
+@pytest.mark.parametrize("exec_mode", MODES)
+def test_more_than_128_ranks_use_the_pointer_table(exec_mode):
+    """p > 128: rank pointers no longer fit the kernel parameters and travel through the workspace; contributor
+    masks are limited to p <= 128 (R17), so optcc_verify must refuse with EUNSUPPORTED."""
+    p, n, k = 160, 20001, 4
+    w = _wl(p, 1, {7: 2.0}, n, W.F32, seed=160)
+    plan, s = _run_and_check(w, k, exec_mode)
+    assert plan.info["mask_words"] == 0
+    with pytest.raises(B.OptccError) as e:
+        s.verify()
+    assert e.value.name == "EUNSUPPORTED"
