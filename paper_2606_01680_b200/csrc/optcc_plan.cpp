@@ -25,11 +25,21 @@ struct Builder {
     return lo + (i * (hi - lo)) / parts;
   }
   uint64_t E(uint64_t u) const { return std::min(u * A, n); }
+  std::vector<uint64_t> sec_tab;   // section boundaries [(lam * k + b) * (nsec + 1) + c], filled once by build_sec_tab
+  void build_sec_tab() {
+    sec_tab.resize(ring.size() * size_t(k) * (nsec + 1));
+    for (size_t lam = 0; lam < ring.size(); ++lam)
+      for (uint32_t b = 0; b < k; ++b) {
+        const uint64_t s0 = split(ring[lam].first, ring[lam].second, k, b);
+        const uint64_t s1 = split(ring[lam].first, ring[lam].second, k, b + 1);
+        uint64_t* row = sec_tab.data() + (lam * k + b) * (nsec + 1);
+        for (uint32_t c = 0; c <= nsec; ++c) row[c] = split(s0, s1, nsec, c);
+      }
+  }
   void sec_units(uint32_t lam, uint32_t b, uint32_t c, uint64_t* lo, uint64_t* hi) const {
-    uint64_t s0 = split(ring[lam].first, ring[lam].second, k, b);
-    uint64_t s1 = split(ring[lam].first, ring[lam].second, k, b + 1);
-    *lo = split(s0, s1, nsec, c);
-    *hi = split(s0, s1, nsec, c + 1);
+    const uint64_t* row = sec_tab.data() + (size_t(lam) * k + b) * (nsec + 1);
+    *lo = row[c];
+    *hi = row[c + 1];
   }
   void emit_units(uint32_t step, uint8_t op, uint8_t stage, uint8_t link, uint32_t part, uint32_t src,
                   uint32_t dst, uint32_t seg, uint32_t sec, uint64_t ulo, uint64_t uhi) {
@@ -58,6 +68,34 @@ bool flow_less(const optcc_flow_t& a, const optcc_flow_t& b) {
   if (a.src != b.src) return a.src < b.src;
   if (a.dst != b.dst) return a.dst < b.dst;
   return a.off < b.off;
+}
+
+// PLAN_SPEC 3 order (step, link, stage, src, dst, off): counting sort by step, then each step's few flows by a
+// packed key -- the table has O(p k H) records, a comparison sort of whole records dominated the build time.
+void sort_flows(std::vector<optcc_flow_t>& flows, uint32_t n_steps) {
+  struct Key { uint64_t hi, lo; uint32_t idx; };
+  const size_t nf = flows.size();
+  std::vector<uint32_t> begin(size_t(n_steps) + 2, 0);
+  for (const auto& f : flows) begin[f.step + 1]++;
+  for (size_t t = 0; t <= n_steps; ++t) begin[t + 1] += begin[t];
+  std::vector<Key> keys(nf);
+  {
+    std::vector<uint32_t> pos(begin.begin(), begin.end() - 1);
+    for (size_t i = 0; i < nf; ++i) {
+      const optcc_flow_t& f = flows[i];
+      Key k;
+      k.hi = (uint64_t(f.link) << 35) | (uint64_t(f.stage) << 32) | (uint64_t(f.src) << 16) | uint64_t(f.dst);
+      k.lo = f.off;
+      k.idx = (uint32_t)i;
+      keys[pos[f.step]++] = k;
+    }
+  }
+  for (size_t t = 0; t <= n_steps; ++t)
+    std::sort(keys.begin() + begin[t], keys.begin() + begin[t + 1],
+              [](const Key& a, const Key& b) { return a.hi != b.hi ? a.hi < b.hi : a.lo < b.lo; });
+  std::vector<optcc_flow_t> out(nf);
+  for (size_t i = 0; i < nf; ++i) out[i] = flows[keys[i].idx];
+  flows.swap(out);
 }
 
 // Storage kinds for bf16 plans: walk the table once with the number of contributors every
@@ -180,6 +218,14 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
   B.k = k;
   B.nsec = construction == OPTCC_C0 ? (uint32_t)p : H;
   auto p2p_lo = [&](uint32_t b) { return Builder::split(U_ring, U, k, b); };
+  try {
+    B.build_sec_tab();
+    // flows: 2 (p-1) n elements in sections of about U / (g k nsec) units
+    pl->flows.reserve(size_t(2) * (k + 1) * (p - 1) * (B.nsec + m) * (g > 1 ? 2 : 1));
+  } catch (const std::bad_alloc&) {
+    delete pl;
+    return OPTCC_ENOMEM;
+  }
   const bool bubbles = construction == OPTCC_C1 && ell1 < 2.0;
 
   // ---- PLAN_SPEC 4: constructions ----
@@ -278,7 +324,7 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
         }
       }
     }
-    std::sort(pl->flows.begin(), pl->flows.end(), flow_less);
+    sort_flows(pl->flows, n_steps);
     pl->step_begin.assign(n_steps + 1, 0);
     {
       size_t i = 0;
@@ -338,17 +384,18 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
       while (tu < OPTCC_TILE_UNITS_DEFAULT && uint64_t(tu) * 3 / 2 < per) tu *= 2;
       pl->tile_units = tu;
     }
-    std::vector<std::pair<uint64_t, uint64_t>> regs;
-    regs.reserve(pl->flows.size());
-    for (const auto& f : pl->flows) regs.push_back({f.off, f.len});
-    std::sort(regs.begin(), regs.end());
-    regs.erase(std::unique(regs.begin(), regs.end()), regs.end());
+    // regions = the sections and P2P pieces themselves: consecutive exported boundaries (ascending, contiguous)
     uint64_t tiles = 0;
-    for (const auto& r : regs) {
-      pl->region_offs.push_back(r.first);
-      pl->region_tile0.push_back(tiles);
-      tiles += ((r.second + B.A - 1) / B.A + pl->tile_units - 1) / pl->tile_units;
-    }
+    auto add_regions = [&](const std::vector<uint64_t>& bounds) {
+      for (size_t i = 0; i + 1 < bounds.size(); ++i) {
+        if (bounds[i + 1] <= bounds[i]) continue;
+        pl->region_offs.push_back(bounds[i]);
+        pl->region_tile0.push_back(tiles);
+        tiles += ((bounds[i + 1] - bounds[i] + B.A - 1) / B.A + pl->tile_units - 1) / pl->tile_units;
+      }
+    };
+    add_regions(pl->sec_bounds);
+    add_regions(pl->p2p_bounds);
     pl->tiles_per_rank = tiles;
     for (const auto& f : pl->flows) pl->n_tile_ops += ((f.len + B.A - 1) / B.A + pl->tile_units - 1) / pl->tile_units;
   } catch (const std::bad_alloc&) {
