@@ -180,7 +180,8 @@ OPTCC_API int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* pa
  * the enqueued work every bufs[i] holds sum_j x_j and all p outputs are bitwise identical (PAPER.md:68 (ii)).
  * The reduce-scatter and all-gather steps are carried out exactly as the plan lists them, step by step.
  * workspace [device, >= workspace_bytes, 256-byte aligned] owned by the caller; the first call with a given
- * workspace uploads the tables into it (optcc_prepare does this ahead of time).  stream: a cudaStream_t
+ * workspace (or after another plan used it) uploads the tables into it; optcc_prepare does this ahead of time and
+ * always re-uploads -- call it again if the workspace memory was reused for something else in between.  stream: a cudaStream_t
  * (NULL = default stream).  Asynchronous: never synchronises the device or the stream.
  * Errors: EINVAL (NULL / misaligned pointers), ECUDA. */
 OPTCC_API int optcc_prepare(optcc_plan_t* plan, void* workspace, void* stream);

@@ -8,6 +8,9 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <atomic>
+#include <mutex>
+#include <unordered_map>
 #include <vector>
 
 #include "optcc_internal.h"
@@ -471,12 +474,20 @@ __global__ void __launch_bounds__(256) optcc_mask_check_kernel(const unsigned lo
 // Host side
 // =====================================================================================================
 
+namespace {
+// Which plan's tables a workspace currently holds (by workspace address).  Contents are the caller's to keep intact
+// between calls; after reusing the memory for something else, call optcc_prepare again.
+std::mutex g_ws_mutex;
+std::unordered_map<void*, uint64_t> g_ws_owner;
+std::atomic<uint64_t> g_next_id{1};
+}  // namespace
+
 struct optcc_exec_state {
   int device = -1;
   int sm_count = 0;
   int coop = 0;
   uint32_t G = 0;                 // executor grid (CTAs)
-  void* prepared_ws = nullptr;    // workspace that currently holds the device tables
+  uint64_t id = 0;                // process-unique id of this plan's device tables (see g_ws_owner)
   std::vector<DFlow> dflows;
   std::vector<Slice> slices;      // [n_steps][G + 1]
   // dataflow executor
@@ -557,7 +568,7 @@ int build_state(optcc_plan_t* pl) {
   int dev = 0;
   CU_TRY(cudaGetDevice(&dev));
   if (st->device == dev && st->G != 0) return OPTCC_OK;
-  st->prepared_ws = nullptr;
+  st->id = g_next_id.fetch_add(1);   // new tables: every workspace must be refreshed
   st->device = dev;
   CU_TRY(cudaDeviceGetAttribute(&st->sm_count, cudaDevAttrMultiProcessorCount, dev));
   CU_TRY(cudaDeviceGetAttribute(&st->coop, cudaDevAttrCooperativeLaunch, dev));
@@ -633,9 +644,13 @@ int build_state(optcc_plan_t* pl) {
   return OPTCC_OK;
 }
 
-int upload_tables(optcc_plan_t* pl, void* workspace, cudaStream_t stream) {
+int upload_tables(optcc_plan_t* pl, void* workspace, cudaStream_t stream, bool force) {
   optcc_exec_state* st = pl->exec;
-  if (st->prepared_ws == workspace) return OPTCC_OK;
+  if (!force) {
+    std::lock_guard<std::mutex> lock(g_ws_mutex);
+    auto it = g_ws_owner.find(workspace);
+    if (it != g_ws_owner.end() && it->second == st->id) return OPTCC_OK;   // this plan's tables are already there
+  }
   const optcc_ws_layout L = optcc_layout(pl);
   char* ws = static_cast<char*>(workspace);
   CU_TRY(cudaMemsetAsync(ws + L.ctrl, 0, OPTCC_CTRL_BYTES, stream));
@@ -647,7 +662,10 @@ int upload_tables(optcc_plan_t* pl, void* workspace, cudaStream_t stream) {
     CU_TRY(cudaMemcpyAsync(ws + L.deps, st->deps.data(), st->deps.size() * sizeof(DDep), cudaMemcpyHostToDevice, stream));
     CU_TRY(cudaMemcpyAsync(ws + L.ops, st->ops.data(), st->ops.size() * sizeof(TileOp), cudaMemcpyHostToDevice, stream));
   }
-  st->prepared_ws = workspace;
+  {
+    std::lock_guard<std::mutex> lock(g_ws_mutex);
+    g_ws_owner[workspace] = st->id;
+  }
   return OPTCC_OK;
 }
 
@@ -715,11 +733,19 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
 
 extern "C" int optcc_last_cuda_error(void) { return g_last_cuda_error; }
 
-extern "C" int optcc_prepare(optcc_plan_t* plan, void* workspace, void* stream) {
+namespace {
+int prepare_impl(optcc_plan_t* plan, void* workspace, void* stream, bool force) {
   if (!plan || !workspace || (reinterpret_cast<uintptr_t>(workspace) & 255)) return OPTCC_EINVAL;
   int rc = build_state(plan);
   if (rc != OPTCC_OK) return rc;
-  return upload_tables(plan, workspace, static_cast<cudaStream_t>(stream));
+  return upload_tables(plan, workspace, static_cast<cudaStream_t>(stream), force);
+}
+}  // namespace
+
+// Explicit call: always (re-)uploads.  optcc_execute / optcc_verify upload only if the workspace does not already
+// hold this plan's tables (tracked per workspace address, so two plans may alternate on one workspace).
+extern "C" int optcc_prepare(optcc_plan_t* plan, void* workspace, void* stream) {
+  return prepare_impl(plan, workspace, stream, true);
 }
 
 extern "C" int optcc_execute(optcc_plan_t* plan, void* const* bufs, void* workspace, void* stream_) {
@@ -728,7 +754,7 @@ extern "C" int optcc_execute(optcc_plan_t* plan, void* const* bufs, void* worksp
   for (uint32_t r = 0; r < in.p; ++r)
     if (!bufs[r] || (reinterpret_cast<uintptr_t>(bufs[r]) & 15)) return OPTCC_EINVAL;
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-  int rc = optcc_prepare(plan, workspace, stream_);
+  int rc = prepare_impl(plan, workspace, stream_, false);
   if (rc != OPTCC_OK) return rc;
   ExecParams P;
   fill_common(plan, workspace, P);
@@ -764,7 +790,7 @@ extern "C" int optcc_verify(optcc_plan_t* plan, void* workspace, void* stream_, 
   const optcc_plan_info_t& in = plan->info;
   if (in.mask_words == 0) return OPTCC_EUNSUPPORTED;
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-  int rc = optcc_prepare(plan, workspace, stream_);
+  int rc = prepare_impl(plan, workspace, stream_, false);
   if (rc != OPTCC_OK) return rc;
   const optcc_ws_layout L = optcc_layout(plan);
   char* ws = static_cast<char*>(workspace);

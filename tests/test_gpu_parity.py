@@ -281,3 +281,25 @@ def test_more_than_128_ranks_use_the_pointer_table(exec_mode):
     with pytest.raises(B.OptccError) as e:
         s.verify()
     assert e.value.name == "EUNSUPPORTED"
+
+
+def test_two_plans_alternate_on_one_workspace():
+    """The workspace holds one plan's tables at a time; execute must notice that another plan used it in between."""
+    import torch
+    from paper_2606_01680_b200.device import Session
+    wa = _wl(8, 1, {0: 2.0}, 40001, W.F32, seed=1)
+    wb = _wl(8, 1, {3: 1.5}, 40001, W.F32, seed=2)
+    pa = B.optcc_plan(wa.p, 1, wa.ell, wa.n, wa.dtype, k=4)
+    pb = B.optcc_plan(wb.p, 1, wb.ell, wb.n, wb.dtype, k=8)
+    sa = Session(pa)
+    big = max(pa.info["workspace_bytes"], pb.info["workspace_bytes"])
+    ws = torch.empty(int(big) + 256, dtype=torch.uint8, device=sa.device)
+    ptr = ws.data_ptr() + (-ws.data_ptr()) % 256
+    stream = torch.cuda.current_stream().cuda_stream
+    for plan, w in ((pa, wa), (pb, wb), (pa, wa), (pb, wb)):
+        x = W.all_inputs(w)
+        sa.upload(x)
+        B.optcc_execute(plan, sa.bufs, ptr, stream)
+        y = sa.download()
+        oplan = OP.build_plan(w.p, 1, list(w.ell), w.n, w.dtype, k=plan.info["k"])
+        assert y.tobytes() == OI.run_f32(oplan, x).tobytes()
