@@ -350,6 +350,7 @@ def run_native(args):
                   "lb_tight_over_T0": (cost0["lb_tight"] / cost0["T0"]) if cost0["lb_tight"] == cost0["lb_tight"] else None,
                   "paper_closed_form_over_T0": cost0["T_closed_form"] / cost0["T0"], "limit_over_T0": cost0["T_limit"] / cost0["T0"],
                   "bodies": cost0["bodies"], "k": k,
+                  "with_14pct_fixed_overhead": 0.14 + 0.86 * cost0["T_over_T0"],   # how the paper plots it (PAPER.md:201 fn.5)
                   "ring_on_degraded_topology_over_T0": cost0["T_ring_degraded"] / cost0["T0"],
                   "r2ccl_closed_form_over_T0": (cost0["T_r2ccl"] / cost0["T0"]) if cost0["T_r2ccl"] == cost0["T_r2ccl"] else None,
                   "paper_context": "SimAI: OPTCC within 2-6% of fault-free NCCL ring at <=50% bandwidth loss; prior work up to 57% (PAPER.md:7)"},
