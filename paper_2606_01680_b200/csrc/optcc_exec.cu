@@ -726,7 +726,13 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   P.tile_units = pl->tile_units;
   P.bulk_copy = pl->opts.copy_path == 2 ? 1u : 0u;
   P.l2_hints = 1;   // source loads evict_first, destination loads and stores evict_normal (measured best)
-  P.df_slots = pl->tile_units >= 1792 ? 2 : 4;   // big tiles: short look-ahead keeps the L2 reuse distance small
+  // ring depth by the average tile-op size: big ops -> 2 slots (short look-ahead keeps the L2 reuse distance small),
+  // small ops (small tiles, or flows shorter than a tile) -> 4 slots to hide the claim / fetch / completion latency
+  {
+    uint64_t units = 0;
+    for (const auto& f : pl->flows) units += (f.len + pl->info.unit_elems - 1) / pl->info.unit_elems;
+    P.df_slots = (pl->n_tile_ops && units / pl->n_tile_ops >= 1792) ? 2 : 4;
+  }
 }
 
 }  // namespace
