@@ -203,8 +203,8 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) optcc_exec_kernel(const 
 // streaming warps reach them in order -- progress is guaranteed.
 // ---------------------------------------------------------------------------------------------------------
 // ---- cp.async.bulk (TMA 1-D bulk copy) helpers for the all-gather (copy) tile-ops -----------------------------
-constexpr unsigned int BULK_CHUNK = 8192;     // bytes per bulk transfer
-constexpr unsigned int BULK_STAGES = 3;       // chunks in flight per scheduler agent
+constexpr unsigned int BULK_CHUNK = 4096;     // bytes per bulk transfer
+constexpr unsigned int BULK_STAGES = 4;       // chunks in flight per scheduler agent
 constexpr unsigned int BULK_SMEM_PER_AGENT = BULK_CHUNK * BULK_STAGES;
 
 __device__ __forceinline__ unsigned int smem_u32(const void* p) { return (unsigned int)__cvta_generic_to_shared(p); }
@@ -260,36 +260,35 @@ __device__ __forceinline__ void copy_extent(const ExecParams& P, const DFlow& f,
   *nbytes = e1 > e0 ? (e1 - e0) * esz : 0;
 }
 
-// One thread copies nbytes (src, dst 16-byte aligned) global -> shared -> global with bulk async copies:
-// rounds of up to BULK_STAGES chunks in flight; `parity` holds one phase bit per stage barrier.
+// One thread copies nbytes (src, dst 16-byte aligned) global -> shared -> global with bulk async copies, as a
+// continuous pipeline over a ring of BULK_STAGES chunks: chunk c is stored as soon as it has landed and its stage is
+// reloaded with chunk c + BULK_STAGES once the store has read it, so BULK_STAGES - 1 loads stay in flight.
+// `parity` holds one phase bit per stage barrier.
 __device__ __forceinline__ void bulk_copy(char* stage, unsigned long long* bars, unsigned int& parity,
                                           const char* src, char* dst, unsigned long long nbytes) {
   const unsigned long long n16 = nbytes & ~15ull;
-  for (unsigned long long base = 0; base < n16; base += (unsigned long long)BULK_CHUNK * BULK_STAGES) {
-    unsigned int issued = 0;
-#pragma unroll
-    for (unsigned int c = 0; c < BULK_STAGES; ++c) {
-      const unsigned long long o = base + (unsigned long long)c * BULK_CHUNK;
-      if (o < n16) {
-        const unsigned int b = (unsigned int)(n16 - o < BULK_CHUNK ? n16 - o : BULK_CHUNK);
-        mbar_expect_tx(bars + c, b);
-        bulk_g2s(stage + c * BULK_CHUNK, src + o, b, bars + c);
-        issued = c + 1;
-      }
+  const unsigned long long nch = (n16 + BULK_CHUNK - 1) / BULK_CHUNK;
+  auto chunk_bytes = [&](unsigned long long c) {
+    const unsigned long long o = c * BULK_CHUNK;
+    return (unsigned int)(n16 - o < BULK_CHUNK ? n16 - o : BULK_CHUNK);
+  };
+  auto load = [&](unsigned long long c) {
+    const unsigned int st = (unsigned int)(c % BULK_STAGES), b = chunk_bytes(c);
+    mbar_expect_tx(bars + st, b);
+    bulk_g2s(stage + st * BULK_CHUNK, src + c * BULK_CHUNK, b, bars + st);
+  };
+  for (unsigned long long c = 0; c < nch && c < BULK_STAGES; ++c) load(c);
+  for (unsigned long long c = 0; c < nch; ++c) {
+    const unsigned int st = (unsigned int)(c % BULK_STAGES);
+    mbar_wait(bars + st, (parity >> st) & 1u);
+    parity ^= 1u << st;
+    bulk_s2g(dst + c * BULK_CHUNK, stage + st * BULK_CHUNK, chunk_bytes(c));
+    if (c + BULK_STAGES < nch) {
+      bulk_wait_read_all();        // the store has read its stage: reload it
+      load(c + BULK_STAGES);
     }
-#pragma unroll
-    for (unsigned int c = 0; c < BULK_STAGES; ++c) {
-      if (c < issued) {
-        const unsigned long long o = base + (unsigned long long)c * BULK_CHUNK;
-        const unsigned int b = (unsigned int)(n16 - o < BULK_CHUNK ? n16 - o : BULK_CHUNK);
-        mbar_wait(bars + c, (parity >> c) & 1u);
-        parity ^= 1u << c;
-        bulk_s2g(dst + o, stage + c * BULK_CHUNK, b);
-      }
-    }
-    bulk_wait_read_all();   // the stages may be overwritten by the next round
   }
-  bulk_wait_all();          // every store has been performed
+  bulk_wait_all();                 // every store has been performed
   for (unsigned long long o = n16; o < nbytes; ++o) dst[o] = src[o];   // ragged end of a buffer (< 16 bytes)
 }
 
@@ -731,7 +730,7 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   {
     uint64_t units = 0;
     for (const auto& f : pl->flows) units += (f.len + pl->info.unit_elems - 1) / pl->info.unit_elems;
-    P.df_slots = (pl->n_tile_ops && units / pl->n_tile_ops >= 1792) ? 2 : 4;
+    P.df_slots = (pl->n_tile_ops && units / pl->n_tile_ops >= 1792 && !P.bulk_copy) ? 2 : 4;   // copying agents hold their slots
   }
 }
 
