@@ -1,0 +1,59 @@
+"""Randomised stress of the dataflow executor's dependency protocol (pytest -m gpu): many small seeded plans with tiny
+tiles and odd grids, so that tile-ops of different steps interleave as much as possible; every output must equal the
+oracle's plan-order walk bit for bit and the verifier's masks must be complete."""
+import numpy as np
+import pytest
+
+from paper_2606_01680_b200 import binding as B
+from paper_2606_01680_b200 import workloads as W
+from oracle import planner as OP
+from oracle import interpreter as OI
+
+pytestmark = pytest.mark.gpu
+
+
+def _random_case(rng):
+    kind = rng.integers(0, 5)
+    if kind == 0:      # one straggler, bubble filling or not
+        p = int(rng.integers(3, 25)); g = 1
+        st = {int(rng.integers(0, p)): float(rng.choice([8 / 7, 4 / 3, 1.6, 2.0, 3.0]))}
+    elif kind == 1:    # several stragglers
+        p = int(rng.integers(5, 20)); g = 1
+        m = int(rng.integers(2, min(4, p - 2) + 1))
+        st = {int(r): float(rng.choice([8 / 7, 4 / 3, 2.0])) for r in rng.choice(p, size=m, replace=False)}
+    elif kind == 2:    # multi-GPU servers, one straggler server
+        g = int(rng.choice([2, 4])); q = int(rng.integers(3, 7)); p = g * q
+        v = int(rng.integers(0, q)); l = float(rng.choice([8 / 7, 2.0]))
+        st = {v * g + i: l for i in range(g)}
+    elif kind == 3:    # no straggler: plain ring
+        p = int(rng.integers(3, 20)); g = 1; st = {}
+    else:              # ordering (1)
+        p = int(rng.integers(3, 16)); g = 1
+        st = {int(rng.integers(0, p)): float(rng.choice([1.5, 2.0, 3.0]))}
+    ell = [float(st.get(i, 1.0)) for i in range(p)]
+    n = int(rng.integers(1, 60000))
+    k = int(rng.choice([0, 4, 8]))
+    dtype = int(rng.integers(0, 2))
+    tile = int(rng.choice([1, 2, 7, 64, 224, 0]))
+    grid = int(rng.choice([0, 0, 3, 37, 148]))
+    return p, g, ell, n, k, dtype, tile, grid, (1 if kind == 4 else 0)
+
+
+@pytest.mark.parametrize("seed", range(40))
+def test_dataflow_random_plans(seed):
+    from paper_2606_01680_b200.device import Session
+    rng = np.random.default_rng(1000 + seed)
+    p, g, ell, n, k, dtype, tile, grid, ordering = _random_case(rng)
+    plan = B.optcc_plan(p, g, ell, n, dtype, k=k, exec_mode=B.OPTCC_EXEC_DATAFLOW, tile_units=tile, grid_ctas=grid, ordering=ordering)
+    oplan = OP.build_plan(p, g, ell, n, dtype, k=k, ordering=ordering or 2)
+    w = W.Workload("stress", p, g, tuple(ell), n, dtype, "normal", 1.0, 5000 + seed)
+    x = W.all_inputs(w)
+    s = Session(plan, verify=(p <= 128))
+    for _ in range(2):          # twice on the same session: counters and ticket must reset cleanly
+        s.upload(x)
+        s.execute()
+        y = s.download()
+        y_or = OI.run_f32(oplan, x) if dtype == W.F32 else OI.run_bf16(oplan, x)
+        assert y.tobytes() == y_or.tobytes()
+    res = s.verify()
+    assert res["bad_elements"] == 0 and res["overlap_elements"] == 0
