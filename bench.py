@@ -330,7 +330,7 @@ def run_native(args):
     kname = "optcc_dataflow_kernel" if args.exec_mode == 2 else "optcc_exec_kernel"
     kern = kname + ("<MODE_F32>" if w.dtype == W.F32 else "<MODE_BF16>")
     achieved = sched_bytes / t_exec / 1e6
-    mask_bytes = 5 * (w.p - 1) * w.n * 8 * plan0.info["mask_words"]
+    mask_bytes = 5 * (w.p - 1) * w.n * plan0.info["mask_bytes"]   # the same schedule on mask elements
     line = {
         "metric": METRIC, "value": world * w.n * esize / t_step / 1e6, "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": t_step, "higher_is_better": True,
@@ -357,7 +357,7 @@ def run_native(args):
         "roofline": {"bound": "hbm", "kernel": kern, "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": ncu_traffic(w.name.split("[")[0], kern),
                      "algorithmic_bytes_per_launch": sched_bytes, "share_of_step": t_exec / t_step},
-        "roofline_verify": {"bound": "hbm", "kernel": "%s<MODE_MASK%d> (+init, check)" % (kname, plan0.info["mask_words"]),
+        "roofline_verify": {"bound": "hbm", "kernel": "%s<masks of %d bits> (+init, check)" % (kname, 8 * plan0.info["mask_bytes"]),
                             "achieved": mask_bytes / t_ver / 1e6, "peak": peak, "unit": "GB/s", "frac": mask_bytes / t_ver / 1e6 / peak,
                             "share_of_step": t_ver / t_step},
         "parity_spot_check": {"sampled_elements": int(len(idx)), "within_tolerance": parity_ok},

@@ -97,7 +97,7 @@ typedef struct optcc_plan_info {
   uint32_t construction;       /* OPTCC_C* */
   uint32_t dtype;              /* OPTCC_F32 | OPTCC_BF16 */
   uint32_t unit_elems;         /* A = 16/sizeof(dtype) (PLAN_SPEC 2) */
-  uint32_t mask_words;         /* 64-bit words per contributor mask: 1 (p<=64) or 2 (p<=128); 0 if p>128 */
+  uint32_t mask_words;         /* 64-bit words a contributor mask is reported in: 1 (p<=64) or 2 (p<=128); 0 if p>128 */
   uint64_t n, n_ring, n_p2p;   /* elements per rank; on the ring path; on the P2P (bubble) path */
   uint64_t U, U_ring, U_p2p;   /* the same in 16-byte units */
   uint32_t n_steps;
@@ -105,13 +105,14 @@ typedef struct optcc_plan_info {
   uint32_t max_flows_per_step;
   uint32_t n_sec_bounds;       /* entries of sec_bounds */
   uint32_t n_p2p_bounds;       /* entries of p2p_bounds (0 if no P2P path) */
-  uint32_t reserved;
+  uint32_t mask_bytes;         /* bytes per contributor mask in the workspace: 2 (p<=16, bf16 plans), 4 (p<=32), 8 (p<=64), 16 (p<=128);
+                                  0 if p>128 (optcc_verify: EUNSUPPORTED) */
   uint64_t reduce_elems;       /* sum of len over reduce flows  = (p-1) n  (Lemma 4) */
   uint64_t copy_elems;         /* sum of len over copy flows    = (p-1) n */
   uint64_t workspace_bytes;    /* device workspace optcc_execute needs (tables, barrier, bf16 fp32 partials) */
   uint64_t verify_workspace_bytes; /* device workspace optcc_verify needs (>= workspace_bytes) */
-  uint64_t mask_offset_bytes;  /* after optcc_verify: masks of (rank r, element e, word w) at
-                                  workspace + mask_offset_bytes + ((r*padded_n + e)*mask_words + w)*8 */
+  uint64_t mask_offset_bytes;  /* after optcc_verify: the mask of (rank r, element e) is at
+                                  workspace + mask_offset_bytes + (r*padded_n + e)*mask_bytes, little endian, bit i = rank i */
   uint64_t padded_n;           /* n rounded up to a multiple of 8: per-rank stride of masks and fp32 partials */
   double   plan_build_seconds; /* wall time optcc_plan spent ("< 1 ms at p=1024") */
 } optcc_plan_info_t;

@@ -36,7 +36,7 @@ class optcc_opts_t(C.Structure):
 class optcc_plan_info_t(C.Structure):
     _fields_ = [(n, C.c_uint32) for n in ("p", "g", "q", "m", "H", "k", "construction", "dtype", "unit_elems", "mask_words")] + \
                [(n, C.c_uint64) for n in ("n", "n_ring", "n_p2p", "U", "U_ring", "U_p2p")] + \
-               [(n, C.c_uint32) for n in ("n_steps", "n_flows", "max_flows_per_step", "n_sec_bounds", "n_p2p_bounds", "reserved")] + \
+               [(n, C.c_uint32) for n in ("n_steps", "n_flows", "max_flows_per_step", "n_sec_bounds", "n_p2p_bounds", "mask_bytes")] + \
                [(n, C.c_uint64) for n in ("reduce_elems", "copy_elems", "workspace_bytes", "verify_workspace_bytes",
                                           "mask_offset_bytes", "padded_n")] + \
                [("plan_build_seconds", C.c_double)]

@@ -41,6 +41,8 @@ template <> struct ModeTraits<MODE_F32>   { static constexpr int ESIZE = 4,  VE 
 template <> struct ModeTraits<MODE_BF16>  { static constexpr int ESIZE = 2,  VE = 8; };
 template <> struct ModeTraits<MODE_MASK1> { static constexpr int ESIZE = 8,  VE = 2; };
 template <> struct ModeTraits<MODE_MASK2> { static constexpr int ESIZE = 16, VE = 1; };
+template <> struct ModeTraits<MODE_MASK16> { static constexpr int ESIZE = 2, VE = 8; };
+template <> struct ModeTraits<MODE_MASK32> { static constexpr int ESIZE = 4, VE = 4; };
 
 __device__ __forceinline__ char* rank_ptr(const ExecParams& P, unsigned int r) {
   return reinterpret_cast<char*>(P.ptr_table ? P.ptr_table[r] : P.bufs[r]);
@@ -71,22 +73,29 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
       if (f.op == 0) x = __fadd_rn(__ldcg(df + e), x);
       __stcg(df + e, x);
     }
-  } else if (MODE == MODE_MASK1 || MODE == MODE_MASK2) {
-    constexpr int W = MODE == MODE_MASK1 ? 1 : 2;
-    const char* s = rank_ptr(P, f.src) + f.off * (8 * W);
-    char* d = rank_ptr(P, f.dst) + f.off * (8 * W);
-    if (f.op == 0) range_or_mask<4, W, NT>(s, d, vbeg, vend, overlaps, pol); else range_copy16<4, NT>(s, d, vbeg, vend, pol);
-    if (threadIdx.x < tail) {  // MASK1 only: one odd element
-      unsigned long long e = vend * 2;
-      const unsigned long long* sm = reinterpret_cast<const unsigned long long*>(s);
-      unsigned long long* dm = reinterpret_cast<unsigned long long*>(d);
-      unsigned long long x = __ldcg(sm + e);
-      if (f.op == 0) {
-        unsigned long long y = __ldcg(dm + e);
-        overlaps += (x & y) != 0ull;
-        x |= y;
+  } else if (is_mask_mode(MODE)) {
+    constexpr int EB = MT::ESIZE;
+    const char* s = rank_ptr(P, f.src) + f.off * EB;
+    char* d = rank_ptr(P, f.dst) + f.off * EB;
+    if (f.op == 0) range_or_mask<4, EB, NT>(s, d, vbeg, vend, overlaps, pol); else range_copy16<4, NT>(s, d, vbeg, vend, pol);
+    if (threadIdx.x < tail) {  // ragged end (n not a multiple of the elements per vector): one element per thread
+      const unsigned long long e = vend * MT::VE + threadIdx.x;
+      unsigned long long x, y = 0;
+      if (EB == 2) {
+        x = __ldcg(reinterpret_cast<const unsigned short*>(s) + e);
+        if (f.op == 0) y = __ldcg(reinterpret_cast<const unsigned short*>(d) + e);
+      } else if (EB == 4) {
+        x = __ldcg(reinterpret_cast<const unsigned int*>(s) + e);
+        if (f.op == 0) y = __ldcg(reinterpret_cast<const unsigned int*>(d) + e);
+      } else {
+        x = __ldcg(reinterpret_cast<const unsigned long long*>(s) + e);
+        if (f.op == 0) y = __ldcg(reinterpret_cast<const unsigned long long*>(d) + e);
       }
-      __stcg(dm + e, x);
+      overlaps += (x & y) != 0ull;
+      x |= y;
+      if (EB == 2) __stcg(reinterpret_cast<unsigned short*>(d) + e, (unsigned short)x);
+      else if (EB == 4) __stcg(reinterpret_cast<unsigned int*>(d) + e, (unsigned int)x);
+      else __stcg(reinterpret_cast<unsigned long long*>(d) + e, x);
     }
   } else {  // MODE_BF16
     const char* s = f.ksrc ? reinterpret_cast<const char*>(P.shadow + (unsigned long long)f.src * P.padded_n + f.off)
@@ -183,7 +192,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) optcc_exec_kernel(const 
     }
   }
 
-  if (MODE == MODE_MASK1 || MODE == MODE_MASK2) {
+  if (is_mask_mode(MODE)) {
     // warp-shuffle reduction of the per-thread overlap counts, one atomic per warp
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) overlaps += __shfl_xor_sync(0xFFFFFFFFu, overlaps, o);
@@ -246,8 +255,8 @@ __device__ __forceinline__ void copy_extent(const ExecParams& P, const DFlow& f,
   char* d;
   if (MODE == MODE_F32) {
     esz = 4; s = rank_ptr(P, f.src); d = rank_ptr(P, f.dst);
-  } else if (MODE == MODE_MASK1 || MODE == MODE_MASK2) {
-    esz = MODE == MODE_MASK1 ? 8 : 16; s = rank_ptr(P, f.src); d = rank_ptr(P, f.dst);
+  } else if (is_mask_mode(MODE)) {
+    esz = mask_bytes_of(MODE); s = rank_ptr(P, f.src); d = rank_ptr(P, f.dst);
   } else if (f.ksrc == 0) {
     esz = 2; s = rank_ptr(P, f.src); d = rank_ptr(P, f.dst);
   } else {
@@ -402,7 +411,7 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
       __syncwarp();
       if ((threadIdx.x & 31) == 0) red_release_cta_shared_add(&s_done[s], 1u);
     }
-    if (MODE == MODE_MASK1 || MODE == MODE_MASK2) {
+    if (is_mask_mode(MODE)) {
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) overlaps += __shfl_xor_sync(0xFFFFFFFFu, overlaps, o);
       if ((threadIdx.x & 31) == 0 && overlaps) atomicAdd(&P.ctrl->overlap, (unsigned long long)overlaps);
@@ -410,49 +419,58 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
   }
 }
 
-// masks[r][e][w] = {r}: blockIdx.y = rank, 16-byte stores over the rank's padded array
-__global__ void __launch_bounds__(256) optcc_mask_init_kernel(unsigned long long* masks, unsigned long long padded_n,
-                                                              unsigned int W) {
+// A 16-byte vector of masks, every element = `bits` (the low EB*8 bits of a 128-bit value given as lo, hi)
+__device__ __forceinline__ uint4 mask_vector(unsigned long long lo, unsigned long long hi, unsigned int eb) {
+  if (eb == 2) { const unsigned int w = (unsigned int)(lo & 0xFFFFull) * 0x10001u; return make_uint4(w, w, w, w); }
+  if (eb == 4) { const unsigned int w = (unsigned int)lo; return make_uint4(w, w, w, w); }
+  if (eb == 8) return make_uint4((unsigned int)lo, (unsigned int)(lo >> 32), (unsigned int)lo, (unsigned int)(lo >> 32));
+  return make_uint4((unsigned int)lo, (unsigned int)(lo >> 32), (unsigned int)hi, (unsigned int)(hi >> 32));
+}
+
+// masks[r][e] = {r}: blockIdx.y = rank, 16-byte stores over the rank's padded array; eb = bytes per mask
+__global__ void __launch_bounds__(256) optcc_mask_init_kernel(char* masks, unsigned long long padded_n, unsigned int eb) {
   const unsigned int r = blockIdx.y;
-  const unsigned long long w0 = r < 64 ? 1ull << r : 0ull, w1 = r >= 64 ? 1ull << (r - 64) : 0ull;
-  // a 16-byte vector is two one-word masks or one two-word mask
-  const ulonglong2 v = W == 1 ? make_ulonglong2(w0, w0) : make_ulonglong2(w0, w1);
-  ulonglong2* m = reinterpret_cast<ulonglong2*>(masks + (unsigned long long)r * padded_n * W);
-  const unsigned long long nvec = padded_n * W / 2;
+  const uint4 v = mask_vector(r < 64 ? 1ull << r : 0ull, r >= 64 ? 1ull << (r - 64) : 0ull, eb);
+  uint4* m = reinterpret_cast<uint4*>(masks + (unsigned long long)r * padded_n * eb);
+  const unsigned long long nvec = padded_n * eb / 16;
   for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < nvec;
        i += (unsigned long long)gridDim.x * blockDim.x)
     __stcg(m + i, v);
 }
 
 // every (rank, element) must hold every rank exactly once: mask == all p bits (PAPER.md:68 (ii))
-__global__ void __launch_bounds__(256) optcc_mask_check_kernel(const unsigned long long* masks, unsigned int p,
-                                                               unsigned long long n, unsigned long long padded_n,
-                                                               unsigned int W, Ctrl* ctrl) {
+__global__ void __launch_bounds__(256) optcc_mask_check_kernel(const char* masks, unsigned int p, unsigned long long n,
+                                                               unsigned long long padded_n, unsigned int eb, Ctrl* ctrl) {
   const unsigned int r = blockIdx.y;
   const unsigned long long full0 = p >= 64 ? ~0ull : ((1ull << p) - 1ull);
   const unsigned long long full1 = p > 64 ? (p >= 128 ? ~0ull : ((1ull << (p - 64)) - 1ull)) : 0ull;
-  const ulonglong2* m = reinterpret_cast<const ulonglong2*>(masks + (unsigned long long)r * padded_n * W);
-  const unsigned long long nvec = (n * W + 1) / 2;
-  unsigned long long bad = 0, first = ~0ull;
+  const uint4 F = mask_vector(full0, full1, eb);
+  const uint4* m = reinterpret_cast<const uint4*>(masks + (unsigned long long)r * padded_n * eb);
+  const unsigned int epv = 16 / eb;                                  // elements per vector
+  const unsigned long long nvec = (n + epv - 1) / epv;
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  unsigned long long bad = 0, first = ~0ull;
   for (unsigned long long i0 = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i0 < nvec; i0 += 4 * stride) {
-    ulonglong2 vv[4];
+    uint4 vv[4];
 #pragma unroll
-    for (int q = 0; q < 4; ++q) vv[q] = i0 + q * stride < nvec ? __ldcg(m + i0 + q * stride) : make_ulonglong2(full0, W == 1 ? full0 : full1);
+    for (int q = 0; q < 4; ++q) vv[q] = i0 + q * stride < nvec ? __ldcg(m + i0 + q * stride) : F;
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
-    const unsigned long long i = i0 + q * stride;
-    if (i >= nvec) break;
-    const ulonglong2 v = vv[q];
-    if (W == 1) {
-      const unsigned long long e = 2 * i;
-      if (v.x != full0) { ++bad; const unsigned long long g = (unsigned long long)r * n + e; first = first < g ? first : g; }
-      if (e + 1 < n && v.y != full0) { ++bad; const unsigned long long g = (unsigned long long)r * n + e + 1; first = first < g ? first : g; }
-    } else if (v.x != full0 || v.y != full1) {
-      ++bad;
-      const unsigned long long g = (unsigned long long)r * n + i;
-      first = first < g ? first : g;
-    }
+      const unsigned long long i = i0 + q * stride;
+      if (i >= nvec) break;
+      const unsigned int dx = vv[q].x ^ F.x, dy = vv[q].y ^ F.y, dz = vv[q].z ^ F.z, dw = vv[q].w ^ F.w;
+      if ((dx | dy | dz | dw) == 0u) continue;
+      const unsigned int d[4] = {dx, dy, dz, dw};
+      for (unsigned int j = 0; j < epv; ++j) {                      // rare path: locate the wrong elements
+        const unsigned long long e = i * epv + j;
+        if (e >= n) break;
+        bool wrong;
+        if (eb == 2) wrong = ((d[j >> 1] >> ((j & 1u) * 16)) & 0xFFFFu) != 0u;
+        else if (eb == 4) wrong = d[j] != 0u;
+        else if (eb == 8) wrong = (d[2 * j] | d[2 * j + 1]) != 0u;
+        else wrong = true;
+        if (wrong) { ++bad; const unsigned long long g = (unsigned long long)r * n + e; first = first < g ? first : g; }
+      }
     }
   }
 #pragma unroll
@@ -580,6 +598,10 @@ int build_state(optcc_plan_t* pl) {
   occ = std::min(occ, o);
   if ((rc = kernel_occupancy<MODE_MASK2>(&o)) != OPTCC_OK) return rc;
   occ = std::min(occ, o);
+  if ((rc = kernel_occupancy<MODE_MASK16>(&o)) != OPTCC_OK) return rc;
+  occ = std::min(occ, o);
+  if ((rc = kernel_occupancy<MODE_MASK32>(&o)) != OPTCC_OK) return rc;
+  occ = std::min(occ, o);
   if (occ < 1) { g_last_cuda_error = (int)cudaErrorLaunchOutOfResources; return OPTCC_ECUDA; }
   occ = std::min(occ, CTAS_PER_SM);
   uint32_t maxG = std::min<uint32_t>(uint32_t(st->sm_count) * uint32_t(occ), OPTCC_MAX_GRID);
@@ -594,6 +616,10 @@ int build_state(optcc_plan_t* pl) {
     if ((rc = df_kernel_occupancy<MODE_MASK1>(&o2)) != OPTCC_OK) return rc;
     od = std::min(od, o2);
     if ((rc = df_kernel_occupancy<MODE_MASK2>(&o2)) != OPTCC_OK) return rc;
+    od = std::min(od, o2);
+    if ((rc = df_kernel_occupancy<MODE_MASK16>(&o2)) != OPTCC_OK) return rc;
+    od = std::min(od, o2);
+    if ((rc = df_kernel_occupancy<MODE_MASK32>(&o2)) != OPTCC_OK) return rc;
     od = std::min(std::min(od, o2), CTAS_PER_SM);
     uint32_t maxGd = std::min<uint32_t>(uint32_t(st->sm_count) * uint32_t(std::max(od, 0)), OPTCC_MAX_GRID);
     st->G_df = pl->opts.grid_ctas ? std::min(pl->opts.grid_ctas, maxGd) : maxGd;
@@ -793,29 +819,32 @@ extern "C" int optcc_execute_host(optcc_plan_t* plan, const void* const* host_in
 extern "C" int optcc_verify(optcc_plan_t* plan, void* workspace, void* stream_, optcc_verify_result_t* out) {
   if (!plan || !workspace || !out) return OPTCC_EINVAL;
   const optcc_plan_info_t& in = plan->info;
-  if (in.mask_words == 0) return OPTCC_EUNSUPPORTED;
+  if (in.mask_bytes == 0) return OPTCC_EUNSUPPORTED;
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   int rc = prepare_impl(plan, workspace, stream_, false);
   if (rc != OPTCC_OK) return rc;
   const optcc_ws_layout L = optcc_layout(plan);
   char* ws = static_cast<char*>(workspace);
-  unsigned long long* masks = reinterpret_cast<unsigned long long*>(ws + L.masks);
+  char* masks = ws + L.masks;
+  const uint32_t eb = in.mask_bytes;
   ExecParams P;
   fill_common(plan, workspace, P);
-  for (uint32_t r = 0; r < in.p; ++r) P.bufs[r] = masks + uint64_t(r) * in.padded_n * in.mask_words;
+  for (uint32_t r = 0; r < in.p; ++r) P.bufs[r] = masks + uint64_t(r) * in.padded_n * eb;
   Ctrl init;
   std::memset(&init, 0, sizeof init);
   init.first_bad = ~0ull;
   CU_TRY(cudaMemcpyAsync(P.ctrl, &init, sizeof init, cudaMemcpyHostToDevice, stream));
-  const uint64_t vec_per_rank = in.padded_n * in.mask_words / 2;
+  const uint64_t vec_per_rank = in.padded_n * eb / 16;
   const unsigned int bx = (unsigned int)std::max<uint64_t>(1, std::min<uint64_t>((vec_per_rank + 1023) / 1024,
                                                           std::max<uint64_t>(1, uint64_t(plan->exec->sm_count) * 16 / in.p)));
   const dim3 blocks(bx, in.p);
-  optcc_mask_init_kernel<<<blocks, 256, 0, stream>>>(masks, in.padded_n, in.mask_words);
+  optcc_mask_init_kernel<<<blocks, 256, 0, stream>>>(masks, in.padded_n, eb);
   CU_TRY(cudaGetLastError());
-  rc = in.mask_words == 1 ? launch_plan<MODE_MASK1>(plan, P, stream) : launch_plan<MODE_MASK2>(plan, P, stream);
+  rc = eb == 2 ? launch_plan<MODE_MASK16>(plan, P, stream)
+               : eb == 4 ? launch_plan<MODE_MASK32>(plan, P, stream)
+                         : eb == 8 ? launch_plan<MODE_MASK1>(plan, P, stream) : launch_plan<MODE_MASK2>(plan, P, stream);
   if (rc != OPTCC_OK) return rc;
-  optcc_mask_check_kernel<<<blocks, 256, 0, stream>>>(masks, in.p, in.n, in.padded_n, in.mask_words, P.ctrl);
+  optcc_mask_check_kernel<<<blocks, 256, 0, stream>>>(masks, in.p, in.n, in.padded_n, eb, P.ctrl);
   CU_TRY(cudaGetLastError());
   Ctrl res;
   CU_TRY(cudaMemcpyAsync(&res, P.ctrl, sizeof res, cudaMemcpyDeviceToHost, stream));

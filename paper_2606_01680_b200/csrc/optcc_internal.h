@@ -70,7 +70,7 @@ static inline optcc_ws_layout optcc_layout(const optcc_plan_t* pl) {
   uint64_t n_pad = (in.n + 7) & ~uint64_t(7);
   L.end_exec = optcc_align256(L.shadow + (in.dtype == OPTCC_BF16 ? uint64_t(in.p) * n_pad * 4 : 0));
   L.masks = L.end_exec;
-  L.end_verify = optcc_align256(L.masks + uint64_t(in.p) * n_pad * in.mask_words * 8);
+  L.end_verify = optcc_align256(L.masks + uint64_t(in.p) * n_pad * in.mask_bytes);
   return L;
 }
 

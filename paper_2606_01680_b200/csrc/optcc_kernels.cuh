@@ -19,7 +19,10 @@
 
 namespace optcc_dev {
 
-enum { MODE_F32 = 0, MODE_BF16 = 1, MODE_MASK1 = 2, MODE_MASK2 = 3 };
+enum { MODE_F32 = 0, MODE_BF16 = 1, MODE_MASK1 = 2, MODE_MASK2 = 3, MODE_MASK16 = 4, MODE_MASK32 = 5 };
+__host__ __device__ constexpr bool is_mask_mode(int m) { return m >= MODE_MASK1; }
+// bytes per contributor mask: 16 bits (p <= 16), 32 (p <= 32), 64 (p <= 64), 128 (p <= 128)
+__host__ __device__ constexpr int mask_bytes_of(int m) { return m == MODE_MASK16 ? 2 : m == MODE_MASK32 ? 4 : m == MODE_MASK1 ? 8 : 16; }
 
 constexpr int THREADS = 512;      // threads per CTA
 constexpr int CTAS_PER_SM = 2;    // resident CTAs per SM the kernels are tuned for (<= 64 registers/thread)
@@ -181,15 +184,24 @@ __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* 
   for (; v < vend; v += NT) st16(d + v * 16, add_f32x4(ld16(d + v * 16, pol.ldd), ld16(s + v * 16, pol.lds)), pol);
 }
 
-// masks: OR with overlap detection.  WORDS = 64-bit words per element (1 or 2); a 16-byte vector holds 2/WORDS elements
-template <int UNROLL, int WORDS, int NT>
+// masks: OR with overlap detection.  EB = bytes per mask element (2, 4, 8 or 16); a 16-byte vector holds 16/EB elements
+template <int UNROLL, int EB, int NT>
 __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* __restrict__ d,
                                               unsigned long long vbeg, unsigned long long vend,
                                               unsigned int& overlaps, const Pol& pol) {
   unsigned long long v = vbeg + threadIdx.x;
   auto join = [&](uint4 a, uint4 b) {
-    unsigned int lo = ((a.x & b.x) | (a.y & b.y)) != 0u, hi = ((a.z & b.z) | (a.w & b.w)) != 0u;
-    overlaps += (WORDS == 1) ? (lo + hi) : ((lo | hi) ? 1u : 0u);
+    const unsigned int cx = a.x & b.x, cy = a.y & b.y, cz = a.z & b.z, cw = a.w & b.w;   // elements whose sets overlap
+    if (EB == 2) {
+      auto hw = [](unsigned int w) { return ((w & 0xFFFFu) != 0u) + ((w >> 16) != 0u); };
+      overlaps += hw(cx) + hw(cy) + hw(cz) + hw(cw);
+    } else if (EB == 4) {
+      overlaps += (cx != 0u) + (cy != 0u) + (cz != 0u) + (cw != 0u);
+    } else if (EB == 8) {
+      overlaps += ((cx | cy) != 0u) + ((cz | cw) != 0u);
+    } else {
+      overlaps += ((cx | cy | cz | cw) != 0u);
+    }
     return make_uint4(a.x | b.x, a.y | b.y, a.z | b.z, a.w | b.w);
   };
   for (; v + (UNROLL - 1) * (unsigned long long)NT < vend; v += UNROLL * (unsigned long long)NT) {

@@ -355,7 +355,10 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
   optcc_plan_info_t& in = pl->info;
   in.p = p; in.g = g; in.q = q; in.m = m; in.H = H; in.k = k;
   in.construction = construction; in.dtype = dtype; in.unit_elems = (uint32_t)B.A;
-  in.mask_words = p <= 64 ? 1 : (p <= 128 ? 2 : 0);
+  // narrowest mask that holds p bits and keeps every flow offset (a multiple of A elements) 16-byte aligned: >= 16/A bytes
+  in.mask_bytes = p <= 16 ? 2 : (p <= 32 ? 4 : (p <= 64 ? 8 : (p <= 128 ? 16 : 0)));
+  if (in.mask_bytes) in.mask_bytes = std::max<uint32_t>(in.mask_bytes, uint32_t(16 / B.A));
+  in.mask_words = (in.mask_bytes + 7) / 8;
   in.n = n; in.n_ring = B.E(U_ring); in.n_p2p = n - B.E(U_ring);
   in.U = U; in.U_ring = U_ring; in.U_p2p = U_p2p;
   in.n_steps = n_steps; in.n_flows = (uint32_t)pl->flows.size();

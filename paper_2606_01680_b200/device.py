@@ -57,12 +57,19 @@ class Session:
         return out
 
     def masks(self):
-        """After verify(): contributor masks as numpy uint64 [p, n, W] (copied from the workspace)."""
+        """After verify(): contributor masks as numpy uint64 [p, n, W] (W = mask_words), widened from the
+        workspace's mask_bytes-wide little-endian storage."""
         i = self.plan.info
-        W, pn = i["mask_words"], i["padded_n"]
+        eb, W, pn = i["mask_bytes"], i["mask_words"], i["padded_n"]
         start = self._ws_off + i["mask_offset_bytes"]
-        raw = self.workspace[start:start + self.p * pn * W * 8].view(torch.int64).cpu().numpy().view(np.uint64)
-        return raw.reshape(self.p, pn, W)[:, :self.n, :].copy()
+        raw = self.workspace[start:start + self.p * pn * eb].cpu().numpy()
+        if eb == 2:
+            m = raw.view("<u2").reshape(self.p, pn)[:, :self.n].astype(np.uint64)[:, :, None]
+        elif eb == 4:
+            m = raw.view("<u4").reshape(self.p, pn)[:, :self.n].astype(np.uint64)[:, :, None]
+        else:
+            m = raw.view("<u8").reshape(self.p, pn, W)[:, :self.n, :]
+        return np.ascontiguousarray(m)
 
     # -- the C-ABI calls --
     def _stream(self, stream):
