@@ -575,20 +575,13 @@ inline uint64_t unit_cost(const optcc_plan_t* pl, size_t i) {
   return c;
 }
 
-int build_state(optcc_plan_t* pl) {
-  optcc_exec_state* st = pl->exec;
-  if (!st) {
-    st = new (std::nothrow) optcc_exec_state();
-    if (!st) return OPTCC_ENOMEM;
-    pl->exec = st;
-  }
-  int dev = 0;
-  CU_TRY(cudaGetDevice(&dev));
-  if (st->device == dev && st->G != 0) return OPTCC_OK;
-  st->id = g_next_id.fetch_add(1);   // new tables: every workspace must be refreshed
-  st->device = dev;
-  CU_TRY(cudaDeviceGetAttribute(&st->sm_count, cudaDevAttrMultiProcessorCount, dev));
-  CU_TRY(cudaDeviceGetAttribute(&st->coop, cudaDevAttrCooperativeLaunch, dev));
+// Per-device launch limits (SM count, resident CTAs of every kernel instantiation), queried once per process and device.
+struct DeviceLimits { int sm_count = 0, coop = 0; uint32_t max_grid = 0, max_grid_df = 0; };
+
+int query_device_limits(int dev, DeviceLimits* out) {
+  DeviceLimits lim;
+  CU_TRY(cudaDeviceGetAttribute(&lim.sm_count, cudaDevAttrMultiProcessorCount, dev));
+  CU_TRY(cudaDeviceGetAttribute(&lim.coop, cudaDevAttrCooperativeLaunch, dev));
   int occ = 0, o = 0, rc;
   if ((rc = kernel_occupancy<MODE_F32>(&o)) != OPTCC_OK) return rc;
   occ = o;
@@ -604,26 +597,60 @@ int build_state(optcc_plan_t* pl) {
   occ = std::min(occ, o);
   if (occ < 1) { g_last_cuda_error = (int)cudaErrorLaunchOutOfResources; return OPTCC_ECUDA; }
   occ = std::min(occ, CTAS_PER_SM);
-  uint32_t maxG = std::min<uint32_t>(uint32_t(st->sm_count) * uint32_t(occ), OPTCC_MAX_GRID);
-  uint32_t G = pl->opts.grid_ctas ? std::min(pl->opts.grid_ctas, maxG) : maxG;
-  st->G = G;
-  {
-    int od = 0, o2 = 0;
-    if ((rc = df_kernel_occupancy<MODE_F32>(&o2)) != OPTCC_OK) return rc;
-    od = o2;
-    if ((rc = df_kernel_occupancy<MODE_BF16>(&o2)) != OPTCC_OK) return rc;
-    od = std::min(od, o2);
-    if ((rc = df_kernel_occupancy<MODE_MASK1>(&o2)) != OPTCC_OK) return rc;
-    od = std::min(od, o2);
-    if ((rc = df_kernel_occupancy<MODE_MASK2>(&o2)) != OPTCC_OK) return rc;
-    od = std::min(od, o2);
-    if ((rc = df_kernel_occupancy<MODE_MASK16>(&o2)) != OPTCC_OK) return rc;
-    od = std::min(od, o2);
-    if ((rc = df_kernel_occupancy<MODE_MASK32>(&o2)) != OPTCC_OK) return rc;
-    od = std::min(std::min(od, o2), CTAS_PER_SM);
-    uint32_t maxGd = std::min<uint32_t>(uint32_t(st->sm_count) * uint32_t(std::max(od, 0)), OPTCC_MAX_GRID);
-    st->G_df = pl->opts.grid_ctas ? std::min(pl->opts.grid_ctas, maxGd) : maxGd;
+  lim.max_grid = std::min<uint32_t>(uint32_t(lim.sm_count) * uint32_t(occ), OPTCC_MAX_GRID);
+  int od = 0;
+  if ((rc = df_kernel_occupancy<MODE_F32>(&o)) != OPTCC_OK) return rc;
+  od = o;
+  if ((rc = df_kernel_occupancy<MODE_BF16>(&o)) != OPTCC_OK) return rc;
+  od = std::min(od, o);
+  if ((rc = df_kernel_occupancy<MODE_MASK1>(&o)) != OPTCC_OK) return rc;
+  od = std::min(od, o);
+  if ((rc = df_kernel_occupancy<MODE_MASK2>(&o)) != OPTCC_OK) return rc;
+  od = std::min(od, o);
+  if ((rc = df_kernel_occupancy<MODE_MASK16>(&o)) != OPTCC_OK) return rc;
+  od = std::min(od, o);
+  if ((rc = df_kernel_occupancy<MODE_MASK32>(&o)) != OPTCC_OK) return rc;
+  od = std::min(std::min(od, o), CTAS_PER_SM);
+  lim.max_grid_df = std::min<uint32_t>(uint32_t(lim.sm_count) * uint32_t(std::max(od, 0)), OPTCC_MAX_GRID);
+  *out = lim;
+  return OPTCC_OK;
+}
+
+int device_limits(int dev, DeviceLimits* out) {
+  static std::mutex mu;
+  static std::unordered_map<int, DeviceLimits> cache;
+  std::lock_guard<std::mutex> lock(mu);
+  auto it = cache.find(dev);
+  if (it == cache.end()) {
+    DeviceLimits lim;
+    int rc = query_device_limits(dev, &lim);
+    if (rc != OPTCC_OK) return rc;
+    it = cache.emplace(dev, lim).first;
   }
+  *out = it->second;
+  return OPTCC_OK;
+}
+
+int build_state(optcc_plan_t* pl) {
+  optcc_exec_state* st = pl->exec;
+  if (!st) {
+    st = new (std::nothrow) optcc_exec_state();
+    if (!st) return OPTCC_ENOMEM;
+    pl->exec = st;
+  }
+  int dev = 0;
+  CU_TRY(cudaGetDevice(&dev));
+  if (st->device == dev && st->G != 0) return OPTCC_OK;
+  st->id = g_next_id.fetch_add(1);   // new tables: every workspace must be refreshed
+  st->device = dev;
+  DeviceLimits lim;
+  int rc = device_limits(dev, &lim);
+  if (rc != OPTCC_OK) return rc;
+  st->sm_count = lim.sm_count;
+  st->coop = lim.coop;
+  const uint32_t G = pl->opts.grid_ctas ? std::min(pl->opts.grid_ctas, lim.max_grid) : lim.max_grid;
+  st->G = G;
+  st->G_df = pl->opts.grid_ctas ? std::min(pl->opts.grid_ctas, lim.max_grid_df) : lim.max_grid_df;
 
   const optcc_plan_info_t& in = pl->info;
   const uint64_t A = in.unit_elems;
