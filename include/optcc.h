@@ -83,7 +83,8 @@ typedef struct optcc_opts {
   uint32_t k;         /* segments; 0 = auto (PLAN_SPEC 2 "k"); else a multiple of 4 */
   uint32_t exec_mode; /* OPTCC_EXEC_* */
   uint32_t grid_ctas; /* 0 = auto (SM count x resident CTAs per SM); else CTAs of the executor grid */
-  uint32_t copy_path; /* 0 = auto, 1 = LDG/STG vector copy, 2 = cp.async.bulk (TMA 1-D) copy */
+  uint32_t copy_path; /* copy (all-gather) tile-ops: 0 = auto (= 1, the faster one on the large configs), 1 = LDG/STG vector
+                         copy by the streaming warps, 2 = cp.async.bulk (TMA 1-D) copy by the scheduler agents (dataflow only) */
   uint32_t step_limit;/* 0 = all steps; else execute / verify only the first step_limit steps (debugging and
                          profiling: a truncated schedule must FAIL verification) */
   uint32_t tile_units;/* dataflow executor: 16-byte units per tile-op; 0 = auto (224..3584: about two tile-ops per CTA and step, whole streaming rounds) */

@@ -1,16 +1,16 @@
 // Device code of the OPTCC executor (sm_100a).  Included only by optcc_exec.cu.
 //
-// One kernel template walks the plan's step tables for all element types:
-//   MODE_F32    rank buffers of float; reduce = one IEEE fp32 add per element ("adds its own section")
-//   MODE_BF16   rank buffers of bf16, fp32 partial sums in a shadow array, one RNE rounding when a sum completes (R12)
-//   MODE_MASK1  contributor bitmasks, one 64-bit word per element  (p <= 64)   reduce = disjoint OR, copy = assign
-//   MODE_MASK2  contributor bitmasks, two 64-bit words per element (p <= 128)
+// Shared device definitions: the device flow / dependency records, the launch parameters and the 16-byte-vector
+// range operations every executor uses, for all element types:
+//   MODE_F32     rank buffers of float; reduce = one IEEE fp32 add per element ("adds its own section")
+//   MODE_BF16    rank buffers of bf16, fp32 partial sums in a shadow array, one RNE rounding when a sum completes (R12)
+//   MODE_MASK16 / 32 / 1 / 2   contributor bitmasks of 16 / 32 / 64 / 128 bits: reduce = disjoint OR, copy = assign
 // so the verifier (PAPER.md:68 correctness (ii)) runs exactly the tables the executor runs.
 //
-// Work distribution: a step's flows are concatenated in table order and cut into gridDim.x slices of equal
-// HBM bytes (host-built slice table); CTA c streams slice c with 16-byte vector loads/stores, fully coalesced,
-// UNROLL independent vectors in flight per thread.  The CTA's part of the step table is staged in shared memory
-// one step ahead.  Steps are separated by a grid-wide barrier (persistent mode) or by kernel boundaries.
+// Executors (optcc_exec.cu): the dataflow kernel (tile-ops claimed in table order, per-range completion counters, no
+// grid barrier; the default), the persistent kernel (host-built slices of equal HBM bytes per step and CTA, grid
+// barrier between steps) and the same kernel launched once per step.  All stream 16-byte vectors, fully coalesced,
+// UNROLL independent vectors in flight per thread and stream.
 #ifndef OPTCC_KERNELS_CUH_
 #define OPTCC_KERNELS_CUH_
 
