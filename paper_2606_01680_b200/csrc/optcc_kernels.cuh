@@ -15,6 +15,7 @@
 #define OPTCC_KERNELS_CUH_
 
 #include <cstdint>
+#include <type_traits>
 #include <cuda_runtime.h>
 
 namespace optcc_dev {
@@ -153,6 +154,18 @@ __device__ __forceinline__ void grid_barrier(unsigned long long* ctr, unsigned l
 // Range operations.  All ranges are given in 16-byte vectors [vbeg, vend) relative to the flow's start.
 // =====================================================================================================
 
+// calls f(std::integral_constant<int, rem>) for rem in 1 .. UNROLL-1 (UNROLL <= 8)
+template <int UNROLL, class F>
+__device__ __forceinline__ void remainder_dispatch(unsigned int rem, F&& f) {
+  if (UNROLL > 7 && rem >= 7) f(std::integral_constant<int, 7>());
+  else if (UNROLL > 6 && rem == 6) f(std::integral_constant<int, 6>());
+  else if (UNROLL > 5 && rem == 5) f(std::integral_constant<int, 5>());
+  else if (UNROLL > 4 && rem == 4) f(std::integral_constant<int, 4>());
+  else if (UNROLL > 3 && rem >= 3) f(std::integral_constant<int, 3>());
+  else if (UNROLL > 2 && rem == 2) f(std::integral_constant<int, 2>());
+  else f(std::integral_constant<int, 1>());
+}
+
 template <int UNROLL, int NT>
 __device__ __forceinline__ void range_copy16(const char* __restrict__ s, char* __restrict__ d,
                                              unsigned long long vbeg, unsigned long long vend, const Pol& pol) {
@@ -164,7 +177,18 @@ __device__ __forceinline__ void range_copy16(const char* __restrict__ s, char* _
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, x[j], pol);
   }
-  for (; v < vend; v += NT) st16(d + v * 16, ld16(s + v * 16, pol.lds), pol);
+  if (v < vend) {   // remainder (< UNROLL vectors for this thread): still one batch of loads, then the stores
+    const unsigned int rem = (unsigned int)((vend - v + NT - 1) / NT);
+    auto batch = [&](auto K) {
+      constexpr int KK = decltype(K)::value;
+      uint4 x[KK];
+#pragma unroll
+      for (int j = 0; j < KK; ++j) x[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds);
+#pragma unroll
+      for (int j = 0; j < KK; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, x[j], pol);
+    };
+    remainder_dispatch<UNROLL>(rem, batch);
+  }
 }
 
 template <int UNROLL, int NT>
@@ -181,7 +205,21 @@ __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* 
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, add_f32x4(b[j], a[j]), pol);
   }
-  for (; v < vend; v += NT) st16(d + v * 16, add_f32x4(ld16(d + v * 16, pol.ldd), ld16(s + v * 16, pol.lds)), pol);
+  if (v < vend) {   // remainder: one batch of loads, then the adds and stores
+    const unsigned int rem = (unsigned int)((vend - v + NT - 1) / NT);
+    auto batch = [&](auto K) {
+      constexpr int KK = decltype(K)::value;
+      uint4 a[KK], b[KK];
+#pragma unroll
+      for (int j = 0; j < KK; ++j) {
+        a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds);
+        b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd);
+      }
+#pragma unroll
+      for (int j = 0; j < KK; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, add_f32x4(b[j], a[j]), pol);
+    };
+    remainder_dispatch<UNROLL>(rem, batch);
+  }
 }
 
 // masks: OR with overlap detection.  EB = bytes per mask element (2, 4, 8 or 16); a 16-byte vector holds 16/EB elements
@@ -214,7 +252,21 @@ __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* 
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, join(a[j], b[j]), pol);
   }
-  for (; v < vend; v += NT) st16(d + v * 16, join(ld16(s + v * 16, pol.lds), ld16(d + v * 16, pol.ldd)), pol);
+  if (v < vend) {   // remainder: one batch of loads, then the joins and stores
+    const unsigned int rem = (unsigned int)((vend - v + NT - 1) / NT);
+    auto batch = [&](auto K) {
+      constexpr int KK = decltype(K)::value;
+      uint4 a[KK], b[KK];
+#pragma unroll
+      for (int j = 0; j < KK; ++j) {
+        a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds);
+        b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd);
+      }
+#pragma unroll
+      for (int j = 0; j < KK; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, join(a[j], b[j]), pol);
+    };
+    remainder_dispatch<UNROLL>(rem, batch);
+  }
 }
 
 // bf16 plans: a unit is 8 elements = 16 bytes in a rank buffer or 32 bytes in the fp32 shadow.
