@@ -510,6 +510,7 @@ struct optcc_exec_state {
   // dataflow executor
   uint32_t G_df = 0;              // grid of the dataflow kernel
   bool df_ok = false;             // counters fit 32-bit indices
+  bool big_ops = false;           // average tile-op >= 1792 units (decides the ring depth)
   std::vector<DDep> deps;         // [n_flows]
   std::vector<TileOp> ops;        // [n_tile_ops], table order
   std::vector<uint64_t> step_op_begin;   // [n_steps + 1]
@@ -534,6 +535,11 @@ void build_dataflow_tables(optcc_plan_t* pl, optcc_exec_state* st) {
   const optcc_plan_info_t& in = pl->info;
   const uint64_t A = in.unit_elems, TU = pl->tile_units, nr = pl->region_offs.size();
   st->df_ok = uint64_t(in.p) * pl->tiles_per_rank < (uint64_t(1) << 32) && pl->n_tile_ops < (uint64_t(1) << 40);
+  {
+    uint64_t units = 0;
+    for (const auto& f : pl->flows) units += (f.len + A - 1) / A;
+    st->big_ops = pl->n_tile_ops && units / pl->n_tile_ops >= 1792;
+  }
   if (!st->df_ok) return;
   std::vector<uint32_t> count(size_t(in.p) * nr, 0), lastw(size_t(in.p) * nr, 0);
   st->deps.resize(in.n_flows);
@@ -778,13 +784,10 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   P.tile_units = pl->tile_units;
   P.bulk_copy = pl->opts.copy_path == 2 ? 1u : 0u;
   P.l2_hints = 1;   // source loads evict_first, destination loads and stores evict_normal (measured best)
-  // ring depth by the average tile-op size: big ops -> 2 slots (short look-ahead keeps the L2 reuse distance small),
-  // small ops (small tiles, or flows shorter than a tile) -> 4 slots to hide the claim / fetch / completion latency
-  {
-    uint64_t units = 0;
-    for (const auto& f : pl->flows) units += (f.len + pl->info.unit_elems - 1) / pl->info.unit_elems;
-    P.df_slots = (pl->n_tile_ops && units / pl->n_tile_ops >= 1792 && !P.bulk_copy) ? 2 : 4;   // copying agents hold their slots
-  }
+  // ring depth by the average tile-op size (computed once in build_state): big ops -> 2 slots (short look-ahead keeps
+  // the L2 reuse distance small), small ops (small tiles, or flows shorter than a tile) -> 4 slots to hide the claim /
+  // fetch / completion latency; copying agents hold their slots, so the bulk path also uses 4
+  P.df_slots = (pl->exec && pl->exec->big_ops && !P.bulk_copy) ? 2 : 4;
 }
 
 }  // namespace
