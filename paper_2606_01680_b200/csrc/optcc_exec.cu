@@ -201,15 +201,15 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) optcc_exec_kernel(const 
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Dataflow executor: no grid barrier.  12 streaming warps + up to 4 scheduler agents (one lane each) per CTA.
+// Dataflow executor: no grid barrier.  14 streaming warps + up to 4 scheduler agents (one lane each) per CTA.
 // Agent w owns slot w of a small ring in shared memory (this CTA's staged part of the segment table): it claims the
-// next tile-op (global ticket, table order), fetches its flow record into the slot, waits until the accesses the op
-// depends on have completed (per-(rank, region, tile) counters, ld.acquire.gpu), publishes the slot, waits for the
-// streaming warps to finish it, then fences and bumps the counters of the two ranges the op touched.  Streaming
-// warps never synchronise with each other: each polls the slot's sequence number, streams its share and bumps a
-// shared done-counter.  Tickets are claimed in local order (s_turn), so inside a CTA the local order is the table
-// order; an op only waits on ops with smaller tickets, each held by a resident CTA (cooperative launch), whose
-// streaming warps reach them in order -- progress is guaranteed.
+// next tile-op (global ticket, table order; claims are made in turn), fetches its flow record into the slot, waits
+// until the accesses the op depends on have completed (per-(rank, region, tile) counters, ld.acquire.gpu), puts the
+// slot into the CTA's ready queue, waits for the streaming warps to finish it, then fences and bumps the counters of
+// the two ranges the op touched.  Streaming warps never synchronise with each other: each takes the next entry of the
+// ready queue, streams its share and bumps a shared done-counter.  An op only waits on ops with smaller tickets, each
+// held by a resident CTA (cooperative launch), and streaming warps only see ops whose dependencies are satisfied --
+// progress is guaranteed.
 // ---------------------------------------------------------------------------------------------------------
 // ---- cp.async.bulk (TMA 1-D bulk copy) helpers for the all-gather (copy) tile-ops -----------------------------
 constexpr unsigned int BULK_CHUNK = 4096;     // bytes per bulk transfer
@@ -330,14 +330,22 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
   constexpr unsigned int NW = DF_COMPUTE_THREADS / 32;   // streaming warps
   const unsigned int NS = P.df_slots;                    // slots in the ring = scheduler agents in use (<= DF_SLOTS)
   __shared__ DfSlot s_slot[DF_SLOTS];
-  __shared__ unsigned int s_full[DF_SLOTS];   // sequence number of the op published in the slot (j + 1)
+  constexpr unsigned int QN = 2 * DF_SLOTS;   // ready queue: slots in the order their dependencies were satisfied
+  __shared__ unsigned int s_queue[QN];        // entry q % QN: slot number, or QSTOP
+  __shared__ unsigned int s_qflag[QN];        // entry q % QN is valid when the flag reads q + 1
+  __shared__ unsigned int s_tail;             // next queue position
+  __shared__ unsigned int s_exhausted;        // agents that found no ticket left
+  constexpr unsigned int QSTOP = 0xFFFFFFFFu;
   __shared__ unsigned int s_done[DF_SLOTS];   // streaming warps that finished ops of the slot (monotone)
   __shared__ unsigned int s_turn;             // local sequence number whose ticket is claimed next
   __shared__ __align__(8) unsigned long long s_bar[DF_SLOTS][BULK_STAGES];   // mbarriers of the bulk-copy stages
   extern __shared__ __align__(128) char s_stage[];   // bulk-copy staging: BULK_SMEM_PER_AGENT per agent (copy_path 2)
-  if (threadIdx.x < DF_SLOTS) { s_full[threadIdx.x] = 0; s_done[threadIdx.x] = 0; }
+  if (threadIdx.x < DF_SLOTS) s_done[threadIdx.x] = 0;
+  if (threadIdx.x < QN) s_qflag[threadIdx.x] = 0;
   if (threadIdx.x == 0) {
     s_turn = 0;
+    s_tail = 0;
+    s_exhausted = 0;
     for (unsigned int a = 0; a < DF_SLOTS; ++a)
       for (unsigned int c = 0; c < BULK_STAGES; ++c) mbar_init(&s_bar[a][c], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -357,9 +365,12 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
       while (ld_acquire_cta_shared_u32(&s_turn) != j) { }
       const unsigned long long t = atomicAdd(&P.ctrl->ticket, 1ull);
       st_release_cta_shared_u32(&s_turn, j + 1);
-      if (t >= P.n_ops) {              // nothing left: stop marker (the streaming warps stop at the first one)
-        sl.valid = 0;
-        st_release_cta_shared_u32(&s_full[w], j + 1);
+      if (t >= P.n_ops) {              // nothing left; the last agent to get here queues the stop marker
+        if (atomicAdd(&s_exhausted, 1u) == NS - 1) {
+          const unsigned int pos = atomicAdd(&s_tail, 1u);
+          s_queue[pos % QN] = QSTOP;
+          st_release_cta_shared_u32(&s_qflag[pos % QN], pos + 1);
+        }
         return;
       }
       const unsigned long long opw = __ldg(reinterpret_cast<const unsigned long long*>(P.ops + t));
@@ -379,7 +390,12 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
       // the accesses this op depends on (PAPER.md:138 data dependencies), per (rank, region, tile)
       while (ld_acquire_gpu_u32(c_src) < dp.z) { }
       while (ld_acquire_gpu_u32(c_dst) < dp.w) { }
-      st_release_cta_shared_u32(&s_full[w], j + 1);
+      {   // ready: queue the slot.  The streaming warps take slots in readiness order, so an op that still waits
+          // for its dependencies never holds up a later one that is ready.
+        const unsigned int pos = atomicAdd(&s_tail, 1u);
+        s_queue[pos % QN] = w;
+        st_release_cta_shared_u32(&s_qflag[pos % QN], pos + 1);
+      }
       if (bulk) {
         const char* src;
         char* dst;
@@ -398,11 +414,11 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
     }
   } else {
     // ---------------- streaming warps ----------------
-    for (unsigned int j = 0;; ++j) {
-      const unsigned int s = j % NS;
-      while (ld_acquire_cta_shared_u32(&s_full[s]) < j + 1) { }
+    for (unsigned int q = 0;; ++q) {
+      while (ld_acquire_cta_shared_u32(&s_qflag[q % QN]) != q + 1) { }
+      const unsigned int s = s_queue[q % QN];
+      if (s == QSTOP) break;
       const unsigned int kind = s_slot[s].valid;
-      if (!kind) break;
       if (kind == 1) {   // kind 2: the agent copies it with cp.async.bulk; the streaming warps move on
         const DFlow f = s_slot[s].f;
         const unsigned long long ubeg = s_slot[s].ubeg, uend = s_slot[s].uend;
