@@ -360,12 +360,39 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
     if ((threadIdx.x & 31) != 0 || w >= NS) return;
     DfSlot& sl = s_slot[w];
     unsigned int bulk_parity = 0;
+    // state of the op streaming from my slot (cur) and of the op fetched ahead into registers (nxt)
+    unsigned int* cur_src = nullptr; unsigned int* cur_dst = nullptr;
+    unsigned int cur_target = 0;
+    bool cur_pending = false;                    // queued, not yet completed
+    auto try_complete = [&]() {                  // every streaming warp is done with cur -> publish its writes
+      if (cur_pending && ld_acquire_cta_shared_u32(&s_done[w]) >= cur_target) {
+        __threadfence();
+        atomicAdd(cur_src, 1u);
+        atomicAdd(cur_dst, 1u);
+        cur_pending = false;
+      }
+    };
     for (unsigned int j = w;; j += NS) {
-      // tickets are claimed in local order, so that local order == table order inside the CTA
-      while (ld_acquire_cta_shared_u32(&s_turn) != j) { }
+      // ---- claim and fetch op j (while the previous op of this slot may still be streaming) ----
+      // tickets are claimed in turn, so that inside a CTA the local order is the table order
+      while (ld_acquire_cta_shared_u32(&s_turn) != j) try_complete();
       const unsigned long long t = atomicAdd(&P.ctrl->ticket, 1ull);
       st_release_cta_shared_u32(&s_turn, j + 1);
-      if (t >= P.n_ops) {              // nothing left; the last agent to get here queues the stop marker
+      try_complete();
+      const bool valid = t < P.n_ops;
+      unsigned long long opw = 0;
+      if (valid) opw = __ldg(reinterpret_cast<const unsigned long long*>(P.ops + t));
+      try_complete();
+      const unsigned int flow = (unsigned int)opw, tile = (unsigned int)(opw >> 32);
+      uint4 f0 = make_uint4(0, 0, 0, 0), f1 = f0, dp = f0;
+      if (valid) {
+        const uint4* fr = reinterpret_cast<const uint4*>(P.flows + flow);
+        f0 = __ldg(fr); f1 = __ldg(fr + 1);
+        dp = __ldg(reinterpret_cast<const uint4*>(P.deps + flow));
+      }
+      // ---- the slot must be free before it is refilled ----
+      while (cur_pending) try_complete();
+      if (!valid) {                    // nothing left; the last agent to get here queues the stop marker
         if (atomicAdd(&s_exhausted, 1u) == NS - 1) {
           const unsigned int pos = atomicAdd(&s_tail, 1u);
           s_queue[pos % QN] = QSTOP;
@@ -373,11 +400,6 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
         }
         return;
       }
-      const unsigned long long opw = __ldg(reinterpret_cast<const unsigned long long*>(P.ops + t));
-      const unsigned int flow = (unsigned int)opw, tile = (unsigned int)(opw >> 32);
-      const uint4* fr = reinterpret_cast<const uint4*>(P.flows + flow);
-      const uint4 f0 = __ldg(fr), f1 = __ldg(fr + 1);
-      const uint4 dp = __ldg(reinterpret_cast<const uint4*>(P.deps + flow));
       memcpy(&sl.f, &f0, 16);
       memcpy(reinterpret_cast<char*>(&sl.f) + 16, &f1, 16);
       const unsigned long long A = P.unit_elems, nunits = (sl.f.len + A - 1) / A;
@@ -385,17 +407,19 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
       sl.uend = sl.ubeg + P.tile_units < nunits ? sl.ubeg + P.tile_units : nunits;
       const bool bulk = P.bulk_copy && sl.f.op == 1;   // all-gather tile-op: this agent moves it with cp.async.bulk
       sl.valid = bulk ? 2 : 1;
-      unsigned int* c_src = P.counters + dp.x + tile;
-      unsigned int* c_dst = P.counters + dp.y + tile;
+      cur_src = P.counters + dp.x + tile;
+      cur_dst = P.counters + dp.y + tile;
       // the accesses this op depends on (PAPER.md:138 data dependencies), per (rank, region, tile)
-      while (ld_acquire_gpu_u32(c_src) < dp.z) { }
-      while (ld_acquire_gpu_u32(c_dst) < dp.w) { }
+      while (ld_acquire_gpu_u32(cur_src) < dp.z) { }
+      while (ld_acquire_gpu_u32(cur_dst) < dp.w) { }
       {   // ready: queue the slot.  The streaming warps take slots in readiness order, so an op that still waits
           // for its dependencies never holds up a later one that is ready.
         const unsigned int pos = atomicAdd(&s_tail, 1u);
         s_queue[pos % QN] = w;
         st_release_cta_shared_u32(&s_qflag[pos % QN], pos + 1);
       }
+      cur_target = NW * (j / NS + 1);
+      cur_pending = true;
       if (bulk) {
         const char* src;
         char* dst;
@@ -405,12 +429,7 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
         bulk_copy(s_stage + w * BULK_SMEM_PER_AGENT, s_bar[w], bulk_parity, src, dst, nbytes);
         fence_proxy_async();
       }
-      // completion: every streaming warp is done with it (bulk ops: has passed it) -> make the writes visible, bump the range counters
-      const unsigned int target = NW * (j / NS + 1);
-      while (ld_acquire_cta_shared_u32(&s_done[w]) < target) { }
-      __threadfence();
-      atomicAdd(c_src, 1u);
-      atomicAdd(c_dst, 1u);
+      // completion happens inside the next iteration's claim / fetch (try_complete), overlapped with it
     }
   } else {
     // ---------------- streaming warps ----------------
