@@ -410,8 +410,9 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
       cur_src = P.counters + dp.x + tile;
       cur_dst = P.counters + dp.y + tile;
       // the accesses this op depends on (PAPER.md:138 data dependencies), per (rank, region, tile)
-      while (ld_acquire_gpu_u32(cur_src) < dp.z) { }
-      while (ld_acquire_gpu_u32(cur_dst) < dp.w) { }
+      // (a range nobody has touched yet needs no look at its counter: raw inputs, first writes)
+      if (dp.z) while (ld_acquire_gpu_u32(cur_src) < dp.z) { }
+      if (dp.w) while (ld_acquire_gpu_u32(cur_dst) < dp.w) { }
       {   // ready: queue the slot.  The streaming warps take slots in readiness order, so an op that still waits
           // for its dependencies never holds up a later one that is ready.
         const unsigned int pos = atomicAdd(&s_tail, 1u);
