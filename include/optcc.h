@@ -33,7 +33,8 @@ enum { OPTCC_F32 = 0, OPTCC_BF16 = 1 };
 enum {
   OPTCC_OK = 0,
   OPTCC_EINVAL = 1,       /* arguments violate PLAN_SPEC 1 (p<3 PAPER.md:68, g does not divide p, ell<1, ...) */
-  OPTCC_EUNSUPPORTED = 2, /* g>1 with m!=1 (PAPER.md:943 gives no construction); p>128 for masks */
+  OPTCC_EUNSUPPORTED = 2, /* g>1 without a straggler (NCCL's own ring); ordering 1 / ring baseline outside their
+                             scope; p>128 for masks */
   OPTCC_ENOMEM = 3,
   OPTCC_ECUDA = 4,        /* a CUDA runtime call failed; optcc_last_cuda_error() has the code */
   OPTCC_EVERIFY = 5       /* contributor-mask verification found a wrong element */
@@ -44,7 +45,7 @@ enum { OPTCC_OP_REDUCE = 0, OPTCC_OP_COPY = 1 };
 enum { OPTCC_S1 = 0, OPTCC_S2, OPTCC_S3, OPTCC_S4, OPTCC_BUB_UP, OPTCC_BUB_DOWN, OPTCC_N_COLLECT, OPTCC_N_DISTRIBUTE };
 enum { OPTCC_LINK_NIC = 0, OPTCC_LINK_NVLINK = 1 };
 /* constructions (PLAN_SPEC 4): C0 plain ring, C1 one straggler (4.1-4.2, App. C),
- * C2 m>=2 stragglers (App. D), C3 g>1 with one straggler server (App. E) */
+ * C2 m>=2 stragglers (App. D), C3 g>1 with one straggler server (App. E) or several (composition, E.5 :943) */
 enum { OPTCC_C0 = 0, OPTCC_C1 = 1, OPTCC_C2 = 2, OPTCC_C3 = 3 };
 /* schedules (PLAN_SPEC 1 option `schedule`): the baseline runs in the same executor and cost model */
 enum {

@@ -194,3 +194,13 @@ def T_ring_degraded(p, ells, n=1):
     """Plain ring on the degraded topology (the ICCL comparison point, :199, :217) under the bandwidth model: every
     one of the 2(p-1) ring steps moves n/p elements over every link and waits for the slowest one: max(l) T0."""
     return max([_fr(l) for l in ells] + [Fr(1)]) * T0(p, n)
+
+
+def T_multigpu_multi_composed(p, g, ells, k, n):
+    """m >= 2 straggler servers with g GPUs each: NOT from the paper (E.5 :943 omits it).  Composition of D.3's body
+    max{2(q-1), l_1(q-m) + 2(m-1)} s (:805) on the n/g elements of one leader cycle with E.4's body count k + 5.5
+    (:916); an upper-bound form for the canonical composed plan, checked against the event simulation only."""
+    ls = [_fr(l) for l in ells]
+    m, q = len(ls), p // g
+    body = max(Fr(2 * (q - 1)), max(ls) * (q - m) + 2 * (m - 1)) / (q - m)
+    return Fr(n, g) * body * Fr(2 * k + 11, 2 * k)

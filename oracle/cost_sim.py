@@ -58,6 +58,10 @@ def lower_bounds(plan):
     if plan.m == 0:
         t0 = cf.T0(p, n, g)
         return {"table1": t0, "tight": t0}
+    if g > 1 and plan.m > 1:
+        # E.5 (:943) gives no bound for several straggler servers; every single-straggler bound stays valid (making the
+        # other stragglers healthy cannot slow the AllReduce down), so the largest Theorem-3 value is a lower bound
+        return {"table1": max(cf.lb_thm3(p, g, l, n) for l in ells), "tight": None}
     if g > 1:
         return {"table1": cf.lb_thm3(p, g, ells[0], n), "tight": cf.lb_thm13(p, g, ells[0], n)}
     if plan.m == 1:
@@ -74,6 +78,8 @@ def paper_closed_form(plan):
         return cf.T_ring_degraded(p, ells, n)
     if plan.m == 0:
         return cf.T0(p, n, g)
+    if g > 1 and plan.m > 1:
+        return cf.T_multigpu_multi_composed(p, g, ells, k, n)
     if g > 1:
         return cf.T_multigpu_bound(p, g, ells[0], k, n)
     if plan.m == 1 and getattr(plan, "ordering", 2) == 1:

@@ -82,8 +82,8 @@ def classify(p, g, ell):
     healthy = [v for v in range(q) if not ell[v * g] > 1.0]
     if len(healthy) < 2:
         raise PlanError("EINVAL", "at least two healthy servers required")
-    if g > 1 and len(stragglers) != 1:
-        raise PlanError("EUNSUPPORTED", "g > 1 needs exactly one straggler server (E.5 :943)")
+    if g > 1 and len(stragglers) == 0:
+        raise PlanError("EUNSUPPORTED", "g > 1 without a straggler is NCCL's multi-channel ring (:88), a comparison system")
     return q, stragglers, healthy
 
 
@@ -209,8 +209,8 @@ def build_plan(p, g, ell, n, dtype, k=0, _u_p2p_override=None, schedule=OPTCC, o
         nstr = m                       # stragglers seen by the NIC schedule
         P = H + nstr - 1               # windows per body: H (C1/C3) or p-1 (C2, :788)
         if construction == C3:
-            D = 1 + -(-(g - 2) // H)
-            n_steps = (k + D + 2) * H + g - 2
+            D = 1 + -(-(g - 2) // P)
+            n_steps = (k + D + 2) * P + g - 2
         else:
             D = 0
             n_steps = (k + 1) * P
@@ -253,10 +253,10 @@ def build_plan(p, g, ell, n, dtype, k=0, _u_p2p_override=None, schedule=OPTCC, o
                             rng = sec_units(lam, b, c)
                             for h in range(g - 1):
                                 # collect on the backward local ring, leader only receives (:862, :875, :894)
-                                emit(b * H + c + h, REDUCE, N_COLLECT, NVLINK, lam,
+                                emit(b * P + c + h, REDUCE, N_COLLECT, NVLINK, lam,
                                      v * g + (lam - 1 - h) % g, v * g + (lam - 2 - h) % g, b, c, rng)
                                 # distribute on the forward local ring, leader sends first (:863, :876, :894)
-                                emit((b + D + 2) * H + c + h, COPY, N_DISTRIBUTE, NVLINK, lam,
+                                emit((b + D + 2) * P + c + h, COPY, N_DISTRIBUTE, NVLINK, lam,
                                      v * g + (lam + h) % g, v * g + (lam + h + 1) % g, b, c, rng)
 
     arr = np.array(flows, dtype=FLOW_DTYPE) if flows else np.zeros(0, dtype=FLOW_DTYPE)

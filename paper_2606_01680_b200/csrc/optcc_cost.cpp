@@ -85,7 +85,24 @@ extern "C" int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* p
     c.lb_table1_thm = 0; c.lb_tight_thm = 0; c.regime = 0;
   } else {
     const double l1 = plan->ell[r_str];
-    if (in.construction == OPTCC_C3) {
+    if (in.construction == OPTCC_C3 && m > 1) {
+      // several straggler servers with g GPUs each: E.5 (:943) gives neither bound nor time.  Every single-straggler
+      // Theorem-3 bound stays valid (making the other stragglers healthy cannot slow the AllReduce down); the time form
+      // composes D.3's body (:805) on n/g elements with E.4's body count k + 5.5 (:916) -- ours, not the paper's.
+      const double Q = double(q), M = double(m);
+      double lb = 0.0;
+      for (uint32_t v : plan->stragglers) {
+        const double l = plan->ell[v * g];
+        lb = std::max(lb, beta * (n / g) * std::max(2.0 * l * (Q - 1.0) / (1.0 + l * (Q - 1.0)), l));
+      }
+      c.lb_table1 = lb;
+      c.lb_tight = nan;
+      c.lb_table1_thm = 3; c.lb_tight_thm = 0;
+      const double ring_body = 2.0 * (Q - 1.0), str_body = l1 * (Q - M) + 2.0 * (M - 1.0);
+      c.T_limit = beta * (n / g) * std::max(ring_body, str_body) / (Q - M);
+      c.T_closed_form = c.T_limit * (double(k) + 5.5) / double(k);
+      c.regime = str_body > ring_body ? 2 : 1;
+    } else if (in.construction == OPTCC_C3) {
       const double Q = double(q);
       c.lb_table1 = beta * (n / g) * std::max(2.0 * l1 * (Q - 1.0) / (1.0 + l1 * (Q - 1.0)), l1);   // Thm 3 (:112, :538)
       c.lb_tight = beta * (n / g) * std::max(2.0 * l1 * (Q - 1.0) / (l1 * (Q - 2.0) + 2.0), l1);     // Thm 13 (:664)

@@ -157,7 +157,7 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
   std::stable_sort(stragglers.begin(), stragglers.end(),
                    [&](uint32_t a, uint32_t b) { return ell[a * g] > ell[b * g]; });  // l1 >= l2 >= ... (:78)
   if (healthy.size() < 2) return OPTCC_EINVAL;
-  if (g > 1 && stragglers.size() != 1) return OPTCC_EUNSUPPORTED;  // E.5 (:943); all-healthy g>1 is NCCL's ring (:88)
+  if (g > 1 && stragglers.empty()) return OPTCC_EUNSUPPORTED;      // all-healthy g>1 is NCCL's multi-channel ring (:88)
   if (g > 255) return OPTCC_EUNSUPPORTED;                           // `part` is a byte
   const uint32_t ordering = (opts && opts->ordering) ? opts->ordering : 2;   // 0 = default = ordering (2)
   if (ordering != 1 && ordering != 2) return OPTCC_EINVAL;                   // the two valid orderings of :138
@@ -273,8 +273,8 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
       const uint32_t P = H + m - 1;  // windows per body: H for C1/C3, p-1 for C2 (:788)
       uint32_t D = 0;
       if (construction == OPTCC_C3) {
-        D = 1 + (uint32_t)((g - 2 + H - 1) / H);  // NIC body of segment b is body b + D (PLAN_SPEC C3)
-        n_steps = (k + D + 2) * H + g - 2;
+        D = 1 + (uint32_t)((g - 2 + P - 1) / P);  // NIC body of segment b is body b + D (PLAN_SPEC C3)
+        n_steps = (k + D + 2) * P + g - 2;
       } else {
         n_steps = (k + 1) * P;
       }
@@ -315,10 +315,10 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
               for (uint32_t c = 0; c < H; ++c)
                 for (int h = 0; h + 1 < g; ++h) {
                   // N1/N3 collect on the backward local ring, the leader only receives (:862, :875, :894)
-                  B.emit_sec(b * H + c + h, OPTCC_OP_REDUCE, OPTCC_N_COLLECT, OPTCC_LINK_NVLINK, lam,
+                  B.emit_sec(b * P + c + h, OPTCC_OP_REDUCE, OPTCC_N_COLLECT, OPTCC_LINK_NVLINK, lam,
                              v * g + modH(lam - 1 - h, g), v * g + modH(lam - 2 - h, g), b, c);
                   // N2/N4 distribute on the forward local ring, the leader sends first (:863, :876, :894)
-                  B.emit_sec((b + D + 2) * H + c + h, OPTCC_OP_COPY, OPTCC_N_DISTRIBUTE, OPTCC_LINK_NVLINK, lam,
+                  B.emit_sec((b + D + 2) * P + c + h, OPTCC_OP_COPY, OPTCC_N_DISTRIBUTE, OPTCC_LINK_NVLINK, lam,
                              v * g + modH(lam + h, g), v * g + modH(lam + h + 1, g), b, c);
                 }
         }
@@ -445,7 +445,7 @@ extern "C" const char* optcc_strerror(int code) {
   switch (code) {
     case OPTCC_OK: return "ok";
     case OPTCC_EINVAL: return "invalid argument (PLAN_SPEC 1)";
-    case OPTCC_EUNSUPPORTED: return "unsupported configuration (g>1 needs exactly one straggler server, PAPER.md:943; masks need p<=128)";
+    case OPTCC_EUNSUPPORTED: return "unsupported configuration (g>1 needs a straggler server; ordering 1 and the ring baseline need g=1; masks need p<=128)";
     case OPTCC_ENOMEM: return "out of host memory";
     case OPTCC_ECUDA: return "CUDA runtime error (see optcc_last_cuda_error)";
     case OPTCC_EVERIFY: return "contributor-mask verification failed";

@@ -77,6 +77,8 @@ GRID = [
     (12, 2, {0: 1.5, 1: 1.5}, 4097, 1, 12), (32, 1, {0: 2.0 - 1.0 / 31.0}, 1 << 20, 0, 20), (32, 1, {31: 3.0}, 999983, 1, 0),
     (9, 3, {3: 8.0 / 7.0, 4: 8.0 / 7.0, 5: 8.0 / 7.0}, 30011, 0, 8), (6, 1, {1: 1.0 + 2 ** -40}, 5000, 0, 4),
     (64, 1, {5: 8.0 / 7.0, 17: 4.0 / 3.0, 40: 2.0}, 70001, 1, 4), (40, 8, {r: 2.0 for r in range(8, 16)}, 262147, 0, 8),
+    (12, 2, {0: 2.0, 1: 2.0, 6: 1.5, 7: 1.5}, 30011, 0, 4),          # g > 1 with two straggler servers (composed C3)
+    (32, 4, {**{r: 2.0 for r in range(4, 8)}, **{r: 8.0 / 7.0 for r in range(20, 24)}, **{r: 2.0 for r in range(28, 32)}}, 100003, 1, 8),
 ]
 
 
@@ -95,7 +97,6 @@ def test_tables_equal_oracle_on_grid(p, g, st, n, dtype, k):
     ((4, 1, [2.0, 1.0, 1.0, 1.0], 0, 0, 0), "EINVAL"),        # n > 0
     ((4, 1, [2.0, 1.0, 1.0, 1.0], 10, 0, 6), "EINVAL"),       # k multiple of 4 (:155)
     ((4, 1, [2.0, 1.0, 1.0, 1.0], 10, 7, 0), "EINVAL"),       # dtype
-    ((8, 2, [2.0, 2.0, 1.5, 1.5, 1.0, 1.0, 1.0, 1.0], 10, 0, 0), "EUNSUPPORTED"),  # g>1, m>1 (:943)
     ((8, 2, [1.0] * 8, 10, 0, 0), "EUNSUPPORTED"),
 ])
 def test_error_codes_match_oracle(args, code):

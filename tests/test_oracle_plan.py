@@ -178,8 +178,9 @@ def test_validation_errors():
         P.build_plan(8, 2, [2, 1, 1, 1, 1, 1, 1, 1], 100, P.F32)
     assert e.value.code == "EINVAL"                                  # mixed ell in a server (:274)
     with pytest.raises(P.PlanError) as e:
-        P.build_plan(8, 2, [2, 2, 1.5, 1.5, 1, 1, 1, 1], 100, P.F32)
-    assert e.value.code == "EUNSUPPORTED"                            # E.5 :943
+        P.build_plan(8, 2, [1] * 8, 100, P.F32)
+    assert e.value.code == "EUNSUPPORTED"                            # g > 1 without a straggler: NCCL's own ring (:88)
+    assert P.build_plan(8, 2, [2, 2, 1.5, 1.5, 1, 1, 1, 1], 100, P.F32).construction == P.C3   # E.5 :943: composed plan
     with pytest.raises(P.PlanError):
         P.build_plan(4, 1, [2, 1, 1, 1], 100, P.F32, k=6)            # k multiple of 4 (:155)
     with pytest.raises(P.PlanError):
