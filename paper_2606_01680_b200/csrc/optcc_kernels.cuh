@@ -35,7 +35,8 @@ struct __align__(16) DFlow {      // 32 bytes: what the device needs of an optcc
   unsigned long long len;         // elements
   unsigned short src, dst;
   unsigned char op, ksrc, kdin, kdout;  // op: 0 reduce, 1 copy; k*: 0 rank buffer, 1 fp32 shadow (bf16 plans)
-  unsigned int pad0, pad1;
+  unsigned int flags;             // bit 0: the source range is dead after this flow has read it (see discard_line16)
+  unsigned int pad1;
 };
 static_assert(sizeof(DFlow) == 32, "DFlow must be 32 bytes");
 
@@ -154,6 +155,22 @@ __device__ __forceinline__ void grid_barrier(unsigned long long* ctr, unsigned l
 // Range operations.  All ranges are given in 16-byte vectors [vbeg, vend) relative to the flow's start.
 // =====================================================================================================
 
+// Dead-source discard.  When the planner knows that the next access to a flow's source range is a plain overwrite (the
+// all-gather copy of the final sum), the data is dead once this flow has read it; dropping its lines from L2
+// (discard.global.L2 -> CCTL.RML2) saves the write-back of a partial sum nobody will read again.  A lane discards
+// the 128-byte line that starts at its own vector when the line's other vectors were loaded by the following lanes of
+// the same warp in the same instruction (so every load of the line has completed before the discard is issued).
+__device__ __forceinline__ void discard_line16(const char* addr, unsigned long long v, unsigned long long vend) {
+  // 16-byte vectors: a line is 8 consecutive lanes
+  if ((reinterpret_cast<unsigned long long>(addr) & 127ull) == 0ull && (threadIdx.x & 31u) <= 24u && v + 7 < vend)
+    asm volatile("discard.global.L2 [%0], 128;" ::"l"(addr) : "memory");
+}
+__device__ __forceinline__ void discard_line32(const char* addr, unsigned long long u, unsigned long long uend) {
+  // 32 bytes per lane (fp32 shadow of a bf16 unit): a line is 4 consecutive lanes
+  if ((reinterpret_cast<unsigned long long>(addr) & 127ull) == 0ull && (threadIdx.x & 31u) <= 28u && u + 3 < uend)
+    asm volatile("discard.global.L2 [%0], 128;" ::"l"(addr) : "memory");
+}
+
 // calls f(std::integral_constant<int, rem>) for rem in 1 .. UNROLL-1 (UNROLL <= 8)
 template <int UNROLL, class F>
 __device__ __forceinline__ void remainder_dispatch(unsigned int rem, F&& f) {
@@ -193,7 +210,7 @@ __device__ __forceinline__ void range_copy16(const char* __restrict__ s, char* _
 
 template <int UNROLL, int NT>
 __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* __restrict__ d,
-                                              unsigned long long vbeg, unsigned long long vend, const Pol& pol) {
+                                              unsigned long long vbeg, unsigned long long vend, const Pol& pol, bool dead_src) {
   unsigned long long v = vbeg + threadIdx.x;
   for (; v + (UNROLL - 1) * (unsigned long long)NT < vend; v += UNROLL * (unsigned long long)NT) {
     uint4 a[UNROLL], b[UNROLL];
@@ -204,6 +221,10 @@ __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* 
     }
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, add_f32x4(b[j], a[j]), pol);
+    if (dead_src) {
+#pragma unroll
+      for (int j = 0; j < UNROLL; ++j) discard_line16(s + (v + j * (unsigned long long)NT) * 16, v + j * (unsigned long long)NT, vend);
+    }
   }
   if (v < vend) {   // remainder: one batch of loads, then the adds and stores
     const unsigned int rem = (unsigned int)((vend - v + NT - 1) / NT);
@@ -226,7 +247,7 @@ __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* 
 template <int UNROLL, int EB, int NT>
 __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* __restrict__ d,
                                               unsigned long long vbeg, unsigned long long vend,
-                                              unsigned int& overlaps, const Pol& pol) {
+                                              unsigned int& overlaps, const Pol& pol, bool dead_src) {
   unsigned long long v = vbeg + threadIdx.x;
   auto join = [&](uint4 a, uint4 b) {
     const unsigned int cx = a.x & b.x, cy = a.y & b.y, cz = a.z & b.z, cw = a.w & b.w;   // elements whose sets overlap
@@ -251,6 +272,10 @@ __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* 
     }
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, join(a[j], b[j]), pol);
+    if (dead_src) {
+#pragma unroll
+      for (int j = 0; j < UNROLL; ++j) discard_line16(s + (v + j * (unsigned long long)NT) * 16, v + j * (unsigned long long)NT, vend);
+    }
   }
   if (v < vend) {   // remainder: one batch of loads, then the joins and stores
     const unsigned int rem = (unsigned int)((vend - v + NT - 1) / NT);
@@ -302,7 +327,7 @@ __device__ __forceinline__ void store8(char* base, unsigned long long unit, cons
 template <int KS, int KD, int KO, int NT>
 __device__ __forceinline__ void range_add_bf16(const char* __restrict__ s, const char* __restrict__ din,
                                                char* __restrict__ dout, unsigned long long ubeg,
-                                               unsigned long long uend, const Pol& pol) {
+                                               unsigned long long uend, const Pol& pol, bool dead_src) {
   constexpr int UNROLL = 2;
   unsigned long long u = ubeg + threadIdx.x;
   for (; u + (UNROLL - 1) * (unsigned long long)NT < uend; u += UNROLL * (unsigned long long)NT) {
@@ -317,6 +342,13 @@ __device__ __forceinline__ void range_add_bf16(const char* __restrict__ s, const
 #pragma unroll
       for (int e = 0; e < 8; ++e) b[j][e] = __fadd_rn(b[j][e], a[j][e]);
       store8<KO>(dout, u + j * (unsigned long long)NT, b[j], pol);
+    }
+    if (dead_src) {
+#pragma unroll
+      for (int j = 0; j < UNROLL; ++j) {
+        const unsigned long long uu = u + j * (unsigned long long)NT;
+        if (KS == 0) discard_line16(s + uu * 16, uu, uend); else discard_line32(s + uu * 32, uu, uend);
+      }
     }
   }
   for (; u < uend; u += NT) {
