@@ -221,7 +221,8 @@ __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* 
     }
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, add_f32x4(b[j], a[j]), pol);
-    if (dead_src) {
+    // (only when every lane of the warp is in this round: the line's other vectors were loaded by this instruction)
+    if (dead_src && (v - (threadIdx.x & 31u) + 31) + (UNROLL - 1) * (unsigned long long)NT < vend) {
 #pragma unroll
       for (int j = 0; j < UNROLL; ++j) discard_line16(s + (v + j * (unsigned long long)NT) * 16, v + j * (unsigned long long)NT, vend);
     }
@@ -272,7 +273,8 @@ __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* 
     }
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, join(a[j], b[j]), pol);
-    if (dead_src) {
+    // (only when every lane of the warp is in this round: the line's other vectors were loaded by this instruction)
+    if (dead_src && (v - (threadIdx.x & 31u) + 31) + (UNROLL - 1) * (unsigned long long)NT < vend) {
 #pragma unroll
       for (int j = 0; j < UNROLL; ++j) discard_line16(s + (v + j * (unsigned long long)NT) * 16, v + j * (unsigned long long)NT, vend);
     }
@@ -343,7 +345,7 @@ __device__ __forceinline__ void range_add_bf16(const char* __restrict__ s, const
       for (int e = 0; e < 8; ++e) b[j][e] = __fadd_rn(b[j][e], a[j][e]);
       store8<KO>(dout, u + j * (unsigned long long)NT, b[j], pol);
     }
-    if (dead_src) {
+    if (dead_src && (u - (threadIdx.x & 31u) + 31) + (UNROLL - 1) * (unsigned long long)NT < uend) {
 #pragma unroll
       for (int j = 0; j < UNROLL; ++j) {
         const unsigned long long uu = u + j * (unsigned long long)NT;

@@ -303,3 +303,27 @@ def test_two_plans_alternate_on_one_workspace():
         y = sa.download()
         oplan = OP.build_plan(w.p, 1, list(w.ell), w.n, w.dtype, k=plan.info["k"])
         assert y.tobytes() == OI.run_f32(oplan, x).tobytes()
+
+
+@pytest.mark.parametrize("dtype", [W.F32, W.BF16])
+@pytest.mark.parametrize("sec_units", [3584 * 2 + 1561, 3584 + 217, 448 * 4 + 100, 3584 * 3])
+def test_partial_last_tiles_with_divergent_warps(sec_units, dtype):
+    """Geometry of the full-size configs at small scale: sections of several 3584-unit tiles plus a partial last tile
+    whose last streaming round is entered by only some lanes of a warp (the others take the remainder path).  The
+    dead-source discard must not drop a line whose other vectors are loaded by a later instruction: outputs and masks
+    are compared with the oracle bit for bit."""
+    p, k = 5, 4
+    A = 4 if dtype == W.F32 else 8
+    n = (p - 1) * k * sec_units * A
+    w = _wl(p, 1, {0: 2.0}, n, dtype, seed=77)
+    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=k, exec_mode=B.OPTCC_EXEC_DATAFLOW, tile_units=3584)
+    oplan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=k)
+    x = W.all_inputs(w)
+    s = _session(plan, verify=True)
+    s.upload(x)
+    s.execute()
+    y = s.download()
+    y_or = OI.run_f32(oplan, x) if dtype == W.F32 else OI.run_bf16(oplan, x)
+    assert y.tobytes() == y_or.tobytes()
+    res = s.verify()
+    assert res["bad_elements"] == 0 and res["overlap_elements"] == 0
