@@ -48,6 +48,17 @@ def _check_full(w, k, exec_mode, n_samples=2048):
         y_or = OI.run_bf16_at(oplan, xs, idx)
         assert ys[0].tobytes() == y_or[0].tobytes() and ys[1].tobytes() == y_or[w.p - 1].tobytes()
         assert OR.check_bf16(OI.bf16_bits_to_f32(ys[0]), OI.bf16_bits_to_f32(xs)).all()
+    if exec_mode == B.OPTCC_EXEC_DATAFLOW:
+        # every element of every rank, device against device: the per-step executor (kernel boundaries as barriers, no
+        # dependency counters, no dead-source discard) must produce the same bits as the dataflow executor
+        plan2 = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=k, exec_mode=B.OPTCC_EXEC_PER_STEP)
+        s2 = Session(plan2)
+        s2.upload(x)
+        s2.execute()
+        torch.cuda.synchronize()
+        for r in (0, w.p // 2, w.p - 1):
+            assert torch.equal(s.bufs[r].view(it), s2.bufs[r].view(it)), f"executors disagree on rank {r}"
+        del s2
     del x
     res = s.verify()
     assert res["bad_elements"] == 0 and res["overlap_elements"] == 0 and res["checked"] == w.p * w.n
