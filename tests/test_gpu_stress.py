@@ -57,3 +57,34 @@ def test_dataflow_random_plans(seed):
         assert y.tobytes() == y_or.tobytes()
     res = s.verify()
     assert res["bad_elements"] == 0 and res["overlap_elements"] == 0
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_dataflow_random_midsize_plans(seed):
+    """Mid-size plans (sections of several thousand 16-byte units, odd tile sizes): the full streaming rounds, the
+    partially entered last rounds, the remainder batches and the dead-source discard all occur; outputs bit-equal to
+    the oracle, masks complete, and the per-step executor agrees on every element."""
+    from paper_2606_01680_b200.device import Session
+    rng = np.random.default_rng(7000 + seed)
+    p = int(rng.integers(3, 10))
+    st = {int(rng.integers(0, p)): float(rng.choice([8 / 7, 1.5, 2.0, 3.0]))}
+    if seed % 4 == 3 and p >= 6:
+        st[int((list(st)[0] + 2) % p)] = 4.0 / 3.0
+    ell = [float(st.get(i, 1.0)) for i in range(p)]
+    dtype = int(rng.integers(0, 2))
+    n = int(rng.integers(300_000, 1_500_000))
+    k = int(rng.choice([4, 8]))
+    tile = int(rng.choice([0, 1792, 3584, 1000, 5000, 3583]))
+    plan = B.optcc_plan(p, 1, ell, n, dtype, k=k, exec_mode=B.OPTCC_EXEC_DATAFLOW, tile_units=tile)
+    oplan = OP.build_plan(p, 1, ell, n, dtype, k=k)
+    w = W.Workload("mid", p, 1, tuple(ell), n, dtype, "normal", 1.0, 9000 + seed)
+    x = W.all_inputs(w)
+    s = Session(plan, verify=True)
+    s.upload(x)
+    s.execute()
+    y = s.download()
+    y_or = OI.run_f32(oplan, x) if dtype == W.F32 else OI.run_bf16(oplan, x)
+    assert y.tobytes() == y_or.tobytes()
+    res = s.verify()
+    assert res["bad_elements"] == 0 and res["overlap_elements"] == 0
+    assert s.masks().tobytes() == OI.element_masks(oplan)[0].tobytes()
