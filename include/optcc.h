@@ -92,6 +92,8 @@ typedef struct optcc_opts {
   uint32_t schedule;  /* OPTCC_SCHED_*: 0 = OPTCC (default), 1 = plain ring on the degraded topology (baseline) */
   uint32_t ordering;  /* stage ordering of PAPER.md:138 for one straggler, g = 1: 0 or 2 = ordering (2) S3->S1->S4->S2 (the
                          canonical plan, k+1 bodies), 1 = ordering (1) S1->S2->S3->S4 (PLAN_SPEC C1', k+3 bodies) */
+  uint32_t no_discard;/* 1 = keep dead source lines in L2 (disables the discard.global.L2 optimisation; for bisecting) */
+  uint32_t reserved;  /* 0 */
 } optcc_opts_t;
 
 typedef struct optcc_plan_info {

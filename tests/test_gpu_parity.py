@@ -327,3 +327,15 @@ def test_partial_last_tiles_with_divergent_warps(sec_units, dtype):
     assert y.tobytes() == y_or.tobytes()
     res = s.verify()
     assert res["bad_elements"] == 0 and res["overlap_elements"] == 0
+
+
+def test_discard_can_be_disabled_and_changes_nothing():
+    w = _wl(8, 1, {0: 2.0}, 4 * 7 * 4 * (3584 + 300), W.F32, seed=13)
+    outs = []
+    for nd in (0, 1):
+        plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=4, exec_mode=B.OPTCC_EXEC_DATAFLOW, tile_units=3584, no_discard=nd)
+        s = _session(plan)
+        s.upload(W.all_inputs(w))
+        s.execute()
+        outs.append(s.download().tobytes())
+    assert outs[0] == outs[1]
