@@ -617,7 +617,8 @@ void build_dataflow_tables(optcc_plan_t* pl, optcc_exec_state* st) {
     const size_t reg = size_t(std::lower_bound(pl->region_offs.begin(), pl->region_offs.end(), f.off) - pl->region_offs.begin());
     const size_t ls = size_t(f.src) * nr + reg, ld = size_t(f.dst) * nr + reg;
     // (first and last reader since the last write = the only one: no other flow may still be reading the range)
-    st->dflows[i].flags = (!pl->opts.no_discard && f.op == OPTCC_OP_REDUCE && next[ls] == NEXT_COPY_WRITE && sole_reader[i]) ? 1u : 0u;
+    // (not for truncated schedules, step_limit: the overwrite that makes the range dead might never run)
+    st->dflows[i].flags = (!pl->opts.no_discard && !pl->opts.step_limit && f.op == OPTCC_OP_REDUCE && next[ls] == NEXT_COPY_WRITE && sole_reader[i]) ? 1u : 0u;
     next[ld] = f.op == OPTCC_OP_COPY ? NEXT_COPY_WRITE : NEXT_REDUCE_WRITE;
     next[ls] = NEXT_READ;
   }
