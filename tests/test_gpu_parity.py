@@ -339,3 +339,19 @@ def test_discard_can_be_disabled_and_changes_nothing():
         s.execute()
         outs.append(s.download().tobytes())
     assert outs[0] == outs[1]
+
+
+def test_truncated_schedule_midsize_masks_equal_oracle():
+    """A truncated schedule at a size where full streaming rounds run: the masks must still equal the oracle's for
+    the same truncated table (so nothing may be dropped from L2 on the assumption that a later step overwrites it)."""
+    import dataclasses
+    p, k, limit = 5, 4, 9
+    n = 4 * (p - 1) * k * (3584 + 300)
+    ell = [1.0, 1.0, 2.0, 1.0, 1.0]
+    plan = B.optcc_plan(p, 1, ell, n, W.F32, k=k, exec_mode=B.OPTCC_EXEC_DATAFLOW, step_limit=limit, tile_units=3584)
+    oplan = OP.build_plan(p, 1, ell, n, W.F32, k=k)
+    s = _session(plan, verify=True)
+    res = s.verify(raise_on_fail=False)
+    m_or, _ = OI.element_masks(dataclasses.replace(oplan, n_steps=limit))
+    assert s.masks().tobytes() == m_or.tobytes()
+    assert res["bad_elements"] == int((m_or != OI.full_mask_words(p)[None, None, :]).any(axis=2).sum()) > 0
