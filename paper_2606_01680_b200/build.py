@@ -39,7 +39,7 @@ def build(force=False, verbose=False):
         return LIB
     cmd = [_nvcc(), "-shared", "-o", LIB, "-std=c++17", "-O3", "-lineinfo",
            "-gencode", "arch=compute_100a,code=sm_100a",
-           "-Xcompiler", "-fPIC,-ffp-contract=off,-fvisibility=hidden,-Wall",
+           "-Xcompiler", "-fPIC,-pthread,-ffp-contract=off,-fvisibility=hidden,-Wall",
            "-I", os.path.join(ROOT, "include"), "-I", CSRC]
     if verbose:
         cmd += ["-Xptxas", "-v"]

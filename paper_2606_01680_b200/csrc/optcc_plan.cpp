@@ -8,6 +8,8 @@
 #include <chrono>
 #include <cmath>
 #include <cstring>
+#include <atomic>
+#include <thread>
 #include <new>
 
 #include "optcc_internal.h"
@@ -70,8 +72,25 @@ bool flow_less(const optcc_flow_t& a, const optcc_flow_t& b) {
   return a.off < b.off;
 }
 
+// Run body(i) for i in [0, n) on a few host threads when the table is large enough to pay for them; the
+// iterations are independent (each sorts or moves a disjoint range).
+template <class F>
+void parallel_chunks(size_t n, size_t work, F body) {
+  unsigned hw = std::thread::hardware_concurrency();
+  unsigned nt = work < (size_t(1) << 17) ? 1u : std::min(8u, hw ? hw : 1u);
+  if (nt <= 1 || n <= 1) { for (size_t i = 0; i < n; ++i) body(i); return; }
+  std::atomic<size_t> next{0};
+  auto worker = [&]() { for (size_t i; (i = next.fetch_add(1, std::memory_order_relaxed)) < n;) body(i); };
+  std::vector<std::thread> th;
+  th.reserve(nt - 1);
+  for (unsigned t = 1; t < nt; ++t) th.emplace_back(worker);
+  worker();
+  for (auto& t : th) t.join();
+}
+
 // PLAN_SPEC 3 order (step, link, stage, src, dst, off): counting sort by step, then each step's few flows by a
 // packed key -- the table has O(p k H) records, a comparison sort of whole records dominated the build time.
+// The per-step sorts and the final gather touch disjoint ranges and are split over host threads.
 void sort_flows(std::vector<optcc_flow_t>& flows, uint32_t n_steps) {
   struct Key { uint64_t hi, lo; uint32_t idx; };
   const size_t nf = flows.size();
@@ -90,11 +109,12 @@ void sort_flows(std::vector<optcc_flow_t>& flows, uint32_t n_steps) {
       keys[pos[f.step]++] = k;
     }
   }
-  for (size_t t = 0; t <= n_steps; ++t)
+  std::vector<optcc_flow_t> out(nf);
+  parallel_chunks(size_t(n_steps) + 1, nf, [&](size_t t) {
     std::sort(keys.begin() + begin[t], keys.begin() + begin[t + 1],
               [](const Key& a, const Key& b) { return a.hi != b.hi ? a.hi < b.hi : a.lo < b.lo; });
-  std::vector<optcc_flow_t> out(nf);
-  for (size_t i = 0; i < nf; ++i) out[i] = flows[keys[i].idx];
+    for (size_t i = begin[t]; i < begin[t + 1]; ++i) out[i] = flows[keys[i].idx];
+  });
   flows.swap(out);
 }
 
