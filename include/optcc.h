@@ -93,7 +93,9 @@ typedef struct optcc_opts {
   uint32_t ordering;  /* stage ordering of PAPER.md:138 for one straggler, g = 1: 0 or 2 = ordering (2) S3->S1->S4->S2 (the
                          canonical plan, k+1 bodies), 1 = ordering (1) S1->S2->S3->S4 (PLAN_SPEC C1', k+3 bodies) */
   uint32_t no_discard;/* 1 = keep dead source lines in L2 (disables the discard.global.L2 optimisation; for bisecting) */
-  uint32_t reserved;  /* 0 */
+  uint32_t verify_eager; /* 1 = optcc_verify initialises the mask arrays and checks them with separate passes even when
+                            the plan allows the lazy form (initial masks as constants, final masks checked by their last
+                            writer); same result, for bisecting.  Truncated plans (step_limit) are always eager. */
 } optcc_opts_t;
 
 typedef struct optcc_plan_info {
@@ -119,6 +121,11 @@ typedef struct optcc_plan_info {
                                   workspace + mask_offset_bytes + (r*padded_n + e)*mask_bytes, little endian, bit i = rank i */
   uint64_t padded_n;           /* n rounded up to a multiple of 8: per-rank stride of masks and fp32 partials */
   double   plan_build_seconds; /* wall time optcc_plan spent ("< 1 ms at p=1024") */
+  uint32_t lazy_verify;        /* 1: the executed steps write every (rank, section) at least once, so optcc_verify keeps
+                                  the initial masks {r} as constants and lets the last writer of every range check the
+                                  final mask (no initialising / checking pass over the arrays); 0: separate passes
+                                  (some range keeps its initial mask, opts.verify_eager, or p > 128) */
+  uint32_t reserved;           /* 0 */
 } optcc_plan_info_t;
 
 typedef struct optcc_cost_params {

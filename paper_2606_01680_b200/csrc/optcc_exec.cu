@@ -78,22 +78,43 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
     constexpr int EB = MT::ESIZE;
     const char* s = rank_ptr(P, f.src) + f.off * EB;
     char* d = rank_ptr(P, f.dst) + f.off * EB;
-    if (f.op == 0) range_or_mask<4, EB, NT>(s, d, vbeg, vend, overlaps, pol, dead_src); else range_copy16<4, NT>(s, d, vbeg, vend, pol);
+    const unsigned int lazy = f.flags & (DFLOW_SRC_INIT | DFLOW_DST_INIT | DFLOW_FINAL);
+    const unsigned long long full0 = P.n_ranks >= 64 ? ~0ull : ((1ull << P.n_ranks) - 1ull);
+    if (lazy) {   // lazy verifier: initial masks are constants, the last writer checks the final mask (range_mask_lazy)
+      const unsigned long long full1 = P.n_ranks > 64 ? (P.n_ranks >= 128 ? ~0ull : ((1ull << (P.n_ranks - 64)) - 1ull)) : 0ull;
+      const uint4 SC = mask_vector(f.src < 64 ? 1ull << f.src : 0ull, f.src >= 64 ? 1ull << (f.src - 64) : 0ull, EB);
+      const uint4 DC = mask_vector(f.dst < 64 ? 1ull << f.dst : 0ull, f.dst >= 64 ? 1ull << (f.dst - 64) : 0ull, EB);
+      range_mask_lazy<4, EB, NT>(s, d, vbeg, vend, overlaps, pol, f.flags, f.op == 0, SC, DC, mask_vector(full0, full1, EB),
+                                 P.ctrl, (unsigned long long)f.dst * P.n + f.off);
+    } else if (f.op == 0) {
+      range_or_mask<4, EB, NT>(s, d, vbeg, vend, overlaps, pol, dead_src);
+    } else {
+      range_copy16<4, NT>(s, d, vbeg, vend, pol);
+    }
     if (threadIdx.x < tail) {  // ragged end (n not a multiple of the elements per vector): one element per thread
-      const unsigned long long e = vend * MT::VE + threadIdx.x;
+      const unsigned long long e = vend * MT::VE + threadIdx.x;   // (EB <= 8 here: a 16-byte mask is a whole vector)
       unsigned long long x, y = 0;
-      if (EB == 2) {
+      if (lazy & DFLOW_SRC_INIT) {
+        x = 1ull << f.src;
+      } else if (EB == 2) {
         x = __ldcg(reinterpret_cast<const unsigned short*>(s) + e);
-        if (f.op == 0) y = __ldcg(reinterpret_cast<const unsigned short*>(d) + e);
       } else if (EB == 4) {
         x = __ldcg(reinterpret_cast<const unsigned int*>(s) + e);
-        if (f.op == 0) y = __ldcg(reinterpret_cast<const unsigned int*>(d) + e);
       } else {
         x = __ldcg(reinterpret_cast<const unsigned long long*>(s) + e);
-        if (f.op == 0) y = __ldcg(reinterpret_cast<const unsigned long long*>(d) + e);
+      }
+      if (f.op == 0) {
+        if (lazy & DFLOW_DST_INIT) y = 1ull << f.dst;
+        else if (EB == 2) y = __ldcg(reinterpret_cast<const unsigned short*>(d) + e);
+        else if (EB == 4) y = __ldcg(reinterpret_cast<const unsigned int*>(d) + e);
+        else y = __ldcg(reinterpret_cast<const unsigned long long*>(d) + e);
       }
       overlaps += (x & y) != 0ull;
       x |= y;
+      if ((lazy & DFLOW_FINAL) && x != full0) {
+        atomicAdd(&P.ctrl->bad, 1ull);
+        atomicMin(&P.ctrl->first_bad, (unsigned long long)f.dst * P.n + f.off + e);
+      }
       if (EB == 2) __stcg(reinterpret_cast<unsigned short*>(d) + e, (unsigned short)x);
       else if (EB == 4) __stcg(reinterpret_cast<unsigned int*>(d) + e, (unsigned int)x);
       else __stcg(reinterpret_cast<unsigned long long*>(d) + e, x);
@@ -457,14 +478,6 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
   }
 }
 
-// A 16-byte vector of masks, every element = `bits` (the low EB*8 bits of a 128-bit value given as lo, hi)
-__device__ __forceinline__ uint4 mask_vector(unsigned long long lo, unsigned long long hi, unsigned int eb) {
-  if (eb == 2) { const unsigned int w = (unsigned int)(lo & 0xFFFFull) * 0x10001u; return make_uint4(w, w, w, w); }
-  if (eb == 4) { const unsigned int w = (unsigned int)lo; return make_uint4(w, w, w, w); }
-  if (eb == 8) return make_uint4((unsigned int)lo, (unsigned int)(lo >> 32), (unsigned int)lo, (unsigned int)(lo >> 32));
-  return make_uint4((unsigned int)lo, (unsigned int)(lo >> 32), (unsigned int)hi, (unsigned int)(hi >> 32));
-}
-
 // masks[r][e] = {r}: blockIdx.y = rank, 16-byte stores over the rank's padded array; eb = bytes per mask
 __global__ void __launch_bounds__(256) optcc_mask_init_kernel(char* masks, unsigned long long padded_n, unsigned int eb) {
   const unsigned int r = blockIdx.y;
@@ -549,6 +562,7 @@ struct optcc_exec_state {
   uint32_t G_df = 0;              // grid of the dataflow kernel
   bool df_ok = false;             // counters fit 32-bit indices
   bool big_ops = false;           // average tile-op >= 1792 units (decides the ring depth)
+  bool lazy_masks = false;        // the verifier needs no init / check passes (see assign_mask_flags)
   std::vector<DDep> deps;         // [n_flows]
   std::vector<TileOp> ops;        // [n_tile_ops], table order
   std::vector<uint64_t> step_op_begin;   // [n_steps + 1]
@@ -622,6 +636,37 @@ void build_dataflow_tables(optcc_plan_t* pl, optcc_exec_state* st) {
     next[ld] = f.op == OPTCC_OP_COPY ? NEXT_COPY_WRITE : NEXT_REDUCE_WRITE;
     next[ls] = NEXT_READ;
   }
+}
+
+// Lazy verifier (range_mask_lazy; the planner decides, info.lazy_verify): the executed part of the table writes every
+// (rank, region) at least once, so no mask the run reads or leaves behind is one it has not written -- the arrays
+// need no initialising pass and the last writer of every range checks the final mask.  Sets the DFLOW_*_INIT / FINAL
+// bits; otherwise the flags stay clear and optcc_verify initialises and checks the arrays with separate passes.
+void assign_mask_flags(optcc_plan_t* pl, optcc_exec_state* st) {
+  const optcc_plan_info_t& in = pl->info;
+  st->lazy_masks = false;
+  if (!in.lazy_verify) return;
+  const uint32_t steps = pl->opts.step_limit ? std::min(pl->opts.step_limit, in.n_steps) : in.n_steps;
+  const uint32_t nf = pl->step_begin[steps];            // flows of the executed steps
+  const size_t nr = pl->region_offs.size();
+  std::vector<uint8_t> written(size_t(in.p) * nr, 0);
+  std::vector<uint32_t> reg(nf);
+  for (uint32_t i = 0; i < nf; ++i) {                   // forwards: has the range been written before flow i?
+    const optcc_flow_t& f = pl->flows[i];
+    reg[i] = uint32_t(std::lower_bound(pl->region_offs.begin(), pl->region_offs.end(), f.off) - pl->region_offs.begin());
+    uint32_t fl = 0;
+    if (!written[size_t(f.src) * nr + reg[i]]) fl |= DFLOW_SRC_INIT;
+    if (!written[size_t(f.dst) * nr + reg[i]]) fl |= DFLOW_DST_INIT;
+    written[size_t(f.dst) * nr + reg[i]] = 1;
+    st->dflows[i].flags |= fl;
+  }
+  std::fill(written.begin(), written.end(), 0);
+  for (uint32_t i = nf; i-- > 0;) {                     // backwards: is the range written after flow i?
+    const optcc_flow_t& f = pl->flows[i];
+    if (!written[size_t(f.dst) * nr + reg[i]]) st->dflows[i].flags |= DFLOW_FINAL;
+    written[size_t(f.dst) * nr + reg[i]] = 1;
+  }
+  st->lazy_masks = true;
 }
 
 template <int MODE>
@@ -731,6 +776,7 @@ int build_state(optcc_plan_t* pl) {
     // dataflow tables when that executor will run; otherwise the slice table of the barrier executors
     st->df_ok = false;
     if (pl->opts.exec_mode == OPTCC_EXEC_DATAFLOW && st->coop && st->G_df > 0) build_dataflow_tables(pl, st);
+    assign_mask_flags(pl, st);
     // slice table: cut every step into G slices of equal HBM bytes
     st->slices.clear();
     if (!st->df_ok) st->slices.assign(size_t(in.n_steps) * (G + 1), Slice{0, 0, 0});
@@ -835,6 +881,8 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   P.ctrl = reinterpret_cast<Ctrl*>(ws + L.ctrl);
   P.shadow = reinterpret_cast<float*>(ws + L.shadow);
   P.padded_n = pl->info.padded_n;
+  P.n = pl->info.n;
+  P.n_ranks = pl->info.p;
   P.unit_elems = pl->info.unit_elems;
   P.deps = reinterpret_cast<const DDep*>(ws + L.deps);
   P.ops = reinterpret_cast<const TileOp*>(ws + L.ops);
@@ -926,14 +974,24 @@ extern "C" int optcc_verify(optcc_plan_t* plan, void* workspace, void* stream_, 
   const unsigned int bx = (unsigned int)std::max<uint64_t>(1, std::min<uint64_t>((vec_per_rank + 1023) / 1024,
                                                           std::max<uint64_t>(1, uint64_t(plan->exec->sm_count) * 16 / in.p)));
   const dim3 blocks(bx, in.p);
-  optcc_mask_init_kernel<<<blocks, 256, 0, stream>>>(masks, in.padded_n, eb);
-  CU_TRY(cudaGetLastError());
+  const bool lazy = plan->exec->lazy_masks;
+  if (lazy) {
+    // initial masks are constants and the last writer of every range checks the final mask (assign_mask_flags); the
+    // bulk-copy path would move raw memory, so the streaming warps take the copies too
+    P.bulk_copy = 0;
+    P.df_slots = plan->exec->big_ops ? 2 : 4;
+  } else {
+    optcc_mask_init_kernel<<<blocks, 256, 0, stream>>>(masks, in.padded_n, eb);
+    CU_TRY(cudaGetLastError());
+  }
   rc = eb == 2 ? launch_plan<MODE_MASK16>(plan, P, stream)
                : eb == 4 ? launch_plan<MODE_MASK32>(plan, P, stream)
                          : eb == 8 ? launch_plan<MODE_MASK1>(plan, P, stream) : launch_plan<MODE_MASK2>(plan, P, stream);
   if (rc != OPTCC_OK) return rc;
-  optcc_mask_check_kernel<<<blocks, 256, 0, stream>>>(masks, in.p, in.n, in.padded_n, eb, P.ctrl);
-  CU_TRY(cudaGetLastError());
+  if (!lazy) {
+    optcc_mask_check_kernel<<<blocks, 256, 0, stream>>>(masks, in.p, in.n, in.padded_n, eb, P.ctrl);
+    CU_TRY(cudaGetLastError());
+  }
   Ctrl res;
   CU_TRY(cudaMemcpyAsync(&res, P.ctrl, sizeof res, cudaMemcpyDeviceToHost, stream));
   CU_TRY(cudaStreamSynchronize(stream));

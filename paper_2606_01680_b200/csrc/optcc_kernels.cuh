@@ -35,10 +35,17 @@ struct __align__(16) DFlow {      // 32 bytes: what the device needs of an optcc
   unsigned long long len;         // elements
   unsigned short src, dst;
   unsigned char op, ksrc, kdin, kdout;  // op: 0 reduce, 1 copy; k*: 0 rank buffer, 1 fp32 shadow (bf16 plans)
-  unsigned int flags;             // bit 0: the source range is dead after this flow has read it (see discard_line16)
+  unsigned int flags;             // DFLOW_* bits
   unsigned int pad1;
 };
 static_assert(sizeof(DFlow) == 32, "DFlow must be 32 bytes");
+enum : unsigned int {
+  DFLOW_DEAD_SRC = 1u,   // the source range is dead after this flow has read it (see discard_line16)
+  // contributor-mask runs only (lazy verifier, see range_mask_lazy); never set for truncated or eager runs:
+  DFLOW_SRC_INIT = 2u,   // no earlier flow wrote the source range: it holds the initial mask {src}
+  DFLOW_DST_INIT = 4u,   // no earlier flow wrote the destination range: it holds the initial mask {dst}
+  DFLOW_FINAL = 8u,      // no later flow writes the destination range: what this flow writes is the final mask
+};
 
 struct __align__(16) Slice {      // start of a CTA's slice of a step: flow index and 16-byte unit inside it
   unsigned int flow;
@@ -76,6 +83,9 @@ struct ExecParams {
   Ctrl* ctrl;
   float* shadow;                  // bf16 plans: fp32 partials, [p][padded_n]
   unsigned long long padded_n;
+  unsigned long long n;           // elements per rank (index of a wrong final mask = rank * n + element)
+  unsigned int n_ranks;           // p
+  unsigned int pad0;
   unsigned int step_lo, step_hi;  // steps [lo, hi) are executed by this launch
   unsigned int unit_elems;        // A (PLAN_SPEC 2)
   unsigned int use_barrier;       // 1: grid barrier between steps (cooperative launch)
@@ -293,6 +303,100 @@ __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* 
       for (int j = 0; j < KK; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, join(a[j], b[j]), pol);
     };
     remainder_dispatch<UNROLL>(rem, batch);
+  }
+}
+
+// A 16-byte vector of masks, every element = `bits` (the low EB*8 bits of a 128-bit value given as lo, hi)
+__device__ __forceinline__ uint4 mask_vector(unsigned long long lo, unsigned long long hi, unsigned int eb) {
+  if (eb == 2) { const unsigned int w = (unsigned int)(lo & 0xFFFFull) * 0x10001u; return make_uint4(w, w, w, w); }
+  if (eb == 4) { const unsigned int w = (unsigned int)lo; return make_uint4(w, w, w, w); }
+  if (eb == 8) return make_uint4((unsigned int)lo, (unsigned int)(lo >> 32), (unsigned int)lo, (unsigned int)(lo >> 32));
+  return make_uint4((unsigned int)lo, (unsigned int)(lo >> 32), (unsigned int)hi, (unsigned int)(hi >> 32));
+}
+
+// ---- lazy verifier ----------------------------------------------------------------------------------------------
+// The initial mask of rank r is the constant {r}, and the final mask of a range is whatever its last writer stores.
+// When the host has seen that every (rank, region) is written by the table (so nothing depends on memory the run
+// never wrote), the mask arrays need neither an initialising pass nor a checking pass: a flow whose source /
+// destination range has not been written yet takes the constant instead of loading it (DFLOW_SRC_INIT / DST_INIT),
+// and the last writer of a range compares what it stores with the full set (DFLOW_FINAL).  Same sets, same stores.
+
+// a wrong final vector (never on a correct plan): count its wrong elements, keep the smallest index
+template <int EB>
+__device__ __noinline__ void report_bad_masks(unsigned long long* bad_ctr, unsigned long long* first_ctr, uint4 diff,
+                                              unsigned long long g) {
+  const unsigned int d[4] = {diff.x, diff.y, diff.z, diff.w};
+  unsigned long long bad = 0, first = ~0ull;
+#pragma unroll
+  for (unsigned int j = 0; j < 16 / EB; ++j) {
+    bool wrong;
+    if (EB == 2) wrong = ((d[j >> 1] >> ((j & 1u) * 16)) & 0xFFFFu) != 0u;
+    else if (EB == 4) wrong = d[j] != 0u;
+    else if (EB == 8) wrong = (d[2 * j] | d[2 * j + 1]) != 0u;
+    else wrong = true;
+    if (wrong) { ++bad; if (first == ~0ull) first = g + j; }
+  }
+  if (bad) {
+    atomicAdd(bad_ctr, bad);
+    atomicMin(first_ctr, first);
+  }
+}
+
+// SC / DC: the initial vectors of the source / destination rank, F: the full set; g0 = dst * n + f.off (the global
+// index of the flow's first element at its destination); reduce: OR with overlap detection, else assign.
+template <int UNROLL, int EB, int NT>
+__device__ __forceinline__ void range_mask_lazy(const char* __restrict__ s, char* __restrict__ d,
+                                                unsigned long long vbeg, unsigned long long vend, unsigned int& overlaps,
+                                                const Pol& pol, unsigned int flags, bool reduce, uint4 SC, uint4 DC, uint4 F,
+                                                Ctrl* ctrl, unsigned long long g0) {
+  const bool src_init = (flags & DFLOW_SRC_INIT) != 0u, dst_init = (flags & DFLOW_DST_INIT) != 0u;
+  const bool fin = (flags & DFLOW_FINAL) != 0u, dead_src = (flags & DFLOW_DEAD_SRC) != 0u && !src_init;
+  auto join = [&](uint4 a, uint4 b) {
+    const unsigned int cx = a.x & b.x, cy = a.y & b.y, cz = a.z & b.z, cw = a.w & b.w;   // elements whose sets overlap
+    if (EB == 2) {
+      auto hw = [](unsigned int w) { return ((w & 0xFFFFu) != 0u) + ((w >> 16) != 0u); };
+      overlaps += hw(cx) + hw(cy) + hw(cz) + hw(cw);
+    } else if (EB == 4) {
+      overlaps += (cx != 0u) + (cy != 0u) + (cz != 0u) + (cw != 0u);
+    } else if (EB == 8) {
+      overlaps += ((cx | cy) != 0u) + ((cz | cw) != 0u);
+    } else {
+      overlaps += ((cx | cy | cz | cw) != 0u);
+    }
+    return make_uint4(a.x | b.x, a.y | b.y, a.z | b.z, a.w | b.w);
+  };
+  const uint4 Z = make_uint4(0u, 0u, 0u, 0u);
+  auto batch = [&](unsigned long long v, auto K) {
+    constexpr int KK = decltype(K)::value;
+    uint4 a[KK], b[KK];
+#pragma unroll
+    for (int j = 0; j < KK; ++j) {
+      a[j] = src_init ? SC : ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds);
+      b[j] = !reduce ? Z : (dst_init ? DC : ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd));
+    }
+#pragma unroll
+    for (int j = 0; j < KK; ++j) {
+      const uint4 o = join(a[j], b[j]);
+      st16(d + (v + j * (unsigned long long)NT) * 16, o, pol);
+      if (fin) {
+        const uint4 df = make_uint4(o.x ^ F.x, o.y ^ F.y, o.z ^ F.z, o.w ^ F.w);
+        if ((df.x | df.y | df.z | df.w) != 0u)
+          report_bad_masks<EB>(&ctrl->bad, &ctrl->first_bad, df, g0 + (v + j * (unsigned long long)NT) * (16 / EB));
+      }
+    }
+  };
+  unsigned long long v = vbeg + threadIdx.x;
+  for (; v + (UNROLL - 1) * (unsigned long long)NT < vend; v += UNROLL * (unsigned long long)NT) {
+    batch(v, std::integral_constant<int, UNROLL>());
+    // (only when every lane of the warp is in this round: the line's other vectors were loaded by this instruction)
+    if (dead_src && (v - (threadIdx.x & 31u) + 31) + (UNROLL - 1) * (unsigned long long)NT < vend) {
+#pragma unroll
+      for (int j = 0; j < UNROLL; ++j) discard_line16(s + (v + j * (unsigned long long)NT) * 16, v + j * (unsigned long long)NT, vend);
+    }
+  }
+  if (v < vend) {
+    const unsigned int rem = (unsigned int)((vend - v + NT - 1) / NT);
+    remainder_dispatch<UNROLL>(rem, [&](auto K) { batch(v, K); });
   }
 }
 

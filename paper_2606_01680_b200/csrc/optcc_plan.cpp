@@ -425,6 +425,27 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     delete pl;
     return OPTCC_ENOMEM;
   }
+  // lazy verifier (optcc.h, lazy_verify): every (rank, region) is written by a flow of the executed steps
+  try {
+    in.lazy_verify = 0;
+    if (in.mask_bytes && !pl->opts.verify_eager) {
+      const uint32_t steps = pl->opts.step_limit ? std::min(pl->opts.step_limit, n_steps) : n_steps;
+      const size_t nr = pl->region_offs.size();
+      std::vector<uint8_t> written(size_t(p) * nr, 0);
+      size_t left = written.size();
+      for (uint32_t i = 0; i < pl->step_begin[steps]; ++i) {
+        const optcc_flow_t& f = pl->flows[i];
+        const size_t r = size_t(std::lower_bound(pl->region_offs.begin(), pl->region_offs.end(), f.off) - pl->region_offs.begin());
+        uint8_t& w = written[size_t(f.dst) * nr + r];
+        left -= !w;
+        w = 1;
+      }
+      in.lazy_verify = left == 0;
+    }
+  } catch (const std::bad_alloc&) {
+    delete pl;
+    return OPTCC_ENOMEM;
+  }
   optcc_ws_layout L = optcc_layout(pl);
   in.workspace_bytes = L.end_exec;
   in.verify_workspace_bytes = L.end_verify;

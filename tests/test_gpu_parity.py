@@ -149,11 +149,15 @@ MASK_CASES = [
 ]
 
 
+@pytest.mark.parametrize("eager", [0, 1])
 @pytest.mark.parametrize("exec_mode", MODES)
 @pytest.mark.parametrize("p,g,st,n,dtype,k", MASK_CASES)
-def test_verifier_masks_equal_oracle(p, g, st, n, dtype, k, exec_mode):
+def test_verifier_masks_equal_oracle(p, g, st, n, dtype, k, exec_mode, eager):
+    """eager = 0: the lazy verifier (initial masks as constants, final masks checked by their last writer);
+    eager = 1: the mask arrays are initialised and checked by separate passes.  Same masks, same verdict."""
     ell = [float(st.get(i, 1.0)) for i in range(p)]
-    plan = B.optcc_plan(p, g, ell, n, dtype, k=k, exec_mode=exec_mode)
+    plan = B.optcc_plan(p, g, ell, n, dtype, k=k, exec_mode=exec_mode, verify_eager=eager)
+    assert plan.info["lazy_verify"] == 1 - eager          # a complete schedule writes every (rank, section)
     oplan = OP.build_plan(p, g, ell, n, dtype, k=k)
     s = _session(plan, verify=True)
     res = s.verify()
@@ -188,6 +192,40 @@ def test_verifier_detects_a_truncated_schedule(limit, exec_mode):
     with pytest.raises(B.OptccError) as e:
         s.verify()
     assert e.value.name == "EVERIFY"
+
+
+LAZY_TRUNCATED = [
+    # p, ell, k, ordering, schedule, limits that still write every (rank, section) -- so the lazy verifier runs
+    (5, [1.0] * 5, 0, 0, 0, (5, 7)),                                   # C0: 8 steps, cut inside the all-gather
+    (5, [1.0, 1.0, 1.5, 1.0, 1.0], 4, 1, 0, (24, 27)),                 # C1' (ordering 1): 28 steps
+    (5, [1.0, 1.0, 2.5, 1.0, 1.0], 0, 0, 1, (6,)),                     # ring on the degraded topology
+]
+
+
+@pytest.mark.parametrize("exec_mode", MODES)
+@pytest.mark.parametrize("n", [4099, 150001])
+@pytest.mark.parametrize("p,ell,k,ordering,schedule,limits", LAZY_TRUNCATED)
+def test_lazy_verifier_detects_a_truncated_schedule(p, ell, k, ordering, schedule, limits, n, exec_mode):
+    """Truncated schedules that still write every (rank, section) at least once are verified lazily: the wrong final
+    masks are found by the last writer of each range (no pass over the arrays).  Count, first index and the masks
+    themselves must equal the oracle's for the same truncated table -- and the eager verifier's."""
+    import dataclasses
+    oplan = OP.build_plan(p, 1, ell, n, W.F32, k=k, ordering=ordering or 2, schedule=schedule)
+    for limit in limits:
+        assert limit < oplan.n_steps
+        m_or, _ = OI.element_masks(dataclasses.replace(oplan, n_steps=limit))
+        bad = (m_or != OI.full_mask_words(p)[None, None, :]).any(axis=2)
+        assert bad.sum() > 0
+        for eager in (0, 1):
+            plan = B.optcc_plan(p, 1, ell, n, W.F32, k=k, exec_mode=exec_mode, step_limit=limit, ordering=ordering,
+                                schedule=schedule, verify_eager=eager)
+            assert plan.info["lazy_verify"] == 1 - eager
+            s = _session(plan, verify=True)
+            res = s.verify(raise_on_fail=False)
+            assert s.masks().tobytes() == m_or.tobytes()
+            assert res["bad_elements"] == int(bad.sum())
+            assert res["first_bad"] == int(np.flatnonzero(bad.reshape(-1))[0])
+            assert res["overlap_elements"] == 0
 
 
 def test_execute_rejects_bad_arguments():
