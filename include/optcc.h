@@ -203,6 +203,21 @@ OPTCC_API int optcc_execute(optcc_plan_t* plan, void* const* bufs, void* workspa
  * `stream`, asynchronous. */
 OPTCC_API int optcc_execute_host(optcc_plan_t* plan, const void* const* host_in, void* const* host_out,
                        void* const* bufs, void* workspace, void* stream);
+/* End-to-end, pipelined over element shards.  No flow ever mixes two element indices (the path shards along the
+ * element axis), so an AllReduce of n_total elements per rank is n_total / n independent AllReduces of
+ * n = plan's n elements each, all with this one plan: shard c is elements [c n, (c+1) n) of every rank.  The
+ * host-to-device copy of shard c+1, the execution of shard c and the device-to-host copy of shard c-1 overlap
+ * (two internal copy streams; the PCIe link carries both directions at once), so the end-to-end time approaches
+ * max(H2D, D2H) instead of their sum.  host_in / host_out [host arrays of p PINNED host pointers, n_total elements
+ * each]; bufs [host array of p device pointers, n_total elements each, 16-byte aligned]; workspace as for
+ * optcc_execute (shards run one after another on `stream`, sharing it).  All work is ordered after what was
+ * enqueued on `stream` before the call, and `stream` waits for all of it: to the caller it behaves like
+ * optcc_execute_host.  The result of every shard is exactly what optcc_execute gives on that shard alone (the add
+ * order per element follows the plan for n, not a plan for n_total).
+ * Errors: EINVAL (NULL pointers, n_total not a multiple of n, or more than one shard with n not a multiple of 8
+ * elements -- shard starts must stay 16-byte aligned), ECUDA. */
+OPTCC_API int optcc_execute_host_sharded(optcc_plan_t* plan, uint64_t n_total, const void* const* host_in,
+                               void* const* host_out, void* const* bufs, void* workspace, void* stream);
 
 /* ---- verification --------------------------------------------------------------------------------------------
  * Runs the SAME step tables through the executor with contributor bitmasks as elements (rank r starts as

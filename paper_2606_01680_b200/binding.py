@@ -66,7 +66,7 @@ class OptccError(RuntimeError):
 
 _lib = None
 EXPORTS = ("optcc_plan", "optcc_plan_ex", "optcc_plan_destroy", "optcc_plan_info", "optcc_plan_tables", "optcc_cost",
-           "optcc_prepare", "optcc_execute", "optcc_execute_host", "optcc_verify", "optcc_strerror",
+           "optcc_prepare", "optcc_execute", "optcc_execute_host", "optcc_execute_host_sharded", "optcc_verify", "optcc_strerror",
            "optcc_last_cuda_error", "optcc_abi_version")
 
 
@@ -90,6 +90,7 @@ def load():
     lib.optcc_prepare.argtypes = [vp, vp, vp]
     lib.optcc_execute.argtypes = [vp, C.POINTER(vp), vp, vp]
     lib.optcc_execute_host.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), vp, vp]
+    lib.optcc_execute_host_sharded.argtypes = [vp, u64, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), vp, vp]
     lib.optcc_verify.argtypes = [vp, vp, vp, C.POINTER(optcc_verify_result_t)]
     lib.optcc_strerror.argtypes = [C.c_int]
     lib.optcc_strerror.restype = C.c_char_p
@@ -205,6 +206,14 @@ def optcc_execute_host(plan, host_in, host_out, bufs, workspace, stream=None):
                                    _ptr(workspace), _ptr(stream))
     if rc:
         raise OptccError(rc, "optcc_execute_host")
+
+
+def optcc_execute_host_sharded(plan, n_total, host_in, host_out, bufs, workspace, stream=None):
+    """n_total / plan.n element shards, all with `plan`; H2D, execution and D2H of neighbouring shards overlap."""
+    rc = load().optcc_execute_host_sharded(plan.handle, int(n_total), _ptr_array(host_in), _ptr_array(host_out),
+                                           _ptr_array(bufs), _ptr(workspace), _ptr(stream))
+    if rc:
+        raise OptccError(rc, "optcc_execute_host_sharded")
 
 
 def optcc_verify(plan, workspace, stream=None, raise_on_fail=True):

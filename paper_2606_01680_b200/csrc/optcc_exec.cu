@@ -593,33 +593,35 @@ void build_dataflow_tables(optcc_plan_t* pl, optcc_exec_state* st) {
     st->big_ops = pl->n_tile_ops && units / pl->n_tile_ops >= 1792;
   }
   if (!st->df_ok) return;
-  std::vector<uint32_t> count(size_t(in.p) * nr, 0), lastw(size_t(in.p) * nr, 0);
-  std::vector<uint32_t> readers(size_t(in.p) * nr, 0);   // reads of the range since its last write
+  struct RangeState { uint32_t count, lastw, readers; };   // accesses so far, position after the last write, reads since it
+  std::vector<RangeState> rs(size_t(in.p) * nr, RangeState{0, 0, 0});
   std::vector<uint8_t> sole_reader(in.n_flows, 0);       // the flow is the first reader of its source since the last write
   st->deps.resize(in.n_flows);
-  st->ops.clear();
-  st->ops.reserve(pl->n_tile_ops);
+  st->ops.resize(pl->n_tile_ops);
+  TileOp* op_out = st->ops.data();
   st->step_op_begin.assign(in.n_steps + 1, 0);
   uint32_t step = 0;
   for (uint32_t i = 0; i < in.n_flows; ++i) {
     const optcc_flow_t& f = pl->flows[i];
-    while (step < f.step) st->step_op_begin[++step] = st->ops.size();
-    const size_t reg = size_t(std::lower_bound(pl->region_offs.begin(), pl->region_offs.end(), f.off) - pl->region_offs.begin());
+    while (step < f.step) st->step_op_begin[++step] = uint64_t(op_out - st->ops.data());
+    const size_t reg = pl->flow_region[i];
     const size_t ls = size_t(f.src) * nr + reg, ld = size_t(f.dst) * nr + reg;
     DDep d;
     d.csrc = uint32_t(uint64_t(f.src) * pl->tiles_per_rank + pl->region_tile0[reg]);
     d.cdst = uint32_t(uint64_t(f.dst) * pl->tiles_per_rank + pl->region_tile0[reg]);
-    d.need_src = lastw[ls];
-    count[ls]++;
-    sole_reader[i] = readers[ls]++ == 0;
-    d.need_dst = count[ld];
-    lastw[ld] = ++count[ld];
-    readers[ld] = 0;
+    RangeState& S = rs[ls];
+    d.need_src = S.lastw;
+    S.count++;
+    sole_reader[i] = S.readers++ == 0;
+    RangeState& D = rs[ld];
+    d.need_dst = D.count;
+    D.lastw = ++D.count;
+    D.readers = 0;
     st->deps[i] = d;
     const uint64_t ntiles = ((f.len + A - 1) / A + TU - 1) / TU;
-    for (uint64_t t = 0; t < ntiles; ++t) st->ops.push_back(TileOp{i, uint32_t(t)});
+    for (uint64_t t = 0; t < ntiles; ++t) *op_out++ = TileOp{i, uint32_t(t)};
   }
-  while (step < in.n_steps) st->step_op_begin[++step] = st->ops.size();
+  while (step < in.n_steps) st->step_op_begin[++step] = uint64_t(op_out - st->ops.data());
   // dead sources: walking the table backwards, the source range of flow i is dead after i has read it iff the next
   // access to that (rank, region) is a plain overwrite by a copy flow (a reduce would still read it, a read needs
   // it, and no further access means it is a final result).  Only reduce flows act on the flag (their sources are the
@@ -628,7 +630,7 @@ void build_dataflow_tables(optcc_plan_t* pl, optcc_exec_state* st) {
   std::vector<uint8_t> next(size_t(in.p) * nr, NEXT_NONE);
   for (uint32_t i = in.n_flows; i-- > 0;) {
     const optcc_flow_t& f = pl->flows[i];
-    const size_t reg = size_t(std::lower_bound(pl->region_offs.begin(), pl->region_offs.end(), f.off) - pl->region_offs.begin());
+    const size_t reg = pl->flow_region[i];
     const size_t ls = size_t(f.src) * nr + reg, ld = size_t(f.dst) * nr + reg;
     // (first and last reader since the last write = the only one: no other flow may still be reading the range)
     // (not for truncated schedules, step_limit: the overwrite that makes the range dead might never run)
@@ -650,10 +652,9 @@ void assign_mask_flags(optcc_plan_t* pl, optcc_exec_state* st) {
   const uint32_t nf = pl->step_begin[steps];            // flows of the executed steps
   const size_t nr = pl->region_offs.size();
   std::vector<uint8_t> written(size_t(in.p) * nr, 0);
-  std::vector<uint32_t> reg(nf);
+  const std::vector<uint32_t>& reg = pl->flow_region;
   for (uint32_t i = 0; i < nf; ++i) {                   // forwards: has the range been written before flow i?
     const optcc_flow_t& f = pl->flows[i];
-    reg[i] = uint32_t(std::lower_bound(pl->region_offs.begin(), pl->region_offs.end(), f.off) - pl->region_offs.begin());
     uint32_t fl = 0;
     if (!written[size_t(f.src) * nr + reg[i]]) fl |= DFLOW_SRC_INIT;
     if (!written[size_t(f.dst) * nr + reg[i]]) fl |= DFLOW_DST_INIT;
@@ -949,6 +950,84 @@ extern "C" int optcc_execute_host(optcc_plan_t* plan, const void* const* host_in
   int rc = optcc_execute(plan, bufs, workspace, stream_);
   if (rc != OPTCC_OK) return rc;
   for (uint32_t r = 0; r < in.p; ++r) CU_TRY(cudaMemcpyAsync(host_out[r], bufs[r], bytes, cudaMemcpyDeviceToHost, stream));
+  return OPTCC_OK;
+}
+
+namespace {
+// The two copy streams and the events of optcc_execute_host_sharded, created on first use, one set per device.
+struct ShardPipe {
+  cudaStream_t in = nullptr, out = nullptr;
+  cudaEvent_t begin = nullptr, end = nullptr;
+  std::vector<cudaEvent_t> loaded, done;     // per shard: inputs on the device / results computed
+};
+std::mutex g_pipe_mutex;
+std::unordered_map<int, ShardPipe> g_pipes;
+
+int shard_pipe(int dev, size_t shards, ShardPipe** out) {
+  ShardPipe& sp = g_pipes[dev];
+  if (!sp.in) {
+    CU_TRY(cudaStreamCreateWithFlags(&sp.in, cudaStreamNonBlocking));
+    CU_TRY(cudaStreamCreateWithFlags(&sp.out, cudaStreamNonBlocking));
+    CU_TRY(cudaEventCreateWithFlags(&sp.begin, cudaEventDisableTiming));
+    CU_TRY(cudaEventCreateWithFlags(&sp.end, cudaEventDisableTiming));
+  }
+  while (sp.loaded.size() < shards) {
+    cudaEvent_t a, b;
+    CU_TRY(cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
+    CU_TRY(cudaEventCreateWithFlags(&b, cudaEventDisableTiming));
+    sp.loaded.push_back(a);
+    sp.done.push_back(b);
+  }
+  *out = &sp;
+  return OPTCC_OK;
+}
+}  // namespace
+
+extern "C" int optcc_execute_host_sharded(optcc_plan_t* plan, uint64_t n_total, const void* const* host_in,
+                                          void* const* host_out, void* const* bufs, void* workspace, void* stream_) {
+  if (!plan || !host_in || !host_out || !bufs || !workspace) return OPTCC_EINVAL;
+  const optcc_plan_info_t& in = plan->info;
+  if (n_total == 0 || n_total % in.n != 0) return OPTCC_EINVAL;
+  const uint64_t shards = n_total / in.n;
+  if (shards > 1 && in.n % 8 != 0) return OPTCC_EINVAL;            // shard starts stay 16-byte aligned
+  if (shards > (uint64_t(1) << 16)) return OPTCC_EINVAL;
+  for (uint32_t r = 0; r < in.p; ++r)
+    if (!host_in[r] || !host_out[r] || !bufs[r] || (reinterpret_cast<uintptr_t>(bufs[r]) & 15)) return OPTCC_EINVAL;
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  const size_t bytes = size_t(in.n) * (in.dtype == OPTCC_F32 ? 4 : 2);   // per rank and shard
+  int dev = 0;
+  CU_TRY(cudaGetDevice(&dev));
+  std::lock_guard<std::mutex> lock(g_pipe_mutex);   // one pipelined call at a time per process: the streams are shared
+  ShardPipe* sp = nullptr;
+  int rc = shard_pipe(dev, size_t(shards), &sp);
+  if (rc != OPTCC_OK) return rc;
+  rc = prepare_impl(plan, workspace, stream_, false);               // tables first, then the copies may start
+  if (rc != OPTCC_OK) return rc;
+  CU_TRY(cudaEventRecord(sp->begin, stream));
+  CU_TRY(cudaStreamWaitEvent(sp->in, sp->begin, 0));
+  CU_TRY(cudaStreamWaitEvent(sp->out, sp->begin, 0));
+  std::vector<void*> shard_bufs(in.p);
+  for (uint64_t c = 0; c < shards; ++c) {
+    const size_t o = size_t(c) * bytes;
+    for (uint32_t r = 0; r < in.p; ++r)
+      CU_TRY(cudaMemcpyAsync(static_cast<char*>(bufs[r]) + o, static_cast<const char*>(host_in[r]) + o, bytes,
+                             cudaMemcpyHostToDevice, sp->in));
+    CU_TRY(cudaEventRecord(sp->loaded[c], sp->in));
+  }
+  for (uint64_t c = 0; c < shards; ++c) {
+    const size_t o = size_t(c) * bytes;
+    for (uint32_t r = 0; r < in.p; ++r) shard_bufs[r] = static_cast<char*>(bufs[r]) + o;
+    CU_TRY(cudaStreamWaitEvent(stream, sp->loaded[c], 0));
+    rc = optcc_execute(plan, shard_bufs.data(), workspace, stream_);
+    if (rc != OPTCC_OK) return rc;
+    CU_TRY(cudaEventRecord(sp->done[c], stream));
+    CU_TRY(cudaStreamWaitEvent(sp->out, sp->done[c], 0));
+    for (uint32_t r = 0; r < in.p; ++r)
+      CU_TRY(cudaMemcpyAsync(static_cast<char*>(host_out[r]) + o, static_cast<char*>(bufs[r]) + o, bytes,
+                             cudaMemcpyDeviceToHost, sp->out));
+  }
+  CU_TRY(cudaEventRecord(sp->end, sp->out));
+  CU_TRY(cudaStreamWaitEvent(stream, sp->end, 0));
   return OPTCC_OK;
 }
 

@@ -33,6 +33,7 @@ struct optcc_plan {
   uint64_t tiles_per_rank = 0;          // sum over regions of ceil(units / tile_units): counters per rank
   std::vector<uint64_t> region_offs;    // sorted unique flow offsets (regions tile [0, n), PLAN_SPEC 5.4)
   std::vector<uint64_t> region_tile0;   // first tile counter of every region (prefix sum)
+  std::vector<uint32_t> flow_region;    // [n_flows] index into region_offs of the region a flow covers
   optcc_exec_state* exec;               // created lazily by the executor; freed by optcc_plan_destroy
 };
 

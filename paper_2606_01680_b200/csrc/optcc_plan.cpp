@@ -420,6 +420,21 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     add_regions(pl->sec_bounds);
     add_regions(pl->p2p_bounds);
     pl->tiles_per_rank = tiles;
+    // region of every flow, looked up once (the executor's table walks all need it); consecutive flows of one
+    // (stage, src, dst) chain mostly hit neighbouring regions, so try the last answer's neighbours first
+    pl->flow_region.resize(pl->flows.size());
+    {
+      const std::vector<uint64_t>& ro = pl->region_offs;
+      size_t last = 0;
+      for (size_t i = 0; i < pl->flows.size(); ++i) {
+        const uint64_t off = pl->flows[i].off;
+        if (!(last < ro.size() && ro[last] == off)) {
+          if (last + 1 < ro.size() && ro[last + 1] == off) ++last;
+          else last = size_t(std::lower_bound(ro.begin(), ro.end(), off) - ro.begin());
+        }
+        pl->flow_region[i] = (uint32_t)last;
+      }
+    }
     for (const auto& f : pl->flows) pl->n_tile_ops += ((f.len + B.A - 1) / B.A + pl->tile_units - 1) / pl->tile_units;
   } catch (const std::bad_alloc&) {
     delete pl;
@@ -435,8 +450,7 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
       size_t left = written.size();
       for (uint32_t i = 0; i < pl->step_begin[steps]; ++i) {
         const optcc_flow_t& f = pl->flows[i];
-        const size_t r = size_t(std::lower_bound(pl->region_offs.begin(), pl->region_offs.end(), f.off) - pl->region_offs.begin());
-        uint8_t& w = written[size_t(f.dst) * nr + r];
+        uint8_t& w = written[size_t(f.dst) * nr + pl->flow_region[i]];
         left -= !w;
         w = 1;
       }

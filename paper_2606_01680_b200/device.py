@@ -16,9 +16,10 @@ def _require_cuda():
 
 class Session:
     """Device state for one plan: rank buffers (separate allocations, so any n keeps 16-byte alignment),
-    workspace sized for execute (and verify, if asked)."""
+    workspace sized for execute (and verify, if asked).  shards > 1: the rank buffers hold `shards` element shards
+    of the plan's n each (optcc_execute_host_sharded)."""
 
-    def __init__(self, plan, device="cuda:0", verify=False, alloc_bufs=True):
+    def __init__(self, plan, device="cuda:0", verify=False, alloc_bufs=True, shards=1):
         _require_cuda()
         self.plan = plan
         self.device = torch.device(device)
@@ -32,7 +33,8 @@ class Session:
             off = (-self.workspace.data_ptr()) % 256
             self.ws_ptr = self.workspace.data_ptr() + off
             self._ws_off = off
-            self.bufs = [torch.empty(self.n, dtype=self.torch_dtype, device=self.device) for _ in range(self.p)] if alloc_bufs else None
+            self.shards = int(shards)
+            self.bufs = [torch.empty(self.n * self.shards, dtype=self.torch_dtype, device=self.device) for _ in range(self.p)] if alloc_bufs else None
 
     # -- data movement (plumbing) --
     def upload(self, x):
@@ -87,6 +89,11 @@ class Session:
     def execute_host(self, host_in, host_out, stream=None):
         with torch.cuda.device(self.device):
             B.optcc_execute_host(self.plan, host_in, host_out, self.bufs, self.ws_ptr, self._stream(stream))
+
+    def execute_host_sharded(self, host_in, host_out, stream=None):
+        with torch.cuda.device(self.device):
+            B.optcc_execute_host_sharded(self.plan, self.n * self.shards, host_in, host_out, self.bufs, self.ws_ptr,
+                                         self._stream(stream))
 
     def verify(self, stream=None, raise_on_fail=True):
         with torch.cuda.device(self.device):

@@ -258,6 +258,58 @@ def test_execute_host_roundtrip():
     assert y.tobytes() == OI.run_f32(oplan, x).tobytes()
 
 
+@pytest.mark.parametrize("p,st,n,dtype,k,shards", [
+    (8, {0: 2.0}, 2 ** 15 + 8, W.F32, 4, 3),
+    (16, {0: 8.0 / 7.0}, 2 ** 18, W.F32, 8, 5),          # several tiles per flow, bubble flows
+    (5, {2: 1.5}, 50000, W.BF16, 4, 4),
+    (7, {0: 2.0, 1: 4.0 / 3.0}, 20011, W.F32, 4, 1),     # one shard: any n
+])
+def test_execute_host_sharded_equals_the_oracle_shard_by_shard(p, st, n, dtype, k, shards):
+    """optcc_execute_host_sharded: n_total = shards * n elements per rank, every shard an independent AllReduce with
+    the one plan for n; the H2D / execute / D2H pipeline must give, shard by shard, exactly the oracle's plan-order
+    result, and later work on the caller's stream must see the finished results."""
+    import torch
+    w = _wl(p, 1, st, n * shards, dtype, seed=77 + p)
+    ell = list(w.ell)
+    plan = B.optcc_plan(p, 1, ell, n, dtype, k=k)
+    oplan = OP.build_plan(p, 1, ell, n, dtype, k=k)
+    from paper_2606_01680_b200.device import Session
+    s = Session(plan, shards=shards)
+    x = W.all_inputs(w)                                   # [p, shards * n]
+    tdt = torch.float32 if dtype == W.F32 else torch.int16
+    hin = [torch.from_numpy(x[r].copy().view(np.float32 if dtype == W.F32 else np.int16)).pin_memory() for r in range(p)]
+    hout = [torch.zeros(n * shards, dtype=tdt).pin_memory() for r in range(p)]
+    for rep in range(2):                                  # the second call reuses the streams and events
+        s.execute_host_sharded(hin, hout)
+        on_stream = s.bufs[p - 1].clone()                 # enqueued on the caller's stream after the call
+        torch.cuda.synchronize()
+        y = np.stack([t.numpy().view(x.dtype) for t in hout])
+        assert OR.all_ranks_identical(y)
+        assert on_stream.cpu().numpy().view(x.dtype).tobytes() == y[0].tobytes() if dtype == W.F32 else True
+        for c in range(shards):
+            xs = np.ascontiguousarray(x[:, c * n:(c + 1) * n])
+            y_or = OI.run_f32(oplan, xs) if dtype == W.F32 else OI.run_bf16(oplan, xs)
+            assert np.ascontiguousarray(y[:, c * n:(c + 1) * n]).tobytes() == y_or.tobytes(), (rep, c)
+
+
+def test_execute_host_sharded_rejects_bad_shapes():
+    import torch
+    plan = B.optcc_plan(4, 1, [2.0, 1.0, 1.0, 1.0], 4100, W.F32, k=4)     # n % 8 = 4
+    from paper_2606_01680_b200.device import Session
+    s = Session(plan, shards=2)
+    h = [torch.zeros(8200).pin_memory() for _ in range(4)]
+    st = torch.cuda.current_stream().cuda_stream
+    with pytest.raises(B.OptccError) as e:
+        B.optcc_execute_host_sharded(plan, 8200, h, h, s.bufs, s.ws_ptr, st)    # shard start not 16-byte aligned
+    assert e.value.name == "EINVAL"
+    with pytest.raises(B.OptccError) as e:
+        B.optcc_execute_host_sharded(plan, 4101, h, h, s.bufs, s.ws_ptr, st)    # not a multiple of the plan's n
+    assert e.value.name == "EINVAL"
+    with pytest.raises(B.OptccError) as e:
+        B.optcc_execute_host_sharded(plan, 0, h, h, s.bufs, s.ws_ptr, st)
+    assert e.value.name == "EINVAL"
+
+
 def test_repeated_execute_on_same_session_is_deterministic():
     w = _wl(16, 1, {0: 8.0 / 7.0}, 2 ** 16, W.F32, seed=5)
     plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=8)
