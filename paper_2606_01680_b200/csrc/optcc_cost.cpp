@@ -22,16 +22,13 @@ extern "C" int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* p
   const double n = double(in.n);
 
   // ---- event simulation (PLAN_SPEC 6) ----
-  std::vector<uint64_t> offs;
-  offs.reserve(plan->flows.size());
-  for (const auto& f : plan->flows) offs.push_back(f.off);
-  std::sort(offs.begin(), offs.end());
-  offs.erase(std::unique(offs.begin(), offs.end()), offs.end());
-  const size_t nr = offs.size();
-  std::vector<double> wfin, rfin, send_free, recv_free;
+  // per (rank, region): when its last write and its last read finish; regions = the plan's sections / P2P pieces
+  struct RangeTimes { double wfin, rfin; };
+  const size_t nr = plan->region_offs.size();
+  std::vector<RangeTimes> rt;
+  std::vector<double> send_free, recv_free;
   try {
-    wfin.assign(size_t(p) * nr, 0.0);
-    rfin.assign(size_t(p) * nr, 0.0);
+    rt.assign(size_t(p) * nr, RangeTimes{0.0, 0.0});
     send_free.assign(size_t(p) * 2, 0.0);
     recv_free.assign(size_t(p) * 2, 0.0);
   } catch (const std::bad_alloc&) {
@@ -40,8 +37,9 @@ extern "C" int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* p
   double T = 0.0;
   const uint32_t r_str = m ? plan->stragglers[0] * g : 0;
   double sent = 0.0, recvd = 0.0;
-  for (const auto& f : plan->flows) {
-    size_t reg = size_t(std::lower_bound(offs.begin(), offs.end(), f.off) - offs.begin());
+  for (size_t i = 0; i < plan->flows.size(); ++i) {
+    const optcc_flow_t& f = plan->flows[i];
+    const size_t reg = plan->flow_region[i];
     double dur;
     if (f.link == OPTCC_LINK_NIC)
       dur = alpha + beta * double(f.len) * std::max(plan->ell[f.src], plan->ell[f.dst]);
@@ -49,10 +47,12 @@ extern "C" int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* p
       dur = alpha + beta * double(f.len) / double(g - 1);
     double& sf = send_free[size_t(f.src) * 2 + f.link];
     double& rf = recv_free[size_t(f.dst) * 2 + f.link];
-    double& ws = wfin[size_t(f.src) * nr + reg];
-    double& wd = wfin[size_t(f.dst) * nr + reg];
-    double& rd = rfin[size_t(f.dst) * nr + reg];
-    double& rs = rfin[size_t(f.src) * nr + reg];
+    RangeTimes& S = rt[size_t(f.src) * nr + reg];
+    RangeTimes& D = rt[size_t(f.dst) * nr + reg];
+    double& ws = S.wfin;
+    double& wd = D.wfin;
+    double& rd = D.rfin;
+    double& rs = S.rfin;
     double start = std::max(std::max(sf, rf), std::max(ws, std::max(wd, rd)));
     double fin = start + dur;
     sf = fin;
