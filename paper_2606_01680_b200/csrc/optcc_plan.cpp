@@ -128,23 +128,18 @@ void assign_kinds(optcc_plan_t* pl) {
   pl->kind_dst_in.assign(nf, OPTCC_KIND_BUF);
   pl->kind_dst_out.assign(nf, OPTCC_KIND_BUF);
   if (pl->info.dtype != OPTCC_BF16) return;
-  std::vector<uint64_t> offs;
-  offs.reserve(nf);
-  for (const auto& f : pl->flows) offs.push_back(f.off);
-  std::sort(offs.begin(), offs.end());
-  offs.erase(std::unique(offs.begin(), offs.end()), offs.end());
-  const size_t nr = offs.size();
+  const size_t nr = pl->region_offs.size();
   std::vector<uint16_t> cnt(size_t(p) * nr, 1);
-  auto region = [&](uint64_t off) { return size_t(std::lower_bound(offs.begin(), offs.end(), off) - offs.begin()); };
+  auto region = [&](uint32_t i) { return size_t(pl->flow_region[i]); };
   auto kind_of = [&](uint16_t c) -> uint8_t { return (c == 1 || c >= p) ? OPTCC_KIND_BUF : OPTCC_KIND_F32; };
   std::vector<uint16_t> src_cnt;
   for (uint32_t t = 0; t < pl->info.n_steps; ++t) {
     uint32_t lo = pl->step_begin[t], hi = pl->step_begin[t + 1];
     src_cnt.resize(hi - lo);
-    for (uint32_t i = lo; i < hi; ++i) src_cnt[i - lo] = cnt[size_t(pl->flows[i].src) * nr + region(pl->flows[i].off)];
+    for (uint32_t i = lo; i < hi; ++i) src_cnt[i - lo] = cnt[size_t(pl->flows[i].src) * nr + region(i)];
     for (uint32_t i = lo; i < hi; ++i) {
       const optcc_flow_t& f = pl->flows[i];
-      uint16_t& cd = cnt[size_t(f.dst) * nr + region(f.off)];
+      uint16_t& cd = cnt[size_t(f.dst) * nr + region(i)];
       uint16_t cs = src_cnt[i - lo];
       pl->kind_src[i] = kind_of(cs);
       pl->kind_dst_in[i] = kind_of(cd);
@@ -386,12 +381,6 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
   for (uint32_t t = 0; t < n_steps; ++t)
     in.max_flows_per_step = std::max(in.max_flows_per_step, pl->step_begin[t + 1] - pl->step_begin[t]);
   for (const auto& f : pl->flows) (f.op == OPTCC_OP_REDUCE ? in.reduce_elems : in.copy_elems) += f.len;
-  try {
-    assign_kinds(pl);
-  } catch (const std::bad_alloc&) {
-    delete pl;
-    return OPTCC_ENOMEM;
-  }
   // dataflow tiling: regions (unique offsets; all flows over one offset share a length, PLAN_SPEC 5.4) and tile counts
   try {
     if (pl->opts.tile_units) {
@@ -409,33 +398,51 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     }
     // regions = the sections and P2P pieces themselves: consecutive exported boundaries (ascending, contiguous)
     uint64_t tiles = 0;
-    auto add_regions = [&](const std::vector<uint64_t>& bounds) {
+    std::vector<uint32_t> sec_reg, p2p_reg;     // boundary interval -> region (UINT32_MAX: empty interval)
+    bool region_error = false;
+    auto add_regions = [&](const std::vector<uint64_t>& bounds, std::vector<uint32_t>& reg_of) {
+      reg_of.assign(bounds.empty() ? 0 : bounds.size() - 1, UINT32_MAX);
       for (size_t i = 0; i + 1 < bounds.size(); ++i) {
         if (bounds[i + 1] <= bounds[i]) continue;
+        reg_of[i] = (uint32_t)pl->region_offs.size();
         pl->region_offs.push_back(bounds[i]);
         pl->region_tile0.push_back(tiles);
         tiles += ((bounds[i + 1] - bounds[i] + B.A - 1) / B.A + pl->tile_units - 1) / pl->tile_units;
       }
     };
-    add_regions(pl->sec_bounds);
-    add_regions(pl->p2p_bounds);
+    add_regions(pl->sec_bounds, sec_reg);
+    add_regions(pl->p2p_bounds, p2p_reg);
     pl->tiles_per_rank = tiles;
-    // region of every flow, looked up once (the executor's table walks all need it); consecutive flows of one
-    // (stage, src, dst) chain mostly hit neighbouring regions, so try the last answer's neighbours first
+    // region of every flow, looked up once (the executor's and the cost model's table walks all need it): a flow
+    // carries its (part, segment, section), i.e. its interval of sec_bounds (bubble flows: of p2p_bounds)
     pl->flow_region.resize(pl->flows.size());
     {
       const std::vector<uint64_t>& ro = pl->region_offs;
-      size_t last = 0;
       for (size_t i = 0; i < pl->flows.size(); ++i) {
-        const uint64_t off = pl->flows[i].off;
-        if (!(last < ro.size() && ro[last] == off)) {
-          if (last + 1 < ro.size() && ro[last + 1] == off) ++last;
-          else last = size_t(std::lower_bound(ro.begin(), ro.end(), off) - ro.begin());
+        const optcc_flow_t& f = pl->flows[i];
+        uint32_t r = UINT32_MAX;
+        if (f.stage == OPTCC_BUB_UP || f.stage == OPTCC_BUB_DOWN) {
+          if (f.seg < p2p_reg.size()) r = p2p_reg[f.seg];
+        } else {
+          const size_t idx = (size_t(f.part) * k + f.seg) * B.nsec + f.sec;
+          if (idx < sec_reg.size()) r = sec_reg[idx];
         }
-        pl->flow_region[i] = (uint32_t)last;
+        if (r == UINT32_MAX || ro[r] != f.off) r = uint32_t(std::lower_bound(ro.begin(), ro.end(), f.off) - ro.begin());
+        if (r >= ro.size() || ro[r] != f.off) { region_error = true; break; }   // PLAN_SPEC 5.4 violated: a planner bug
+        pl->flow_region[i] = r;
       }
     }
+    if (region_error) {
+      delete pl;
+      return OPTCC_EINVAL;
+    }
     for (const auto& f : pl->flows) pl->n_tile_ops += ((f.len + B.A - 1) / B.A + pl->tile_units - 1) / pl->tile_units;
+  } catch (const std::bad_alloc&) {
+    delete pl;
+    return OPTCC_ENOMEM;
+  }
+  try {
+    assign_kinds(pl);      // (needs flow_region)
   } catch (const std::bad_alloc&) {
     delete pl;
     return OPTCC_ENOMEM;
