@@ -263,6 +263,7 @@ def test_execute_host_roundtrip():
     (16, {0: 8.0 / 7.0}, 2 ** 18, W.F32, 8, 5),          # several tiles per flow, bubble flows
     (5, {2: 1.5}, 50000, W.BF16, 4, 4),
     (7, {0: 2.0, 1: 4.0 / 3.0}, 20011, W.F32, 4, 1),     # one shard: any n
+    (130, {0: 2.0}, 1024, W.F32, 4, 2),                  # p > 128: the rank-pointer table is rewritten per shard
 ])
 def test_execute_host_sharded_equals_the_oracle_shard_by_shard(p, st, n, dtype, k, shards):
     """optcc_execute_host_sharded: n_total = shards * n elements per rank, every shard an independent AllReduce with
@@ -308,6 +309,30 @@ def test_execute_host_sharded_rejects_bad_shapes():
     with pytest.raises(B.OptccError) as e:
         B.optcc_execute_host_sharded(plan, 0, h, h, s.bufs, s.ws_ptr, st)
     assert e.value.name == "EINVAL"
+
+
+def test_execute_is_capturable_in_a_cuda_graph():
+    """optcc_execute only enqueues work (two memsets and one cooperative launch once the tables are resident): it can
+    be captured into a CUDA graph and replayed; every replay must reproduce the oracle's result."""
+    import torch
+    w = _wl(8, 1, {0: 2.0}, 2 ** 16 + 4, W.F32, seed=41)
+    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=4)
+    oplan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=4)
+    x = W.all_inputs(w)
+    y_or = OI.run_f32(oplan, x)
+    s = _session(plan)
+    s.upload(x)
+    s.execute()                                    # warm-up: tables uploaded, kernel attributes set
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        s.execute(stream=side)
+    for _ in range(3):
+        s.upload(x)
+        graph.replay()
+        torch.cuda.synchronize()
+        assert s.download().tobytes() == y_or.tobytes()
 
 
 def test_repeated_execute_on_same_session_is_deterministic():
