@@ -195,8 +195,8 @@ OPTCC_API int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* pa
  * workspace (or after another plan used it) uploads the tables into it; optcc_prepare does this ahead of time and
  * always re-uploads -- call it again if the workspace memory was reused for something else in between.  stream: a cudaStream_t
  * (NULL = default stream).  Asynchronous: never synchronises the device or the stream; once the tables are resident
- * (after optcc_prepare or a first call) it only enqueues two memsets and one launch, so it can be captured into a
- * CUDA graph on `stream` and replayed.
+ * (after optcc_prepare or a first call) it only enqueues memsets and kernel launches (dataflow executor: two memsets
+ * and one cooperative launch), so it can be captured into a CUDA graph on `stream` and replayed.
  * Errors: EINVAL (NULL / misaligned pointers), ECUDA. */
 OPTCC_API int optcc_prepare(optcc_plan_t* plan, void* workspace, void* stream);
 OPTCC_API int optcc_execute(optcc_plan_t* plan, void* const* bufs, void* workspace, void* stream);
