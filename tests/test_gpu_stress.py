@@ -88,3 +88,43 @@ def test_dataflow_random_midsize_plans(seed):
     res = s.verify()
     assert res["bad_elements"] == 0 and res["overlap_elements"] == 0
     assert s.masks().tobytes() == OI.element_masks(oplan)[0].tobytes()
+
+
+@pytest.mark.parametrize("seed", range(150))
+def test_random_plans_any_executor_any_verifier(seed):
+    """Random plans through a random executor, with the lazy or the eager verifier, complete or cut after a random
+    step: outputs (complete schedules) bit-equal to the oracle; masks, number of wrong final masks, first wrong
+    index and overlap count equal to the oracle's walk of the same (possibly truncated) table."""
+    import dataclasses
+    from paper_2606_01680_b200.device import Session
+    rng = np.random.default_rng(31337 + seed)
+    p, g, ell, n, k, dtype, tile, grid, ordering = _random_case(rng)
+    mode = int(rng.integers(0, 3))
+    eager = int(rng.integers(0, 2))
+    oplan = OP.build_plan(p, g, ell, n, dtype, k=k, ordering=ordering or 2)
+    limit = 0
+    if rng.integers(0, 3) == 0 and oplan.n_steps > 2:
+        limit = int(rng.integers(max(1, oplan.n_steps - 6), oplan.n_steps))
+    plan = B.optcc_plan(p, g, ell, n, dtype, k=k, exec_mode=mode, tile_units=tile, grid_ctas=grid, ordering=ordering,
+                        verify_eager=eager, step_limit=limit)
+    if eager:
+        assert plan.info["lazy_verify"] == 0
+    elif not limit:
+        assert plan.info["lazy_verify"] == 1
+    s = Session(plan, verify=True)
+    if not limit:
+        x = W.all_inputs(W.Workload("s", p, g, tuple(ell), n, dtype, "normal", 1.0, 77000 + seed))
+        s.upload(x)
+        s.execute()
+        y_or = OI.run_f32(oplan, x) if dtype == W.F32 else OI.run_bf16(oplan, x)
+        assert s.download().tobytes() == y_or.tobytes()
+    else:
+        oplan = dataclasses.replace(oplan, n_steps=limit)
+    res = s.verify(raise_on_fail=False)
+    m_or, overlaps = OI.element_masks(oplan)
+    assert s.masks().tobytes() == m_or.tobytes()
+    bad = (m_or != OI.full_mask_words(p)[None, None, :]).any(axis=2)
+    assert res["bad_elements"] == int(bad.sum())
+    assert res["overlap_elements"] == overlaps
+    if bad.any():
+        assert res["first_bad"] == int(np.flatnonzero(bad.reshape(-1))[0])
