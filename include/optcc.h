@@ -60,6 +60,12 @@ enum {
   OPTCC_EXEC_DATAFLOW = 2    /* one cooperative kernel, no grid barrier: every flow is cut into tiles, tile-ops are
                                 claimed in table order and wait on per-(rank, range) completion counters, so a
                                 tile-op starts as soon as the flows it depends on have finished there */
+  ,
+  OPTCC_EXEC_COLUMN = 3      /* one kernel, no synchronisation between CTAs at all: no flow ever mixes two element
+                                indices (a flow moves a range rank to rank), so every dependency of :138
+                                lies inside one element column.  A CTA takes a tile of one region and runs every flow
+                                over that region on it, in table order, each flow's loads and stores performed as
+                                listed; the tile's working set (p ranks) stays in L2 from the first hop to the last */
 };
 
 typedef struct optcc_plan optcc_plan_t; /* opaque; immutable after creation except for cached device state */

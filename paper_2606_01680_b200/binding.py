@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(HERE, "liboptcc.so")
 
 OPTCC_F32, OPTCC_BF16 = 0, 1
 OPTCC_OK, OPTCC_EINVAL, OPTCC_EUNSUPPORTED, OPTCC_ENOMEM, OPTCC_ECUDA, OPTCC_EVERIFY = range(6)
-OPTCC_EXEC_PERSISTENT, OPTCC_EXEC_PER_STEP, OPTCC_EXEC_DATAFLOW = 0, 1, 2
+OPTCC_EXEC_PERSISTENT, OPTCC_EXEC_PER_STEP, OPTCC_EXEC_DATAFLOW, OPTCC_EXEC_COLUMN = 0, 1, 2, 3
 OPTCC_SCHED_OPTCC, OPTCC_SCHED_RING_DEGRADED = 0, 1
 ERROR_NAMES = {1: "EINVAL", 2: "EUNSUPPORTED", 3: "ENOMEM", 4: "ECUDA", 5: "EVERIFY"}
 

@@ -49,9 +49,9 @@ __device__ __forceinline__ char* rank_ptr(const ExecParams& P, unsigned int r) {
 }
 
 // One piece of one flow: 16-byte units [ubeg, uend) of the flow, executed by the whole CTA.
-template <int MODE, int NT>
+template <int MODE, int NT, class PolX>
 __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& f, unsigned long long ubeg,
-                                              unsigned long long uend, unsigned int& overlaps, const Pol& pol) {
+                                              unsigned long long uend, unsigned int& overlaps, const PolX& pol) {
   using MT = ModeTraits<MODE>;
   const unsigned long long A = P.unit_elems;
   const unsigned long long e0 = ubeg * A;
@@ -478,6 +478,97 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Column executor: no synchronisation between CTAs.  A flow moves a range from one rank to another at the same
+// offset, so no flow mixes two element indices and every data dependency of :138 lies inside one
+// element column.  A work item is one tile of one region; the CTA that claims it runs every flow over that region
+// on the tile, in table order (the flow records are stored region by region).  Thread i handles the same vectors of
+// the tile in every flow, so the ordering a dependent flow needs is the thread's own program order: each flow still
+// loads its operands from and stores its result to memory (L2) as listed -- nothing is carried in registers -- and
+// the tile's p ranks stay in L2 from the first hop to the last.
+// ---------------------------------------------------------------------------------------------------------
+constexpr int COL_THREADS = DF_COMPUTE_THREADS;
+
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
+// The operands of the next flow that the current flow does not write (a ring hop's destination is the next rank's
+// raw section: its first touch, a DRAM access) are requested while the current flow streams.  Every thread asks for
+// the vectors it will load itself (NT-strided, like the range operations).  f32 and bf16 data only: the verifier's
+// first touches are constants.
+template <int MODE, int NT>
+__device__ __forceinline__ void prefetch_operands(const ExecParams& P, const DFlow& f, unsigned int cur_dst,
+                                                  unsigned long long ubeg, unsigned long long uend) {
+  if (is_mask_mode(MODE)) return;
+  auto span = [&](const char* base, unsigned int bytes_per_unit) {
+    for (unsigned long long u = ubeg + threadIdx.x; u < uend; u += NT) prefetch_l1(base + u * bytes_per_unit);
+  };
+  if (MODE == MODE_F32) {
+    if (f.src != cur_dst) span(rank_ptr(P, f.src) + f.off * 4, 16);
+    if (f.op == 0 && f.dst != cur_dst) span(rank_ptr(P, f.dst) + f.off * 4, 16);
+  } else {
+    // raw bf16 operands only (partial sums in the shadow were written by this CTA a moment ago)
+    if (f.src != cur_dst && f.ksrc == 0) span(rank_ptr(P, f.src) + f.off * 2, 16);
+    if (f.op == 0 && f.dst != cur_dst && f.kdin == 0) span(rank_ptr(P, f.dst) + f.off * 2, 16);
+  }
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(const __grid_constant__ ExecParams P) {
+  __shared__ unsigned long long s_item;
+  unsigned int overlaps = 0;
+  // A tile is private to its CTA for the whole launch, so loads and stores go through L1 (PolL1): the value a flow
+  // stores is the next flow's source.  L2 policies all evict_normal (a dirty line marked evict_first is written back).
+  const Pol pol0 = make_policies(P.l2_hints);
+  PolL1 pol;
+  pol.lds = pol0.lds; pol.ldd = pol0.ldd; pol.st = pol0.st;
+  const unsigned long long A = P.unit_elems;
+  auto fetch = [&](unsigned int i) {
+    DFlow f;
+    const uint4* fr = reinterpret_cast<const uint4*>(P.flows + i);
+    const uint4 f0 = __ldg(fr), f1 = __ldg(fr + 1);
+    memcpy(&f, &f0, 16);
+    memcpy(reinterpret_cast<char*>(&f) + 16, &f1, 16);
+    return f;
+  };
+  for (;;) {
+    __syncthreads();                 // every thread has read the previous item
+    if (threadIdx.x == 0) s_item = atomicAdd(&P.ctrl->ticket, 1ull);
+    __syncthreads();
+    const unsigned long long it = s_item;
+    if (it >= P.col_n_items) break;
+    const uint2 item = __ldg(P.col_items + it);   // (region, tile)
+    const unsigned int fb = __ldg(P.col_reg_begin + item.x), fe = __ldg(P.col_reg_begin + item.x + 1);
+    const unsigned long long ubeg = (unsigned long long)item.y * P.tile_units;
+    if (fb >= fe) continue;
+    int prev_cls = -1;
+    // records i and i + 1 are resident at the top of iteration i; record i + 2 is requested there
+    DFlow cur = fetch(fb), nxt = cur;
+    if (fb + 1 < fe) nxt = fetch(fb + 1);
+    for (unsigned int i = fb; i < fe; ++i) {
+      DFlow nn = nxt;
+      if (i + 2 < fe) nn = fetch(i + 2);
+      const unsigned long long nunits = (cur.len + A - 1) / A;   // (all flows over a region have the same length)
+      const unsigned long long uend = ubeg + P.tile_units < nunits ? ubeg + P.tile_units : nunits;
+      if (i + 1 < fe) prefetch_operands<MODE, COL_THREADS>(P, nxt, cur.dst, ubeg, uend);
+      if (MODE == MODE_BF16) {
+        // a copy of fp32 partials moves two vectors per unit, thread i taking vector i instead of unit i: when the
+        // thread-to-element mapping changes between consecutive flows the CTA synchronises (block-wide ordering)
+        const int cls = (cur.op == 1 && cur.ksrc != 0) ? 1 : 0;
+        if (prev_cls >= 0 && cls != prev_cls) __syncthreads();
+        prev_cls = cls;
+      }
+      process_piece<MODE, COL_THREADS>(P, cur, ubeg, uend, overlaps, pol);
+      cur = nxt;
+      nxt = nn;
+    }
+  }
+  if (is_mask_mode(MODE)) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) overlaps += __shfl_xor_sync(0xFFFFFFFFu, overlaps, o);
+    if ((threadIdx.x & 31) == 0 && overlaps) atomicAdd(&P.ctrl->overlap, (unsigned long long)overlaps);
+  }
+}
+
 // masks[r][e] = {r}: blockIdx.y = rank, 16-byte stores over the rank's padded array; eb = bytes per mask
 __global__ void __launch_bounds__(256) optcc_mask_init_kernel(char* masks, unsigned long long padded_n, unsigned int eb) {
   const unsigned int r = blockIdx.y;
@@ -566,6 +657,11 @@ struct optcc_exec_state {
   std::vector<DDep> deps;         // [n_flows]
   std::vector<TileOp> ops;        // [n_tile_ops], table order
   std::vector<uint64_t> step_op_begin;   // [n_steps + 1]
+  // column executor
+  bool column = false;
+  std::vector<DFlow> col_dflows;         // the executed flows, region by region (table order inside a region)
+  std::vector<uint32_t> col_reg_begin;   // [regions + 1]
+  std::vector<uint2> col_items;          // (region, tile)
 };
 
 void optcc_exec_state_free(optcc_exec_state* s) { delete s; }
@@ -668,6 +764,30 @@ void assign_mask_flags(optcc_plan_t* pl, optcc_exec_state* st) {
     written[size_t(f.dst) * nr + reg[i]] = 1;
   }
   st->lazy_masks = true;
+}
+
+// Column executor tables: the flows of the executed steps region by region (a stable counting sort of the table by
+// region, so table order is kept inside a region) and one work item per (region, tile).
+void build_column_tables(optcc_plan_t* pl, optcc_exec_state* st) {
+  const optcc_plan_info_t& in = pl->info;
+  const uint64_t A = in.unit_elems, TU = pl->tile_units;
+  const size_t nr = pl->region_offs.size();
+  const uint32_t steps = pl->opts.step_limit ? std::min(pl->opts.step_limit, in.n_steps) : in.n_steps;
+  const uint32_t nf = pl->step_begin[steps];
+  st->col_reg_begin.assign(nr + 1, 0);
+  for (uint32_t i = 0; i < nf; ++i) st->col_reg_begin[pl->flow_region[i] + 1]++;
+  for (size_t r = 0; r < nr; ++r) st->col_reg_begin[r + 1] += st->col_reg_begin[r];
+  st->col_dflows.resize(nf);
+  std::vector<uint32_t> pos(st->col_reg_begin.begin(), st->col_reg_begin.end() - 1);
+  for (uint32_t i = 0; i < nf; ++i) st->col_dflows[pos[pl->flow_region[i]]++] = st->dflows[i];
+  st->col_items.clear();
+  st->col_items.reserve(pl->tiles_per_rank);
+  for (size_t r = 0; r < nr; ++r) {
+    const uint64_t t0 = pl->region_tile0[r], t1 = r + 1 < nr ? pl->region_tile0[r + 1] : pl->tiles_per_rank;
+    if (st->col_reg_begin[r] == st->col_reg_begin[r + 1]) continue;   // no executed flow touches the region
+    for (uint64_t t = 0; t < t1 - t0; ++t) st->col_items.push_back(make_uint2((unsigned int)r, (unsigned int)t));
+  }
+  (void)A; (void)TU;
 }
 
 template <int MODE>
@@ -778,10 +898,12 @@ int build_state(optcc_plan_t* pl) {
     st->df_ok = false;
     if (pl->opts.exec_mode == OPTCC_EXEC_DATAFLOW && st->coop && st->G_df > 0) build_dataflow_tables(pl, st);
     assign_mask_flags(pl, st);
+    st->column = pl->opts.exec_mode == OPTCC_EXEC_COLUMN && pl->tiles_per_rank < (uint64_t(1) << 32);
+    if (st->column) build_column_tables(pl, st);
     // slice table: cut every step into G slices of equal HBM bytes
     st->slices.clear();
-    if (!st->df_ok) st->slices.assign(size_t(in.n_steps) * (G + 1), Slice{0, 0, 0});
-    for (uint32_t t = 0; t < in.n_steps && !st->df_ok; ++t) {
+    if (!st->df_ok && !st->column) st->slices.assign(size_t(in.n_steps) * (G + 1), Slice{0, 0, 0});
+    for (uint32_t t = 0; t < in.n_steps && !st->df_ok && !st->column; ++t) {
       const uint32_t lo = pl->step_begin[t], hi = pl->step_begin[t + 1];
       uint64_t Wtot = 0;
       for (uint32_t i = lo; i < hi; ++i) Wtot += ((pl->flows[i].len + A - 1) / A) * unit_cost(pl, i);
@@ -817,7 +939,14 @@ int upload_tables(optcc_plan_t* pl, void* workspace, cudaStream_t stream, bool f
   const optcc_ws_layout L = optcc_layout(pl);
   char* ws = static_cast<char*>(workspace);
   CU_TRY(cudaMemsetAsync(ws + L.ctrl, 0, OPTCC_CTRL_BYTES, stream));
-  if (!st->dflows.empty())
+  if (st->column) {
+    if (!st->col_dflows.empty())
+      CU_TRY(cudaMemcpyAsync(ws + L.dflows, st->col_dflows.data(), st->col_dflows.size() * sizeof(DFlow), cudaMemcpyHostToDevice, stream));
+    if (!st->col_items.empty())
+      CU_TRY(cudaMemcpyAsync(ws + L.col, st->col_items.data(), st->col_items.size() * sizeof(uint2), cudaMemcpyHostToDevice, stream));
+    CU_TRY(cudaMemcpyAsync(ws + L.col + pl->tiles_per_rank * 8, st->col_reg_begin.data(), st->col_reg_begin.size() * sizeof(uint32_t),
+                           cudaMemcpyHostToDevice, stream));
+  } else if (!st->dflows.empty())
     CU_TRY(cudaMemcpyAsync(ws + L.dflows, st->dflows.data(), st->dflows.size() * sizeof(DFlow), cudaMemcpyHostToDevice, stream));
   if (!st->slices.empty())
     CU_TRY(cudaMemcpyAsync(ws + L.slices, st->slices.data(), st->slices.size() * sizeof(Slice), cudaMemcpyHostToDevice, stream));
@@ -845,7 +974,15 @@ int launch_plan(optcc_plan_t* pl, ExecParams& P, cudaStream_t stream) {
   if (n_steps == 0) return OPTCC_OK;
   const bool persistent = pl->opts.exec_mode == OPTCC_EXEC_PERSISTENT && st->coop;
   const bool dataflow = pl->opts.exec_mode == OPTCC_EXEC_DATAFLOW && st->coop && st->df_ok && st->G_df > 0;
-  if (dataflow) {
+  if (st->column) {
+    P.col_n_items = st->col_items.size();
+    if (P.col_n_items == 0) return OPTCC_OK;
+    CU_TRY(cudaMemsetAsync(&P.ctrl->ticket, 0, sizeof(unsigned long long), stream));
+    const uint32_t G = pl->opts.grid_ctas ? pl->opts.grid_ctas : uint32_t(st->sm_count) * CTAS_PER_SM;
+    const unsigned int grid = (unsigned int)std::min<uint64_t>(G, P.col_n_items);
+    optcc_column_kernel<MODE><<<grid, COL_THREADS, 0, stream>>>(P);
+    CU_TRY(cudaGetLastError());
+  } else if (dataflow) {
     P.n_ops = st->step_op_begin[n_steps];
     if (P.n_ops == 0) return OPTCC_OK;
     CU_TRY(cudaMemsetAsync(P.counters, 0, size_t(in.p) * pl->tiles_per_rank * sizeof(unsigned int), stream));
@@ -888,6 +1025,9 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   P.deps = reinterpret_cast<const DDep*>(ws + L.deps);
   P.ops = reinterpret_cast<const TileOp*>(ws + L.ops);
   P.counters = reinterpret_cast<unsigned int*>(ws + L.counters);
+  P.col_items = reinterpret_cast<const uint2*>(ws + L.col);
+  P.col_reg_begin = reinterpret_cast<const unsigned int*>(ws + L.col + pl->tiles_per_rank * 8);
+  P.col_n_items = 0;
   P.tile_units = pl->tile_units;
   P.bulk_copy = pl->opts.copy_path == 2 ? 1u : 0u;
   P.l2_hints = 1;   // source loads evict_first, destination loads and stores evict_normal (measured best)
@@ -895,6 +1035,7 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   // the L2 reuse distance small), small ops (small tiles, or flows shorter than a tile) -> 4 slots to hide the claim /
   // fetch / completion latency; copying agents hold their slots, so the bulk path also uses 4
   P.df_slots = (pl->exec && pl->exec->big_ops && !P.bulk_copy) ? 2 : 4;
+  if (pl->opts.exec_mode == OPTCC_EXEC_COLUMN) P.l2_hints = 0;   // see optcc_column_kernel
 }
 
 }  // namespace

@@ -41,14 +41,14 @@ struct optcc_plan {
 void optcc_exec_state_free(optcc_exec_state*);
 
 // ---- device workspace layout (bytes from the workspace base; every region 256-byte aligned) -----------------
-//   control block | rank pointers | device flow records | per-(step, CTA) slice table | dataflow deps, tile-ops, counters | fp32 shadow (bf16 plans) | masks (verify)
+//   control block | rank pointers | device flow records | per-(step, CTA) slice table | dataflow deps, tile-ops | column items | dataflow counters | fp32 shadow (bf16 plans) | masks (verify)
 constexpr uint32_t OPTCC_MAX_GRID = 1024;       // upper bound on executor CTAs (sizes the slice table)
 constexpr uint64_t OPTCC_CTRL_BYTES = 256;
 constexpr uint64_t OPTCC_DFLOW_BYTES = 32;      // sizeof(DFlow) in optcc_exec.cu
 constexpr uint64_t OPTCC_SLICE_BYTES = 16;      // sizeof(Slice)
 
 struct optcc_ws_layout {
-  uint64_t ctrl, ptrs, dflows, slices, deps, ops, counters, shadow, masks, end_exec, end_verify;
+  uint64_t ctrl, ptrs, dflows, slices, deps, ops, col, counters, shadow, masks, end_exec, end_verify;
 };
 
 static inline uint64_t optcc_align256(uint64_t x) { return (x + 255) & ~uint64_t(255); }
@@ -66,7 +66,8 @@ static inline optcc_ws_layout optcc_layout(const optcc_plan_t* pl) {
   L.slices = optcc_align256(L.dflows + uint64_t(in.n_flows) * OPTCC_DFLOW_BYTES);
   L.deps = optcc_align256(L.slices + uint64_t(in.n_steps) * (OPTCC_MAX_GRID + 1) * OPTCC_SLICE_BYTES);
   L.ops = optcc_align256(L.deps + uint64_t(in.n_flows) * OPTCC_DEP_BYTES);
-  L.counters = optcc_align256(L.ops + pl->n_tile_ops * OPTCC_OP_BYTES);
+  L.col = optcc_align256(L.ops + pl->n_tile_ops * OPTCC_OP_BYTES);   // column executor: items (8 B per (region, tile)), then region -> first flow (4 B)
+  L.counters = optcc_align256(L.col + pl->tiles_per_rank * 8 + (uint64_t(pl->region_offs.size()) + 1) * 4);
   L.shadow = optcc_align256(L.counters + uint64_t(in.p) * pl->tiles_per_rank * 4);
   uint64_t n_pad = (in.n + 7) & ~uint64_t(7);
   L.end_exec = optcc_align256(L.shadow + (in.dtype == OPTCC_BF16 ? uint64_t(in.p) * n_pad * 4 : 0));

@@ -96,6 +96,10 @@ struct ExecParams {
   unsigned long long n_ops;
   unsigned int tile_units;
   unsigned int df_slots;          // ring depth: tile-ops a CTA holds (claimed, waiting or streaming), <= DF_SLOTS
+  // column executor: flows are stored region by region (table order inside a region)
+  const uint2* col_items;         // [col_n_items] (region, tile)
+  const unsigned int* col_reg_begin;   // [regions + 1] first flow of every region in `flows`
+  unsigned long long col_n_items;
   unsigned int bulk_copy;         // 1: copy tile-ops are moved by the scheduler agents with cp.async.bulk
   unsigned int l2_hints;          // kind(src loads) + 4 kind(dst loads) + 16 kind(stores); kind: 0 normal, 1 evict_first, 2 evict_last
 };
@@ -103,7 +107,8 @@ struct ExecParams {
 // ---- memory access helpers: L2-only loads (data written by other SMs in the previous step), streaming stores ----
 // L2 eviction policies (createpolicy): loads of the streams are evict_first -- a section is dead once the next hop has
 // read it, raw destination data is dead once summed -- so that what was just written (the next step's source) stays.
-struct Pol { unsigned long long lds, ldd, st; };   // source loads, destination loads, stores
+struct Pol { unsigned long long lds, ldd, st; static constexpr unsigned int l1 = 0; };   // source loads, destination loads, stores
+struct PolL1 { unsigned long long lds, ldd, st; static constexpr unsigned int l1 = 1; }; // the same, loads and stores through L1
 __device__ __forceinline__ unsigned long long make_policy(unsigned int kind) {   // 0 normal, 1 evict_first, 2 evict_last
   unsigned long long p;
   if (kind == 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
@@ -119,17 +124,27 @@ __device__ __forceinline__ Pol make_policies(unsigned int mode) {
   p.st = make_policy((mode >> 4) & 3u);
   return p;
 }
-__device__ __forceinline__ uint4 ld16(const void* p, unsigned long long policy) {
+// l1 = 0: L2 only (.cg) -- the data may have been written by another SM.  l1 = 1 (column executor: a tile is only
+// ever touched by the CTA that owns it): default caching, so a value the thread stored one flow earlier is found in L1.
+__device__ __forceinline__ uint4 ld16(const void* p, unsigned long long policy, unsigned int l1) {
   uint4 v;
-  asm volatile("ld.global.cg.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
-               : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p), "l"(policy) : "memory");
+  if (l1)
+    asm volatile("ld.global.ca.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p), "l"(policy) : "memory");
+  else
+    asm volatile("ld.global.cg.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p), "l"(policy) : "memory");
   return v;
 }
-__device__ __forceinline__ void st16(void* p, uint4 v, const Pol& pol) {
-  asm volatile("st.global.cg.L2::cache_hint.v4.u32 [%0], {%1,%2,%3,%4}, %5;"
-               ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(pol.st) : "memory");
+template <class PolX>
+__device__ __forceinline__ void st16(void* p, uint4 v, const PolX& pol) {
+  if (pol.l1)
+    asm volatile("st.global.wb.L2::cache_hint.v4.u32 [%0], {%1,%2,%3,%4}, %5;"
+                 ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(pol.st) : "memory");
+  else
+    asm volatile("st.global.cg.L2::cache_hint.v4.u32 [%0], {%1,%2,%3,%4}, %5;"
+                 ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(pol.st) : "memory");
 }
-
 __device__ __forceinline__ float bf16_to_f32(unsigned int h) { return __uint_as_float(h << 16); }
 // float -> bf16 bits, round to nearest even; NaN stays a quiet NaN
 __device__ __forceinline__ unsigned int f32_to_bf16_rne(float f) {
@@ -193,14 +208,14 @@ __device__ __forceinline__ void remainder_dispatch(unsigned int rem, F&& f) {
   else f(std::integral_constant<int, 1>());
 }
 
-template <int UNROLL, int NT>
+template <int UNROLL, int NT, class PolX>
 __device__ __forceinline__ void range_copy16(const char* __restrict__ s, char* __restrict__ d,
-                                             unsigned long long vbeg, unsigned long long vend, const Pol& pol) {
+                                             unsigned long long vbeg, unsigned long long vend, const PolX& pol) {
   unsigned long long v = vbeg + threadIdx.x;
   for (; v + (UNROLL - 1) * (unsigned long long)NT < vend; v += UNROLL * (unsigned long long)NT) {
     uint4 x[UNROLL];
 #pragma unroll
-    for (int j = 0; j < UNROLL; ++j) x[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds);
+    for (int j = 0; j < UNROLL; ++j) x[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds, pol.l1);
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, x[j], pol);
   }
@@ -210,7 +225,7 @@ __device__ __forceinline__ void range_copy16(const char* __restrict__ s, char* _
       constexpr int KK = decltype(K)::value;
       uint4 x[KK];
 #pragma unroll
-      for (int j = 0; j < KK; ++j) x[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds);
+      for (int j = 0; j < KK; ++j) x[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds, pol.l1);
 #pragma unroll
       for (int j = 0; j < KK; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, x[j], pol);
     };
@@ -218,16 +233,16 @@ __device__ __forceinline__ void range_copy16(const char* __restrict__ s, char* _
   }
 }
 
-template <int UNROLL, int NT>
+template <int UNROLL, int NT, class PolX>
 __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* __restrict__ d,
-                                              unsigned long long vbeg, unsigned long long vend, const Pol& pol, bool dead_src) {
+                                              unsigned long long vbeg, unsigned long long vend, const PolX& pol, bool dead_src) {
   unsigned long long v = vbeg + threadIdx.x;
   for (; v + (UNROLL - 1) * (unsigned long long)NT < vend; v += UNROLL * (unsigned long long)NT) {
     uint4 a[UNROLL], b[UNROLL];
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) {
-      a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds);
-      b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd);
+      a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds, pol.l1);
+      b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd, pol.l1);
     }
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, add_f32x4(b[j], a[j]), pol);
@@ -244,8 +259,8 @@ __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* 
       uint4 a[KK], b[KK];
 #pragma unroll
       for (int j = 0; j < KK; ++j) {
-        a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds);
-        b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd);
+        a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds, pol.l1);
+        b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd, pol.l1);
       }
 #pragma unroll
       for (int j = 0; j < KK; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, add_f32x4(b[j], a[j]), pol);
@@ -255,10 +270,10 @@ __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* 
 }
 
 // masks: OR with overlap detection.  EB = bytes per mask element (2, 4, 8 or 16); a 16-byte vector holds 16/EB elements
-template <int UNROLL, int EB, int NT>
+template <int UNROLL, int EB, int NT, class PolX>
 __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* __restrict__ d,
                                               unsigned long long vbeg, unsigned long long vend,
-                                              unsigned int& overlaps, const Pol& pol, bool dead_src) {
+                                              unsigned int& overlaps, const PolX& pol, bool dead_src) {
   unsigned long long v = vbeg + threadIdx.x;
   auto join = [&](uint4 a, uint4 b) {
     const unsigned int cx = a.x & b.x, cy = a.y & b.y, cz = a.z & b.z, cw = a.w & b.w;   // elements whose sets overlap
@@ -278,8 +293,8 @@ __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* 
     uint4 a[UNROLL], b[UNROLL];
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) {
-      a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds);
-      b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd);
+      a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds, pol.l1);
+      b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd, pol.l1);
     }
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, join(a[j], b[j]), pol);
@@ -296,8 +311,8 @@ __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* 
       uint4 a[KK], b[KK];
 #pragma unroll
       for (int j = 0; j < KK; ++j) {
-        a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds);
-        b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd);
+        a[j] = ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds, pol.l1);
+        b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd, pol.l1);
       }
 #pragma unroll
       for (int j = 0; j < KK; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, join(a[j], b[j]), pol);
@@ -344,10 +359,10 @@ __device__ __noinline__ void report_bad_masks(unsigned long long* bad_ctr, unsig
 
 // SC / DC: the initial vectors of the source / destination rank, F: the full set; g0 = dst * n + f.off (the global
 // index of the flow's first element at its destination); reduce: OR with overlap detection, else assign.
-template <int UNROLL, int EB, int NT>
+template <int UNROLL, int EB, int NT, class PolX>
 __device__ __forceinline__ void range_mask_lazy(const char* __restrict__ s, char* __restrict__ d,
                                                 unsigned long long vbeg, unsigned long long vend, unsigned int& overlaps,
-                                                const Pol& pol, unsigned int flags, bool reduce, uint4 SC, uint4 DC, uint4 F,
+                                                const PolX& pol, unsigned int flags, bool reduce, uint4 SC, uint4 DC, uint4 F,
                                                 Ctrl* ctrl, unsigned long long g0) {
   const bool src_init = (flags & DFLOW_SRC_INIT) != 0u, dst_init = (flags & DFLOW_DST_INIT) != 0u;
   const bool fin = (flags & DFLOW_FINAL) != 0u, dead_src = (flags & DFLOW_DEAD_SRC) != 0u && !src_init;
@@ -371,8 +386,8 @@ __device__ __forceinline__ void range_mask_lazy(const char* __restrict__ s, char
     uint4 a[KK], b[KK];
 #pragma unroll
     for (int j = 0; j < KK; ++j) {
-      a[j] = src_init ? SC : ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds);
-      b[j] = !reduce ? Z : (dst_init ? DC : ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd));
+      a[j] = src_init ? SC : ld16(s + (v + j * (unsigned long long)NT) * 16, pol.lds, pol.l1);
+      b[j] = !reduce ? Z : (dst_init ? DC : ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd, pol.l1));
     }
 #pragma unroll
     for (int j = 0; j < KK; ++j) {
@@ -402,21 +417,21 @@ __device__ __forceinline__ void range_mask_lazy(const char* __restrict__ s, char
 
 // bf16 plans: a unit is 8 elements = 16 bytes in a rank buffer or 32 bytes in the fp32 shadow.
 template <int KIND>
-__device__ __forceinline__ void load8(const char* base, unsigned long long unit, float (&x)[8], unsigned long long pol) {
+__device__ __forceinline__ void load8(const char* base, unsigned long long unit, float (&x)[8], unsigned long long pol, unsigned int l1) {
   if (KIND == 0) {
-    uint4 r = ld16(base + unit * 16, pol);
+    uint4 r = ld16(base + unit * 16, pol, l1);
     x[0] = bf16_to_f32(r.x & 0xFFFFu); x[1] = bf16_to_f32(r.x >> 16);
     x[2] = bf16_to_f32(r.y & 0xFFFFu); x[3] = bf16_to_f32(r.y >> 16);
     x[4] = bf16_to_f32(r.z & 0xFFFFu); x[5] = bf16_to_f32(r.z >> 16);
     x[6] = bf16_to_f32(r.w & 0xFFFFu); x[7] = bf16_to_f32(r.w >> 16);
   } else {
-    uint4 r0 = ld16(base + unit * 32, pol), r1 = ld16(base + unit * 32 + 16, pol);
+    uint4 r0 = ld16(base + unit * 32, pol, l1), r1 = ld16(base + unit * 32 + 16, pol, l1);
     x[0] = __uint_as_float(r0.x); x[1] = __uint_as_float(r0.y); x[2] = __uint_as_float(r0.z); x[3] = __uint_as_float(r0.w);
     x[4] = __uint_as_float(r1.x); x[5] = __uint_as_float(r1.y); x[6] = __uint_as_float(r1.z); x[7] = __uint_as_float(r1.w);
   }
 }
-template <int KIND>
-__device__ __forceinline__ void store8(char* base, unsigned long long unit, const float (&x)[8], const Pol& pol) {
+template <int KIND, class PolX>
+__device__ __forceinline__ void store8(char* base, unsigned long long unit, const float (&x)[8], const PolX& pol) {
   if (KIND == 0) {
     uint4 r;
     r.x = f32_to_bf16_rne(x[0]) | (f32_to_bf16_rne(x[1]) << 16);
@@ -430,18 +445,18 @@ __device__ __forceinline__ void store8(char* base, unsigned long long unit, cons
   }
 }
 
-template <int KS, int KD, int KO, int NT>
+template <int KS, int KD, int KO, int NT, class PolX>
 __device__ __forceinline__ void range_add_bf16(const char* __restrict__ s, const char* __restrict__ din,
                                                char* __restrict__ dout, unsigned long long ubeg,
-                                               unsigned long long uend, const Pol& pol, bool dead_src) {
+                                               unsigned long long uend, const PolX& pol, bool dead_src) {
   constexpr int UNROLL = 2;
   unsigned long long u = ubeg + threadIdx.x;
   for (; u + (UNROLL - 1) * (unsigned long long)NT < uend; u += UNROLL * (unsigned long long)NT) {
     float a[UNROLL][8], b[UNROLL][8];
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) {
-      load8<KS>(s, u + j * (unsigned long long)NT, a[j], pol.lds);
-      load8<KD>(din, u + j * (unsigned long long)NT, b[j], pol.ldd);
+      load8<KS>(s, u + j * (unsigned long long)NT, a[j], pol.lds, pol.l1);
+      load8<KD>(din, u + j * (unsigned long long)NT, b[j], pol.ldd, pol.l1);
     }
 #pragma unroll
     for (int j = 0; j < UNROLL; ++j) {
@@ -459,8 +474,8 @@ __device__ __forceinline__ void range_add_bf16(const char* __restrict__ s, const
   }
   for (; u < uend; u += NT) {
     float a[8], b[8];
-    load8<KS>(s, u, a, pol.lds);
-    load8<KD>(din, u, b, pol.ldd);
+    load8<KS>(s, u, a, pol.lds, pol.l1);
+    load8<KD>(din, u, b, pol.ldd, pol.l1);
 #pragma unroll
     for (int e = 0; e < 8; ++e) b[e] = __fadd_rn(b[e], a[e]);
     store8<KO>(dout, u, b, pol);

@@ -48,9 +48,9 @@ def _check_full(w, k, exec_mode, n_samples=2048):
         y_or = OI.run_bf16_at(oplan, xs, idx)
         assert ys[0].tobytes() == y_or[0].tobytes() and ys[1].tobytes() == y_or[w.p - 1].tobytes()
         assert OR.check_bf16(OI.bf16_bits_to_f32(ys[0]), OI.bf16_bits_to_f32(xs)).all()
-    if exec_mode == B.OPTCC_EXEC_DATAFLOW:
+    if exec_mode in (B.OPTCC_EXEC_DATAFLOW, B.OPTCC_EXEC_COLUMN):
         # every element of every rank, device against device: the per-step executor (kernel boundaries as barriers, no
-        # dependency counters, no dead-source discard) must produce the same bits as the dataflow executor
+        # dependency counters, no dead-source discard) must produce the same bits as the dataflow / column executor
         plan2 = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=k, exec_mode=B.OPTCC_EXEC_PER_STEP)
         s2 = Session(plan2)
         s2.upload(x)
@@ -71,7 +71,7 @@ def test_c1_full_every_element():
     """configs[0] (p=4, l=2, n=2^20 f32) is small enough for the oracle to compute every element."""
     from paper_2606_01680_b200.device import Session
     w = W.config(0)
-    for mode in (B.OPTCC_EXEC_DATAFLOW, B.OPTCC_EXEC_PERSISTENT):
+    for mode in (B.OPTCC_EXEC_DATAFLOW, B.OPTCC_EXEC_PERSISTENT, B.OPTCC_EXEC_COLUMN):
         plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=BENCH_K[0], exec_mode=mode)
         oplan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=BENCH_K[0])
         x = W.all_inputs(w)
@@ -88,6 +88,13 @@ def test_c1_full_every_element():
 def test_c2_full_sampled():
     c = _check_full(W.config(1), BENCH_K[1], B.OPTCC_EXEC_DATAFLOW)
     assert c["T_over_T0"] < 1.06           # within the paper's reported gap
+
+
+@pytest.mark.parametrize("ci,k", [(1, 16), (2, 8), (3, 8), (1, 32)])
+def test_full_sampled_column_executor(ci, k):
+    """the column executor (one CTA runs a region's whole flow list on a tile, no inter-CTA synchronisation) at the
+    full sizes in its bench configuration: sampled elements against the oracle, every element against the per-step executor"""
+    _check_full(W.config(ci), k, B.OPTCC_EXEC_COLUMN, n_samples=1024)
 
 
 def test_c2_full_sampled_persistent_mode():

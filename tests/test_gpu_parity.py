@@ -19,7 +19,7 @@ from oracle import reference as OR
 
 pytestmark = pytest.mark.gpu
 
-MODES = [B.OPTCC_EXEC_PERSISTENT, B.OPTCC_EXEC_PER_STEP, B.OPTCC_EXEC_DATAFLOW]
+MODES = [B.OPTCC_EXEC_PERSISTENT, B.OPTCC_EXEC_PER_STEP, B.OPTCC_EXEC_DATAFLOW, B.OPTCC_EXEC_COLUMN]
 
 
 def _session(plan, verify=False):

@@ -59,8 +59,9 @@ def test_dataflow_random_plans(seed):
     assert res["bad_elements"] == 0 and res["overlap_elements"] == 0
 
 
+@pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_DATAFLOW, B.OPTCC_EXEC_COLUMN])
 @pytest.mark.parametrize("seed", range(16))
-def test_dataflow_random_midsize_plans(seed):
+def test_dataflow_random_midsize_plans(seed, exec_mode):
     """Mid-size plans (sections of several thousand 16-byte units, odd tile sizes): the full streaming rounds, the
     partially entered last rounds, the remainder batches and the dead-source discard all occur; outputs bit-equal to
     the oracle, masks complete, and the per-step executor agrees on every element."""
@@ -75,7 +76,7 @@ def test_dataflow_random_midsize_plans(seed):
     n = int(rng.integers(300_000, 1_500_000))
     k = int(rng.choice([4, 8]))
     tile = int(rng.choice([0, 1792, 3584, 1000, 5000, 3583]))
-    plan = B.optcc_plan(p, 1, ell, n, dtype, k=k, exec_mode=B.OPTCC_EXEC_DATAFLOW, tile_units=tile)
+    plan = B.optcc_plan(p, 1, ell, n, dtype, k=k, exec_mode=exec_mode, tile_units=tile)
     oplan = OP.build_plan(p, 1, ell, n, dtype, k=k)
     w = W.Workload("mid", p, 1, tuple(ell), n, dtype, "normal", 1.0, 9000 + seed)
     x = W.all_inputs(w)
@@ -90,16 +91,22 @@ def test_dataflow_random_midsize_plans(seed):
     assert s.masks().tobytes() == OI.element_masks(oplan)[0].tobytes()
 
 
-@pytest.mark.parametrize("seed", range(150))
+@pytest.mark.parametrize("seed", list(range(150)) + [f"column-{i}" for i in range(80)])
 def test_random_plans_any_executor_any_verifier(seed):
     """Random plans through a random executor, with the lazy or the eager verifier, complete or cut after a random
     step: outputs (complete schedules) bit-equal to the oracle; masks, number of wrong final masks, first wrong
-    index and overlap count equal to the oracle's walk of the same (possibly truncated) table."""
+    index and overlap count equal to the oracle's walk of the same (possibly truncated) table.  The "column-i" cases
+    run the column executor (twice on the same session: its ticket must reset cleanly)."""
     import dataclasses
     from paper_2606_01680_b200.device import Session
+    column = isinstance(seed, str)
+    if column:
+        seed = 500 + int(seed.split("-")[1])
     rng = np.random.default_rng(31337 + seed)
     p, g, ell, n, k, dtype, tile, grid, ordering = _random_case(rng)
     mode = int(rng.integers(0, 3))
+    if column:
+        mode = B.OPTCC_EXEC_COLUMN
     eager = int(rng.integers(0, 2))
     oplan = OP.build_plan(p, g, ell, n, dtype, k=k, ordering=ordering or 2)
     limit = 0
@@ -114,10 +121,11 @@ def test_random_plans_any_executor_any_verifier(seed):
     s = Session(plan, verify=True)
     if not limit:
         x = W.all_inputs(W.Workload("s", p, g, tuple(ell), n, dtype, "normal", 1.0, 77000 + seed))
-        s.upload(x)
-        s.execute()
         y_or = OI.run_f32(oplan, x) if dtype == W.F32 else OI.run_bf16(oplan, x)
-        assert s.download().tobytes() == y_or.tobytes()
+        for _ in range(2 if column else 1):
+            s.upload(x)
+            s.execute()
+            assert s.download().tobytes() == y_or.tobytes()
     else:
         oplan = dataclasses.replace(oplan, n_steps=limit)
     res = s.verify(raise_on_fail=False)
