@@ -42,8 +42,10 @@ def parse_args():
     ap.add_argument("--ell", type=float, default=1.6, help="ell for config 4 (the C5 sweep)")
     ap.add_argument("--k", type=int, default=-1,
                     help="segments (PAPER.md:124); -1 = bench default per config (16 for C2, see profiles/ k-sweep), 0 = planner's auto rule")
-    ap.add_argument("--exec-mode", type=int, default=2,
-                    help="2 dataflow kernel (default), 0 persistent kernel with grid barriers, 1 one launch per step")
+    ap.add_argument("--exec-mode", type=int, default=-1,
+                    help="-1 = bench default per config (BENCH_EXEC: the faster of the column and the dataflow executor, "
+                         "profiles/ executor table), 3 column kernel, 2 dataflow kernel, 0 persistent kernel with grid barriers, "
+                         "1 one launch per step")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--e2e-shards", type=int, default=16,
                     help="element shards of the end-to-end leg (optcc_execute_host_sharded: H2D, execute and D2H of "
@@ -52,10 +54,19 @@ def parse_args():
                     help="log2 of n per rank for the CPU-oracle sample (0 = 24 for the cpu_baseline leg, 22 per --impl reference step)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    return ap.parse_args()
+    a = ap.parse_args()
+    if a.exec_mode < 0:
+        a.exec_mode = BENCH_EXEC[a.config]
+    return a
 
 
 BENCH_K = {0: 8, 1: 16, 2: 8, 3: 8, 4: 8}   # per config; k is free in BASELINE.json's configs
+
+
+# executor per config: the column executor (no synchronisation between CTAs) where it is faster, the dataflow
+# executor for C4 (regions of ~1 k units: one small tile per region, 960 work items)
+BENCH_EXEC = {0: 3, 1: 3, 2: 3, 3: 2, 4: 3}
+EXEC_KERNEL = {0: "optcc_exec_kernel", 1: "optcc_exec_kernel", 2: "optcc_dataflow_kernel", 3: "optcc_column_kernel"}
 
 
 def bench_k(args):
@@ -370,7 +381,7 @@ def run_native(args):
         return 0
 
     peak, peak_src = measured_peak()
-    kname = "optcc_dataflow_kernel" if args.exec_mode == 2 else "optcc_exec_kernel"
+    kname = EXEC_KERNEL[args.exec_mode]
     kern = kname + ("<MODE_F32>" if w.dtype == W.F32 else "<MODE_BF16>")
     achieved = sched_bytes / t_exec / 1e6
     mask_bytes = 5 * (w.p - 1) * w.n * plan0.info["mask_bytes"]   # the same schedule on mask elements
@@ -381,7 +392,9 @@ def run_native(args):
         "data": "synthetic",
         "config": {"workload": workload_name(w, k), "step": "optcc_plan + optcc_cost + optcc_execute + optcc_verify (SURVEY 8(a) a1-a8)",
                    "exec_mode": {0: "persistent cooperative kernel, grid barrier per step", 1: "one launch per step",
-                                 2: "dataflow cooperative kernel: tile-ops in table order, per-range completion counters, no grid barrier"}[args.exec_mode],
+                                 2: "dataflow cooperative kernel: tile-ops in table order, per-range completion counters, no grid barrier",
+                                 3: "column kernel: a CTA runs a region's whole flow list on one tile in table order, no synchronisation "
+                                    "between CTAs (every dependency lies inside one element column)"}[args.exec_mode],
                    "plan_steps": plan0.info["n_steps"], "plan_flows": plan0.info["n_flows"], "parallelism": f"replicas x{world} (element-axis shards, no collective)",
                    "l2": "inputs larger than L2 (footprint %.2f GB) and restored from a pristine copy between steps, untimed" % (w.p * w.n * esize / 1e9)},
         "execute_only": {"algbw": world * w.n * esize / t_exec / 1e6, "unit": UNIT, "ms": t_exec,

@@ -265,14 +265,15 @@ def test_execute_host_roundtrip():
     (7, {0: 2.0, 1: 4.0 / 3.0}, 20011, W.F32, 4, 1),     # one shard: any n
     (130, {0: 2.0}, 1024, W.F32, 4, 2),                  # p > 128: the rank-pointer table is rewritten per shard
 ])
-def test_execute_host_sharded_equals_the_oracle_shard_by_shard(p, st, n, dtype, k, shards):
+@pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_DATAFLOW, B.OPTCC_EXEC_COLUMN])
+def test_execute_host_sharded_equals_the_oracle_shard_by_shard(p, st, n, dtype, k, shards, exec_mode):
     """optcc_execute_host_sharded: n_total = shards * n elements per rank, every shard an independent AllReduce with
     the one plan for n; the H2D / execute / D2H pipeline must give, shard by shard, exactly the oracle's plan-order
     result, and later work on the caller's stream must see the finished results."""
     import torch
     w = _wl(p, 1, st, n * shards, dtype, seed=77 + p)
     ell = list(w.ell)
-    plan = B.optcc_plan(p, 1, ell, n, dtype, k=k)
+    plan = B.optcc_plan(p, 1, ell, n, dtype, k=k, exec_mode=exec_mode)
     oplan = OP.build_plan(p, 1, ell, n, dtype, k=k)
     from paper_2606_01680_b200.device import Session
     s = Session(plan, shards=shards)
@@ -311,12 +312,13 @@ def test_execute_host_sharded_rejects_bad_shapes():
     assert e.value.name == "EINVAL"
 
 
-def test_execute_is_capturable_in_a_cuda_graph():
+@pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_DATAFLOW, B.OPTCC_EXEC_COLUMN])
+def test_execute_is_capturable_in_a_cuda_graph(exec_mode):
     """optcc_execute only enqueues work (two memsets and one cooperative launch once the tables are resident): it can
     be captured into a CUDA graph and replayed; every replay must reproduce the oracle's result."""
     import torch
     w = _wl(8, 1, {0: 2.0}, 2 ** 16 + 4, W.F32, seed=41)
-    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=4)
+    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=4, exec_mode=exec_mode)
     oplan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=4)
     x = W.all_inputs(w)
     y_or = OI.run_f32(oplan, x)
