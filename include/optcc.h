@@ -94,7 +94,8 @@ typedef struct optcc_opts {
                          copy by the streaming warps, 2 = cp.async.bulk (TMA 1-D) copy by the scheduler agents (dataflow only) */
   uint32_t step_limit;/* 0 = all steps; else execute / verify only the first step_limit steps (debugging and
                          profiling: a truncated schedule must FAIL verification) */
-  uint32_t tile_units;/* dataflow executor: 16-byte units per tile-op; 0 = auto (224..3584: about two tile-ops per CTA and step, whole streaming rounds) */
+  uint32_t tile_units;/* dataflow executor: 16-byte units per tile-op; 0 = auto (224..3584: about two tile-ops per CTA and step, whole streaming rounds).
+                         column executor: units per work item; 0 = auto (1792 for f32, 896 for bf16, at most the longest region) */
   uint32_t schedule;  /* OPTCC_SCHED_*: 0 = OPTCC (default), 1 = plain ring on the degraded topology (baseline) */
   uint32_t ordering;  /* stage ordering of PAPER.md:138 for one straggler, g = 1: 0 or 2 = ordering (2) S3->S1->S4->S2 (the
                          canonical plan, k+1 bodies), 1 = ordering (1) S1->S2->S3->S4 (PLAN_SPEC C1', k+3 bodies) */

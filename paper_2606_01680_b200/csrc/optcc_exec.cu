@@ -127,16 +127,18 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
     char* dout = f.kdout ? reinterpret_cast<char*>(P.shadow + (unsigned long long)f.dst * P.padded_n + f.off)
                          : rank_ptr(P, f.dst) + f.off * 2;
     if (f.op == 0) {
-      // (dead-source discard is off for bf16 plans: measured 3 % slower on C3, which is not DRAM-bound)
+      // (dead-source discard is off for bf16 plans in the dataflow executor: measured 3 % slower on C3, which is not
+      // DRAM-bound there; on in the column executor)
+      const bool bf_dead = PolX::l1 != 0 && dead_src;
       switch ((f.ksrc << 2) | (f.kdin << 1) | f.kdout) {
-        case 0: range_add_bf16<0, 0, 0, NT>(s, di, dout, vbeg, vend, pol, false); break;
-        case 1: range_add_bf16<0, 0, 1, NT>(s, di, dout, vbeg, vend, pol, false); break;
-        case 2: range_add_bf16<0, 1, 0, NT>(s, di, dout, vbeg, vend, pol, false); break;
-        case 3: range_add_bf16<0, 1, 1, NT>(s, di, dout, vbeg, vend, pol, false); break;
-        case 4: range_add_bf16<1, 0, 0, NT>(s, di, dout, vbeg, vend, pol, false); break;
-        case 5: range_add_bf16<1, 0, 1, NT>(s, di, dout, vbeg, vend, pol, false); break;
-        case 6: range_add_bf16<1, 1, 0, NT>(s, di, dout, vbeg, vend, pol, false); break;
-        default: range_add_bf16<1, 1, 1, NT>(s, di, dout, vbeg, vend, pol, false); break;
+        case 0: range_add_bf16<0, 0, 0, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
+        case 1: range_add_bf16<0, 0, 1, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
+        case 2: range_add_bf16<0, 1, 0, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
+        case 3: range_add_bf16<0, 1, 1, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
+        case 4: range_add_bf16<1, 0, 0, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
+        case 5: range_add_bf16<1, 0, 1, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
+        case 6: range_add_bf16<1, 1, 0, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
+        default: range_add_bf16<1, 1, 1, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
       }
     } else if (f.ksrc == 0) {
       range_copy16<4, NT>(s, dout, vbeg, vend, pol);                 // bf16 -> bf16: one vector per unit
@@ -558,6 +560,7 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
         prev_cls = cls;
       }
       process_piece<MODE, COL_THREADS>(P, cur, ubeg, uend, overlaps, pol);
+      __syncwarp();   // orders a lane's dead-source discard of a 128-byte line before the other lanes' later stores to it
       cur = nxt;
       nxt = nn;
     }
@@ -766,6 +769,33 @@ void assign_mask_flags(optcc_plan_t* pl, optcc_exec_state* st) {
   st->lazy_masks = true;
 }
 
+// Dead-source flags without the dataflow tables (column executor): flow i is the only reader of its source range since
+// the last write and the next access to that (rank, region) is a plain overwrite by a copy flow -- the same rule as in
+// build_dataflow_tables.
+void assign_dead_source_flags(optcc_plan_t* pl, optcc_exec_state* st) {
+  const optcc_plan_info_t& in = pl->info;
+  if (pl->opts.no_discard || pl->opts.step_limit) return;
+  const size_t nr = pl->region_offs.size();
+  std::vector<uint32_t> readers(size_t(in.p) * nr, 0);
+  std::vector<uint8_t> sole_reader(in.n_flows, 0);
+  for (uint32_t i = 0; i < in.n_flows; ++i) {
+    const optcc_flow_t& f = pl->flows[i];
+    const size_t reg = pl->flow_region[i];
+    sole_reader[i] = readers[size_t(f.src) * nr + reg]++ == 0;
+    readers[size_t(f.dst) * nr + reg] = 0;
+  }
+  enum : uint8_t { NEXT_NONE = 0, NEXT_READ, NEXT_COPY_WRITE, NEXT_REDUCE_WRITE };
+  std::vector<uint8_t> next(size_t(in.p) * nr, NEXT_NONE);
+  for (uint32_t i = in.n_flows; i-- > 0;) {
+    const optcc_flow_t& f = pl->flows[i];
+    const size_t reg = pl->flow_region[i];
+    const size_t ls = size_t(f.src) * nr + reg, ld = size_t(f.dst) * nr + reg;
+    if (f.op == OPTCC_OP_REDUCE && next[ls] == NEXT_COPY_WRITE && sole_reader[i]) st->dflows[i].flags |= 1u;
+    next[ld] = f.op == OPTCC_OP_COPY ? NEXT_COPY_WRITE : NEXT_REDUCE_WRITE;
+    next[ls] = NEXT_READ;
+  }
+}
+
 // Column executor tables: the flows of the executed steps region by region (a stable counting sort of the table by
 // region, so table order is kept inside a region) and one work item per (region, tile).
 void build_column_tables(optcc_plan_t* pl, optcc_exec_state* st) {
@@ -899,7 +929,10 @@ int build_state(optcc_plan_t* pl) {
     if (pl->opts.exec_mode == OPTCC_EXEC_DATAFLOW && st->coop && st->G_df > 0) build_dataflow_tables(pl, st);
     assign_mask_flags(pl, st);
     st->column = pl->opts.exec_mode == OPTCC_EXEC_COLUMN && pl->tiles_per_rank < (uint64_t(1) << 32);
-    if (st->column) build_column_tables(pl, st);
+    if (st->column) {
+      assign_dead_source_flags(pl, st);
+      build_column_tables(pl, st);
+    }
     // slice table: cut every step into G slices of equal HBM bytes
     st->slices.clear();
     if (!st->df_ok && !st->column) st->slices.assign(size_t(in.n_steps) * (G + 1), Slice{0, 0, 0});

@@ -387,9 +387,10 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
       pl->tile_units = pl->opts.tile_units;
     } else if (pl->opts.exec_mode == OPTCC_EXEC_COLUMN) {
       // column executor: a CTA runs a region's whole flow list on one tile, so the tile size does not depend on the
-      // number of steps.  Measured on a B200: 3 vectors per thread (1344 units) for f32, 2 (896) for
-      // bf16 plans, whose fp32 shadow triples the bytes per unit; a region shorter than that is one tile.
-      uint32_t tu = dtype == OPTCC_BF16 ? 896 : 1344;
+      // number of steps.  One whole streaming round of the CTA (448 threads x 4 vectors = 1792 units for f32, x 2
+      // units = 896 for bf16 plans, whose fp32 shadow triples the bytes per unit): whole rounds are what the
+      // dead-source discard acts on (measured on a B200); a region shorter than that is one tile.
+      uint32_t tu = dtype == OPTCC_BF16 ? 896 : 1792;
       uint64_t longest = 0;
       for (size_t i = 0; i + 1 < pl->sec_bounds.size(); ++i) longest = std::max(longest, pl->sec_bounds[i + 1] - pl->sec_bounds[i]);
       for (size_t i = 0; i + 1 < pl->p2p_bounds.size(); ++i) longest = std::max(longest, pl->p2p_bounds[i + 1] - pl->p2p_bounds[i]);

@@ -182,3 +182,22 @@ def test_modeled_time_within_the_papers_gap_on_every_config(ci, ell, k, gap):
     lb = c["lb_table1"] if math.isnan(c["lb_tight"]) else c["lb_tight"]
     assert c["T"] / lb <= gap
     assert c["T"] <= c["T_closed_form"] * (1 + 1e-3)      # never above the paper's own finite-k form (up to unit rounding)
+
+
+@pytest.mark.parametrize("ci,k", [(0, 8), (1, 16), (2, 8), (3, 8), (4, 8)])
+def test_column_executor_plans_are_the_same_tables(ci, k):
+    """exec_mode only selects the executor: the plan tables, the cost and the mask layout of a column-executor plan are
+    those of the default plan; its workspace additionally holds one work item per (region, tile)."""
+    from paper_2606_01680_b200 import workloads as W
+    w = W.config(ci)
+    n = min(w.n, 2 ** 20)
+    a = B.optcc_plan(w.p, w.g, w.ell, n, w.dtype, k=k)
+    b = B.optcc_plan(w.p, w.g, w.ell, n, w.dtype, k=k, exec_mode=B.OPTCC_EXEC_COLUMN)
+    ta, tb = B.optcc_plan_tables(a), B.optcc_plan_tables(b)
+    for x, y in zip(ta, tb):
+        assert np.asarray(x).tobytes() == np.asarray(y).tobytes()
+    ia, ib = a.info, b.info
+    for key in ("n_steps", "n_flows", "k", "mask_bytes", "lazy_verify", "padded_n", "reduce_elems", "copy_elems"):
+        assert ia[key] == ib[key]
+    assert ib["workspace_bytes"] % 256 == 0 and ib["verify_workspace_bytes"] >= ib["workspace_bytes"]
+    assert B.optcc_cost(a)["T"] == B.optcc_cost(b)["T"]
