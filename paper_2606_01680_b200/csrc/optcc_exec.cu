@@ -498,25 +498,26 @@ __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefe
 // the vectors it will load itself (NT-strided, like the range operations).  f32 and bf16 data only: the verifier's
 // first touches are constants.
 template <int MODE, int NT>
-__device__ __forceinline__ void prefetch_operands(const ExecParams& P, const DFlow& f, unsigned int cur_dst,
+__device__ __forceinline__ void prefetch_operands(const ExecParams& P, const DFlow& f, unsigned int w0,
                                                   unsigned long long ubeg, unsigned long long uend) {
   if (is_mask_mode(MODE)) return;
-  auto span = [&](const char* base, unsigned int bytes_per_unit) {
-    for (unsigned long long u = ubeg + threadIdx.x; u < uend; u += NT) prefetch_l1(base + u * bytes_per_unit);
+  const unsigned int n = (unsigned int)(uend - ubeg);   // (a tile: far below 2^32 units)
+  auto span = [&](const char* base) {
+    const char* q = base + (ubeg + threadIdx.x) * 16;
+    for (unsigned int u = threadIdx.x; u < n; u += NT, q += NT * 16) prefetch_l1(q);
   };
-  if (MODE == MODE_F32) {
-    if (f.src != cur_dst) span(rank_ptr(P, f.src) + f.off * 4, 16);
-    if (f.op == 0 && f.dst != cur_dst) span(rank_ptr(P, f.dst) + f.off * 4, 16);
-  } else {
-    // raw bf16 operands only (partial sums in the shadow were written by this CTA a moment ago)
-    if (f.src != cur_dst && f.ksrc == 0) span(rank_ptr(P, f.src) + f.off * 2, 16);
-    if (f.op == 0 && f.dst != cur_dst && f.kdin == 0) span(rank_ptr(P, f.dst) + f.off * 2, 16);
-  }
+  const unsigned int esz = MODE == MODE_F32 ? 4 : 2;
+  // (bf16 plans: raw operands only -- partial sums in the shadow were written by this CTA a moment ago)
+  if (f.src != w0 && (MODE == MODE_F32 || f.ksrc == 0)) span(rank_ptr(P, f.src) + f.off * esz);
+  if (f.op == 0 && f.dst != w0 && (MODE == MODE_F32 || f.kdin == 0)) span(rank_ptr(P, f.dst) + f.off * esz);
 }
+
+constexpr unsigned int COL_REC = 128;   // flow records staged in shared memory at a time (4 KB)
 
 template <int MODE>
 __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(const __grid_constant__ ExecParams P) {
   __shared__ unsigned long long s_item;
+  __shared__ __align__(16) DFlow s_rec[COL_REC];   // this CTA's staged part of the region's flow list
   unsigned int overlaps = 0;
   // A tile is private to its CTA for the whole launch, so loads and stores go through L1 (PolL1): the value a flow
   // stores is the next flow's source.  L2 policies all evict_normal (a dirty line marked evict_first is written back).
@@ -524,45 +525,53 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
   PolL1 pol;
   pol.lds = pol0.lds; pol.ldd = pol0.ldd; pol.st = pol0.st;
   const unsigned long long A = P.unit_elems;
-  auto fetch = [&](unsigned int i) {
-    DFlow f;
-    const uint4* fr = reinterpret_cast<const uint4*>(P.flows + i);
-    const uint4 f0 = __ldg(fr), f1 = __ldg(fr + 1);
-    memcpy(&f, &f0, 16);
-    memcpy(reinterpret_cast<char*>(&f) + 16, &f1, 16);
-    return f;
-  };
   for (;;) {
-    __syncthreads();                 // every thread has read the previous item
+    __syncthreads();                 // every thread has read the previous item (and its last records)
     if (threadIdx.x == 0) s_item = atomicAdd(&P.ctrl->ticket, 1ull);
     __syncthreads();
     const unsigned long long it = s_item;
     if (it >= P.col_n_items) break;
     const uint2 item = __ldg(P.col_items + it);   // (region, tile)
     const unsigned int fb = __ldg(P.col_reg_begin + item.x), fe = __ldg(P.col_reg_begin + item.x + 1);
-    const unsigned long long ubeg = (unsigned long long)item.y * P.tile_units;
     if (fb >= fe) continue;
+    // all flows over a region have the same length (PLAN_SPEC 5.4): the tile's unit range is fixed for the item
+    const unsigned long long len = __ldg(&P.flows[fb].len), nunits = (len + A - 1) / A;
+    const unsigned long long ubeg = (unsigned long long)item.y * P.tile_units;
+    const unsigned long long uend = ubeg + P.tile_units < nunits ? ubeg + P.tile_units : nunits;
     int prev_cls = -1;
-    // records i and i + 1 are resident at the top of iteration i; record i + 2 is requested there
-    DFlow cur = fetch(fb), nxt = cur;
-    if (fb + 1 < fe) nxt = fetch(fb + 1);
-    for (unsigned int i = fb; i < fe; ++i) {
-      DFlow nn = nxt;
-      if (i + 2 < fe) nn = fetch(i + 2);
-      const unsigned long long nunits = (cur.len + A - 1) / A;   // (all flows over a region have the same length)
-      const unsigned long long uend = ubeg + P.tile_units < nunits ? ubeg + P.tile_units : nunits;
-      if (i + 1 < fe) prefetch_operands<MODE, COL_THREADS>(P, nxt, cur.dst, ubeg, uend);
-      if (MODE == MODE_BF16) {
-        // a copy of fp32 partials moves two vectors per unit, thread i taking vector i instead of unit i: when the
-        // thread-to-element mapping changes between consecutive flows the CTA synchronises (block-wide ordering)
-        const int cls = (cur.op == 1 && cur.ksrc != 0) ? 1 : 0;
-        if (prev_cls >= 0 && cls != prev_cls) __syncthreads();
-        prev_cls = cls;
+    for (unsigned int base = fb; base < fe; base += COL_REC) {
+      const unsigned int cnt = fe - base < COL_REC ? fe - base : COL_REC;
+      if (base != fb) __syncthreads();             // the previous records have been read by every thread
+      for (unsigned int t = threadIdx.x; t < 2 * cnt; t += COL_THREADS)
+        reinterpret_cast<uint4*>(s_rec)[t] = __ldg(reinterpret_cast<const uint4*>(P.flows + base) + t);
+      __syncthreads();
+      auto run_flow = [&](const DFlow& cur, const DFlow& nxt, bool has_next) {
+        // the raw operands of the next flow (a ring hop's destination is the next rank's untouched section: a DRAM
+        // first touch) are requested while this one streams -- not the range this flow writes
+        if (has_next) prefetch_operands<MODE, COL_THREADS>(P, nxt, cur.dst, ubeg, uend);
+        if (MODE == MODE_BF16) {
+          // a copy of fp32 partials moves two vectors per unit, thread i taking vector i instead of unit i: when the
+          // thread-to-element mapping changes between consecutive flows the CTA synchronises (block-wide ordering)
+          const int cls = (cur.op == 1 && cur.ksrc != 0) ? 1 : 0;
+          if (prev_cls >= 0 && cls != prev_cls) __syncthreads();
+          prev_cls = cls;
+        }
+        process_piece<MODE, COL_THREADS>(P, cur, ubeg, uend, overlaps, pol);
+        __syncwarp();   // orders a lane's dead-source discard of a 128-byte line before the other lanes' later stores to it
+      };
+      if (is_mask_mode(MODE)) {
+        // the verifier is bound by instruction issue (ncu: 79 % of the issue slots): records are read in place
+        for (unsigned int j = 0; j < cnt; ++j) run_flow(s_rec[j], s_rec[j], false);
+      } else {
+        // data: the next record is in registers before its flow starts (its loads issue without waiting for shared memory)
+        DFlow cur = s_rec[0];
+        for (unsigned int j = 0; j < cnt; ++j) {
+          const bool has_next = j + 1 < cnt;
+          const DFlow nxt = s_rec[has_next ? j + 1 : j];
+          run_flow(cur, nxt, has_next);
+          cur = nxt;
+        }
       }
-      process_piece<MODE, COL_THREADS>(P, cur, ubeg, uend, overlaps, pol);
-      __syncwarp();   // orders a lane's dead-source discard of a 128-byte line before the other lanes' later stores to it
-      cur = nxt;
-      nxt = nn;
     }
   }
   if (is_mask_mode(MODE)) {
