@@ -524,20 +524,17 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
   const Pol pol0 = make_policies(P.l2_hints);
   PolL1 pol;
   pol.lds = pol0.lds; pol.ldd = pol0.ldd; pol.st = pol0.st;
-  const unsigned long long A = P.unit_elems;
   for (;;) {
     __syncthreads();                 // every thread has read the previous item (and its last records)
     if (threadIdx.x == 0) s_item = atomicAdd(&P.ctrl->ticket, 1ull);
     __syncthreads();
     const unsigned long long it = s_item;
     if (it >= P.col_n_items) break;
-    const uint2 item = __ldg(P.col_items + it);   // (region, tile)
-    const unsigned int fb = __ldg(P.col_reg_begin + item.x), fe = __ldg(P.col_reg_begin + item.x + 1);
-    if (fb >= fe) continue;
-    // all flows over a region have the same length (PLAN_SPEC 5.4): the tile's unit range is fixed for the item
-    const unsigned long long len = __ldg(&P.flows[fb].len), nunits = (len + A - 1) / A;
-    const unsigned long long ubeg = (unsigned long long)item.y * P.tile_units;
-    const unsigned long long uend = ubeg + P.tile_units < nunits ? ubeg + P.tile_units : nunits;
+    // one record per item: the region's flows [fb, fe), the tile and its length in units (all flows over a region have
+    // the same length, PLAN_SPEC 5.4, so the tile's unit range is fixed for the item)
+    const uint4 item = __ldg(P.col_items + it);
+    const unsigned int fb = item.x, fe = item.y;
+    const unsigned long long ubeg = (unsigned long long)item.z * P.tile_units, uend = ubeg + item.w;
     int prev_cls = -1;
     for (unsigned int base = fb; base < fe; base += COL_REC) {
       const unsigned int cnt = fe - base < COL_REC ? fe - base : COL_REC;
@@ -673,7 +670,7 @@ struct optcc_exec_state {
   bool column = false;
   std::vector<DFlow> col_dflows;         // the executed flows, region by region (table order inside a region)
   std::vector<uint32_t> col_reg_begin;   // [regions + 1]
-  std::vector<uint2> col_items;          // (region, tile)
+  std::vector<uint4> col_items;          // (first flow, end flow, tile, units in the tile)
 };
 
 void optcc_exec_state_free(optcc_exec_state* s) { delete s; }
@@ -823,10 +820,14 @@ void build_column_tables(optcc_plan_t* pl, optcc_exec_state* st) {
   st->col_items.reserve(pl->tiles_per_rank);
   for (size_t r = 0; r < nr; ++r) {
     const uint64_t t0 = pl->region_tile0[r], t1 = r + 1 < nr ? pl->region_tile0[r + 1] : pl->tiles_per_rank;
-    if (st->col_reg_begin[r] == st->col_reg_begin[r + 1]) continue;   // no executed flow touches the region
-    for (uint64_t t = 0; t < t1 - t0; ++t) st->col_items.push_back(make_uint2((unsigned int)r, (unsigned int)t));
+    const uint32_t fb = st->col_reg_begin[r], fe = st->col_reg_begin[r + 1];
+    if (fb == fe) continue;   // no executed flow touches the region
+    const uint64_t nunits = (st->col_dflows[fb].len + A - 1) / A;
+    for (uint64_t t = 0; t < t1 - t0; ++t) {
+      const uint64_t ubeg = t * TU, left = nunits > ubeg ? nunits - ubeg : 0;
+      st->col_items.push_back(make_uint4(fb, fe, (unsigned int)t, (unsigned int)std::min<uint64_t>(left, TU)));
+    }
   }
-  (void)A; (void)TU;
 }
 
 template <int MODE>
@@ -985,9 +986,7 @@ int upload_tables(optcc_plan_t* pl, void* workspace, cudaStream_t stream, bool f
     if (!st->col_dflows.empty())
       CU_TRY(cudaMemcpyAsync(ws + L.dflows, st->col_dflows.data(), st->col_dflows.size() * sizeof(DFlow), cudaMemcpyHostToDevice, stream));
     if (!st->col_items.empty())
-      CU_TRY(cudaMemcpyAsync(ws + L.col, st->col_items.data(), st->col_items.size() * sizeof(uint2), cudaMemcpyHostToDevice, stream));
-    CU_TRY(cudaMemcpyAsync(ws + L.col + pl->tiles_per_rank * 8, st->col_reg_begin.data(), st->col_reg_begin.size() * sizeof(uint32_t),
-                           cudaMemcpyHostToDevice, stream));
+      CU_TRY(cudaMemcpyAsync(ws + L.col, st->col_items.data(), st->col_items.size() * sizeof(uint4), cudaMemcpyHostToDevice, stream));
   } else if (!st->dflows.empty())
     CU_TRY(cudaMemcpyAsync(ws + L.dflows, st->dflows.data(), st->dflows.size() * sizeof(DFlow), cudaMemcpyHostToDevice, stream));
   if (!st->slices.empty())
@@ -1067,8 +1066,7 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   P.deps = reinterpret_cast<const DDep*>(ws + L.deps);
   P.ops = reinterpret_cast<const TileOp*>(ws + L.ops);
   P.counters = reinterpret_cast<unsigned int*>(ws + L.counters);
-  P.col_items = reinterpret_cast<const uint2*>(ws + L.col);
-  P.col_reg_begin = reinterpret_cast<const unsigned int*>(ws + L.col + pl->tiles_per_rank * 8);
+  P.col_items = reinterpret_cast<const uint4*>(ws + L.col);
   P.col_n_items = 0;
   P.tile_units = pl->tile_units;
   P.bulk_copy = pl->opts.copy_path == 2 ? 1u : 0u;

@@ -66,8 +66,8 @@ static inline optcc_ws_layout optcc_layout(const optcc_plan_t* pl) {
   L.slices = optcc_align256(L.dflows + uint64_t(in.n_flows) * OPTCC_DFLOW_BYTES);
   L.deps = optcc_align256(L.slices + uint64_t(in.n_steps) * (OPTCC_MAX_GRID + 1) * OPTCC_SLICE_BYTES);
   L.ops = optcc_align256(L.deps + uint64_t(in.n_flows) * OPTCC_DEP_BYTES);
-  L.col = optcc_align256(L.ops + pl->n_tile_ops * OPTCC_OP_BYTES);   // column executor: items (8 B per (region, tile)), then region -> first flow (4 B)
-  L.counters = optcc_align256(L.col + pl->tiles_per_rank * 8 + (uint64_t(pl->region_offs.size()) + 1) * 4);
+  L.col = optcc_align256(L.ops + pl->n_tile_ops * OPTCC_OP_BYTES);   // column executor: work items, 16 B per (region, tile)
+  L.counters = optcc_align256(L.col + pl->tiles_per_rank * 16);
   L.shadow = optcc_align256(L.counters + uint64_t(in.p) * pl->tiles_per_rank * 4);
   uint64_t n_pad = (in.n + 7) & ~uint64_t(7);
   L.end_exec = optcc_align256(L.shadow + (in.dtype == OPTCC_BF16 ? uint64_t(in.p) * n_pad * 4 : 0));

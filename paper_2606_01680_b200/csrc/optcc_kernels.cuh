@@ -97,8 +97,7 @@ struct ExecParams {
   unsigned int tile_units;
   unsigned int df_slots;          // ring depth: tile-ops a CTA holds (claimed, waiting or streaming), <= DF_SLOTS
   // column executor: flows are stored region by region (table order inside a region)
-  const uint2* col_items;         // [col_n_items] (region, tile)
-  const unsigned int* col_reg_begin;   // [regions + 1] first flow of every region in `flows`
+  const uint4* col_items;         // [col_n_items] (first flow, end flow of the region in `flows`, tile, units in the tile)
   unsigned long long col_n_items;
   unsigned int bulk_copy;         // 1: copy tile-ops are moved by the scheduler agents with cp.async.bulk
   unsigned int l2_hints;          // kind(src loads) + 4 kind(dst loads) + 16 kind(stores); kind: 0 normal, 1 evict_first, 2 evict_last
