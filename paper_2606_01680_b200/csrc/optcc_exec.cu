@@ -804,7 +804,7 @@ void assign_dead_source_flags(optcc_plan_t* pl, optcc_exec_state* st) {
 
 // Column executor tables: the flows of the executed steps region by region (a stable counting sort of the table by
 // region, so table order is kept inside a region) and one work item per (region, tile).
-void build_column_tables(optcc_plan_t* pl, optcc_exec_state* st) {
+bool build_column_tables(optcc_plan_t* pl, optcc_exec_state* st) {   // false: PLAN_SPEC 5.4 violated (a planner bug)
   const optcc_plan_info_t& in = pl->info;
   const uint64_t A = in.unit_elems, TU = pl->tile_units;
   const size_t nr = pl->region_offs.size();
@@ -822,12 +822,15 @@ void build_column_tables(optcc_plan_t* pl, optcc_exec_state* st) {
     const uint64_t t0 = pl->region_tile0[r], t1 = r + 1 < nr ? pl->region_tile0[r + 1] : pl->tiles_per_rank;
     const uint32_t fb = st->col_reg_begin[r], fe = st->col_reg_begin[r + 1];
     if (fb == fe) continue;   // no executed flow touches the region
+    for (uint32_t i = fb + 1; i < fe; ++i)
+      if (st->col_dflows[i].len != st->col_dflows[fb].len || st->col_dflows[i].off != st->col_dflows[fb].off) return false;
     const uint64_t nunits = (st->col_dflows[fb].len + A - 1) / A;
     for (uint64_t t = 0; t < t1 - t0; ++t) {
       const uint64_t ubeg = t * TU, left = nunits > ubeg ? nunits - ubeg : 0;
       st->col_items.push_back(make_uint4(fb, fe, (unsigned int)t, (unsigned int)std::min<uint64_t>(left, TU)));
     }
   }
+  return true;
 }
 
 template <int MODE>
@@ -941,7 +944,7 @@ int build_state(optcc_plan_t* pl) {
     st->column = pl->opts.exec_mode == OPTCC_EXEC_COLUMN && pl->tiles_per_rank < (uint64_t(1) << 32);
     if (st->column) {
       assign_dead_source_flags(pl, st);
-      build_column_tables(pl, st);
+      if (!build_column_tables(pl, st)) { st->G = 0; return OPTCC_EINVAL; }   // (G = 0: the state is rebuilt on the next call)
     }
     // slice table: cut every step into G slices of equal HBM bytes
     st->slices.clear();

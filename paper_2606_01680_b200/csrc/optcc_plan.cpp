@@ -63,15 +63,6 @@ struct Builder {
 
 inline uint32_t modH(int64_t x, int64_t H) { int64_t r = x % H; return (uint32_t)(r < 0 ? r + H : r); }
 
-bool flow_less(const optcc_flow_t& a, const optcc_flow_t& b) {
-  if (a.step != b.step) return a.step < b.step;
-  if (a.link != b.link) return a.link < b.link;
-  if (a.stage != b.stage) return a.stage < b.stage;
-  if (a.src != b.src) return a.src < b.src;
-  if (a.dst != b.dst) return a.dst < b.dst;
-  return a.off < b.off;
-}
-
 // Run body(i) for i in [0, n) on a few host threads when the table is large enough to pay for them; the
 // iterations are independent (each sorts or moves a disjoint range).
 template <class F>
