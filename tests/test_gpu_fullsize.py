@@ -90,7 +90,7 @@ def test_c2_full_sampled():
     assert c["T_over_T0"] < 1.06           # within the paper's reported gap
 
 
-@pytest.mark.parametrize("ci,k", [(1, 16), (2, 8), (3, 8), (1, 32)])
+@pytest.mark.parametrize("ci,k", [(1, 16), (2, 8), (3, 8), (4, 8), (1, 32)])
 def test_full_sampled_column_executor(ci, k):
     """the column executor (one CTA runs a region's whole flow list on a tile, no inter-CTA synchronisation) at the
     full sizes in its bench configuration: sampled elements against the oracle, every element against the per-step executor"""
