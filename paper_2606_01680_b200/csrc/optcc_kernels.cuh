@@ -358,12 +358,15 @@ __device__ __noinline__ void report_bad_masks(unsigned long long* bad_ctr, unsig
 
 // SC / DC: the initial vectors of the source / destination rank, F: the full set; g0 = dst * n + f.off (the global
 // index of the flow's first element at its destination); reduce: OR with overlap detection, else assign.
-template <int UNROLL, int EB, int NT, class PolX>
-__device__ __forceinline__ void range_mask_lazy(const char* __restrict__ s, char* __restrict__ d,
-                                                unsigned long long vbeg, unsigned long long vend, unsigned int& overlaps,
-                                                const PolX& pol, unsigned int flags, bool reduce, uint4 SC, uint4 DC, uint4 F,
-                                                Ctrl* ctrl, unsigned long long g0) {
-  const bool src_init = (flags & DFLOW_SRC_INIT) != 0u, dst_init = (flags & DFLOW_DST_INIT) != 0u;
+// SRC_INIT: the source is the constant SC; DSTM: 0 = copy (no destination operand), 1 = reduce with the destination
+// loaded, 2 = reduce with the destination constant DC -- compile-time, so the constants are used in place (the
+// verifier is bound by instruction issue, and selecting them at run time cost a register fill per vector).
+template <int UNROLL, int EB, int NT, bool SRC_INIT, int DSTM, class PolX>
+__device__ __forceinline__ void range_mask_lazy_t(const char* __restrict__ s, char* __restrict__ d,
+                                                  unsigned long long vbeg, unsigned long long vend, unsigned int& overlaps,
+                                                  const PolX& pol, unsigned int flags, uint4 SC, uint4 DC, uint4 F,
+                                                  Ctrl* ctrl, unsigned long long g0) {
+  constexpr bool src_init = SRC_INIT, dst_init = DSTM == 2, reduce = DSTM != 0;
   const bool fin = (flags & DFLOW_FINAL) != 0u, dead_src = (flags & DFLOW_DEAD_SRC) != 0u && !src_init;
   auto join = [&](uint4 a, uint4 b) {
     const unsigned int cx = a.x & b.x, cy = a.y & b.y, cz = a.z & b.z, cw = a.w & b.w;   // elements whose sets overlap
@@ -411,6 +414,24 @@ __device__ __forceinline__ void range_mask_lazy(const char* __restrict__ s, char
   if (v < vend) {
     const unsigned int rem = (unsigned int)((vend - v + NT - 1) / NT);
     remainder_dispatch<UNROLL>(rem, [&](auto K) { batch(v, K); });
+  }
+}
+
+template <int UNROLL, int EB, int NT, class PolX>
+__device__ __forceinline__ void range_mask_lazy(const char* __restrict__ s, char* __restrict__ d,
+                                                unsigned long long vbeg, unsigned long long vend, unsigned int& overlaps,
+                                                const PolX& pol, unsigned int flags, bool reduce, uint4 SC, uint4 DC, uint4 F,
+                                                Ctrl* ctrl, unsigned long long g0) {
+  const bool src_init = (flags & DFLOW_SRC_INIT) != 0u;
+  const int dm = !reduce ? 0 : ((flags & DFLOW_DST_INIT) != 0u ? 2 : 1);
+  if (src_init) {
+    if (dm == 0) range_mask_lazy_t<UNROLL, EB, NT, true, 0>(s, d, vbeg, vend, overlaps, pol, flags, SC, DC, F, ctrl, g0);
+    else if (dm == 1) range_mask_lazy_t<UNROLL, EB, NT, true, 1>(s, d, vbeg, vend, overlaps, pol, flags, SC, DC, F, ctrl, g0);
+    else range_mask_lazy_t<UNROLL, EB, NT, true, 2>(s, d, vbeg, vend, overlaps, pol, flags, SC, DC, F, ctrl, g0);
+  } else {
+    if (dm == 0) range_mask_lazy_t<UNROLL, EB, NT, false, 0>(s, d, vbeg, vend, overlaps, pol, flags, SC, DC, F, ctrl, g0);
+    else if (dm == 1) range_mask_lazy_t<UNROLL, EB, NT, false, 1>(s, d, vbeg, vend, overlaps, pol, flags, SC, DC, F, ctrl, g0);
+    else range_mask_lazy_t<UNROLL, EB, NT, false, 2>(s, d, vbeg, vend, overlaps, pol, flags, SC, DC, F, ctrl, g0);
   }
 }
 
