@@ -109,7 +109,10 @@ def test_c4_full_sampled_multi_gpu_servers():
     _check_full(W.config(3), BENCH_K[3], B.OPTCC_EXEC_DATAFLOW)
 
 
-@pytest.mark.parametrize("ell", [1.0, 1.6, 2.0 - 1.0 / 31.0, 3.0])
-def test_c5_full_sampled(ell):
-    """both lower-bound regimes of the C5 sweep: no straggler, bubble filling, the Thm-1 switch, straggler-bound"""
-    _check_full(W.config(4, ell), BENCH_K[4], B.OPTCC_EXEC_DATAFLOW, n_samples=1024)
+@pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_COLUMN, B.OPTCC_EXEC_DATAFLOW])
+@pytest.mark.parametrize("ell", W.C5_ELLS)
+def test_c5_full_sampled(ell, exec_mode):
+    """every ell of the C5 sweep (BASELINE.json configs[4]) at n = 2^25, through the executor bench.py times (column)
+    and the dataflow executor: no straggler (C0 ring), bubble filling at 8/7, 4/3, 1.6, the Thm-1 switch 2 - 1/31,
+    the algorithm's own switch ell = 2 where bubble filling turns off, and the straggler-bound regime"""
+    _check_full(W.config(4, ell), BENCH_K[4], exec_mode, n_samples=1024)

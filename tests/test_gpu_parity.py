@@ -472,3 +472,70 @@ def test_truncated_schedule_midsize_masks_equal_oracle():
     m_or, _ = OI.element_masks(dataclasses.replace(oplan, n_steps=limit))
     assert s.masks().tobytes() == m_or.tobytes()
     assert res["bad_elements"] == int((m_or != OI.full_mask_words(p)[None, None, :]).any(axis=2).sum()) > 0
+
+
+def _oracle_prefix(oplan, limit):
+    """the oracle's plan cut after `limit` steps: the table rows of steps < limit (PLAN_SPEC 3: step_begin)"""
+    import dataclasses
+    return dataclasses.replace(oplan, n_steps=limit, flows=oplan.flows[:int(oplan.step_begin[limit])],
+                               step_begin=oplan.step_begin[:limit + 1])
+
+
+TRUNC_CASES = [
+    # p, g, stragglers, n, k, tile_units (0 = auto): sizes that reach full streaming rounds and partial last rounds
+    (5, 1, {2: 2.0}, 4 * 4 * 4 * (3584 + 300), 4, 3584),
+    (5, 1, {2: 1.5}, 4 * 4 * 4 * (1792 + 77) + 3, 4, 0),          # bubble filling, ragged n
+    (16, 1, {0: 8.0 / 7.0}, 4 * 15 * 8 * 2000, 8, 0),             # C2 shape
+    (7, 1, {0: 2.0, 1: 4.0 / 3.0}, 400003, 4, 0),                 # several stragglers
+    (16, 4, {r: 2.0 for r in range(4)}, 4 * 4 * 3 * 4 * 1900, 4, 0),   # g > 1: collect / NIC / distribute
+    (6, 1, {}, 6 * 4 * 2500 + 1, 0, 0),                           # plain ring
+]
+
+
+@pytest.mark.parametrize("exec_mode", MODES)
+@pytest.mark.parametrize("case", range(len(TRUNC_CASES)))
+def test_truncated_schedule_data_equals_oracle_prefix(case, exec_mode):
+    """"Steps exactly as the plan lists them" (north_star; PAPER.md:138 data dependencies), made observable: after the
+    first t steps (opts.step_limit = t) EVERY element of EVERY rank buffer must hold exactly what the oracle holds
+    after walking the table rows of steps < t -- the intermediate state of the p memories, not only the final one.
+    In particular the column executor, which runs a tile's flows in table order without any global step order, must
+    have materialised every flow's destination in memory, and nothing may have been dropped from the caches on the
+    assumption that a later step overwrites it."""
+    p, g, st, n, k, tile = TRUNC_CASES[case]
+    w = _wl(p, g, st, n, W.F32, seed=4242 + case)
+    oplan = OP.build_plan(p, g, list(w.ell), n, W.F32, k=k)
+    x = W.all_inputs(w)
+    rng = np.random.default_rng(900 + case)
+    limits = sorted(set([1, oplan.n_steps - 1] + [int(t) for t in rng.integers(1, oplan.n_steps, size=3)]))
+    for limit in limits:
+        plan = B.optcc_plan(p, g, w.ell, n, W.F32, k=k, exec_mode=exec_mode, step_limit=limit, tile_units=tile)
+        s = _session(plan)
+        s.upload(x)
+        s.execute()
+        y = s.download()
+        y_or = OI.run_f32(_oracle_prefix(oplan, limit), x)
+        assert y.tobytes() == y_or.tobytes(), f"state after {limit} of {oplan.n_steps} steps differs from the oracle's"
+        del s, plan
+
+
+@pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_COLUMN, B.OPTCC_EXEC_DATAFLOW])
+def test_truncated_schedule_data_at_c2_full_size(exec_mode):
+    """the same at BASELINE.json configs[1] (n = 2^26, bench.py's k): sampled elements of every rank against the
+    oracle's walk of the table prefix, for a cut inside the pipeline (some sections reduced, some already gathered)"""
+    import torch
+    w = W.config(1)
+    k = 16
+    oplan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=k)
+    limit = (oplan.n_steps * 3) // 5 + 4
+    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=k, exec_mode=exec_mode, step_limit=limit)
+    s = _session(plan)
+    x = W.all_inputs(w)
+    s.upload(x)
+    s.execute()
+    torch.cuda.synchronize()
+    idx = W.sample_indices(w, 1024)
+    ti = torch.from_numpy(idx).to(s.device)
+    ys = np.stack([s.bufs[r][ti].cpu().numpy() for r in range(w.p)])
+    y_or = OI.run_f32_at(_oracle_prefix(oplan, limit), np.ascontiguousarray(x[:, idx]), idx)
+    assert ys.tobytes() == y_or.tobytes()
+    assert not np.array_equal(ys[0], ys[1])      # (the cut really is mid-schedule: the ranks still differ)
