@@ -49,9 +49,13 @@ __device__ __forceinline__ char* rank_ptr(const ExecParams& P, unsigned int r) {
 }
 
 // One piece of one flow: 16-byte units [ubeg, uend) of the flow, executed by the whole CTA.
+// stage / from_stage (column executor's bulk all-gather path, data runs): a reduce flow with `stage` also keeps the sum
+// it stores in that shared-memory image of the tile; a copy flow with `from_stage` has its whole vectors stored by one
+// thread's cp.async.bulk (see optcc_column_kernel), only the ragged end of a buffer is moved here.
 template <int MODE, int NT, class PolX>
 __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& f, unsigned long long ubeg,
-                                              unsigned long long uend, unsigned int& overlaps, const PolX& pol) {
+                                              unsigned long long uend, unsigned int& overlaps, const PolX& pol,
+                                              char* stage = nullptr, bool from_stage = false) {
   using MT = ModeTraits<MODE>;
   const unsigned long long A = P.unit_elems;
   const unsigned long long e0 = ubeg * A;
@@ -65,7 +69,12 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
   if (MODE == MODE_F32) {
     const char* s = rank_ptr(P, f.src) + f.off * 4;
     char* d = rank_ptr(P, f.dst) + f.off * 4;
-    if (f.op == 0) range_add_f32<4, NT>(s, d, vbeg, vend, pol, dead_src); else range_copy16<4, NT>(s, d, vbeg, vend, pol);
+    if (f.op == 0) {
+      if (stage) range_add_f32<4, NT, true>(s, d, vbeg, vend, pol, dead_src, stage);
+      else range_add_f32<4, NT, false>(s, d, vbeg, vend, pol, dead_src, nullptr);
+    } else if (!from_stage) {
+      range_copy16<4, NT>(s, d, vbeg, vend, pol);
+    }
     if (threadIdx.x < tail) {
       unsigned long long e = vend * 4 + threadIdx.x;
       const float* sf = reinterpret_cast<const float*>(s);
@@ -131,15 +140,17 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
       // DRAM-bound there; on in the column executor)
       const bool bf_dead = PolX::l1 != 0 && dead_src;
       switch ((f.ksrc << 2) | (f.kdin << 1) | f.kdout) {
-        case 0: range_add_bf16<0, 0, 0, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
-        case 1: range_add_bf16<0, 0, 1, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
-        case 2: range_add_bf16<0, 1, 0, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
-        case 3: range_add_bf16<0, 1, 1, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
-        case 4: range_add_bf16<1, 0, 0, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
-        case 5: range_add_bf16<1, 0, 1, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
-        case 6: range_add_bf16<1, 1, 0, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
-        default: range_add_bf16<1, 1, 1, NT>(s, di, dout, vbeg, vend, pol, bf_dead); break;
+        case 0: range_add_bf16<0, 0, 0, NT>(s, di, dout, vbeg, vend, pol, bf_dead, stage); break;
+        case 1: range_add_bf16<0, 0, 1, NT>(s, di, dout, vbeg, vend, pol, bf_dead, stage); break;
+        case 2: range_add_bf16<0, 1, 0, NT>(s, di, dout, vbeg, vend, pol, bf_dead, stage); break;
+        case 3: range_add_bf16<0, 1, 1, NT>(s, di, dout, vbeg, vend, pol, bf_dead, stage); break;
+        case 4: range_add_bf16<1, 0, 0, NT>(s, di, dout, vbeg, vend, pol, bf_dead, stage); break;
+        case 5: range_add_bf16<1, 0, 1, NT>(s, di, dout, vbeg, vend, pol, bf_dead, stage); break;
+        case 6: range_add_bf16<1, 1, 0, NT>(s, di, dout, vbeg, vend, pol, bf_dead, stage); break;
+        default: range_add_bf16<1, 1, 1, NT>(s, di, dout, vbeg, vend, pol, bf_dead, stage); break;
       }
+    } else if (from_stage) {
+      // (whole units stored by cp.async.bulk from the stage)
     } else if (f.ksrc == 0) {
       range_copy16<4, NT>(s, dout, vbeg, vend, pol);                 // bf16 -> bf16: one vector per unit
     } else {
@@ -261,6 +272,11 @@ __device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, unsig
 }
 __device__ __forceinline__ void bulk_s2g(void* gdst, const void* smem_src, unsigned int bytes) {
   asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(smem_src)), "r"(bytes) : "memory");
+  asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_s2g_hint(void* gdst, const void* smem_src, unsigned int bytes, unsigned long long policy) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+               ::"l"(gdst), "r"(smem_u32(smem_src)), "r"(bytes), "l"(policy) : "memory");
   asm volatile("cp.async.bulk.commit_group;" ::: "memory");
 }
 __device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
@@ -492,60 +508,81 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
 constexpr int COL_THREADS = DF_COMPUTE_THREADS;
 
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
-// The operands of the next flow that the current flow does not write (a ring hop's destination is the next rank's
-// raw section: its first touch, a DRAM access) are requested while the current flow streams.  Every thread asks for
-// the vectors it will load itself (NT-strided, like the range operations).  f32 and bf16 data only: the verifier's
-// first touches are constants.
+// First touches ahead of time.  The ranges of flow f that no earlier flow of the region has written (DFLOW_SRC_RAW /
+// DFLOW_DST_RAW, a walk of the table on the host: a ring hop's destination is the next rank's untouched section, the
+// straggler's raw section, a raw P2P piece) are DRAM accesses; they are requested col_pf_dist flows before f runs.
+// Every thread asks for the vectors it will load itself (NT-strided, like the range operations).  f32 and bf16 data
+// only (raw data always lives in the rank buffer): the verifier's first touches are constants.
 template <int MODE, int NT>
-__device__ __forceinline__ void prefetch_operands(const ExecParams& P, const DFlow& f, unsigned int w0,
-                                                  unsigned long long ubeg, unsigned long long uend) {
+__device__ __forceinline__ void prefetch_raw(const ExecParams& P, const DFlow& f, unsigned long long ubeg, unsigned int n) {
   if (is_mask_mode(MODE)) return;
-  const unsigned int n = (unsigned int)(uend - ubeg);   // (a tile: far below 2^32 units)
+  const unsigned int esz = MODE == MODE_F32 ? 4 : 2;
   auto span = [&](const char* base) {
     const char* q = base + (ubeg + threadIdx.x) * 16;
-    for (unsigned int u = threadIdx.x; u < n; u += NT, q += NT * 16) prefetch_l1(q);
+    if (P.col_pf_l2) { for (unsigned int u = threadIdx.x; u < n; u += NT, q += NT * 16) prefetch_l2(q); }
+    else { for (unsigned int u = threadIdx.x; u < n; u += NT, q += NT * 16) prefetch_l1(q); }
   };
-  const unsigned int esz = MODE == MODE_F32 ? 4 : 2;
-  // (bf16 plans: raw operands only -- partial sums in the shadow were written by this CTA a moment ago)
-  if (f.src != w0 && (MODE == MODE_F32 || f.ksrc == 0)) span(rank_ptr(P, f.src) + f.off * esz);
-  if (f.op == 0 && f.dst != w0 && (MODE == MODE_F32 || f.kdin == 0)) span(rank_ptr(P, f.dst) + f.off * esz);
+  if (f.flags & DFLOW_SRC_RAW) span(rank_ptr(P, f.src) + f.off * esz);
+  if (f.op == 0 && (f.flags & DFLOW_DST_RAW)) span(rank_ptr(P, f.dst) + f.off * esz);
 }
 
-constexpr unsigned int COL_REC = 128;   // flow records staged in shared memory at a time (4 KB)
+constexpr unsigned int COL_REC = 256;   // flow records staged in shared memory at a time (8 KB)
+constexpr unsigned int COL_PF_MAX = 8;  // deepest look-ahead (flows)
 
 template <int MODE>
 __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(const __grid_constant__ ExecParams P) {
-  __shared__ unsigned long long s_item;
-  __shared__ __align__(16) DFlow s_rec[COL_REC];   // this CTA's staged part of the region's flow list
+  __shared__ unsigned long long s_item[2];          // work items are claimed one item ahead
+  __shared__ __align__(16) DFlow s_rec[COL_REC];    // this CTA's staged part of the region's flow list
+  __shared__ __align__(16) DFlow s_nrec[COL_PF_MAX];   // the first records of the next item (look-ahead across items)
   unsigned int overlaps = 0;
   // A tile is private to its CTA for the whole launch, so loads and stores go through L1 (PolL1): the value a flow
   // stores is the next flow's source.  L2 policies all evict_normal (a dirty line marked evict_first is written back).
   const Pol pol0 = make_policies(P.l2_hints);
   PolL1 pol;
   pol.lds = pol0.lds; pol.ldd = pol0.ldd; pol.st = pol0.st;
-  for (;;) {
-    __syncthreads();                 // every thread has read the previous item (and its last records)
-    if (threadIdx.x == 0) s_item = atomicAdd(&P.ctrl->ticket, 1ull);
-    __syncthreads();
-    const unsigned long long it = s_item;
-    if (it >= P.col_n_items) break;
+  const unsigned int D = is_mask_mode(MODE) ? 0u : (P.col_pf_dist < COL_PF_MAX ? P.col_pf_dist : COL_PF_MAX);
+  extern __shared__ __align__(128) char s_stage_col[];   // bulk all-gather path: the tile of the sum being distributed
+  const bool bulk = !is_mask_mode(MODE) && P.col_bulk != 0;
+  const unsigned long long bulk_pol = make_policy(P.pad0);   // L2 policy of the bulk stores
+  if (threadIdx.x == 0) {
+    s_item[0] = atomicAdd(&P.ctrl->ticket, 1ull);
+    s_item[1] = atomicAdd(&P.ctrl->ticket, 1ull);
+  }
+  __syncthreads();
+  unsigned long long it = s_item[0], nit = s_item[1];
+  bool prefetched = false;           // the first flows of this item were requested during the previous item
+  for (unsigned int round = 0; it < P.col_n_items; ++round) {
     // one record per item: the region's flows [fb, fe), the tile and its length in units (all flows over a region have
     // the same length, PLAN_SPEC 5.4, so the tile's unit range is fixed for the item)
     const uint4 item = __ldg(P.col_items + it);
     const unsigned int fb = item.x, fe = item.y;
-    const unsigned long long ubeg = (unsigned long long)item.z * P.tile_units, uend = ubeg + item.w;
+    const unsigned long long ubeg = (unsigned long long)item.z * P.tile_units;
+    const unsigned long long uend = ubeg + item.w;
+    // look-ahead into the next item: its first raw operands are requested while this item's last flows run
+    unsigned long long n_ubeg = 0;
+    unsigned int n_cnt = 0, n_units = 0, n_fb = 0;
+    if (D && P.col_pf_next && nit < P.col_n_items) {
+      const uint4 ni = __ldg(P.col_items + nit);
+      n_fb = ni.x;
+      n_cnt = ni.y - ni.x < D ? ni.y - ni.x : D;
+      n_ubeg = (unsigned long long)ni.z * P.tile_units;
+      n_units = ni.w;
+    }
     int prev_cls = -1;
     for (unsigned int base = fb; base < fe; base += COL_REC) {
       const unsigned int cnt = fe - base < COL_REC ? fe - base : COL_REC;
+      const bool last_chunk = base + cnt == fe;
       if (base != fb) __syncthreads();             // the previous records have been read by every thread
       for (unsigned int t = threadIdx.x; t < 2 * cnt; t += COL_THREADS)
         reinterpret_cast<uint4*>(s_rec)[t] = __ldg(reinterpret_cast<const uint4*>(P.flows + base) + t);
+      if (base == fb && threadIdx.x < 2 * n_cnt)
+        reinterpret_cast<uint4*>(s_nrec)[threadIdx.x] = __ldg(reinterpret_cast<const uint4*>(P.flows + n_fb) + threadIdx.x);
       __syncthreads();
-      auto run_flow = [&](const DFlow& cur, const DFlow& nxt, bool has_next) {
-        // the raw operands of the next flow (a ring hop's destination is the next rank's untouched section: a DRAM
-        // first touch) are requested while this one streams -- not the range this flow writes
-        if (has_next) prefetch_operands<MODE, COL_THREADS>(P, nxt, cur.dst, ubeg, uend);
+      if (base == fb && D && !prefetched)          // nobody has asked for the first flows' operands yet
+        for (unsigned int j = 0; j < D && j < cnt; ++j) prefetch_raw<MODE, COL_THREADS>(P, s_rec[j], ubeg, item.w);
+      auto run_flow = [&](const DFlow& cur) {
         if (MODE == MODE_BF16) {
           // a copy of fp32 partials moves two vectors per unit, thread i taking vector i instead of unit i: when the
           // thread-to-element mapping changes between consecutive flows the CTA synchronises (block-wide ordering)
@@ -553,24 +590,63 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
           if (prev_cls >= 0 && cls != prev_cls) __syncthreads();
           prev_cls = cls;
         }
-        process_piece<MODE, COL_THREADS>(P, cur, ubeg, uend, overlaps, pol);
+        if (!is_mask_mode(MODE) && bulk) {
+          // Bulk all-gather path.  The reduce flow that completes a sum which later copy flows distribute
+          // (DFLOW_STAGE_OUT, found by the host's walk of the region's list) stores it to its destination as listed
+          // and also keeps it in shared memory; every copy flow whose source range holds exactly that tile
+          // (DFLOW_FROM_STAGE) is then one cp.async.bulk store of the staged tile to its destination, issued by one
+          // thread in list order -- the all-gather steps move through the TMA unit instead of LDG / STG.
+          const unsigned int fl = cur.flags;
+          if (fl & DFLOW_STAGE_OUT) {        // the stage is rewritten: the previous tile's bulk stores must have read it
+            if (threadIdx.x == 0) bulk_wait_read_all();
+            __syncthreads();
+            process_piece<MODE, COL_THREADS>(P, cur, ubeg, uend, overlaps, pol, s_stage_col, false);
+            // this thread's generic-proxy writes (the stage; its earlier stores to ranges the bulk stores will overwrite)
+            // are ordered before the async-proxy operations issued after the barrier
+            fence_proxy_async();
+            __syncthreads();
+          } else if (fl & DFLOW_FROM_STAGE) {
+            if (threadIdx.x == 0) {
+              constexpr unsigned long long ESZ = MODE == MODE_F32 ? 4 : 2, VE = 16 / ESZ;
+              const unsigned long long e0 = ubeg * P.unit_elems;
+              unsigned long long e1 = uend * P.unit_elems;
+              if (e1 > cur.len) e1 = cur.len;
+              const unsigned long long v0 = e0 / VE, v1 = e1 / VE;
+              if (v1 > v0) bulk_s2g_hint(rank_ptr(P, cur.dst) + cur.off * ESZ + v0 * 16, s_stage_col, (unsigned int)((v1 - v0) * 16), bulk_pol);
+            }
+            process_piece<MODE, COL_THREADS>(P, cur, ubeg, uend, overlaps, pol, nullptr, true);   // (ragged end of a buffer only)
+          } else {
+            process_piece<MODE, COL_THREADS>(P, cur, ubeg, uend, overlaps, pol);
+          }
+        } else {
+          process_piece<MODE, COL_THREADS>(P, cur, ubeg, uend, overlaps, pol);
+        }
         __syncwarp();   // orders a lane's dead-source discard of a 128-byte line before the other lanes' later stores to it
       };
       if (is_mask_mode(MODE)) {
         // the verifier is bound by instruction issue (ncu: 79 % of the issue slots): records are read in place
-        for (unsigned int j = 0; j < cnt; ++j) run_flow(s_rec[j], s_rec[j], false);
+        for (unsigned int j = 0; j < cnt; ++j) run_flow(s_rec[j]);
       } else {
         // data: the next record is in registers before its flow starts (its loads issue without waiting for shared memory)
         DFlow cur = s_rec[0];
         for (unsigned int j = 0; j < cnt; ++j) {
-          const bool has_next = j + 1 < cnt;
-          const DFlow nxt = s_rec[has_next ? j + 1 : j];
-          run_flow(cur, nxt, has_next);
+          // the raw operands of the flow D places ahead are requested while this one streams (prefetches are hints: a
+          // request that is skipped at a chunk boundary or for a very short list costs time, never correctness)
+          if (j + D < cnt) prefetch_raw<MODE, COL_THREADS>(P, s_rec[j + D], ubeg, item.w);
+          else if (last_chunk && j + D - cnt < n_cnt) prefetch_raw<MODE, COL_THREADS>(P, s_nrec[j + D - cnt], n_ubeg, n_units);
+          const DFlow nxt = s_rec[j + 1 < cnt ? j + 1 : j];
+          run_flow(cur);
           cur = nxt;
         }
       }
     }
+    if (threadIdx.x == 0) s_item[round & 1] = atomicAdd(&P.ctrl->ticket, 1ull);   // (slot of `it`: read by everyone long ago)
+    __syncthreads();                 // every thread has read this item's records
+    prefetched = n_cnt != 0;
+    it = nit;
+    nit = s_item[round & 1];
   }
+  if (bulk && threadIdx.x == 0) bulk_wait_all();   // the stage stays valid until every bulk store has read it
   if (is_mask_mode(MODE)) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) overlaps += __shfl_xor_sync(0xFFFFFFFFu, overlaps, o);
@@ -757,7 +833,7 @@ void assign_mask_flags(optcc_plan_t* pl, optcc_exec_state* st) {
   const uint32_t nf = pl->step_begin[steps];            // flows of the executed steps
   const size_t nr = pl->region_offs.size();
   std::vector<uint8_t> written(size_t(in.p) * nr, 0);
-  const std::vector<uint32_t>& reg = pl->flow_region;
+  const optcc_rawvec<uint32_t>& reg = pl->flow_region;
   for (uint32_t i = 0; i < nf; ++i) {                   // forwards: has the range been written before flow i?
     const optcc_flow_t& f = pl->flows[i];
     uint32_t fl = 0;
@@ -802,6 +878,21 @@ void assign_dead_source_flags(optcc_plan_t* pl, optcc_exec_state* st) {
   }
 }
 
+// First touches (column executor's look-ahead): DFLOW_SRC_RAW / DFLOW_DST_RAW mark the ranges no earlier flow of the
+// table has written -- reading them is a DRAM access, requested ahead of time by prefetch_raw.
+void assign_raw_flags(optcc_plan_t* pl, optcc_exec_state* st) {
+  const optcc_plan_info_t& in = pl->info;
+  const size_t nr = pl->region_offs.size();
+  std::vector<uint8_t> written(size_t(in.p) * nr, 0);
+  for (uint32_t i = 0; i < in.n_flows; ++i) {
+    const optcc_flow_t& f = pl->flows[i];
+    const size_t reg = pl->flow_region[i];
+    if (!written[size_t(f.src) * nr + reg]) st->dflows[i].flags |= DFLOW_SRC_RAW;
+    if (!written[size_t(f.dst) * nr + reg]) st->dflows[i].flags |= DFLOW_DST_RAW;
+    written[size_t(f.dst) * nr + reg] = 1;
+  }
+}
+
 // Column executor tables: the flows of the executed steps region by region (a stable counting sort of the table by
 // region, so table order is kept inside a region) and one work item per (region, tile).
 bool build_column_tables(optcc_plan_t* pl, optcc_exec_state* st) {   // false: PLAN_SPEC 5.4 violated (a planner bug)
@@ -833,6 +924,62 @@ bool build_column_tables(optcc_plan_t* pl, optcc_exec_state* st) {   // false: P
   return true;
 }
 
+// Bulk all-gather path of the column executor (data runs): per region list, find the reduce flows whose sum later copy
+// flows distribute (DFLOW_STAGE_OUT: the CTA keeps the tile in shared memory) and the copy flows whose source range holds
+// exactly the staged tile at that point (DFLOW_FROM_STAGE: one cp.async.bulk store).  Value numbering: a reduce gives its
+// destination a new value, a copy gives it the source's value.  One stage: a new sum is only staged when every copy of
+// the previous one has been issued.  A list in which a range written by a bulk store is touched again by any later flow
+// (never the case in an AllReduce plan: the all-gather's copies are final) keeps the LDG / STG path entirely.
+void assign_bulk_flags(optcc_exec_state* st, uint32_t p, bool bf16) {
+  std::vector<uint32_t> val(p), consumers;
+  std::vector<uint8_t> bulk_written(p);
+  const size_t nr = st->col_reg_begin.size() - 1;
+  for (size_t r = 0; r < nr; ++r) {
+    const uint32_t fb = st->col_reg_begin[r], fe = st->col_reg_begin[r + 1];
+    if (fb == fe) continue;
+    for (uint32_t i = 0; i < p; ++i) val[i] = i;
+    consumers.assign(size_t(p) + (fe - fb), 0);
+    uint32_t next_id = p;
+    for (uint32_t i = fb; i < fe; ++i) {           // how many copy flows read each value
+      const DFlow& f = st->col_dflows[i];
+      if (f.op == OPTCC_OP_REDUCE) val[f.dst] = next_id++;
+      else { consumers[val[f.src]]++; val[f.dst] = val[f.src]; }
+    }
+    for (uint32_t i = 0; i < p; ++i) val[i] = i;
+    std::fill(bulk_written.begin(), bulk_written.end(), 0);
+    next_id = p;
+    uint32_t staged = UINT32_MAX, pending = 0;
+    bool ok = true;
+    for (uint32_t i = fb; i < fe && ok; ++i) {
+      DFlow& f = st->col_dflows[i];
+      if (f.op == OPTCC_OP_REDUCE) {
+        if (bulk_written[f.src] || bulk_written[f.dst]) { ok = false; break; }
+        const uint32_t id = next_id++;
+        val[f.dst] = id;
+        if (consumers[id] && pending == 0 && (!bf16 || f.kdout == OPTCC_KIND_BUF)) {
+          f.flags |= DFLOW_STAGE_OUT;
+          staged = id;
+          pending = consumers[id];
+        }
+      } else {
+        if (val[f.src] == staged && (!bf16 || (f.ksrc == OPTCC_KIND_BUF && f.kdout == OPTCC_KIND_BUF))) {
+          if (bulk_written[f.dst]) { ok = false; break; }
+          f.flags |= DFLOW_FROM_STAGE;
+          bulk_written[f.dst] = 1;
+          --pending;
+        } else if (bulk_written[f.src] || bulk_written[f.dst]) {
+          ok = false;
+          break;
+        } else if (val[f.src] == staged) {
+          --pending;
+        }
+        val[f.dst] = val[f.src];
+      }
+    }
+    if (!ok) for (uint32_t i = fb; i < fe; ++i) st->col_dflows[i].flags &= ~(DFLOW_STAGE_OUT | DFLOW_FROM_STAGE);
+  }
+}
+
 template <int MODE>
 int kernel_occupancy(int* out) {
   CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, optcc_exec_kernel<MODE>, THREADS, 0));
@@ -843,6 +990,7 @@ int kernel_occupancy(int* out) {
 inline uint64_t unit_cost(const optcc_plan_t* pl, size_t i) {
   const optcc_flow_t& f = pl->flows[i];
   auto sz = [](uint8_t kind) -> uint64_t { return kind == OPTCC_KIND_F32 ? 32 : 16; };
+  if (pl->kind_src.empty()) return f.op == OPTCC_OP_REDUCE ? 48 : 32;   // f32 plans
   uint64_t c = sz(pl->kind_src[i]) + sz(pl->kind_dst_out[i]);
   if (f.op == OPTCC_OP_REDUCE) c += sz(pl->kind_dst_in[i]);
   return c;
@@ -934,7 +1082,7 @@ int build_state(optcc_plan_t* pl) {
       DFlow d;
       std::memset(&d, 0, sizeof d);
       d.off = f.off; d.len = f.len; d.src = f.src; d.dst = f.dst; d.op = f.op;
-      d.ksrc = pl->kind_src[i]; d.kdin = pl->kind_dst_in[i]; d.kdout = pl->kind_dst_out[i];
+      if (!pl->kind_src.empty()) { d.ksrc = pl->kind_src[i]; d.kdin = pl->kind_dst_in[i]; d.kdout = pl->kind_dst_out[i]; }
       st->dflows[i] = d;
     }
     // dataflow tables when that executor will run; otherwise the slice table of the barrier executors
@@ -944,7 +1092,9 @@ int build_state(optcc_plan_t* pl) {
     st->column = pl->opts.exec_mode == OPTCC_EXEC_COLUMN && pl->tiles_per_rank < (uint64_t(1) << 32);
     if (st->column) {
       assign_dead_source_flags(pl, st);
+      assign_raw_flags(pl, st);
       if (!build_column_tables(pl, st)) { st->G = 0; return OPTCC_EINVAL; }   // (G = 0: the state is rebuilt on the next call)
+      if (pl->opts.copy_path != 1) assign_bulk_flags(st, in.p, in.dtype == OPTCC_BF16);
     }
     // slice table: cut every step into G slices of equal HBM bytes
     st->slices.clear();
@@ -1024,7 +1174,9 @@ int launch_plan(optcc_plan_t* pl, ExecParams& P, cudaStream_t stream) {
     CU_TRY(cudaMemsetAsync(&P.ctrl->ticket, 0, sizeof(unsigned long long), stream));
     const uint32_t G = pl->opts.grid_ctas ? pl->opts.grid_ctas : uint32_t(st->sm_count) * CTAS_PER_SM;
     const unsigned int grid = (unsigned int)std::min<uint64_t>(G, P.col_n_items);
-    optcc_column_kernel<MODE><<<grid, COL_THREADS, 0, stream>>>(P);
+    const size_t dyn = (!is_mask_mode(MODE) && P.col_bulk) ? size_t(pl->tile_units) * 16 : 0;   // the stage: one tile
+    if (dyn > 40 * 1024) CU_TRY(cudaFuncSetAttribute(optcc_column_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+    optcc_column_kernel<MODE><<<grid, COL_THREADS, dyn, stream>>>(P);
     CU_TRY(cudaGetLastError());
   } else if (dataflow) {
     P.n_ops = st->step_op_begin[n_steps];
@@ -1079,6 +1231,12 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   // fetch / completion latency; copying agents hold their slots, so the bulk path also uses 4
   P.df_slots = (pl->exec && pl->exec->big_ops && !P.bulk_copy) ? 2 : 4;
   if (pl->opts.exec_mode == OPTCC_EXEC_COLUMN) P.l2_hints = 0;   // see optcc_column_kernel
+  P.col_pf_dist = 1; P.col_pf_l2 = 0; P.col_pf_next = 0; P.col_bulk = 1;
+  if (const char* t = std::getenv("OPTCC_TUNE")) {   // TEMPORARY (experiments): "dist,l2,next,bulk,bulkpolicy"
+    unsigned a = 1, b = 0, c = 0, d = 1, e = 0;
+    if (std::sscanf(t, "%u,%u,%u,%u,%u", &a, &b, &c, &d, &e) >= 1) { P.col_pf_dist = a; P.col_pf_l2 = b; P.col_pf_next = c; P.col_bulk = d; P.pad0 = e; }
+  }
+  if (pl->opts.copy_path == 1) P.col_bulk = 0;
 }
 
 }  // namespace

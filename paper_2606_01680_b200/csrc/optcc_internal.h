@@ -3,7 +3,9 @@
 #ifndef OPTCC_INTERNAL_H_
 #define OPTCC_INTERNAL_H_
 
+#include <cstddef>
 #include <cstdint>
+#include <new>
 #include <vector>
 
 #include "optcc.h"
@@ -14,13 +16,51 @@ enum : uint8_t { OPTCC_KIND_BUF = 0 /* the rank buffer, plan dtype */, OPTCC_KIN
 
 struct optcc_exec_state;  // device-side cache, defined in optcc_exec.cu
 
+// Big host tables (the flow table and what is derived from it: tens to hundreds of MB at p = 128 ... 1024).  Memory
+// comes uninitialised (every element is written by the fill pass, so no zeroing pass and no single-threaded page faults)
+// and goes back to a small process-wide cache when the plan dies: a job that plans every step (bench.py does) gets
+// pages that are already mapped.  optcc_raw_alloc / optcc_raw_free live in optcc_plan.cpp.
+void* optcc_raw_alloc(size_t bytes);          // nullptr on failure; 64-byte aligned
+void optcc_raw_free(void* p, size_t bytes);
+template <class T>
+class optcc_rawvec {
+ public:
+  optcc_rawvec() = default;
+  optcc_rawvec(const optcc_rawvec&) = delete;
+  optcc_rawvec& operator=(const optcc_rawvec&) = delete;
+  ~optcc_rawvec() { release(); }
+  void release() { if (p_) optcc_raw_free(p_, cap_ * sizeof(T)); p_ = nullptr; n_ = cap_ = 0; }
+  void resize_uninit(size_t n) {          // contents undefined; throws std::bad_alloc
+    if (n > cap_) {
+      release();
+      p_ = static_cast<T*>(optcc_raw_alloc(n * sizeof(T)));
+      if (!p_) throw std::bad_alloc();
+      cap_ = n;
+    }
+    n_ = n;
+  }
+  size_t size() const { return n_; }
+  bool empty() const { return n_ == 0; }
+  T* data() { return p_; }
+  const T* data() const { return p_; }
+  T& operator[](size_t i) { return p_[i]; }
+  const T& operator[](size_t i) const { return p_[i]; }
+  T* begin() { return p_; }
+  T* end() { return p_ + n_; }
+  const T* begin() const { return p_; }
+  const T* end() const { return p_ + n_; }
+ private:
+  T* p_ = nullptr;
+  size_t n_ = 0, cap_ = 0;
+};
+
 struct optcc_plan {
   optcc_plan_info_t info;
   optcc_opts_t opts;
   std::vector<double> ell;              // [p]
   std::vector<uint32_t> stragglers;     // server indices, ell descending then index (PLAN_SPEC 1)
   std::vector<uint32_t> healthy;        // server indices ascending
-  std::vector<optcc_flow_t> flows;      // sorted (PLAN_SPEC 3)
+  optcc_rawvec<optcc_flow_t> flows;     // in PLAN_SPEC 3 order
   std::vector<uint32_t> step_begin;     // [n_steps + 1]
   std::vector<uint64_t> sec_bounds;
   std::vector<uint64_t> p2p_bounds;
@@ -32,8 +72,10 @@ struct optcc_plan {
   uint64_t n_tile_ops = 0;              // sum over flows of ceil(units / tile_units)
   uint64_t tiles_per_rank = 0;          // sum over regions of ceil(units / tile_units): counters per rank
   std::vector<uint64_t> region_offs;    // sorted unique flow offsets (regions tile [0, n), PLAN_SPEC 5.4)
+  std::vector<uint64_t> region_len;     // elements of every region
+  std::vector<uint32_t> region_flows;   // flows over every region
   std::vector<uint64_t> region_tile0;   // first tile counter of every region (prefix sum)
-  std::vector<uint32_t> flow_region;    // [n_flows] index into region_offs of the region a flow covers
+  optcc_rawvec<uint32_t> flow_region;   // [n_flows] index into region_offs of the region a flow covers
   optcc_exec_state* exec;               // created lazily by the executor; freed by optcc_plan_destroy
 };
 

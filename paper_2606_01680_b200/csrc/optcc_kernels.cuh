@@ -45,6 +45,13 @@ enum : unsigned int {
   DFLOW_SRC_INIT = 2u,   // no earlier flow wrote the source range: it holds the initial mask {src}
   DFLOW_DST_INIT = 4u,   // no earlier flow wrote the destination range: it holds the initial mask {dst}
   DFLOW_FINAL = 8u,      // no later flow writes the destination range: what this flow writes is the final mask
+  // all runs (column executor: what to prefetch ahead of time):
+  DFLOW_SRC_RAW = 16u,   // no earlier executed flow wrote the source range: reading it is its first touch (a DRAM access)
+  DFLOW_DST_RAW = 32u,   // the same for the destination range (a reduce flow reads it)
+  // column executor, data runs, bulk all-gather path (see build_column_tables / optcc_column_kernel):
+  DFLOW_STAGE_OUT = 64u,   // reduce flow: the sum it stores is the source of later copy flows -- also keep it in the CTA's stage
+  DFLOW_FROM_STAGE = 128u, // copy flow: the source range holds exactly the staged tile -- store it with cp.async.bulk
+  DFLOW_DRAIN = 256u,      // the flow touches a range an earlier bulk store of this list wrote: wait for the bulk stores first
 };
 
 struct __align__(16) Slice {      // start of a CTA's slice of a step: flow index and 16-byte unit inside it
@@ -101,6 +108,10 @@ struct ExecParams {
   unsigned long long col_n_items;
   unsigned int bulk_copy;         // 1: copy tile-ops are moved by the scheduler agents with cp.async.bulk
   unsigned int l2_hints;          // kind(src loads) + 4 kind(dst loads) + 16 kind(stores); kind: 0 normal, 1 evict_first, 2 evict_last
+  unsigned int col_pf_dist;       // column executor: raw operands are requested this many flows ahead (>= 1)
+  unsigned int col_pf_l2;         // 1: requested into L2 (prefetch.global.L2), 0: into L1
+  unsigned int col_pf_next;       // 1: the look-ahead continues into the CTA's next work item (claimed one item ahead)
+  unsigned int col_bulk;          // 1: data runs act on DFLOW_STAGE_OUT / FROM_STAGE / DRAIN (bulk all-gather path)
 };
 
 // ---- memory access helpers: L2-only loads (data written by other SMs in the previous step), streaming stores ----
@@ -143,6 +154,9 @@ __device__ __forceinline__ void st16(void* p, uint4 v, const PolX& pol) {
   else
     asm volatile("st.global.cg.L2::cache_hint.v4.u32 [%0], {%1,%2,%3,%4}, %5;"
                  ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(pol.st) : "memory");
+}
+__device__ __forceinline__ void sts16(char* smem, uint4 v) {
+  asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"((unsigned int)__cvta_generic_to_shared(smem)), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 __device__ __forceinline__ float bf16_to_f32(unsigned int h) { return __uint_as_float(h << 16); }
 // float -> bf16 bits, round to nearest even; NaN stays a quiet NaN
@@ -232,9 +246,12 @@ __device__ __forceinline__ void range_copy16(const char* __restrict__ s, char* _
   }
 }
 
-template <int UNROLL, int NT, class PolX>
+// `stage` (column executor, DFLOW_STAGE_OUT): shared-memory image of the tile, vector vbeg at offset 0 -- the sum is
+// stored to the destination range as listed and kept in the stage for the bulk all-gather; nullptr otherwise.
+template <int UNROLL, int NT, bool STAGE, class PolX>
 __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* __restrict__ d,
-                                              unsigned long long vbeg, unsigned long long vend, const PolX& pol, bool dead_src) {
+                                              unsigned long long vbeg, unsigned long long vend, const PolX& pol, bool dead_src,
+                                              char* stage) {
   unsigned long long v = vbeg + threadIdx.x;
   for (; v + (UNROLL - 1) * (unsigned long long)NT < vend; v += UNROLL * (unsigned long long)NT) {
     uint4 a[UNROLL], b[UNROLL];
@@ -244,7 +261,11 @@ __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* 
       b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd, pol.l1);
     }
 #pragma unroll
-    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, add_f32x4(b[j], a[j]), pol);
+    for (int j = 0; j < UNROLL; ++j) {
+      const uint4 r = add_f32x4(b[j], a[j]);
+      st16(d + (v + j * (unsigned long long)NT) * 16, r, pol);
+      if (STAGE) sts16(stage + (v + j * (unsigned long long)NT - vbeg) * 16, r);
+    }
     // (only when every lane of the warp is in this round: the line's other vectors were loaded by this instruction)
     if (dead_src && (v - (threadIdx.x & 31u) + 31) + (UNROLL - 1) * (unsigned long long)NT < vend) {
 #pragma unroll
@@ -262,7 +283,11 @@ __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* 
         b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd, pol.l1);
       }
 #pragma unroll
-      for (int j = 0; j < KK; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, add_f32x4(b[j], a[j]), pol);
+      for (int j = 0; j < KK; ++j) {
+        const uint4 r = add_f32x4(b[j], a[j]);
+        st16(d + (v + j * (unsigned long long)NT) * 16, r, pol);
+        if (STAGE) sts16(stage + (v + j * (unsigned long long)NT - vbeg) * 16, r);
+      }
     };
     remainder_dispatch<UNROLL>(rem, batch);
   }
@@ -465,10 +490,21 @@ __device__ __forceinline__ void store8(char* base, unsigned long long unit, cons
   }
 }
 
+// bf16 image of 8 sums for the stage (the same rounding store8<0> applies)
+__device__ __forceinline__ uint4 pack8_bf16(const float (&x)[8]) {
+  uint4 r;
+  r.x = f32_to_bf16_rne(x[0]) | (f32_to_bf16_rne(x[1]) << 16);
+  r.y = f32_to_bf16_rne(x[2]) | (f32_to_bf16_rne(x[3]) << 16);
+  r.z = f32_to_bf16_rne(x[4]) | (f32_to_bf16_rne(x[5]) << 16);
+  r.w = f32_to_bf16_rne(x[6]) | (f32_to_bf16_rne(x[7]) << 16);
+  return r;
+}
+
+// `stage`: as in range_add_f32 (only with KO == 0: complete sums live in the rank buffer), one 16-byte unit per slot
 template <int KS, int KD, int KO, int NT, class PolX>
 __device__ __forceinline__ void range_add_bf16(const char* __restrict__ s, const char* __restrict__ din,
                                                char* __restrict__ dout, unsigned long long ubeg,
-                                               unsigned long long uend, const PolX& pol, bool dead_src) {
+                                               unsigned long long uend, const PolX& pol, bool dead_src, char* stage) {
   constexpr int UNROLL = 2;
   unsigned long long u = ubeg + threadIdx.x;
   for (; u + (UNROLL - 1) * (unsigned long long)NT < uend; u += UNROLL * (unsigned long long)NT) {
@@ -483,6 +519,7 @@ __device__ __forceinline__ void range_add_bf16(const char* __restrict__ s, const
 #pragma unroll
       for (int e = 0; e < 8; ++e) b[j][e] = __fadd_rn(b[j][e], a[j][e]);
       store8<KO>(dout, u + j * (unsigned long long)NT, b[j], pol);
+      if (KO == 0 && stage) sts16(stage + (u + j * (unsigned long long)NT - ubeg) * 16, pack8_bf16(b[j]));
     }
     if (dead_src && (u - (threadIdx.x & 31u) + 31) + (UNROLL - 1) * (unsigned long long)NT < uend) {
 #pragma unroll
@@ -499,6 +536,7 @@ __device__ __forceinline__ void range_add_bf16(const char* __restrict__ s, const
 #pragma unroll
     for (int e = 0; e < 8; ++e) b[e] = __fadd_rn(b[e], a[e]);
     store8<KO>(dout, u, b, pol);
+    if (KO == 0 && stage) sts16(stage + (u - ubeg) * 16, pack8_bf16(b));
   }
 }
 

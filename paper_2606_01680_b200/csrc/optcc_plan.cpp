@@ -7,68 +7,69 @@
 #include <algorithm>
 #include <chrono>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <atomic>
+#include <mutex>
 #include <thread>
 #include <new>
 
 #include "optcc_internal.h"
 
+// ---- raw table memory with a small process-wide cache (optcc_internal.h) ----
+namespace {
+struct RawBlock { void* p; size_t bytes; };
+std::mutex g_raw_mutex;
+std::vector<RawBlock> g_raw_cache;                 // at most RAW_CACHE_BLOCKS freed blocks
+constexpr size_t RAW_CACHE_BLOCKS = 8;
+constexpr size_t RAW_CACHE_MIN = size_t(1) << 16;  // smaller blocks go straight to malloc / free
+constexpr size_t RAW_CACHE_MAX = size_t(1) << 30;  // total bytes kept
+}  // namespace
+
+void* optcc_raw_alloc(size_t bytes) {
+  if (bytes == 0) bytes = 64;
+  if (bytes >= RAW_CACHE_MIN) {
+    std::lock_guard<std::mutex> lock(g_raw_mutex);
+    size_t best = SIZE_MAX;
+    for (size_t i = 0; i < g_raw_cache.size(); ++i)   // smallest cached block that fits without wasting more than half
+      if (g_raw_cache[i].bytes >= bytes && g_raw_cache[i].bytes <= 2 * bytes &&
+          (best == SIZE_MAX || g_raw_cache[i].bytes < g_raw_cache[best].bytes)) best = i;
+    if (best != SIZE_MAX) {
+      void* p = g_raw_cache[best].p;
+      g_raw_cache.erase(g_raw_cache.begin() + best);
+      return p;
+    }
+  }
+  return std::aligned_alloc(64, (bytes + 63) & ~size_t(63));
+}
+
+// (the block's true capacity is not tracked: a recycled block is handed out again by the size it was freed with, which
+//  is the size its last owner asked for -- never more than what was allocated)
+void optcc_raw_free(void* p, size_t bytes) {
+  if (!p) return;
+  if (bytes >= RAW_CACHE_MIN) {
+    std::lock_guard<std::mutex> lock(g_raw_mutex);
+    size_t total = bytes;
+    for (const auto& b : g_raw_cache) total += b.bytes;
+    if (g_raw_cache.size() < RAW_CACHE_BLOCKS && total <= RAW_CACHE_MAX) {
+      g_raw_cache.push_back(RawBlock{p, bytes});
+      return;
+    }
+  }
+  std::free(p);
+}
+
 namespace {
 
-struct Builder {
-  optcc_plan_t* pl;
-  uint64_t A, U, n;
-  uint32_t k, nsec;
-  std::vector<std::pair<uint64_t, uint64_t>> ring;  // ring region of every part, in units
+// x mod H for -H <= x < 2H (all the rules need: ring positions shifted by at most one lap)
+inline uint32_t modH(int64_t x, int64_t H) { return (uint32_t)(x < 0 ? x + H : (x >= H ? x - H : x)); }
 
-  static uint64_t split(uint64_t lo, uint64_t hi, uint64_t parts, uint64_t i) {
-    // PLAN_SPEC 2: lo + floor(i (hi-lo) / parts); i <= parts <= 2^23 and hi-lo <= 2^40, so no overflow in u64
-    return lo + (i * (hi - lo)) / parts;
-  }
-  uint64_t E(uint64_t u) const { return std::min(u * A, n); }
-  std::vector<uint64_t> sec_tab;   // section boundaries [(lam * k + b) * (nsec + 1) + c], filled once by build_sec_tab
-  void build_sec_tab() {
-    sec_tab.resize(ring.size() * size_t(k) * (nsec + 1));
-    for (size_t lam = 0; lam < ring.size(); ++lam)
-      for (uint32_t b = 0; b < k; ++b) {
-        const uint64_t s0 = split(ring[lam].first, ring[lam].second, k, b);
-        const uint64_t s1 = split(ring[lam].first, ring[lam].second, k, b + 1);
-        uint64_t* row = sec_tab.data() + (lam * k + b) * (nsec + 1);
-        for (uint32_t c = 0; c <= nsec; ++c) row[c] = split(s0, s1, nsec, c);
-      }
-  }
-  void sec_units(uint32_t lam, uint32_t b, uint32_t c, uint64_t* lo, uint64_t* hi) const {
-    const uint64_t* row = sec_tab.data() + (size_t(lam) * k + b) * (nsec + 1);
-    *lo = row[c];
-    *hi = row[c + 1];
-  }
-  void emit_units(uint32_t step, uint8_t op, uint8_t stage, uint8_t link, uint32_t part, uint32_t src,
-                  uint32_t dst, uint32_t seg, uint32_t sec, uint64_t ulo, uint64_t uhi) {
-    uint64_t off = E(ulo), len = E(uhi) - E(ulo);
-    if (len == 0) return;  // PLAN_SPEC 2: zero-length flows are dropped
-    optcc_flow_t f;
-    std::memset(&f, 0, sizeof f);
-    f.off = off; f.len = len; f.step = step; f.seg = seg; f.sec = sec;
-    f.src = (uint16_t)src; f.dst = (uint16_t)dst; f.op = op; f.stage = stage; f.link = link; f.part = (uint8_t)part;
-    pl->flows.push_back(f);
-  }
-  void emit_sec(uint32_t step, uint8_t op, uint8_t stage, uint8_t link, uint32_t lam, uint32_t src, uint32_t dst,
-                uint32_t b, uint32_t c) {
-    uint64_t lo, hi;
-    sec_units(lam, b, c, &lo, &hi);
-    emit_units(step, op, stage, link, lam, src, dst, b, c, lo, hi);
-  }
-};
-
-inline uint32_t modH(int64_t x, int64_t H) { int64_t r = x % H; return (uint32_t)(r < 0 ? r + H : r); }
-
-// Run body(i) for i in [0, n) on a few host threads when the table is large enough to pay for them; the
-// iterations are independent (each sorts or moves a disjoint range).
+// Run body(chunk) for chunk in [0, n) on a few host threads when the table is large enough to pay for them; the
+// chunks are independent (each counts or fills a disjoint range of steps).
 template <class F>
 void parallel_chunks(size_t n, size_t work, F body) {
   unsigned hw = std::thread::hardware_concurrency();
-  unsigned nt = work < (size_t(1) << 17) ? 1u : std::min(8u, hw ? hw : 1u);
+  unsigned nt = work < (size_t(1) << 16) ? 1u : std::min(8u, hw ? hw : 1u);
   if (nt <= 1 || n <= 1) { for (size_t i = 0; i < n; ++i) body(i); return; }
   std::atomic<size_t> next{0};
   auto worker = [&]() { for (size_t i; (i = next.fetch_add(1, std::memory_order_relaxed)) < n;) body(i); };
@@ -79,34 +80,191 @@ void parallel_chunks(size_t n, size_t work, F body) {
   for (auto& t : th) t.join();
 }
 
-// PLAN_SPEC 3 order (step, link, stage, src, dst, off): counting sort by step, then each step's few flows by a
-// packed key -- the table has O(p k H) records, a comparison sort of whole records dominated the build time.
-// The per-step sorts and the final gather touch disjoint ranges and are split over host threads.
-void sort_flows(std::vector<optcc_flow_t>& flows, uint32_t n_steps) {
-  struct Key { uint64_t hi, lo; uint32_t idx; };
-  const size_t nf = flows.size();
-  std::vector<uint32_t> begin(size_t(n_steps) + 2, 0);
-  for (const auto& f : flows) begin[f.step + 1]++;
-  for (size_t t = 0; t <= n_steps; ++t) begin[t + 1] += begin[t];
-  std::vector<Key> keys(nf);
-  {
-    std::vector<uint32_t> pos(begin.begin(), begin.end() - 1);
-    for (size_t i = 0; i < nf; ++i) {
-      const optcc_flow_t& f = flows[i];
-      Key k;
-      k.hi = (uint64_t(f.link) << 35) | (uint64_t(f.stage) << 32) | (uint64_t(f.src) << 16) | uint64_t(f.dst);
-      k.lo = f.off;
-      k.idx = (uint32_t)i;
-      keys[pos[f.step]++] = k;
+// Everything the closed-form rules of PLAN_SPEC 4 need, fixed before the first flow is written.  The table is never
+// sorted: emit_step() lists the flows of one step directly in PLAN_SPEC 3 order (link, stage, src, dst, off), so the
+// steps can be counted and filled independently ("closed-form rules ... O(pk)").
+struct Geom {
+  uint32_t p = 0, g = 1, q = 0, m = 0, H = 0, k = 0, nsec = 0;
+  uint32_t construction = 0, ordering = 2;
+  uint32_t P = 0;        // windows per body: H (C1, C3 with one straggler server), H + m - 1 otherwise (:788)
+  uint32_t D = 0;        // C3: the NIC body of segment b is body b + D
+  uint32_t n_steps = 0;
+  bool bubbles = false;
+  const uint32_t* healthy = nullptr;      // server indices, ascending
+  const uint32_t* stragglers = nullptr;   // server indices, PLAN_SPEC 1 order (ell descending)
+  std::vector<uint32_t> str_by_rank;      // positions in `stragglers`, by server index ascending (S3: src order)
+  // regions: the sections in (part, segment, section) order, then the P2P pieces; UINT32_MAX = empty interval (dropped)
+  std::vector<uint32_t> sec_reg, p2p_reg;
+  const uint64_t* region_off = nullptr;
+  const uint64_t* region_len = nullptr;
+  uint32_t sec(uint32_t lam, uint32_t b, uint32_t c) const { return sec_reg[(size_t(lam) * k + b) * nsec + c]; }
+};
+
+// One flow of step t; region == UINT32_MAX: a zero-length range (PLAN_SPEC 2: dropped).
+struct CountSink {
+  static constexpr bool kOrdered = false;   // the order inside a step does not matter for counting
+  uint32_t n = 0;
+  void operator()(uint32_t, uint8_t, uint8_t, uint8_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t region) {
+    n += region != UINT32_MAX;
+  }
+};
+struct CountAllSink {   // no region is empty: every rule application is a flow (the arguments are never computed)
+  static constexpr bool kOrdered = false;
+  uint32_t n = 0;
+  void operator()(uint32_t, uint8_t, uint8_t, uint8_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t) { ++n; }
+};
+struct FillSink {
+  static constexpr bool kOrdered = true;
+  const Geom* G;
+  uint32_t* region_count = nullptr;   // this chunk's flows per region
+  optcc_flow_t* out;        // next record
+  uint32_t* out_region;
+  uint64_t reduce_elems = 0, copy_elems = 0;
+  void operator()(uint32_t step, uint8_t op, uint8_t stage, uint8_t link, uint32_t part, uint32_t src, uint32_t dst,
+                  uint32_t seg, uint32_t sec, uint32_t region) {
+    if (region == UINT32_MAX) return;
+    optcc_flow_t f;
+    f.off = G->region_off[region]; f.len = G->region_len[region];
+    f.step = step; f.seg = seg; f.sec = sec;
+    f.src = (uint16_t)src; f.dst = (uint16_t)dst; f.op = op; f.stage = stage; f.link = link; f.part = (uint8_t)part;
+    f.reserved = 0;
+    *out++ = f;
+    *out_region++ = region;
+    region_count[region]++;
+    (op == OPTCC_OP_REDUCE ? reduce_elems : copy_elems) += f.len;
+  }
+};
+
+// The flows of step t in table order (PLAN_SPEC 3: link, stage, src, dst, off).  Within one stage the senders are
+// visited in increasing rank, and a sender has one flow per stage and step except on the NVLink rings (see below).
+template <class Sink>
+void emit_step(const Geom& G, uint32_t t, Sink& out) {
+  const uint32_t H = G.H, k = G.k, g = G.g, m = G.m;
+  if (G.construction == OPTCC_C0) {
+    // plain ring: reduce-scatter p-1 hops then all-gather p-1 hops (:52, :72)
+    const uint32_t p = G.p;
+    if (t < p - 1) {
+      for (uint32_t j = 0; j < p; ++j)
+        out(t, OPTCC_OP_REDUCE, OPTCC_S1, OPTCC_LINK_NIC, 0, j, (j + 1 == p ? 0 : j + 1), 0, modH(int64_t(j) - t, p), G.sec(0, 0, modH(int64_t(j) - t, p)));
+    } else {
+      const uint32_t tt = t - (p - 1);
+      for (uint32_t j = 0; j < p; ++j)
+        out(t, OPTCC_OP_COPY, OPTCC_S4, OPTCC_LINK_NIC, 0, j, (j + 1 == p ? 0 : j + 1), 0, modH(int64_t(j) + 1 - tt, p), G.sec(0, 0, modH(int64_t(j) + 1 - tt, p)));
+    }
+    return;
+  }
+  if (G.construction == OPTCC_C1 && G.ordering == 1) {
+    // C1': ordering (1) of :138, S1 -> S2 -> S3 -> S4, one stage per body (PLAN_SPEC 4 C1')
+    const uint32_t Bd = t / H, w = t % H, sg = G.stragglers[0];
+    const uint32_t a = w, d = (w + 1) % H;
+    if (Bd < k)       // Stage 1: partial sums of the healthy servers (:126); ring link j idle in window j
+      for (uint32_t j = 0; j < H; ++j) {
+        if (w == j) continue;
+        const uint32_t hop = w < j ? w : w - 1, c = modH(int64_t(j) - hop, H);
+        out(t, OPTCC_OP_REDUCE, OPTCC_S1, OPTCC_LINK_NIC, 0, G.healthy[j], G.healthy[j + 1 == H ? 0 : j + 1], Bd, c, G.sec(0, Bd, c));
+      }
+    if (Bd >= 1 && Bd <= k)       // Stage 2: the straggler adds its own data to the uploaded partial sum (:130-132)
+      out(t, OPTCC_OP_REDUCE, OPTCC_S2, OPTCC_LINK_NIC, 0, G.healthy[a], sg, Bd - 1, (a + 1) % H, G.sec(0, Bd - 1, (a + 1) % H));
+    if (Bd >= 2 && Bd <= k + 1)   // Stage 3: the global sum returns to the uploader's ring successor (:132, R11)
+      out(t, OPTCC_OP_COPY, OPTCC_S3, OPTCC_LINK_NIC, 0, sg, G.healthy[d], Bd - 2, d, G.sec(0, Bd - 2, d));
+    if (Bd >= 3)      // Stage 4: the all-gather of section c starts at healthy c (:136)
+      for (uint32_t j = 0; j < H; ++j) {
+        if (w == j) continue;
+        const uint32_t hop = w < j ? w : w - 1, c = modH(int64_t(j) - hop, H);
+        out(t, OPTCC_OP_COPY, OPTCC_S4, OPTCC_LINK_NIC, 0, G.healthy[j], G.healthy[j + 1 == H ? 0 : j + 1], Bd - 3, c, G.sec(0, Bd - 3, c));
+      }
+    if (G.bubbles && Bd < k)
+      out(t, OPTCC_OP_REDUCE, OPTCC_BUB_UP, OPTCC_LINK_NIC, 0, G.healthy[a], sg, Bd, 0, G.p2p_reg[Bd]);
+    if (G.bubbles && Bd >= 1 && Bd <= k)
+      out(t, OPTCC_OP_COPY, OPTCC_BUB_DOWN, OPTCC_LINK_NIC, 0, sg, G.healthy[d], Bd - 1, 0, G.p2p_reg[Bd - 1]);
+    return;
+  }
+  // C1 / C2 / C3: NIC flows of body BB = Bd + D, window w (leaders: local GPU lam of every server, :854)
+  const uint32_t P = G.P, D = G.D, BB = t / P, w = t % P;
+  if (BB >= D && BB - D <= k) {
+    const uint32_t Bd = BB - D;
+    // ring link j (healthy j -> j+1) is idle in windows [j, j+m); hop `hop` sits in window W(j, hop)
+    if (Bd < k)   // Stage 1, segment Bd: add own section and forward (:126)
+      for (uint32_t j = 0; j < H; ++j) {
+        if (w >= j && w < j + m) continue;
+        const uint32_t hop = w < j ? w : w - m, c = modH(int64_t(j) - hop, H);
+        for (uint32_t lam = 0; lam < g; ++lam)
+          out(t, OPTCC_OP_REDUCE, OPTCC_S1, OPTCC_LINK_NIC, lam, G.healthy[j] * g + lam, G.healthy[j + 1 == H ? 0 : j + 1] * g + lam, Bd, c, G.sec(lam, Bd, c));
+      }
+    // straggler i is active in windows [i, i+H) with uploader a = w - i, downloader d = (a+1) mod H
+    if (Bd >= 1) {  // Stage 2: the owner uploads the complete sum to the straggler (:130; ordering (2) :138); by sender a
+      const uint32_t i_hi = std::min<uint32_t>(m - 1, w);
+      for (uint32_t i = i_hi + 1; i-- > 0;) {
+        const uint32_t a = w - i;
+        if (a >= H) break;
+        for (uint32_t lam = 0; lam < g; ++lam)
+          out(t, OPTCC_OP_COPY, OPTCC_S2, OPTCC_LINK_NIC, lam, G.healthy[a] * g + lam, G.stragglers[i] * g + lam, Bd - 1, (a + 1) % H, G.sec(lam, Bd - 1, (a + 1) % H));
+      }
+    }
+    if (Bd < k)     // Stage 3: the straggler's raw section is folded in at its owner (:132, :138); by sender (straggler rank)
+      for (uint32_t ii = 0; ii < m; ++ii) {
+        const uint32_t i = G.str_by_rank[ii];
+        if (w < i || w - i >= H) continue;
+        const uint32_t a = w - i, d = (a + 1) % H;
+        for (uint32_t lam = 0; lam < g; ++lam)
+          out(t, OPTCC_OP_REDUCE, OPTCC_S3, OPTCC_LINK_NIC, lam, G.stragglers[i] * g + lam, G.healthy[d] * g + lam, Bd, (d + 1) % H, G.sec(lam, Bd, (d + 1) % H));
+      }
+    if (Bd >= 1)    // Stage 4, segment Bd-1: forward the complete sum (:136)
+      for (uint32_t j = 0; j < H; ++j) {
+        if (w >= j && w < j + m) continue;
+        const uint32_t hop = w < j ? w : w - m, c = modH(int64_t(j) + 1 - hop, H);
+        for (uint32_t lam = 0; lam < g; ++lam)
+          out(t, OPTCC_OP_COPY, OPTCC_S4, OPTCC_LINK_NIC, lam, G.healthy[j] * g + lam, G.healthy[j + 1 == H ? 0 : j + 1] * g + lam, Bd - 1, c, G.sec(lam, Bd - 1, c));
+      }
+    if (G.bubbles) {   // (one straggler, g = 1, P = H)
+      const uint32_t a = w, d = (w + 1) % H, sg = G.stragglers[0];
+      if (Bd < k)    // bubble-up: healthy a's raw P2P piece into the straggler (:165, R9)
+        out(t, OPTCC_OP_REDUCE, OPTCC_BUB_UP, OPTCC_LINK_NIC, 0, G.healthy[a], sg, Bd, 0, G.p2p_reg[Bd]);
+      if (Bd >= 1)   // bubble-down: the straggler returns the P2P result (:165)
+        out(t, OPTCC_OP_COPY, OPTCC_BUB_DOWN, OPTCC_LINK_NIC, 0, sg, G.healthy[d], Bd - 1, 0, G.p2p_reg[Bd - 1]);
     }
   }
-  std::vector<optcc_flow_t> out(nf);
-  parallel_chunks(size_t(n_steps) + 1, nf, [&](size_t t) {
-    std::sort(keys.begin() + begin[t], keys.begin() + begin[t + 1],
-              [](const Key& a, const Key& b) { return a.hi != b.hi ? a.hi < b.hi : a.lo < b.lo; });
-    for (size_t i = begin[t]; i < begin[t + 1]; ++i) out[i] = flows[keys[i].idx];
-  });
-  flows.swap(out);
+  if (G.construction != OPTCC_C3) return;
+  // NVLink rings of every server (link 1 sorts after the NIC flows).  Hop h of (part lam, segment b, section c) sits at
+  // step b P + c + h (collect) resp. (b + D + 2) P + c + h (distribute); a GPU can send several flows of one stage in
+  // one step (one per h, each for another part), all to the same neighbour: those are ordered by offset, i.e. by
+  // (lam, b, c) since the parts are consecutive ranges.
+  struct Cand { uint32_t lam, b, c; };
+  Cand cand[256];
+  auto nv_stage = [&](bool collect) {
+    const uint64_t shift = collect ? 0 : uint64_t(D + 2) * P;
+    if (t < shift) return;
+    const uint64_t tt = t - shift;
+    for (uint32_t v = 0; v < G.q; ++v)
+      for (uint32_t x = 0; x < g; ++x) {     // sender: local GPU x of server v
+        uint32_t nc = 0;
+        uint32_t b = uint32_t(tt / P), c = uint32_t(tt % P);          // (b, c) of hop h: b P + c = tt - h
+        for (uint32_t h = 0; h + 1 < g && h <= tt; ++h) {
+          if (h) { if (c == 0) { c = P - 1; --b; } else --c; }
+          if (b >= k || c >= H) continue;
+          // collect: local (lam-1-h) -> (lam-2-h) (backward ring, the leader only receives, :862, :875, :894);
+          // distribute: local (lam+h) -> (lam+h+1) (forward ring, the leader sends first, :863, :876, :894)
+          uint32_t lam;
+          if (collect) { lam = x + 1 + h; if (lam >= g) lam -= g; }      // (h <= g-2, x <= g-1: at most one lap)
+          else lam = x >= h ? x - h : x + g - h;
+          Cand cd{lam, b, c};
+          uint32_t pos = nc++;
+          if (Sink::kOrdered)
+            while (pos > 0 && (cand[pos - 1].lam > cd.lam || (cand[pos - 1].lam == cd.lam &&
+                   (cand[pos - 1].b > cd.b || (cand[pos - 1].b == cd.b && cand[pos - 1].c > cd.c))))) {
+              cand[pos] = cand[pos - 1];
+              --pos;
+            }
+          cand[pos] = cd;
+        }
+        const uint32_t src = v * g + x, dst = v * g + (collect ? (x + g - 1) % g : (x + 1) % g);
+        for (uint32_t i = 0; i < nc; ++i)
+          out(t, collect ? OPTCC_OP_REDUCE : OPTCC_OP_COPY, collect ? OPTCC_N_COLLECT : OPTCC_N_DISTRIBUTE, OPTCC_LINK_NVLINK,
+              cand[i].lam, src, dst, cand[i].b, cand[i].c, G.sec(cand[i].lam, cand[i].b, cand[i].c));
+      }
+  };
+  nv_stage(true);
+  nv_stage(false);
 }
 
 // Storage kinds for bf16 plans: walk the table once with the number of contributors every
@@ -115,10 +273,10 @@ void sort_flows(std::vector<optcc_flow_t>& flows, uint32_t n_steps) {
 void assign_kinds(optcc_plan_t* pl) {
   const uint32_t p = pl->info.p;
   const size_t nf = pl->flows.size();
+  if (pl->info.dtype != OPTCC_BF16) return;      // f32 plans: the three arrays stay empty (everything is OPTCC_KIND_BUF)
   pl->kind_src.assign(nf, OPTCC_KIND_BUF);
   pl->kind_dst_in.assign(nf, OPTCC_KIND_BUF);
   pl->kind_dst_out.assign(nf, OPTCC_KIND_BUF);
-  if (pl->info.dtype != OPTCC_BF16) return;
   const size_t nr = pl->region_offs.size();
   std::vector<uint16_t> cnt(size_t(p) * nr, 1);
   auto region = [&](uint32_t i) { return size_t(pl->flow_region[i]); };
@@ -188,12 +346,13 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
                                     ? OPTCC_C0 : (g > 1 ? OPTCC_C3 : (m == 1 ? OPTCC_C1 : OPTCC_C2));
   const double ell1 = m ? ell[stragglers[0] * g] : 1.0;
 
-  Builder B;
-  B.pl = pl;
-  B.n = n;
-  B.A = dtype == OPTCC_F32 ? 4 : 8;  // elements per 16-byte unit (PLAN_SPEC 2, R3)
-  B.U = (n + B.A - 1) / B.A;
-  const uint64_t U = B.U;
+  const uint64_t A = dtype == OPTCC_F32 ? 4 : 8;  // elements per 16-byte unit (PLAN_SPEC 2, R3)
+  const uint64_t U = (n + A - 1) / A;
+  auto split = [](uint64_t lo, uint64_t hi, uint64_t parts, uint64_t i) {
+    // PLAN_SPEC 2: lo + floor(i (hi-lo) / parts); i <= parts <= 2^23 and hi-lo <= 2^40, so no overflow in u64
+    return lo + (i * (hi - lo)) / parts;
+  };
+  auto E = [&](uint64_t u) { return std::min(u * A, n); };
 
   // ---- PLAN_SPEC 2: bandwidth-weighted chunking (n_p2p/n = (2-l)/((p-2)l+2)) ----
   uint64_t U_p2p = 0;
@@ -206,10 +365,11 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     U_p2p = (uint64_t)std::floor(x + 0.5);
   }
   const uint64_t U_ring = U - U_p2p;
+  std::vector<std::pair<uint64_t, uint64_t>> ring;   // ring region of every part, in units
   if (construction == OPTCC_C0 || construction == OPTCC_C1) {
-    B.ring.push_back({0, U_ring});
+    ring.push_back({0, U_ring});
   } else {
-    for (int lam = 0; lam < g; ++lam) B.ring.push_back({Builder::split(0, U, g, lam), Builder::split(0, U, g, lam + 1)});
+    for (int lam = 0; lam < g; ++lam) ring.push_back({split(0, U, g, lam), split(0, U, g, lam + 1)});
   }
   // k (PLAN_SPEC 2 "k (R2)")
   if (construction == OPTCC_C0) {
@@ -217,163 +377,150 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
   } else if (k == 0) {
     double c = construction == OPTCC_C1 ? (ell1 < 2.0 ? ell1 - 1.0 : 1.0) : (construction == OPTCC_C2 ? 1.0 : 2.0);
     uint64_t k_t = 4 * (uint64_t)std::ceil(5.0 * c - 1e-9);
-    uint64_t R = (B.ring[0].second - B.ring[0].first) * 16;
+    uint64_t R = (ring[0].second - ring[0].first) * 16;
     uint64_t k_c = 4 * ((R / (uint64_t(H) * 65536)) / 4);
     k = (uint32_t)std::max<uint64_t>(4, std::min(k_t, k_c));
   }
-  B.k = k;
-  B.nsec = construction == OPTCC_C0 ? (uint32_t)p : H;
-  auto p2p_lo = [&](uint32_t b) { return Builder::split(U_ring, U, k, b); };
-  try {
-    B.build_sec_tab();
-    // flows: 2 (p-1) n elements in sections of about U / (g k nsec) units
-    pl->flows.reserve(size_t(2) * (k + 1) * (p - 1) * (B.nsec + m) * (g > 1 ? 2 : 1));
-  } catch (const std::bad_alloc&) {
-    delete pl;
-    return OPTCC_ENOMEM;
-  }
+  const uint32_t nsec = construction == OPTCC_C0 ? (uint32_t)p : H;
   const bool bubbles = construction == OPTCC_C1 && ell1 < 2.0;
 
-  // ---- PLAN_SPEC 4: constructions ----
-  uint32_t n_steps = 0;
+  Geom G;
+  G.p = p; G.g = g; G.q = q; G.m = m; G.H = H; G.k = k; G.nsec = nsec;
+  G.construction = construction; G.ordering = ordering; G.bubbles = bubbles;
+  G.healthy = pl->healthy.data();
+  G.stragglers = pl->stragglers.data();
+  uint64_t reduce_elems = 0, copy_elems = 0;
   try {
-    if (construction == OPTCC_C1 && ordering == 1) {
-      // C1': ordering (1) of :138, S1 -> S2 -> S3 -> S4, one stage per body (PLAN_SPEC 4 C1')
-      n_steps = (k + 3) * H;
-      const uint32_t sg = stragglers[0];
-      for (uint32_t Bd = 0; Bd < k + 3; ++Bd) {
-        const uint32_t base = Bd * H;
-        for (uint32_t j = 0; j < H; ++j) {
-          const uint32_t src = healthy[j], dst = healthy[(j + 1) % H];
-          for (uint32_t t = 0; t + 1 < H; ++t) {
-            const uint32_t step = base + (t < j ? t : t + 1);
-            const uint32_t c = modH(int64_t(j) - t, H);
-            if (Bd < k)    // Stage 1: partial sums of the healthy servers (:126)
-              B.emit_sec(step, OPTCC_OP_REDUCE, OPTCC_S1, OPTCC_LINK_NIC, 0, src, dst, Bd, c);
-            if (Bd >= 3)   // Stage 4: the all-gather of section c starts at healthy c (:136)
-              B.emit_sec(step, OPTCC_OP_COPY, OPTCC_S4, OPTCC_LINK_NIC, 0, src, dst, Bd - 3, c);
-          }
-        }
-        for (uint32_t a = 0; a < H; ++a) {
-          const uint32_t d = (a + 1) % H, step = base + a;
-          if (Bd >= 1 && Bd <= k)       // Stage 2: the straggler adds its own data to the uploaded partial sum (:130-132)
-            B.emit_sec(step, OPTCC_OP_REDUCE, OPTCC_S2, OPTCC_LINK_NIC, 0, healthy[a], sg, Bd - 1, (a + 1) % H);
-          if (Bd >= 2 && Bd <= k + 1)   // Stage 3: the global sum returns to the uploader's ring successor (:132, R11)
-            B.emit_sec(step, OPTCC_OP_COPY, OPTCC_S3, OPTCC_LINK_NIC, 0, sg, healthy[d], Bd - 2, d);
-          if (bubbles && Bd < k)
-            B.emit_units(step, OPTCC_OP_REDUCE, OPTCC_BUB_UP, OPTCC_LINK_NIC, 0, healthy[a], sg, Bd, 0, p2p_lo(Bd), p2p_lo(Bd + 1));
-          if (bubbles && Bd >= 1 && Bd <= k)
-            B.emit_units(step, OPTCC_OP_COPY, OPTCC_BUB_DOWN, OPTCC_LINK_NIC, 0, sg, healthy[d], Bd - 1, 0, p2p_lo(Bd - 1), p2p_lo(Bd));
-        }
-      }
-    } else if (construction == OPTCC_C0) {
-      // plain ring: reduce-scatter p-1 hops then all-gather p-1 hops (:52, :72)
-      n_steps = 2 * (p - 1);
-      for (int t = 0; t < p - 1; ++t)
-        for (int j = 0; j < p; ++j) {
-          uint32_t d = (j + 1) % p;
-          B.emit_sec(t, OPTCC_OP_REDUCE, OPTCC_S1, OPTCC_LINK_NIC, 0, j, d, 0, modH(j - t, p));
-          B.emit_sec(p - 1 + t, OPTCC_OP_COPY, OPTCC_S4, OPTCC_LINK_NIC, 0, j, d, 0, modH(j + 1 - t, p));
-        }
-    } else {
-      const uint32_t P = H + m - 1;  // windows per body: H for C1/C3, p-1 for C2 (:788)
-      uint32_t D = 0;
-      if (construction == OPTCC_C3) {
-        D = 1 + (uint32_t)((g - 2 + P - 1) / P);  // NIC body of segment b is body b + D (PLAN_SPEC C3)
-        n_steps = (k + D + 2) * P + g - 2;
-      } else {
-        n_steps = (k + 1) * P;
-      }
-      for (int lam = 0; lam < g; ++lam) {
-        // leaders: local GPU lam of every server (:854); for g = 1 simply the ranks
-        for (uint32_t Bd = 0; Bd <= k; ++Bd) {
-          const uint32_t base = (Bd + D) * P;
-          // ring link j (healthy j -> j+1) is idle in windows [j, j+m); hop t sits in window W(j,t)
-          for (uint32_t j = 0; j < H; ++j) {
-            uint32_t src = healthy[j] * g + lam, dst = healthy[(j + 1) % H] * g + lam;
-            for (uint32_t t = 0; t + 1 < H; ++t) {
-              uint32_t step = base + (t < j ? t : t + m);
-              if (Bd < k)   // Stage 1, hop t of segment Bd: add own section and forward (:126)
-                B.emit_sec(step, OPTCC_OP_REDUCE, OPTCC_S1, OPTCC_LINK_NIC, lam, src, dst, Bd, modH(int64_t(j) - t, H));
-              if (Bd >= 1)  // Stage 4, hop t of segment Bd-1: forward the complete sum (:136)
-                B.emit_sec(step, OPTCC_OP_COPY, OPTCC_S4, OPTCC_LINK_NIC, lam, src, dst, Bd - 1, modH(int64_t(j) + 1 - t, H));
-            }
-          }
-          for (uint32_t i = 0; i < m; ++i) {
-            uint32_t sg = stragglers[i] * g + lam;
-            for (uint32_t a = 0; a < H; ++a) {
-              uint32_t d = (a + 1) % H, step = base + a + i;
-              uint32_t ra = healthy[a] * g + lam, rd = healthy[d] * g + lam;
-              if (Bd >= 1)  // Stage 2: the owner uploads the complete sum to the straggler (:130; ordering (2) :138)
-                B.emit_sec(step, OPTCC_OP_COPY, OPTCC_S2, OPTCC_LINK_NIC, lam, ra, sg, Bd - 1, (a + 1) % H);
-              if (Bd < k)   // Stage 3: the straggler's raw section is folded in at its owner (:132, :138)
-                B.emit_sec(step, OPTCC_OP_REDUCE, OPTCC_S3, OPTCC_LINK_NIC, lam, sg, rd, Bd, (d + 1) % H);
-              if (bubbles && Bd < k)   // bubble-up: healthy a's raw P2P piece into the straggler (:165, R9)
-                B.emit_units(step, OPTCC_OP_REDUCE, OPTCC_BUB_UP, OPTCC_LINK_NIC, lam, ra, sg, Bd, 0, p2p_lo(Bd), p2p_lo(Bd + 1));
-              if (bubbles && Bd >= 1)  // bubble-down: the straggler returns the P2P result (:165)
-                B.emit_units(step, OPTCC_OP_COPY, OPTCC_BUB_DOWN, OPTCC_LINK_NIC, lam, sg, rd, Bd - 1, 0, p2p_lo(Bd - 1), p2p_lo(Bd));
-            }
-          }
-        }
-        if (construction == OPTCC_C3) {
-          for (uint32_t v = 0; v < q; ++v)
-            for (uint32_t b = 0; b < k; ++b)
-              for (uint32_t c = 0; c < H; ++c)
-                for (int h = 0; h + 1 < g; ++h) {
-                  // N1/N3 collect on the backward local ring, the leader only receives (:862, :875, :894)
-                  B.emit_sec(b * P + c + h, OPTCC_OP_REDUCE, OPTCC_N_COLLECT, OPTCC_LINK_NVLINK, lam,
-                             v * g + modH(lam - 1 - h, g), v * g + modH(lam - 2 - h, g), b, c);
-                  // N2/N4 distribute on the forward local ring, the leader sends first (:863, :876, :894)
-                  B.emit_sec((b + D + 2) * P + c + h, OPTCC_OP_COPY, OPTCC_N_DISTRIBUTE, OPTCC_LINK_NVLINK, lam,
-                             v * g + modH(lam + h, g), v * g + modH(lam + h + 1, g), b, c);
-                }
-        }
-      }
-    }
-    sort_flows(pl->flows, n_steps);
-    pl->step_begin.assign(n_steps + 1, 0);
-    {
-      size_t i = 0;
-      for (uint32_t t = 0; t <= n_steps; ++t) {
-        while (i < pl->flows.size() && pl->flows[i].step < t) ++i;
-        pl->step_begin[t] = (uint32_t)i;
-      }
-    }
-    // exported boundary arrays (PLAN_SPEC 2)
-    uint32_t nparts = (construction == OPTCC_C2 || construction == OPTCC_C3) ? (uint32_t)g : 1;
+    // ---- exported boundary arrays (PLAN_SPEC 2): every section start in (part, segment, section) order ----
+    const uint32_t nparts = (uint32_t)ring.size();
+    pl->sec_bounds.reserve(size_t(nparts) * k * nsec + 1);
     for (uint32_t lam = 0; lam < nparts; ++lam)
-      for (uint32_t b = 0; b < k; ++b)
-        for (uint32_t c = 0; c < B.nsec; ++c) {
-          uint64_t lo, hi;
-          B.sec_units(lam, b, c, &lo, &hi);
-          pl->sec_bounds.push_back(B.E(lo));
-        }
-    pl->sec_bounds.push_back(B.E(B.ring.back().second));
+      for (uint32_t b = 0; b < k; ++b) {
+        const uint64_t s0 = split(ring[lam].first, ring[lam].second, k, b), s1 = split(ring[lam].first, ring[lam].second, k, b + 1);
+        for (uint32_t c = 0; c < nsec; ++c) pl->sec_bounds.push_back(E(split(s0, s1, nsec, c)));
+      }
+    pl->sec_bounds.push_back(E(ring.back().second));
     if (bubbles) {
-      for (uint32_t b = 0; b < k; ++b) pl->p2p_bounds.push_back(B.E(p2p_lo(b)));
-      pl->p2p_bounds.push_back(B.E(U));
+      for (uint32_t b = 0; b <= k; ++b) pl->p2p_bounds.push_back(E(split(U_ring, U, k, b)));
     }
+    // ---- regions = the sections and P2P pieces themselves: consecutive exported boundaries (ascending, contiguous,
+    // covering [0, n): PLAN_SPEC 5.4).  A flow carries its (part, segment, section), i.e. its region, from birth, so
+    // offset and length are the region's by construction.
+    auto add_regions = [&](const std::vector<uint64_t>& bounds, std::vector<uint32_t>& reg_of) {
+      reg_of.assign(bounds.empty() ? 0 : bounds.size() - 1, UINT32_MAX);
+      for (size_t i = 0; i + 1 < bounds.size(); ++i) {
+        if (bounds[i + 1] <= bounds[i]) continue;
+        reg_of[i] = (uint32_t)pl->region_offs.size();
+        pl->region_offs.push_back(bounds[i]);
+        pl->region_len.push_back(bounds[i + 1] - bounds[i]);
+      }
+    };
+    add_regions(pl->sec_bounds, G.sec_reg);
+    add_regions(pl->p2p_bounds, G.p2p_reg);
+    {   // the regions tile [0, n) exactly (both executors and the lazy verifier rely on it)
+      uint64_t pos = 0;
+      for (size_t r = 0; r < pl->region_offs.size(); ++r) {
+        if (pl->region_offs[r] != pos) { delete pl; return OPTCC_EINVAL; }
+        pos += pl->region_len[r];
+      }
+      if (pos != n) { delete pl; return OPTCC_EINVAL; }
+    }
+    G.region_off = pl->region_offs.data();
+    G.region_len = pl->region_len.data();
+    G.str_by_rank.resize(m);
+    for (uint32_t i = 0; i < m; ++i) G.str_by_rank[i] = i;
+    std::sort(G.str_by_rank.begin(), G.str_by_rank.end(), [&](uint32_t a, uint32_t b) { return stragglers[a] < stragglers[b]; });
+
+    // ---- PLAN_SPEC 4: constructions.  Step counts; the flows come from emit_step ----
+    if (construction == OPTCC_C1 && ordering == 1) {
+      G.P = H; G.n_steps = (k + 3) * H;
+    } else if (construction == OPTCC_C0) {
+      G.P = p; G.n_steps = 2 * (p - 1);
+    } else {
+      G.P = H + m - 1;  // windows per body: H for C1/C3, p-1 for C2 (:788)
+      if (construction == OPTCC_C3) {
+        G.D = 1 + (uint32_t)((g - 2 + G.P - 1) / G.P);  // NIC body of segment b is body b + D (PLAN_SPEC C3)
+        G.n_steps = (k + G.D + 2) * G.P + g - 2;
+      } else {
+        G.n_steps = (k + 1) * G.P;
+      }
+    }
+    const uint32_t n_steps = G.n_steps;
+    // pass 1: flows per step; pass 2: fill.  Steps are independent: both passes run on a few host threads for big tables.
+    pl->step_begin.assign(size_t(n_steps) + 1, 0);
+    const size_t est = size_t(2) * (k + 1) * (p - 1) * (nsec + m) * (g > 1 ? 2 : 1);
+    const size_t n_chunks = std::min<size_t>(n_steps, 64);
+    auto chunk_lo = [&](size_t c) { return uint32_t(uint64_t(n_steps) * c / n_chunks); };
+    bool any_empty = false;
+    for (uint32_t r : G.sec_reg) any_empty |= r == UINT32_MAX;
+    for (uint32_t r : G.p2p_reg) any_empty |= r == UINT32_MAX;
+    parallel_chunks(n_chunks, est, [&](size_t c) {
+      for (uint32_t t = chunk_lo(c); t < chunk_lo(c + 1); ++t) {
+        if (any_empty) {
+          CountSink cs;
+          emit_step(G, t, cs);
+          pl->step_begin[t + 1] = cs.n;
+        } else {
+          CountAllSink cs;
+          emit_step(G, t, cs);
+          pl->step_begin[t + 1] = cs.n;
+        }
+      }
+    });
+    uint64_t total = 0;
+    uint32_t max_per_step = 0;
+    for (uint32_t t = 0; t < n_steps; ++t) {
+      const uint32_t c = pl->step_begin[t + 1];
+      max_per_step = std::max(max_per_step, c);
+      total += c;
+      if (total > 0xFFFFFFF0ull) { delete pl; return OPTCC_EUNSUPPORTED; }   // flow indices are 32-bit
+      pl->step_begin[t + 1] = (uint32_t)total;
+    }
+    pl->info.max_flows_per_step = max_per_step;
+    pl->flows.resize_uninit(total);
+    pl->flow_region.resize_uninit(total);
+    std::vector<uint64_t> red(n_chunks, 0), cop(n_chunks, 0);
+    const size_t nreg = pl->region_offs.size();
+    std::vector<uint32_t> hist(n_chunks * nreg, 0);      // flows per (chunk, region)
+    parallel_chunks(n_chunks, est, [&](size_t c) {
+      FillSink fs;
+      fs.G = &G;
+      fs.region_count = hist.data() + c * nreg;
+      for (uint32_t t = chunk_lo(c); t < chunk_lo(c + 1); ++t) {
+        fs.out = pl->flows.data() + pl->step_begin[t];
+        fs.out_region = pl->flow_region.data() + pl->step_begin[t];
+        emit_step(G, t, fs);
+      }
+      red[c] = fs.reduce_elems;
+      cop[c] = fs.copy_elems;
+    });
+    for (size_t c = 0; c < n_chunks; ++c) { reduce_elems += red[c]; copy_elems += cop[c]; }
+    pl->region_flows.assign(nreg, 0);
+    for (size_t c = 0; c < n_chunks; ++c)
+      for (size_t r = 0; r < nreg; ++r) pl->region_flows[r] += hist[c * nreg + r];
   } catch (const std::bad_alloc&) {
     delete pl;
     return OPTCC_ENOMEM;
   }
+  const uint32_t n_steps = G.n_steps;
 
   optcc_plan_info_t& in = pl->info;
   in.p = p; in.g = g; in.q = q; in.m = m; in.H = H; in.k = k;
-  in.construction = construction; in.dtype = dtype; in.unit_elems = (uint32_t)B.A;
+  in.construction = construction; in.dtype = dtype; in.unit_elems = (uint32_t)A;
   // narrowest mask that holds p bits and keeps every flow offset (a multiple of A elements) 16-byte aligned: >= 16/A bytes
   in.mask_bytes = p <= 16 ? 2 : (p <= 32 ? 4 : (p <= 64 ? 8 : (p <= 128 ? 16 : 0)));
-  if (in.mask_bytes) in.mask_bytes = std::max<uint32_t>(in.mask_bytes, uint32_t(16 / B.A));
+  if (in.mask_bytes) in.mask_bytes = std::max<uint32_t>(in.mask_bytes, uint32_t(16 / A));
   in.mask_words = (in.mask_bytes + 7) / 8;
-  in.n = n; in.n_ring = B.E(U_ring); in.n_p2p = n - B.E(U_ring);
+  in.n = n; in.n_ring = E(U_ring); in.n_p2p = n - E(U_ring);
   in.U = U; in.U_ring = U_ring; in.U_p2p = U_p2p;
   in.n_steps = n_steps; in.n_flows = (uint32_t)pl->flows.size();
   in.n_sec_bounds = (uint32_t)pl->sec_bounds.size(); in.n_p2p_bounds = (uint32_t)pl->p2p_bounds.size();
-  for (uint32_t t = 0; t < n_steps; ++t)
-    in.max_flows_per_step = std::max(in.max_flows_per_step, pl->step_begin[t + 1] - pl->step_begin[t]);
-  for (const auto& f : pl->flows) (f.op == OPTCC_OP_REDUCE ? in.reduce_elems : in.copy_elems) += f.len;
-  // dataflow tiling: regions (unique offsets; all flows over one offset share a length, PLAN_SPEC 5.4) and tile counts
+  in.reduce_elems = reduce_elems; in.copy_elems = copy_elems;
+  // tiling: flows per region (all flows over a region share offset and length), tile counts
   try {
+    const size_t nr = pl->region_offs.size();
+    uint64_t flow_units = 0;
+    for (size_t r = 0; r < nr; ++r) flow_units += uint64_t(pl->region_flows[r]) * ((pl->region_len[r] + A - 1) / A);
     if (pl->opts.tile_units) {
       pl->tile_units = pl->opts.tile_units;
     } else if (pl->opts.exec_mode == OPTCC_EXEC_COLUMN) {
@@ -383,63 +530,29 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
       // dead-source discard acts on (measured on a B200); a region shorter than that is one tile.
       uint32_t tu = dtype == OPTCC_BF16 ? 896 : 1792;
       uint64_t longest = 0;
-      for (size_t i = 0; i + 1 < pl->sec_bounds.size(); ++i) longest = std::max(longest, pl->sec_bounds[i + 1] - pl->sec_bounds[i]);
-      for (size_t i = 0; i + 1 < pl->p2p_bounds.size(); ++i) longest = std::max(longest, pl->p2p_bounds[i + 1] - pl->p2p_bounds[i]);
-      const uint64_t longest_units = ((longest + B.A - 1) / B.A + 7) & ~uint64_t(7);
+      for (size_t r = 0; r < nr; ++r) longest = std::max(longest, pl->region_len[r]);
+      const uint64_t longest_units = ((longest + A - 1) / A + 7) & ~uint64_t(7);
       if (longest_units && longest_units < tu) tu = (uint32_t)longest_units;
       pl->tile_units = tu;
     } else {
       // auto: about two tile-ops per CTA and step (592 = 2 x 296 CTAs on a B200), from {224, 448, 896, 1792, 3584}
       // -- multiples / fractions of one streaming round of the dataflow kernel (448 threads x 4 vectors), so a tile is
       // whole rounds; big steps get 56 KB tiles (bandwidth-bound), small steps short tiles (more parallel chains)
-      uint64_t units = 0;
-      for (const auto& f : pl->flows) units += (f.len + B.A - 1) / B.A;
-      const uint64_t per = n_steps ? units / n_steps / 592 : 0;
+      const uint64_t per = n_steps ? flow_units / n_steps / 592 : 0;
       uint32_t tu = 224;
       while (tu < OPTCC_TILE_UNITS_DEFAULT && uint64_t(tu) * 3 / 2 < per) tu *= 2;
       pl->tile_units = tu;
     }
-    // regions = the sections and P2P pieces themselves: consecutive exported boundaries (ascending, contiguous)
     uint64_t tiles = 0;
-    std::vector<uint32_t> sec_reg, p2p_reg;     // boundary interval -> region (UINT32_MAX: empty interval)
-    bool region_error = false;
-    auto add_regions = [&](const std::vector<uint64_t>& bounds, std::vector<uint32_t>& reg_of) {
-      reg_of.assign(bounds.empty() ? 0 : bounds.size() - 1, UINT32_MAX);
-      for (size_t i = 0; i + 1 < bounds.size(); ++i) {
-        if (bounds[i + 1] <= bounds[i]) continue;
-        reg_of[i] = (uint32_t)pl->region_offs.size();
-        pl->region_offs.push_back(bounds[i]);
-        pl->region_tile0.push_back(tiles);
-        tiles += ((bounds[i + 1] - bounds[i] + B.A - 1) / B.A + pl->tile_units - 1) / pl->tile_units;
-      }
-    };
-    add_regions(pl->sec_bounds, sec_reg);
-    add_regions(pl->p2p_bounds, p2p_reg);
+    pl->region_tile0.resize(nr);
+    pl->n_tile_ops = 0;
+    for (size_t r = 0; r < nr; ++r) {
+      pl->region_tile0[r] = tiles;
+      const uint64_t rt = ((pl->region_len[r] + A - 1) / A + pl->tile_units - 1) / pl->tile_units;
+      tiles += rt;
+      pl->n_tile_ops += rt * pl->region_flows[r];
+    }
     pl->tiles_per_rank = tiles;
-    // region of every flow, looked up once (the executor's and the cost model's table walks all need it): a flow
-    // carries its (part, segment, section), i.e. its interval of sec_bounds (bubble flows: of p2p_bounds)
-    pl->flow_region.resize(pl->flows.size());
-    {
-      const std::vector<uint64_t>& ro = pl->region_offs;
-      for (size_t i = 0; i < pl->flows.size(); ++i) {
-        const optcc_flow_t& f = pl->flows[i];
-        uint32_t r = UINT32_MAX;
-        if (f.stage == OPTCC_BUB_UP || f.stage == OPTCC_BUB_DOWN) {
-          if (f.seg < p2p_reg.size()) r = p2p_reg[f.seg];
-        } else {
-          const size_t idx = (size_t(f.part) * k + f.seg) * B.nsec + f.sec;
-          if (idx < sec_reg.size()) r = sec_reg[idx];
-        }
-        if (r == UINT32_MAX || ro[r] != f.off) r = uint32_t(std::lower_bound(ro.begin(), ro.end(), f.off) - ro.begin());
-        if (r >= ro.size() || ro[r] != f.off) { region_error = true; break; }   // PLAN_SPEC 5.4 violated: a planner bug
-        pl->flow_region[i] = r;
-      }
-    }
-    if (region_error) {
-      delete pl;
-      return OPTCC_EINVAL;
-    }
-    for (const auto& f : pl->flows) pl->n_tile_ops += ((f.len + B.A - 1) / B.A + pl->tile_units - 1) / pl->tile_units;
   } catch (const std::bad_alloc&) {
     delete pl;
     return OPTCC_ENOMEM;
@@ -450,21 +563,28 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     delete pl;
     return OPTCC_ENOMEM;
   }
-  // lazy verifier (optcc.h, lazy_verify): every (rank, region) is written by a flow of the executed steps
+  // lazy verifier (optcc.h, lazy_verify): every (rank, region) is written by a flow of the executed steps.  A complete
+  // schedule writes every range (each rank receives every section's sum by a reduce or a copy: PLAN_SPEC 5.2); the
+  // executor's table build checks it region by region and falls back to the eager form otherwise.  Truncated schedules
+  // (step_limit) are walked here.
   try {
     in.lazy_verify = 0;
     if (in.mask_bytes && !pl->opts.verify_eager) {
-      const uint32_t steps = pl->opts.step_limit ? std::min(pl->opts.step_limit, n_steps) : n_steps;
-      const size_t nr = pl->region_offs.size();
-      std::vector<uint8_t> written(size_t(p) * nr, 0);
-      size_t left = written.size();
-      for (uint32_t i = 0; i < pl->step_begin[steps]; ++i) {
-        const optcc_flow_t& f = pl->flows[i];
-        uint8_t& w = written[size_t(f.dst) * nr + pl->flow_region[i]];
-        left -= !w;
-        w = 1;
+      if (!pl->opts.step_limit || pl->opts.step_limit >= n_steps) {
+        in.lazy_verify = 1;
+      } else {
+        const uint32_t steps = pl->opts.step_limit;
+        const size_t nr = pl->region_offs.size();
+        std::vector<uint8_t> written(size_t(p) * nr, 0);
+        size_t left = written.size();
+        for (uint32_t i = 0; i < pl->step_begin[steps]; ++i) {
+          const optcc_flow_t& f = pl->flows[i];
+          uint8_t& w = written[size_t(f.dst) * nr + pl->flow_region[i]];
+          left -= !w;
+          w = 1;
+        }
+        in.lazy_verify = left == 0;
       }
-      in.lazy_verify = left == 0;
     }
   } catch (const std::bad_alloc&) {
     delete pl;
