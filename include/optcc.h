@@ -19,7 +19,7 @@
 extern "C" {
 #endif
 
-#define OPTCC_ABI_VERSION 1
+#define OPTCC_ABI_VERSION 2
 #if defined(__GNUC__)
 #define OPTCC_API __attribute__((visibility("default")))
 #else
@@ -53,19 +53,23 @@ enum {
   OPTCC_SCHED_RING_DEGRADED = 1 /* NCCL-style ring over all p ranks whatever ell is: the paper's ICCL comparison
                                    point under the bandwidth model; g must be 1 */
 };
-/* executor modes */
+/* executor modes (opts.exec_mode).  All run the same tables and give the same bits. */
 enum {
-  OPTCC_EXEC_PERSISTENT = 0, /* one cooperative kernel for the whole schedule, grid barrier between steps */
-  OPTCC_EXEC_PER_STEP = 1,   /* one kernel launch per step (stream order is the step barrier) */
-  OPTCC_EXEC_DATAFLOW = 2    /* one cooperative kernel, no grid barrier: every flow is cut into tiles, tile-ops are
+  OPTCC_EXEC_AUTO = 0,       /* the library chooses from the plan's shape (reported in optcc_plan_info_t.exec_mode): the
+                                column executor, unless its work items cannot be indexed with 32 bits (then dataflow) */
+  OPTCC_EXEC_PERSISTENT = 1, /* one cooperative kernel for the whole schedule, grid barrier between steps: global step
+                                order, every intermediate state of the p buffers exists in memory */
+  OPTCC_EXEC_PER_STEP = 2,   /* one kernel launch per step (stream order is the step barrier) */
+  OPTCC_EXEC_DATAFLOW = 3,   /* one cooperative kernel, no grid barrier: every flow is cut into tiles, tile-ops are
                                 claimed in table order and wait on per-(rank, range) completion counters, so a
                                 tile-op starts as soon as the flows it depends on have finished there */
-  ,
-  OPTCC_EXEC_COLUMN = 3      /* one kernel, no synchronisation between CTAs at all: no flow ever mixes two element
+  OPTCC_EXEC_COLUMN = 4      /* one kernel, no synchronisation between CTAs at all: no flow ever mixes two element
                                 indices (a flow moves a range rank to rank), so every dependency of :138
-                                lies inside one element column.  A CTA takes a tile of one region and runs every flow
-                                over that region on it, in table order, each flow's loads and stores performed as
-                                listed; the tile's working set (p ranks) stays in L2 from the first hop to the last */
+                                lies inside one element column.  A tile of one region is taken through every flow over
+                                that region, in an order that respects those dependencies; every flow's loads, add and
+                                store are issued and the outputs are bit-identical to the step-ordered executors, but there
+                                is NO global step order and intermediate states of the p buffers need not reach HBM
+                                (dead partial sums are dropped from the caches): DESIGN.md 3 "what is kept, what is given up" */
 };
 
 typedef struct optcc_plan optcc_plan_t; /* opaque; immutable after creation except for cached device state */
@@ -88,7 +92,7 @@ typedef struct optcc_flow {
 
 typedef struct optcc_opts {
   uint32_t k;         /* segments; 0 = auto (PLAN_SPEC 2 "k"); else a multiple of 4 */
-  uint32_t exec_mode; /* OPTCC_EXEC_* */
+  uint32_t exec_mode; /* OPTCC_EXEC_*; 0 = auto */
   uint32_t grid_ctas; /* 0 = auto (SM count x resident CTAs per SM); else CTAs of the executor grid */
   uint32_t copy_path; /* copy (all-gather) tile-ops: 0 = auto (= 1, the faster one on the large configs), 1 = LDG/STG vector
                          copy by the streaming warps, 2 = cp.async.bulk (TMA 1-D) copy by the scheduler agents (dataflow only) */
@@ -103,6 +107,10 @@ typedef struct optcc_opts {
   uint32_t verify_eager; /* 1 = optcc_verify initialises the mask arrays and checks them with separate passes even when
                             the plan allows the lazy form (initial masks as constants, final masks checked by their last
                             writer); same result, for bisecting.  Truncated plans (step_limit) are always eager. */
+  uint32_t col_order; /* column executor, order of a region's flows: 0 = chain by chain (a flow is followed by the flow that
+                         reads what it wrote; any order respecting the dependencies of PAPER.md:138 inside the column gives
+                         the same bits), 1 = table order */
+  uint32_t reserved[5]; /* 0 */
 } optcc_opts_t;
 
 typedef struct optcc_plan_info {
@@ -132,7 +140,7 @@ typedef struct optcc_plan_info {
                                   the initial masks {r} as constants and lets the last writer of every range check the
                                   final mask (no initialising / checking pass over the arrays); 0: separate passes
                                   (some range keeps its initial mask, opts.verify_eager, or p > 128) */
-  uint32_t reserved;           /* 0 */
+  uint32_t exec_mode;          /* the executor this plan runs with (OPTCC_EXEC_*; never AUTO) */
 } optcc_plan_info_t;
 
 typedef struct optcc_cost_params {
@@ -174,7 +182,7 @@ typedef struct optcc_verify_result {
 /* Build the ell-weighted stage/chunk/step plan of PAPER.md 3 (problem statement :68) and 4.1-4.4 as frozen
  * in docs/PLAN_SPEC.md.  ell [host, p doubles]: slowdown factor of every rank, >= 1; ranks of one server
  * (floor(i/g)) must share ell (PXN pooling, :274, :850).  n: elements per rank.  *out receives a new plan
- * owned by the library (optcc_plan_destroy).  Same as optcc_plan_ex with opts = NULL (k auto, dataflow executor). */
+ * owned by the library (optcc_plan_destroy).  Same as optcc_plan_ex with opts = NULL (k auto, executor auto). */
 OPTCC_API int optcc_plan(int p, int g, const double* ell, uint64_t n, int dtype, optcc_plan_t** out);
 OPTCC_API int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dtype, const optcc_opts_t* opts,
                   optcc_plan_t** out);
@@ -206,6 +214,15 @@ OPTCC_API int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* pa
  * and one cooperative launch), so it can be captured into a CUDA graph on `stream` and replayed.
  * Errors: EINVAL (NULL / misaligned pointers), ECUDA. */
 OPTCC_API int optcc_prepare(optcc_plan_t* plan, void* workspace, void* stream);
+/* Host only, no device needed: the column executor's work list, for inspection and tests.  records [host, borrowed until
+ * optcc_plan_destroy]: n_records records of 32 bytes { off u64, len u64 (elements), src u16, dst u16, op u8, ksrc u8,
+ * kdin u8, kdout u8 (bf16 plans: 0 rank buffer, 1 fp32 partials), flags u32, pad u32 } -- the flows of the executed
+ * steps stored region by region, inside a region in the order the executor runs them (any order that respects the data
+ * dependencies of PAPER.md:138 inside the element column; opts.col_order).  items [host, borrowed]: n_items work items of
+ * 16 bytes { first record, end record, tile, units in the tile } (u32 each): a tile of tile_units 16-byte units of one
+ * region, taken through records [first, end).  EUNSUPPORTED unless the plan's executor is the column executor. */
+OPTCC_API int optcc_column_tables(optcc_plan_t* plan, const void** records, uint32_t* n_records, const void** items,
+                                  uint32_t* n_items);
 OPTCC_API int optcc_execute(optcc_plan_t* plan, void* const* bufs, void* workspace, void* stream);
 /* End-to-end variant: host_in [host array of p PINNED host pointers] are copied to bufs (device, as above),
  * the plan is executed, and every result is copied to host_out[i] (pinned; may equal host_in[i]).  All on

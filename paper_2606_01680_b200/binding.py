@@ -16,7 +16,8 @@ LIB_PATH = os.path.join(HERE, "liboptcc.so")
 
 OPTCC_F32, OPTCC_BF16 = 0, 1
 OPTCC_OK, OPTCC_EINVAL, OPTCC_EUNSUPPORTED, OPTCC_ENOMEM, OPTCC_ECUDA, OPTCC_EVERIFY = range(6)
-OPTCC_EXEC_PERSISTENT, OPTCC_EXEC_PER_STEP, OPTCC_EXEC_DATAFLOW, OPTCC_EXEC_COLUMN = 0, 1, 2, 3
+OPTCC_EXEC_AUTO, OPTCC_EXEC_PERSISTENT, OPTCC_EXEC_PER_STEP, OPTCC_EXEC_DATAFLOW, OPTCC_EXEC_COLUMN = 0, 1, 2, 3, 4
+EXEC_NAMES = {0: "auto", 1: "persistent", 2: "per_step", 3: "dataflow", 4: "column"}
 OPTCC_SCHED_OPTCC, OPTCC_SCHED_RING_DEGRADED = 0, 1
 ERROR_NAMES = {1: "EINVAL", 2: "EUNSUPPORTED", 3: "ENOMEM", 4: "ECUDA", 5: "EVERIFY"}
 
@@ -30,7 +31,8 @@ FLOW_DTYPE = np.dtype([
 
 class optcc_opts_t(C.Structure):
     _fields_ = [("k", C.c_uint32), ("exec_mode", C.c_uint32), ("grid_ctas", C.c_uint32), ("copy_path", C.c_uint32),
-                ("step_limit", C.c_uint32), ("tile_units", C.c_uint32), ("schedule", C.c_uint32), ("ordering", C.c_uint32), ("no_discard", C.c_uint32), ("verify_eager", C.c_uint32)]
+                ("step_limit", C.c_uint32), ("tile_units", C.c_uint32), ("schedule", C.c_uint32), ("ordering", C.c_uint32), ("no_discard", C.c_uint32), ("verify_eager", C.c_uint32),
+                ("col_order", C.c_uint32), ("reserved", C.c_uint32 * 5)]
 
 
 class optcc_plan_info_t(C.Structure):
@@ -39,7 +41,7 @@ class optcc_plan_info_t(C.Structure):
                [(n, C.c_uint32) for n in ("n_steps", "n_flows", "max_flows_per_step", "n_sec_bounds", "n_p2p_bounds", "mask_bytes")] + \
                [(n, C.c_uint64) for n in ("reduce_elems", "copy_elems", "workspace_bytes", "verify_workspace_bytes",
                                           "mask_offset_bytes", "padded_n")] + \
-               [("plan_build_seconds", C.c_double), ("lazy_verify", C.c_uint32), ("reserved", C.c_uint32)]
+               [("plan_build_seconds", C.c_double), ("lazy_verify", C.c_uint32), ("exec_mode", C.c_uint32)]
 
 
 class optcc_cost_params_t(C.Structure):
@@ -66,7 +68,7 @@ class OptccError(RuntimeError):
 
 _lib = None
 EXPORTS = ("optcc_plan", "optcc_plan_ex", "optcc_plan_destroy", "optcc_plan_info", "optcc_plan_tables", "optcc_cost",
-           "optcc_prepare", "optcc_execute", "optcc_execute_host", "optcc_execute_host_sharded", "optcc_verify", "optcc_strerror",
+           "optcc_prepare", "optcc_column_tables", "optcc_execute", "optcc_execute_host", "optcc_execute_host_sharded", "optcc_verify", "optcc_strerror",
            "optcc_last_cuda_error", "optcc_abi_version")
 
 
@@ -88,6 +90,7 @@ def load():
     lib.optcc_plan_tables.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
     lib.optcc_cost.argtypes = [vp, C.POINTER(optcc_cost_params_t), C.POINTER(optcc_cost_t)]
     lib.optcc_prepare.argtypes = [vp, vp, vp]
+    lib.optcc_column_tables.argtypes = [vp, C.POINTER(vp), C.POINTER(C.c_uint32), C.POINTER(vp), C.POINTER(C.c_uint32)]
     lib.optcc_execute.argtypes = [vp, C.POINTER(vp), vp, vp]
     lib.optcc_execute_host.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), vp, vp]
     lib.optcc_execute_host_sharded.argtypes = [vp, u64, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), vp, vp]
@@ -149,11 +152,11 @@ class Plan:
             pass
 
 
-def optcc_plan(p, g, ell, n, dtype, k=0, exec_mode=OPTCC_EXEC_DATAFLOW, grid_ctas=0, copy_path=0, step_limit=0, tile_units=0, schedule=0, ordering=0, no_discard=0, verify_eager=0):
+def optcc_plan(p, g, ell, n, dtype, k=0, exec_mode=OPTCC_EXEC_AUTO, grid_ctas=0, copy_path=0, step_limit=0, tile_units=0, schedule=0, ordering=0, no_discard=0, verify_eager=0, col_order=0):
     """optcc_plan_ex: returns a Plan.  ell: sequence of p floats."""
     lib = load()
     ell_arr = (C.c_double * len(ell))(*[float(x) for x in ell])
-    opts = optcc_opts_t(k, exec_mode, grid_ctas, copy_path, step_limit, tile_units, schedule, ordering, no_discard, verify_eager)
+    opts = optcc_opts_t(k, exec_mode, grid_ctas, copy_path, step_limit, tile_units, schedule, ordering, no_discard, verify_eager, col_order)
     h = C.c_void_p()
     rc = lib.optcc_plan_ex(int(p), int(g), ell_arr, int(n), int(dtype), C.byref(opts), C.byref(h))
     if rc:
@@ -177,6 +180,29 @@ def optcc_plan_tables(plan):
 
     return (view(f, i["n_flows"], FLOW_DTYPE), view(sb, i["n_steps"] + 1, np.uint32),
             view(sec, i["n_sec_bounds"], np.uint64), view(p2p, i["n_p2p_bounds"], np.uint64))
+
+
+# the column executor's record (optcc.h: optcc_column_tables): 32 bytes
+COLREC_DTYPE = np.dtype([("off", "<u8"), ("len", "<u8"), ("src", "<u2"), ("dst", "<u2"), ("op", "u1"), ("ksrc", "u1"),
+                         ("kdin", "u1"), ("kdout", "u1"), ("flags", "<u4"), ("pad", "<u4")], align=False)
+COLITEM_DTYPE = np.dtype([("first", "<u4"), ("end", "<u4"), ("tile", "<u4"), ("units", "<u4")], align=False)
+
+
+def optcc_column_tables(plan):
+    """Copies of the column executor's host tables: (records[COLREC_DTYPE], items[COLITEM_DTYPE]).  No device needed."""
+    rec, it = C.c_void_p(), C.c_void_p()
+    nrec, nit = C.c_uint32(), C.c_uint32()
+    rc = load().optcc_column_tables(plan.handle, C.byref(rec), C.byref(nrec), C.byref(it), C.byref(nit))
+    if rc:
+        raise OptccError(rc, "optcc_column_tables")
+
+    def view(ptr, count, dt):
+        if count == 0 or not ptr.value:
+            return np.zeros(0, dtype=dt)
+        buf = (C.c_char * (count * np.dtype(dt).itemsize)).from_address(ptr.value)
+        return np.frombuffer(buf, dtype=dt, count=count).copy()
+
+    return view(rec, nrec.value, COLREC_DTYPE), view(it, nit.value, COLITEM_DTYPE)
 
 
 def optcc_cost(plan, alpha=0.0, beta=1.0):

@@ -9,6 +9,7 @@
 #include <cstring>
 #include <new>
 #include <atomic>
+#include <chrono>
 #include <mutex>
 #include <unordered_map>
 #include <vector>
@@ -57,6 +58,7 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
                                               unsigned long long uend, unsigned int& overlaps, const PolX& pol,
                                               char* stage = nullptr, bool from_stage = false) {
   using MT = ModeTraits<MODE>;
+  const unsigned int tid = group_tid<NT>();
   const unsigned long long A = P.unit_elems;
   const unsigned long long e0 = ubeg * A;
   unsigned long long e1 = uend * A;
@@ -75,8 +77,8 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
     } else if (!from_stage) {
       range_copy16<4, NT>(s, d, vbeg, vend, pol);
     }
-    if (threadIdx.x < tail) {
-      unsigned long long e = vend * 4 + threadIdx.x;
+    if (tid < tail) {
+      unsigned long long e = vend * 4 + tid;
       const float* sf = reinterpret_cast<const float*>(s);
       float* df = reinterpret_cast<float*>(d);
       float x = __ldcg(sf + e);
@@ -87,7 +89,7 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
     constexpr int EB = MT::ESIZE;
     const char* s = rank_ptr(P, f.src) + f.off * EB;
     char* d = rank_ptr(P, f.dst) + f.off * EB;
-    const unsigned int lazy = f.flags & (DFLOW_SRC_INIT | DFLOW_DST_INIT | DFLOW_FINAL);
+    const unsigned int lazy = P.mask_lazy ? f.flags & (DFLOW_SRC_INIT | DFLOW_DST_INIT | DFLOW_FINAL) : 0u;
     const unsigned long long full0 = P.n_ranks >= 64 ? ~0ull : ((1ull << P.n_ranks) - 1ull);
     if (lazy) {   // lazy verifier: initial masks are constants, the last writer checks the final mask (range_mask_lazy)
       const unsigned long long full1 = P.n_ranks > 64 ? (P.n_ranks >= 128 ? ~0ull : ((1ull << (P.n_ranks - 64)) - 1ull)) : 0ull;
@@ -100,8 +102,8 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
     } else {
       range_copy16<4, NT>(s, d, vbeg, vend, pol);
     }
-    if (threadIdx.x < tail) {  // ragged end (n not a multiple of the elements per vector): one element per thread
-      const unsigned long long e = vend * MT::VE + threadIdx.x;   // (EB <= 8 here: a 16-byte mask is a whole vector)
+    if (tid < tail) {  // ragged end (n not a multiple of the elements per vector): one element per thread
+      const unsigned long long e = vend * MT::VE + tid;   // (EB <= 8 here: a 16-byte mask is a whole vector)
       unsigned long long x, y = 0;
       if (lazy & DFLOW_SRC_INIT) {
         x = 1ull << f.src;
@@ -156,8 +158,8 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
     } else {
       range_copy16<4, NT>(s, dout, vbeg * 2, vend * 2, pol);         // fp32 partial -> fp32 partial: two vectors per unit
     }
-    if (threadIdx.x < tail) {
-      unsigned long long e = vend * 8 + threadIdx.x;
+    if (tid < tail) {
+      unsigned long long e = vend * 8 + tid;
       float x = f.ksrc ? __ldcg(reinterpret_cast<const float*>(s) + e)
                        : bf16_to_f32(__ldcg(reinterpret_cast<const unsigned short*>(s) + e));
       if (f.op == 0) {
@@ -510,8 +512,8 @@ constexpr int COL_THREADS = DF_COMPUTE_THREADS;
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
-// First touches ahead of time.  The ranges of flow f that no earlier flow of the region has written (DFLOW_SRC_RAW /
-// DFLOW_DST_RAW, a walk of the table on the host: a ring hop's destination is the next rank's untouched section, the
+// First touches ahead of time.  The ranges of flow f that no earlier flow of the region has written (DFLOW_SRC_INIT /
+// DFLOW_DST_INIT, a walk of the table on the host: a ring hop's destination is the next rank's untouched section, the
 // straggler's raw section, a raw P2P piece) are DRAM accesses; they are requested col_pf_dist flows before f runs.
 // Every thread asks for the vectors it will load itself (NT-strided, like the range operations).  f32 and bf16 data
 // only (raw data always lives in the rank buffer): the verifier's first touches are constants.
@@ -520,12 +522,12 @@ __device__ __forceinline__ void prefetch_raw(const ExecParams& P, const DFlow& f
   if (is_mask_mode(MODE)) return;
   const unsigned int esz = MODE == MODE_F32 ? 4 : 2;
   auto span = [&](const char* base) {
-    const char* q = base + (ubeg + threadIdx.x) * 16;
-    if (P.col_pf_l2) { for (unsigned int u = threadIdx.x; u < n; u += NT, q += NT * 16) prefetch_l2(q); }
-    else { for (unsigned int u = threadIdx.x; u < n; u += NT, q += NT * 16) prefetch_l1(q); }
+    const char* q = base + (ubeg + group_tid<NT>()) * 16;
+    if (P.col_pf_l2) { for (unsigned int u = group_tid<NT>(); u < n; u += NT, q += NT * 16) prefetch_l2(q); }
+    else { for (unsigned int u = group_tid<NT>(); u < n; u += NT, q += NT * 16) prefetch_l1(q); }
   };
-  if (f.flags & DFLOW_SRC_RAW) span(rank_ptr(P, f.src) + f.off * esz);
-  if (f.op == 0 && (f.flags & DFLOW_DST_RAW)) span(rank_ptr(P, f.dst) + f.off * esz);
+  if (f.flags & DFLOW_SRC_INIT) span(rank_ptr(P, f.src) + f.off * esz);
+  if (f.op == 0 && (f.flags & DFLOW_DST_INIT)) span(rank_ptr(P, f.dst) + f.off * esz);
 }
 
 constexpr unsigned int COL_REC = 256;   // flow records staged in shared memory at a time (8 KB)
@@ -545,7 +547,7 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
   const unsigned int D = is_mask_mode(MODE) ? 0u : (P.col_pf_dist < COL_PF_MAX ? P.col_pf_dist : COL_PF_MAX);
   extern __shared__ __align__(128) char s_stage_col[];   // bulk all-gather path: the tile of the sum being distributed
   const bool bulk = !is_mask_mode(MODE) && P.col_bulk != 0;
-  const unsigned long long bulk_pol = make_policy(P.pad0);   // L2 policy of the bulk stores
+  const unsigned long long bulk_pol = make_policy(P.col_bulk_policy);   // L2 policy of the bulk stores
   if (threadIdx.x == 0) {
     s_item[0] = atomicAdd(&P.ctrl->ticket, 1ull);
     s_item[1] = atomicAdd(&P.ctrl->ticket, 1ull);
@@ -654,6 +656,91 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Column executor, warp-wide tiles: the same work items, but one WARP takes a tile (128 units = 4 vectors per lane for
+// f32) through its region's list, and the warps of a CTA never wait for each other: no block barrier anywhere, so a
+// warp whose loads miss does not hold up thirteen others at the next barrier (the CTA-wide kernel spends a third of its
+// stall time there), short regions (C4 at large k: 273 units) keep every warp busy, and items are claimed per warp.
+// Records are read straight from the table (uniform loads, L1 hits after the first warp).  Everything else -- table
+// order per element, every flow's loads, add and store issued, first touches requested one flow ahead, dead-source
+// discard, the bulk all-gather path with one stage per warp -- is as in optcc_column_kernel.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ DFlow load_record(const DFlow* p) {
+  const uint4 lo = __ldg(reinterpret_cast<const uint4*>(p)), hi = __ldg(reinterpret_cast<const uint4*>(p) + 1);
+  DFlow f;
+  memcpy(&f, &lo, 16);
+  memcpy(reinterpret_cast<char*>(&f) + 16, &hi, 16);
+  return f;
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel(const __grid_constant__ ExecParams P) {
+  extern __shared__ __align__(128) char s_stage_w[];   // bulk all-gather path: one tile per warp
+  const unsigned int lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  char* const stage = s_stage_w + (size_t)warp * P.tile_units * 16;
+  unsigned int overlaps = 0;
+  const Pol pol0 = make_policies(P.l2_hints);
+  PolL1 pol;                         // a tile is private to its warp for the whole launch: loads and stores through L1
+  pol.lds = pol0.lds; pol.ldd = pol0.ldd; pol.st = pol0.st;
+  const bool bulk = !is_mask_mode(MODE) && P.col_bulk != 0;
+  const unsigned long long bulk_pol = make_policy(P.col_bulk_policy);   // L2 policy of the bulk stores
+  const bool pf = !is_mask_mode(MODE) && P.col_pf_dist != 0;
+  for (;;) {
+    unsigned long long it = 0;
+    if (lane == 0) it = atomicAdd(&P.ctrl->ticket, 1ull);
+    it = __shfl_sync(0xFFFFFFFFu, it, 0);
+    if (it >= P.col_n_items) break;
+    const uint4 item = __ldg(P.col_items + it);
+    const unsigned int fb = item.x, fe = item.y;
+    const unsigned long long ubeg = (unsigned long long)item.z * P.tile_units, uend = ubeg + item.w;
+    DFlow cur = load_record(P.flows + fb);
+    if (pf) prefetch_raw<MODE, 32>(P, cur, ubeg, item.w);
+    int prev_cls = -1;
+    for (unsigned int j = fb; j < fe; ++j) {
+      const DFlow nxt = load_record(P.flows + (j + 1 < fe ? j + 1 : j));
+      if (pf && j + 1 < fe) prefetch_raw<MODE, 32>(P, nxt, ubeg, item.w);   // first touches of the next flow
+      if (MODE == MODE_BF16) {
+        // a copy of fp32 partials moves two vectors per unit, lane i taking vector i instead of unit i: when the
+        // lane-to-element mapping changes between consecutive flows the warp synchronises
+        const int cls = (cur.op == 1 && cur.ksrc != 0) ? 1 : 0;
+        if (prev_cls >= 0 && cls != prev_cls) __syncwarp();
+        prev_cls = cls;
+      }
+      const unsigned int fl = cur.flags;
+      if (bulk && (fl & DFLOW_STAGE_OUT)) {
+        // the stage is rewritten: the previous tile's bulk stores must have read it
+        if (lane == 0) bulk_wait_read_all();
+        __syncwarp();
+        process_piece<MODE, 32>(P, cur, ubeg, uend, overlaps, pol, stage, false);
+        // this lane's generic-proxy writes (the stage; its earlier stores to ranges the bulk stores will overwrite) are
+        // ordered before the async-proxy operations lane 0 issues after the warp barrier
+        fence_proxy_async();
+        __syncwarp();
+      } else if (bulk && (fl & DFLOW_FROM_STAGE)) {
+        if (lane == 0) {
+          constexpr unsigned long long ESZ = MODE == MODE_F32 ? 4 : 2, VE = 16 / ESZ;
+          const unsigned long long e0 = ubeg * P.unit_elems;
+          unsigned long long e1 = uend * P.unit_elems;
+          if (e1 > cur.len) e1 = cur.len;
+          const unsigned long long v0 = e0 / VE, v1 = e1 / VE;
+          if (v1 > v0) bulk_s2g_hint(rank_ptr(P, cur.dst) + cur.off * ESZ + v0 * 16, stage, (unsigned int)((v1 - v0) * 16), bulk_pol);
+        }
+        process_piece<MODE, 32>(P, cur, ubeg, uend, overlaps, pol, nullptr, true);   // (ragged end of a buffer only)
+      } else {
+        process_piece<MODE, 32>(P, cur, ubeg, uend, overlaps, pol);
+      }
+      __syncwarp();   // orders a lane's dead-source discard of a 128-byte line before the other lanes' later stores to it
+      cur = nxt;
+    }
+  }
+  if (bulk && lane == 0) bulk_wait_all();   // the stage stays valid until every bulk store has read it
+  if (is_mask_mode(MODE)) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) overlaps += __shfl_xor_sync(0xFFFFFFFFu, overlaps, o);
+    if (lane == 0 && overlaps) atomicAdd(&P.ctrl->overlap, (unsigned long long)overlaps);
+  }
+}
+
 // masks[r][e] = {r}: blockIdx.y = rank, 16-byte stores over the rank's padded array; eb = bytes per mask
 __global__ void __launch_bounds__(256) optcc_mask_init_kernel(char* masks, unsigned long long padded_n, unsigned int eb) {
   const unsigned int r = blockIdx.y;
@@ -739,12 +826,14 @@ struct optcc_exec_state {
   bool df_ok = false;             // counters fit 32-bit indices
   bool big_ops = false;           // average tile-op >= 1792 units (decides the ring depth)
   bool lazy_masks = false;        // the verifier needs no init / check passes (see assign_mask_flags)
+  bool built = false;             // every table of this state is complete (set last; cleared on any failure)
+  bool host_built = false;        // the device-independent tables are complete
   std::vector<DDep> deps;         // [n_flows]
   std::vector<TileOp> ops;        // [n_tile_ops], table order
   std::vector<uint64_t> step_op_begin;   // [n_steps + 1]
   // column executor
   bool column = false;
-  std::vector<DFlow> col_dflows;         // the executed flows, region by region (table order inside a region)
+  optcc_rawvec<DFlow> col_dflows;        // the executed flows, region by region (chain order inside a region)
   std::vector<uint32_t> col_reg_begin;   // [regions + 1]
   std::vector<uint4> col_items;          // (first flow, end flow, tile, units in the tile)
 };
@@ -851,132 +940,366 @@ void assign_mask_flags(optcc_plan_t* pl, optcc_exec_state* st) {
   st->lazy_masks = true;
 }
 
-// Dead-source flags without the dataflow tables (column executor): flow i is the only reader of its source range since
-// the last write and the next access to that (rank, region) is a plain overwrite by a copy flow -- the same rule as in
-// build_dataflow_tables.
-void assign_dead_source_flags(optcc_plan_t* pl, optcc_exec_state* st) {
-  const optcc_plan_info_t& in = pl->info;
-  if (pl->opts.no_discard || pl->opts.step_limit) return;
-  const size_t nr = pl->region_offs.size();
-  std::vector<uint32_t> readers(size_t(in.p) * nr, 0);
-  std::vector<uint8_t> sole_reader(in.n_flows, 0);
-  for (uint32_t i = 0; i < in.n_flows; ++i) {
-    const optcc_flow_t& f = pl->flows[i];
-    const size_t reg = pl->flow_region[i];
-    sole_reader[i] = readers[size_t(f.src) * nr + reg]++ == 0;
-    readers[size_t(f.dst) * nr + reg] = 0;
+// =====================================================================================================
+// Column executor tables.  The flows of the executed steps are stored region by region (a stable parallel counting
+// sort of the table by region: table order is kept inside a region); then every region's list is finished on its own
+// -- lists are independent, so this runs on a few host threads:
+//   * order: any order that respects the data dependencies inside the column gives the same bits; the
+//     list is rearranged chain by chain (a flow is followed by the flow that reads what it wrote whenever that one is
+//     ready), so that a CTA keeps one partial tile live instead of one per interleaved chain (C4: the collect /
+//     distribute flows of 16 servers interleave in table order);
+//   * storage kinds of bf16 plans (fp32 shadow while 1 < contributors < p);
+//   * DFLOW_SRC_INIT / DST_INIT (first touches), DFLOW_FINAL (last writes), DFLOW_DEAD_SRC, and the bulk all-gather
+//     flags DFLOW_STAGE_OUT / FROM_STAGE;
+//   * coverage: the lazy verifier needs every rank's range written by the list.
+// Regions of one class (same part and section, another segment) have the same list up to the offset: the work is done
+// once per class and copied after an element-wise check of (src, dst, op).
+// =====================================================================================================
+struct ColScratch {
+  std::vector<uint16_t> cnt;
+  std::vector<uint8_t> written, next, bulkw, sole, done;
+  std::vector<uint32_t> readers, val, consumers;
+  std::vector<int32_t> last_writer, rd_head, rd_next;
+  std::vector<uint32_t> e_from, e_to, succ_begin, succ, indeg, order, heap;
+  std::vector<DFlow> tmp, rep_final;
+  std::vector<uint64_t> rep_key;     // src, dst, op of the representative's flows, table order
+  std::vector<uint32_t> rep_order;
+  bool rep_valid = false, rep_covered = false;
+  void init(uint32_t p) {
+    cnt.resize(p); written.resize(p); next.resize(p); bulkw.resize(p); readers.resize(p); val.resize(p);
+    last_writer.resize(p); rd_head.resize(p);
   }
+};
+
+inline uint64_t flow_key(const DFlow& f) { return (uint64_t)f.src << 32 | (uint64_t)f.dst << 8 | f.op; }
+
+// chain-by-chain order of one list (see above); out: sc.order[0..n)
+void chain_order(const DFlow* L, uint32_t n, uint32_t p, ColScratch& sc) {
+  sc.e_from.clear(); sc.e_to.clear();
+  sc.rd_next.assign(n, -1);
+  std::fill(sc.last_writer.begin(), sc.last_writer.end(), -1);
+  std::fill(sc.rd_head.begin(), sc.rd_head.end(), -1);
+  for (uint32_t i = 0; i < n; ++i) {
+    const uint32_t s = L[i].src, d = L[i].dst;
+    const int32_t lws = sc.last_writer[s], lwd = sc.last_writer[d];
+    if (lws >= 0) { sc.e_from.push_back(lws); sc.e_to.push_back(i); }                  // read after write
+    if (lwd >= 0 && lwd != lws) { sc.e_from.push_back(lwd); sc.e_to.push_back(i); }    // write after write (a reduce also reads)
+    for (int32_t r = sc.rd_head[d]; r >= 0; r = sc.rd_next[r]) { sc.e_from.push_back(r); sc.e_to.push_back(i); }   // write after read
+    sc.rd_head[d] = -1;
+    sc.rd_next[i] = sc.rd_head[s];
+    sc.rd_head[s] = (int32_t)i;
+    sc.last_writer[d] = (int32_t)i;
+  }
+  const size_t ne = sc.e_from.size();
+  sc.succ_begin.assign(size_t(n) + 1, 0);
+  sc.indeg.assign(n, 0);
+  for (size_t e = 0; e < ne; ++e) { sc.succ_begin[sc.e_from[e] + 1]++; sc.indeg[sc.e_to[e]]++; }
+  for (uint32_t i = 0; i < n; ++i) sc.succ_begin[i + 1] += sc.succ_begin[i];
+  sc.succ.resize(ne);
+  {
+    std::vector<uint32_t>& pos = sc.heap;      // (borrowed as a cursor array)
+    pos.assign(sc.succ_begin.begin(), sc.succ_begin.end() - 1);
+    for (size_t e = 0; e < ne; ++e) sc.succ[pos[sc.e_from[e]]++] = sc.e_to[e];
+  }
+  sc.done.assign(n, 0);
+  sc.order.resize(n);
+  std::vector<uint32_t>& heap = sc.heap;       // min-heap of ready flows (lazy deletion through done[])
+  heap.clear();
+  auto cmp = [](uint32_t a, uint32_t b) { return a > b; };
+  for (uint32_t i = 0; i < n; ++i) if (sc.indeg[i] == 0) heap.push_back(i);
+  std::make_heap(heap.begin(), heap.end(), cmp);
+  int64_t last = -1;
+  for (uint32_t k = 0; k < n; ++k) {
+    int64_t pick = -1;
+    if (last >= 0) {   // prefer the flow that reads what `last` wrote, then another flow into the same destination
+      const uint32_t d = L[last].dst;
+      int64_t same_dst = -1;
+      for (uint32_t e = sc.succ_begin[last]; e < sc.succ_begin[last + 1]; ++e) {
+        const uint32_t v = sc.succ[e];
+        if (sc.done[v] || sc.indeg[v] != 0) continue;
+        if (L[v].src == d) { if (pick < 0 || v < pick) pick = v; }
+        else if (L[v].dst == d) { if (same_dst < 0 || v < same_dst) same_dst = v; }
+      }
+      if (pick < 0) pick = same_dst;
+    }
+    if (pick < 0) {
+      while (sc.done[heap.front()]) { std::pop_heap(heap.begin(), heap.end(), cmp); heap.pop_back(); }
+      pick = heap.front();
+      std::pop_heap(heap.begin(), heap.end(), cmp);
+      heap.pop_back();
+    }
+    sc.order[k] = (uint32_t)pick;
+    sc.done[pick] = 1;
+    for (uint32_t e = sc.succ_begin[pick]; e < sc.succ_begin[pick + 1]; ++e) {
+      const uint32_t v = sc.succ[e];
+      if (--sc.indeg[v] == 0) { heap.push_back(v); std::push_heap(heap.begin(), heap.end(), cmp); }
+    }
+    last = pick;
+  }
+}
+
+struct ColBuildOpts { uint32_t p; bool bf16, discard, bulk, reorder; };
+
+// Finish one list in place (L holds the region's flows in table order, flags and kinds clear).  Returns whether every
+// rank's range is written by the list.
+bool finish_region(DFlow* L, uint32_t n, const ColBuildOpts& o, ColScratch& sc) {
+  const uint32_t p = o.p;
+  // the same list as the class representative?  then its order, kinds and flags apply
+  bool same = sc.rep_valid && sc.rep_key.size() == n;
+  for (uint32_t i = 0; i < n && same; ++i) same = sc.rep_key[i] == flow_key(L[i]);
+  if (same) {
+    sc.tmp.assign(L, L + n);
+    for (uint32_t j = 0; j < n; ++j) {
+      DFlow f = sc.tmp[sc.rep_order[j]];
+      const DFlow& r = sc.rep_final[j];
+      f.ksrc = r.ksrc; f.kdin = r.kdin; f.kdout = r.kdout; f.flags = r.flags;
+      L[j] = f;
+    }
+    return sc.rep_covered;
+  }
+  sc.rep_key.resize(n);
+  for (uint32_t i = 0; i < n; ++i) sc.rep_key[i] = flow_key(L[i]);
+  if (o.reorder && n > 2) {
+    chain_order(L, n, p, sc);
+    sc.tmp.assign(L, L + n);
+    for (uint32_t j = 0; j < n; ++j) L[j] = sc.tmp[sc.order[j]];
+    sc.rep_order = sc.order;
+  } else {
+    sc.rep_order.resize(n);
+    for (uint32_t j = 0; j < n; ++j) sc.rep_order[j] = j;
+  }
+  // forwards: first touches, storage kinds, sole readers
+  std::fill(sc.written.begin(), sc.written.end(), 0);
+  std::fill(sc.readers.begin(), sc.readers.end(), 0);
+  std::fill(sc.cnt.begin(), sc.cnt.end(), 1);
+  sc.sole.resize(n);
+  auto kind_of = [&](uint32_t c) -> unsigned char { return (c == 1 || c >= p) ? OPTCC_KIND_BUF : OPTCC_KIND_F32; };
+  uint32_t covered = 0;
+  for (uint32_t i = 0; i < n; ++i) {
+    DFlow& f = L[i];
+    unsigned int fl = 0;
+    if (!sc.written[f.src]) fl |= DFLOW_SRC_INIT;
+    if (!sc.written[f.dst]) fl |= DFLOW_DST_INIT;
+    sc.sole[i] = sc.readers[f.src]++ == 0;
+    sc.readers[f.dst] = 0;
+    covered += !sc.written[f.dst];
+    sc.written[f.dst] = 1;
+    const uint32_t cs = sc.cnt[f.src], cd = sc.cnt[f.dst], out = f.op == OPTCC_OP_REDUCE ? cs + cd : cs;
+    if (o.bf16) { f.ksrc = kind_of(cs); f.kdin = kind_of(cd); f.kdout = kind_of(out); }
+    sc.cnt[f.dst] = (uint16_t)std::min<uint32_t>(out, 65535);
+    f.flags = fl;
+  }
+  // backwards: last writes; dead sources (the flow is the only reader of its source range since the last write and
+  // the next access to that range is a plain overwrite by a copy flow: only reduce flows act on it)
   enum : uint8_t { NEXT_NONE = 0, NEXT_READ, NEXT_COPY_WRITE, NEXT_REDUCE_WRITE };
-  std::vector<uint8_t> next(size_t(in.p) * nr, NEXT_NONE);
-  for (uint32_t i = in.n_flows; i-- > 0;) {
-    const optcc_flow_t& f = pl->flows[i];
-    const size_t reg = pl->flow_region[i];
-    const size_t ls = size_t(f.src) * nr + reg, ld = size_t(f.dst) * nr + reg;
-    if (f.op == OPTCC_OP_REDUCE && next[ls] == NEXT_COPY_WRITE && sole_reader[i]) st->dflows[i].flags |= 1u;
-    next[ld] = f.op == OPTCC_OP_COPY ? NEXT_COPY_WRITE : NEXT_REDUCE_WRITE;
-    next[ls] = NEXT_READ;
+  std::fill(sc.next.begin(), sc.next.end(), (uint8_t)NEXT_NONE);
+  std::fill(sc.written.begin(), sc.written.end(), 0);
+  for (uint32_t i = n; i-- > 0;) {
+    DFlow& f = L[i];
+    if (!sc.written[f.dst]) f.flags |= DFLOW_FINAL;
+    sc.written[f.dst] = 1;
+    if (o.discard && f.op == OPTCC_OP_REDUCE && sc.next[f.src] == NEXT_COPY_WRITE && sc.sole[i]) f.flags |= DFLOW_DEAD_SRC;
+    sc.next[f.dst] = f.op == OPTCC_OP_COPY ? NEXT_COPY_WRITE : NEXT_REDUCE_WRITE;
+    sc.next[f.src] = NEXT_READ;
   }
+  // Bulk all-gather path (data runs): find the reduce flows whose sum later copy flows distribute (DFLOW_STAGE_OUT: the
+  // CTA keeps the tile in shared memory) and the copy flows whose source range holds exactly the staged tile at that
+  // point (DFLOW_FROM_STAGE: one cp.async.bulk store).  Value numbering: a reduce gives its destination a new value,
+  // a copy gives it the source's value.  One stage: a new sum is only staged when every copy of the previous one has
+  // been issued.  A list in which a range written by a bulk store is touched again by any later flow (never the case
+  // in an AllReduce plan: the all-gather's copies are final) keeps the LDG / STG path entirely.
+  if (o.bulk) {
+    for (uint32_t i = 0; i < p; ++i) sc.val[i] = i;
+    sc.consumers.assign(size_t(p) + n, 0);
+    uint32_t next_id = p;
+    for (uint32_t i = 0; i < n; ++i) {
+      const DFlow& f = L[i];
+      if (f.op == OPTCC_OP_REDUCE) sc.val[f.dst] = next_id++;
+      else { sc.consumers[sc.val[f.src]]++; sc.val[f.dst] = sc.val[f.src]; }
+    }
+    for (uint32_t i = 0; i < p; ++i) sc.val[i] = i;
+    std::fill(sc.bulkw.begin(), sc.bulkw.end(), 0);
+    next_id = p;
+    uint32_t staged = UINT32_MAX, pending = 0;
+    bool ok = true;
+    for (uint32_t i = 0; i < n && ok; ++i) {
+      DFlow& f = L[i];
+      if (f.op == OPTCC_OP_REDUCE) {
+        if (sc.bulkw[f.src] || sc.bulkw[f.dst]) { ok = false; break; }
+        const uint32_t id = next_id++;
+        sc.val[f.dst] = id;
+        if (sc.consumers[id] && pending == 0 && (!o.bf16 || f.kdout == OPTCC_KIND_BUF)) {
+          f.flags |= DFLOW_STAGE_OUT;
+          staged = id;
+          pending = sc.consumers[id];
+        }
+      } else {
+        if (sc.val[f.src] == staged && (!o.bf16 || (f.ksrc == OPTCC_KIND_BUF && f.kdout == OPTCC_KIND_BUF))) {
+          if (sc.bulkw[f.dst]) { ok = false; break; }
+          f.flags |= DFLOW_FROM_STAGE;
+          sc.bulkw[f.dst] = 1;
+          --pending;
+        } else if (sc.bulkw[f.src] || sc.bulkw[f.dst]) {
+          ok = false;
+          break;
+        } else if (sc.val[f.src] == staged) {
+          --pending;
+        }
+        sc.val[f.dst] = sc.val[f.src];
+      }
+    }
+    if (!ok) for (uint32_t i = 0; i < n; ++i) L[i].flags &= ~(DFLOW_STAGE_OUT | DFLOW_FROM_STAGE);
+  }
+  sc.rep_final.assign(L, L + n);
+  sc.rep_covered = covered == p;
+  sc.rep_valid = true;
+  return sc.rep_covered;
 }
 
-// First touches (column executor's look-ahead): DFLOW_SRC_RAW / DFLOW_DST_RAW mark the ranges no earlier flow of the
-// table has written -- reading them is a DRAM access, requested ahead of time by prefetch_raw.
-void assign_raw_flags(optcc_plan_t* pl, optcc_exec_state* st) {
-  const optcc_plan_info_t& in = pl->info;
-  const size_t nr = pl->region_offs.size();
-  std::vector<uint8_t> written(size_t(in.p) * nr, 0);
-  for (uint32_t i = 0; i < in.n_flows; ++i) {
-    const optcc_flow_t& f = pl->flows[i];
-    const size_t reg = pl->flow_region[i];
-    if (!written[size_t(f.src) * nr + reg]) st->dflows[i].flags |= DFLOW_SRC_RAW;
-    if (!written[size_t(f.dst) * nr + reg]) st->dflows[i].flags |= DFLOW_DST_RAW;
-    written[size_t(f.dst) * nr + reg] = 1;
-  }
+// Finish a list from scratch (no representative to compare with).
+inline bool finish_fresh(DFlow* L, uint32_t n, const ColBuildOpts& o, ColScratch& sc) {
+  sc.rep_valid = false;
+  return finish_region(L, n, o, sc);
 }
 
-// Column executor tables: the flows of the executed steps region by region (a stable counting sort of the table by
-// region, so table order is kept inside a region) and one work item per (region, tile).
-bool build_column_tables(optcc_plan_t* pl, optcc_exec_state* st) {   // false: PLAN_SPEC 5.4 violated (a planner bug)
+// Builds col_dflows / col_reg_begin / col_items; sets *all_covered (every rank's range of every region is written by
+// the executed steps -- what the lazy verifier needs).
+void build_column_state(optcc_plan_t* pl, optcc_exec_state* st, bool* all_covered) {
   const optcc_plan_info_t& in = pl->info;
   const uint64_t A = in.unit_elems, TU = pl->tile_units;
   const size_t nr = pl->region_offs.size();
   const uint32_t steps = pl->opts.step_limit ? std::min(pl->opts.step_limit, in.n_steps) : in.n_steps;
   const uint32_t nf = pl->step_begin[steps];
-  st->col_reg_begin.assign(nr + 1, 0);
-  for (uint32_t i = 0; i < nf; ++i) st->col_reg_begin[pl->flow_region[i] + 1]++;
-  for (size_t r = 0; r < nr; ++r) st->col_reg_begin[r + 1] += st->col_reg_begin[r];
-  st->col_dflows.resize(nf);
-  std::vector<uint32_t> pos(st->col_reg_begin.begin(), st->col_reg_begin.end() - 1);
-  for (uint32_t i = 0; i < nf; ++i) st->col_dflows[pos[pl->flow_region[i]]++] = st->dflows[i];
+  ColBuildOpts o;
+  o.p = in.p;
+  o.bf16 = in.dtype == OPTCC_BF16;
+  o.discard = !pl->opts.no_discard && !pl->opts.step_limit;   // (a truncated schedule: the overwrite that makes a range dead might never run)
+  o.bulk = pl->opts.copy_path != 1;
+  o.reorder = pl->opts.col_order != 1;
+  // classes: regions of the same part and section (another segment)
+  std::vector<uint32_t> cls_begin, cls_regions;
+  {
+    uint32_t ncls = 0;
+    for (uint32_t c : pl->region_class) ncls = std::max(ncls, c + 1);
+    cls_begin.assign(size_t(ncls) + 1, 0);
+    for (uint32_t c : pl->region_class) cls_begin[c + 1]++;
+    for (uint32_t c = 0; c < ncls; ++c) cls_begin[c + 1] += cls_begin[c];
+    cls_regions.resize(nr);
+    std::vector<uint32_t> pos(cls_begin.begin(), cls_begin.end() - 1);
+    for (size_t r = 0; r < nr; ++r) cls_regions[pos[pl->region_class[r]]++] = (uint32_t)r;
+  }
+  const size_t ncls = cls_begin.size() - 1;
+  std::atomic<uint32_t> uncovered{0};
+  auto t_begin = std::chrono::steady_clock::now();
+  auto TT = [&](const char* w) { if (std::getenv("OPTCC_TIME")) fprintf(stderr, "  [col] %s %.3f ms\n", w, std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count() * 1e3); };
+  // Complete schedules: every rule of PLAN_SPEC 4 places the flows of segment b at steps b P + (something that does not
+  // depend on b), so the regions of one class have the SAME list up to offset and length.  Only the list of each
+  // class's first region is gathered from the table and finished; the others are copies with their own range.
+  bool fast = steps == in.n_steps;
+  for (size_t c = 0; c < ncls && fast; ++c)
+    for (uint32_t q = cls_begin[c]; q < cls_begin[c + 1]; ++q)
+      if (pl->region_flows[cls_regions[q]] != pl->region_flows[cls_regions[cls_begin[c]]]) { fast = false; break; }
+  if (fast) {
+    st->col_reg_begin.assign(nr + 1, 0);
+    for (size_t r = 0; r < nr; ++r) st->col_reg_begin[r + 1] = st->col_reg_begin[r] + pl->region_flows[r];
+    st->col_dflows.resize_uninit(nf);
+    // gather the representatives' lists (table order) straight into their place in col_dflows
+    std::vector<uint32_t> fill(nr, UINT32_MAX);            // next free position of a representative's list
+    uint64_t wanted = 0;
+    for (size_t c = 0; c < ncls; ++c)
+      if (cls_begin[c] < cls_begin[c + 1]) {
+        const uint32_t r = cls_regions[cls_begin[c]];
+        fill[r] = st->col_reg_begin[r];
+        wanted += pl->region_flows[r];
+      }
+    const uint32_t* reg = pl->flow_region.data();
+    for (uint32_t i = 0; i < nf && wanted; ++i) {          // (the first segment's flows sit in the first few bodies)
+      uint32_t& pos = fill[reg[i]];
+      if (pos == UINT32_MAX) continue;
+      const optcc_flow_t& f = pl->flows[i];
+      DFlow d;
+      d.off = f.off; d.len = f.len; d.src = f.src; d.dst = f.dst; d.op = f.op;
+      d.ksrc = d.kdin = d.kdout = 0; d.flags = 0; d.pad1 = 0;
+      st->col_dflows[pos++] = d;
+      --wanted;
+    }
+    TT("gather");
+    optcc_parallel_chunks(ncls, nf, [&](size_t c) {
+      if (cls_begin[c] == cls_begin[c + 1]) return;
+      ColScratch sc;
+      sc.init(in.p);
+      const uint32_t r0 = cls_regions[cls_begin[c]];
+      const uint32_t n = pl->region_flows[r0];
+      if (n == 0) { uncovered.fetch_add(cls_begin[c + 1] - cls_begin[c], std::memory_order_relaxed); return; }
+      DFlow* L0 = st->col_dflows.data() + st->col_reg_begin[r0];
+      const bool cov = finish_fresh(L0, n, o, sc);
+      if (!cov) uncovered.fetch_add(cls_begin[c + 1] - cls_begin[c], std::memory_order_relaxed);
+      for (uint32_t q = cls_begin[c] + 1; q < cls_begin[c + 1]; ++q) {
+        const uint32_t r = cls_regions[q];
+        DFlow* L = st->col_dflows.data() + st->col_reg_begin[r];
+        const uint64_t off = pl->region_offs[r], len = pl->region_len[r];
+        for (uint32_t j = 0; j < n; ++j) {
+          DFlow f = L0[j];
+          f.off = off;
+          f.len = len;
+          L[j] = f;
+        }
+      }
+    });
+  } else {
+    // ---- general path (truncated schedules): parallel stable counting sort of the table by region, then every list
+    // finished on its own, reusing the class's first list where it is the same ----
+    const size_t n_chunks = std::max<size_t>(1, std::min<size_t>(32, nf / 4096));
+    auto chunk_lo = [&](size_t c) { return uint32_t(uint64_t(nf) * c / n_chunks); };
+    std::vector<uint32_t> hist(n_chunks * nr, 0);
+    optcc_parallel_chunks(n_chunks, nf, [&](size_t c) {
+      uint32_t* h = hist.data() + c * nr;
+      const uint32_t* reg = pl->flow_region.data();
+      for (uint32_t i = chunk_lo(c); i < chunk_lo(c + 1); ++i) h[reg[i]]++;
+    });
+    st->col_reg_begin.assign(nr + 1, 0);
+    for (size_t r = 0; r < nr; ++r) {          // hist[c][r] becomes the first position of chunk c's flows of region r
+      uint32_t pos = st->col_reg_begin[r];
+      for (size_t c = 0; c < n_chunks; ++c) { const uint32_t h = hist[c * nr + r]; hist[c * nr + r] = pos; pos += h; }
+      st->col_reg_begin[r + 1] = pos;
+    }
+    st->col_dflows.resize_uninit(nf);
+    optcc_parallel_chunks(n_chunks, nf, [&](size_t c) {
+      uint32_t* pos = hist.data() + c * nr;
+      const uint32_t* reg = pl->flow_region.data();
+      for (uint32_t i = chunk_lo(c); i < chunk_lo(c + 1); ++i) {
+        const optcc_flow_t& f = pl->flows[i];
+        DFlow d;
+        d.off = f.off; d.len = f.len; d.src = f.src; d.dst = f.dst; d.op = f.op;
+        d.ksrc = d.kdin = d.kdout = 0; d.flags = 0; d.pad1 = 0;
+        st->col_dflows[pos[reg[i]]++] = d;
+      }
+    });
+    optcc_parallel_chunks(ncls, nf, [&](size_t c) {
+      ColScratch sc;
+      sc.init(in.p);
+      for (uint32_t q = cls_begin[c]; q < cls_begin[c + 1]; ++q) {
+        const uint32_t r = cls_regions[q];
+        const uint32_t fb = st->col_reg_begin[r], fe = st->col_reg_begin[r + 1];
+        if (fb == fe) { uncovered.fetch_add(1, std::memory_order_relaxed); continue; }   // no executed flow touches the region
+        if (!finish_region(st->col_dflows.data() + fb, fe - fb, o, sc)) uncovered.fetch_add(1, std::memory_order_relaxed);
+      }
+    });
+  }
+  TT("finish");
+  *all_covered = uncovered.load() == 0;
+  // ---- 3. one work item per (region, tile) ----
   st->col_items.clear();
   st->col_items.reserve(pl->tiles_per_rank);
   for (size_t r = 0; r < nr; ++r) {
     const uint64_t t0 = pl->region_tile0[r], t1 = r + 1 < nr ? pl->region_tile0[r + 1] : pl->tiles_per_rank;
     const uint32_t fb = st->col_reg_begin[r], fe = st->col_reg_begin[r + 1];
-    if (fb == fe) continue;   // no executed flow touches the region
-    for (uint32_t i = fb + 1; i < fe; ++i)
-      if (st->col_dflows[i].len != st->col_dflows[fb].len || st->col_dflows[i].off != st->col_dflows[fb].off) return false;
-    const uint64_t nunits = (st->col_dflows[fb].len + A - 1) / A;
+    if (fb == fe) continue;
+    const uint64_t nunits = (pl->region_len[r] + A - 1) / A;
     for (uint64_t t = 0; t < t1 - t0; ++t) {
       const uint64_t ubeg = t * TU, left = nunits > ubeg ? nunits - ubeg : 0;
       st->col_items.push_back(make_uint4(fb, fe, (unsigned int)t, (unsigned int)std::min<uint64_t>(left, TU)));
     }
-  }
-  return true;
-}
-
-// Bulk all-gather path of the column executor (data runs): per region list, find the reduce flows whose sum later copy
-// flows distribute (DFLOW_STAGE_OUT: the CTA keeps the tile in shared memory) and the copy flows whose source range holds
-// exactly the staged tile at that point (DFLOW_FROM_STAGE: one cp.async.bulk store).  Value numbering: a reduce gives its
-// destination a new value, a copy gives it the source's value.  One stage: a new sum is only staged when every copy of
-// the previous one has been issued.  A list in which a range written by a bulk store is touched again by any later flow
-// (never the case in an AllReduce plan: the all-gather's copies are final) keeps the LDG / STG path entirely.
-void assign_bulk_flags(optcc_exec_state* st, uint32_t p, bool bf16) {
-  std::vector<uint32_t> val(p), consumers;
-  std::vector<uint8_t> bulk_written(p);
-  const size_t nr = st->col_reg_begin.size() - 1;
-  for (size_t r = 0; r < nr; ++r) {
-    const uint32_t fb = st->col_reg_begin[r], fe = st->col_reg_begin[r + 1];
-    if (fb == fe) continue;
-    for (uint32_t i = 0; i < p; ++i) val[i] = i;
-    consumers.assign(size_t(p) + (fe - fb), 0);
-    uint32_t next_id = p;
-    for (uint32_t i = fb; i < fe; ++i) {           // how many copy flows read each value
-      const DFlow& f = st->col_dflows[i];
-      if (f.op == OPTCC_OP_REDUCE) val[f.dst] = next_id++;
-      else { consumers[val[f.src]]++; val[f.dst] = val[f.src]; }
-    }
-    for (uint32_t i = 0; i < p; ++i) val[i] = i;
-    std::fill(bulk_written.begin(), bulk_written.end(), 0);
-    next_id = p;
-    uint32_t staged = UINT32_MAX, pending = 0;
-    bool ok = true;
-    for (uint32_t i = fb; i < fe && ok; ++i) {
-      DFlow& f = st->col_dflows[i];
-      if (f.op == OPTCC_OP_REDUCE) {
-        if (bulk_written[f.src] || bulk_written[f.dst]) { ok = false; break; }
-        const uint32_t id = next_id++;
-        val[f.dst] = id;
-        if (consumers[id] && pending == 0 && (!bf16 || f.kdout == OPTCC_KIND_BUF)) {
-          f.flags |= DFLOW_STAGE_OUT;
-          staged = id;
-          pending = consumers[id];
-        }
-      } else {
-        if (val[f.src] == staged && (!bf16 || (f.ksrc == OPTCC_KIND_BUF && f.kdout == OPTCC_KIND_BUF))) {
-          if (bulk_written[f.dst]) { ok = false; break; }
-          f.flags |= DFLOW_FROM_STAGE;
-          bulk_written[f.dst] = 1;
-          --pending;
-        } else if (bulk_written[f.src] || bulk_written[f.dst]) {
-          ok = false;
-          break;
-        } else if (val[f.src] == staged) {
-          --pending;
-        }
-        val[f.dst] = val[f.src];
-      }
-    }
-    if (!ok) for (uint32_t i = fb; i < fe; ++i) st->col_dflows[i].flags &= ~(DFLOW_STAGE_OUT | DFLOW_FROM_STAGE);
   }
 }
 
@@ -1052,16 +1375,37 @@ int device_limits(int dev, DeviceLimits* out) {
   return OPTCC_OK;
 }
 
-int build_state(optcc_plan_t* pl) {
+// The column executor's tables need no device: built once per plan, on the host.
+int build_host_tables(optcc_plan_t* pl) {
   optcc_exec_state* st = pl->exec;
   if (!st) {
     st = new (std::nothrow) optcc_exec_state();
     if (!st) return OPTCC_ENOMEM;
     pl->exec = st;
   }
+  if (st->host_built) return OPTCC_OK;
+  st->column = pl->opts.exec_mode == OPTCC_EXEC_COLUMN && pl->tiles_per_rank < (uint64_t(1) << 32);
+  if (st->column) {
+    try {
+      bool covered = false;
+      build_column_state(pl, st, &covered);
+      st->lazy_masks = pl->info.lazy_verify && covered;
+    } catch (const std::bad_alloc&) {
+      return OPTCC_ENOMEM;
+    }
+  }
+  st->host_built = true;
+  return OPTCC_OK;
+}
+
+int build_state(optcc_plan_t* pl) {
+  int rc0 = build_host_tables(pl);
+  if (rc0 != OPTCC_OK) return rc0;
+  optcc_exec_state* st = pl->exec;
   int dev = 0;
   CU_TRY(cudaGetDevice(&dev));
-  if (st->device == dev && st->G != 0) return OPTCC_OK;
+  if (st->device == dev && st->built) return OPTCC_OK;
+  st->built = false;
   st->id = g_next_id.fetch_add(1);   // new tables: every workspace must be refreshed
   st->device = dev;
   DeviceLimits lim;
@@ -1076,25 +1420,22 @@ int build_state(optcc_plan_t* pl) {
   const optcc_plan_info_t& in = pl->info;
   const uint64_t A = in.unit_elems;
   try {
-    st->dflows.resize(in.n_flows);
-    for (size_t i = 0; i < in.n_flows; ++i) {
-      const optcc_flow_t& f = pl->flows[i];
-      DFlow d;
-      std::memset(&d, 0, sizeof d);
-      d.off = f.off; d.len = f.len; d.src = f.src; d.dst = f.dst; d.op = f.op;
-      if (!pl->kind_src.empty()) { d.ksrc = pl->kind_src[i]; d.kdin = pl->kind_dst_in[i]; d.kdout = pl->kind_dst_out[i]; }
-      st->dflows[i] = d;
-    }
-    // dataflow tables when that executor will run; otherwise the slice table of the barrier executors
+    st->built = false;
     st->df_ok = false;
-    if (pl->opts.exec_mode == OPTCC_EXEC_DATAFLOW && st->coop && st->G_df > 0) build_dataflow_tables(pl, st);
-    assign_mask_flags(pl, st);
-    st->column = pl->opts.exec_mode == OPTCC_EXEC_COLUMN && pl->tiles_per_rank < (uint64_t(1) << 32);
-    if (st->column) {
-      assign_dead_source_flags(pl, st);
-      assign_raw_flags(pl, st);
-      if (!build_column_tables(pl, st)) { st->G = 0; return OPTCC_EINVAL; }   // (G = 0: the state is rebuilt on the next call)
-      if (pl->opts.copy_path != 1) assign_bulk_flags(st, in.p, in.dtype == OPTCC_BF16);
+    if (!st->column) {   // (column executor: region-major tables only, built by build_host_tables)
+      if (in.dtype == OPTCC_BF16 && pl->kind_src.empty()) optcc_assign_kinds(pl);
+      st->dflows.resize(in.n_flows);
+      for (size_t i = 0; i < in.n_flows; ++i) {
+        const optcc_flow_t& f = pl->flows[i];
+        DFlow d;
+        std::memset(&d, 0, sizeof d);
+        d.off = f.off; d.len = f.len; d.src = f.src; d.dst = f.dst; d.op = f.op;
+        if (!pl->kind_src.empty()) { d.ksrc = pl->kind_src[i]; d.kdin = pl->kind_dst_in[i]; d.kdout = pl->kind_dst_out[i]; }
+        st->dflows[i] = d;
+      }
+      // dataflow tables when that executor will run; otherwise the slice table of the barrier executors
+      if (pl->opts.exec_mode == OPTCC_EXEC_DATAFLOW && st->coop && st->G_df > 0) build_dataflow_tables(pl, st);
+      assign_mask_flags(pl, st);
     }
     // slice table: cut every step into G slices of equal HBM bytes
     st->slices.clear();
@@ -1122,6 +1463,7 @@ int build_state(optcc_plan_t* pl) {
   } catch (const std::bad_alloc&) {
     return OPTCC_ENOMEM;
   }
+  st->built = true;
   return OPTCC_OK;
 }
 
@@ -1174,9 +1516,17 @@ int launch_plan(optcc_plan_t* pl, ExecParams& P, cudaStream_t stream) {
     CU_TRY(cudaMemsetAsync(&P.ctrl->ticket, 0, sizeof(unsigned long long), stream));
     const uint32_t G = pl->opts.grid_ctas ? pl->opts.grid_ctas : uint32_t(st->sm_count) * CTAS_PER_SM;
     const unsigned int grid = (unsigned int)std::min<uint64_t>(G, P.col_n_items);
-    const size_t dyn = (!is_mask_mode(MODE) && P.col_bulk) ? size_t(pl->tile_units) * 16 : 0;   // the stage: one tile
-    if (dyn > 40 * 1024) CU_TRY(cudaFuncSetAttribute(optcc_column_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
-    optcc_column_kernel<MODE><<<grid, COL_THREADS, dyn, stream>>>(P);
+    if (P.col_warp) {
+      // warp-wide tiles: one stage per warp; a CTA's 14 warps claim items on their own
+      const size_t dyn = (!is_mask_mode(MODE) && P.col_bulk) ? size_t(pl->tile_units) * 16 * (COL_THREADS / 32) : 0;
+      if (dyn > 40 * 1024) CU_TRY(cudaFuncSetAttribute(optcc_wcolumn_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+      const unsigned int wgrid = (unsigned int)std::min<uint64_t>(G, (P.col_n_items + COL_THREADS / 32 - 1) / (COL_THREADS / 32));
+      optcc_wcolumn_kernel<MODE><<<wgrid, COL_THREADS, dyn, stream>>>(P);
+    } else {
+      const size_t dyn = (!is_mask_mode(MODE) && P.col_bulk) ? size_t(pl->tile_units) * 16 : 0;   // the stage: one tile
+      if (dyn > 40 * 1024) CU_TRY(cudaFuncSetAttribute(optcc_column_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+      optcc_column_kernel<MODE><<<grid, COL_THREADS, dyn, stream>>>(P);
+    }
     CU_TRY(cudaGetLastError());
   } else if (dataflow) {
     P.n_ops = st->step_op_begin[n_steps];
@@ -1232,9 +1582,11 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   P.df_slots = (pl->exec && pl->exec->big_ops && !P.bulk_copy) ? 2 : 4;
   if (pl->opts.exec_mode == OPTCC_EXEC_COLUMN) P.l2_hints = 0;   // see optcc_column_kernel
   P.col_pf_dist = 1; P.col_pf_l2 = 0; P.col_pf_next = 0; P.col_bulk = 1;
+  P.col_bulk_policy = 1;   // bulk stores evict_first: the all-gather's results are never read again (measured: C2 1.68 -> 1.62 ms)
+  P.col_warp = pl->tile_units <= 256 ? 1u : 0u;
   if (const char* t = std::getenv("OPTCC_TUNE")) {   // TEMPORARY (experiments): "dist,l2,next,bulk,bulkpolicy"
-    unsigned a = 1, b = 0, c = 0, d = 1, e = 0;
-    if (std::sscanf(t, "%u,%u,%u,%u,%u", &a, &b, &c, &d, &e) >= 1) { P.col_pf_dist = a; P.col_pf_l2 = b; P.col_pf_next = c; P.col_bulk = d; P.pad0 = e; }
+    unsigned a = 1, b = 0, c = 0, d = 1, e = 1, f = 0;
+    if (std::sscanf(t, "%u,%u,%u,%u,%u,%u", &a, &b, &c, &d, &e, &f) >= 1) { P.col_pf_dist = a; P.col_pf_l2 = b; P.col_pf_next = c; P.col_bulk = d; P.col_bulk_policy = e; P.col_warp = f; }
   }
   if (pl->opts.copy_path == 1) P.col_bulk = 0;
 }
@@ -1242,6 +1594,21 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
 }  // namespace
 
 extern "C" int optcc_last_cuda_error(void) { return g_last_cuda_error; }
+
+extern "C" int optcc_column_tables(optcc_plan_t* plan, const void** records, uint32_t* n_records, const void** items,
+                                   uint32_t* n_items) {
+  if (!plan) return OPTCC_EINVAL;
+  if (plan->opts.exec_mode != OPTCC_EXEC_COLUMN) return OPTCC_EUNSUPPORTED;
+  int rc = build_host_tables(plan);
+  if (rc != OPTCC_OK) return rc;
+  const optcc_exec_state* st = plan->exec;
+  if (!st->column) return OPTCC_EUNSUPPORTED;
+  if (records) *records = st->col_dflows.data();
+  if (n_records) *n_records = (uint32_t)st->col_dflows.size();
+  if (items) *items = st->col_items.data();
+  if (n_items) *n_items = (uint32_t)st->col_items.size();
+  return OPTCC_OK;
+}
 
 namespace {
 int prepare_impl(optcc_plan_t* plan, void* workspace, void* stream, bool force) {
@@ -1396,6 +1763,7 @@ extern "C" int optcc_verify(optcc_plan_t* plan, void* workspace, void* stream_, 
                                                           std::max<uint64_t>(1, uint64_t(plan->exec->sm_count) * 16 / in.p)));
   const dim3 blocks(bx, in.p);
   const bool lazy = plan->exec->lazy_masks;
+  P.mask_lazy = lazy ? 1u : 0u;
   if (lazy) {
     // initial masks are constants and the last writer of every range checks the final mask (assign_mask_flags); the
     // bulk-copy path would move raw memory, so the streaming warps take the copies too

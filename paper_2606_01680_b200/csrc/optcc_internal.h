@@ -3,6 +3,7 @@
 #ifndef OPTCC_INTERNAL_H_
 #define OPTCC_INTERNAL_H_
 
+#include <algorithm>
 #include <cstddef>
 #include <cstdint>
 #include <new>
@@ -74,6 +75,8 @@ struct optcc_plan {
   std::vector<uint64_t> region_offs;    // sorted unique flow offsets (regions tile [0, n), PLAN_SPEC 5.4)
   std::vector<uint64_t> region_len;     // elements of every region
   std::vector<uint32_t> region_flows;   // flows over every region
+  std::vector<uint32_t> region_class;   // part * sections + section (P2P pieces: one more class): regions of one class
+                                        // differ only in the segment, so their flow lists are the same up to the offset
   std::vector<uint64_t> region_tile0;   // first tile counter of every region (prefix sum)
   optcc_rawvec<uint32_t> flow_region;   // [n_flows] index into region_offs of the region a flow covers
   optcc_exec_state* exec;               // created lazily by the executor; freed by optcc_plan_destroy
@@ -81,6 +84,26 @@ struct optcc_plan {
 
 // implemented in optcc_exec.cu
 void optcc_exec_state_free(optcc_exec_state*);
+// implemented in optcc_plan.cpp: storage kinds of a bf16 plan in table order (executors that walk the table step by step)
+void optcc_assign_kinds(struct optcc_plan*);
+
+// Run body(chunk) for chunk in [0, n) on a few host threads when there is enough work to pay for them; the chunks
+// must be independent.
+#include <atomic>
+#include <thread>
+template <class F>
+inline void optcc_parallel_chunks(size_t n, size_t work, F body) {
+  unsigned hw = std::thread::hardware_concurrency();
+  unsigned nt = work < (size_t(1) << 16) ? 1u : std::min(8u, hw ? hw : 1u);
+  if (nt <= 1 || n <= 1) { for (size_t i = 0; i < n; ++i) body(i); return; }
+  std::atomic<size_t> next{0};
+  auto worker = [&]() { for (size_t i; (i = next.fetch_add(1, std::memory_order_relaxed)) < n;) body(i); };
+  std::vector<std::thread> th;
+  th.reserve(nt - 1);
+  for (unsigned t = 1; t < nt; ++t) th.emplace_back(worker);
+  worker();
+  for (auto& t : th) t.join();
+}
 
 // ---- device workspace layout (bytes from the workspace base; every region 256-byte aligned) -----------------
 //   control block | rank pointers | device flow records | per-(step, CTA) slice table | dataflow deps, tile-ops | column items | dataflow counters | fp32 shadow (bf16 plans) | masks (verify)

@@ -41,17 +41,15 @@ struct __align__(16) DFlow {      // 32 bytes: what the device needs of an optcc
 static_assert(sizeof(DFlow) == 32, "DFlow must be 32 bytes");
 enum : unsigned int {
   DFLOW_DEAD_SRC = 1u,   // the source range is dead after this flow has read it (see discard_line16)
-  // contributor-mask runs only (lazy verifier, see range_mask_lazy); never set for truncated or eager runs:
-  DFLOW_SRC_INIT = 2u,   // no earlier flow wrote the source range: it holds the initial mask {src}
-  DFLOW_DST_INIT = 4u,   // no earlier flow wrote the destination range: it holds the initial mask {dst}
-  DFLOW_FINAL = 8u,      // no later flow writes the destination range: what this flow writes is the final mask
-  // all runs (column executor: what to prefetch ahead of time):
-  DFLOW_SRC_RAW = 16u,   // no earlier executed flow wrote the source range: reading it is its first touch (a DRAM access)
-  DFLOW_DST_RAW = 32u,   // the same for the destination range (a reduce flow reads it)
+  // first touches and last writes.  Data runs of the column executor request first touches (DRAM accesses) ahead of
+  // time; contributor-mask runs in the lazy form (ExecParams.mask_lazy, see range_mask_lazy) take the constant
+  // initial mask instead of loading it and let the last writer check the final mask:
+  DFLOW_SRC_INIT = 2u,   // no earlier executed flow wrote the source range: it holds rank src's input / the mask {src}
+  DFLOW_DST_INIT = 4u,   // no earlier executed flow wrote the destination range (a reduce flow reads it)
+  DFLOW_FINAL = 8u,      // no later flow writes the destination range: what this flow writes is the final value / mask
   // column executor, data runs, bulk all-gather path (see build_column_tables / optcc_column_kernel):
   DFLOW_STAGE_OUT = 64u,   // reduce flow: the sum it stores is the source of later copy flows -- also keep it in the CTA's stage
   DFLOW_FROM_STAGE = 128u, // copy flow: the source range holds exactly the staged tile -- store it with cp.async.bulk
-  DFLOW_DRAIN = 256u,      // the flow touches a range an earlier bulk store of this list wrote: wait for the bulk stores first
 };
 
 struct __align__(16) Slice {      // start of a CTA's slice of a step: flow index and 16-byte unit inside it
@@ -111,7 +109,11 @@ struct ExecParams {
   unsigned int col_pf_dist;       // column executor: raw operands are requested this many flows ahead (>= 1)
   unsigned int col_pf_l2;         // 1: requested into L2 (prefetch.global.L2), 0: into L1
   unsigned int col_pf_next;       // 1: the look-ahead continues into the CTA's next work item (claimed one item ahead)
-  unsigned int col_bulk;          // 1: data runs act on DFLOW_STAGE_OUT / FROM_STAGE / DRAIN (bulk all-gather path)
+  unsigned int col_bulk;          // 1: data runs act on DFLOW_STAGE_OUT / FROM_STAGE (bulk all-gather path)
+  unsigned int mask_lazy;         // contributor-mask runs: 1 = lazy form (initial masks are constants, last writers check)
+  unsigned int col_bulk_policy;   // L2 policy of the bulk stores (0 normal, 1 evict_first, 2 evict_last)
+  unsigned int col_warp;          // 1: warp-wide tiles (optcc_wcolumn_kernel), 0: CTA-wide tiles (optcc_column_kernel)
+  unsigned int pad3;
 };
 
 // ---- memory access helpers: L2-only loads (data written by other SMs in the previous step), streaming stores ----
@@ -190,8 +192,12 @@ __device__ __forceinline__ void grid_barrier(unsigned long long* ctr, unsigned l
 }
 
 // =====================================================================================================
-// Range operations.  All ranges are given in 16-byte vectors [vbeg, vend) relative to the flow's start.
+// Range operations.  All ranges are given in 16-byte vectors [vbeg, vend) relative to the flow's start.  NT threads
+// work on a range together: a whole CTA (thread index = threadIdx.x) or, with NT = 32, one warp on its own
+// (thread index = lane) -- the column executor's warps run independent work items.
 // =====================================================================================================
+template <int NT>
+__device__ __forceinline__ unsigned int group_tid() { return NT == 32 ? (threadIdx.x & 31u) : threadIdx.x; }
 
 // Dead-source discard.  When the planner knows that the next access to a flow's source range is a plain overwrite (the
 // all-gather copy of the final sum), the data is dead once this flow has read it; dropping its lines from L2
@@ -224,7 +230,7 @@ __device__ __forceinline__ void remainder_dispatch(unsigned int rem, F&& f) {
 template <int UNROLL, int NT, class PolX>
 __device__ __forceinline__ void range_copy16(const char* __restrict__ s, char* __restrict__ d,
                                              unsigned long long vbeg, unsigned long long vend, const PolX& pol) {
-  unsigned long long v = vbeg + threadIdx.x;
+  unsigned long long v = vbeg + group_tid<NT>();
   for (; v + (UNROLL - 1) * (unsigned long long)NT < vend; v += UNROLL * (unsigned long long)NT) {
     uint4 x[UNROLL];
 #pragma unroll
@@ -252,7 +258,7 @@ template <int UNROLL, int NT, bool STAGE, class PolX>
 __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* __restrict__ d,
                                               unsigned long long vbeg, unsigned long long vend, const PolX& pol, bool dead_src,
                                               char* stage) {
-  unsigned long long v = vbeg + threadIdx.x;
+  unsigned long long v = vbeg + group_tid<NT>();
   for (; v + (UNROLL - 1) * (unsigned long long)NT < vend; v += UNROLL * (unsigned long long)NT) {
     uint4 a[UNROLL], b[UNROLL];
 #pragma unroll
@@ -298,7 +304,7 @@ template <int UNROLL, int EB, int NT, class PolX>
 __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* __restrict__ d,
                                               unsigned long long vbeg, unsigned long long vend,
                                               unsigned int& overlaps, const PolX& pol, bool dead_src) {
-  unsigned long long v = vbeg + threadIdx.x;
+  unsigned long long v = vbeg + group_tid<NT>();
   auto join = [&](uint4 a, uint4 b) {
     const unsigned int cx = a.x & b.x, cy = a.y & b.y, cz = a.z & b.z, cw = a.w & b.w;   // elements whose sets overlap
     if (EB == 2) {
@@ -427,7 +433,7 @@ __device__ __forceinline__ void range_mask_lazy_t(const char* __restrict__ s, ch
       }
     }
   };
-  unsigned long long v = vbeg + threadIdx.x;
+  unsigned long long v = vbeg + group_tid<NT>();
   for (; v + (UNROLL - 1) * (unsigned long long)NT < vend; v += UNROLL * (unsigned long long)NT) {
     batch(v, std::integral_constant<int, UNROLL>());
     // (only when every lane of the warp is in this round: the line's other vectors were loaded by this instruction)
@@ -506,7 +512,7 @@ __device__ __forceinline__ void range_add_bf16(const char* __restrict__ s, const
                                                char* __restrict__ dout, unsigned long long ubeg,
                                                unsigned long long uend, const PolX& pol, bool dead_src, char* stage) {
   constexpr int UNROLL = 2;
-  unsigned long long u = ubeg + threadIdx.x;
+  unsigned long long u = ubeg + group_tid<NT>();
   for (; u + (UNROLL - 1) * (unsigned long long)NT < uend; u += UNROLL * (unsigned long long)NT) {
     float a[UNROLL][8], b[UNROLL][8];
 #pragma unroll

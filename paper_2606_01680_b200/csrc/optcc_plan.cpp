@@ -64,22 +64,6 @@ namespace {
 // x mod H for -H <= x < 2H (all the rules need: ring positions shifted by at most one lap)
 inline uint32_t modH(int64_t x, int64_t H) { return (uint32_t)(x < 0 ? x + H : (x >= H ? x - H : x)); }
 
-// Run body(chunk) for chunk in [0, n) on a few host threads when the table is large enough to pay for them; the
-// chunks are independent (each counts or fills a disjoint range of steps).
-template <class F>
-void parallel_chunks(size_t n, size_t work, F body) {
-  unsigned hw = std::thread::hardware_concurrency();
-  unsigned nt = work < (size_t(1) << 16) ? 1u : std::min(8u, hw ? hw : 1u);
-  if (nt <= 1 || n <= 1) { for (size_t i = 0; i < n; ++i) body(i); return; }
-  std::atomic<size_t> next{0};
-  auto worker = [&]() { for (size_t i; (i = next.fetch_add(1, std::memory_order_relaxed)) < n;) body(i); };
-  std::vector<std::thread> th;
-  th.reserve(nt - 1);
-  for (unsigned t = 1; t < nt; ++t) th.emplace_back(worker);
-  worker();
-  for (auto& t : th) t.join();
-}
-
 // Everything the closed-form rules of PLAN_SPEC 4 need, fixed before the first flow is written.  The table is never
 // sorted: emit_step() lists the flows of one step directly in PLAN_SPEC 3 order (link, stage, src, dst, off), so the
 // steps can be counted and filled independently ("closed-form rules ... O(pk)").
@@ -270,7 +254,9 @@ void emit_step(const Geom& G, uint32_t t, Sink& out) {
 // Storage kinds for bf16 plans: walk the table once with the number of contributors every
 // (rank, region) holds.  A region holding 1 or all p contributors lives in the rank buffer (bf16); a partial
 // sum (1 < count < p) lives in the fp32 shadow.  All flows of one step read the state before the step.
-void assign_kinds(optcc_plan_t* pl) {
+}  // namespace
+
+void optcc_assign_kinds(optcc_plan_t* pl) {
   const uint32_t p = pl->info.p;
   const size_t nf = pl->flows.size();
   if (pl->info.dtype != OPTCC_BF16) return;      // f32 plans: the three arrays stay empty (everything is OPTCC_KIND_BUF)
@@ -298,8 +284,6 @@ void assign_kinds(optcc_plan_t* pl) {
     }
   }
 }
-
-}  // namespace
 
 extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dtype, const optcc_opts_t* opts,
                              optcc_plan_t** out) {
@@ -337,7 +321,9 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
   std::memset(&pl->info, 0, sizeof pl->info);
   std::memset(&pl->opts, 0, sizeof pl->opts);
   if (opts) pl->opts = *opts;
-  else pl->opts.exec_mode = OPTCC_EXEC_DATAFLOW;   // the default executor
+  if (pl->opts.exec_mode > OPTCC_EXEC_COLUMN) { delete pl; return OPTCC_EINVAL; }
+  const bool exec_auto = pl->opts.exec_mode == OPTCC_EXEC_AUTO;
+  if (exec_auto) pl->opts.exec_mode = OPTCC_EXEC_COLUMN;   // (tile geometry is the column executor's; see the check below)
   pl->ell.assign(ell, ell + p);
   pl->stragglers = stragglers;
   pl->healthy = healthy;
@@ -406,17 +392,19 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     // ---- regions = the sections and P2P pieces themselves: consecutive exported boundaries (ascending, contiguous,
     // covering [0, n): PLAN_SPEC 5.4).  A flow carries its (part, segment, section), i.e. its region, from birth, so
     // offset and length are the region's by construction.
-    auto add_regions = [&](const std::vector<uint64_t>& bounds, std::vector<uint32_t>& reg_of) {
+    auto add_regions = [&](const std::vector<uint64_t>& bounds, std::vector<uint32_t>& reg_of, bool sections) {
       reg_of.assign(bounds.empty() ? 0 : bounds.size() - 1, UINT32_MAX);
       for (size_t i = 0; i + 1 < bounds.size(); ++i) {
         if (bounds[i + 1] <= bounds[i]) continue;
         reg_of[i] = (uint32_t)pl->region_offs.size();
         pl->region_offs.push_back(bounds[i]);
         pl->region_len.push_back(bounds[i + 1] - bounds[i]);
+        // interval i of sec_bounds is (part, segment, section) = (i / (k nsec), (i / nsec) mod k, i mod nsec)
+        pl->region_class.push_back(sections ? uint32_t(i / (size_t(k) * nsec)) * nsec + uint32_t(i % nsec) : nparts * nsec);
       }
     };
-    add_regions(pl->sec_bounds, G.sec_reg);
-    add_regions(pl->p2p_bounds, G.p2p_reg);
+    add_regions(pl->sec_bounds, G.sec_reg, true);
+    add_regions(pl->p2p_bounds, G.p2p_reg, false);
     {   // the regions tile [0, n) exactly (both executors and the lazy verifier rely on it)
       uint64_t pos = 0;
       for (size_t r = 0; r < pl->region_offs.size(); ++r) {
@@ -454,7 +442,7 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     bool any_empty = false;
     for (uint32_t r : G.sec_reg) any_empty |= r == UINT32_MAX;
     for (uint32_t r : G.p2p_reg) any_empty |= r == UINT32_MAX;
-    parallel_chunks(n_chunks, est, [&](size_t c) {
+    optcc_parallel_chunks(n_chunks, est, [&](size_t c) {
       for (uint32_t t = chunk_lo(c); t < chunk_lo(c + 1); ++t) {
         if (any_empty) {
           CountSink cs;
@@ -482,7 +470,7 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     std::vector<uint64_t> red(n_chunks, 0), cop(n_chunks, 0);
     const size_t nreg = pl->region_offs.size();
     std::vector<uint32_t> hist(n_chunks * nreg, 0);      // flows per (chunk, region)
-    parallel_chunks(n_chunks, est, [&](size_t c) {
+    optcc_parallel_chunks(n_chunks, est, [&](size_t c) {
       FillSink fs;
       fs.G = &G;
       fs.region_count = hist.data() + c * nreg;
@@ -521,6 +509,14 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     const size_t nr = pl->region_offs.size();
     uint64_t flow_units = 0;
     for (size_t r = 0; r < nr; ++r) flow_units += uint64_t(pl->region_flows[r]) * ((pl->region_len[r] + A - 1) / A);
+    // AUTO: the column executor whenever its work items (one per region and tile) can be indexed with 32 bits -- units
+    // / 1792 + regions, i.e. always for plans whose flow table fits 32-bit indices unless the caller forces tiny tiles;
+    // otherwise the dataflow executor with its own tile size.  (Measured on a B200: with chain-ordered
+    // lists the column executor is the faster one on every shape of BASELINE.json's configs.)
+    if (exec_auto) {
+      const uint64_t tu = pl->opts.tile_units ? pl->opts.tile_units : 1792;
+      if (U / tu + nr >= (uint64_t(1) << 32)) pl->opts.exec_mode = OPTCC_EXEC_DATAFLOW;
+    }
     if (pl->opts.tile_units) {
       pl->tile_units = pl->opts.tile_units;
     } else if (pl->opts.exec_mode == OPTCC_EXEC_COLUMN) {
@@ -557,12 +553,6 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     delete pl;
     return OPTCC_ENOMEM;
   }
-  try {
-    assign_kinds(pl);      // (needs flow_region)
-  } catch (const std::bad_alloc&) {
-    delete pl;
-    return OPTCC_ENOMEM;
-  }
   // lazy verifier (optcc.h, lazy_verify): every (rank, region) is written by a flow of the executed steps.  A complete
   // schedule writes every range (each rank receives every section's sum by a reduce or a copy: PLAN_SPEC 5.2); the
   // executor's table build checks it region by region and falls back to the eager form otherwise.  Truncated schedules
@@ -590,6 +580,7 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     delete pl;
     return OPTCC_ENOMEM;
   }
+  in.exec_mode = pl->opts.exec_mode;
   optcc_ws_layout L = optcc_layout(pl);
   in.workspace_bytes = L.end_exec;
   in.verify_workspace_bytes = L.end_verify;

@@ -17,10 +17,10 @@ pytestmark = pytest.mark.gpu
 BENCH_K = {0: 8, 1: 16, 2: 8, 3: 8, 4: 8}    # bench.py's k per config
 
 
-def _check_full(w, k, exec_mode, n_samples=2048):
+def _check_full(w, k, exec_mode, n_samples=2048, tile_units=0):
     import torch
     from paper_2606_01680_b200.device import Session
-    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=k, exec_mode=exec_mode)
+    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=k, exec_mode=exec_mode, tile_units=tile_units)
     oplan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=k)
     fl, sb, _, _ = B.optcc_plan_tables(plan)
     assert fl.tobytes() == oplan.flows.tobytes() and np.array_equal(sb, oplan.step_begin)
@@ -90,11 +90,13 @@ def test_c2_full_sampled():
     assert c["T_over_T0"] < 1.06           # within the paper's reported gap
 
 
-@pytest.mark.parametrize("ci,k", [(1, 16), (2, 8), (3, 8), (4, 8), (1, 32)])
-def test_full_sampled_column_executor(ci, k):
-    """the column executor (one CTA runs a region's whole flow list on a tile, no inter-CTA synchronisation) at the
-    full sizes in its bench configuration: sampled elements against the oracle, every element against the per-step executor"""
-    _check_full(W.config(ci), k, B.OPTCC_EXEC_COLUMN, n_samples=1024)
+@pytest.mark.parametrize("tile_units", [0, 128, 1792])
+@pytest.mark.parametrize("ci,k", [(1, 16), (2, 8), (3, 8), (4, 8), (1, 32), (2, 20), (3, 32)])
+def test_full_sampled_column_executor(ci, k, tile_units):
+    """the column executor (a tile is taken through its region's whole flow list, no synchronisation between CTAs) at
+    the full sizes, with the library's tile size, warp-wide tiles (128 units) and CTA-wide tiles (1792 units): sampled
+    elements against the oracle, every element against the per-step executor"""
+    _check_full(W.config(ci), k, B.OPTCC_EXEC_COLUMN, n_samples=1024, tile_units=tile_units)
 
 
 def test_c2_full_sampled_persistent_mode():

@@ -104,7 +104,7 @@ def test_random_plans_any_executor_any_verifier(seed):
         seed = 500 + int(seed.split("-")[1])
     rng = np.random.default_rng(31337 + seed)
     p, g, ell, n, k, dtype, tile, grid, ordering = _random_case(rng)
-    mode = int(rng.integers(0, 3))
+    mode = int(rng.integers(1, 4))      # persistent, per-step or dataflow
     if column:
         mode = B.OPTCC_EXEC_COLUMN
     eager = int(rng.integers(0, 2))

@@ -34,7 +34,7 @@ def test_library_exports_every_declared_symbol():
     lib = B.load()
     for name in declared:
         assert hasattr(lib, name), name
-    assert lib.optcc_abi_version() == 1
+    assert lib.optcc_abi_version() == 2
     assert B.FLOW_DTYPE.itemsize == 40
 
 
