@@ -42,10 +42,11 @@ def parse_args():
     ap.add_argument("--ell", type=float, default=1.6, help="ell for config 4 (the C5 sweep)")
     ap.add_argument("--k", type=int, default=-1,
                     help="segments (PAPER.md:124); -1 = bench default per config (16 for C2, see profiles/ k-sweep), 0 = planner's auto rule")
-    ap.add_argument("--exec-mode", type=int, default=-1,
-                    help="-1 = bench default per config (BENCH_EXEC: the faster of the column and the dataflow executor, "
-                         "profiles/ executor table), 3 column kernel, 2 dataflow kernel, 0 persistent kernel with grid barriers, "
-                         "1 one launch per step")
+    ap.add_argument("--exec-mode", type=int, default=0,
+                    help="OPTCC_EXEC_*: 0 = auto (the library chooses from the plan's shape; what a user of optcc_plan gets), "
+                         "1 persistent kernel with grid barriers, 2 one launch per step, 3 dataflow kernel, 4 column kernel")
+    ap.add_argument("--tile-units", type=int, default=0, help="opts.tile_units (0 = the library's choice)")
+    ap.add_argument("--col-order", type=int, default=0, help="opts.col_order (column executor: 0 chain by chain, 1 table order)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--e2e-shards", type=int, default=16,
                     help="element shards of the end-to-end leg (optcc_execute_host_sharded: H2D, execute and D2H of "
@@ -54,19 +55,13 @@ def parse_args():
                     help="log2 of n per rank for the CPU-oracle sample (0 = 24 for the cpu_baseline leg, 22 per --impl reference step)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    a = ap.parse_args()
-    if a.exec_mode < 0:
-        a.exec_mode = BENCH_EXEC[a.config]
-    return a
+    return ap.parse_args()
 
 
 BENCH_K = {0: 8, 1: 16, 2: 8, 3: 8, 4: 8}   # per config; k is free in BASELINE.json's configs
 
 
-# executor per config: the column executor (no synchronisation between CTAs) where it is faster, the dataflow
-# executor for C4 (regions of ~1 k units: one small tile per region, 960 work items)
-BENCH_EXEC = {0: 3, 1: 3, 2: 3, 3: 2, 4: 3}
-EXEC_KERNEL = {0: "optcc_exec_kernel", 1: "optcc_exec_kernel", 2: "optcc_dataflow_kernel", 3: "optcc_column_kernel"}
+EXEC_KERNEL = {1: "optcc_exec_kernel", 2: "optcc_exec_kernel", 3: "optcc_dataflow_kernel", 4: "optcc_column_kernel"}
 
 
 def bench_k(args):
@@ -242,7 +237,8 @@ def run_native(args):
 
     w = rep.shard(W.config(args.config, args.ell) if args.config == 4 else W.config(args.config))
     esize = w.elem_bytes
-    mk = lambda: B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=bench_k(args), exec_mode=args.exec_mode)
+    mk = lambda: B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=bench_k(args), exec_mode=args.exec_mode,
+                              tile_units=args.tile_units, col_order=args.col_order)
     plan0 = mk()
     k = plan0.info["k"]
     cost0 = B.optcc_cost(plan0)
@@ -257,7 +253,8 @@ def run_native(args):
     stream = torch.cuda.current_stream(dev)
     ev = lambda: torch.cuda.Event(enable_timing=True)
     # execute + verify; the lazy verifier (plan_info.lazy_verify) needs no init / check kernels around the mask run
-    launches_per_step = (plan0.info["n_steps"] if args.exec_mode == 1 else 1) * 2 + (0 if plan0.info["lazy_verify"] else 2)
+    exec_mode = plan0.info["exec_mode"]          # what OPTCC_EXEC_AUTO resolved to
+    launches_per_step = (plan0.info["n_steps"] if exec_mode == 2 else 1) * 2 + (0 if plan0.info["lazy_verify"] else 2)
 
     def full_step(timed):
         """a1-a3 optcc_plan, a5-a7 optcc_execute (a4 optcc_cost on the host meanwhile), a8 optcc_verify; returns event
@@ -381,7 +378,7 @@ def run_native(args):
         return 0
 
     peak, peak_src = measured_peak()
-    kname = EXEC_KERNEL[args.exec_mode]
+    kname = EXEC_KERNEL[exec_mode]
     kern = kname + ("<MODE_F32>" if w.dtype == W.F32 else "<MODE_BF16>")
     achieved = sched_bytes / t_exec / 1e6
     traffic = ncu_traffic(w.name.split("[")[0], kern)
@@ -392,10 +389,11 @@ def run_native(args):
         "scaling": "weak", "vs_baseline": None, "dtype": "f32" if w.dtype == W.F32 else "bf16(f32 accumulate)",
         "data": "synthetic",
         "config": {"workload": workload_name(w, k), "step": "optcc_plan + optcc_cost + optcc_execute + optcc_verify (SURVEY 8(a) a1-a8)",
-                   "exec_mode": {0: "persistent cooperative kernel, grid barrier per step", 1: "one launch per step",
-                                 2: "dataflow cooperative kernel: tile-ops in table order, per-range completion counters, no grid barrier",
-                                 3: "column kernel: a CTA runs a region's whole flow list on one tile in table order, no synchronisation "
-                                    "between CTAs (every dependency lies inside one element column)"}[args.exec_mode],
+                   "exec_mode": ("auto -> " if args.exec_mode == 0 else "") +
+                                {1: "persistent cooperative kernel, grid barrier per step", 2: "one launch per step",
+                                 3: "dataflow cooperative kernel: tile-ops in table order, per-range completion counters, no grid barrier",
+                                 4: "column kernel: a tile is taken through its region's whole flow list in dependency order, no "
+                                    "synchronisation between CTAs (every dependency lies inside one element column)"}[exec_mode],
                    "plan_steps": plan0.info["n_steps"], "plan_flows": plan0.info["n_flows"], "parallelism": f"replicas x{world} (element-axis shards, no collective)",
                    "l2": "inputs larger than L2 (footprint %.2f GB) and restored from a pristine copy between steps, untimed" % (w.p * w.n * esize / 1e9)},
         "execute_only": {"algbw": world * w.n * esize / t_exec / 1e6, "unit": UNIT, "ms": t_exec,

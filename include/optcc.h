@@ -102,7 +102,8 @@ typedef struct optcc_opts {
                          column executor: units per work item; 0 = auto (1792 for f32, 896 for bf16, at most the longest region) */
   uint32_t schedule;  /* OPTCC_SCHED_*: 0 = OPTCC (default), 1 = plain ring on the degraded topology (baseline) */
   uint32_t ordering;  /* stage ordering of PAPER.md:138 for one straggler, g = 1: 0 or 2 = ordering (2) S3->S1->S4->S2 (the
-                         canonical plan, k+1 bodies), 1 = ordering (1) S1->S2->S3->S4 (PLAN_SPEC C1', k+3 bodies) */
+                         canonical plan, k+1 bodies), 1 = ordering (1) S1->S2->S3->S4 (PLAN_SPEC C1', k+3 bodies), 3 = the
+                         four-pattern mix of PAPER.md:144-155 (A, C ordering (1); B, D ordering (2); PLAN_SPEC C1'', k+1 bodies) */
   uint32_t no_discard;/* 1 = keep dead source lines in L2 (disables the discard.global.L2 optimisation; for bisecting) */
   uint32_t verify_eager; /* 1 = optcc_verify initialises the mask arrays and checks them with separate passes even when
                             the plan allows the lazy form (initial masks as constants, final masks checked by their last

@@ -121,10 +121,10 @@ def build_plan(p, g, ell, n, dtype, k=0, _u_p2p_override=None, schedule=OPTCC, o
         if p >= 3 and g >= 1 and p % g == 0:
             raise PlanError("EUNSUPPORTED", "the ring baseline is defined for g = 1")
     q, stragglers, healthy = classify(p, g, ell)
-    if ordering not in (1, 2):
-        raise PlanError("EINVAL", "ordering is 1 or 2 (:138)")
-    if ordering == 1 and not (g == 1 and len(stragglers) == 1 and schedule == OPTCC):
-        raise PlanError("EUNSUPPORTED", "ordering (1) is constructed for one straggler, g = 1 (PLAN_SPEC C1')")
+    if ordering not in (1, 2, 3):
+        raise PlanError("EINVAL", "ordering is 1 or 2 (:138) or 3 (the four-pattern mix, :144-155)")
+    if ordering in (1, 3) and not (g == 1 and len(stragglers) == 1 and schedule == OPTCC):
+        raise PlanError("EUNSUPPORTED", "ordering (1) and the mix are constructed for one straggler, g = 1 (PLAN_SPEC C1', C1'')")
     if n <= 0 or n > 2 ** 40:
         raise PlanError("EINVAL", "0 < n <= 2^40 required")
     if dtype not in (F32, BF16):
@@ -166,7 +166,48 @@ def build_plan(p, g, ell, n, dtype, k=0, _u_p2p_override=None, schedule=OPTCC, o
         if ln > 0:
             flows.append((off, ln, step, seg, sec, src, dst, op, stage, link, part, 0))
 
-    if construction == C1 and ordering == 1:
+    if construction == C1 and ordering == 3:
+        # C1'': the four-pattern mix of :144-155 (PLAN_SPEC §4 C1'').  A, C: ordering (1); B, D: ordering (2); one
+        # stage per parallel body (2(p-1) slots per stage, :146); A and B start in body 4γ, C and D one body later, so a
+        # group of four segments spans five bodies and the schedule has k+1 bodies (:155, :169).
+        n_steps = (k + 1) * H
+        sg = stragglers[0]
+        hr = list(healthy)
+        bubbles = ell1 < 2.0
+        W = lambda j, t: t if t < j else t + 1          # ring link j idle in window j
+        for b in range(k):
+            gam, pat = divmod(b, 4)
+            s0 = 4 * gam + (1 if pat >= 2 else 0)       # first body of the segment
+            if pat in (0, 2):                           # patterns A, C: S1 -> S2 -> S3 -> S4 (:148, :150)
+                for j in range(H):
+                    for t in range(H - 1):
+                        c = (j - t) % H
+                        emit(s0 * H + W(j, t), REDUCE, S1, NIC, 0, hr[j], hr[(j + 1) % H], b, c, sec_units(0, b, c))
+                        emit((s0 + 3) * H + W(j, t), COPY, S4, NIC, 0, hr[j], hr[(j + 1) % H], b, c, sec_units(0, b, c))
+                for a in range(H):
+                    d = (a + 1) % H
+                    # the straggler adds its own data to the uploaded partial sum (:130-132) ...
+                    emit((s0 + 1) * H + a, REDUCE, S2, NIC, 0, hr[a], sg, b, (a + 1) % H, sec_units(0, b, (a + 1) % H))
+                    # ... and returns the global sum to the uploader's ring successor (:132, R11)
+                    emit((s0 + 2) * H + a, COPY, S3, NIC, 0, sg, hr[d], b, d, sec_units(0, b, d))
+            else:                                       # patterns B, D: S3 -> S1 -> S4 -> S2 (:149, :151)
+                for a in range(H):
+                    d = (a + 1) % H
+                    # the straggler's raw section is folded in at its owner first (:138 ordering (2)) ...
+                    emit(s0 * H + a, REDUCE, S3, NIC, 0, sg, hr[d], b, (d + 1) % H, sec_units(0, b, (d + 1) % H))
+                    # ... and the owner sends the global sum back last
+                    emit((s0 + 3) * H + a, COPY, S2, NIC, 0, hr[a], sg, b, (a + 1) % H, sec_units(0, b, (a + 1) % H))
+                for j in range(H):
+                    for t in range(H - 1):
+                        emit((s0 + 1) * H + W(j, t), REDUCE, S1, NIC, 0, hr[j], hr[(j + 1) % H], b, (j - t) % H,
+                             sec_units(0, b, (j - t) % H))
+                        emit((s0 + 2) * H + W(j, t), COPY, S4, NIC, 0, hr[j], hr[(j + 1) % H], b, (j + 1 - t) % H,
+                             sec_units(0, b, (j + 1 - t) % H))
+            if bubbles:                                 # bubble-up in body b, bubble-down in body b+1, as in C1 (:165)
+                for a in range(H):
+                    emit(b * H + a, REDUCE, BUB_UP, NIC, 0, hr[a], sg, b, 0, p2p_piece(b))
+                    emit((b + 1) * H + a, COPY, BUB_DOWN, NIC, 0, sg, hr[(a + 1) % H], b, 0, p2p_piece(b))
+    elif construction == C1 and ordering == 1:
         # C1': ordering (1) of :138, S1 -> S2 -> S3 -> S4, one stage per body (PLAN_SPEC §4 C1')
         n_steps = (k + 3) * H
         sg = stragglers[0]

@@ -53,10 +53,15 @@ __device__ __forceinline__ char* rank_ptr(const ExecParams& P, unsigned int r) {
 // stage / from_stage (column executor's bulk all-gather path, data runs): a reduce flow with `stage` also keeps the sum
 // it stores in that shared-memory image of the tile; a copy flow with `from_stage` has its whole vectors stored by one
 // thread's cp.async.bulk (see optcc_column_kernel), only the ragged end of a buffer is moved here.
-template <int MODE, int NT, class PolX>
+// carry / use_carry (lazy contributor-mask runs of the column executor): the sets this thread produced in the previous
+// flow of the list, taken instead of a load when the flow says so (DFLOW_SRC_FWD); other callers pass a scratch array.
+// MASK_FWD (column executor, contributor-mask runs): the run is in the lazy form and every tile is one round, so only
+// the forwarding round (range_mask_round) is compiled in -- the kernel then has the registers to keep `carry` live.
+template <int MODE, int NT, bool MASK_FWD = false, class PolX>
 __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& f, unsigned long long ubeg,
                                               unsigned long long uend, unsigned int& overlaps, const PolX& pol,
-                                              char* stage = nullptr, bool from_stage = false) {
+                                              uint4 (&carry)[4], bool use_carry = false,
+                                              char* stage = nullptr, bool from_stage = false, bool* stage_full = nullptr) {
   using MT = ModeTraits<MODE>;
   const unsigned int tid = group_tid<NT>();
   const unsigned long long A = P.unit_elems;
@@ -91,14 +96,25 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
     char* d = rank_ptr(P, f.dst) + f.off * EB;
     const unsigned int lazy = P.mask_lazy ? f.flags & (DFLOW_SRC_INIT | DFLOW_DST_INIT | DFLOW_FINAL) : 0u;
     const unsigned long long full0 = P.n_ranks >= 64 ? ~0ull : ((1ull << P.n_ranks) - 1ull);
-    if (lazy) {   // lazy verifier: initial masks are constants, the last writer checks the final mask (range_mask_lazy)
-      const unsigned long long full1 = P.n_ranks > 64 ? (P.n_ranks >= 128 ? ~0ull : ((1ull << (P.n_ranks - 64)) - 1ull)) : 0ull;
+    const unsigned long long full1 = P.n_ranks > 64 ? (P.n_ranks >= 128 ? ~0ull : ((1ull << (P.n_ranks - 64)) - 1ull)) : 0ull;
+    if (from_stage) {
+      // whole vectors: stored by cp.async.bulk from the stage -- or, when this copy is the last writer of its range
+      // (lazy form) and the staged sets are not all complete, through the LSU with every wrong element reported
+      if (stage)
+        range_copy_stage_checked<EB, NT>(stage, d, vbeg, vend, pol, mask_vector(full0, full1, EB), P.ctrl,
+                                         (unsigned long long)f.dst * P.n + f.off);
+    } else if (MASK_FWD) {      // lazy form, one round per tile: partial sets are forwarded through `carry`
+      const uint4 SC = mask_vector(f.src < 64 ? 1ull << f.src : 0ull, f.src >= 64 ? 1ull << (f.src - 64) : 0ull, EB);
+      const uint4 DC = mask_vector(f.dst < 64 ? 1ull << f.dst : 0ull, f.dst >= 64 ? 1ull << (f.dst - 64) : 0ull, EB);
+      range_mask_round<4, EB, NT>(s, d, vbeg, vend, overlaps, pol, f.flags, f.op == 0, SC, DC, mask_vector(full0, full1, EB),
+                                  P.ctrl, (unsigned long long)f.dst * P.n + f.off, f.op == 0 ? stage : nullptr, stage_full, carry);
+    } else if (P.mask_lazy) {   // lazy verifier: initial masks are constants, the last writer checks the final mask (range_mask_lazy)
       const uint4 SC = mask_vector(f.src < 64 ? 1ull << f.src : 0ull, f.src >= 64 ? 1ull << (f.src - 64) : 0ull, EB);
       const uint4 DC = mask_vector(f.dst < 64 ? 1ull << f.dst : 0ull, f.dst >= 64 ? 1ull << (f.dst - 64) : 0ull, EB);
       range_mask_lazy<4, EB, NT>(s, d, vbeg, vend, overlaps, pol, f.flags, f.op == 0, SC, DC, mask_vector(full0, full1, EB),
-                                 P.ctrl, (unsigned long long)f.dst * P.n + f.off);
+                                 P.ctrl, (unsigned long long)f.dst * P.n + f.off, f.op == 0 ? stage : nullptr, stage_full);
     } else if (f.op == 0) {
-      range_or_mask<4, EB, NT>(s, d, vbeg, vend, overlaps, pol, dead_src);
+      range_or_mask<4, EB, NT>(s, d, vbeg, vend, overlaps, pol, dead_src, stage, mask_vector(full0, full1, EB), stage_full);
     } else {
       range_copy16<4, NT>(s, d, vbeg, vend, pol);
     }
@@ -182,6 +198,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) optcc_exec_kernel(const 
 
   const unsigned int G = gridDim.x, cta = blockIdx.x;
   unsigned int overlaps = 0;
+  uint4 scratch[4];
   const Pol pol = make_policies(P.l2_hints);
 
   auto stage = [&](unsigned int step, int buf, unsigned int lane) {
@@ -222,7 +239,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) optcc_exec_kernel(const 
       const unsigned long long nunits = (f.len + A - 1) / A;
       const unsigned long long ubeg = i == 0 ? ub : 0ull;
       const unsigned long long uend = (i + 1 == nf && ue > 0) ? ue : nunits;
-      process_piece<MODE, THREADS>(P, f, ubeg, uend, overlaps, pol);
+      process_piece<MODE, THREADS>(P, f, ubeg, uend, overlaps, pol, scratch);
     }
     if (step + 1 < P.step_hi) {
       if (P.use_barrier) grid_barrier(&P.ctrl->barrier, (unsigned long long)(step - P.step_lo + 1) * G);
@@ -485,7 +502,8 @@ __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel
       if (kind == 1) {   // kind 2: the agent copies it with cp.async.bulk; the streaming warps move on
         const DFlow f = s_slot[s].f;
         const unsigned long long ubeg = s_slot[s].ubeg, uend = s_slot[s].uend;
-        process_piece<MODE, DF_COMPUTE_THREADS>(P, f, ubeg, uend, overlaps, pol);
+        uint4 scratch[4];
+        process_piece<MODE, DF_COMPUTE_THREADS>(P, f, ubeg, uend, overlaps, pol, scratch);
       }
       __syncwarp();
       if ((threadIdx.x & 31) == 0) red_release_cta_shared_add(&s_done[s], 1u);
@@ -533,7 +551,7 @@ __device__ __forceinline__ void prefetch_raw(const ExecParams& P, const DFlow& f
 constexpr unsigned int COL_REC = 256;   // flow records staged in shared memory at a time (8 KB)
 constexpr unsigned int COL_PF_MAX = 8;  // deepest look-ahead (flows)
 
-template <int MODE>
+template <int MODE, bool MASK_FWD = false>
 __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(const __grid_constant__ ExecParams P) {
   __shared__ unsigned long long s_item[2];          // work items are claimed one item ahead
   __shared__ __align__(16) DFlow s_rec[COL_REC];    // this CTA's staged part of the region's flow list
@@ -546,7 +564,10 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
   pol.lds = pol0.lds; pol.ldd = pol0.ldd; pol.st = pol0.st;
   const unsigned int D = is_mask_mode(MODE) ? 0u : (P.col_pf_dist < COL_PF_MAX ? P.col_pf_dist : COL_PF_MAX);
   extern __shared__ __align__(128) char s_stage_col[];   // bulk all-gather path: the tile of the sum being distributed
-  const bool bulk = !is_mask_mode(MODE) && P.col_bulk != 0;
+  const bool bulk = P.col_bulk != 0;
+  bool stage_ok = true;              // contributor masks: every staged set is the full set
+  unsigned int bulk_turn = 0;        // bulk stores issued so far (the warps' first lanes take turns)
+  uint4 carry[4];                    // lazy contributor-mask runs: what the previous flow produced (DFLOW_SRC_FWD)
   const unsigned long long bulk_pol = make_policy(P.col_bulk_policy);   // L2 policy of the bulk stores
   if (threadIdx.x == 0) {
     s_item[0] = atomicAdd(&P.ctrl->ticket, 1ull);
@@ -592,36 +613,47 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
           if (prev_cls >= 0 && cls != prev_cls) __syncthreads();
           prev_cls = cls;
         }
-        if (!is_mask_mode(MODE) && bulk) {
+        if (bulk) {
           // Bulk all-gather path.  The reduce flow that completes a sum which later copy flows distribute
           // (DFLOW_STAGE_OUT, found by the host's walk of the region's list) stores it to its destination as listed
           // and also keeps it in shared memory; every copy flow whose source range holds exactly that tile
           // (DFLOW_FROM_STAGE) is then one cp.async.bulk store of the staged tile to its destination, issued by one
           // thread in list order -- the all-gather steps move through the TMA unit instead of LDG / STG.
+          // Contributor masks, lazy form: a copy that is the last writer of its range must check what it stores; the
+          // staged sets are checked once (stage_ok), and only if they are not all complete (a wrong or truncated
+          // plan) such copies go through the LSU and report every wrong element.
           const unsigned int fl = cur.flags;
           if (fl & DFLOW_STAGE_OUT) {        // the stage is rewritten: the previous tile's bulk stores must have read it
-            if (threadIdx.x == 0) bulk_wait_read_all();
+            if ((threadIdx.x & 31u) == 0) bulk_wait_read_all();   // (every warp's first lane issues bulk stores, in turn)
             __syncthreads();
-            process_piece<MODE, COL_THREADS>(P, cur, ubeg, uend, overlaps, pol, s_stage_col, false);
+            bool mine = true;
+            process_piece<MODE, COL_THREADS, MASK_FWD>(P, cur, ubeg, uend, overlaps, pol, carry, true, s_stage_col, false, &mine);
             // this thread's generic-proxy writes (the stage; its earlier stores to ranges the bulk stores will overwrite)
             // are ordered before the async-proxy operations issued after the barrier
             fence_proxy_async();
-            __syncthreads();
+            if (is_mask_mode(MODE)) stage_ok = __syncthreads_and(mine) != 0; else __syncthreads();
           } else if (fl & DFLOW_FROM_STAGE) {
-            if (threadIdx.x == 0) {
-              constexpr unsigned long long ESZ = MODE == MODE_F32 ? 4 : 2, VE = 16 / ESZ;
-              const unsigned long long e0 = ubeg * P.unit_elems;
-              unsigned long long e1 = uend * P.unit_elems;
-              if (e1 > cur.len) e1 = cur.len;
-              const unsigned long long v0 = e0 / VE, v1 = e1 / VE;
-              if (v1 > v0) bulk_s2g_hint(rank_ptr(P, cur.dst) + cur.off * ESZ + v0 * 16, s_stage_col, (unsigned int)((v1 - v0) * 16), bulk_pol);
+            if (is_mask_mode(MODE) && P.mask_lazy && (fl & DFLOW_FINAL) && !stage_ok) {
+              process_piece<MODE, COL_THREADS, MASK_FWD>(P, cur, ubeg, uend, overlaps, pol, carry, false, s_stage_col, true);
+            } else {
+              // the copies of one tile are issued by the warps' first lanes in turn: 60+ cp.async.bulk per tile (C3: every
+              // section goes to p - 1 ranks) would otherwise queue behind one thread
+              if (threadIdx.x == (bulk_turn % (COL_THREADS / 32)) * 32) {
+                constexpr unsigned long long ESZ = ModeTraits<MODE>::ESIZE, VE = 16 / ESZ;
+                const unsigned long long e0 = ubeg * P.unit_elems;
+                unsigned long long e1 = uend * P.unit_elems;
+                if (e1 > cur.len) e1 = cur.len;
+                const unsigned long long v0 = e0 / VE, v1 = e1 / VE;
+                if (v1 > v0) bulk_s2g_hint(rank_ptr(P, cur.dst) + cur.off * ESZ + v0 * 16, s_stage_col, (unsigned int)((v1 - v0) * 16), bulk_pol);
+              }
+              ++bulk_turn;
+              process_piece<MODE, COL_THREADS, MASK_FWD>(P, cur, ubeg, uend, overlaps, pol, carry, false, nullptr, true);   // (ragged end of a buffer only)
             }
-            process_piece<MODE, COL_THREADS>(P, cur, ubeg, uend, overlaps, pol, nullptr, true);   // (ragged end of a buffer only)
           } else {
-            process_piece<MODE, COL_THREADS>(P, cur, ubeg, uend, overlaps, pol);
+            process_piece<MODE, COL_THREADS, MASK_FWD>(P, cur, ubeg, uend, overlaps, pol, carry, true);
           }
         } else {
-          process_piece<MODE, COL_THREADS>(P, cur, ubeg, uend, overlaps, pol);
+          process_piece<MODE, COL_THREADS, MASK_FWD>(P, cur, ubeg, uend, overlaps, pol, carry, true);
         }
         __syncwarp();   // orders a lane's dead-source discard of a 128-byte line before the other lanes' later stores to it
       };
@@ -648,7 +680,8 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
     it = nit;
     nit = s_item[round & 1];
   }
-  if (bulk && threadIdx.x == 0) bulk_wait_all();   // the stage stays valid until every bulk store has read it
+  if (bulk && (threadIdx.x & 31u) == 0) bulk_wait_all();   // the stage stays valid until every bulk store has read it
+  __syncthreads();                   // (shared memory is released when the last thread leaves)
   if (is_mask_mode(MODE)) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) overlaps += __shfl_xor_sync(0xFFFFFFFFu, overlaps, o);
@@ -673,23 +706,25 @@ __device__ __forceinline__ DFlow load_record(const DFlow* p) {
   return f;
 }
 
-template <int MODE>
+template <int MODE, bool MASK_FWD = false>
 __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel(const __grid_constant__ ExecParams P) {
   extern __shared__ __align__(128) char s_stage_w[];   // bulk all-gather path: one tile per warp
   const unsigned int lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-  char* const stage = s_stage_w + (size_t)warp * P.tile_units * 16;
+  char* const stage = s_stage_w + (size_t)warp * P.col_stage_bytes;
   unsigned int overlaps = 0;
   const Pol pol0 = make_policies(P.l2_hints);
   PolL1 pol;                         // a tile is private to its warp for the whole launch: loads and stores through L1
   pol.lds = pol0.lds; pol.ldd = pol0.ldd; pol.st = pol0.st;
-  const bool bulk = !is_mask_mode(MODE) && P.col_bulk != 0;
+  const bool bulk = P.col_bulk != 0;
+  bool stage_ok = true;              // contributor masks: every staged set is the full set
+  uint4 carry[4];                    // lazy contributor-mask runs: what the previous flow produced (DFLOW_SRC_FWD)
   const unsigned long long bulk_pol = make_policy(P.col_bulk_policy);   // L2 policy of the bulk stores
   const bool pf = !is_mask_mode(MODE) && P.col_pf_dist != 0;
-  for (;;) {
-    unsigned long long it = 0;
-    if (lane == 0) it = atomicAdd(&P.ctrl->ticket, 1ull);
-    it = __shfl_sync(0xFFFFFFFFu, it, 0);
-    if (it >= P.col_n_items) break;
+  // Items are dealt round-robin to the warps of the grid (neighbouring warps take neighbouring tiles): a global ticket
+  // would be claimed once per warp and item, and same-address atomics from different SMs complete about one per 90 ns
+  // (measured: 131 k items -> 11.7 ms), more than the items' own work.
+  const unsigned long long n_warps = (unsigned long long)gridDim.x * (COL_THREADS / 32);
+  for (unsigned long long it = (unsigned long long)blockIdx.x * (COL_THREADS / 32) + warp; it < P.col_n_items; it += n_warps) {
     const uint4 item = __ldg(P.col_items + it);
     const unsigned int fb = item.x, fe = item.y;
     const unsigned long long ubeg = (unsigned long long)item.z * P.tile_units, uend = ubeg + item.w;
@@ -711,23 +746,28 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel
         // the stage is rewritten: the previous tile's bulk stores must have read it
         if (lane == 0) bulk_wait_read_all();
         __syncwarp();
-        process_piece<MODE, 32>(P, cur, ubeg, uend, overlaps, pol, stage, false);
+        bool mine = true;
+        process_piece<MODE, 32, MASK_FWD>(P, cur, ubeg, uend, overlaps, pol, carry, true, stage, false, &mine);
         // this lane's generic-proxy writes (the stage; its earlier stores to ranges the bulk stores will overwrite) are
         // ordered before the async-proxy operations lane 0 issues after the warp barrier
         fence_proxy_async();
-        __syncwarp();
+        if (is_mask_mode(MODE)) stage_ok = __all_sync(0xFFFFFFFFu, mine) != 0; else __syncwarp();
       } else if (bulk && (fl & DFLOW_FROM_STAGE)) {
-        if (lane == 0) {
-          constexpr unsigned long long ESZ = MODE == MODE_F32 ? 4 : 2, VE = 16 / ESZ;
-          const unsigned long long e0 = ubeg * P.unit_elems;
-          unsigned long long e1 = uend * P.unit_elems;
-          if (e1 > cur.len) e1 = cur.len;
-          const unsigned long long v0 = e0 / VE, v1 = e1 / VE;
-          if (v1 > v0) bulk_s2g_hint(rank_ptr(P, cur.dst) + cur.off * ESZ + v0 * 16, stage, (unsigned int)((v1 - v0) * 16), bulk_pol);
+        if (is_mask_mode(MODE) && P.mask_lazy && (fl & DFLOW_FINAL) && !stage_ok) {
+          process_piece<MODE, 32, MASK_FWD>(P, cur, ubeg, uend, overlaps, pol, carry, false, stage, true);
+        } else {
+          if (lane == 0) {
+            constexpr unsigned long long ESZ = ModeTraits<MODE>::ESIZE, VE = 16 / ESZ;
+            const unsigned long long e0 = ubeg * P.unit_elems;
+            unsigned long long e1 = uend * P.unit_elems;
+            if (e1 > cur.len) e1 = cur.len;
+            const unsigned long long v0 = e0 / VE, v1 = e1 / VE;
+            if (v1 > v0) bulk_s2g_hint(rank_ptr(P, cur.dst) + cur.off * ESZ + v0 * 16, stage, (unsigned int)((v1 - v0) * 16), bulk_pol);
+          }
+          process_piece<MODE, 32, MASK_FWD>(P, cur, ubeg, uend, overlaps, pol, carry, false, nullptr, true);   // (ragged end of a buffer only)
         }
-        process_piece<MODE, 32>(P, cur, ubeg, uend, overlaps, pol, nullptr, true);   // (ragged end of a buffer only)
       } else {
-        process_piece<MODE, 32>(P, cur, ubeg, uend, overlaps, pol);
+        process_piece<MODE, 32, MASK_FWD>(P, cur, ubeg, uend, overlaps, pol, carry, true);
       }
       __syncwarp();   // orders a lane's dead-source discard of a 128-byte line before the other lanes' later stores to it
       cur = nxt;
@@ -836,6 +876,7 @@ struct optcc_exec_state {
   optcc_rawvec<DFlow> col_dflows;        // the executed flows, region by region (chain order inside a region)
   std::vector<uint32_t> col_reg_begin;   // [regions + 1]
   std::vector<uint4> col_items;          // (first flow, end flow, tile, units in the tile)
+  std::vector<uint4> col_items_mask;     // the verifier's items when its tile size differs (plan's mask_tile_units)
 };
 
 void optcc_exec_state_free(optcc_exec_state* s) { delete s; }
@@ -1098,10 +1139,18 @@ bool finish_region(DFlow* L, uint32_t n, const ColBuildOpts& o, ColScratch& sc) 
     DFlow& f = L[i];
     if (!sc.written[f.dst]) f.flags |= DFLOW_FINAL;
     sc.written[f.dst] = 1;
-    if (o.discard && f.op == OPTCC_OP_REDUCE && sc.next[f.src] == NEXT_COPY_WRITE && sc.sole[i]) f.flags |= DFLOW_DEAD_SRC;
+    const bool dead = f.op == OPTCC_OP_REDUCE && sc.next[f.src] == NEXT_COPY_WRITE && sc.sole[i];
+    if (o.discard && dead) f.flags |= DFLOW_DEAD_SRC;
+    // the verifier's forwarding (lazy contributor-mask runs only): the dead source was written by the flow just before
+    // this one, so the sets are still in the thread's registers -- and that flow need not store them, unless its
+    // result is a final value or the staged tile
+    if (dead && i > 0 && L[i - 1].dst == f.src) {
+      f.flags |= DFLOW_SRC_FWD;
+    }
     sc.next[f.dst] = f.op == OPTCC_OP_COPY ? NEXT_COPY_WRITE : NEXT_REDUCE_WRITE;
     sc.next[f.src] = NEXT_READ;
   }
+
   // Bulk all-gather path (data runs): find the reduce flows whose sum later copy flows distribute (DFLOW_STAGE_OUT: the
   // CTA keeps the tile in shared memory) and the copy flows whose source range holds exactly the staged tile at that
   // point (DFLOW_FROM_STAGE: one cp.async.bulk store).  Value numbering: a reduce gives its destination a new value,
@@ -1149,6 +1198,11 @@ bool finish_region(DFlow* L, uint32_t n, const ColBuildOpts& o, ColScratch& sc) 
       }
     }
     if (!ok) for (uint32_t i = 0; i < n; ++i) L[i].flags &= ~(DFLOW_STAGE_OUT | DFLOW_FROM_STAGE);
+  }
+  for (uint32_t i = 1; i < n; ++i) {
+    if (!(L[i].flags & DFLOW_SRC_FWD)) continue;
+    if (L[i - 1].flags & DFLOW_FROM_STAGE) L[i].flags &= ~DFLOW_SRC_FWD;      // (stored by cp.async.bulk: not in registers)
+    else if (!(L[i - 1].flags & (DFLOW_FINAL | DFLOW_STAGE_OUT))) L[i - 1].flags |= DFLOW_NO_STORE;
   }
   sc.rep_final.assign(L, L + n);
   sc.rep_covered = covered == p;
@@ -1289,18 +1343,20 @@ void build_column_state(optcc_plan_t* pl, optcc_exec_state* st, bool* all_covere
   TT("finish");
   *all_covered = uncovered.load() == 0;
   // ---- 3. one work item per (region, tile) ----
-  st->col_items.clear();
-  st->col_items.reserve(pl->tiles_per_rank);
-  for (size_t r = 0; r < nr; ++r) {
-    const uint64_t t0 = pl->region_tile0[r], t1 = r + 1 < nr ? pl->region_tile0[r + 1] : pl->tiles_per_rank;
-    const uint32_t fb = st->col_reg_begin[r], fe = st->col_reg_begin[r + 1];
-    if (fb == fe) continue;
-    const uint64_t nunits = (pl->region_len[r] + A - 1) / A;
-    for (uint64_t t = 0; t < t1 - t0; ++t) {
-      const uint64_t ubeg = t * TU, left = nunits > ubeg ? nunits - ubeg : 0;
-      st->col_items.push_back(make_uint4(fb, fe, (unsigned int)t, (unsigned int)std::min<uint64_t>(left, TU)));
+  auto make_items = [&](std::vector<uint4>& items, uint64_t tu, uint64_t reserve) {
+    items.clear();
+    items.reserve(reserve);
+    for (size_t r = 0; r < nr; ++r) {
+      const uint32_t fb = st->col_reg_begin[r], fe = st->col_reg_begin[r + 1];
+      if (fb == fe) continue;
+      const uint64_t nunits = (pl->region_len[r] + A - 1) / A;
+      for (uint64_t t = 0, ubeg = 0; ubeg < nunits; ++t, ubeg += tu)
+        items.push_back(make_uint4(fb, fe, (unsigned int)t, (unsigned int)std::min<uint64_t>(nunits - ubeg, tu)));
     }
-  }
+  };
+  make_items(st->col_items, TU, pl->tiles_per_rank);
+  if (pl->mask_tile_units != pl->tile_units) make_items(st->col_items_mask, pl->mask_tile_units, pl->mask_tiles_per_rank);
+  else st->col_items_mask.clear();
 }
 
 template <int MODE>
@@ -1482,6 +1538,8 @@ int upload_tables(optcc_plan_t* pl, void* workspace, cudaStream_t stream, bool f
       CU_TRY(cudaMemcpyAsync(ws + L.dflows, st->col_dflows.data(), st->col_dflows.size() * sizeof(DFlow), cudaMemcpyHostToDevice, stream));
     if (!st->col_items.empty())
       CU_TRY(cudaMemcpyAsync(ws + L.col, st->col_items.data(), st->col_items.size() * sizeof(uint4), cudaMemcpyHostToDevice, stream));
+    if (!st->col_items_mask.empty())
+      CU_TRY(cudaMemcpyAsync(ws + L.col_mask, st->col_items_mask.data(), st->col_items_mask.size() * sizeof(uint4), cudaMemcpyHostToDevice, stream));
   } else if (!st->dflows.empty())
     CU_TRY(cudaMemcpyAsync(ws + L.dflows, st->dflows.data(), st->dflows.size() * sizeof(DFlow), cudaMemcpyHostToDevice, stream));
   if (!st->slices.empty())
@@ -1511,21 +1569,44 @@ int launch_plan(optcc_plan_t* pl, ExecParams& P, cudaStream_t stream) {
   const bool persistent = pl->opts.exec_mode == OPTCC_EXEC_PERSISTENT && st->coop;
   const bool dataflow = pl->opts.exec_mode == OPTCC_EXEC_DATAFLOW && st->coop && st->df_ok && st->G_df > 0;
   if (st->column) {
-    P.col_n_items = st->col_items.size();
+    // contributor-mask runs have their own tile size (mask_tile_units) when a unit of masks is wider than 16 bytes
+    const bool own_items = is_mask_mode(MODE) && !st->col_items_mask.empty();
+    if (is_mask_mode(MODE)) P.col_warp = pl->mask_warp;
+    if (own_items) {
+      P.col_items = reinterpret_cast<const uint4*>(static_cast<char*>(static_cast<void*>(P.ctrl)) + optcc_layout(pl).col_mask);
+      P.tile_units = pl->mask_tile_units;
+    }
+    P.col_n_items = own_items ? st->col_items_mask.size() : st->col_items.size();
     if (P.col_n_items == 0) return OPTCC_OK;
     CU_TRY(cudaMemsetAsync(&P.ctrl->ticket, 0, sizeof(unsigned long long), stream));
     const uint32_t G = pl->opts.grid_ctas ? pl->opts.grid_ctas : uint32_t(st->sm_count) * CTAS_PER_SM;
     const unsigned int grid = (unsigned int)std::min<uint64_t>(G, P.col_n_items);
+    // the stage of the bulk all-gather path: one tile (of data, or of masks: unit_elems * mask bytes per unit)
+    const size_t tile_bytes = size_t(P.tile_units) * (is_mask_mode(MODE) ? size_t(in.unit_elems) * mask_bytes_of(MODE) : 16);
+    P.col_stage_bytes = (unsigned int)tile_bytes;
+    // partial sets are forwarded through registers when a thread's vectors are the same in every flow: one round at most
+    P.mask_fwd = (is_mask_mode(MODE) && P.mask_lazy && tile_bytes / 16 <= size_t(4) * (P.col_warp ? 32 : COL_THREADS)) ? 1u : 0u;
+    constexpr bool MASKS = is_mask_mode(MODE);
     if (P.col_warp) {
-      // warp-wide tiles: one stage per warp; a CTA's 14 warps claim items on their own
-      const size_t dyn = (!is_mask_mode(MODE) && P.col_bulk) ? size_t(pl->tile_units) * 16 * (COL_THREADS / 32) : 0;
-      if (dyn > 40 * 1024) CU_TRY(cudaFuncSetAttribute(optcc_wcolumn_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+      // warp-wide tiles: one stage per warp; a CTA's 14 warps take items on their own
+      const size_t dyn = P.col_bulk ? tile_bytes * (COL_THREADS / 32) : 0;
       const unsigned int wgrid = (unsigned int)std::min<uint64_t>(G, (P.col_n_items + COL_THREADS / 32 - 1) / (COL_THREADS / 32));
-      optcc_wcolumn_kernel<MODE><<<wgrid, COL_THREADS, dyn, stream>>>(P);
+      if (MASKS && P.mask_fwd) {
+        if (dyn > 40 * 1024) CU_TRY(cudaFuncSetAttribute(optcc_wcolumn_kernel<MODE, MASKS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+        optcc_wcolumn_kernel<MODE, MASKS><<<wgrid, COL_THREADS, dyn, stream>>>(P);
+      } else {
+        if (dyn > 40 * 1024) CU_TRY(cudaFuncSetAttribute(optcc_wcolumn_kernel<MODE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+        optcc_wcolumn_kernel<MODE, false><<<wgrid, COL_THREADS, dyn, stream>>>(P);
+      }
     } else {
-      const size_t dyn = (!is_mask_mode(MODE) && P.col_bulk) ? size_t(pl->tile_units) * 16 : 0;   // the stage: one tile
-      if (dyn > 40 * 1024) CU_TRY(cudaFuncSetAttribute(optcc_column_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
-      optcc_column_kernel<MODE><<<grid, COL_THREADS, dyn, stream>>>(P);
+      const size_t dyn = P.col_bulk ? tile_bytes : 0;
+      if (MASKS && P.mask_fwd) {
+        if (dyn > 40 * 1024) CU_TRY(cudaFuncSetAttribute(optcc_column_kernel<MODE, MASKS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+        optcc_column_kernel<MODE, MASKS><<<grid, COL_THREADS, dyn, stream>>>(P);
+      } else {
+        if (dyn > 40 * 1024) CU_TRY(cudaFuncSetAttribute(optcc_column_kernel<MODE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+        optcc_column_kernel<MODE, false><<<grid, COL_THREADS, dyn, stream>>>(P);
+      }
     }
     CU_TRY(cudaGetLastError());
   } else if (dataflow) {
@@ -1583,10 +1664,10 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   if (pl->opts.exec_mode == OPTCC_EXEC_COLUMN) P.l2_hints = 0;   // see optcc_column_kernel
   P.col_pf_dist = 1; P.col_pf_l2 = 0; P.col_pf_next = 0; P.col_bulk = 1;
   P.col_bulk_policy = 1;   // bulk stores evict_first: the all-gather's results are never read again (measured: C2 1.68 -> 1.62 ms)
-  P.col_warp = pl->tile_units <= 256 ? 1u : 0u;
+  P.col_warp = pl->col_warp;
   if (const char* t = std::getenv("OPTCC_TUNE")) {   // TEMPORARY (experiments): "dist,l2,next,bulk,bulkpolicy"
     unsigned a = 1, b = 0, c = 0, d = 1, e = 1, f = 0;
-    if (std::sscanf(t, "%u,%u,%u,%u,%u,%u", &a, &b, &c, &d, &e, &f) >= 1) { P.col_pf_dist = a; P.col_pf_l2 = b; P.col_pf_next = c; P.col_bulk = d; P.col_bulk_policy = e; P.col_warp = f; }
+    if (std::sscanf(t, "%u,%u,%u,%u,%u,%u", &a, &b, &c, &d, &e, &f) >= 1) { P.col_pf_dist = a; P.col_pf_l2 = b; P.col_pf_next = c; P.col_bulk = d; P.col_bulk_policy = e; (void)f; }
   }
   if (pl->opts.copy_path == 1) P.col_bulk = 0;
 }

@@ -72,6 +72,13 @@ struct optcc_plan {
   uint32_t tile_units = 0;
   uint64_t n_tile_ops = 0;              // sum over flows of ceil(units / tile_units)
   uint64_t tiles_per_rank = 0;          // sum over regions of ceil(units / tile_units): counters per rank
+  // column executor, contributor-mask runs: a mask tile should have about the bytes of a data tile (the stage of the
+  // bulk all-gather path holds one), but a unit of A elements is A * mask_bytes >= 16 bytes of masks
+  uint32_t mask_tile_units = 0;
+  uint64_t mask_tiles_per_rank = 0;
+  // column executor: a tile is taken through its list by a whole CTA (0) or by one warp (1), chosen from the plan's
+  // shape for the data run and for the contributor-mask run separately
+  uint32_t col_warp = 0, mask_warp = 0;
   std::vector<uint64_t> region_offs;    // sorted unique flow offsets (regions tile [0, n), PLAN_SPEC 5.4)
   std::vector<uint64_t> region_len;     // elements of every region
   std::vector<uint32_t> region_flows;   // flows over every region
@@ -113,7 +120,7 @@ constexpr uint64_t OPTCC_DFLOW_BYTES = 32;      // sizeof(DFlow) in optcc_exec.c
 constexpr uint64_t OPTCC_SLICE_BYTES = 16;      // sizeof(Slice)
 
 struct optcc_ws_layout {
-  uint64_t ctrl, ptrs, dflows, slices, deps, ops, col, counters, shadow, masks, end_exec, end_verify;
+  uint64_t ctrl, ptrs, dflows, slices, deps, ops, col, col_mask, counters, shadow, masks, end_exec, end_verify;
 };
 
 static inline uint64_t optcc_align256(uint64_t x) { return (x + 255) & ~uint64_t(255); }
@@ -132,7 +139,8 @@ static inline optcc_ws_layout optcc_layout(const optcc_plan_t* pl) {
   L.deps = optcc_align256(L.slices + uint64_t(in.n_steps) * (OPTCC_MAX_GRID + 1) * OPTCC_SLICE_BYTES);
   L.ops = optcc_align256(L.deps + uint64_t(in.n_flows) * OPTCC_DEP_BYTES);
   L.col = optcc_align256(L.ops + pl->n_tile_ops * OPTCC_OP_BYTES);   // column executor: work items, 16 B per (region, tile)
-  L.counters = optcc_align256(L.col + pl->tiles_per_rank * 16);
+  L.col_mask = optcc_align256(L.col + pl->tiles_per_rank * 16);      // the verifier's work items when its tiles differ
+  L.counters = optcc_align256(L.col_mask + (pl->mask_tile_units != pl->tile_units ? pl->mask_tiles_per_rank * 16 : 0));
   L.shadow = optcc_align256(L.counters + uint64_t(in.p) * pl->tiles_per_rank * 4);
   uint64_t n_pad = (in.n + 7) & ~uint64_t(7);
   L.end_exec = optcc_align256(L.shadow + (in.dtype == OPTCC_BF16 ? uint64_t(in.p) * n_pad * 4 : 0));

@@ -50,6 +50,11 @@ enum : unsigned int {
   // column executor, data runs, bulk all-gather path (see build_column_tables / optcc_column_kernel):
   DFLOW_STAGE_OUT = 64u,   // reduce flow: the sum it stores is the source of later copy flows -- also keep it in the CTA's stage
   DFLOW_FROM_STAGE = 128u, // copy flow: the source range holds exactly the staged tile -- store it with cp.async.bulk
+  // column executor, contributor-mask runs in the lazy form only (the verifier's own arrays; data runs load and store
+  // every flow's operands as listed):
+  DFLOW_SRC_FWD = 256u,    // the source range was written by the previous flow of the list, this flow is its only
+                           // reader and the range is overwritten later: the sets are taken from the thread's registers
+  DFLOW_NO_STORE = 512u,   // ... and that previous flow does not store them (nobody would ever read them from memory)
 };
 
 struct __align__(16) Slice {      // start of a CTA's slice of a step: flow index and 16-byte unit inside it
@@ -113,7 +118,9 @@ struct ExecParams {
   unsigned int mask_lazy;         // contributor-mask runs: 1 = lazy form (initial masks are constants, last writers check)
   unsigned int col_bulk_policy;   // L2 policy of the bulk stores (0 normal, 1 evict_first, 2 evict_last)
   unsigned int col_warp;          // 1: warp-wide tiles (optcc_wcolumn_kernel), 0: CTA-wide tiles (optcc_column_kernel)
-  unsigned int pad3;
+  unsigned int col_stage_bytes;   // bytes of one staged tile (the warp-wide kernel keeps one per warp)
+  unsigned int mask_fwd;          // lazy contributor-mask runs: act on DFLOW_SRC_FWD / DFLOW_NO_STORE
+  unsigned int pad4[3];
 };
 
 // ---- memory access helpers: L2-only loads (data written by other SMs in the previous step), streaming stores ----
@@ -300,10 +307,19 @@ __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* 
 }
 
 // masks: OR with overlap detection.  EB = bytes per mask element (2, 4, 8 or 16); a 16-byte vector holds 16/EB elements
+// stage / all_full (column executor's bulk all-gather path): with `stage`, the joined sets are also kept in that
+// shared-memory image of the tile (vector vbeg at offset 0) and all_full is cleared if any of them differs from F
 template <int UNROLL, int EB, int NT, class PolX>
 __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* __restrict__ d,
                                               unsigned long long vbeg, unsigned long long vend,
-                                              unsigned int& overlaps, const PolX& pol, bool dead_src) {
+                                              unsigned int& overlaps, const PolX& pol, bool dead_src,
+                                              char* stage = nullptr, uint4 F = make_uint4(0u, 0u, 0u, 0u), bool* all_full = nullptr) {
+  auto keep = [&](unsigned long long vv, uint4 o) {
+    if (stage) {
+      sts16(stage + (vv - vbeg) * 16, o);
+      if (((o.x ^ F.x) | (o.y ^ F.y) | (o.z ^ F.z) | (o.w ^ F.w)) != 0u) *all_full = false;
+    }
+  };
   unsigned long long v = vbeg + group_tid<NT>();
   auto join = [&](uint4 a, uint4 b) {
     const unsigned int cx = a.x & b.x, cy = a.y & b.y, cz = a.z & b.z, cw = a.w & b.w;   // elements whose sets overlap
@@ -327,7 +343,11 @@ __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* 
       b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd, pol.l1);
     }
 #pragma unroll
-    for (int j = 0; j < UNROLL; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, join(a[j], b[j]), pol);
+    for (int j = 0; j < UNROLL; ++j) {
+      const uint4 o = join(a[j], b[j]);
+      st16(d + (v + j * (unsigned long long)NT) * 16, o, pol);
+      keep(v + j * (unsigned long long)NT, o);
+    }
     // (only when every lane of the warp is in this round: the line's other vectors were loaded by this instruction)
     if (dead_src && (v - (threadIdx.x & 31u) + 31) + (UNROLL - 1) * (unsigned long long)NT < vend) {
 #pragma unroll
@@ -345,7 +365,11 @@ __device__ __forceinline__ void range_or_mask(const char* __restrict__ s, char* 
         b[j] = ld16(d + (v + j * (unsigned long long)NT) * 16, pol.ldd, pol.l1);
       }
 #pragma unroll
-      for (int j = 0; j < KK; ++j) st16(d + (v + j * (unsigned long long)NT) * 16, join(a[j], b[j]), pol);
+      for (int j = 0; j < KK; ++j) {
+        const uint4 o = join(a[j], b[j]);
+        st16(d + (v + j * (unsigned long long)NT) * 16, o, pol);
+        keep(v + j * (unsigned long long)NT, o);
+      }
     };
     remainder_dispatch<UNROLL>(rem, batch);
   }
@@ -389,16 +413,16 @@ __device__ __noinline__ void report_bad_masks(unsigned long long* bad_ctr, unsig
 
 // SC / DC: the initial vectors of the source / destination rank, F: the full set; g0 = dst * n + f.off (the global
 // index of the flow's first element at its destination); reduce: OR with overlap detection, else assign.
-// SRC_INIT: the source is the constant SC; DSTM: 0 = copy (no destination operand), 1 = reduce with the destination
-// loaded, 2 = reduce with the destination constant DC -- compile-time, so the constants are used in place (the
-// verifier is bound by instruction issue, and selecting them at run time cost a register fill per vector).
-template <int UNROLL, int EB, int NT, bool SRC_INIT, int DSTM, class PolX>
+// SRCM: 0 = the source is loaded, 1 = it is the constant SC; DSTM: 0 = copy (no destination operand), 1 = reduce with
+// the destination loaded, 2 = reduce with the destination constant DC -- compile-time, so the constants are used in
+// place (selecting them at run time cost a register fill per vector).
+template <int UNROLL, int EB, int NT, int SRCM, int DSTM, class PolX>
 __device__ __forceinline__ void range_mask_lazy_t(const char* __restrict__ s, char* __restrict__ d,
                                                   unsigned long long vbeg, unsigned long long vend, unsigned int& overlaps,
                                                   const PolX& pol, unsigned int flags, uint4 SC, uint4 DC, uint4 F,
-                                                  Ctrl* ctrl, unsigned long long g0) {
-  constexpr bool src_init = SRC_INIT, dst_init = DSTM == 2, reduce = DSTM != 0;
-  const bool fin = (flags & DFLOW_FINAL) != 0u, dead_src = (flags & DFLOW_DEAD_SRC) != 0u && !src_init;
+                                                  Ctrl* ctrl, unsigned long long g0, char* stage, bool* all_full) {
+  constexpr bool src_init = SRCM == 1, dst_init = DSTM == 2, reduce = DSTM != 0;
+  const bool fin = (flags & DFLOW_FINAL) != 0u, dead_src = (flags & DFLOW_DEAD_SRC) != 0u && SRCM == 0;
   auto join = [&](uint4 a, uint4 b) {
     const unsigned int cx = a.x & b.x, cy = a.y & b.y, cz = a.z & b.z, cw = a.w & b.w;   // elements whose sets overlap
     if (EB == 2) {
@@ -426,11 +450,14 @@ __device__ __forceinline__ void range_mask_lazy_t(const char* __restrict__ s, ch
     for (int j = 0; j < KK; ++j) {
       const uint4 o = join(a[j], b[j]);
       st16(d + (v + j * (unsigned long long)NT) * 16, o, pol);
-      if (fin) {
+      if (fin || (reduce && stage)) {
         const uint4 df = make_uint4(o.x ^ F.x, o.y ^ F.y, o.z ^ F.z, o.w ^ F.w);
-        if ((df.x | df.y | df.z | df.w) != 0u)
-          report_bad_masks<EB>(&ctrl->bad, &ctrl->first_bad, df, g0 + (v + j * (unsigned long long)NT) * (16 / EB));
+        if ((df.x | df.y | df.z | df.w) != 0u) {
+          if (fin) report_bad_masks<EB>(&ctrl->bad, &ctrl->first_bad, df, g0 + (v + j * (unsigned long long)NT) * (16 / EB));
+          if (reduce && stage) *all_full = false;
+        }
       }
+      if (reduce && stage) sts16(stage + (v + j * (unsigned long long)NT - vbeg) * 16, o);
     }
   };
   unsigned long long v = vbeg + group_tid<NT>();
@@ -448,21 +475,110 @@ __device__ __forceinline__ void range_mask_lazy_t(const char* __restrict__ s, ch
   }
 }
 
+// One round of the lazy form with forwarding (ExecParams.mask_fwd: the tile is at most one round of UNROLL vectors per
+// thread, so a thread handles the same vectors in every flow of the item).  `carry` holds what the previous flow of
+// the list produced for them: DFLOW_SRC_FWD takes the source from there instead of loading it, DFLOW_NO_STORE skips the
+// store of a result that is only ever read that way and overwritten later.  With both, a ring hop of the verifier is a
+// few ALU instructions per vector: the partial sets never travel through L1 / L2.  Flags are warp-uniform.
+template <int UNROLL, int EB, int NT, class PolX>
+__device__ __forceinline__ void range_mask_round(const char* __restrict__ s, char* __restrict__ d,
+                                                 unsigned long long vbeg, unsigned long long vend, unsigned int& overlaps,
+                                                 const PolX& pol, unsigned int flags, bool reduce, uint4 SC, uint4 DC, uint4 F,
+                                                 Ctrl* ctrl, unsigned long long g0, char* stage, bool* all_full,
+                                                 uint4 (&carry)[UNROLL]) {
+  const bool src_init = (flags & DFLOW_SRC_INIT) != 0u, src_fwd = (flags & DFLOW_SRC_FWD) != 0u;
+  const bool dst_init = (flags & DFLOW_DST_INIT) != 0u, fin = (flags & DFLOW_FINAL) != 0u, ns = (flags & DFLOW_NO_STORE) != 0u;
+  const bool dead_src = (flags & DFLOW_DEAD_SRC) != 0u && !src_init && !src_fwd;
+  const unsigned long long v0 = vbeg + group_tid<NT>();
+  if (v0 >= vend) return;
+  auto batch = [&](auto K) {
+    constexpr int KK = decltype(K)::value;      // this thread's vectors in the tile: v0 + j NT, j < KK
+    uint4 b[KK];
+    if (!src_init && !src_fwd) {
+#pragma unroll
+      for (int j = 0; j < KK; ++j) carry[j] = ld16(s + (v0 + j * (unsigned long long)NT) * 16, pol.lds, pol.l1);
+    } else if (src_init) {
+#pragma unroll
+      for (int j = 0; j < KK; ++j) carry[j] = SC;
+    }
+    if (reduce && !dst_init) {
+#pragma unroll
+      for (int j = 0; j < KK; ++j) b[j] = ld16(d + (v0 + j * (unsigned long long)NT) * 16, pol.ldd, pol.l1);
+    } else {
+      const uint4 c = reduce ? DC : make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+      for (int j = 0; j < KK; ++j) b[j] = c;
+    }
+#pragma unroll
+    for (int j = 0; j < KK; ++j) {
+      const unsigned long long v = v0 + j * (unsigned long long)NT;
+      const uint4 a = carry[j];
+      const unsigned int cx = a.x & b[j].x, cy = a.y & b[j].y, cz = a.z & b[j].z, cw = a.w & b[j].w;   // elements whose sets overlap
+      if (EB == 2) {
+        auto hw = [](unsigned int w) { return ((w & 0xFFFFu) != 0u) + ((w >> 16) != 0u); };
+        overlaps += hw(cx) + hw(cy) + hw(cz) + hw(cw);
+      } else if (EB == 4) {
+        overlaps += (cx != 0u) + (cy != 0u) + (cz != 0u) + (cw != 0u);
+      } else if (EB == 8) {
+        overlaps += ((cx | cy) != 0u) + ((cz | cw) != 0u);
+      } else {
+        overlaps += ((cx | cy | cz | cw) != 0u);
+      }
+      const uint4 o = make_uint4(a.x | b[j].x, a.y | b[j].y, a.z | b[j].z, a.w | b[j].w);
+      carry[j] = o;
+      if (!ns) st16(d + v * 16, o, pol);
+      if (fin || (reduce && stage)) {
+        const uint4 df = make_uint4(o.x ^ F.x, o.y ^ F.y, o.z ^ F.z, o.w ^ F.w);
+        if ((df.x | df.y | df.z | df.w) != 0u) {
+          if (fin) report_bad_masks<EB>(&ctrl->bad, &ctrl->first_bad, df, g0 + v * (16 / EB));
+          if (reduce && stage) *all_full = false;
+        }
+      }
+      if (reduce && stage) sts16(stage + (v - vbeg) * 16, o);
+    }
+  };
+  if (v0 + (UNROLL - 1) * (unsigned long long)NT < vend) {
+    batch(std::integral_constant<int, UNROLL>());
+    // (only when every lane of the warp is in this round: the line's other vectors were loaded by this instruction)
+    if (dead_src && (v0 - (threadIdx.x & 31u) + 31) + (UNROLL - 1) * (unsigned long long)NT < vend) {
+#pragma unroll
+      for (int j = 0; j < UNROLL; ++j) discard_line16(s + (v0 + j * (unsigned long long)NT) * 16, v0 + j * (unsigned long long)NT, vend);
+    }
+  } else {
+    remainder_dispatch<UNROLL>((unsigned int)((vend - v0 + NT - 1) / NT), batch);
+  }
+}
+
 template <int UNROLL, int EB, int NT, class PolX>
 __device__ __forceinline__ void range_mask_lazy(const char* __restrict__ s, char* __restrict__ d,
                                                 unsigned long long vbeg, unsigned long long vend, unsigned int& overlaps,
                                                 const PolX& pol, unsigned int flags, bool reduce, uint4 SC, uint4 DC, uint4 F,
-                                                Ctrl* ctrl, unsigned long long g0) {
-  const bool src_init = (flags & DFLOW_SRC_INIT) != 0u;
+                                                Ctrl* ctrl, unsigned long long g0, char* stage = nullptr, bool* all_full = nullptr) {
+  const int sm = (flags & DFLOW_SRC_INIT) != 0u ? 1 : 0;
   const int dm = !reduce ? 0 : ((flags & DFLOW_DST_INIT) != 0u ? 2 : 1);
-  if (src_init) {
-    if (dm == 0) range_mask_lazy_t<UNROLL, EB, NT, true, 0>(s, d, vbeg, vend, overlaps, pol, flags, SC, DC, F, ctrl, g0);
-    else if (dm == 1) range_mask_lazy_t<UNROLL, EB, NT, true, 1>(s, d, vbeg, vend, overlaps, pol, flags, SC, DC, F, ctrl, g0);
-    else range_mask_lazy_t<UNROLL, EB, NT, true, 2>(s, d, vbeg, vend, overlaps, pol, flags, SC, DC, F, ctrl, g0);
+#define OPTCC_LAZY_CASE(SM, DM) \
+  range_mask_lazy_t<UNROLL, EB, NT, SM, DM>(s, d, vbeg, vend, overlaps, pol, flags, SC, DC, F, ctrl, g0, stage, all_full)
+  if (sm == 1) {
+    if (dm == 0) OPTCC_LAZY_CASE(1, 0); else if (dm == 1) OPTCC_LAZY_CASE(1, 1); else OPTCC_LAZY_CASE(1, 2);
   } else {
-    if (dm == 0) range_mask_lazy_t<UNROLL, EB, NT, false, 0>(s, d, vbeg, vend, overlaps, pol, flags, SC, DC, F, ctrl, g0);
-    else if (dm == 1) range_mask_lazy_t<UNROLL, EB, NT, false, 1>(s, d, vbeg, vend, overlaps, pol, flags, SC, DC, F, ctrl, g0);
-    else range_mask_lazy_t<UNROLL, EB, NT, false, 2>(s, d, vbeg, vend, overlaps, pol, flags, SC, DC, F, ctrl, g0);
+    if (dm == 0) OPTCC_LAZY_CASE(0, 0); else if (dm == 1) OPTCC_LAZY_CASE(0, 1); else OPTCC_LAZY_CASE(0, 2);
+  }
+#undef OPTCC_LAZY_CASE
+}
+
+// A staged tile that is NOT the full set (a wrong or truncated plan) and a copy flow that is the last writer of its
+// range: the tile is stored from the stage through the LSU, and every wrong element is reported as the lazy form does.
+template <int EB, int NT, class PolX>
+__device__ __forceinline__ void range_copy_stage_checked(const char* stage, char* __restrict__ d, unsigned long long vbeg,
+                                                         unsigned long long vend, const PolX& pol, uint4 F, Ctrl* ctrl,
+                                                         unsigned long long g0) {
+  for (unsigned long long v = vbeg + group_tid<NT>(); v < vend; v += NT) {
+    uint4 o;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(o.x), "=r"(o.y), "=r"(o.z), "=r"(o.w)
+                 : "r"((unsigned int)__cvta_generic_to_shared(stage + (v - vbeg) * 16)) : "memory");
+    st16(d + v * 16, o, pol);
+    const uint4 df = make_uint4(o.x ^ F.x, o.y ^ F.y, o.z ^ F.z, o.w ^ F.w);
+    if ((df.x | df.y | df.z | df.w) != 0u) report_bad_masks<EB>(&ctrl->bad, &ctrl->first_bad, df, g0 + v * (16 / EB));
   }
 }
 

@@ -137,6 +137,56 @@ void emit_step(const Geom& G, uint32_t t, Sink& out) {
     }
     return;
   }
+  if (G.construction == OPTCC_C1 && G.ordering == 3) {
+    // C1'': the four-pattern mix of :144-155 (PLAN_SPEC 4 C1'').  Segment b = 4 gamma + pattern; patterns A, C (0, 2) use
+    // ordering (1) S1 -> S2 -> S3 -> S4, patterns B, D (1, 3) ordering (2) S3 -> S1 -> S4 -> S2, one stage per body; A and
+    // B start in body 4 gamma, C and D one body later.  seg_at: the segment of `pattern` whose stage number `idx` (in
+    // its own ordering) falls into this body, or none.
+    const uint32_t beta = t / H, w = t % H, sg = G.stragglers[0];
+    const uint32_t a = w, d = (w + 1) % H;
+    auto seg_at = [&](uint32_t pattern, uint32_t idx, uint32_t* b) {
+      const uint32_t shift = (pattern >= 2 ? 1u : 0u) + idx;
+      if (beta < shift || (beta - shift) % 4 != 0) return false;
+      *b = beta - shift + pattern;
+      return *b < k;
+    };
+    uint32_t b;
+    // Stage 1: A, C in their first body, B, D in their second; ring link j idle in window j (ascending b = ascending offset)
+    for (uint32_t j = 0; j < H; ++j) {
+      if (w == j) continue;
+      const uint32_t hop = w < j ? w : w - 1, c = modH(int64_t(j) - hop, H);
+      for (uint32_t pat = 0; pat < 4; ++pat)
+        if (seg_at(pat, pat & 1u ? 1 : 0, &b))
+          out(t, OPTCC_OP_REDUCE, OPTCC_S1, OPTCC_LINK_NIC, 0, G.healthy[j], G.healthy[j + 1 == H ? 0 : j + 1], b, c, G.sec(0, b, c));
+    }
+    // Stage 2: A, C (second body) the straggler adds its own data to the uploaded partial sum (:130-132);
+    //          B, D (fourth body) the owner sends the global sum to the straggler (:138 ordering (2))
+    for (uint32_t pat = 0; pat < 4; ++pat)
+      if (seg_at(pat, pat & 1u ? 3 : 1, &b))
+        out(t, pat & 1u ? OPTCC_OP_COPY : OPTCC_OP_REDUCE, OPTCC_S2, OPTCC_LINK_NIC, 0, G.healthy[a], sg, b, (a + 1) % H, G.sec(0, b, (a + 1) % H));
+    // Stage 3: A, C (third body) the global sum returns to the uploader's ring successor (:132, R11);
+    //          B, D (first body) the straggler's raw section is folded in at its owner (:138)
+    for (uint32_t pat = 0; pat < 4; ++pat)
+      if (seg_at(pat, pat & 1u ? 0 : 2, &b)) {
+        if (pat & 1u) out(t, OPTCC_OP_REDUCE, OPTCC_S3, OPTCC_LINK_NIC, 0, sg, G.healthy[d], b, (d + 1) % H, G.sec(0, b, (d + 1) % H));
+        else out(t, OPTCC_OP_COPY, OPTCC_S3, OPTCC_LINK_NIC, 0, sg, G.healthy[d], b, d, G.sec(0, b, d));
+      }
+    // Stage 4: A, C in their fourth body (the all-gather of section c starts at healthy c), B, D in their third
+    for (uint32_t j = 0; j < H; ++j) {
+      if (w == j) continue;
+      const uint32_t hop = w < j ? w : w - 1;
+      for (uint32_t pat = 0; pat < 4; ++pat)
+        if (seg_at(pat, pat & 1u ? 2 : 3, &b)) {
+          const uint32_t c = pat & 1u ? modH(int64_t(j) + 1 - hop, H) : modH(int64_t(j) - hop, H);
+          out(t, OPTCC_OP_COPY, OPTCC_S4, OPTCC_LINK_NIC, 0, G.healthy[j], G.healthy[j + 1 == H ? 0 : j + 1], b, c, G.sec(0, b, c));
+        }
+    }
+    if (G.bubbles && beta < k)
+      out(t, OPTCC_OP_REDUCE, OPTCC_BUB_UP, OPTCC_LINK_NIC, 0, G.healthy[a], sg, beta, 0, G.p2p_reg[beta]);
+    if (G.bubbles && beta >= 1)
+      out(t, OPTCC_OP_COPY, OPTCC_BUB_DOWN, OPTCC_LINK_NIC, 0, sg, G.healthy[d], beta - 1, 0, G.p2p_reg[beta - 1]);
+    return;
+  }
   if (G.construction == OPTCC_C1 && G.ordering == 1) {
     // C1': ordering (1) of :138, S1 -> S2 -> S3 -> S4, one stage per body (PLAN_SPEC 4 C1')
     const uint32_t Bd = t / H, w = t % H, sg = G.stragglers[0];
@@ -308,8 +358,8 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
   if (g > 1 && stragglers.empty()) return OPTCC_EUNSUPPORTED;      // all-healthy g>1 is NCCL's multi-channel ring (:88)
   if (g > 255) return OPTCC_EUNSUPPORTED;                           // `part` is a byte
   const uint32_t ordering = (opts && opts->ordering) ? opts->ordering : 2;   // 0 = default = ordering (2)
-  if (ordering != 1 && ordering != 2) return OPTCC_EINVAL;                   // the two valid orderings of :138
-  if (ordering == 1 && !(g == 1 && stragglers.size() == 1 && schedule == OPTCC_SCHED_OPTCC)) return OPTCC_EUNSUPPORTED;
+  if (ordering != 1 && ordering != 2 && ordering != 3) return OPTCC_EINVAL;  // the two valid orderings of :138, or their mix (:144-155)
+  if (ordering != 2 && !(g == 1 && stragglers.size() == 1 && schedule == OPTCC_SCHED_OPTCC)) return OPTCC_EUNSUPPORTED;
   if (n == 0 || n > (uint64_t(1) << 40)) return OPTCC_EINVAL;
   if (dtype != OPTCC_F32 && dtype != OPTCC_BF16) return OPTCC_EINVAL;
   uint32_t k = opts ? opts->k : 0;
@@ -420,7 +470,9 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     std::sort(G.str_by_rank.begin(), G.str_by_rank.end(), [&](uint32_t a, uint32_t b) { return stragglers[a] < stragglers[b]; });
 
     // ---- PLAN_SPEC 4: constructions.  Step counts; the flows come from emit_step ----
-    if (construction == OPTCC_C1 && ordering == 1) {
+    if (construction == OPTCC_C1 && ordering == 3) {
+      G.P = H; G.n_steps = (k + 1) * H;
+    } else if (construction == OPTCC_C1 && ordering == 1) {
       G.P = H; G.n_steps = (k + 3) * H;
     } else if (construction == OPTCC_C0) {
       G.P = p; G.n_steps = 2 * (p - 1);
@@ -519,17 +571,20 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
     }
     if (pl->opts.tile_units) {
       pl->tile_units = pl->opts.tile_units;
+      pl->col_warp = pl->opts.exec_mode == OPTCC_EXEC_COLUMN && pl->tile_units <= 256;   // (small tiles: one warp each)
     } else if (pl->opts.exec_mode == OPTCC_EXEC_COLUMN) {
-      // column executor: a CTA runs a region's whole flow list on one tile, so the tile size does not depend on the
-      // number of steps.  One whole streaming round of the CTA (448 threads x 4 vectors = 1792 units for f32, x 2
-      // units = 896 for bf16 plans, whose fp32 shadow triples the bytes per unit): whole rounds are what the
-      // dead-source discard acts on (measured on a B200); a region shorter than that is one tile.
-      uint32_t tu = dtype == OPTCC_BF16 ? 896 : 1792;
+      // column executor: a tile is taken through its region's whole flow list, so the tile size does not depend on the
+      // number of steps.  CTA-wide tiles are one whole streaming round of the CTA (448 threads x 4 vectors = 1792
+      // units for f32, x 2 units = 896 for bf16 plans, whose fp32 shadow triples the bytes per unit): whole rounds are
+      // what the dead-source discard acts on.  Plans whose regions are shorter than two such tiles (C4: 1092 units at
+      // k = 8, 273 at k = 32; C3 at k = 20) take warp-wide tiles of 128 units instead -- a CTA-wide tile would leave
+      // most of the CTA idle -- (measured on a B200).
+      const uint32_t cta_tile = dtype == OPTCC_BF16 ? 896 : 1792;
       uint64_t longest = 0;
       for (size_t r = 0; r < nr; ++r) longest = std::max(longest, pl->region_len[r]);
       const uint64_t longest_units = ((longest + A - 1) / A + 7) & ~uint64_t(7);
-      if (longest_units && longest_units < tu) tu = (uint32_t)longest_units;
-      pl->tile_units = tu;
+      pl->col_warp = longest_units < 2 * uint64_t(cta_tile);
+      pl->tile_units = pl->col_warp ? 128 : cta_tile;
     } else {
       // auto: about two tile-ops per CTA and step (592 = 2 x 296 CTAs on a B200), from {224, 448, 896, 1792, 3584}
       // -- multiples / fractions of one streaming round of the dataflow kernel (448 threads x 4 vectors), so a tile is
@@ -549,6 +604,31 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
       pl->n_tile_ops += rt * pl->region_flows[r];
     }
     pl->tiles_per_rank = tiles;
+    // the verifier's tiles (column executor): about as many bytes of masks as a data tile has bytes of data -- a unit
+    // of A elements is A * mask_bytes >= 16 bytes of masks; CTA-wide unless the regions are shorter than one such tile
+    pl->mask_tile_units = pl->tile_units;
+    pl->mask_tiles_per_rank = tiles;
+    pl->mask_warp = pl->col_warp;
+    if (pl->opts.exec_mode == OPTCC_EXEC_COLUMN && in.mask_bytes) {
+      const uint64_t mb = A * in.mask_bytes;     // bytes of masks per unit
+      auto scaled = [&](uint64_t units) { return std::max<uint64_t>(8, (units * 16 / mb) & ~uint64_t(7)); };
+      uint64_t mtu;
+      if (pl->opts.tile_units) {
+        mtu = scaled(pl->tile_units);
+      } else {
+        const uint64_t cta_tile = scaled(dtype == OPTCC_BF16 ? 896 : 1792);
+        uint64_t longest = 0;
+        for (size_t r = 0; r < nr; ++r) longest = std::max(longest, pl->region_len[r]);
+        pl->mask_warp = (longest + A - 1) / A < cta_tile;
+        mtu = pl->mask_warp ? scaled(128) : cta_tile;
+      }
+      if (mtu != pl->tile_units) {
+        pl->mask_tile_units = (uint32_t)mtu;
+        uint64_t mt = 0;
+        for (size_t r = 0; r < nr; ++r) mt += ((pl->region_len[r] + A - 1) / A + mtu - 1) / mtu;
+        pl->mask_tiles_per_rank = mt;
+      }
+    }
   } catch (const std::bad_alloc&) {
     delete pl;
     return OPTCC_ENOMEM;

@@ -99,10 +99,10 @@ def test_ordering1_errors():
             B.optcc_plan(kw["p"], 1, kw["ell"], 1000, B.OPTCC_F32, ordering=1)
         assert el.value.name == code
     with pytest.raises(B.OptccError) as el:
-        B.optcc_plan(5, 1, _ell(5, 0, 2.0), 1000, B.OPTCC_F32, ordering=3)
+        B.optcc_plan(5, 1, _ell(5, 0, 2.0), 1000, B.OPTCC_F32, ordering=4)
     assert el.value.name == "EINVAL"
     with pytest.raises(OP.PlanError):
-        OP.build_plan(5, 1, _ell(5, 0, 2.0), 1000, OP.F32, ordering=3)
+        OP.build_plan(5, 1, _ell(5, 0, 2.0), 1000, OP.F32, ordering=4)
     assert B.optcc_plan_tables(B.optcc_plan(5, 1, _ell(5, 0, 2.0), 1000, B.OPTCC_F32, ordering=2))[0].tobytes() == \
         B.optcc_plan_tables(B.optcc_plan(5, 1, _ell(5, 0, 2.0), 1000, B.OPTCC_F32))[0].tobytes()
 
