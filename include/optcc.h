@@ -37,7 +37,8 @@ enum {
                              scope; p>128 for masks */
   OPTCC_ENOMEM = 3,
   OPTCC_ECUDA = 4,        /* a CUDA runtime call failed; optcc_last_cuda_error() has the code */
-  OPTCC_EVERIFY = 5       /* contributor-mask verification found a wrong element */
+  OPTCC_EVERIFY = 5,      /* contributor-mask verification found a wrong element */
+  OPTCC_ESTALE = 6        /* the workspace did not hold this plan's tables when a kernel ran (see optcc_workspace_check) */
 };
 
 /* PLAN_SPEC 3 enumerations */
@@ -245,6 +246,18 @@ OPTCC_API int optcc_execute_host(optcc_plan_t* plan, const void* const* host_in,
  * elements -- shard starts must stay 16-byte aligned), ECUDA. */
 OPTCC_API int optcc_execute_host_sharded(optcc_plan_t* plan, uint64_t n_total, const void* const* host_in,
                                void* const* host_out, void* const* bufs, void* workspace, void* stream);
+
+/* Workspace contract.  optcc_prepare (and the first optcc_execute / optcc_verify with a workspace) writes the plan's
+ * tables AND a stamp into the workspace; the library remembers per workspace address which plan's tables it holds, so
+ * later calls skip the upload.  If the caller reuses that memory for something else in between (or frees it and gets
+ * the same address back from its allocator) that memory no longer holds the tables: every kernel therefore compares
+ * the stamp with its own before touching a table, and a launch that finds another value does NOTHING except count
+ * itself.  optcc_workspace_check synchronises `stream` and returns OPTCC_ESTALE if any launch since the last
+ * optcc_prepare was such a no-op (the rank buffers are then unchanged) -- call optcc_prepare and run again;
+ * optcc_verify reports the same.  optcc_workspace_forget drops the library's memory of a workspace address (call it
+ * before freeing the workspace; optcc_plan_destroy forgets the workspaces of its plan). */
+OPTCC_API int optcc_workspace_check(optcc_plan_t* plan, void* workspace, void* stream);
+OPTCC_API void optcc_workspace_forget(void* workspace);
 
 /* ---- verification --------------------------------------------------------------------------------------------
  * Runs the SAME step tables through the executor with contributor bitmasks as elements (rank r starts as

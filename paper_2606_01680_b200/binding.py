@@ -15,11 +15,11 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "liboptcc.so")
 
 OPTCC_F32, OPTCC_BF16 = 0, 1
-OPTCC_OK, OPTCC_EINVAL, OPTCC_EUNSUPPORTED, OPTCC_ENOMEM, OPTCC_ECUDA, OPTCC_EVERIFY = range(6)
+OPTCC_OK, OPTCC_EINVAL, OPTCC_EUNSUPPORTED, OPTCC_ENOMEM, OPTCC_ECUDA, OPTCC_EVERIFY, OPTCC_ESTALE = range(7)
 OPTCC_EXEC_AUTO, OPTCC_EXEC_PERSISTENT, OPTCC_EXEC_PER_STEP, OPTCC_EXEC_DATAFLOW, OPTCC_EXEC_COLUMN = 0, 1, 2, 3, 4
 EXEC_NAMES = {0: "auto", 1: "persistent", 2: "per_step", 3: "dataflow", 4: "column"}
 OPTCC_SCHED_OPTCC, OPTCC_SCHED_RING_DEGRADED = 0, 1
-ERROR_NAMES = {1: "EINVAL", 2: "EUNSUPPORTED", 3: "ENOMEM", 4: "ECUDA", 5: "EVERIFY"}
+ERROR_NAMES = {1: "EINVAL", 2: "EUNSUPPORTED", 3: "ENOMEM", 4: "ECUDA", 5: "EVERIFY", 6: "ESTALE"}
 
 # optcc_flow_t (PLAN_SPEC 3): 40 bytes
 FLOW_DTYPE = np.dtype([
@@ -68,7 +68,8 @@ class OptccError(RuntimeError):
 
 _lib = None
 EXPORTS = ("optcc_plan", "optcc_plan_ex", "optcc_plan_destroy", "optcc_plan_info", "optcc_plan_tables", "optcc_cost",
-           "optcc_prepare", "optcc_column_tables", "optcc_execute", "optcc_execute_host", "optcc_execute_host_sharded", "optcc_verify", "optcc_strerror",
+           "optcc_prepare", "optcc_column_tables", "optcc_execute", "optcc_execute_host", "optcc_execute_host_sharded", "optcc_workspace_check", "optcc_workspace_forget",
+           "optcc_verify", "optcc_strerror",
            "optcc_last_cuda_error", "optcc_abi_version")
 
 
@@ -95,12 +96,15 @@ def load():
     lib.optcc_execute_host.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), vp, vp]
     lib.optcc_execute_host_sharded.argtypes = [vp, u64, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), vp, vp]
     lib.optcc_verify.argtypes = [vp, vp, vp, C.POINTER(optcc_verify_result_t)]
+    lib.optcc_workspace_check.argtypes = [vp, vp, vp]
+    lib.optcc_workspace_forget.argtypes = [vp]
+    lib.optcc_workspace_forget.restype = None
     lib.optcc_strerror.argtypes = [C.c_int]
     lib.optcc_strerror.restype = C.c_char_p
     lib.optcc_last_cuda_error.argtypes = []
     lib.optcc_abi_version.argtypes = []
     for name in EXPORTS:
-        if name not in ("optcc_plan_destroy", "optcc_strerror"):
+        if name not in ("optcc_plan_destroy", "optcc_strerror", "optcc_workspace_forget"):
             getattr(lib, name).restype = C.c_int
     _lib = lib
     return lib
@@ -240,6 +244,17 @@ def optcc_execute_host_sharded(plan, n_total, host_in, host_out, bufs, workspace
                                            _ptr_array(bufs), _ptr(workspace), _ptr(stream))
     if rc:
         raise OptccError(rc, "optcc_execute_host_sharded")
+
+
+def optcc_workspace_check(plan, workspace, stream=None):
+    """Synchronises `stream`; raises OptccError (ESTALE) if a launch did not find this plan's tables in the workspace."""
+    rc = load().optcc_workspace_check(plan.handle, _ptr(workspace), _ptr(stream))
+    if rc:
+        raise OptccError(rc, "optcc_workspace_check")
+
+
+def optcc_workspace_forget(workspace):
+    load().optcc_workspace_forget(_ptr(workspace))
 
 
 def optcc_verify(plan, workspace, stream=None, raise_on_fail=True):

@@ -47,8 +47,9 @@ extern "C" int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* p
       dur = alpha + beta * double(f.len) / double(g - 1);
     double& sf = send_free[size_t(f.src) * 2 + f.link];
     double& rf = recv_free[size_t(f.dst) * 2 + f.link];
-    RangeTimes& S = rt[size_t(f.src) * nr + reg];
-    RangeTimes& D = rt[size_t(f.dst) * nr + reg];
+    // (region-major: the regions of a few segments are active at a time, so their p entries stay in the cache)
+    RangeTimes& S = rt[reg * p + f.src];
+    RangeTimes& D = rt[reg * p + f.dst];
     double& ws = S.wfin;
     double& wd = D.wfin;
     double& rd = D.rfin;

@@ -192,6 +192,7 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
 // The executor kernel.  gridDim.x CTAs; CTA c executes slice c of every step in [step_lo, step_hi).
 template <int MODE>
 __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) optcc_exec_kernel(const __grid_constant__ ExecParams P) {
+  if (tables_are_stale(P)) return;
   __shared__ DFlow s_flow[2][STAGE];             // the CTA's part of the step table, staged one step ahead
   __shared__ unsigned long long s_ubeg[2], s_uend[2];
   __shared__ unsigned int s_f0[2], s_nf[2];
@@ -387,6 +388,7 @@ __device__ __forceinline__ void red_release_cta_shared_add(unsigned int* p, unsi
 
 template <int MODE>
 __global__ void __launch_bounds__(DF_THREADS, CTAS_PER_SM) optcc_dataflow_kernel(const __grid_constant__ ExecParams P) {
+  if (tables_are_stale(P)) return;
   constexpr unsigned int NW = DF_COMPUTE_THREADS / 32;   // streaming warps
   const unsigned int NS = P.df_slots;                    // slots in the ring = scheduler agents in use (<= DF_SLOTS)
   __shared__ DfSlot s_slot[DF_SLOTS];
@@ -553,6 +555,7 @@ constexpr unsigned int COL_PF_MAX = 8;  // deepest look-ahead (flows)
 
 template <int MODE, bool MASK_FWD = false>
 __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(const __grid_constant__ ExecParams P) {
+  if (tables_are_stale(P)) return;
   __shared__ unsigned long long s_item[2];          // work items are claimed one item ahead
   __shared__ __align__(16) DFlow s_rec[COL_REC];    // this CTA's staged part of the region's flow list
   __shared__ __align__(16) DFlow s_nrec[COL_PF_MAX];   // the first records of the next item (look-ahead across items)
@@ -708,6 +711,7 @@ __device__ __forceinline__ DFlow load_record(const DFlow* p) {
 
 template <int MODE, bool MASK_FWD = false>
 __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel(const __grid_constant__ ExecParams P) {
+  if (tables_are_stale(P)) return;
   extern __shared__ __align__(128) char s_stage_w[];   // bulk all-gather path: one tile per warp
   const unsigned int lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
   char* const stage = s_stage_w + (size_t)warp * P.col_stage_bytes;
@@ -859,6 +863,7 @@ struct optcc_exec_state {
   int coop = 0;
   uint32_t G = 0;                 // executor grid (CTAs)
   uint64_t id = 0;                // process-unique id of this plan's device tables (see g_ws_owner)
+  unsigned long long stamp_host = 0;   // table_stamp(id), the value upload_tables writes into the control block
   std::vector<DFlow> dflows;
   std::vector<Slice> slices;      // [n_steps][G + 1]
   // dataflow executor
@@ -879,7 +884,17 @@ struct optcc_exec_state {
   std::vector<uint4> col_items_mask;     // the verifier's items when its tile size differs (plan's mask_tile_units)
 };
 
-void optcc_exec_state_free(optcc_exec_state* s) { delete s; }
+// The stamp a workspace carries while it holds the tables of state `id`: kernels compare it with their launch parameter.
+static inline unsigned long long table_stamp(uint64_t id) { return 0x4F50544343000000ull ^ (id * 0x9E3779B97F4A7C15ull); }
+
+void optcc_exec_state_free(optcc_exec_state* s) {
+  if (s) {   // the workspaces that held this plan's tables no longer count as prepared
+    std::lock_guard<std::mutex> lock(g_ws_mutex);
+    for (auto it = g_ws_owner.begin(); it != g_ws_owner.end();)
+      it = it->second == s->id ? g_ws_owner.erase(it) : std::next(it);
+  }
+  delete s;
+}
 
 namespace {
 
@@ -1257,17 +1272,17 @@ void build_column_state(optcc_plan_t* pl, optcc_exec_state* st, bool* all_covere
     st->col_reg_begin.assign(nr + 1, 0);
     for (size_t r = 0; r < nr; ++r) st->col_reg_begin[r + 1] = st->col_reg_begin[r] + pl->region_flows[r];
     st->col_dflows.resize_uninit(nf);
-    // gather the representatives' lists (table order) straight into their place in col_dflows
-    std::vector<uint32_t> fill(nr, UINT32_MAX);            // next free position of a representative's list
-    uint64_t wanted = 0;
+    // gather the lists (table order) of every class's first region -- and of its last one, which is compared with the
+    // first before anything is replicated -- straight into their place in col_dflows
+    std::vector<uint32_t> fill(nr, UINT32_MAX);            // next free position of a gathered list
     for (size_t c = 0; c < ncls; ++c)
       if (cls_begin[c] < cls_begin[c + 1]) {
-        const uint32_t r = cls_regions[cls_begin[c]];
-        fill[r] = st->col_reg_begin[r];
-        wanted += pl->region_flows[r];
+        const uint32_t r0 = cls_regions[cls_begin[c]], r1 = cls_regions[cls_begin[c + 1] - 1];
+        fill[r0] = st->col_reg_begin[r0];
+        fill[r1] = st->col_reg_begin[r1];
       }
     const uint32_t* reg = pl->flow_region.data();
-    for (uint32_t i = 0; i < nf && wanted; ++i) {          // (the first segment's flows sit in the first few bodies)
+    for (uint32_t i = 0; i < nf; ++i) {
       uint32_t& pos = fill[reg[i]];
       if (pos == UINT32_MAX) continue;
       const optcc_flow_t& f = pl->flows[i];
@@ -1275,8 +1290,16 @@ void build_column_state(optcc_plan_t* pl, optcc_exec_state* st, bool* all_covere
       d.off = f.off; d.len = f.len; d.src = f.src; d.dst = f.dst; d.op = f.op;
       d.ksrc = d.kdin = d.kdout = 0; d.flags = 0; d.pad1 = 0;
       st->col_dflows[pos++] = d;
-      --wanted;
     }
+    for (size_t c = 0; c < ncls && fast; ++c) {
+      if (cls_begin[c] == cls_begin[c + 1]) continue;
+      const uint32_t r0 = cls_regions[cls_begin[c]], r1 = cls_regions[cls_begin[c + 1] - 1];
+      const DFlow* a = st->col_dflows.data() + st->col_reg_begin[r0];
+      const DFlow* b = st->col_dflows.data() + st->col_reg_begin[r1];
+      for (uint32_t j = 0; j < pl->region_flows[r0] && fast; ++j) fast = flow_key(a[j]) == flow_key(b[j]);
+    }
+  }
+  if (fast) {
     TT("gather");
     optcc_parallel_chunks(ncls, nf, [&](size_t c) {
       if (cls_begin[c] == cls_begin[c + 1]) return;
@@ -1533,6 +1556,8 @@ int upload_tables(optcc_plan_t* pl, void* workspace, cudaStream_t stream, bool f
   const optcc_ws_layout L = optcc_layout(pl);
   char* ws = static_cast<char*>(workspace);
   CU_TRY(cudaMemsetAsync(ws + L.ctrl, 0, OPTCC_CTRL_BYTES, stream));
+  st->stamp_host = table_stamp(st->id);       // (a member: the copy below reads it when the stream gets there)
+  CU_TRY(cudaMemcpyAsync(ws + L.ctrl + offsetof(Ctrl, stamp), &st->stamp_host, sizeof(unsigned long long), cudaMemcpyHostToDevice, stream));
   if (st->column) {
     if (!st->col_dflows.empty())
       CU_TRY(cudaMemcpyAsync(ws + L.dflows, st->col_dflows.data(), st->col_dflows.size() * sizeof(DFlow), cudaMemcpyHostToDevice, stream));
@@ -1662,6 +1687,7 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   // fetch / completion latency; copying agents hold their slots, so the bulk path also uses 4
   P.df_slots = (pl->exec && pl->exec->big_ops && !P.bulk_copy) ? 2 : 4;
   if (pl->opts.exec_mode == OPTCC_EXEC_COLUMN) P.l2_hints = 0;   // see optcc_column_kernel
+  P.stamp = pl->exec ? table_stamp(pl->exec->id) : 0;
   P.col_pf_dist = 1; P.col_pf_l2 = 0; P.col_pf_next = 0; P.col_bulk = 1;
   P.col_bulk_policy = 1;   // bulk stores evict_first: the all-gather's results are never read again (measured: C2 1.68 -> 1.62 ms)
   P.col_warp = pl->col_warp;
@@ -1838,7 +1864,8 @@ extern "C" int optcc_verify(optcc_plan_t* plan, void* workspace, void* stream_, 
   Ctrl init;
   std::memset(&init, 0, sizeof init);
   init.first_bad = ~0ull;
-  CU_TRY(cudaMemcpyAsync(P.ctrl, &init, sizeof init, cudaMemcpyHostToDevice, stream));
+  // (counters only: the stamp and the stale count written with the tables stay as they are)
+  CU_TRY(cudaMemcpyAsync(P.ctrl, &init, offsetof(Ctrl, stamp), cudaMemcpyHostToDevice, stream));
   const uint64_t vec_per_rank = in.padded_n * eb / 16;
   const unsigned int bx = (unsigned int)std::max<uint64_t>(1, std::min<uint64_t>((vec_per_rank + 1023) / 1024,
                                                           std::max<uint64_t>(1, uint64_t(plan->exec->sm_count) * 16 / in.p)));
@@ -1870,6 +1897,21 @@ extern "C" int optcc_verify(optcc_plan_t* plan, void* workspace, void* stream_, 
   r.overlap_elements = res.overlap;
   r.first_bad = res.first_bad;
   r.checked = uint64_t(in.p) * in.n;
+  if (res.stale || res.stamp != P.stamp) return OPTCC_ESTALE;   // some launch did not find this plan's tables: nothing was verified
   *out = r;
   return (r.bad_elements || r.overlap_elements) ? OPTCC_EVERIFY : OPTCC_OK;
+}
+
+extern "C" int optcc_workspace_check(optcc_plan_t* plan, void* workspace, void* stream_) {
+  if (!plan || !workspace || !plan->exec) return OPTCC_EINVAL;
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  Ctrl res;
+  CU_TRY(cudaMemcpyAsync(&res, static_cast<char*>(workspace) + optcc_layout(plan).ctrl, sizeof res, cudaMemcpyDeviceToHost, stream));
+  CU_TRY(cudaStreamSynchronize(stream));
+  return (res.stale || res.stamp != table_stamp(plan->exec->id)) ? OPTCC_ESTALE : OPTCC_OK;
+}
+
+extern "C" void optcc_workspace_forget(void* workspace) {
+  std::lock_guard<std::mutex> lock(g_ws_mutex);
+  g_ws_owner.erase(workspace);
 }

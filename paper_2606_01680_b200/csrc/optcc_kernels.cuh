@@ -83,6 +83,8 @@ struct Ctrl {                     // control block at the start of the workspace
   unsigned long long overlap;     // verify: reduce over overlapping contributor sets
   unsigned long long first_bad;   // verify: smallest bad r*n+e
   unsigned long long ticket;      // dataflow: next tile-op to claim
+  unsigned long long stamp;       // which plan's tables the workspace holds (written with the tables; see ExecParams.stamp)
+  unsigned long long stale;       // launches that found another stamp than theirs and did nothing
 };
 
 struct ExecParams {
@@ -120,7 +122,10 @@ struct ExecParams {
   unsigned int col_warp;          // 1: warp-wide tiles (optcc_wcolumn_kernel), 0: CTA-wide tiles (optcc_column_kernel)
   unsigned int col_stage_bytes;   // bytes of one staged tile (the warp-wide kernel keeps one per warp)
   unsigned int mask_fwd;          // lazy contributor-mask runs: act on DFLOW_SRC_FWD / DFLOW_NO_STORE
-  unsigned int pad4[3];
+  unsigned int pad4;
+  unsigned long long stamp;       // the launching plan's table stamp: a kernel whose workspace holds another one (the
+                                  // memory was reused, or freed and allocated again at the same address) must not walk
+                                  // the tables it finds there -- it counts itself in Ctrl.stale and returns
 };
 
 // ---- memory access helpers: L2-only loads (data written by other SMs in the previous step), streaming stores ----
@@ -182,6 +187,13 @@ __device__ __forceinline__ uint4 add_f32x4(uint4 a, uint4 b) {
   r.z = __float_as_uint(__fadd_rn(__uint_as_float(a.z), __uint_as_float(b.z)));
   r.w = __float_as_uint(__fadd_rn(__uint_as_float(a.w), __uint_as_float(b.w)));
   return r;
+}
+
+// every thread of every kernel starts with this (all threads of the grid take the same branch)
+__device__ __forceinline__ bool tables_are_stale(const ExecParams& P) {
+  if (__ldcg(&P.ctrl->stamp) == P.stamp) return false;
+  if (threadIdx.x == 0 && blockIdx.x == 0) atomicAdd(&P.ctrl->stale, 1ull);
+  return true;
 }
 
 // ---- grid-wide barrier: every CTA arrives once per step; counter is monotone, target = arrivals expected so far ----

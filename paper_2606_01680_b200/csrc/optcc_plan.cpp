@@ -449,8 +449,12 @@ extern "C" int optcc_plan_ex(int p, int g, const double* ell, uint64_t n, int dt
         reg_of[i] = (uint32_t)pl->region_offs.size();
         pl->region_offs.push_back(bounds[i]);
         pl->region_len.push_back(bounds[i + 1] - bounds[i]);
-        // interval i of sec_bounds is (part, segment, section) = (i / (k nsec), (i / nsec) mod k, i mod nsec)
-        pl->region_class.push_back(sections ? uint32_t(i / (size_t(k) * nsec)) * nsec + uint32_t(i % nsec) : nparts * nsec);
+        // interval i of sec_bounds is (part, segment, section) = (i / (k nsec), (i / nsec) mod k, i mod nsec).  Class =
+        // (part, pattern, section): the segments of the four-pattern mix repeat with period 4, all others with period 1.
+        const uint32_t period = ordering == 3 ? 4 : 1;
+        const uint32_t seg = uint32_t((i / nsec) % k);
+        pl->region_class.push_back(sections ? (uint32_t(i / (size_t(k) * nsec)) * period + seg % period) * nsec + uint32_t(i % nsec)
+                                            : nparts * period * nsec);
       }
     };
     add_regions(pl->sec_bounds, G.sec_reg, true);
@@ -705,6 +709,7 @@ extern "C" const char* optcc_strerror(int code) {
     case OPTCC_ENOMEM: return "out of host memory";
     case OPTCC_ECUDA: return "CUDA runtime error (see optcc_last_cuda_error)";
     case OPTCC_EVERIFY: return "contributor-mask verification failed";
+    case OPTCC_ESTALE: return "the workspace did not hold this plan's tables when a kernel ran: call optcc_prepare and run again";
     default: return "unknown optcc error";
   }
 }

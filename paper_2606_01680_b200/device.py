@@ -95,6 +95,16 @@ class Session:
             B.optcc_execute_host_sharded(self.plan, self.n * self.shards, host_in, host_out, self.bufs, self.ws_ptr,
                                          self._stream(stream))
 
+    def check(self, stream=None):
+        with torch.cuda.device(self.device):
+            B.optcc_workspace_check(self.plan, self.ws_ptr, self._stream(stream))
+
+    def __del__(self):
+        try:
+            B.optcc_workspace_forget(self.ws_ptr)     # the address may come back from the allocator for something else
+        except Exception:
+            pass
+
     def verify(self, stream=None, raise_on_fail=True):
         with torch.cuda.device(self.device):
             return B.optcc_verify(self.plan, self.ws_ptr, self._stream(stream), raise_on_fail=raise_on_fail)

@@ -111,8 +111,6 @@ def test_column_tables_reproduce_the_oracle(case):
     ell = [float(st.get(i, 1.0)) for i in range(p)]
     plan = B.optcc_plan(p, g, ell, n, dtype, k=k, exec_mode=B.OPTCC_EXEC_COLUMN, **extra)
     okw = {key: extra[key] for key in ("ordering", "schedule") if key in extra}
-    if okw.get("ordering") == 3:
-        pass
     oplan = OP.build_plan(p, g, ell, n, dtype, k=k, **okw)
     x = W.all_inputs(W.Workload("t", p, g, tuple(ell), n, dtype, "normal", 1.0, 300 + case))
     y, items, lists = _simulate(plan, x, bulk=extra.get("copy_path", 0) != 1)
@@ -139,7 +137,7 @@ def test_column_tables_reproduce_the_oracle(case):
         assert [t for t, _ in tiles] == list(range(len(tiles))) and sum(u for _, u in tiles) == units
 
 
-@pytest.mark.parametrize("case", [1, 2, 5, 6, 11])
+@pytest.mark.parametrize("case", [1, 2, 5, 6, 10, 13])
 @pytest.mark.parametrize("frac", [0.3, 0.7])
 def test_column_tables_of_a_truncated_schedule(case, frac):
     """step_limit: the lists hold the flows of the executed steps only (general path, no class replication) and
@@ -147,7 +145,7 @@ def test_column_tables_of_a_truncated_schedule(case, frac):
     import dataclasses
     p, g, st, n, dtype, k, extra = CASES[case]
     ell = [float(st.get(i, 1.0)) for i in range(p)]
-    oplan = OP.build_plan(p, g, ell, n, dtype, k=k)
+    oplan = OP.build_plan(p, g, ell, n, dtype, k=k, **{key: extra[key] for key in ("ordering", "schedule") if key in extra})
     limit = max(1, int(oplan.n_steps * frac))
     plan = B.optcc_plan(p, g, ell, n, dtype, k=k, exec_mode=B.OPTCC_EXEC_COLUMN, step_limit=limit, **extra)
     x = W.all_inputs(W.Workload("t", p, g, tuple(ell), n, dtype, "normal", 1.0, 500 + case))

@@ -539,3 +539,35 @@ def test_truncated_schedule_data_at_c2_full_size(exec_mode):
     y_or = OI.run_f32_at(_oracle_prefix(oplan, limit), np.ascontiguousarray(x[:, idx]), idx)
     assert ys.tobytes() == y_or.tobytes()
     assert not np.array_equal(ys[0], ys[1])      # (the cut really is mid-schedule: the ranks still differ)
+
+
+@pytest.mark.parametrize("exec_mode", MODES)
+def test_a_clobbered_workspace_is_detected_not_executed(exec_mode):
+    """optcc.h "Workspace contract": the library remembers which plan's tables a workspace holds.  If the caller reuses
+    that memory in between, a later launch must not walk whatever it finds there: every kernel compares the stamp
+    written with the tables and does nothing when it differs; optcc_workspace_check / optcc_verify report ESTALE, and
+    after optcc_prepare everything works again."""
+    import torch
+    w = _wl(8, 1, {3: 1.5}, 300007, W.F32, seed=31)
+    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=4, exec_mode=exec_mode)
+    oplan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=4)
+    x = W.all_inputs(w)
+    s = _session(plan, verify=True)
+    s.upload(x)
+    s.prepare()
+    torch.cuda.synchronize()
+    s.workspace.random_(0, 255)             # the caller used the memory for something else
+    s.execute()                             # (the library still believes the tables are there: no re-upload)
+    torch.cuda.synchronize()
+    assert s.download().tobytes() == x.tobytes()          # nothing was executed
+    with pytest.raises(B.OptccError) as e:
+        s.check()
+    assert e.value.name == "ESTALE"
+    with pytest.raises(B.OptccError) as e:
+        s.verify()
+    assert e.value.name == "ESTALE"
+    s.prepare()                             # tables and stamp written again
+    s.execute()
+    s.check()
+    assert s.download().tobytes() == OI.run_f32(oplan, x).tobytes()
+    assert s.verify()["bad_elements"] == 0
