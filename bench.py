@@ -1,20 +1,29 @@
 #!/usr/bin/env python
-"""bench.py -- OPTCC-schedule AllReduce on B200: algbw GB/s, schedule bytes vs the HBM roofline, modeled T/T0.
+"""bench.py -- OPTCC-schedule AllReduce on B200: algbw GB/s, the executor against its HBM roofline, modeled T/T0.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--k 0] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--k -1] [--exec-mode 0] [--impl reference]
 
-One "step" = one pass of the whole hot path over one batch of seeded synthetic input:
-optcc_plan (classify, bandwidth-weighted chunking, flow/step tables) -> optcc_cost (alpha-beta model) ->
-optcc_execute (reduce + copy steps with step barriers) -> optcc_verify (contributor masks), all through the C-ABI.
-`value` = n*sizeof(dtype) / step time (algorithm bandwidth, BASELINE.json metric) summed over ranks; the
-`execute_only` object gives the same metric for the AllReduce proper (optcc_execute alone), and `roofline` is the
-executor kernel's schedule bytes (5 (p-1) n sizeof) over its measured duration against the measured
-HBM copy peak.  Inputs are restored from a pristine device copy between steps, outside the timed events (the
-AllReduce is in place); that restore also flushes L2 (footprint >> 126 MB).
+One "step" = one pass of the whole hot path over one batch of seeded synthetic input,
+all through the C ABI: optcc_plan (classify, bandwidth-weighted chunking, flow / step tables), then optcc_cost (the
+alpha-beta model, on a second host thread) beside optcc_prepare + optcc_execute (reduce and copy steps) +
+optcc_verify (contributor masks).  `value` = n*sizeof(dtype) / step time (algorithm bandwidth, BASELINE.json's
+metric) summed over ranks; `execute_only` gives the same metric for the AllReduce proper (optcc_execute alone).
+The executor and k are the library's and the model's: exec_mode 0 = OPTCC_EXEC_AUTO (what a user of optcc_plan
+gets), k = the k at which the modelled T/T0 is within the paper's reported gap (BENCH_K).
+
+`roofline.frac` is an HBM fraction: for the column / dataflow executors the compulsory DRAM bytes 2 p n sizeof
+(inputs read once, outputs written once) over the kernel's CUDA-event time against the measured copy peak -- their
+partial sums live in L1 / L2, so the schedule's 5 (p-1) n sizeof bytes never reach HBM (`schedule_over_peak` keeps
+that ratio); `roofline_stepwise` times the step-ordered persistent executor on the same workload in the same run and
+reports SURVEY 8(d)'s literal number, schedule bytes / time.  `other_configs` carries C1, C3, C4 and the whole C5
+sweep (execute ms, verify ms, both fractions, k, modelled T/T0, a parity spot check each).
+Inputs are restored from a pristine device copy between steps, outside the timed events (the AllReduce is in place);
+that restore also flushes L2 (footprint >> 126 MB).
 
 --impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
-Multi-GPU (torchrun): every rank runs the same workload on its own GPU -- the path shards along the element axis
-with no data-path collective; scaling is "weak".
+--gpus N: N independent replicas, one per GPU -- the path shards along the element axis with no data-path collective
+(SURVEY 8(e)); under torchrun each rank is one replica, without it bench.py starts the N workers itself; NCCL is used
+for the barrier and the max over ranks of the device times only; scaling is "weak".
 """
 import argparse
 import json
@@ -41,7 +50,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1 = C2, the metric's config)")
     ap.add_argument("--ell", type=float, default=1.6, help="ell for config 4 (the C5 sweep)")
     ap.add_argument("--k", type=int, default=-1,
-                    help="segments (PAPER.md:124); -1 = bench default per config (16 for C2, see profiles/ k-sweep), 0 = planner's auto rule")
+                    help="segments (PAPER.md:124); -1 = bench default per config (BENCH_K: the modelled-gap k), 0 = planner's auto rule")
     ap.add_argument("--exec-mode", type=int, default=0,
                     help="OPTCC_EXEC_*: 0 = auto (the library chooses from the plan's shape; what a user of optcc_plan gets), "
                          "1 persistent kernel with grid barriers, 2 one launch per step, 3 dataflow kernel, 4 column kernel")
@@ -54,11 +63,15 @@ def parse_args():
     ap.add_argument("--cpu-sample-log2", type=int, default=0,
                     help="log2 of n per rank for the CPU-oracle sample (0 = 24 for the cpu_baseline leg, 22 per --impl reference step)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--only-main", action="store_true", help="skip roofline_stepwise and other_configs (profiling runs)")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
 
 
-BENCH_K = {0: 8, 1: 16, 2: 8, 3: 8, 4: 8}   # per config; k is free in BASELINE.json's configs
+# k per config: free in BASELINE.json's configs; the k at which the modelled T/T0 is within the paper's
+# reported gap (<= 1.06 single straggler, <= 1.085 multi-straggler, <= 1.06 multi-GPU) -- the column
+# executor's time does not depend on k, so the timed k is the modelled-gap k
+BENCH_K = {0: 20, 1: 16, 2: 20, 3: 32, 4: 24}
 
 
 EXEC_KERNEL = {1: "optcc_exec_kernel", 2: "optcc_exec_kernel", 3: "optcc_dataflow_kernel", 4: "optcc_column_kernel"}
@@ -194,139 +207,231 @@ def measured_peak():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
         try:
-            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, device copy)"
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, device copy, burst: the kernel is timed alone)"
         except Exception:
             pass
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
 def ncu_traffic(workload, kernel):
-    """dram bytes per launch of `kernel` from the committed ncu --set full capture, or None."""
+    """(dram bytes per launch, commit the capture was taken at, source) of `kernel` from the committed ncu --set full
+    captures (profiles/exec_kernel_traffic.csv), or (None, None, None).  ncu cannot run inside the bench: the line says
+    which commit the byte count belongs to."""
     path = os.path.join(ROOT, "profiles", "exec_kernel_traffic.csv")
     if not os.path.exists(path):
-        return None
+        return None, None, None
     for line in open(path):
+        if line.startswith("#"):
+            continue
         parts = [s.strip() for s in line.split(",")]
-        if len(parts) >= 3 and parts[0] == workload and parts[1] == kernel:
+        if len(parts) >= 5 and parts[0] == workload and parts[1] == kernel:
             try:
-                return float(parts[2])
+                return float(parts[2]), parts[3], parts[4]
             except ValueError:
-                return None
-    return None
+                return None, None, None
+    return None, None, None
+
+
+EXEC_NAME = {1: "persistent cooperative kernel, grid barrier per step", 2: "one launch per step",
+             3: "dataflow cooperative kernel: tile-ops in table order, per-range completion counters, no grid barrier",
+             4: "column kernel: a tile is taken through its region's whole flow list in dependency order, no "
+                "synchronisation between CTAs (every dependency lies inside one element column)"}
+
+
+def roofline_of(kernel, exec_mode, p, n, esize, t_ms, peak, peak_src):
+    """HBM roofline of one executor launch.  Step-ordered executors (persistent, per-step): SURVEY 8(d)'s schedule
+    bytes 5 (p-1) n sizeof -- every flow's operands travel through HBM / L2 in global step order.  Column and dataflow
+    executors: the partial sums of a tile stay in L1 / L2, so what HBM must carry is the compulsory 2 p n sizeof
+    (every input read once, every output written once); the schedule-bytes ratio is kept beside it."""
+    sched = 5 * (p - 1) * n * esize
+    comp = 2 * p * n * esize
+    stepwise = exec_mode in (1, 2)
+    nbytes = sched if stepwise else comp
+    return {"bound": "hbm", "kernel": kernel, "achieved": nbytes / t_ms / 1e6, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
+            "frac": nbytes / t_ms / 1e6 / peak,
+            "definition": ("schedule bytes 5 (p-1) n sizeof / kernel time (SURVEY 8(d)): this executor keeps global step order, "
+                           "every flow's operands go through HBM / L2") if stepwise else
+                          ("compulsory DRAM bytes 2 p n sizeof (every input read once, every output written once) / kernel time: "
+                           "this executor takes a tile through its whole flow list inside L1 / L2 and drops dead partial sums from "
+                           "the caches, so the schedule's 5 (p-1) n sizeof bytes never reach HBM (see schedule_over_peak)"),
+            "algorithmic_bytes_per_launch": nbytes, "schedule_bytes_per_launch": sched,
+            "schedule_over_peak": sched / t_ms / 1e6 / peak, "ms": t_ms}
+
+
+class Bench:
+    """Device state shared by the measurements of one bench run."""
+
+    def __init__(self, args):
+        import torch
+        from paper_2606_01680_b200 import binding as B, workloads as W
+        from paper_2606_01680_b200 import build as optcc_build
+        from paper_2606_01680_b200.device import Session
+        from paper_2606_01680_b200.replicas import Replicas
+        self.torch, self.B, self.W, self.Session = torch, B, W, Session
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device: liboptcc has no CPU fallback (use --impl reference for the oracle)")
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        torch.cuda.set_device(self.local)
+        self.dev = torch.device("cuda", self.local)
+        self.rep = Replicas(backend="nccl", device=self.dev)
+        if self.rep.rank == 0:
+            optcc_build.build()
+        self.rep.barrier()
+        B.load()
+        self.stream = torch.cuda.current_stream(self.dev)
+        self.args = args
+        self.peak, self.peak_src = measured_peak()
+
+    def ev(self):
+        return self.torch.cuda.Event(enable_timing=True)
+
+    def measure(self, w, k, steps, warmup, x=None, sampler=None, keep=False, exec_mode=None, execute_only=False):
+        """`steps` timed passes of the whole hot path on workload w (inputs resident in HBM, restored from a pristine
+        device copy between passes, untimed: the AllReduce is in place and the restore flushes L2).  One pass =
+        optcc_plan -> {optcc_cost on a second host thread} || {optcc_prepare, optcc_execute, optcc_verify} -> join."""
+        torch, B, W, args = self.torch, self.B, self.W, self.args
+        import numpy as np
+        esize = w.elem_bytes
+        mode = args.exec_mode if exec_mode is None else exec_mode
+        mk = lambda: B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=k, exec_mode=mode, tile_units=args.tile_units,
+                                  col_order=args.col_order)
+        plan0 = mk()
+        info = plan0.info
+        cost0 = B.optcc_cost(plan0)
+        sess = self.Session(plan0, device=self.dev, verify=not execute_only)
+        if x is None:
+            x = W.all_inputs(w)
+        sess.upload(x)
+        pristine = [b.clone() for b in sess.bufs]
+        restore = lambda: [b.copy_(s) for b, s in zip(sess.bufs, pristine)]
+        stream = self.stream
+
+        def one_pass():
+            e = [self.ev() for _ in range(5)]
+            box = {}
+            e[0].record(stream)
+            t0 = time.perf_counter()
+            plan = mk()                                   # a1-a3: classify, chunk, flow / step tables
+            t1 = time.perf_counter()
+
+            def cost():                                   # a4 on a second host thread (ctypes releases the GIL)
+                tc = time.perf_counter()
+                box["cost"] = B.optcc_cost(plan)
+                box["cost_ms"] = (time.perf_counter() - tc) * 1e3
+            th = threading.Thread(target=cost)
+            if not execute_only:
+                th.start()
+            sess.plan = plan
+            sess.prepare()                                # the executor's tables, built on the host and uploaded
+            stream.synchronize()                          # (the upload belongs to plan_to_launch, not to the executor's time)
+            e[1].record(stream)
+            sess.execute()                                # a5-a7
+            e[2].record(stream)
+            res = None if execute_only else sess.verify() # a8 (synchronises the stream once to read the counters)
+            e[3].record(stream)
+            if not execute_only:
+                th.join()
+            e[4].record(stream)
+            torch.cuda.synchronize(self.dev)
+            if res is not None and (res["bad_elements"] or res["overlap_elements"]):
+                raise RuntimeError(f"verification failed: {res}")
+            return {"total": e[0].elapsed_time(e[4]), "plan_host": (t1 - t0) * 1e3, "cost_host": box.get("cost_ms", 0.0),
+                    "plan_to_launch": e[0].elapsed_time(e[1]), "execute": e[1].elapsed_time(e[2]),
+                    "verify": e[2].elapsed_time(e[3]), "cost_not_hidden": e[3].elapsed_time(e[4])}
+
+        for _ in range(warmup):
+            restore()
+            one_pass()
+        if sampler is not None:
+            for _ in range(200):         # nvidia-smi takes longer to start than a short timed region lasts
+                if sampler.count_since(0.0) or not sampler.proc:
+                    break
+                restore()
+                one_pass()
+        self.rep.barrier()
+        torch.cuda.synchronize(self.dev)
+        recs = []
+        wall0 = time.perf_counter()
+        for _ in range(steps):
+            restore()
+            torch.cuda.synchronize(self.dev)
+            recs.append(one_pass())
+        torch.cuda.synchronize(self.dev)
+        wall = time.perf_counter() - wall0
+        clocks = None
+        if sampler is not None:
+            in_region = sampler.count_since(wall0)
+            extra = 0
+            while sampler.proc and sampler.count_since(wall0) < 3 and extra < 400:
+                restore()                # region shorter than three sampling periods: keep the same load running, untimed
+                one_pass()
+                extra += 1
+            clocks = sampler.stop(wall0)
+            clocks["samples_in_timed_region"] = in_region
+            clocks["untimed_steps_of_the_same_load_added_for_sampling"] = extra
+        self.rep.barrier()
+        mean = lambda key: sum(r[key] for r in recs) / len(recs)
+        t_step, t_exec, t_ver = self.rep.max_over_ranks([mean("total"), mean("execute"), mean("verify")])
+        # parity spot-check of the last timed pass against the fp64 sum on sampled elements (cheap, outside timing)
+        idx = W.sample_indices(w, 4096)
+        y0 = sess.bufs[0][torch.from_numpy(idx).to(self.dev)].float().cpu().numpy().astype(np.float64)
+        if w.dtype == W.F32:
+            xs = x[:, idx].astype(np.float64)
+            tol = w.p * 2.0 ** -23 * np.abs(xs).sum(0)
+        else:
+            xs = (x[:, idx].astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+            tol = 2.0 ** -7 * np.abs(xs.sum(0)) + w.p * 2.0 ** -23 * np.abs(xs).sum(0)
+        parity_ok = bool((np.abs(y0 - xs.sum(0)) <= tol).all())
+        ranks_equal = all(torch.equal(sess.bufs[0].view(torch.int16 if w.dtype == W.BF16 else torch.int32),
+                                      b.view(torch.int16 if w.dtype == W.BF16 else torch.int32)) for b in sess.bufs[1:])
+        parity_ok = self.rep.all_true(parity_ok and ranks_equal)
+        out = {"w": w, "k": info["k"], "info": info, "cost": cost0, "t_step": t_step, "t_exec": t_exec, "t_ver": t_ver,
+               "breakdown_ms": {"plan_host": mean("plan_host"), "plan_to_launch": mean("plan_to_launch"), "execute": t_exec,
+                                "verify": t_ver, "cost_host_on_second_thread": mean("cost_host"),
+                                "cost_host_not_hidden": mean("cost_not_hidden")},
+               "parity_ok": parity_ok, "idx": idx, "xs": xs, "tol": tol, "wall": wall, "clocks": clocks, "steps": steps}
+        if keep:
+            out["sess"], out["x"] = sess, x
+        else:
+            del sess, pristine
+            torch.cuda.empty_cache()
+        return out
+
+    def summary(self, m):
+        """The per-config object of `other_configs` (and the pieces of the headline line)."""
+        w, info, c = m["w"], m["info"], m["cost"]
+        esize = w.elem_bytes
+        mode = info["exec_mode"]
+        kern = EXEC_KERNEL[mode] + ("<MODE_F32>" if w.dtype == self.W.F32 else "<MODE_BF16>")
+        roof = roofline_of(kern, mode, w.p, w.n, esize, m["t_exec"], self.peak, self.peak_src)
+        mask_final = w.p * w.n * info["mask_bytes"]
+        lb = c["lb_table1"] / c["T0"]
+        return {"workload": workload_name(w, m["k"]), "k": m["k"], "executor": EXEC_NAME[mode], "step_ms": m["t_step"],
+                "algbw_GBs": self.rep.world * w.n * esize / m["t_step"] / 1e6,
+                "execute_ms": m["t_exec"], "execute_algbw_GBs": self.rep.world * w.n * esize / m["t_exec"] / 1e6,
+                "verify_ms": m["t_ver"], "breakdown_ms": m["breakdown_ms"], "plan_steps": info["n_steps"], "plan_flows": info["n_flows"],
+                "roofline_frac": roof["frac"], "schedule_over_peak": roof["schedule_over_peak"],
+                "roofline_verify_frac": mask_final / m["t_ver"] / 1e6 / self.peak,
+                "model": {"T_over_T0": c["T_over_T0"], "lb_table1_over_T0": lb, "T_over_lb_table1": c["T_over_T0"] / lb,
+                          "lb_tight_over_T0": (c["lb_tight"] / c["T0"]) if c["lb_tight"] == c["lb_tight"] else None},
+                "parity_spot_check": {"sampled_elements": int(len(m["idx"])), "within_tolerance_and_all_ranks_identical": m["parity_ok"]}}
 
 
 def run_native(args):
     import numpy as np
-    import torch
-    from paper_2606_01680_b200 import binding as B, workloads as W
-    from paper_2606_01680_b200 import build as optcc_build
-    from paper_2606_01680_b200.device import Session
-
-    from paper_2606_01680_b200.replicas import Replicas
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: liboptcc has no CPU fallback (use --impl reference for the oracle)")
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    rep = Replicas(backend="nccl", device=dev)
-    rank, world = rep.rank, rep.world
-    if rank == 0:
-        optcc_build.build()
-    rep.barrier()
-    B.load()
-
+    bench = Bench(args)
+    torch, B, W, rep = bench.torch, bench.B, bench.W, bench.rep
+    rank, world, dev, stream = rep.rank, rep.world, bench.dev, bench.stream
     w = rep.shard(W.config(args.config, args.ell) if args.config == 4 else W.config(args.config))
     esize = w.elem_bytes
-    mk = lambda: B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=bench_k(args), exec_mode=args.exec_mode,
-                              tile_units=args.tile_units, col_order=args.col_order)
-    plan0 = mk()
-    k = plan0.info["k"]
-    cost0 = B.optcc_cost(plan0)
-    sched_bytes = 5 * (w.p - 1) * w.n * esize            # SURVEY 8(d): 3 sizeof per reduce element + 2 per copy element
-    sess = Session(plan0, device=dev, verify=True)
-
-    # seeded synthetic inputs -> pristine device copy (restored between steps, untimed)
-    x = W.all_inputs(w)
-    sess.upload(x)
-    pristine = [b.clone() for b in sess.bufs]
-    restore = lambda: [b.copy_(s) for b, s in zip(sess.bufs, pristine)]
-    stream = torch.cuda.current_stream(dev)
-    ev = lambda: torch.cuda.Event(enable_timing=True)
-    # execute + verify; the lazy verifier (plan_info.lazy_verify) needs no init / check kernels around the mask run
-    exec_mode = plan0.info["exec_mode"]          # what OPTCC_EXEC_AUTO resolved to
-    launches_per_step = (plan0.info["n_steps"] if exec_mode == 2 else 1) * 2 + (0 if plan0.info["lazy_verify"] else 2)
-
-    def full_step(timed):
-        """a1-a3 optcc_plan, a5-a7 optcc_execute (a4 optcc_cost on the host meanwhile), a8 optcc_verify; returns event
-        times + host times."""
-        e = [ev() for _ in range(5)]
-        e[0].record(stream)
-        t0 = time.perf_counter()
-        plan = mk()
-        t1 = time.perf_counter()
-        sess.plan = plan
-        sess.prepare()
-        stream.synchronize()         # the table upload belongs to plan_to_launch, not to the executor's time
-        e[1].record(stream)
-        sess.execute()               # asynchronous: the host evaluates the cost model while the GPU runs the plan
-        e[2].record(stream)
-        t1b = time.perf_counter()
-        cost = B.optcc_cost(plan)
-        t2 = time.perf_counter()
-        e[4].record(stream)          # (completes when the executor has: the verifier's own time starts here)
-        res = sess.verify()          # synchronises the stream once to read the counters
-        e[3].record(stream)
-        torch.cuda.synchronize(dev)
-        if res["bad_elements"] or res["overlap_elements"]:
-            raise RuntimeError(f"verification failed: {res}")
-        return {"total": e[0].elapsed_time(e[3]), "plan_host": (t1 - t0) * 1e3, "cost_host": (t2 - t1b) * 1e3,
-                "plan_to_launch": e[0].elapsed_time(e[1]), "execute": e[1].elapsed_time(e[2]),
-                "verify": e[4].elapsed_time(e[3]), "cost_not_hidden": e[2].elapsed_time(e[4]), "T_over_T0": cost["T_over_T0"]}
-
-    for _ in range(max(args.warmup, 3)):
-        restore()
-        full_step(False)
-    sampler = ClockSampler(local)
-    sampler.start()                  # nvidia-smi takes longer to start than a short timed region lasts: start it early
-    for _ in range(200):             # (and keep the GPU in the same state meanwhile) until the first sample is in
-        if sampler.count_since(0.0) or not sampler.proc:
-            break
-        restore()
-        full_step(False)
-    rep.barrier()
-    torch.cuda.synchronize(dev)
-    recs = []
-    wall0 = time.perf_counter()
-    for _ in range(args.steps):
-        restore()
-        torch.cuda.synchronize(dev)
-        recs.append(full_step(True))
-    torch.cuda.synchronize(dev)
-    wall = time.perf_counter() - wall0
-    in_region = sampler.count_since(wall0)
-    extra = 0
-    while sampler.proc and sampler.count_since(wall0) < 3 and extra < 400:
-        restore()                    # region shorter than three sampling periods: keep the same load running, untimed,
-        full_step(False)             # until three samples exist (reported separately below)
-        extra += 1
-    clocks = sampler.stop(wall0)
-    clocks["samples_in_timed_region"] = in_region
-    clocks["untimed_steps_of_the_same_load_added_for_sampling"] = extra
-    rep.barrier()
-    mean = lambda key: sum(r[key] for r in recs) / len(recs)
-    t_step, t_exec, t_ver = mean("total"), mean("execute"), mean("verify")
-    t_step, t_exec, t_ver = rep.max_over_ranks([t_step, t_exec, t_ver])
-
-    # parity spot-check of the last timed step against the fp64 sum on sampled elements (cheap, outside timing)
-    idx = W.sample_indices(w, 4096)
-    y0 = sess.bufs[0][torch.from_numpy(idx).to(dev)].float().cpu().numpy().astype(np.float64)
-    if w.dtype == W.F32:
-        xs = x[:, idx].astype(np.float64)
-        tol = w.p * 2.0 ** -23 * np.abs(xs).sum(0)
-    else:
-        xs = (x[:, idx].astype(np.uint32) << 16).view(np.float32).astype(np.float64)
-        tol = 2.0 ** -7 * np.abs(xs.sum(0)) + w.p * 2.0 ** -23 * np.abs(xs).sum(0)
-    parity_ok = bool((np.abs(y0 - xs.sum(0)) <= tol).all())
+    sampler = ClockSampler(bench.local)
+    sampler.start()
+    m = bench.measure(w, bench_k(args), args.steps, max(args.warmup, 3), sampler=sampler, keep=True)
+    sess, x, info, cost0, k = m["sess"], m["x"], m["info"], m["cost"], m["k"]
+    t_step, t_exec, t_ver = m["t_step"], m["t_exec"], m["t_ver"]
+    idx, xs, tol = m["idx"], m["xs"], m["tol"]
+    exec_mode = info["exec_mode"]          # what OPTCC_EXEC_AUTO resolved to
+    launches_per_step = (info["n_steps"] if exec_mode == 2 else 1) * 2 + (0 if info["lazy_verify"] else 2)
 
     # e2e: the same step through the C-ABI call with HOST buffers, H2D + D2H inside the timed region.  The path shards
     # along the element axis (DESIGN.md 8), so the host call pipelines S element shards, each an AllReduce with the
@@ -336,15 +441,16 @@ def run_native(args):
         S = max(1, args.e2e_shards)
         while S > 1 and (w.n % S or (w.n // S) % 8):
             S //= 2
-        mk_e = (lambda: B.optcc_plan(w.p, w.g, w.ell, w.n // S, w.dtype, k=bench_k(args), exec_mode=args.exec_mode)) if S > 1 else mk
-        se = Session(mk_e(), device=dev, verify=True, alloc_bufs=False, shards=S) if S > 1 else sess
+        mk_e = lambda: B.optcc_plan(w.p, w.g, w.ell, w.n // S, w.dtype, k=bench_k(args), exec_mode=args.exec_mode,
+                                    tile_units=args.tile_units, col_order=args.col_order)
+        se = bench.Session(mk_e(), device=dev, verify=True, alloc_bufs=False, shards=S)
         se.bufs = sess.bufs
         hin = [torch.from_numpy(x[r]).pin_memory() if w.dtype == W.F32 else
                torch.from_numpy(x[r].view(np.int16)).pin_memory() for r in range(w.p)]
         hout = [torch.empty_like(t).pin_memory() for t in hin]
         ts = []
         for i in range(1 + args.e2e_steps):
-            a, b_ = ev(), ev()
+            a, b_ = bench.ev(), bench.ev()
             torch.cuda.synchronize(dev)
             a.record(stream)
             plan = mk_e()
@@ -354,13 +460,12 @@ def run_native(args):
             else:
                 se.execute_host(hin, hout)
             B.optcc_cost(plan)       # on the host while the copies and the plan run
-            res = se.verify()
+            se.verify()
             b_.record(stream)
             torch.cuda.synchronize(dev)
             if i:
                 ts.append(a.elapsed_time(b_))
-        t_e2e = sum(ts) / len(ts)
-        t_e2e = rep.max_over_ranks([t_e2e])[0]
+        t_e2e = rep.max_over_ranks([sum(ts) / len(ts)])[0]
         ok = all(torch.equal(hout[0], h) for h in hout[1:])
         y_e = hout[0].numpy()[idx].astype(np.float64) if w.dtype == W.F32 else \
             (hout[0].numpy().view(np.uint16)[idx].astype(np.uint32) << 16).view(np.float32).astype(np.float64)
@@ -370,38 +475,71 @@ def run_native(args):
                "call": ("optcc_execute_host_sharded: %d element shards of n/%d, one plan, H2D / execute / D2H overlapped" % (S, S))
                        if S > 1 else "optcc_execute_host",
                "all_ranks_identical_and_within_tolerance": bool(ok)}
-        del hin, hout
+        del hin, hout, se
 
-    parity_ok = rep.all_true(parity_ok)
+    # the number SURVEY 8(d) literally defines: a step-ordered executor (global step order, every intermediate state
+    # of the p buffers in HBM / L2) at its best k, on the same workload in the same run
+    stepwise = None
+    if not args.only_main and args.config == 1 and rank == 0 and world == 1:
+        del sess
+        m.pop("sess")
+        torch.cuda.empty_cache()
+        ms = bench.measure(w, 4, 5, 3, x=x, exec_mode=B.OPTCC_EXEC_PERSISTENT, execute_only=True)
+        kern = "optcc_exec_kernel<MODE_F32>"
+        stepwise = roofline_of(kern, 1, w.p, w.n, esize, ms["t_exec"], bench.peak, bench.peak_src)
+        stepwise["k"] = ms["k"]
+        stepwise["executor"] = EXEC_NAME[1]
+        tr, sha, src = ncu_traffic("C2", kern)
+        stepwise["traffic"] = tr
+        stepwise["traffic_captured_at_commit"] = sha
+
+    others = None
+    if not args.only_main and world == 1 and args.config == 1:
+        m.pop("sess", None)
+        sess = None
+        del x
+        torch.cuda.empty_cache()
+        others = {}
+        for ci in (0, 2, 3):
+            wo = W.config(ci)
+            others[wo.name] = bench.summary(bench.measure(wo, BENCH_K[ci], 3, 3))
+        x5 = None
+        for ell in W.C5_ELLS:      # the whole sweep of configs[4]; the inputs do not depend on ell
+            wo = W.config(4, ell)
+            if x5 is None:
+                x5 = W.all_inputs(wo)
+            others[wo.name] = bench.summary(bench.measure(wo, BENCH_K[4], 3, 3, x=x5))
+        del x5
+
     if rank != 0:
         rep.close()
         return 0
 
-    peak, peak_src = measured_peak()
-    kname = EXEC_KERNEL[exec_mode]
-    kern = kname + ("<MODE_F32>" if w.dtype == W.F32 else "<MODE_BF16>")
-    achieved = sched_bytes / t_exec / 1e6
-    traffic = ncu_traffic(w.name.split("[")[0], kern)
-    mask_bytes = 5 * (w.p - 1) * w.n * plan0.info["mask_bytes"]   # the same schedule on mask elements
+    peak, peak_src = bench.peak, bench.peak_src
+    kern = EXEC_KERNEL[exec_mode] + ("<MODE_F32>" if w.dtype == W.F32 else "<MODE_BF16>")
+    roof = roofline_of(kern, exec_mode, w.p, w.n, esize, t_exec, peak, peak_src)
+    traffic, sha, src = ncu_traffic(w.name.split("[")[0], kern)
+    roof.update({"traffic": traffic, "traffic_captured_at_commit": sha, "traffic_source": src,
+                 "traffic_frac_of_peak": (traffic / t_exec / 1e6 / peak) if traffic else None,
+                 "share_of_step": t_exec / t_step})
+    mask_final = w.p * w.n * info["mask_bytes"]
+    lb = cost0["lb_table1"] / cost0["T0"]
     line = {
         "metric": METRIC, "value": world * w.n * esize / t_step / 1e6, "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": t_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32" if w.dtype == W.F32 else "bf16(f32 accumulate)",
         "data": "synthetic",
-        "config": {"workload": workload_name(w, k), "step": "optcc_plan + optcc_cost + optcc_execute + optcc_verify (SURVEY 8(a) a1-a8)",
-                   "exec_mode": ("auto -> " if args.exec_mode == 0 else "") +
-                                {1: "persistent cooperative kernel, grid barrier per step", 2: "one launch per step",
-                                 3: "dataflow cooperative kernel: tile-ops in table order, per-range completion counters, no grid barrier",
-                                 4: "column kernel: a tile is taken through its region's whole flow list in dependency order, no "
-                                    "synchronisation between CTAs (every dependency lies inside one element column)"}[exec_mode],
-                   "plan_steps": plan0.info["n_steps"], "plan_flows": plan0.info["n_flows"], "parallelism": f"replicas x{world} (element-axis shards, no collective)",
+        "config": {"workload": workload_name(w, k),
+                   "step": "optcc_plan -> {optcc_cost on a second host thread} || {optcc_prepare, optcc_execute, optcc_verify} "
+                           "(SURVEY 8(a) a1-a8, all through the C ABI)",
+                   "exec_mode": ("auto -> " if args.exec_mode == 0 else "") + EXEC_NAME[exec_mode],
+                   "k": "%d: the k at which the modelled T/T0 is within the paper's reported gap of the Table-1 bound" % k,
+                   "plan_steps": info["n_steps"], "plan_flows": info["n_flows"],
+                   "parallelism": f"replicas x{world} (element-axis shards, no collective)",
                    "l2": "inputs larger than L2 (footprint %.2f GB) and restored from a pristine copy between steps, untimed" % (w.p * w.n * esize / 1e9)},
-        "execute_only": {"algbw": world * w.n * esize / t_exec / 1e6, "unit": UNIT, "ms": t_exec,
-                         "schedule_GBs": achieved, "pct_of_8TBs_nominal": achieved / 8000 * 100,
-                         "pct_of_measured_peak": achieved / peak * 100},
-        "breakdown_ms": {"plan_host": mean("plan_host"), "cost_host": mean("cost_host"), "plan_to_launch": mean("plan_to_launch"),
-                         "execute": t_exec, "cost_host_not_hidden_by_execute": mean("cost_not_hidden"), "verify": t_ver},
-        "model": {"T_over_T0": cost0["T_over_T0"], "lb_table1_over_T0": cost0["lb_table1"] / cost0["T0"],
+        "execute_only": {"algbw": world * w.n * esize / t_exec / 1e6, "unit": UNIT, "ms": t_exec},
+        "breakdown_ms": m["breakdown_ms"],
+        "model": {"T_over_T0": cost0["T_over_T0"], "lb_table1_over_T0": lb, "T_over_lb_table1": cost0["T_over_T0"] / lb,
                   "lb_tight_over_T0": (cost0["lb_tight"] / cost0["T0"]) if cost0["lb_tight"] == cost0["lb_tight"] else None,
                   "paper_closed_form_over_T0": cost0["T_closed_form"] / cost0["T0"], "limit_over_T0": cost0["T_limit"] / cost0["T0"],
                   "bodies": cost0["bodies"], "k": k,
@@ -409,21 +547,21 @@ def run_native(args):
                   "ring_on_degraded_topology_over_T0": cost0["T_ring_degraded"] / cost0["T0"],
                   "r2ccl_closed_form_over_T0": (cost0["T_r2ccl"] / cost0["T0"]) if cost0["T_r2ccl"] == cost0["T_r2ccl"] else None,
                   "paper_context": "SimAI: OPTCC within 2-6% of fault-free NCCL ring at <=50% bandwidth loss; prior work up to 57% (PAPER.md:7)"},
-        "roofline": {"bound": "hbm", "kernel": kern, "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": traffic,
-                     "algorithmic_bytes_per_launch": sched_bytes, "share_of_step": t_exec / t_step,
-                     # the same launch seen from DRAM: ncu's bytes (committed capture) over this run's live duration
-                     "traffic_frac_of_peak": (traffic / t_exec / 1e6 / peak) if traffic else None,
-                     "note": "frac > 1: a tile's p ranks go from the first hop to the last inside L1/L2, so DRAM sees about "
-                             "2 p n sizeof (inputs once, outputs once) for 5 (p-1) n sizeof algorithmic bytes"},
-        "roofline_verify": {"bound": "hbm", "kernel": "%s<masks of %d bits>%s" % (kname, 8 * plan0.info["mask_bytes"],
-                                                                  " (lazy: initial masks are constants, final masks checked by their last writer)"
-                                                                  if plan0.info["lazy_verify"] else " (+init, check)"),
-                            "achieved": mask_bytes / t_ver / 1e6, "peak": peak, "unit": "GB/s", "frac": mask_bytes / t_ver / 1e6 / peak,
-                            "share_of_step": t_ver / t_step},
-        "parity_spot_check": {"sampled_elements": int(len(idx)), "within_tolerance": parity_ok},
-        "clocks": clocks, "gpu_launches": launches_per_step * args.steps, "wall_s_timed_region": wall,
+        "roofline": roof,
+        "roofline_verify": {"bound": "hbm", "kernel": "%s<masks of %d bits>%s" % (EXEC_KERNEL[exec_mode], 8 * info["mask_bytes"],
+                                                                  " (lazy: initial masks are constants, partial sets forwarded in registers, "
+                                                                  "final masks checked by their last writer)"
+                                                                  if info["lazy_verify"] else " (+init, check)"),
+                            "achieved": mask_final / t_ver / 1e6, "peak": peak, "unit": "GB/s", "frac": mask_final / t_ver / 1e6 / peak,
+                            "definition": "compulsory DRAM bytes p n mask_bytes (every final mask written once) / kernel time",
+                            "ms": t_ver, "share_of_step": t_ver / t_step},
+        "parity_spot_check": {"sampled_elements": int(len(idx)), "within_tolerance_and_all_ranks_identical": m["parity_ok"]},
+        "clocks": m["clocks"], "gpu_launches": launches_per_step * args.steps, "wall_s_timed_region": m["wall"],
     }
+    if stepwise:
+        line["roofline_stepwise"] = stepwise
+    if others:
+        line["other_configs"] = others
     if e2e:
         line["e2e"] = e2e
     if world == 1 and not args.no_cpu_baseline:
@@ -432,13 +570,25 @@ def run_native(args):
         line["cpu_baseline"] = {"value": ws.n * esize / t / 1e9, "unit": UNIT, "cores": cpu_threads_used(), "kind": "oracle",
                                 "sample": f"n={ws.n} elements per rank of the config's n={w.n}, all p={w.p} ranks, every flow; {t:.1f} s",
                                 "host_cores": os.cpu_count()}
-    if not parity_ok:
+    ok = m["parity_ok"] and (not others or all(o["parity_spot_check"]["within_tolerance_and_all_ranks_identical"] for o in others.values()))
+    if not ok:
         line["error"] = "parity spot check failed"
     print(json.dumps(line), flush=True)
     rep.close()
-    return 0 if parity_ok else 1
+    return 0 if ok else 1
+
+
+def launch_replicas(args):
+    """`bench.py --gpus N` without torchrun: start N workers of this script (one per GPU, NCCL barrier + max over ranks
+    as in replicas.py) and hand their output through; rank 0 prints the line with n_gpus = N."""
+    from paper_2606_01680_b200.replicas import launch
+    return launch(args.gpus, os.path.abspath(__file__), sys.argv[1:])
 
 
 if __name__ == "__main__":
     a = parse_args()
-    sys.exit(run_reference(a) if a.impl == "reference" else run_native(a))
+    if a.impl == "reference":
+        sys.exit(run_reference(a))
+    if a.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(launch_replicas(a))
+    sys.exit(run_native(a))

@@ -146,8 +146,13 @@ typedef struct optcc_plan_info {
 } optcc_plan_info_t;
 
 typedef struct optcc_cost_params {
-  double alpha; /* fixed cost per flow (PAPER.md:68 excludes it: default 0; :201 reports a 14% fixed share) */
+  double alpha; /* fixed cost per flow that OCCUPIES its send and receive port (PAPER.md:68 excludes it: default 0) */
   double beta;  /* time per element on a healthy NIC (default 1) */
+  double alpha_latency; /* latency-type fixed cost (PLAN_SPEC 6; PAPER.md:201 fn.5: about 14% of the fault-free ring's
+                           time is fixed overhead): the ports are busy for the transfer only, the data is usable
+                           alpha_latency later -- neighbouring windows overlap it.  Default 0 */
+  double sync;  /* P2P sync message for inter-GPU dependencies: a flow that waits for data (not
+                   for a port) starts `sync` after the data is usable.  Default 0 */
 } optcc_cost_params_t;
 
 typedef struct optcc_cost {

@@ -11,11 +11,17 @@ from . import planner as P
 from . import closed_forms as cf
 
 
-def simulate(plan, alpha=0, beta=1):
-    """Returns dict(T, T0, ratio, port loads ...) with Fractions.  Flows are processed in table order."""
+def simulate(plan, alpha=0, beta=1, alpha_latency=0, sync=0):
+    """Returns dict(T, T0, ratio, port loads ...) with Fractions.  Flows are processed in table order.
+
+    alpha occupies the ports (a fixed cost per flow on its send and receive port).  alpha_latency and sync are the
+    latency-type fixed costs of PLAN_SPEC 6 (PAPER.md:201 fn.5: about 14 % of the fault-free ring's time is fixed
+    overhead; :199, :217: inter-GPU dependencies are enforced with P2P sync messages): the ports are busy for the
+    transfer only, the data is usable alpha_latency after the transfer ends, and a flow that has to wait for data
+    (rather than for a port) learns about it `sync` later."""
     p, g = plan.p, plan.g
     ell = [Fr(x) for x in plan.ell]
-    alpha, beta = Fr(alpha), Fr(beta)
+    alpha, beta, alat, sync = Fr(alpha), Fr(beta), Fr(alpha_latency), Fr(sync)
     send = {}   # (rank, link) -> free time
     recv = {}
     wfin, rfin = {}, {}
@@ -31,15 +37,15 @@ def simulate(plan, alpha=0, beta=1):
             dur = alpha + beta * ln * max(ell[s], ell[d])
         else:
             dur = alpha + beta * Fr(ln, g - 1)
-        start = max(send.get((s, link), zero), recv.get((d, link), zero),
-                    wfin.get((s, off), zero), wfin.get((d, off), zero), rfin.get((d, off), zero))
+        dep = max(wfin.get((s, off), zero), wfin.get((d, off), zero), rfin.get((d, off), zero))
+        start = max(send.get((s, link), zero), recv.get((d, link), zero), dep + sync if dep > zero else zero)
         fin = start + dur
         send[(s, link)] = fin
         recv[(d, link)] = fin
-        rfin[(s, off)] = max(rfin.get((s, off), zero), fin)
-        wfin[(d, off)] = fin
-        if fin > T:
-            T = fin
+        rfin[(s, off)] = max(rfin.get((s, off), zero), fin)   # the source range may be overwritten once it has been sent
+        wfin[(d, off)] = fin + alat                            # the data is usable alpha_latency after the transfer
+        if fin + alat > T:
+            T = fin + alat
         if link == P.NIC:
             load_send[s] += dur
             load_recv[d] += dur

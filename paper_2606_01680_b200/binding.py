@@ -45,7 +45,7 @@ class optcc_plan_info_t(C.Structure):
 
 
 class optcc_cost_params_t(C.Structure):
-    _fields_ = [("alpha", C.c_double), ("beta", C.c_double)]
+    _fields_ = [("alpha", C.c_double), ("beta", C.c_double), ("alpha_latency", C.c_double), ("sync", C.c_double)]
 
 
 class optcc_cost_t(C.Structure):
@@ -209,9 +209,9 @@ def optcc_column_tables(plan):
     return view(rec, nrec.value, COLREC_DTYPE), view(it, nit.value, COLITEM_DTYPE)
 
 
-def optcc_cost(plan, alpha=0.0, beta=1.0):
+def optcc_cost(plan, alpha=0.0, beta=1.0, alpha_latency=0.0, sync=0.0):
     out = optcc_cost_t()
-    params = optcc_cost_params_t(alpha, beta)
+    params = optcc_cost_params_t(alpha, beta, alpha_latency, sync)
     rc = load().optcc_cost(plan.handle, C.byref(params), C.byref(out))
     if rc:
         raise OptccError(rc, "optcc_cost")

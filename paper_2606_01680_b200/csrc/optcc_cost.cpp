@@ -17,7 +17,9 @@ extern "C" int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* p
   if (!plan || !out) return OPTCC_EINVAL;
   const optcc_plan_info_t& in = plan->info;
   const double alpha = params ? params->alpha : 0.0, beta = params ? params->beta : 1.0;
+  const double alat = params ? params->alpha_latency : 0.0, sync = params ? params->sync : 0.0;
   if (!(alpha >= 0.0) || !(beta > 0.0) || !std::isfinite(alpha) || !std::isfinite(beta)) return OPTCC_EINVAL;
+  if (!(alat >= 0.0) || !(sync >= 0.0) || !std::isfinite(alat) || !std::isfinite(sync)) return OPTCC_EINVAL;
   const uint32_t p = in.p, g = in.g, q = in.q, m = in.m, k = in.k;
   const double n = double(in.n);
 
@@ -54,13 +56,14 @@ extern "C" int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* p
     double& wd = D.wfin;
     double& rd = D.rfin;
     double& rs = S.rfin;
-    double start = std::max(std::max(sf, rf), std::max(ws, std::max(wd, rd)));
+    const double dep = std::max(ws, std::max(wd, rd));         // data dependencies
+    double start = std::max(std::max(sf, rf), dep > 0.0 ? dep + sync : 0.0);
     double fin = start + dur;
     sf = fin;
     rf = fin;
     rs = std::max(rs, fin);
-    wd = fin;
-    T = std::max(T, fin);
+    wd = fin + alat;                                            // usable alpha_latency after the transfer
+    T = std::max(T, fin + alat);
     if (m && f.link == OPTCC_LINK_NIC) {
       if (f.src == r_str) sent += double(f.len);
       if (f.dst == r_str) recvd += double(f.len);

@@ -6,6 +6,9 @@ used only for the barrier around the timed region and the max-over-ranks of the 
 GPUs, "gloo" in the CPU tests.
 """
 import os
+import socket
+import subprocess
+import sys
 
 import torch
 import torch.distributed as dist
@@ -56,3 +59,20 @@ class Replicas:
     def close(self):
         if self.active and dist.is_initialized():
             dist.destroy_process_group()
+
+
+def launch(nproc, script, argv, extra_env=None, timeout=None):
+    """Start `nproc` replicas of `script argv` on this node, one process per GPU, through torch.distributed.run
+    (rendezvous on 127.0.0.1, a free port): what `bench.py --gpus N` does when it is not already running under
+    torchrun.  The workers' output is handed through; returns the launcher's exit code."""
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "WARN")
+    if extra_env:
+        env.update(extra_env)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={int(nproc)}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), script] + list(argv)
+    return subprocess.run(cmd, env=env, timeout=timeout).returncode

@@ -201,3 +201,62 @@ def test_column_executor_plans_are_the_same_tables(ci, k):
         assert ia[key] == ib[key]
     assert ib["workspace_bytes"] % 256 == 0 and ib["verify_workspace_bytes"] >= ib["workspace_bytes"]
     assert B.optcc_cost(a)["T"] == B.optcc_cost(b)["T"]
+
+
+# ---- latency-type fixed cost and sync messages (PLAN_SPEC 6; PAPER.md:201 fn.5, :199, :217) ----
+@pytest.mark.parametrize("p", [3, 4, 8, 16, 33])
+def test_latency_alpha_on_the_fault_free_ring_is_the_textbook_alpha_beta_time(p):
+    """The fault-free ring with a latency-type alpha: T = 2(p-1)(n/p beta + alpha) -- the alpha-beta model of a ring
+    AllReduce (the closed form the 86 % / 14 % split of PAPER.md:201 fn.5 is calibrated on) -- as an equality of
+    rationals in the oracle, and 1e-12 in the library."""
+    from fractions import Fraction as Fr
+    n = 4 * p * 250
+    oplan = OP.build_plan(p, 1, [1.0] * p, n, OP.F32)
+    al, beta = Fr(7, 3), Fr(5, 4)
+    sim = cost_sim.simulate(oplan, beta=beta, alpha_latency=al)
+    assert sim["T"] == 2 * (p - 1) * (Fr(n, p) * beta + al)
+    c = B.optcc_cost(B.optcc_plan(p, 1, [1.0] * p, n, B.OPTCC_F32), beta=float(beta), alpha_latency=float(al))
+    assert abs(c["T"] - float(sim["T"])) <= 1e-12 * float(sim["T"])
+    # calibrated to 14 % fixed overhead: alpha = (0.14 / 0.86) n beta / p  =>  bandwidth share of T is exactly 86 %
+    al = Fr(14, 86) * Fr(n, p) * beta
+    sim = cost_sim.simulate(oplan, beta=beta, alpha_latency=al)
+    assert cf.T0(p, n, 1) * beta / sim["T"] == Fr(86, 100)
+
+
+@pytest.mark.parametrize("p,g,st,n,k,kw", [
+    (5, 1, {0: 2.0}, 4 * 4 * 4 * 25, 4, {}), (16, 1, {3: 8.0 / 7.0}, 123456, 8, {}), (9, 1, {1: 1.5}, 99999, 12, {"ordering": 3}),
+    (7, 1, {0: 2.0, 1: 4.0 / 3.0}, 65539, 4, {}), (16, 4, {r: 2.0 for r in range(4)}, 40001, 4, {}), (6, 1, {}, 7777, 0, {}),
+])
+def test_latency_alpha_and_sync_agree_with_the_oracles_rationals(p, g, st, n, k, kw):
+    from fractions import Fraction as Fr
+    ell = [float(st.get(i, 1.0)) for i in range(p)]
+    oplan = OP.build_plan(p, g, ell, n, OP.F32, k=k, **kw)
+    plan = B.optcc_plan(p, g, ell, n, B.OPTCC_F32, k=k, **kw)
+    base = cost_sim.simulate(oplan)
+    prev = base["T"]
+    for al, sy, a_occ in ((Fr(0), Fr(0), Fr(0)), (Fr(37, 2), Fr(0), Fr(0)), (Fr(37, 2), Fr(5, 4), Fr(0)), (Fr(1000), Fr(3), Fr(1, 4))):
+        sim = cost_sim.simulate(oplan, alpha=a_occ, alpha_latency=al, sync=sy)
+        c = B.optcc_cost(plan, alpha=float(a_occ), alpha_latency=float(al), sync=float(sy))
+        assert abs(c["T"] - float(sim["T"])) <= 1e-12 * float(sim["T"])
+        assert sim["T"] >= prev                      # fixed costs never speed a plan up
+        prev = sim["T"]
+    assert cost_sim.simulate(oplan, alpha_latency=0, sync=0)["T"] == base["T"]
+
+
+def test_a_latency_shorter_than_a_slot_is_hidden_by_the_neighbouring_stage():
+    """What makes the fixed cost a latency and not an occupancy: in the canonical plan a ring link
+    carries Stage 1 of one segment and Stage 4 of another back to back, so a chain's next hop starts one slot after the
+    previous one ended; a latency up to one slot only delays the drain of the pipeline, an occupancy of the same size
+    is paid in every one of the (k+1)(p-1) windows."""
+    from fractions import Fraction as Fr
+    p, k = 9, 8
+    n = 4 * (p - 1) * k * 50
+    ell = [1.0] * p
+    ell[0] = 2.0
+    oplan = OP.build_plan(p, 1, ell, n, OP.F32, k=k)
+    s = Fr(n, k * (p - 1))                                   # one slot (PAPER.md:124)
+    base = cost_sim.simulate(oplan)["T"]
+    lat = cost_sim.simulate(oplan, alpha_latency=s / 2)["T"]
+    occ = cost_sim.simulate(oplan, alpha=s / 2)["T"]
+    assert lat - base <= 2 * (p - 1) * (s / 2)               # at most one latency per hop of the last segment's chains
+    assert occ - base >= (k + 1) * (p - 1) * (s / 2)         # one occupancy per window

@@ -71,3 +71,29 @@ def test_single_process_is_a_noop():
             "assert r.aggregate(10.0, 2.0) == 5.0; r.barrier(); r.close(); print('ok')\n") % ROOT
     res = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=240)
     assert res.returncode == 0 and "ok" in res.stdout, res.stderr[-2000:]
+
+
+def test_launcher_starts_the_replicas_itself(tmp_path):
+    """`bench.py --gpus N` without torchrun goes through replicas.launch: N workers on 127.0.0.1, the same barrier and
+    max-over-ranks; here two CPU workers over gloo."""
+    import json
+    from paper_2606_01680_b200.replicas import launch
+    script = tmp_path / "worker.py"
+    script.write_text(WORKER)
+    out = tmp_path / "out.txt"
+    wrapper = tmp_path / "wrap.py"
+    wrapper.write_text(textwrap.dedent("""
+        import os, runpy, sys, io, contextlib
+        buf = io.StringIO()
+        with contextlib.redirect_stdout(buf):
+            runpy.run_path(%r, run_name="__main__")
+        with open(%r + "." + os.environ["RANK"], "w") as f:
+            f.write(buf.getvalue())
+    """) % (str(script), str(out)))
+    rc = launch(2, str(wrapper), [], extra_env={"CUDA_VISIBLE_DEVICES": ""}, timeout=300)
+    assert rc == 0
+    outs = []
+    for r in range(2):
+        text = open(str(out) + "." + str(r)).read()
+        outs.append(json.loads([l for l in text.splitlines() if l.startswith("RESULT ")][0][7:]))
+    assert sorted(o["rank"] for o in outs) == [0, 1] and all(o["world"] == 2 and o["t"] == [2.0, 5.0] for o in outs)
