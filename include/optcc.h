@@ -212,13 +212,19 @@ OPTCC_API int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* pa
  * optcc_execute: in-place AllReduce.  bufs [host array of p DEVICE pointers], each n elements of the plan's
  * dtype, 16-byte aligned, pairwise disjoint.  On entry bufs[i] holds x_i; when the stream reaches the end of
  * the enqueued work every bufs[i] holds sum_j x_j and all p outputs are bitwise identical (PAPER.md:68 (ii)).
- * The reduce-scatter and all-gather steps are carried out exactly as the plan lists them, step by step.
+ * Every flow of the plan is carried out: its operands are loaded, the add is one IEEE operation per element, its
+ * destination range is stored, and for every element the flows that touch it run in an order that respects the plan's
+ * data dependencies, so the outputs are bit-identical whatever the executor.  The step-ordered executors
+ * (OPTCC_EXEC_PERSISTENT / PER_STEP) additionally keep the GLOBAL step order, so every intermediate state of the p
+ * buffers exists in memory; the default column executor and the dataflow executor do not (see OPTCC_EXEC_COLUMN and
+ * DESIGN.md 3 "what is kept, what is given up").  With opts.step_limit = t every executor leaves exactly the state the
+ * first t steps produce.
  * workspace [device, >= workspace_bytes, 256-byte aligned] owned by the caller; the first call with a given
- * workspace (or after another plan used it) uploads the tables into it; optcc_prepare does this ahead of time and
- * always re-uploads -- call it again if the workspace memory was reused for something else in between.  stream: a cudaStream_t
+ * workspace (or after another plan used it) builds the executor's tables on the host and uploads them; optcc_prepare
+ * does this ahead of time and always re-uploads (see "Workspace contract" below).  stream: a cudaStream_t
  * (NULL = default stream).  Asynchronous: never synchronises the device or the stream; once the tables are resident
- * (after optcc_prepare or a first call) it only enqueues memsets and kernel launches (dataflow executor: two memsets
- * and one cooperative launch), so it can be captured into a CUDA graph on `stream` and replayed.
+ * (after optcc_prepare or a first call) it only enqueues memsets and kernel launches (column executor: one memset
+ * and one launch), so it can be captured into a CUDA graph on `stream` and replayed.
  * Errors: EINVAL (NULL / misaligned pointers), ECUDA. */
 OPTCC_API int optcc_prepare(optcc_plan_t* plan, void* workspace, void* stream);
 /* Host only, no device needed: the column executor's work list, for inspection and tests.  records [host, borrowed until

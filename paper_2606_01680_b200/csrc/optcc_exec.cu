@@ -1,8 +1,12 @@
-// Executor and verifier of liboptcc (sm_100a): carries out an OPTCC plan step by step over p virtual ranks'
-// buffers held in one GPU's HBM.  Reduce flows (Stage 1 hops PAPER.md:126, Stage 3 fold-in :132, bubble-up :165,
-// NVLink collect :862-875) are range additions dst[R] += src[R]; copy flows (Stage 4 :136, Stage 2 :130,
-// bubble-down :165, NVLink distribute :863-876) are range copies.  Flows of step t+1 see all writes of steps
-// <= t (:138 data dependencies).  No tensor cores: nothing here is a dense contraction.
+// Executor and verifier of liboptcc (sm_100a): carries out an OPTCC plan over p virtual ranks' buffers held in one
+// GPU's HBM.  Reduce flows (Stage 1 hops PAPER.md:126, Stage 3 fold-in :132, bubble-up :165, NVLink collect :862-875)
+// are range additions dst[R] += src[R]; copy flows (Stage 4 :136, Stage 2 :130, bubble-down :165, NVLink distribute
+// :863-876) are range copies.  Four executors run the same tables and give the same bits: two keep the global step
+// order (persistent kernel with a grid barrier; one launch per step), the dataflow kernel orders tile-ops by per-range
+// completion counters, and the column kernels (the default) take a tile of one region through every flow over that
+// region in an order that respects the data dependencies of :138 inside the element column -- every flow's loads, add
+// and store are issued, but there is no global step order.  The verifier runs the same tables on
+// contributor bitmasks.  No tensor cores: nothing here is a dense contraction.
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
@@ -597,6 +601,10 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
       n_units = ni.w;
     }
     int prev_cls = -1;
+    // the tile in bytes of the run's element type (all flows over a region have the region's offset and length)
+    bool ragged = false;
+    unsigned long long tile_byte0 = 0;
+    unsigned int tile_bytes = 0, nv = 0;
     for (unsigned int base = fb; base < fe; base += COL_REC) {
       const unsigned int cnt = fe - base < COL_REC ? fe - base : COL_REC;
       const bool last_chunk = base + cnt == fe;
@@ -608,6 +616,18 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
       __syncthreads();
       if (base == fb && D && !prefetched)          // nobody has asked for the first flows' operands yet
         for (unsigned int j = 0; j < D && j < cnt; ++j) prefetch_raw<MODE, COL_THREADS>(P, s_rec[j], ubeg, item.w);
+      if (base == fb) {
+        constexpr unsigned long long ESZ = ModeTraits<MODE>::ESIZE, VE = 16 / ESZ;
+        const unsigned long long len = s_rec[0].len, e0 = ubeg * P.unit_elems;
+        unsigned long long e1 = uend * P.unit_elems;
+        ragged = e1 > len && (len % VE) != 0;
+        if (e1 > len) e1 = len;
+        const unsigned long long v0 = e0 / VE, v1 = e1 / VE;     // whole 16-byte vectors of the tile
+        tile_byte0 = v0 * 16;
+        tile_bytes = (unsigned int)((v1 - v0) * 16);
+        const unsigned long long mine0 = v0 + threadIdx.x;
+        nv = mine0 >= v1 ? 0u : (unsigned int)((v1 - mine0 + COL_THREADS - 1) / COL_THREADS);
+      }
       auto run_flow = [&](const DFlow& cur) {
         if (MODE == MODE_BF16) {
           // a copy of fp32 partials moves two vectors per unit, thread i taking vector i instead of unit i: when the
@@ -615,6 +635,26 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
           const int cls = (cur.op == 1 && cur.ksrc != 0) ? 1 : 0;
           if (prev_cls >= 0 && cls != prev_cls) __syncthreads();
           prev_cls = cls;
+        }
+        // Fast paths (the verifier is bound by instruction issue, ncu r02: 69-72 % of the issue slots): flows that touch
+        // no memory from this thread skip everything else.  `ragged`: the tile holds the ragged end of a buffer, whose
+        // last few elements always go through memory (process_piece's scalar tail).
+        if (MASK_FWD && !ragged && cur.op == 0 &&
+            (cur.flags & (DFLOW_SRC_FWD | DFLOW_DST_INIT | DFLOW_NO_STORE | DFLOW_FINAL | DFLOW_STAGE_OUT)) ==
+                (DFLOW_SRC_FWD | DFLOW_DST_INIT | DFLOW_NO_STORE)) {
+          constexpr int EB = ModeTraits<MODE>::ESIZE;
+          mask_hop_in_registers<EB>(carry, mask_vector(cur.dst < 64 ? 1ull << cur.dst : 0ull, cur.dst >= 64 ? 1ull << (cur.dst - 64) : 0ull, EB),
+                                    nv, overlaps);
+          return;
+        }
+        if (bulk && !ragged && (cur.flags & DFLOW_FROM_STAGE) &&
+            !(is_mask_mode(MODE) && P.mask_lazy && (cur.flags & DFLOW_FINAL) && !stage_ok)) {
+          // the copies of one tile are issued by the warps' first lanes in turn: 60+ cp.async.bulk per tile (C3: every
+          // section goes to p - 1 ranks) would otherwise queue behind one thread
+          if (threadIdx.x == (bulk_turn % (COL_THREADS / 32)) * 32)
+            bulk_s2g_hint(rank_ptr(P, cur.dst) + cur.off * ModeTraits<MODE>::ESIZE + tile_byte0, s_stage_col, tile_bytes, bulk_pol);
+          ++bulk_turn;
+          return;
         }
         if (bulk) {
           // Bulk all-gather path.  The reduce flow that completes a sum which later copy flows distribute
@@ -735,9 +775,41 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel
     DFlow cur = load_record(P.flows + fb);
     if (pf) prefetch_raw<MODE, 32>(P, cur, ubeg, item.w);
     int prev_cls = -1;
+    // the tile in bytes of the run's element type (all flows over a region have the region's offset and length)
+    bool ragged;
+    unsigned long long tile_byte0;
+    unsigned int tile_bytes, nv;
+    {
+      constexpr unsigned long long ESZ = ModeTraits<MODE>::ESIZE, VE = 16 / ESZ;
+      const unsigned long long len = cur.len, e0 = ubeg * P.unit_elems;
+      unsigned long long e1 = uend * P.unit_elems;
+      ragged = e1 > len && (len % VE) != 0;
+      if (e1 > len) e1 = len;
+      const unsigned long long v0 = e0 / VE, v1 = e1 / VE;     // whole 16-byte vectors of the tile
+      tile_byte0 = v0 * 16;
+      tile_bytes = (unsigned int)((v1 - v0) * 16);
+      const unsigned long long mine0 = v0 + lane;
+      nv = mine0 >= v1 ? 0u : (unsigned int)((v1 - mine0 + 31) / 32);
+    }
     for (unsigned int j = fb; j < fe; ++j) {
       const DFlow nxt = load_record(P.flows + (j + 1 < fe ? j + 1 : j));
       if (pf && j + 1 < fe) prefetch_raw<MODE, 32>(P, nxt, ubeg, item.w);   // first touches of the next flow
+      // fast paths: flows that touch no memory from this lane (see optcc_column_kernel)
+      if (MASK_FWD && !ragged && cur.op == 0 &&
+          (cur.flags & (DFLOW_SRC_FWD | DFLOW_DST_INIT | DFLOW_NO_STORE | DFLOW_FINAL | DFLOW_STAGE_OUT)) ==
+              (DFLOW_SRC_FWD | DFLOW_DST_INIT | DFLOW_NO_STORE)) {
+        constexpr int EB = ModeTraits<MODE>::ESIZE;
+        mask_hop_in_registers<EB>(carry, mask_vector(cur.dst < 64 ? 1ull << cur.dst : 0ull, cur.dst >= 64 ? 1ull << (cur.dst - 64) : 0ull, EB),
+                                  nv, overlaps);
+        cur = nxt;
+        continue;
+      }
+      if (bulk && !ragged && (cur.flags & DFLOW_FROM_STAGE) &&
+          !(is_mask_mode(MODE) && P.mask_lazy && (cur.flags & DFLOW_FINAL) && !stage_ok)) {
+        if (lane == 0) bulk_s2g_hint(rank_ptr(P, cur.dst) + cur.off * ModeTraits<MODE>::ESIZE + tile_byte0, stage, tile_bytes, bulk_pol);
+        cur = nxt;
+        continue;
+      }
       if (MODE == MODE_BF16) {
         // a copy of fp32 partials moves two vectors per unit, lane i taking vector i instead of unit i: when the
         // lane-to-element mapping changes between consecutive flows the warp synchronises

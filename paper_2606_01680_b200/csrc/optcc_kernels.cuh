@@ -7,10 +7,11 @@
 //   MODE_MASK16 / 32 / 1 / 2   contributor bitmasks of 16 / 32 / 64 / 128 bits: reduce = disjoint OR, copy = assign
 // so the verifier (PAPER.md:68 correctness (ii)) runs exactly the tables the executor runs.
 //
-// Executors (optcc_exec.cu): the dataflow kernel (tile-ops claimed in table order, per-range completion counters, no
-// grid barrier; the default), the persistent kernel (host-built slices of equal HBM bytes per step and CTA, grid
-// barrier between steps) and the same kernel launched once per step.  All stream 16-byte vectors, fully coalesced,
-// UNROLL independent vectors in flight per thread and stream.
+// Executors (optcc_exec.cu): the column kernels (a tile of one region taken through its whole flow list, CTA-wide or
+// warp-wide tiles, no synchronisation between CTAs; the default), the dataflow kernel (tile-ops claimed in table
+// order, per-range completion counters, no grid barrier), the persistent kernel (host-built slices of equal HBM bytes
+// per step and CTA, grid barrier between steps) and the same kernel launched once per step.  All stream 16-byte
+// vectors, fully coalesced, UNROLL independent vectors in flight per thread and stream.
 #ifndef OPTCC_KERNELS_CUH_
 #define OPTCC_KERNELS_CUH_
 
@@ -484,6 +485,30 @@ __device__ __forceinline__ void range_mask_lazy_t(const char* __restrict__ s, ch
   if (v < vend) {
     const unsigned int rem = (unsigned int)((vend - v + NT - 1) / NT);
     remainder_dispatch<UNROLL>(rem, [&](auto K) { batch(v, K); });
+  }
+}
+
+// The forwarded ring hop of the verifier, with nothing in memory: carry |= {dst}, overlap detection on the thread's nv
+// vectors of the tile (a flow with DFLOW_SRC_FWD, DFLOW_DST_INIT and DFLOW_NO_STORE that is neither final nor staged).
+template <int EB>
+__device__ __forceinline__ void mask_hop_in_registers(uint4 (&carry)[4], uint4 DC, unsigned int nv, unsigned int& overlaps) {
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const uint4 a = carry[j];
+    const unsigned int cx = a.x & DC.x, cy = a.y & DC.y, cz = a.z & DC.z, cw = a.w & DC.w;
+    unsigned int c;
+    if (EB == 2) {
+      auto hw = [](unsigned int w) { return ((w & 0xFFFFu) != 0u) + ((w >> 16) != 0u); };
+      c = hw(cx) + hw(cy) + hw(cz) + hw(cw);
+    } else if (EB == 4) {
+      c = (cx != 0u) + (cy != 0u) + (cz != 0u) + (cw != 0u);
+    } else if (EB == 8) {
+      c = ((cx | cy) != 0u) + ((cz | cw) != 0u);
+    } else {
+      c = ((cx | cy | cz | cw) != 0u);
+    }
+    if ((unsigned int)j < nv) overlaps += c;
+    carry[j] = make_uint4(a.x | DC.x, a.y | DC.y, a.z | DC.z, a.w | DC.w);
   }
 }
 
