@@ -8,12 +8,9 @@
 // and store are issued, but there is no global step order.  The verifier runs the same tables on
 // contributor bitmasks.  No tensor cores: nothing here is a dense contraction.
 #include <algorithm>
-#include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <atomic>
-#include <chrono>
 #include <mutex>
 #include <unordered_map>
 #include <vector>
@@ -1331,8 +1328,6 @@ void build_column_state(optcc_plan_t* pl, optcc_exec_state* st, bool* all_covere
   }
   const size_t ncls = cls_begin.size() - 1;
   std::atomic<uint32_t> uncovered{0};
-  auto t_begin = std::chrono::steady_clock::now();
-  auto TT = [&](const char* w) { if (std::getenv("OPTCC_TIME")) fprintf(stderr, "  [col] %s %.3f ms\n", w, std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count() * 1e3); };
   // Complete schedules: every rule of PLAN_SPEC 4 places the flows of segment b at steps b P + (something that does not
   // depend on b), so the regions of one class have the SAME list up to offset and length.  Only the list of each
   // class's first region is gathered from the table and finished; the others are copies with their own range.
@@ -1372,7 +1367,6 @@ void build_column_state(optcc_plan_t* pl, optcc_exec_state* st, bool* all_covere
     }
   }
   if (fast) {
-    TT("gather");
     optcc_parallel_chunks(ncls, nf, [&](size_t c) {
       if (cls_begin[c] == cls_begin[c + 1]) return;
       ColScratch sc;
@@ -1435,7 +1429,6 @@ void build_column_state(optcc_plan_t* pl, optcc_exec_state* st, bool* all_covere
       }
     });
   }
-  TT("finish");
   *all_covered = uncovered.load() == 0;
   // ---- 3. one work item per (region, tile) ----
   auto make_items = [&](std::vector<uint4>& items, uint64_t tu, uint64_t reserve) {
@@ -1763,10 +1756,6 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   P.col_pf_dist = 1; P.col_pf_l2 = 0; P.col_pf_next = 0; P.col_bulk = 1;
   P.col_bulk_policy = 1;   // bulk stores evict_first: the all-gather's results are never read again (measured: C2 1.68 -> 1.62 ms)
   P.col_warp = pl->col_warp;
-  if (const char* t = std::getenv("OPTCC_TUNE")) {   // TEMPORARY (experiments): "dist,l2,next,bulk,bulkpolicy"
-    unsigned a = 1, b = 0, c = 0, d = 1, e = 1, f = 0;
-    if (std::sscanf(t, "%u,%u,%u,%u,%u,%u", &a, &b, &c, &d, &e, &f) >= 1) { P.col_pf_dist = a; P.col_pf_l2 = b; P.col_pf_next = c; P.col_bulk = d; P.col_bulk_policy = e; (void)f; }
-  }
   if (pl->opts.copy_path == 1) P.col_bulk = 0;
 }
 
@@ -1871,26 +1860,13 @@ int shard_pipe(int dev, size_t shards, ShardPipe** out) {
 }
 }  // namespace
 
-extern "C" int optcc_execute_host_sharded(optcc_plan_t* plan, uint64_t n_total, const void* const* host_in,
-                                          void* const* host_out, void* const* bufs, void* workspace, void* stream_) {
-  if (!plan || !host_in || !host_out || !bufs || !workspace) return OPTCC_EINVAL;
+namespace {
+// The body of optcc_execute_host_sharded once the pipe exists: every return below leaves work queued on sp->in / sp->out
+// that still reads the caller's host buffers, so the caller of this function joins those streams on any failure.
+int sharded_pipeline(optcc_plan_t* plan, uint64_t shards, size_t bytes, const void* const* host_in, void* const* host_out,
+                     void* const* bufs, void* workspace, void* stream_, ShardPipe* sp) {
   const optcc_plan_info_t& in = plan->info;
-  if (n_total == 0 || n_total % in.n != 0) return OPTCC_EINVAL;
-  const uint64_t shards = n_total / in.n;
-  if (shards > 1 && in.n % 8 != 0) return OPTCC_EINVAL;            // shard starts stay 16-byte aligned
-  if (shards > (uint64_t(1) << 16)) return OPTCC_EINVAL;
-  for (uint32_t r = 0; r < in.p; ++r)
-    if (!host_in[r] || !host_out[r] || !bufs[r] || (reinterpret_cast<uintptr_t>(bufs[r]) & 15)) return OPTCC_EINVAL;
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-  const size_t bytes = size_t(in.n) * (in.dtype == OPTCC_F32 ? 4 : 2);   // per rank and shard
-  int dev = 0;
-  CU_TRY(cudaGetDevice(&dev));
-  std::lock_guard<std::mutex> lock(g_pipe_mutex);   // one pipelined call at a time per process: the streams are shared
-  ShardPipe* sp = nullptr;
-  int rc = shard_pipe(dev, size_t(shards), &sp);
-  if (rc != OPTCC_OK) return rc;
-  rc = prepare_impl(plan, workspace, stream_, false);               // tables first, then the copies may start
-  if (rc != OPTCC_OK) return rc;
   CU_TRY(cudaEventRecord(sp->begin, stream));
   CU_TRY(cudaStreamWaitEvent(sp->in, sp->begin, 0));
   CU_TRY(cudaStreamWaitEvent(sp->out, sp->begin, 0));
@@ -1906,7 +1882,7 @@ extern "C" int optcc_execute_host_sharded(optcc_plan_t* plan, uint64_t n_total, 
     const size_t o = size_t(c) * bytes;
     for (uint32_t r = 0; r < in.p; ++r) shard_bufs[r] = static_cast<char*>(bufs[r]) + o;
     CU_TRY(cudaStreamWaitEvent(stream, sp->loaded[c], 0));
-    rc = optcc_execute(plan, shard_bufs.data(), workspace, stream_);
+    int rc = optcc_execute(plan, shard_bufs.data(), workspace, stream_);
     if (rc != OPTCC_OK) return rc;
     CU_TRY(cudaEventRecord(sp->done[c], stream));
     CU_TRY(cudaStreamWaitEvent(sp->out, sp->done[c], 0));
@@ -1917,6 +1893,37 @@ extern "C" int optcc_execute_host_sharded(optcc_plan_t* plan, uint64_t n_total, 
   CU_TRY(cudaEventRecord(sp->end, sp->out));
   CU_TRY(cudaStreamWaitEvent(stream, sp->end, 0));
   return OPTCC_OK;
+}
+}  // namespace
+
+extern "C" int optcc_execute_host_sharded(optcc_plan_t* plan, uint64_t n_total, const void* const* host_in,
+                                          void* const* host_out, void* const* bufs, void* workspace, void* stream_) {
+  if (!plan || !host_in || !host_out || !bufs || !workspace) return OPTCC_EINVAL;
+  const optcc_plan_info_t& in = plan->info;
+  if (n_total == 0 || n_total % in.n != 0) return OPTCC_EINVAL;
+  const uint64_t shards = n_total / in.n;
+  if (shards > 1 && in.n % 8 != 0) return OPTCC_EINVAL;            // shard starts stay 16-byte aligned
+  if (shards > (uint64_t(1) << 16)) return OPTCC_EINVAL;
+  for (uint32_t r = 0; r < in.p; ++r)
+    if (!host_in[r] || !host_out[r] || !bufs[r] || (reinterpret_cast<uintptr_t>(bufs[r]) & 15)) return OPTCC_EINVAL;
+  const size_t bytes = size_t(in.n) * (in.dtype == OPTCC_F32 ? 4 : 2);   // per rank and shard
+  int dev = 0;
+  CU_TRY(cudaGetDevice(&dev));
+  std::lock_guard<std::mutex> lock(g_pipe_mutex);   // one pipelined call at a time per process: the streams are shared
+  ShardPipe* sp = nullptr;
+  int rc = shard_pipe(dev, size_t(shards), &sp);
+  if (rc != OPTCC_OK) return rc;
+  rc = prepare_impl(plan, workspace, stream_, false);               // tables first, then the copies may start
+  if (rc != OPTCC_OK) return rc;
+  rc = sharded_pipeline(plan, shards, bytes, host_in, host_out, bufs, workspace, stream_, sp);
+  if (rc != OPTCC_OK) {
+    // a failed call returns only once nothing it queued can still touch host_in / host_out / bufs: the internal copy
+    // streams are not the caller's to wait on (return codes ignored: the first error is the one reported)
+    cudaStreamSynchronize(sp->in);
+    cudaStreamSynchronize(sp->out);
+    cudaStreamSynchronize(static_cast<cudaStream_t>(stream_));
+  }
+  return rc;
 }
 
 extern "C" int optcc_verify(optcc_plan_t* plan, void* workspace, void* stream_, optcc_verify_result_t* out) {
