@@ -38,7 +38,8 @@ enum {
   OPTCC_ENOMEM = 3,
   OPTCC_ECUDA = 4,        /* a CUDA runtime call failed; optcc_last_cuda_error() has the code */
   OPTCC_EVERIFY = 5,      /* contributor-mask verification found a wrong element */
-  OPTCC_ESTALE = 6        /* the workspace did not hold this plan's tables when a kernel ran (see optcc_workspace_check) */
+  OPTCC_ESTALE = 6,       /* the workspace did not hold this plan's tables when a kernel ran (see optcc_workspace_check) */
+  OPTCC_ETOOBIG = 7       /* optcc_execute_static: the plan needs more than OPTCC_STATIC_WORKSPACE_BYTES of workspace */
 };
 
 /* PLAN_SPEC 3 enumerations */
@@ -257,6 +258,23 @@ OPTCC_API int optcc_execute_host(optcc_plan_t* plan, const void* const* host_in,
  * elements -- shard starts must stay 16-byte aligned), ECUDA. */
 OPTCC_API int optcc_execute_host_sharded(optcc_plan_t* plan, uint64_t n_total, const void* const* host_in,
                                void* const* host_out, void* const* bufs, void* workspace, void* stream);
+
+/* optcc_execute without a caller workspace, for callers that cannot allocate device memory (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): the workspace is a static device array of
+ * OPTCC_STATIC_WORKSPACE_BYTES inside the library (every GPU that loads the library holds it until the process exits).
+ * The call itself allocates no device memory: no cudaMalloc / cudaFree / allocating library routine on any path; the
+ * array's device address is looked up once per device (cudaGetSymbolAddress, on the first call with that device
+ * current).  bufs, stream, the result and asynchrony are exactly optcc_execute's, whatever the plan's executor; the
+ * first call with a plan (or after another plan used the array) builds the tables on the host and uploads them.
+ * Limit: plans with info.workspace_bytes <= OPTCC_STATIC_WORKSPACE_BYTES (8 MiB: fp32 plans up to BASELINE config 1 =
+ * C2, p = 16, n = 2^26, k = 16; bf16 plans only while their fp32 partials, 4 p n bytes, fit), else OPTCC_ETOOBIG and
+ * nothing is enqueued.  ONE array per device is shared by every call and every plan and keeps the last call's
+ * contents: the library re-uploads / clears what it needs, but two calls whose work overlaps on the GPU (different
+ * streams without an ordering between them, or two host threads) race on it -- order them on one stream or with
+ * events.  Calls through optcc_execute with a caller workspace are unaffected.
+ * Errors: EINVAL, ETOOBIG, ECUDA. */
+#define OPTCC_STATIC_WORKSPACE_BYTES (8u << 20)
+OPTCC_API int optcc_execute_static(optcc_plan_t* plan, void* const* bufs, void* stream);
 
 /* Workspace contract.  optcc_prepare (and the first optcc_execute / optcc_verify with a workspace) writes the plan's
  * tables AND a stamp into the workspace; the library remembers per workspace address which plan's tables it holds, so

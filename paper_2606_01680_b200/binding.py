@@ -15,11 +15,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "liboptcc.so")
 
 OPTCC_F32, OPTCC_BF16 = 0, 1
-OPTCC_OK, OPTCC_EINVAL, OPTCC_EUNSUPPORTED, OPTCC_ENOMEM, OPTCC_ECUDA, OPTCC_EVERIFY, OPTCC_ESTALE = range(7)
+OPTCC_OK, OPTCC_EINVAL, OPTCC_EUNSUPPORTED, OPTCC_ENOMEM, OPTCC_ECUDA, OPTCC_EVERIFY, OPTCC_ESTALE, OPTCC_ETOOBIG = range(8)
+OPTCC_STATIC_WORKSPACE_BYTES = 8 << 20   # include/optcc.h
 OPTCC_EXEC_AUTO, OPTCC_EXEC_PERSISTENT, OPTCC_EXEC_PER_STEP, OPTCC_EXEC_DATAFLOW, OPTCC_EXEC_COLUMN = 0, 1, 2, 3, 4
 EXEC_NAMES = {0: "auto", 1: "persistent", 2: "per_step", 3: "dataflow", 4: "column"}
 OPTCC_SCHED_OPTCC, OPTCC_SCHED_RING_DEGRADED = 0, 1
-ERROR_NAMES = {1: "EINVAL", 2: "EUNSUPPORTED", 3: "ENOMEM", 4: "ECUDA", 5: "EVERIFY", 6: "ESTALE"}
+ERROR_NAMES = {1: "EINVAL", 2: "EUNSUPPORTED", 3: "ENOMEM", 4: "ECUDA", 5: "EVERIFY", 6: "ESTALE", 7: "ETOOBIG"}
 
 # optcc_flow_t (PLAN_SPEC 3): 40 bytes
 FLOW_DTYPE = np.dtype([
@@ -68,7 +69,7 @@ class OptccError(RuntimeError):
 
 _lib = None
 EXPORTS = ("optcc_plan", "optcc_plan_ex", "optcc_plan_destroy", "optcc_plan_info", "optcc_plan_tables", "optcc_cost",
-           "optcc_prepare", "optcc_column_tables", "optcc_execute", "optcc_execute_host", "optcc_execute_host_sharded", "optcc_workspace_check", "optcc_workspace_forget",
+           "optcc_prepare", "optcc_column_tables", "optcc_execute", "optcc_execute_static", "optcc_execute_host", "optcc_execute_host_sharded", "optcc_workspace_check", "optcc_workspace_forget",
            "optcc_verify", "optcc_strerror",
            "optcc_last_cuda_error", "optcc_abi_version")
 
@@ -93,6 +94,7 @@ def load():
     lib.optcc_prepare.argtypes = [vp, vp, vp]
     lib.optcc_column_tables.argtypes = [vp, C.POINTER(vp), C.POINTER(C.c_uint32), C.POINTER(vp), C.POINTER(C.c_uint32)]
     lib.optcc_execute.argtypes = [vp, C.POINTER(vp), vp, vp]
+    lib.optcc_execute_static.argtypes = [vp, C.POINTER(vp), vp]
     lib.optcc_execute_host.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), vp, vp]
     lib.optcc_execute_host_sharded.argtypes = [vp, u64, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), vp, vp]
     lib.optcc_verify.argtypes = [vp, vp, vp, C.POINTER(optcc_verify_result_t)]
@@ -229,6 +231,14 @@ def optcc_execute(plan, bufs, workspace, stream=None):
     rc = load().optcc_execute(plan.handle, _ptr_array(bufs), _ptr(workspace), _ptr(stream))
     if rc:
         raise OptccError(rc, "optcc_execute")
+
+
+def optcc_execute_static(plan, bufs, stream=None):
+    """optcc_execute on the library's static device workspace (no device allocation; plans up to
+    OPTCC_STATIC_WORKSPACE_BYTES of workspace, else OptccError ETOOBIG)."""
+    rc = load().optcc_execute_static(plan.handle, _ptr_array(bufs), _ptr(stream))
+    if rc:
+        raise OptccError(rc, "optcc_execute_static")
 
 
 def optcc_execute_host(plan, host_in, host_out, bufs, workspace, stream=None):

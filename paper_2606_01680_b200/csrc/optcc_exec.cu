@@ -1814,6 +1814,45 @@ extern "C" int optcc_execute(optcc_plan_t* plan, void* const* bufs, void* worksp
   return in.dtype == OPTCC_F32 ? launch_plan<MODE_F32>(plan, P, stream) : launch_plan<MODE_BF16>(plan, P, stream);
 }
 
+// ---- optcc_execute_static: optcc_execute for callers that cannot allocate device memory --------------------------
+// The workspace (control block, executor tables, dataflow counters, bf16 fp32 partials) is this file-scope array instead
+// of caller memory.  In host code the NAME of the array is only a stand-in of the host compiler, not a device address:
+// the address comes from cudaGetSymbolAddress, asked once per device with that device current, and goes to the kernels
+// through ExecParams like any caller workspace.  Every GPU that loads the library holds these bytes until the process exits.
+static __device__ __align__(256) unsigned char g_static_workspace[OPTCC_STATIC_WORKSPACE_BYTES];
+
+namespace {
+std::mutex g_static_mutex;
+std::unordered_map<int, void*> g_static_ptr;      // device ordinal -> device address of g_static_workspace there
+
+int static_workspace(void** out) {
+  int dev = 0;
+  CU_TRY(cudaGetDevice(&dev));
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  auto it = g_static_ptr.find(dev);
+  if (it == g_static_ptr.end()) {
+    void* ptr = nullptr;
+    CU_TRY(cudaGetSymbolAddress(&ptr, g_static_workspace));
+    if (!ptr || (reinterpret_cast<uintptr_t>(ptr) & 255)) return OPTCC_ECUDA;
+    it = g_static_ptr.emplace(dev, ptr).first;
+  }
+  *out = it->second;
+  return OPTCC_OK;
+}
+}  // namespace
+
+extern "C" int optcc_execute_static(optcc_plan_t* plan, void* const* bufs, void* stream_) {
+  if (!plan || !bufs) return OPTCC_EINVAL;
+  if (plan->info.workspace_bytes > uint64_t(OPTCC_STATIC_WORKSPACE_BYTES)) return OPTCC_ETOOBIG;
+  void* ws = nullptr;
+  int rc = static_workspace(&ws);
+  if (rc != OPTCC_OK) return rc;
+  // Same path as a caller workspace from here on.  The array keeps what the last call left in it: the tables are
+  // uploaded again (control block cleared, stamp rewritten) whenever the last plan to use it was another one, and every
+  // launch clears its own ticket / barrier / completion counters first (launch_plan), so nothing is assumed to be zero.
+  return optcc_execute(plan, bufs, ws, stream_);
+}
+
 extern "C" int optcc_execute_host(optcc_plan_t* plan, const void* const* host_in, void* const* host_out,
                                   void* const* bufs, void* workspace, void* stream_) {
   if (!plan || !host_in || !host_out || !bufs) return OPTCC_EINVAL;

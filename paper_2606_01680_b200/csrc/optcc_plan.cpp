@@ -713,6 +713,7 @@ extern "C" const char* optcc_strerror(int code) {
     case OPTCC_ECUDA: return "CUDA runtime error (see optcc_last_cuda_error)";
     case OPTCC_EVERIFY: return "contributor-mask verification failed";
     case OPTCC_ESTALE: return "the workspace did not hold this plan's tables when a kernel ran: call optcc_prepare and run again";
+    case OPTCC_ETOOBIG: return "the plan needs more workspace than the library's static array holds (OPTCC_STATIC_WORKSPACE_BYTES): use optcc_execute with a caller workspace";
     default: return "unknown optcc error";
   }
 }
