@@ -56,6 +56,7 @@ def parse_args():
                          "1 persistent kernel with grid barriers, 2 one launch per step, 3 dataflow kernel, 4 column kernel")
     ap.add_argument("--tile-units", type=int, default=0, help="opts.tile_units (0 = the library's choice)")
     ap.add_argument("--col-order", type=int, default=0, help="opts.col_order (column executor: 0 chain by chain, 1 table order)")
+    ap.add_argument("--no-forward", type=int, default=0, help="opts.no_forward (column executor, f32: 1 = every reduce flow loads both operands)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--e2e-shards", type=int, default=16,
                     help="element shards of the end-to-end leg (optcc_execute_host_sharded: H2D, execute and D2H of "
@@ -234,8 +235,9 @@ def ncu_traffic(workload, kernel):
 
 EXEC_NAME = {1: "persistent cooperative kernel, grid barrier per step", 2: "one launch per step",
              3: "dataflow cooperative kernel: tile-ops in table order, per-range completion counters, no grid barrier",
-             4: "column kernel: a tile is taken through its region's whole flow list in dependency order, no "
-                "synchronisation between CTAs (every dependency lies inside one element column)"}
+             4: "column kernel: a tile is taken through its region's whole flow list in dependency order, partial sums "
+                "forwarded in registers between consecutive flows, no synchronisation between CTAs (every dependency lies "
+                "inside one element column)"}
 
 
 def roofline_of(kernel, exec_mode, p, n, esize, t_ms, peak, peak_src):
@@ -252,8 +254,9 @@ def roofline_of(kernel, exec_mode, p, n, esize, t_ms, peak, peak_src):
             "definition": ("schedule bytes 5 (p-1) n sizeof / kernel time (SURVEY 8(d)): this executor keeps global step order, "
                            "every flow's operands go through HBM / L2") if stepwise else
                           ("compulsory DRAM bytes 2 p n sizeof (every input read once, every output written once) / kernel time: "
-                           "this executor takes a tile through its whole flow list inside L1 / L2 and drops dead partial sums from "
-                           "the caches, so the schedule's 5 (p-1) n sizeof bytes never reach HBM (see schedule_over_peak)"),
+                           "this executor takes a tile through its whole flow list, partial sums travel between consecutive flows "
+                           "in registers (column executor) or through L1 / L2, so the schedule's 5 (p-1) n sizeof bytes never reach "
+                           "HBM (see schedule_over_peak; roofline_every_load_and_store: the same with opts.no_forward = 1)"),
             "algorithmic_bytes_per_launch": nbytes, "schedule_bytes_per_launch": sched,
             "schedule_over_peak": sched / t_ms / 1e6 / peak, "ms": t_ms}
 
@@ -285,7 +288,7 @@ class Bench:
     def ev(self):
         return self.torch.cuda.Event(enable_timing=True)
 
-    def measure(self, w, k, steps, warmup, x=None, sampler=None, keep=False, exec_mode=None, execute_only=False):
+    def measure(self, w, k, steps, warmup, x=None, sampler=None, keep=False, exec_mode=None, execute_only=False, no_forward=None):
         """`steps` timed passes of the whole hot path on workload w (inputs resident in HBM, restored from a pristine
         device copy between passes, untimed: the AllReduce is in place and the restore flushes L2).  One pass =
         optcc_plan -> {optcc_cost on a second host thread} || {optcc_prepare, optcc_execute, optcc_verify} -> join."""
@@ -293,8 +296,9 @@ class Bench:
         import numpy as np
         esize = w.elem_bytes
         mode = args.exec_mode if exec_mode is None else exec_mode
+        nf = args.no_forward if no_forward is None else no_forward
         mk = lambda: B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=k, exec_mode=mode, tile_units=args.tile_units,
-                                  col_order=args.col_order)
+                                  col_order=args.col_order, no_forward=nf)
         plan0 = mk()
         info = plan0.info
         cost0 = B.optcc_cost(plan0)
@@ -442,7 +446,7 @@ def run_native(args):
         while S > 1 and (w.n % S or (w.n // S) % 8):
             S //= 2
         mk_e = lambda: B.optcc_plan(w.p, w.g, w.ell, w.n // S, w.dtype, k=bench_k(args), exec_mode=args.exec_mode,
-                                    tile_units=args.tile_units, col_order=args.col_order)
+                                    tile_units=args.tile_units, col_order=args.col_order, no_forward=args.no_forward)
         se = bench.Session(mk_e(), device=dev, verify=True, alloc_bufs=False, shards=S)
         se.bufs = sess.bufs
         hin = [torch.from_numpy(x[r]).pin_memory() if w.dtype == W.F32 else
@@ -480,6 +484,7 @@ def run_native(args):
     # the number SURVEY 8(d) literally defines: a step-ordered executor (global step order, every intermediate state
     # of the p buffers in HBM / L2) at its best k, on the same workload in the same run
     stepwise = None
+    stepwise_extra = None
     if not args.only_main and args.config == 1 and rank == 0 and world == 1:
         del sess
         m.pop("sess")
@@ -492,6 +497,17 @@ def run_native(args):
         tr, sha, src = ncu_traffic("C2", kern)
         stepwise["traffic"] = tr
         stepwise["traffic_captured_at_commit"] = sha
+        # ... and the column executor with every load and store of every flow issued (opts.no_forward = 1): what the
+        # register forwarding of partial sums is worth, measured in the same run
+        if exec_mode == B.OPTCC_EXEC_COLUMN and not args.no_forward:
+            mn = bench.measure(w, k, 5, 3, x=x, execute_only=True, no_forward=1)
+            every = roofline_of(EXEC_KERNEL[exec_mode] + "<MODE_F32>, opts.no_forward = 1", exec_mode, w.p, w.n, esize, mn["t_exec"],
+                                bench.peak, bench.peak_src)
+            every["definition"] = ("the same executor with every flow's two loads and its store issued (no partial sum kept in "
+                                   "registers between flows); compulsory DRAM bytes 2 p n sizeof / kernel time")
+            stepwise_extra = every
+        else:
+            stepwise_extra = None
 
     others = None
     if not args.only_main and world == 1 and args.config == 1:
@@ -560,6 +576,8 @@ def run_native(args):
     }
     if stepwise:
         line["roofline_stepwise"] = stepwise
+    if stepwise_extra:
+        line["roofline_every_load_and_store"] = stepwise_extra
     if others:
         line["other_configs"] = others
     if e2e:

@@ -68,10 +68,14 @@ enum {
   OPTCC_EXEC_COLUMN = 4      /* one kernel, no synchronisation between CTAs at all: no flow ever mixes two element
                                 indices (a flow moves a range rank to rank), so every dependency of :138
                                 lies inside one element column.  A tile of one region is taken through every flow over
-                                that region, in an order that respects those dependencies; every flow's loads, add and
-                                store are issued and the outputs are bit-identical to the step-ordered executors, but there
-                                is NO global step order and intermediate states of the p buffers need not reach HBM
-                                (dead partial sums are dropped from the caches): DESIGN.md 3 "what is kept, what is given up" */
+                                that region, in an order that respects those dependencies; every flow's add is carried out
+                                (one IEEE operation per element, in the plan's order along the column) and the outputs are
+                                bit-identical to the step-ordered executors, but there is NO global step order, and a partial
+                                sum that only the next flow of the list reads and a later flow overwrites travels to that
+                                flow in registers: it is not stored (opts.no_forward restores every load and store).  What
+                                memory holds when the executed schedule ends -- the whole plan or its first step_limit
+                                steps -- is exactly what the step-ordered executors leave: DESIGN.md 3 "what is kept, what is
+                                given up" */
 };
 
 typedef struct optcc_plan optcc_plan_t; /* opaque; immutable after creation except for cached device state */
@@ -113,7 +117,14 @@ typedef struct optcc_opts {
   uint32_t col_order; /* column executor, order of a region's flows: 0 = chain by chain (a flow is followed by the flow that
                          reads what it wrote; any order respecting the dependencies of PAPER.md:138 inside the column gives
                          the same bits), 1 = table order */
-  uint32_t reserved[5]; /* 0 */
+  uint32_t no_forward;/* column executor, data runs.  0 (default): a reduce flow whose source range is what the flow just
+                         before it in the region's list produced adds that flow's registers instead of loading them back,
+                         and a partial sum that is read only this way and overwritten by a later flow of the executed
+                         schedule is not stored at all (it would be dropped from the caches before reaching HBM anyway).
+                         1 = every flow loads both operands and stores its result; 2 = registers are forwarded but every
+                         result is stored.  Same output bits in all three; 1 and 2 are for bisecting and A/B timing
+                         (bench.py reports the time with 1 beside the default) */
+  uint32_t reserved[4]; /* 0 */
 } optcc_opts_t;
 
 typedef struct optcc_plan_info {
@@ -213,9 +224,11 @@ OPTCC_API int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* pa
  * optcc_execute: in-place AllReduce.  bufs [host array of p DEVICE pointers], each n elements of the plan's
  * dtype, 16-byte aligned, pairwise disjoint.  On entry bufs[i] holds x_i; when the stream reaches the end of
  * the enqueued work every bufs[i] holds sum_j x_j and all p outputs are bitwise identical (PAPER.md:68 (ii)).
- * Every flow of the plan is carried out: its operands are loaded, the add is one IEEE operation per element, its
- * destination range is stored, and for every element the flows that touch it run in an order that respects the plan's
- * data dependencies, so the outputs are bit-identical whatever the executor.  The step-ordered executors
+ * Every flow of the plan is carried out: the add is one IEEE operation per element, and for every element the flows that
+ * touch it run in an order that respects the plan's data dependencies, so the outputs are bit-identical
+ * whatever the executor.  The step-ordered and dataflow executors load both operands of every flow from memory and store
+ * every destination range; the column executor keeps a partial sum in registers between two consecutive flows of a
+ * column when nothing else would ever read it (OPTCC_EXEC_COLUMN, opts.no_forward).  The step-ordered executors
  * (OPTCC_EXEC_PERSISTENT / PER_STEP) additionally keep the GLOBAL step order, so every intermediate state of the p
  * buffers exists in memory; the default column executor and the dataflow executor do not (see OPTCC_EXEC_COLUMN and
  * DESIGN.md 3 "what is kept, what is given up").  With opts.step_limit = t every executor leaves exactly the state the

@@ -33,7 +33,7 @@ FLOW_DTYPE = np.dtype([
 class optcc_opts_t(C.Structure):
     _fields_ = [("k", C.c_uint32), ("exec_mode", C.c_uint32), ("grid_ctas", C.c_uint32), ("copy_path", C.c_uint32),
                 ("step_limit", C.c_uint32), ("tile_units", C.c_uint32), ("schedule", C.c_uint32), ("ordering", C.c_uint32), ("no_discard", C.c_uint32), ("verify_eager", C.c_uint32),
-                ("col_order", C.c_uint32), ("reserved", C.c_uint32 * 5)]
+                ("col_order", C.c_uint32), ("no_forward", C.c_uint32), ("reserved", C.c_uint32 * 4)]
 
 
 class optcc_plan_info_t(C.Structure):
@@ -158,11 +158,11 @@ class Plan:
             pass
 
 
-def optcc_plan(p, g, ell, n, dtype, k=0, exec_mode=OPTCC_EXEC_AUTO, grid_ctas=0, copy_path=0, step_limit=0, tile_units=0, schedule=0, ordering=0, no_discard=0, verify_eager=0, col_order=0):
+def optcc_plan(p, g, ell, n, dtype, k=0, exec_mode=OPTCC_EXEC_AUTO, grid_ctas=0, copy_path=0, step_limit=0, tile_units=0, schedule=0, ordering=0, no_discard=0, verify_eager=0, col_order=0, no_forward=0):
     """optcc_plan_ex: returns a Plan.  ell: sequence of p floats."""
     lib = load()
     ell_arr = (C.c_double * len(ell))(*[float(x) for x in ell])
-    opts = optcc_opts_t(k, exec_mode, grid_ctas, copy_path, step_limit, tile_units, schedule, ordering, no_discard, verify_eager, col_order)
+    opts = optcc_opts_t(k, exec_mode, grid_ctas, copy_path, step_limit, tile_units, schedule, ordering, no_discard, verify_eager, col_order, no_forward)
     h = C.c_void_p()
     rc = lib.optcc_plan_ex(int(p), int(g), ell_arr, int(n), int(dtype), C.byref(opts), C.byref(h))
     if rc:

@@ -4,8 +4,9 @@
 // :863-876) are range copies.  Four executors run the same tables and give the same bits: two keep the global step
 // order (persistent kernel with a grid barrier; one launch per step), the dataflow kernel orders tile-ops by per-range
 // completion counters, and the column kernels (the default) take a tile of one region through every flow over that
-// region in an order that respects the data dependencies of :138 inside the element column -- every flow's loads, add
-// and store are issued, but there is no global step order.  The verifier runs the same tables on
+// region in an order that respects the data dependencies of :138 inside the element column -- every flow's add is
+// carried out in the plan's order, a partial sum that only the next flow of the column reads and a later flow
+// overwrites stays in registers, and there is no global step order.  The verifier runs the same tables on
 // contributor bitmasks.  No tensor cores: nothing here is a dense contraction.
 #include <algorithm>
 #include <cstring>
@@ -58,10 +59,12 @@ __device__ __forceinline__ char* rank_ptr(const ExecParams& P, unsigned int r) {
 // flow of the list, taken instead of a load when the flow says so (DFLOW_SRC_FWD); other callers pass a scratch array.
 // MASK_FWD (column executor, contributor-mask runs): the run is in the lazy form and every tile is one round, so only
 // the forwarding round (range_mask_round) is compiled in -- the kernel then has the registers to keep `carry` live.
-template <int MODE, int NT, bool MASK_FWD = false, class PolX>
+// MASK_FWD with MODE_F32 (column executor, ExecParams.data_fwd): every tile is one round, reduce flows run as
+// range_add_f32_round and take a source the previous flow stored (DFLOW_SRC_REG) from `carry` instead of loading it.
+template <int MODE, int NT, bool MASK_FWD = false, class PolX, int CN>
 __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& f, unsigned long long ubeg,
                                               unsigned long long uend, unsigned int& overlaps, const PolX& pol,
-                                              uint4 (&carry)[4], bool use_carry = false,
+                                              uint4 (&carry)[CN], bool use_carry = false,
                                               char* stage = nullptr, bool from_stage = false, bool* stage_full = nullptr) {
   using MT = ModeTraits<MODE>;
   const unsigned int tid = group_tid<NT>();
@@ -77,7 +80,15 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
   if (MODE == MODE_F32) {
     const char* s = rank_ptr(P, f.src) + f.off * 4;
     char* d = rank_ptr(P, f.dst) + f.off * 4;
-    if (f.op == 0) {
+    if (f.op == 0 && MASK_FWD) {   // (data runs: FWD = ExecParams.data_fwd, the tile is one round)
+      const bool src_reg = use_carry && (f.flags & DFLOW_SRC_REG) != 0u;
+      const bool elide = (P.data_fwd & 2u) != 0u;
+      const bool no_store = elide && (f.flags & DFLOW_NO_STORE) != 0u;
+      const bool dead = dead_src && !(elide && (f.flags & DFLOW_SRC_FWD));   // (a source that was never stored has no dirty line)
+      uint4 (&c4)[4] = reinterpret_cast<uint4 (&)[4]>(carry);
+      if (stage) range_add_f32_round<NT, true>(s, d, vbeg, vend, pol, dead, src_reg, stage, c4, no_store);
+      else range_add_f32_round<NT, false>(s, d, vbeg, vend, pol, dead, src_reg, nullptr, c4, no_store);
+    } else if (f.op == 0) {
       if (stage) range_add_f32<4, NT, true>(s, d, vbeg, vend, pol, dead_src, stage);
       else range_add_f32<4, NT, false>(s, d, vbeg, vend, pol, dead_src, nullptr);
     } else if (!from_stage) {
@@ -108,7 +119,8 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
       const uint4 SC = mask_vector(f.src < 64 ? 1ull << f.src : 0ull, f.src >= 64 ? 1ull << (f.src - 64) : 0ull, EB);
       const uint4 DC = mask_vector(f.dst < 64 ? 1ull << f.dst : 0ull, f.dst >= 64 ? 1ull << (f.dst - 64) : 0ull, EB);
       range_mask_round<4, EB, NT>(s, d, vbeg, vend, overlaps, pol, f.flags, f.op == 0, SC, DC, mask_vector(full0, full1, EB),
-                                  P.ctrl, (unsigned long long)f.dst * P.n + f.off, f.op == 0 ? stage : nullptr, stage_full, carry);
+                                  P.ctrl, (unsigned long long)f.dst * P.n + f.off, f.op == 0 ? stage : nullptr, stage_full,
+                                  reinterpret_cast<uint4 (&)[4]>(carry));
     } else if (P.mask_lazy) {   // lazy verifier: initial masks are constants, the last writer checks the final mask (range_mask_lazy)
       const uint4 SC = mask_vector(f.src < 64 ? 1ull << f.src : 0ull, f.src >= 64 ? 1ull << (f.src - 64) : 0ull, EB);
       const uint4 DC = mask_vector(f.dst < 64 ? 1ull << f.dst : 0ull, f.dst >= 64 ? 1ull << (f.dst - 64) : 0ull, EB);
@@ -158,6 +170,23 @@ __device__ __forceinline__ void process_piece(const ExecParams& P, const DFlow& 
       // (dead-source discard is off for bf16 plans in the dataflow executor: measured 3 % slower on C3, which is not
       // DRAM-bound there; on in the column executor)
       const bool bf_dead = PolX::l1 != 0 && dead_src;
+      if (MASK_FWD) {   // (data runs: FWD = ExecParams.data_fwd, the tile is one round of CN / 2 units per thread)
+        constexpr int U = CN / 2;
+        const bool src_reg = use_carry && (f.flags & DFLOW_SRC_REG) != 0u;
+        const bool elide = (P.data_fwd & 2u) != 0u;
+        const bool ns = elide && (f.flags & DFLOW_NO_STORE) != 0u;
+        const bool dd = bf_dead && !(elide && (f.flags & DFLOW_SRC_FWD));
+        switch ((f.ksrc << 2) | (f.kdin << 1) | f.kdout) {
+          case 0: range_add_bf16_round<0, 0, 0, NT, U>(s, di, dout, vbeg, vend, pol, dd, src_reg, ns, stage, carry); break;
+          case 1: range_add_bf16_round<0, 0, 1, NT, U>(s, di, dout, vbeg, vend, pol, dd, src_reg, ns, stage, carry); break;
+          case 2: range_add_bf16_round<0, 1, 0, NT, U>(s, di, dout, vbeg, vend, pol, dd, src_reg, ns, stage, carry); break;
+          case 3: range_add_bf16_round<0, 1, 1, NT, U>(s, di, dout, vbeg, vend, pol, dd, src_reg, ns, stage, carry); break;
+          case 4: range_add_bf16_round<1, 0, 0, NT, U>(s, di, dout, vbeg, vend, pol, dd, src_reg, ns, stage, carry); break;
+          case 5: range_add_bf16_round<1, 0, 1, NT, U>(s, di, dout, vbeg, vend, pol, dd, src_reg, ns, stage, carry); break;
+          case 6: range_add_bf16_round<1, 1, 0, NT, U>(s, di, dout, vbeg, vend, pol, dd, src_reg, ns, stage, carry); break;
+          default: range_add_bf16_round<1, 1, 1, NT, U>(s, di, dout, vbeg, vend, pol, dd, src_reg, ns, stage, carry); break;
+        }
+      } else
       switch ((f.ksrc << 2) | (f.kdin << 1) | f.kdout) {
         case 0: range_add_bf16<0, 0, 0, NT>(s, di, dout, vbeg, vend, pol, bf_dead, stage); break;
         case 1: range_add_bf16<0, 0, 1, NT>(s, di, dout, vbeg, vend, pol, bf_dead, stage); break;
@@ -636,11 +665,11 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
         // Fast paths (the verifier is bound by instruction issue, ncu r02: 69-72 % of the issue slots): flows that touch
         // no memory from this thread skip everything else.  `ragged`: the tile holds the ragged end of a buffer, whose
         // last few elements always go through memory (process_piece's scalar tail).
-        if (MASK_FWD && !ragged && cur.op == 0 &&
+        if (MASK_FWD && is_mask_mode(MODE) && !ragged && cur.op == 0 &&
             (cur.flags & (DFLOW_SRC_FWD | DFLOW_DST_INIT | DFLOW_NO_STORE | DFLOW_FINAL | DFLOW_STAGE_OUT)) ==
                 (DFLOW_SRC_FWD | DFLOW_DST_INIT | DFLOW_NO_STORE)) {
           constexpr int EB = ModeTraits<MODE>::ESIZE;
-          mask_hop_in_registers<EB>(carry, mask_vector(cur.dst < 64 ? 1ull << cur.dst : 0ull, cur.dst >= 64 ? 1ull << (cur.dst - 64) : 0ull, EB),
+          mask_hop_in_registers<EB>(reinterpret_cast<uint4 (&)[4]>(carry), mask_vector(cur.dst < 64 ? 1ull << cur.dst : 0ull, cur.dst >= 64 ? 1ull << (cur.dst - 64) : 0ull, EB),
                                     nv, overlaps);
           return;
         }
@@ -735,7 +764,7 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
 // warp whose loads miss does not hold up thirteen others at the next barrier (the CTA-wide kernel spends a third of its
 // stall time there), short regions (C4 at large k: 273 units) keep every warp busy, and items are claimed per warp.
 // Records are read straight from the table (uniform loads, L1 hits after the first warp).  Everything else -- table
-// order per element, every flow's loads, add and store issued, first touches requested one flow ahead, dead-source
+// order per element, every flow's add carried out, partial sums forwarded in registers, first touches requested one flow ahead, dead-source
 // discard, the bulk all-gather path with one stage per warp -- is as in optcc_column_kernel.
 // ---------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ DFlow load_record(const DFlow* p) {
@@ -758,7 +787,9 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel
   pol.lds = pol0.lds; pol.ldd = pol0.ldd; pol.st = pol0.st;
   const bool bulk = P.col_bulk != 0;
   bool stage_ok = true;              // contributor masks: every staged set is the full set
-  uint4 carry[4];                    // lazy contributor-mask runs: what the previous flow produced (DFLOW_SRC_FWD)
+  // what the previous flow of the list produced for this lane's vectors (lazy contributor-mask runs: DFLOW_SRC_FWD; data
+  // runs: DFLOW_SRC_REG -- a bf16 unit is 8 fp32 values, four units per lane)
+  uint4 carry[MODE == MODE_BF16 ? 8 : 4];
   const unsigned long long bulk_pol = make_policy(P.col_bulk_policy);   // L2 policy of the bulk stores
   const bool pf = !is_mask_mode(MODE) && P.col_pf_dist != 0;
   // Items are dealt round-robin to the warps of the grid (neighbouring warps take neighbouring tiles): a global ticket
@@ -792,11 +823,11 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel
       const DFlow nxt = load_record(P.flows + (j + 1 < fe ? j + 1 : j));
       if (pf && j + 1 < fe) prefetch_raw<MODE, 32>(P, nxt, ubeg, item.w);   // first touches of the next flow
       // fast paths: flows that touch no memory from this lane (see optcc_column_kernel)
-      if (MASK_FWD && !ragged && cur.op == 0 &&
+      if (MASK_FWD && is_mask_mode(MODE) && !ragged && cur.op == 0 &&
           (cur.flags & (DFLOW_SRC_FWD | DFLOW_DST_INIT | DFLOW_NO_STORE | DFLOW_FINAL | DFLOW_STAGE_OUT)) ==
               (DFLOW_SRC_FWD | DFLOW_DST_INIT | DFLOW_NO_STORE)) {
         constexpr int EB = ModeTraits<MODE>::ESIZE;
-        mask_hop_in_registers<EB>(carry, mask_vector(cur.dst < 64 ? 1ull << cur.dst : 0ull, cur.dst >= 64 ? 1ull << (cur.dst - 64) : 0ull, EB),
+        mask_hop_in_registers<EB>(reinterpret_cast<uint4 (&)[4]>(carry), mask_vector(cur.dst < 64 ? 1ull << cur.dst : 0ull, cur.dst >= 64 ? 1ull << (cur.dst - 64) : 0ull, EB),
                                   nv, overlaps);
         cur = nxt;
         continue;
@@ -926,6 +957,85 @@ std::unordered_map<void*, uint64_t> g_ws_owner;
 std::atomic<uint64_t> g_next_id{1};
 }  // namespace
 
+namespace {
+// Page-locked host memory for the one big table that is built and uploaded again for every plan (the column executor's
+// records: 31 MB at C4 / k = 32).  A cudaMemcpyAsync from pageable memory is staged through the driver's bounce buffers
+// ON THE CALLING THREAD; from page-locked memory it is one DMA the host does not wait for.  Blocks go back to a small
+// process-wide cache (cudaHostAlloc costs more than the copy it saves; a job that plans every step reuses the block).
+// Without a driver (planning on a CPU box: optcc_column_tables), or when the calling thread forbids allocating CUDA
+// calls (optcc_execute_static), the memory is pageable, from optcc_raw_alloc.
+struct PinnedBlock { void* p; size_t bytes; };
+std::mutex g_pinned_mutex;
+std::vector<PinnedBlock> g_pinned_cache;
+constexpr size_t PINNED_MIN = size_t(1) << 20, PINNED_CACHE_BLOCKS = 4, PINNED_CACHE_MAX = size_t(512) << 20;
+thread_local bool tl_no_cuda_alloc = false;
+
+void* pinned_alloc(size_t bytes) {                       // nullptr: use pageable memory
+  if (bytes < PINNED_MIN || tl_no_cuda_alloc) return nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_pinned_mutex);
+    size_t best = SIZE_MAX;
+    for (size_t i = 0; i < g_pinned_cache.size(); ++i)
+      if (g_pinned_cache[i].bytes >= bytes && g_pinned_cache[i].bytes <= 2 * bytes &&
+          (best == SIZE_MAX || g_pinned_cache[i].bytes < g_pinned_cache[best].bytes)) best = i;
+    if (best != SIZE_MAX) {
+      void* q = g_pinned_cache[best].p;
+      g_pinned_cache.erase(g_pinned_cache.begin() + best);
+      return q;
+    }
+  }
+  void* q = nullptr;
+  if (cudaHostAlloc(&q, bytes, cudaHostAllocDefault) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  return q;
+}
+
+void pinned_free(void* q, size_t bytes) {
+  {
+    std::lock_guard<std::mutex> lock(g_pinned_mutex);
+    size_t total = bytes;
+    for (const auto& b : g_pinned_cache) total += b.bytes;
+    if (g_pinned_cache.size() < PINNED_CACHE_BLOCKS && total <= PINNED_CACHE_MAX) { g_pinned_cache.push_back(PinnedBlock{q, bytes}); return; }
+  }
+  cudaFreeHost(q);
+}
+
+template <class T>
+class HostTable {
+ public:
+  HostTable() = default;
+  HostTable(const HostTable&) = delete;
+  HostTable& operator=(const HostTable&) = delete;
+  ~HostTable() { release(); }
+  void release() {
+    if (p_) { if (pinned_) pinned_free(p_, cap_ * sizeof(T)); else optcc_raw_free(p_, cap_ * sizeof(T)); }
+    p_ = nullptr; n_ = cap_ = 0; pinned_ = false;
+  }
+  void resize_uninit(size_t n) {          // contents undefined; throws std::bad_alloc
+    if (n > cap_) {
+      release();
+      void* q = pinned_alloc(n * sizeof(T));
+      pinned_ = q != nullptr;
+      if (!q) q = optcc_raw_alloc(n * sizeof(T));
+      if (!q) throw std::bad_alloc();
+      p_ = static_cast<T*>(q);
+      cap_ = n;
+    }
+    n_ = n;
+  }
+  bool pinned() const { return pinned_; }
+  size_t size() const { return n_; }
+  bool empty() const { return n_ == 0; }
+  T* data() { return p_; }
+  const T* data() const { return p_; }
+  T& operator[](size_t i) { return p_[i]; }
+  const T& operator[](size_t i) const { return p_[i]; }
+ private:
+  T* p_ = nullptr;
+  size_t n_ = 0, cap_ = 0;
+  bool pinned_ = false;
+};
+}  // namespace
+
 struct optcc_exec_state {
   int device = -1;
   int sm_count = 0;
@@ -947,7 +1057,8 @@ struct optcc_exec_state {
   std::vector<uint64_t> step_op_begin;   // [n_steps + 1]
   // column executor
   bool column = false;
-  optcc_rawvec<DFlow> col_dflows;        // the executed flows, region by region (chain order inside a region)
+  HostTable<DFlow> col_dflows;           // the executed flows, region by region (chain order inside a region)
+  cudaEvent_t uploaded = nullptr;        // recorded after an upload from page-locked tables: they may not be recycled before it
   std::vector<uint32_t> col_reg_begin;   // [regions + 1]
   std::vector<uint4> col_items;          // (first flow, end flow, tile, units in the tile)
   std::vector<uint4> col_items_mask;     // the verifier's items when its tile size differs (plan's mask_tile_units)
@@ -961,6 +1072,11 @@ void optcc_exec_state_free(optcc_exec_state* s) {
     std::lock_guard<std::mutex> lock(g_ws_mutex);
     for (auto it = g_ws_owner.begin(); it != g_ws_owner.end();)
       it = it->second == s->id ? g_ws_owner.erase(it) : std::next(it);
+  }
+  if (s && s->uploaded) {   // a copy from the page-locked table may still be in flight: its block goes back to a cache
+    cudaEventSynchronize(s->uploaded);
+    cudaEventDestroy(s->uploaded);
+    cudaGetLastError();
   }
   delete s;
 }
@@ -1231,6 +1347,9 @@ bool finish_region(DFlow* L, uint32_t n, const ColBuildOpts& o, ColScratch& sc) 
     if (dead && i > 0 && L[i - 1].dst == f.src) {
       f.flags |= DFLOW_SRC_FWD;
     }
+    // data runs: the source range holds what the reduce flow just before this one stored -- with the same threads on the
+    // same vectors (one-round tiles, ExecParams.data_fwd) the operand is still in registers
+    if (f.op == OPTCC_OP_REDUCE && i > 0 && L[i - 1].op == OPTCC_OP_REDUCE && L[i - 1].dst == f.src) f.flags |= DFLOW_SRC_REG;
     sc.next[f.dst] = f.op == OPTCC_OP_COPY ? NEXT_COPY_WRITE : NEXT_REDUCE_WRITE;
     sc.next[f.src] = NEXT_READ;
   }
@@ -1638,6 +1757,14 @@ int upload_tables(optcc_plan_t* pl, void* workspace, cudaStream_t stream, bool f
     CU_TRY(cudaMemcpyAsync(ws + L.deps, st->deps.data(), st->deps.size() * sizeof(DDep), cudaMemcpyHostToDevice, stream));
     CU_TRY(cudaMemcpyAsync(ws + L.ops, st->ops.data(), st->ops.size() * sizeof(TileOp), cudaMemcpyHostToDevice, stream));
   }
+  if (st->column && st->col_dflows.pinned()) {
+    if (!st->uploaded && tl_no_cuda_alloc) {
+      CU_TRY(cudaStreamSynchronize(stream));   // (optcc_execute_static creates nothing: wait for the copy instead)
+    } else {
+      if (!st->uploaded) CU_TRY(cudaEventCreateWithFlags(&st->uploaded, cudaEventDisableTiming));
+      CU_TRY(cudaEventRecord(st->uploaded, stream));
+    }
+  }
   {
     std::lock_guard<std::mutex> lock(g_ws_mutex);
     g_ws_owner[workspace] = st->id;
@@ -1676,7 +1803,15 @@ int launch_plan(optcc_plan_t* pl, ExecParams& P, cudaStream_t stream) {
     P.col_stage_bytes = (unsigned int)tile_bytes;
     // partial sets are forwarded through registers when a thread's vectors are the same in every flow: one round at most
     P.mask_fwd = (is_mask_mode(MODE) && P.mask_lazy && tile_bytes / 16 <= size_t(4) * (P.col_warp ? 32 : COL_THREADS)) ? 1u : 0u;
-    constexpr bool MASKS = is_mask_mode(MODE);
+    // f32 sums likewise (DFLOW_SRC_REG): a reduce flow adds what the flow before it stored without loading it back
+    // (one-round tiles: four vectors per thread of f32; of bf16, two units per thread CTA-wide and four per lane warp-wide)
+    const size_t round_units = MODE == MODE_F32 ? size_t(4) * (P.col_warp ? 32 : COL_THREADS)
+                                                : (P.col_warp ? size_t(4) * 32 : size_t(2) * COL_THREADS);
+    if (!is_mask_mode(MODE)) {
+      P.data_fwd = (pl->opts.no_forward != 1 && P.tile_units <= round_units) ? (pl->opts.no_forward == 2 ? 1u : 3u) : 0u;
+      P.mask_fwd = P.data_fwd;                          // (one switch selects the forwarding instantiation below)
+    }
+    constexpr bool MASKS = true;                        // every mode has a forwarding instantiation
     if (P.col_warp) {
       // warp-wide tiles: one stage per warp; a CTA's 14 warps take items on their own
       const size_t dyn = P.col_bulk ? tile_bytes * (COL_THREADS / 32) : 0;
@@ -1850,7 +1985,8 @@ extern "C" int optcc_execute_static(optcc_plan_t* plan, void* const* bufs, void*
   // Same path as a caller workspace from here on.  The array keeps what the last call left in it: the tables are
   // uploaded again (control block cleared, stamp rewritten) whenever the last plan to use it was another one, and every
   // launch clears its own ticket / barrier / completion counters first (launch_plan), so nothing is assumed to be zero.
-  return optcc_execute(plan, bufs, ws, stream_);
+  struct NoAlloc { bool was = tl_no_cuda_alloc; NoAlloc() { tl_no_cuda_alloc = true; } ~NoAlloc() { tl_no_cuda_alloc = was; } } guard;
+  return optcc_execute(plan, bufs, ws, stream_);   // (tables this call has to build go to pageable host memory)
 }
 
 extern "C" int optcc_execute_host(optcc_plan_t* plan, const void* const* host_in, void* const* host_out,

@@ -51,11 +51,16 @@ enum : unsigned int {
   // column executor, data runs, bulk all-gather path (see build_column_tables / optcc_column_kernel):
   DFLOW_STAGE_OUT = 64u,   // reduce flow: the sum it stores is the source of later copy flows -- also keep it in the CTA's stage
   DFLOW_FROM_STAGE = 128u, // copy flow: the source range holds exactly the staged tile -- store it with cp.async.bulk
-  // column executor, contributor-mask runs in the lazy form only (the verifier's own arrays; data runs load and store
-  // every flow's operands as listed):
+  // column executor, one-round tiles (a thread handles the same vectors in every flow of the item): contributor-mask
+  // runs in the lazy form (ExecParams.mask_fwd) and data runs (ExecParams.data_fwd bit 1, opts.no_forward = 0):
   DFLOW_SRC_FWD = 256u,    // the source range was written by the previous flow of the list, this flow is its only
-                           // reader and the range is overwritten later: the sets are taken from the thread's registers
-  DFLOW_NO_STORE = 512u,   // ... and that previous flow does not store them (nobody would ever read them from memory)
+                           // reader and the range is overwritten later: the values are taken from the thread's registers
+  DFLOW_NO_STORE = 512u,   // ... and that previous flow does not store them (nobody would ever read them from memory;
+                           // never set on a final value, on the staged tile or on a copy the bulk path stores)
+  // column executor, data runs (ExecParams.data_fwd bit 0):
+  DFLOW_SRC_REG = 1024u,   // reduce flow whose source range is what the reduce flow just before it in the list produced:
+                           // every thread still holds exactly those vectors in registers and adds them instead of loading
+                           // them back through L1 (same bits whether or not that flow stored them)
 };
 
 struct __align__(16) Slice {      // start of a CTA's slice of a step: flow index and 16-byte unit inside it
@@ -123,6 +128,8 @@ struct ExecParams {
   unsigned int col_warp;          // 1: warp-wide tiles (optcc_wcolumn_kernel), 0: CTA-wide tiles (optcc_column_kernel)
   unsigned int col_stage_bytes;   // bytes of one staged tile (the warp-wide kernel keeps one per warp)
   unsigned int mask_fwd;          // lazy contributor-mask runs: act on DFLOW_SRC_FWD / DFLOW_NO_STORE
+  unsigned int data_fwd;          // data runs, one-round tiles: bit 0 = act on DFLOW_SRC_REG (range_add_f32_round /
+                                  // range_add_bf16_round), bit 1 = also on DFLOW_NO_STORE (dead partial sums stay in registers)
   unsigned int pad4;
   unsigned long long stamp;       // the launching plan's table stamp: a kernel whose workspace holds another one (the
                                   // memory was reused, or freed and allocated again at the same address) must not walk
@@ -316,6 +323,46 @@ __device__ __forceinline__ void range_add_f32(const char* __restrict__ s, char* 
       }
     };
     remainder_dispatch<UNROLL>(rem, batch);
+  }
+}
+
+// One round of range_add_f32 with forwarding (ExecParams.data_fwd: the tile is at most one round of four vectors per
+// thread, so a thread handles the same vectors in every flow of the item).  `carry` holds the sums this thread stored in
+// the previous flow of the list; with src_reg (DFLOW_SRC_REG: that flow's destination is this flow's source) they are
+// the source operand -- the load that would return the bits the thread has just stored is not issued.  The add and the
+// store to the destination range are issued as listed, so memory holds what the step-ordered executors leave there.
+template <int NT, bool STAGE, class PolX>
+__device__ __forceinline__ void range_add_f32_round(const char* __restrict__ s, char* __restrict__ d,
+                                                    unsigned long long vbeg, unsigned long long vend, const PolX& pol,
+                                                    bool dead_src, bool src_reg, char* stage, uint4 (&carry)[4], bool no_store = false) {
+  const unsigned long long v0 = vbeg + group_tid<NT>();
+  if (v0 >= vend) return;
+  auto batch = [&](auto K) {
+    constexpr int KK = decltype(K)::value;      // this thread's vectors in the tile: v0 + j NT, j < KK
+    uint4 b[KK];
+#pragma unroll
+    for (int j = 0; j < KK; ++j) b[j] = ld16(d + (v0 + j * (unsigned long long)NT) * 16, pol.ldd, pol.l1);
+    if (!src_reg) {
+#pragma unroll
+      for (int j = 0; j < KK; ++j) carry[j] = ld16(s + (v0 + j * (unsigned long long)NT) * 16, pol.lds, pol.l1);
+    }
+#pragma unroll
+    for (int j = 0; j < KK; ++j) {
+      const uint4 r = add_f32x4(b[j], carry[j]);
+      carry[j] = r;
+      if (!no_store) st16(d + (v0 + j * (unsigned long long)NT) * 16, r, pol);
+      if (STAGE) sts16(stage + (v0 + j * (unsigned long long)NT - vbeg) * 16, r);
+    }
+  };
+  if (v0 + 3 * (unsigned long long)NT < vend) {
+    batch(std::integral_constant<int, 4>());
+    // (only when every lane of the warp is in this round: the line's other vectors are this warp's too)
+    if (dead_src && (v0 - (threadIdx.x & 31u) + 31) + 3 * (unsigned long long)NT < vend) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) discard_line16(s + (v0 + j * (unsigned long long)NT) * 16, v0 + j * (unsigned long long)NT, vend);
+    }
+  } else {
+    remainder_dispatch<4>((unsigned int)((vend - v0 + NT - 1) / NT), batch);
   }
 }
 
@@ -696,6 +743,89 @@ __device__ __forceinline__ void range_add_bf16(const char* __restrict__ s, const
     for (int e = 0; e < 8; ++e) b[e] = __fadd_rn(b[e], a[e]);
     store8<KO>(dout, u, b, pol);
     if (KO == 0 && stage) sts16(stage + (u - ubeg) * 16, pack8_bf16(b));
+  }
+}
+
+// One round of range_add_bf16 with forwarding (ExecParams.data_fwd: the tile is at most one round of U units per thread).
+// `carry` holds, as 8 fp32 values per unit (two uint4), what this thread produced in the previous flow of the list:
+// with src_reg (DFLOW_SRC_REG) that is the source operand.  no_store (DFLOW_NO_STORE, fp32 partials only): the result is
+// read by the next flow from `carry` alone and its range is overwritten later, so the partial sum is not written to the
+// library's fp32 scratch at all.  Rank buffers see exactly the stores range_add_bf16 issues.
+// (the KK units of one thread: u0 + j NT, j < KK)
+template <int KS, int KD, int KO, int NT, int KK, int CN, class PolX>
+__device__ __forceinline__ void bf16_round_batch(const char* __restrict__ s, const char* __restrict__ din, char* __restrict__ dout,
+                                                 unsigned long long ubeg, unsigned long long u0, const PolX& pol, bool src_reg,
+                                                 bool no_store, char* stage, uint4 (&carry)[CN]) {
+  constexpr int W = KD ? 2 : 1;               // the destination operand stays packed until its unit is added
+  uint4 braw[KK][W];
+#pragma unroll
+  for (int j = 0; j < KK; ++j) {
+    const char* q = din + (u0 + j * (unsigned long long)NT) * (KD ? 32 : 16);
+    braw[j][0] = ld16(q, pol.ldd, pol.l1);
+    if (KD) braw[j][W - 1] = ld16(q + 16, pol.ldd, pol.l1);
+  }
+  if (!src_reg) {
+#pragma unroll
+    for (int j = 0; j < KK; ++j) {
+      const char* q = s + (u0 + j * (unsigned long long)NT) * (KS ? 32 : 16);
+      const uint4 r0 = ld16(q, pol.lds, pol.l1);
+      if (KS) {
+        carry[2 * j] = r0;
+        carry[2 * j + 1] = ld16(q + 16, pol.lds, pol.l1);
+      } else {
+        carry[2 * j] = make_uint4(r0.x << 16, r0.x & 0xFFFF0000u, r0.y << 16, r0.y & 0xFFFF0000u);
+        carry[2 * j + 1] = make_uint4(r0.z << 16, r0.z & 0xFFFF0000u, r0.w << 16, r0.w & 0xFFFF0000u);
+      }
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < KK; ++j) {
+    float b[8];
+    if (KD) {
+      b[0] = __uint_as_float(braw[j][0].x); b[1] = __uint_as_float(braw[j][0].y); b[2] = __uint_as_float(braw[j][0].z); b[3] = __uint_as_float(braw[j][0].w);
+      b[4] = __uint_as_float(braw[j][W - 1].x); b[5] = __uint_as_float(braw[j][W - 1].y); b[6] = __uint_as_float(braw[j][W - 1].z); b[7] = __uint_as_float(braw[j][W - 1].w);
+    } else {
+      const uint4 r = braw[j][0];
+      b[0] = bf16_to_f32(r.x & 0xFFFFu); b[1] = bf16_to_f32(r.x >> 16); b[2] = bf16_to_f32(r.y & 0xFFFFu); b[3] = bf16_to_f32(r.y >> 16);
+      b[4] = bf16_to_f32(r.z & 0xFFFFu); b[5] = bf16_to_f32(r.z >> 16); b[6] = bf16_to_f32(r.w & 0xFFFFu); b[7] = bf16_to_f32(r.w >> 16);
+    }
+    const uint4 c0 = carry[2 * j], c1 = carry[2 * j + 1];
+    b[0] = __fadd_rn(b[0], __uint_as_float(c0.x)); b[1] = __fadd_rn(b[1], __uint_as_float(c0.y));
+    b[2] = __fadd_rn(b[2], __uint_as_float(c0.z)); b[3] = __fadd_rn(b[3], __uint_as_float(c0.w));
+    b[4] = __fadd_rn(b[4], __uint_as_float(c1.x)); b[5] = __fadd_rn(b[5], __uint_as_float(c1.y));
+    b[6] = __fadd_rn(b[6], __uint_as_float(c1.z)); b[7] = __fadd_rn(b[7], __uint_as_float(c1.w));
+    if (KO == 0) {   // the complete sum is rounded when it is stored: `carry` holds what a load of it would return
+#pragma unroll
+      for (int e = 0; e < 8; ++e) b[e] = bf16_to_f32(f32_to_bf16_rne(b[e]));
+    }
+    carry[2 * j] = make_uint4(__float_as_uint(b[0]), __float_as_uint(b[1]), __float_as_uint(b[2]), __float_as_uint(b[3]));
+    carry[2 * j + 1] = make_uint4(__float_as_uint(b[4]), __float_as_uint(b[5]), __float_as_uint(b[6]), __float_as_uint(b[7]));
+    if (!no_store) store8<KO>(dout, u0 + j * (unsigned long long)NT, b, pol);
+    if (KO == 0 && stage) sts16(stage + (u0 + j * (unsigned long long)NT - ubeg) * 16, pack8_bf16(b));
+  }
+}
+
+template <int KS, int KD, int KO, int NT, int U, class PolX>
+__device__ __forceinline__ void range_add_bf16_round(const char* __restrict__ s, const char* __restrict__ din,
+                                                     char* __restrict__ dout, unsigned long long ubeg, unsigned long long uend,
+                                                     const PolX& pol, bool dead_src, bool src_reg, bool no_store, char* stage,
+                                                     uint4 (&carry)[2 * U]) {
+  const unsigned long long u0 = ubeg + group_tid<NT>();
+  if (u0 >= uend) return;
+  if (u0 + (U - 1) * (unsigned long long)NT < uend) {
+    bf16_round_batch<KS, KD, KO, NT, U>(s, din, dout, ubeg, u0, pol, src_reg, no_store, stage, carry);
+    if (dead_src && (u0 - (threadIdx.x & 31u) + 31) + (U - 1) * (unsigned long long)NT < uend) {
+#pragma unroll
+      for (int j = 0; j < U; ++j) {
+        const unsigned long long uu = u0 + j * (unsigned long long)NT;
+        if (KS == 0) discard_line16(s + uu * 16, uu, uend); else discard_line32(s + uu * 32, uu, uend);
+      }
+    }
+  } else {
+    const unsigned int rem = (unsigned int)((uend - u0 + NT - 1) / NT);
+    if (U > 3 && rem >= 3) bf16_round_batch<KS, KD, KO, NT, (U > 3 ? 3 : 1)>(s, din, dout, ubeg, u0, pol, src_reg, no_store, stage, carry);
+    else if (U > 2 && rem == 2) bf16_round_batch<KS, KD, KO, NT, (U > 2 ? 2 : 1)>(s, din, dout, ubeg, u0, pol, src_reg, no_store, stage, carry);
+    else bf16_round_batch<KS, KD, KO, NT, 1>(s, din, dout, ubeg, u0, pol, src_reg, no_store, stage, carry);
   }
 }
 

@@ -12,7 +12,7 @@ from paper_2606_01680_b200 import workloads as W
 from oracle import planner as OP
 from oracle import interpreter as OI
 
-DEAD_SRC, SRC_INIT, DST_INIT, FINAL, STAGE_OUT, FROM_STAGE, SRC_FWD, NO_STORE = 1, 2, 4, 8, 64, 128, 256, 512
+DEAD_SRC, SRC_INIT, DST_INIT, FINAL, STAGE_OUT, FROM_STAGE, SRC_FWD, NO_STORE, SRC_REG = 1, 2, 4, 8, 64, 128, 256, 512, 1024
 
 
 def _simulate(plan, x, bulk=True, fwd=False):
@@ -49,6 +49,12 @@ def _simulate(plan, x, bulk=True, fwd=False):
             assert not final_seen[d], "a flow writes a range after its DFLOW_FINAL write"
             src = shadow[s, a:b] if (bf16 and f["ksrc"]) else buf[s, a:b]
             if fwd and (fl & SRC_FWD):
+                src = prev
+            if fl & SRC_REG:   # data runs: the registers the previous (reduce) flow stored are this flow's source operand
+                assert i > 0 and f["op"] == 0 and L[i - 1]["op"] == 0 and int(L[i - 1]["dst"]) == s
+                assert not bf16 or int(L[i - 1]["kdout"]) == int(f["ksrc"])
+                if not fwd:
+                    assert src.tobytes() == prev.tobytes()     # memory holds the same bits: the store was issued
                 src = prev
             if f["op"] == 0:
                 din = shadow[d, a:b] if (bf16 and f["kdin"]) else buf[d, a:b]
@@ -116,9 +122,10 @@ def test_column_tables_reproduce_the_oracle(case):
     y, items, lists = _simulate(plan, x, bulk=extra.get("copy_path", 0) != 1)
     y_or = OI.run_f32(oplan, x) if dtype == W.F32 else OI.run_bf16(oplan, x)
     assert y.tobytes() == y_or.tobytes()
-    if dtype == W.F32:     # the verifier's forwarding flags, interpreted on data: same outputs, partial sums never stored
-        y2, _, _ = _simulate(plan, x, bulk=extra.get("copy_path", 0) != 1, fwd=True)
-        assert y2.tobytes() == y_or.tobytes()
+    # the forwarding flags as the default data run (opts.no_forward = 0) and the lazy verifier act on them: a partial sum
+    # with DFLOW_NO_STORE is never stored (its range is poisoned here), the flow after it takes it from registers
+    y2, _, _ = _simulate(plan, x, bulk=extra.get("copy_path", 0) != 1, fwd=True)
+    assert y2.tobytes() == y_or.tobytes()
     rec, _ = B.optcc_column_tables(plan)
     if extra.get("copy_path", 0) == 1:
         assert not (rec["flags"] & (STAGE_OUT | FROM_STAGE)).any()
@@ -149,7 +156,7 @@ def test_column_tables_of_a_truncated_schedule(case, frac):
     limit = max(1, int(oplan.n_steps * frac))
     plan = B.optcc_plan(p, g, ell, n, dtype, k=k, exec_mode=B.OPTCC_EXEC_COLUMN, step_limit=limit, **extra)
     x = W.all_inputs(W.Workload("t", p, g, tuple(ell), n, dtype, "normal", 1.0, 500 + case))
-    y, _, _ = _simulate(plan, x)
+    y, _, _ = _simulate(plan, x, fwd=True)    # as the default data run: unstored partial sums are poisoned
     rec, _ = B.optcc_column_tables(plan)
     assert not (rec["flags"] & DEAD_SRC).any()
     prefix = dataclasses.replace(oplan, n_steps=limit, flows=oplan.flows[:int(oplan.step_begin[limit])],
@@ -188,3 +195,18 @@ def test_auto_executor_is_reported():
     assert plan.info["exec_mode"] == B.OPTCC_EXEC_DATAFLOW
     with pytest.raises(B.OptccError):
         B.optcc_column_tables(plan)
+
+
+def test_ring_hops_take_their_source_from_registers():
+    """DFLOW_SRC_REG: in a chain-ordered list every reduce hop after the first follows the flow that stored its source
+    (plain ring: p - 1 reduce flows per region, p - 2 of them flagged); in table order with k > 1 nothing changes for a
+    ring either (one chain per region), and copies are never flagged."""
+    p, n = 6, 7777
+    plan = B.optcc_plan(p, 1, [1.0] * p, n, W.F32, k=0, exec_mode=B.OPTCC_EXEC_COLUMN)
+    rec, items = B.optcc_column_tables(plan)
+    lists = sorted({(int(i["first"]), int(i["end"])) for i in items})
+    for first, end in lists:
+        L = rec[first:end]
+        red = L[L["op"] == 0]
+        assert len(red) == p - 1 and int(((red["flags"] & SRC_REG) != 0).sum()) == p - 2
+        assert not (L["flags"][L["op"] == 1] & SRC_REG).any()

@@ -32,8 +32,8 @@ def _wl(p, g, st, n, dtype, seed, dist="normal"):
     return W.Workload(f"t{p}x{n}", p, g, ell, n, dtype, dist, 1.0, seed)
 
 
-def _run_and_check(w, k, exec_mode, grid_ctas=0):
-    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=k, exec_mode=exec_mode, grid_ctas=grid_ctas)
+def _run_and_check(w, k, exec_mode, grid_ctas=0, **opts):
+    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=k, exec_mode=exec_mode, grid_ctas=grid_ctas, **opts)
     oplan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=k)
     x = W.all_inputs(w)
     s = _session(plan)
@@ -89,6 +89,31 @@ BF16_CASES = [
 @pytest.mark.parametrize("p,g,st,n,k", BF16_CASES)
 def test_bf16_parity(p, g, st, n, k, exec_mode):
     _run_and_check(_wl(p, g, st, n, W.BF16, seed=200 + p), k, exec_mode)
+
+
+# Column executor, opts.no_forward: 0 = partial sums travel between consecutive flows of a column in registers and a
+# partial sum nobody else reads is not stored; 1 = every flow loads both operands and stores its result; 2 = registers
+# are forwarded, every result is stored.  Tile sizes: CTA-wide one-round tiles (1792 units f32 / 896 bf16), warp-wide
+# tiles (128), and tiles of more than one round (3584: the forwarding instantiation is not used).
+FWD_CASES = [
+    # p, g, stragglers, n, dtype, k, tile_units
+    (16, 1, {0: 8.0 / 7.0}, 2 ** 21 + 6, W.F32, 4, 0),        # C2 shape: regions of several CTA-wide tiles + a short one
+    (16, 1, {0: 8.0 / 7.0}, 2 ** 17 + 2, W.F32, 8, 0),        # warp-wide tiles
+    (5, 1, {2: 1.5}, 500001, W.F32, 4, 1792),                 # bubble filling, ragged end inside a CTA-wide tile
+    (7, 1, {0: 2.0, 1: 4.0 / 3.0}, 655390, W.F32, 4, 3584),   # two rounds per tile
+    (16, 4, {r: 2.0 for r in range(4)}, 400001, W.F32, 4, 0), # g > 1: collect / NIC / distribute chains
+    (64, 1, {5: 8.0 / 7.0, 17: 4.0 / 3.0, 40: 2.0}, 2 ** 20 + 24, W.BF16, 4, 0),   # C3 shape, fp32 partials, warp-wide
+    (64, 1, {5: 8.0 / 7.0, 17: 4.0 / 3.0, 40: 2.0}, 2 ** 20 + 24, W.BF16, 4, 896), # CTA-wide
+    (5, 1, {2: 1.5}, 500003, W.BF16, 4, 0),
+    (12, 2, {0: 1.5, 1: 1.5}, 409700, W.BF16, 12, 1792),      # bf16 tiles of two rounds
+]
+
+
+@pytest.mark.parametrize("no_forward", [0, 1, 2])
+@pytest.mark.parametrize("case", range(len(FWD_CASES)))
+def test_column_executor_forwarding_modes_give_the_oracle_bits(case, no_forward):
+    p, g, st, n, dtype, k, tile = FWD_CASES[case]
+    _run_and_check(_wl(p, g, st, n, dtype, seed=700 + case), k, B.OPTCC_EXEC_COLUMN, tile_units=tile, no_forward=no_forward)
 
 
 @pytest.mark.parametrize("exec_mode", [B.OPTCC_EXEC_PERSISTENT, B.OPTCC_EXEC_DATAFLOW])
@@ -498,9 +523,10 @@ def test_truncated_schedule_data_equals_oracle_prefix(case, exec_mode):
     """"Steps exactly as the plan lists them" (north_star; PAPER.md:138 data dependencies), made observable: after the
     first t steps (opts.step_limit = t) EVERY element of EVERY rank buffer must hold exactly what the oracle holds
     after walking the table rows of steps < t -- the intermediate state of the p memories, not only the final one.
-    In particular the column executor, which runs a tile's flows in table order without any global step order, must
-    have materialised every flow's destination in memory, and nothing may have been dropped from the caches on the
-    assumption that a later step overwrites it."""
+    In particular the column executor, which runs a tile's flows in table order without any global step order and keeps
+    partial sums in registers between consecutive flows, must have stored every destination that no later EXECUTED flow
+    overwrites, and nothing may have been elided or dropped from the caches on the assumption that a step beyond the
+    cut overwrites it."""
     p, g, st, n, k, tile = TRUNC_CASES[case]
     w = _wl(p, g, st, n, W.F32, seed=4242 + case)
     oplan = OP.build_plan(p, g, list(w.ell), n, W.F32, k=k)
