@@ -39,36 +39,54 @@ extern "C" int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* p
   double T = 0.0;
   const uint32_t r_str = m ? plan->stragglers[0] * g : 0;
   double sent = 0.0, recvd = 0.0;
-  for (size_t i = 0; i < plan->flows.size(); ++i) {
-    const optcc_flow_t& f = plan->flows[i];
-    const size_t reg = plan->flow_region[i];
-    double dur;
-    if (f.link == OPTCC_LINK_NIC)
-      dur = alpha + beta * double(f.len) * std::max(plan->ell[f.src], plan->ell[f.dst]);
-    else
-      dur = alpha + beta * double(f.len) / double(g - 1);
-    double& sf = send_free[size_t(f.src) * 2 + f.link];
-    double& rf = recv_free[size_t(f.dst) * 2 + f.link];
+  const size_t nf = plan->flows.size();
+  const double nv_per_elem = g > 1 ? beta / double(g - 1) : 0.0;   // NVLink lane: (g-1)x NIC speed (one division, not one per flow)
+  const optcc_flow_t* const flows = plan->flows.data();
+  const uint32_t* const fregion = plan->flow_region.data();
+  const double* const ell = plan->ell.data();
+  RangeTimes* const rtp = rt.data();
+  double* const sfree = send_free.data();
+  double* const rfree = recv_free.data();
+  // The table lists the flows of a step by (link, stage, src, dst, off): runs of flows leave the same port one after
+  // another (and often enter the same port), so a port's time is a serial (max, +) chain from flow to flow.  Both are carried
+  // in registers for the length of the run (written back when the port changes) -- the loop is bound by that chain, not by memory.
+  size_t cur_port = SIZE_MAX, cur_rport = SIZE_MAX;
+  double sf = 0.0, rf = 0.0;
+  for (size_t i = 0; i < nf; ++i) {
+    const optcc_flow_t& f = flows[i];
+    const size_t reg = fregion[i];
+    const size_t port = size_t(f.src) * 2 + f.link;
+    if (port != cur_port) {
+      if (cur_port != SIZE_MAX) sfree[cur_port] = sf;
+      cur_port = port;
+      sf = sfree[port];
+    }
+    const double dur = alpha + (f.link == OPTCC_LINK_NIC ? beta * double(f.len) * std::max(ell[f.src], ell[f.dst])
+                                                         : double(f.len) * nv_per_elem);
+    const size_t rport = size_t(f.dst) * 2 + f.link;
+    if (rport != cur_rport) {
+      if (cur_rport != SIZE_MAX) rfree[cur_rport] = rf;
+      cur_rport = rport;
+      rf = rfree[rport];
+    }
     // (region-major: the regions of a few segments are active at a time, so their p entries stay in the cache)
-    RangeTimes& S = rt[reg * p + f.src];
-    RangeTimes& D = rt[reg * p + f.dst];
-    double& ws = S.wfin;
-    double& wd = D.wfin;
-    double& rd = D.rfin;
-    double& rs = S.rfin;
-    const double dep = std::max(ws, std::max(wd, rd));         // data dependencies
-    double start = std::max(std::max(sf, rf), dep > 0.0 ? dep + sync : 0.0);
-    double fin = start + dur;
+    RangeTimes& S = rtp[reg * p + f.src];
+    RangeTimes& D = rtp[reg * p + f.dst];
+    const double dep = std::max(S.wfin, std::max(D.wfin, D.rfin));   // data dependencies
+    const double other = std::max(rf, dep > 0.0 ? dep + sync : 0.0);
+    const double fin = std::max(sf, other) + dur;
     sf = fin;
     rf = fin;
-    rs = std::max(rs, fin);
-    wd = fin + alat;                                            // usable alpha_latency after the transfer
+    S.rfin = std::max(S.rfin, fin);
+    D.wfin = fin + alat;                                             // usable alpha_latency after the transfer
     T = std::max(T, fin + alat);
     if (m && f.link == OPTCC_LINK_NIC) {
       if (f.src == r_str) sent += double(f.len);
       if (f.dst == r_str) recvd += double(f.len);
     }
   }
+  if (cur_port != SIZE_MAX) sfree[cur_port] = sf;
+  if (cur_rport != SIZE_MAX) rfree[cur_rport] = rf;
 
   // ---- closed forms ----
   optcc_cost_t c;
