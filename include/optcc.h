@@ -289,6 +289,36 @@ OPTCC_API int optcc_execute_host_sharded(optcc_plan_t* plan, uint64_t n_total, c
 #define OPTCC_STATIC_WORKSPACE_BYTES (8u << 20)
 OPTCC_API int optcc_execute_static(optcc_plan_t* plan, void* const* bufs, void* stream);
 
+/* ---- ranks on several GPUs of one NVLink / NVSwitch domain -------------
+ * One process per GPU.  Every process owns the buffers of some of the p ranks (optcc_peer_alloc: device memory plus a
+ * 64-byte handle other processes can open), exchanges the handles with the others by whatever means it has (the Python
+ * binding uses torch.distributed), opens theirs (optcc_peer_open) and so holds p device pointers: its own ranks' in
+ * local HBM, the others' mapped over NVLink.  The path shards along the element axis (no flow mixes two element
+ * indices), so G processes split the WORK ITEMS of the column executor: optcc_execute_shard(..., s, S) takes the tiles
+ * i = s (mod S) of the plan through their whole flow lists exactly as optcc_execute does -- the loads of a flow whose
+ * source rank lives on another GPU and the stores of a flow whose destination does are peer accesses, the transfer
+ * overlaps the adds tile by tile, and there is no separate collective call.  When all S shards have run (the caller
+ * joins them: stream synchronisation + a barrier among the processes) every rank buffer on every GPU holds the
+ * AllReduce result, bit-identical to optcc_execute's.  Before the call every process's inputs must be in place (a
+ * barrier), and nobody may touch a rank buffer until all shards are done.  shard = 0, n_shards = 1 is optcc_execute.
+ * workspace: local to the calling process, as for optcc_execute.  optcc_verify_shard checks the contributor masks of
+ * the shard's own tiles on arrays in the local workspace (lazy form only, else EUNSUPPORTED); `checked` counts them.
+ * Errors: EINVAL (shard >= n_shards), EUNSUPPORTED (n_shards > 1 with another executor than the column executor), ECUDA.
+ * Status: the host logic and the kernels run under test with two processes sharing ONE GPU (handles opened across
+ * processes; tests/test_peer_shards.py); no box of this pool has a second GPU, so nothing here is measured over NVLink. */
+OPTCC_API int optcc_execute_shard(optcc_plan_t* plan, void* const* bufs, void* workspace, void* stream, uint32_t shard,
+                                  uint32_t n_shards);
+OPTCC_API int optcc_verify_shard(optcc_plan_t* plan, void* workspace, void* stream, uint32_t shard, uint32_t n_shards,
+                                 optcc_verify_result_t* out);
+/* dev_ptr [out]: cudaMalloc'ed memory of `bytes` bytes on the current device; handle64 [out, host, 64 bytes]: its
+ * cudaIpcMemHandle_t, valid in other processes of this machine.  optcc_peer_open maps such a handle (of ANOTHER process)
+ * into the calling process; optcc_peer_close unmaps it; optcc_peer_free frees what optcc_peer_alloc returned (after
+ * every peer has closed it). */
+OPTCC_API int optcc_peer_alloc(uint64_t bytes, void** dev_ptr, void* handle64);
+OPTCC_API int optcc_peer_open(const void* handle64, void** dev_ptr);
+OPTCC_API int optcc_peer_close(void* dev_ptr);
+OPTCC_API int optcc_peer_free(void* dev_ptr);
+
 /* Workspace contract.  optcc_prepare (and the first optcc_execute / optcc_verify with a workspace) writes the plan's
  * tables AND a stamp into the workspace; the library remembers per workspace address which plan's tables it holds, so
  * later calls skip the upload.  If the caller reuses that memory for something else in between (or frees it and gets

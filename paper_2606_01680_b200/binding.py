@@ -69,7 +69,7 @@ class OptccError(RuntimeError):
 
 _lib = None
 EXPORTS = ("optcc_plan", "optcc_plan_ex", "optcc_plan_destroy", "optcc_plan_info", "optcc_plan_tables", "optcc_cost",
-           "optcc_prepare", "optcc_column_tables", "optcc_execute", "optcc_execute_static", "optcc_execute_host", "optcc_execute_host_sharded", "optcc_workspace_check", "optcc_workspace_forget",
+           "optcc_prepare", "optcc_column_tables", "optcc_execute", "optcc_execute_static", "optcc_execute_shard", "optcc_verify_shard", "optcc_peer_alloc", "optcc_peer_open", "optcc_peer_close", "optcc_peer_free", "optcc_execute_host", "optcc_execute_host_sharded", "optcc_workspace_check", "optcc_workspace_forget",
            "optcc_verify", "optcc_strerror",
            "optcc_last_cuda_error", "optcc_abi_version")
 
@@ -95,6 +95,12 @@ def load():
     lib.optcc_column_tables.argtypes = [vp, C.POINTER(vp), C.POINTER(C.c_uint32), C.POINTER(vp), C.POINTER(C.c_uint32)]
     lib.optcc_execute.argtypes = [vp, C.POINTER(vp), vp, vp]
     lib.optcc_execute_static.argtypes = [vp, C.POINTER(vp), vp]
+    lib.optcc_execute_shard.argtypes = [vp, C.POINTER(vp), vp, vp, C.c_uint32, C.c_uint32]
+    lib.optcc_verify_shard.argtypes = [vp, vp, vp, C.c_uint32, C.c_uint32, C.POINTER(optcc_verify_result_t)]
+    lib.optcc_peer_alloc.argtypes = [u64, C.POINTER(vp), C.c_char_p]
+    lib.optcc_peer_open.argtypes = [C.c_char_p, C.POINTER(vp)]
+    lib.optcc_peer_close.argtypes = [vp]
+    lib.optcc_peer_free.argtypes = [vp]
     lib.optcc_execute_host.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), vp, vp]
     lib.optcc_execute_host_sharded.argtypes = [vp, u64, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), vp, vp]
     lib.optcc_verify.argtypes = [vp, vp, vp, C.POINTER(optcc_verify_result_t)]
@@ -239,6 +245,51 @@ def optcc_execute_static(plan, bufs, stream=None):
     rc = load().optcc_execute_static(plan.handle, _ptr_array(bufs), _ptr(stream))
     if rc:
         raise OptccError(rc, "optcc_execute_static")
+
+
+def optcc_execute_shard(plan, bufs, workspace, shard, n_shards, stream=None):
+    """The work items i = shard (mod n_shards) of the plan; bufs may be peer-mapped pointers (see peers.py)."""
+    rc = load().optcc_execute_shard(plan.handle, _ptr_array(bufs), _ptr(workspace), _ptr(stream), int(shard), int(n_shards))
+    if rc:
+        raise OptccError(rc, "optcc_execute_shard")
+
+
+def optcc_verify_shard(plan, workspace, shard, n_shards, stream=None, raise_on_fail=True):
+    out = optcc_verify_result_t()
+    rc = load().optcc_verify_shard(plan.handle, _ptr(workspace), _ptr(stream), int(shard), int(n_shards), C.byref(out))
+    if rc and (rc != OPTCC_EVERIFY or raise_on_fail):
+        raise OptccError(rc, "optcc_verify_shard")
+    return _struct_dict(out)
+
+
+def optcc_peer_alloc(nbytes):
+    """-> (device pointer, 64-byte handle other processes can open)"""
+    ptr = C.c_void_p()
+    handle = C.create_string_buffer(64)
+    rc = load().optcc_peer_alloc(int(nbytes), C.byref(ptr), handle)
+    if rc:
+        raise OptccError(rc, "optcc_peer_alloc")
+    return ptr.value, handle.raw
+
+
+def optcc_peer_open(handle):
+    ptr = C.c_void_p()
+    rc = load().optcc_peer_open(C.create_string_buffer(bytes(handle), 64), C.byref(ptr))
+    if rc:
+        raise OptccError(rc, "optcc_peer_open")
+    return ptr.value
+
+
+def optcc_peer_close(ptr):
+    rc = load().optcc_peer_close(int(ptr))
+    if rc:
+        raise OptccError(rc, "optcc_peer_close")
+
+
+def optcc_peer_free(ptr):
+    rc = load().optcc_peer_free(int(ptr))
+    if rc:
+        raise OptccError(rc, "optcc_peer_free")
 
 
 def optcc_execute_host(plan, host_in, host_out, bufs, workspace, stream=None):

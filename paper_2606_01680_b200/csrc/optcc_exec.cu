@@ -612,7 +612,7 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
   for (unsigned int round = 0; it < P.col_n_items; ++round) {
     // one record per item: the region's flows [fb, fe), the tile and its length in units (all flows over a region have
     // the same length, PLAN_SPEC 5.4, so the tile's unit range is fixed for the item)
-    const uint4 item = __ldg(P.col_items + it);
+    const uint4 item = __ldg(P.col_items + (it * P.item_stride + P.item_first));
     const unsigned int fb = item.x, fe = item.y;
     const unsigned long long ubeg = (unsigned long long)item.z * P.tile_units;
     const unsigned long long uend = ubeg + item.w;
@@ -620,7 +620,7 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
     unsigned long long n_ubeg = 0;
     unsigned int n_cnt = 0, n_units = 0, n_fb = 0;
     if (D && P.col_pf_next && nit < P.col_n_items) {
-      const uint4 ni = __ldg(P.col_items + nit);
+      const uint4 ni = __ldg(P.col_items + (nit * P.item_stride + P.item_first));
       n_fb = ni.x;
       n_cnt = ni.y - ni.x < D ? ni.y - ni.x : D;
       n_ubeg = (unsigned long long)ni.z * P.tile_units;
@@ -797,7 +797,7 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel
   // (measured: 131 k items -> 11.7 ms), more than the items' own work.
   const unsigned long long n_warps = (unsigned long long)gridDim.x * (COL_THREADS / 32);
   for (unsigned long long it = (unsigned long long)blockIdx.x * (COL_THREADS / 32) + warp; it < P.col_n_items; it += n_warps) {
-    const uint4 item = __ldg(P.col_items + it);
+    const uint4 item = __ldg(P.col_items + (it * P.item_stride + P.item_first));
     const unsigned int fb = item.x, fe = item.y;
     const unsigned long long ubeg = (unsigned long long)item.z * P.tile_units, uend = ubeg + item.w;
     DFlow cur = load_record(P.flows + fb);
@@ -1794,6 +1794,8 @@ int launch_plan(optcc_plan_t* pl, ExecParams& P, cudaStream_t stream) {
       P.tile_units = pl->mask_tile_units;
     }
     P.col_n_items = own_items ? st->col_items_mask.size() : st->col_items.size();
+    if (P.item_stride > 1)   // one shard of the items (the others run on peer GPUs, or in other calls)
+      P.col_n_items = P.col_n_items > P.item_first ? (P.col_n_items - P.item_first + P.item_stride - 1) / P.item_stride : 0;
     if (P.col_n_items == 0) return OPTCC_OK;
     CU_TRY(cudaMemsetAsync(&P.ctrl->ticket, 0, sizeof(unsigned long long), stream));
     const uint32_t G = pl->opts.grid_ctas ? pl->opts.grid_ctas : uint32_t(st->sm_count) * CTAS_PER_SM;
@@ -1879,6 +1881,8 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   P.counters = reinterpret_cast<unsigned int*>(ws + L.counters);
   P.col_items = reinterpret_cast<const uint4*>(ws + L.col);
   P.col_n_items = 0;
+  P.item_first = 0;
+  P.item_stride = 1;
   P.tile_units = pl->tile_units;
   P.bulk_copy = pl->opts.copy_path == 2 ? 1u : 0u;
   P.l2_hints = 1;   // source loads evict_first, destination loads and stores evict_normal (measured best)
@@ -1928,7 +1932,20 @@ extern "C" int optcc_prepare(optcc_plan_t* plan, void* workspace, void* stream) 
   return prepare_impl(plan, workspace, stream, true);
 }
 
+namespace {
+int execute_impl(optcc_plan_t* plan, void* const* bufs, void* workspace, void* stream_, uint32_t shard, uint32_t n_shards);
+}
 extern "C" int optcc_execute(optcc_plan_t* plan, void* const* bufs, void* workspace, void* stream_) {
+  return execute_impl(plan, bufs, workspace, stream_, 0, 1);
+}
+extern "C" int optcc_execute_shard(optcc_plan_t* plan, void* const* bufs, void* workspace, void* stream_, uint32_t shard,
+                                   uint32_t n_shards) {
+  if (!plan || n_shards == 0 || shard >= n_shards) return OPTCC_EINVAL;
+  if (n_shards > 1 && plan->opts.exec_mode != OPTCC_EXEC_COLUMN) return OPTCC_EUNSUPPORTED;   // only the column executor has independent items
+  return execute_impl(plan, bufs, workspace, stream_, shard, n_shards);
+}
+namespace {
+int execute_impl(optcc_plan_t* plan, void* const* bufs, void* workspace, void* stream_, uint32_t shard, uint32_t n_shards) {
   if (!plan || !bufs || !workspace) return OPTCC_EINVAL;
   const optcc_plan_info_t& in = plan->info;
   for (uint32_t r = 0; r < in.p; ++r)
@@ -1946,8 +1963,11 @@ extern "C" int optcc_execute(optcc_plan_t* plan, void* const* bufs, void* worksp
     CU_TRY(cudaMemcpyAsync(ws + L.ptrs, bufs, size_t(in.p) * sizeof(void*), cudaMemcpyHostToDevice, stream));
     P.ptr_table = reinterpret_cast<void* const*>(ws + L.ptrs);
   }
+  P.item_first = shard;
+  P.item_stride = n_shards;
   return in.dtype == OPTCC_F32 ? launch_plan<MODE_F32>(plan, P, stream) : launch_plan<MODE_BF16>(plan, P, stream);
 }
+}  // namespace
 
 // ---- optcc_execute_static: optcc_execute for callers that cannot allocate device memory --------------------------
 // The workspace (control block, executor tables, dataflow counters, bf16 fp32 partials) is this file-scope array instead
@@ -2101,13 +2121,29 @@ extern "C" int optcc_execute_host_sharded(optcc_plan_t* plan, uint64_t n_total, 
   return rc;
 }
 
+namespace {
+int verify_impl(optcc_plan_t* plan, void* workspace, void* stream_, optcc_verify_result_t* out, uint32_t shard, uint32_t n_shards);
+}
 extern "C" int optcc_verify(optcc_plan_t* plan, void* workspace, void* stream_, optcc_verify_result_t* out) {
+  return verify_impl(plan, workspace, stream_, out, 0, 1);
+}
+extern "C" int optcc_verify_shard(optcc_plan_t* plan, void* workspace, void* stream_, uint32_t shard, uint32_t n_shards,
+                                  optcc_verify_result_t* out) {
+  if (!plan || n_shards == 0 || shard >= n_shards) return OPTCC_EINVAL;
+  if (n_shards > 1 && plan->opts.exec_mode != OPTCC_EXEC_COLUMN) return OPTCC_EUNSUPPORTED;
+  return verify_impl(plan, workspace, stream_, out, shard, n_shards);
+}
+namespace {
+int verify_impl(optcc_plan_t* plan, void* workspace, void* stream_, optcc_verify_result_t* out, uint32_t shard, uint32_t n_shards) {
   if (!plan || !workspace || !out) return OPTCC_EINVAL;
   const optcc_plan_info_t& in = plan->info;
   if (in.mask_bytes == 0) return OPTCC_EUNSUPPORTED;
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   int rc = prepare_impl(plan, workspace, stream_, false);
   if (rc != OPTCC_OK) return rc;
+  // a shard checks the masks of its own items only: possible in the lazy form (final masks are checked by their last
+  // writer); the eager form's passes run over whole arrays
+  if (n_shards > 1 && !(plan->exec->column && plan->exec->lazy_masks)) return OPTCC_EUNSUPPORTED;
   const optcc_ws_layout L = optcc_layout(plan);
   char* ws = static_cast<char*>(workspace);
   char* masks = ws + L.masks;
@@ -2126,6 +2162,8 @@ extern "C" int optcc_verify(optcc_plan_t* plan, void* workspace, void* stream_, 
   const dim3 blocks(bx, in.p);
   const bool lazy = plan->exec->lazy_masks;
   P.mask_lazy = lazy ? 1u : 0u;
+  P.item_first = shard;
+  P.item_stride = n_shards;
   if (lazy) {
     // initial masks are constants and the last writer of every range checks the final mask (assign_mask_flags); the
     // bulk-copy path would move raw memory, so the streaming warps take the copies too
@@ -2151,9 +2189,55 @@ extern "C" int optcc_verify(optcc_plan_t* plan, void* workspace, void* stream_, 
   r.overlap_elements = res.overlap;
   r.first_bad = res.first_bad;
   r.checked = uint64_t(in.p) * in.n;
+  if (n_shards > 1) {   // the elements of this shard's tiles, on every rank
+    const optcc_exec_state* st = plan->exec;
+    const std::vector<uint4>& items = st->col_items_mask.empty() ? st->col_items : st->col_items_mask;
+    const uint64_t TU = st->col_items_mask.empty() ? plan->tile_units : plan->mask_tile_units, A = in.unit_elems;
+    uint64_t elems = 0;
+    for (size_t i = shard; i < items.size(); i += n_shards) {
+      const uint64_t len = st->col_dflows[items[i].x].len, e0 = uint64_t(items[i].z) * TU * A;
+      elems += std::min<uint64_t>(uint64_t(items[i].w) * A, len - e0);
+    }
+    r.checked = uint64_t(in.p) * elems;
+  }
   if (res.stale || res.stamp != P.stamp) return OPTCC_ESTALE;   // some launch did not find this plan's tables: nothing was verified
   *out = r;
   return (r.bad_elements || r.overlap_elements) ? OPTCC_EVERIFY : OPTCC_OK;
+}
+}  // namespace
+
+// ---- buffers other processes can map (one process per GPU: optcc_execute_shard over peers' rank buffers) ----------
+extern "C" int optcc_peer_alloc(uint64_t bytes, void** dev_ptr, void* handle64) {
+  if (!dev_ptr || !handle64 || bytes == 0) return OPTCC_EINVAL;
+  static_assert(sizeof(cudaIpcMemHandle_t) == 64, "handle size is part of the ABI");
+  void* q = nullptr;
+  CU_TRY(cudaMalloc(&q, size_t(bytes)));
+  cudaIpcMemHandle_t h;
+  if (cudaIpcGetMemHandle(&h, q) != cudaSuccess) {
+    g_last_cuda_error = (int)cudaGetLastError();
+    cudaFree(q);
+    return OPTCC_ECUDA;
+  }
+  std::memcpy(handle64, &h, 64);
+  *dev_ptr = q;
+  return OPTCC_OK;
+}
+extern "C" int optcc_peer_open(const void* handle64, void** dev_ptr) {
+  if (!handle64 || !dev_ptr) return OPTCC_EINVAL;
+  cudaIpcMemHandle_t h;
+  std::memcpy(&h, handle64, 64);
+  CU_TRY(cudaIpcOpenMemHandle(dev_ptr, h, cudaIpcMemLazyEnablePeerAccess));
+  return OPTCC_OK;
+}
+extern "C" int optcc_peer_close(void* dev_ptr) {
+  if (!dev_ptr) return OPTCC_EINVAL;
+  CU_TRY(cudaIpcCloseMemHandle(dev_ptr));
+  return OPTCC_OK;
+}
+extern "C" int optcc_peer_free(void* dev_ptr) {
+  if (!dev_ptr) return OPTCC_EINVAL;
+  CU_TRY(cudaFree(dev_ptr));
+  return OPTCC_OK;
 }
 
 extern "C" int optcc_workspace_check(optcc_plan_t* plan, void* workspace, void* stream_) {

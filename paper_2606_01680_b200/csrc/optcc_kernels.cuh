@@ -116,7 +116,8 @@ struct ExecParams {
   unsigned int df_slots;          // ring depth: tile-ops a CTA holds (claimed, waiting or streaming), <= DF_SLOTS
   // column executor: flows are stored region by region (table order inside a region)
   const uint4* col_items;         // [col_n_items] (first flow, end flow of the region in `flows`, tile, units in the tile)
-  unsigned long long col_n_items;
+  unsigned long long col_n_items;  // items this launch runs: item i of the launch is entry i * item_stride + item_first of col_items
+  unsigned int item_first, item_stride;   // (0, 1) = all items; (s, S) = shard s of S (optcc_execute_shard: peers on other GPUs run the rest)
   unsigned int bulk_copy;         // 1: copy tile-ops are moved by the scheduler agents with cp.async.bulk
   unsigned int l2_hints;          // kind(src loads) + 4 kind(dst loads) + 16 kind(stores); kind: 0 normal, 1 evict_first, 2 evict_last
   unsigned int col_pf_dist;       // column executor: raw operands are requested this many flows ahead (>= 1)

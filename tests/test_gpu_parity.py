@@ -597,3 +597,37 @@ def test_a_clobbered_workspace_is_detected_not_executed(exec_mode):
     s.check()
     assert s.download().tobytes() == OI.run_f32(oplan, x).tobytes()
     assert s.verify()["bad_elements"] == 0
+
+
+@pytest.mark.parametrize("n_shards", [2, 3, 7])
+@pytest.mark.parametrize("dtype", [W.F32, W.BF16])
+def test_the_shards_of_the_work_items_together_are_the_whole_allreduce(n_shards, dtype):
+    """optcc_execute_shard (include/optcc.h "ranks on several GPUs"): shard s of S runs the work items i = s (mod S); run
+    one after another in ONE process on the same buffers, the S shards leave exactly optcc_execute's result, and the S
+    optcc_verify_shard calls check every element once."""
+    import torch
+    w = _wl(16, 1, {0: 8.0 / 7.0}, 2 ** 19 + 6, dtype, seed=61)
+    plan = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=4)
+    oplan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=4)
+    x = W.all_inputs(w)
+    s = _session(plan, verify=True)
+    s.upload(x)
+    stream = torch.cuda.current_stream().cuda_stream
+    for shard in reversed(range(n_shards)):            # any order: the shards touch disjoint element columns
+        B.optcc_execute_shard(plan, s.bufs, s.ws_ptr, shard, n_shards, stream)
+    torch.cuda.synchronize()
+    y = s.download()
+    y_or = OI.run_f32(oplan, x) if dtype == W.F32 else OI.run_bf16(oplan, x)
+    assert y.tobytes() == y_or.tobytes()
+    checked = 0
+    for shard in range(n_shards):
+        v = B.optcc_verify_shard(plan, s.ws_ptr, shard, n_shards, stream)
+        assert v["bad_elements"] == 0 and v["overlap_elements"] == 0
+        checked += v["checked"]
+    assert checked == w.p * w.n
+    with pytest.raises(B.OptccError):
+        B.optcc_execute_shard(plan, s.bufs, s.ws_ptr, n_shards, n_shards, stream)      # shard out of range
+    plan_df = B.optcc_plan(w.p, w.g, w.ell, w.n, w.dtype, k=4, exec_mode=B.OPTCC_EXEC_DATAFLOW)
+    with pytest.raises(B.OptccError) as e:
+        B.optcc_execute_shard(plan_df, s.bufs, s.ws_ptr, 0, 2, stream)                 # only the column executor shards
+    assert e.value.code == B.OPTCC_EUNSUPPORTED
