@@ -113,6 +113,22 @@ def oracle_step(w, k):
     return dt
 
 
+def oracle_walk_compiled(w, k):
+    """The oracle's flow walk restated in C (oracle/walk.c: same table, same order, one IEEE add per element of a
+    reduce flow, the independent flows of a step spread over the host threads), on workload w (fp32).  Only the walk is
+    timed -- no planning, cost simulation, masks or fp64 check.  Returns (seconds, threads)."""
+    from paper_2606_01680_b200 import workloads as W
+    from oracle import planner as OP, cwalk
+    plan = OP.build_plan(w.p, w.g, list(w.ell), w.n, w.dtype, k=k)
+    x = W.all_inputs(w)
+    t0 = time.perf_counter()
+    y = cwalk.run_f32(plan, x, copy=False)
+    dt = time.perf_counter() - t0
+    if not all(y[r, :4096].tobytes() == y[0, :4096].tobytes() for r in range(1, w.p)):
+        raise RuntimeError("compiled oracle walk: outputs differ between ranks")
+    return dt, cwalk.threads()
+
+
 def cpu_threads_used():
     """Threads the oracle actually uses: its numpy work is elementwise slicing/adding (no BLAS), one thread."""
     return 1
@@ -588,6 +604,11 @@ def run_native(args):
         line["cpu_baseline"] = {"value": ws.n * esize / t / 1e9, "unit": UNIT, "cores": cpu_threads_used(), "kind": "oracle",
                                 "sample": f"n={ws.n} elements per rank of the config's n={w.n}, all p={w.p} ranks, every flow; {t:.1f} s",
                                 "host_cores": os.cpu_count()}
+        if w.dtype == W.F32:      # the same walk compiled (the numpy figure is an interpreter number)
+            tc, nthreads = oracle_walk_compiled(ws, k)
+            line["cpu_baseline"]["compiled_walk"] = {
+                "value": ws.n * esize / tc / 1e9, "unit": UNIT, "cores": nthreads, "kind": "oracle/walk.c",
+                "what": "flow walk only (no planning, cost model, masks or fp64 check), gcc -O2 -fopenmp, same sample", "s": tc}
     ok = m["parity_ok"] and (not others or all(o["parity_spot_check"]["within_tolerance_and_all_ranks_identical"] for o in others.values()))
     if not ok:
         line["error"] = "parity spot check failed"

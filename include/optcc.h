@@ -239,7 +239,9 @@ OPTCC_API int optcc_cost(const optcc_plan_t* plan, const optcc_cost_params_t* pa
  * (NULL = default stream).  Asynchronous: never synchronises the device or the stream; once the tables are resident
  * (after optcc_prepare or a first call) it only enqueues memsets and kernel launches (column executor: one memset
  * and one launch), so it can be captured into a CUDA graph on `stream` and replayed.
- * Errors: EINVAL (NULL / misaligned pointers), ECUDA. */
+ * Errors: EINVAL (NULL / misaligned pointers), ECUDA, EUNSUPPORTED (the plan names the persistent or dataflow executor
+ * and the device has no cooperative launch, or the dataflow tables do not fit 32-bit counters: the executor is never
+ * changed silently -- plan_info.exec_mode is what runs). */
 OPTCC_API int optcc_prepare(optcc_plan_t* plan, void* workspace, void* stream);
 /* Host only, no device needed: the column executor's work list, for inspection and tests.  records [host, borrowed until
  * optcc_plan_destroy]: n_records records of 32 bytes { off u64, len u64 (elements), src u16, dst u16, op u8, ksrc u8,

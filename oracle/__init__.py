@@ -12,6 +12,8 @@ Modules
   cost_sim      port-model event simulation in exact rationals                   (pinned)
   reference     fp64 per-element reference sum and the tolerance predicates      (pinned)
   brute_force   exhaustive search over chunk splits for p <= 5                   (pinned)
+  cwalk/walk.c  interpreter.run_f32 restated in plain C (OpenMP over the independent flows of a
+                step): the compiled CPU baseline bench.py times; pinned against run_f32 bit for bit
 
 Parity unpinned: the slot-exact pattern layouts of Figs 5-7, 11-19 (figures absent from
 PAPER.md); they are replaced by the canonical constructions of docs/PLAN_SPEC.md, which are

@@ -1785,6 +1785,10 @@ int launch_plan(optcc_plan_t* pl, ExecParams& P, cudaStream_t stream) {
   if (n_steps == 0) return OPTCC_OK;
   const bool persistent = pl->opts.exec_mode == OPTCC_EXEC_PERSISTENT && st->coop;
   const bool dataflow = pl->opts.exec_mode == OPTCC_EXEC_DATAFLOW && st->coop && st->df_ok && st->G_df > 0;
+  // no silent change of executor: a device without cooperative launch (or a plan whose completion counters do not fit
+  // the dataflow tables) cannot run the executor the plan names -- the caller asks for OPTCC_EXEC_PER_STEP / COLUMN itself
+  if ((pl->opts.exec_mode == OPTCC_EXEC_PERSISTENT && !persistent) || (pl->opts.exec_mode == OPTCC_EXEC_DATAFLOW && !dataflow))
+    return OPTCC_EUNSUPPORTED;
   if (st->column) {
     // contributor-mask runs have their own tile size (mask_tile_units) when a unit of masks is wider than 16 bytes
     const bool own_items = is_mask_mode(MODE) && !st->col_items_mask.empty();
