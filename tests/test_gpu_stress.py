@@ -136,3 +136,34 @@ def test_random_plans_any_executor_any_verifier(seed):
     assert res["overlap_elements"] == overlaps
     if bad.any():
         assert res["first_bad"] == int(np.flatnonzero(bad.reshape(-1))[0])
+
+
+_SOAK = int(__import__("os").environ.get("OPTCC_SOAK", "0"))      # extra seeds for a one-off soak run
+
+
+@pytest.mark.parametrize("seed", range(60 + _SOAK))
+def test_column_executor_random_cuts_leave_the_oracles_state(seed):
+    """The column executor keeps partial sums in registers and does not store the ones a later EXECUTED flow overwrites
+    (opts.no_forward = 0): whatever the plan, the tile size (one round or several, CTA- or warp-wide), the forwarding
+    mode and the step the schedule is cut at, every element of every rank buffer must hold what the oracle holds after
+    walking the same table prefix (fp32 plans: the rank buffers show every partial sum)."""
+    import dataclasses
+    from paper_2606_01680_b200.device import Session
+    rng = np.random.default_rng(424242 + seed)
+    p, g, ell, n, k, _, _, grid, ordering = _random_case(rng)
+    n = int(rng.integers(1, 400000))
+    tile = int(rng.choice([0, 0, 128, 64, 1792, 896, 3584, 224]))
+    no_forward = int(rng.choice([0, 0, 0, 1, 2]))
+    oplan = OP.build_plan(p, g, ell, n, W.F32, k=k, ordering=ordering or 2)
+    limit = 0 if (oplan.n_steps < 2 or rng.integers(0, 4) == 0) else int(rng.integers(1, oplan.n_steps))
+    plan = B.optcc_plan(p, g, ell, n, W.F32, k=k, exec_mode=B.OPTCC_EXEC_COLUMN, tile_units=tile, grid_ctas=grid,
+                        ordering=ordering, step_limit=limit, no_forward=no_forward)
+    x = W.all_inputs(W.Workload("cut", p, g, tuple(ell), n, W.F32, "normal", 1.0, 88000 + seed))
+    s = Session(plan)
+    s.upload(x)
+    s.execute()
+    y = s.download()
+    if limit:
+        oplan = dataclasses.replace(oplan, n_steps=limit, flows=oplan.flows[:int(oplan.step_begin[limit])],
+                                    step_begin=oplan.step_begin[:limit + 1])
+    assert y.tobytes() == OI.run_f32(oplan, x).tobytes(), (p, g, n, k, tile, no_forward, limit)
