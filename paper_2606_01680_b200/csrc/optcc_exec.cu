@@ -792,11 +792,23 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel
   uint4 carry[MODE == MODE_BF16 ? 8 : 4];
   const unsigned long long bulk_pol = make_policy(P.col_bulk_policy);   // L2 policy of the bulk stores
   const bool pf = !is_mask_mode(MODE) && P.col_pf_dist != 0;
-  // Items are dealt round-robin to the warps of the grid (neighbouring warps take neighbouring tiles): a global ticket
-  // would be claimed once per warp and item, and same-address atomics from different SMs complete about one per 90 ns
-  // (measured: 131 k items -> 11.7 ms), more than the items' own work.
+  // Items are dealt round-robin to the warps of the grid (neighbouring warps take neighbouring tiles) or, when there
+  // are only a few per warp, claimed one at a time through the global ticket (ExecParams.col_chunk, see launch_plan).
   const unsigned long long n_warps = (unsigned long long)gridDim.x * (COL_THREADS / 32);
-  for (unsigned long long it = (unsigned long long)blockIdx.x * (COL_THREADS / 32) + warp; it < P.col_n_items; it += n_warps) {
+  const unsigned int CH = P.col_chunk;               // 0: static dealing; else items a warp claims at a time
+  unsigned long long it = (unsigned long long)blockIdx.x * (COL_THREADS / 32) + warp, it_end = 0;
+  if (CH) it = 0;
+  for (;; it += CH ? 1 : n_warps) {
+    if (CH) {
+      if (it == it_end) {
+        unsigned long long b = 0;
+        if (lane == 0) b = atomicAdd(&P.ctrl->ticket, (unsigned long long)CH);
+        b = __shfl_sync(0xFFFFFFFFu, b, 0);
+        it = b;
+        it_end = b + CH;
+      }
+    }
+    if (it >= P.col_n_items) break;
     const uint4 item = __ldg(P.col_items + (it * P.item_stride + P.item_first));
     const unsigned int fb = item.x, fe = item.y;
     const unsigned long long ubeg = (unsigned long long)item.z * P.tile_units, uend = ubeg + item.w;
@@ -1827,6 +1839,12 @@ int launch_plan(optcc_plan_t* pl, ExecParams& P, cudaStream_t stream) {
       // warp-wide tiles: one stage per warp; a CTA's 14 warps take items on their own
       const size_t dyn = P.col_bulk ? tile_bytes * (COL_THREADS / 32) : 0;
       const unsigned int wgrid = (unsigned int)std::min<uint64_t>(G, (P.col_n_items + COL_THREADS / 32 - 1) / (COL_THREADS / 32));
+      // Few items per warp: a global ticket per item (a warp that finishes early takes the next tile; with 4.1 items per
+      // warp static dealing runs 5 rounds for 4.1 rounds of work: C3 1.47 -> 1.31 ms).  Many items per warp: dealt
+      // round-robin -- same-address atomics complete about one per 90 ns and would cap the kernel (131 k items: 11.7 ms).
+      // Claims of several consecutive items at a time are worse than either (2 / 4 / 8 / 16 per claim: C3 1.49 / 1.80 /
+      // 2.28 / 4.38 ms): neighbouring tiles must run on neighbouring warps at the same time, not one after another.
+      P.col_chunk = P.col_n_items <= uint64_t(8) * wgrid * (COL_THREADS / 32) ? 1u : 0u;
       if (MASKS && P.mask_fwd) {
         if (dyn > 40 * 1024) CU_TRY(cudaFuncSetAttribute(optcc_wcolumn_kernel<MODE, MASKS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
         optcc_wcolumn_kernel<MODE, MASKS><<<wgrid, COL_THREADS, dyn, stream>>>(P);
@@ -1904,6 +1922,7 @@ void fill_common(const optcc_plan_t* pl, void* workspace, ExecParams& P) {
   P.col_pf_dist = 1; P.col_pf_l2 = 0; P.col_pf_next = 0; P.col_bulk = 1;
   P.col_bulk_policy = 1;   // bulk stores evict_first: the all-gather's results are never read again (measured: C2 1.68 -> 1.62 ms)
   P.col_warp = pl->col_warp;
+  P.col_chunk = 0;
   if (pl->opts.copy_path == 1) P.col_bulk = 0;
 }
 

@@ -129,6 +129,7 @@ struct ExecParams {
   unsigned int col_warp;          // 1: warp-wide tiles (optcc_wcolumn_kernel), 0: CTA-wide tiles (optcc_column_kernel)
   unsigned int col_stage_bytes;   // bytes of one staged tile (the warp-wide kernel keeps one per warp)
   unsigned int mask_fwd;          // lazy contributor-mask runs: act on DFLOW_SRC_FWD / DFLOW_NO_STORE
+  unsigned int col_chunk;         // warp-wide tiles: 0 = items dealt round-robin to the grid's warps; else a warp claims this many consecutive items at a time
   unsigned int data_fwd;          // data runs, one-round tiles: bit 0 = act on DFLOW_SRC_REG (range_add_f32_round /
                                   // range_add_bf16_round), bit 1 = also on DFLOW_NO_STORE (dead partial sums stay in registers)
   unsigned int pad4;
