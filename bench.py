@@ -300,6 +300,21 @@ class Bench:
         self.stream = torch.cuda.current_stream(self.dev)
         self.args = args
         self.peak, self.peak_src = measured_peak()
+        import queue
+        self.cost_in, self.cost_out = queue.SimpleQueue(), queue.SimpleQueue()
+        threading.Thread(target=self._cost_worker, daemon=True).start()
+
+    def _cost_worker(self):
+        """The second host thread: optcc_cost of every plan it is handed (started once: creating a Python thread per
+        step costs 50-100 us of the step)."""
+        while True:
+            plan = self.cost_in.get()
+            if plan is None:
+                return
+            tc = time.perf_counter()
+            c = self.B.optcc_cost(plan)
+            self.cost_out.put((c, (time.perf_counter() - tc) * 1e3))
+            del plan
 
     def ev(self):
         return self.torch.cuda.Event(enable_timing=True)
@@ -334,23 +349,20 @@ class Bench:
             plan = mk()                                   # a1-a3: classify, chunk, flow / step tables
             t1 = time.perf_counter()
 
-            def cost():                                   # a4 on a second host thread (ctypes releases the GIL)
-                tc = time.perf_counter()
-                box["cost"] = B.optcc_cost(plan)
-                box["cost_ms"] = (time.perf_counter() - tc) * 1e3
-            th = threading.Thread(target=cost)
             if not execute_only:
-                th.start()
+                self.cost_in.put(plan)                    # a4 on a second host thread (ctypes releases the GIL)
+            old = sess.plan
             sess.plan = plan
             sess.prepare()                                # the executor's tables, built on the host and uploaded
             stream.synchronize()                          # (the upload belongs to plan_to_launch, not to the executor's time)
             e[1].record(stream)
             sess.execute()                                # a5-a7
             e[2].record(stream)
+            del old                                       # the previous step's plan is destroyed while the GPU works
             res = None if execute_only else sess.verify() # a8 (synchronises the stream once to read the counters)
             e[3].record(stream)
             if not execute_only:
-                th.join()
+                box["cost"], box["cost_ms"] = self.cost_out.get()
             e[4].record(stream)
             torch.cuda.synchronize(self.dev)
             if res is not None and (res["bad_elements"] or res["overlap_elements"]):

@@ -1009,9 +1009,19 @@ void* pinned_alloc(size_t bytes) {                       // nullptr: use pageabl
 void pinned_free(void* q, size_t bytes) {
   {
     std::lock_guard<std::mutex> lock(g_pinned_mutex);
-    size_t total = bytes;
-    for (const auto& b : g_pinned_cache) total += b.bytes;
-    if (g_pinned_cache.size() < PINNED_CACHE_BLOCKS && total <= PINNED_CACHE_MAX) { g_pinned_cache.push_back(PinnedBlock{q, bytes}); return; }
+    // the newest block stays, the oldest ones go (a job that moves on to another plan shape must find ITS blocks cached;
+    // cudaFreeHost waits for the device, so it must not happen on every step)
+    if (bytes <= PINNED_CACHE_MAX) {
+      g_pinned_cache.push_back(PinnedBlock{q, bytes});
+      size_t total = 0;
+      for (const auto& b : g_pinned_cache) total += b.bytes;
+      while (g_pinned_cache.size() > PINNED_CACHE_BLOCKS || total > PINNED_CACHE_MAX) {
+        total -= g_pinned_cache.front().bytes;
+        cudaFreeHost(g_pinned_cache.front().p);
+        g_pinned_cache.erase(g_pinned_cache.begin());
+      }
+      return;
+    }
   }
   cudaFreeHost(q);
 }

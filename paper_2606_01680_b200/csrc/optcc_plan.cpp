@@ -21,7 +21,7 @@ namespace {
 struct RawBlock { void* p; size_t bytes; };
 std::mutex g_raw_mutex;
 std::vector<RawBlock> g_raw_cache;                 // at most RAW_CACHE_BLOCKS freed blocks
-constexpr size_t RAW_CACHE_BLOCKS = 8;
+constexpr size_t RAW_CACHE_BLOCKS = 12;
 constexpr size_t RAW_CACHE_MIN = size_t(1) << 16;  // smaller blocks go straight to malloc / free
 constexpr size_t RAW_CACHE_MAX = size_t(1) << 30;  // total bytes kept
 }  // namespace
@@ -49,10 +49,16 @@ void optcc_raw_free(void* p, size_t bytes) {
   if (!p) return;
   if (bytes >= RAW_CACHE_MIN) {
     std::lock_guard<std::mutex> lock(g_raw_mutex);
-    size_t total = bytes;
-    for (const auto& b : g_raw_cache) total += b.bytes;
-    if (g_raw_cache.size() < RAW_CACHE_BLOCKS && total <= RAW_CACHE_MAX) {
+    // the newest block stays, the oldest ones go: a job that moves on to another plan shape must find ITS blocks cached
+    if (bytes <= RAW_CACHE_MAX) {
       g_raw_cache.push_back(RawBlock{p, bytes});
+      size_t total = 0;
+      for (const auto& b : g_raw_cache) total += b.bytes;
+      while (g_raw_cache.size() > RAW_CACHE_BLOCKS || total > RAW_CACHE_MAX) {
+        total -= g_raw_cache.front().bytes;
+        std::free(g_raw_cache.front().p);
+        g_raw_cache.erase(g_raw_cache.begin());
+      }
       return;
     }
   }
