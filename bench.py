@@ -354,8 +354,7 @@ class Bench:
             old = sess.plan
             sess.plan = plan
             sess.prepare()                                # the executor's tables, built on the host and uploaded
-            stream.synchronize()                          # (the upload belongs to plan_to_launch, not to the executor's time)
-            e[1].record(stream)
+            e[1].record(stream)                           # (in stream order after the upload: plan_to_launch ends here)
             sess.execute()                                # a5-a7
             e[2].record(stream)
             del old                                       # the previous step's plan is destroyed while the GPU works

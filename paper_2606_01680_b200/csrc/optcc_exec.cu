@@ -602,12 +602,11 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
   unsigned int bulk_turn = 0;        // bulk stores issued so far (the warps' first lanes take turns)
   uint4 carry[4];                    // lazy contributor-mask runs: what the previous flow produced (DFLOW_SRC_FWD)
   const unsigned long long bulk_pol = make_policy(P.col_bulk_policy);   // L2 policy of the bulk stores
-  if (threadIdx.x == 0) {
-    s_item[0] = atomicAdd(&P.ctrl->ticket, 1ull);
-    s_item[1] = atomicAdd(&P.ctrl->ticket, 1ull);
-  }
-  __syncthreads();
-  unsigned long long it = s_item[0], nit = s_item[1];
+  // The first two items of every CTA are dealt statically, the ticket hands out the rest (counting from 2 gridDim.x):
+  // same-address atomics from 148 SMs complete about one per 90 ns, and 2 x 296 of them at the start of the kernel kept
+  // the last CTA waiting for 50 us (all of C1's kernel time).
+  const unsigned long long ticket0 = 2ull * gridDim.x;
+  unsigned long long it = blockIdx.x, nit = (unsigned long long)blockIdx.x + gridDim.x;
   bool prefetched = false;           // the first flows of this item were requested during the previous item
   for (unsigned int round = 0; it < P.col_n_items; ++round) {
     // one record per item: the region's flows [fb, fe), the tile and its length in units (all flows over a region have
@@ -743,7 +742,7 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_column_kernel(
         }
       }
     }
-    if (threadIdx.x == 0) s_item[round & 1] = atomicAdd(&P.ctrl->ticket, 1ull);   // (slot of `it`: read by everyone long ago)
+    if (threadIdx.x == 0) s_item[round & 1] = ticket0 + atomicAdd(&P.ctrl->ticket, 1ull);   // (slot of `it`: read by everyone long ago)
     __syncthreads();                 // every thread has read this item's records
     prefetched = n_cnt != 0;
     it = nit;
@@ -796,13 +795,13 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel
   // are only a few per warp, claimed one at a time through the global ticket (ExecParams.col_chunk, see launch_plan).
   const unsigned long long n_warps = (unsigned long long)gridDim.x * (COL_THREADS / 32);
   const unsigned int CH = P.col_chunk;               // 0: static dealing; else items a warp claims at a time
-  unsigned long long it = (unsigned long long)blockIdx.x * (COL_THREADS / 32) + warp, it_end = 0;
-  if (CH) it = 0;
+  // (a warp's first item is always its own number: 4144 claims at the start of the kernel would queue for 0.4 ms)
+  unsigned long long it = (unsigned long long)blockIdx.x * (COL_THREADS / 32) + warp, it_end = it + 1;
   for (;; it += CH ? 1 : n_warps) {
     if (CH) {
       if (it == it_end) {
         unsigned long long b = 0;
-        if (lane == 0) b = atomicAdd(&P.ctrl->ticket, (unsigned long long)CH);
+        if (lane == 0) b = n_warps + atomicAdd(&P.ctrl->ticket, (unsigned long long)CH);
         b = __shfl_sync(0xFFFFFFFFu, b, 0);
         it = b;
         it_end = b + CH;
