@@ -260,3 +260,27 @@ def test_a_latency_shorter_than_a_slot_is_hidden_by_the_neighbouring_stage():
     occ = cost_sim.simulate(oplan, alpha=s / 2)["T"]
     assert lat - base <= 2 * (p - 1) * (s / 2)               # at most one latency per hop of the last segment's chains
     assert occ - base >= (k + 1) * (p - 1) * (s / 2)         # one occupancy per window
+
+
+def test_entry_points_reject_bad_arguments_before_touching_a_device():
+    """Argument checks that need no GPU: optcc_execute_static refuses a plan whose workspace exceeds the static array
+    (OPTCC_ETOOBIG) and optcc_execute_shard / optcc_verify_shard refuse a shard out of range (EINVAL) or a plan whose
+    executor has no independent work items (EUNSUPPORTED) -- all before the first CUDA call, so this runs on a CPU box."""
+    import ctypes as C
+    lib = B.load()
+    p, n = 4, 2 ** 20
+    ell = [2.0, 1.0, 1.0, 1.0]
+    big = B.optcc_plan(p, 1, ell, n, W.BF16, k=4)                       # fp32 partials alone: 16 MiB
+    assert big.info["workspace_bytes"] > B.OPTCC_STATIC_WORKSPACE_BYTES
+    fake = (C.c_void_p * p)(*[0x1000 * (i + 1) for i in range(p)])      # never dereferenced
+    assert lib.optcc_execute_static(big.handle, fake, None) == B.OPTCC_ETOOBIG
+    assert b"OPTCC_STATIC_WORKSPACE_BYTES" in lib.optcc_strerror(B.OPTCC_ETOOBIG)
+    small = B.optcc_plan(p, 1, ell, 4096, W.F32, k=4)
+    assert small.info["workspace_bytes"] <= B.OPTCC_STATIC_WORKSPACE_BYTES
+    assert lib.optcc_execute_shard(small.handle, fake, C.c_void_p(0x100), None, 2, 2) == B.OPTCC_EINVAL
+    assert lib.optcc_execute_shard(small.handle, fake, C.c_void_p(0x100), None, 0, 0) == B.OPTCC_EINVAL
+    out = B.optcc_verify_result_t()
+    assert lib.optcc_verify_shard(small.handle, C.c_void_p(0x100), None, 3, 2, C.byref(out)) == B.OPTCC_EINVAL
+    df = B.optcc_plan(p, 1, ell, 4096, W.F32, k=4, exec_mode=B.OPTCC_EXEC_DATAFLOW)
+    assert lib.optcc_execute_shard(df.handle, fake, C.c_void_p(0x100), None, 0, 2) == B.OPTCC_EUNSUPPORTED
+    assert lib.optcc_verify_shard(df.handle, C.c_void_p(0x100), None, 0, 2, C.byref(out)) == B.OPTCC_EUNSUPPORTED
