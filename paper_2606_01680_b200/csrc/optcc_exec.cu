@@ -774,6 +774,78 @@ __device__ __forceinline__ DFlow load_record(const DFlow* p) {
   return f;
 }
 
+// A FULL warp-wide tile of an fp32 plan with forwarding (128 units, four vectors per lane, no ragged end) through its
+// region's records [fb, fe): the same flows, flags and arithmetic as the generic path (process_piece /
+// range_add_f32_round), written as the tight loop a stand-alone probe of this access pattern runs at 0.96 of the copy
+// peak with: only the second half of a record is read (src, dst, op, flags -- offset and length are the
+// region's), a lane's byte offset is formed once per item, and a flow is its loads, adds and stores.  Measured against
+// the generic path in the same run: C4 0.91 vs 1.06 ms, C4 at k = 8 0.95 vs 1.00, C2 on warp-wide tiles 1.43 vs 1.54.
+// tile_off: bytes from the start of a rank buffer to the tile; v0 / vend: the lane's first vector and the tile's end
+// in the region's vectors (the discard's whole-line test).
+template <class PolX>
+__device__ __forceinline__ void lean_item_f32(const ExecParams& P, unsigned int fb, unsigned int fe, unsigned long long tile_off,
+                                              unsigned int lane, char* stage, const PolX& pol, unsigned long long bulk_pol,
+                                              unsigned long long v0, unsigned long long vend) {
+  const bool elide = (P.data_fwd & 2u) != 0u, bulk = P.col_bulk != 0u, pf = P.col_pf_dist != 0u;
+  const unsigned long long lane_off = tile_off + lane * 16ull;
+  const uint4* const rec = reinterpret_cast<const uint4*>(P.flows + fb) + 1;     // second 16 bytes of record fb
+  uint4 cur = __ldg(rec);
+  uint4 acc[4];
+  auto first_touches = [&](const uint4& r) {     // the raw operands of a flow are DRAM accesses: requested a flow ahead
+    if (r.z & DFLOW_SRC_INIT) { const char* q = rank_ptr(P, r.x & 0xFFFFu) + lane_off; for (int k = 0; k < 4; ++k) prefetch_l1(q + k * 512); }
+    if ((r.y & 0xFFu) == 0u && (r.z & DFLOW_DST_INIT)) { const char* q = rank_ptr(P, r.x >> 16) + lane_off; for (int k = 0; k < 4; ++k) prefetch_l1(q + k * 512); }
+  };
+  if (pf) first_touches(cur);
+  for (unsigned int j = fb; j < fe; ++j) {
+    const uint4 nxt = __ldg(rec + 2 * ((j + 1 < fe ? j + 1 : j) - fb));
+    const unsigned int src = cur.x & 0xFFFFu, dst = cur.x >> 16, fl = cur.z;
+    if (pf && j + 1 < fe) first_touches(nxt);
+    if ((cur.y & 0xFFu) != 0u) {       // copy
+      if (bulk && (fl & DFLOW_FROM_STAGE)) {
+        if (lane == 0) bulk_s2g_hint(rank_ptr(P, dst) + tile_off, stage, 128u * 16u, bulk_pol);
+      } else {
+        const char* sp = rank_ptr(P, src) + lane_off;
+        char* dp = rank_ptr(P, dst) + lane_off;
+        uint4 x[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) x[k] = ld16(sp + k * 512, pol.lds, pol.l1);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) st16(dp + k * 512, x[k], pol);
+        __syncwarp();
+      }
+    } else {                           // reduce: dst += src, one IEEE add per element
+      char* dp = rank_ptr(P, dst) + lane_off;
+      const char* sp = rank_ptr(P, src) + lane_off;
+      uint4 b[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) b[k] = ld16(dp + k * 512, pol.ldd, pol.l1);
+      if (!(fl & DFLOW_SRC_REG)) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) acc[k] = ld16(sp + k * 512, pol.lds, pol.l1);
+      }
+      const bool staged = bulk && (fl & DFLOW_STAGE_OUT) != 0u;
+      if (staged) {                    // the stage is rewritten: the previous tile's bulk stores must have read it
+        if (lane == 0) bulk_wait_read_all();
+        __syncwarp();
+      }
+      const bool store = !(elide && (fl & DFLOW_NO_STORE));
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        acc[k] = add_f32x4(b[k], acc[k]);
+        if (store) st16(dp + k * 512, acc[k], pol);
+        if (staged) sts16(stage + (lane + k * 32) * 16, acc[k]);
+      }
+      if (staged) fence_proxy_async();
+      if ((fl & DFLOW_DEAD_SRC) && !(elide && (fl & DFLOW_SRC_FWD))) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) discard_line16(sp + k * 512, v0 + k * 32, vend);
+      }
+      __syncwarp();   // stage writes before lane 0's bulk stores; a lane's discard before other lanes' later stores to the line
+    }
+    cur = nxt;
+  }
+}
+
 template <int MODE, bool MASK_FWD = false>
 __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel(const __grid_constant__ ExecParams P) {
   if (tables_are_stale(P)) return;
@@ -812,6 +884,12 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel
     const unsigned int fb = item.x, fe = item.y;
     const unsigned long long ubeg = (unsigned long long)item.z * P.tile_units, uend = ubeg + item.w;
     DFlow cur = load_record(P.flows + fb);
+    if (MASK_FWD && MODE == MODE_F32 && item.w == 128u && (ubeg + 128u) * P.unit_elems <= cur.len) {
+      // (a full tile inside the region: no ragged end, four vectors per lane.  The bf16 counterpart -- 32 carried
+      // registers per lane -- spilled 1 KB and was slower than the generic path, C3 1.47 vs 1.25 ms: not kept)
+      lean_item_f32(P, fb, fe, cur.off * 4 + ubeg * 16, lane, stage, pol, bulk_pol, ubeg + lane, ubeg + 128u);
+      continue;
+    }
     if (pf) prefetch_raw<MODE, 32>(P, cur, ubeg, item.w);
     int prev_cls = -1;
     // the tile in bytes of the run's element type (all flows over a region have the region's offset and length)
@@ -1848,12 +1926,11 @@ int launch_plan(optcc_plan_t* pl, ExecParams& P, cudaStream_t stream) {
       // warp-wide tiles: one stage per warp; a CTA's 14 warps take items on their own
       const size_t dyn = P.col_bulk ? tile_bytes * (COL_THREADS / 32) : 0;
       const unsigned int wgrid = (unsigned int)std::min<uint64_t>(G, (P.col_n_items + COL_THREADS / 32 - 1) / (COL_THREADS / 32));
-      // Few items per warp: a global ticket per item (a warp that finishes early takes the next tile; with 4.1 items per
-      // warp static dealing runs 5 rounds for 4.1 rounds of work: C3 1.47 -> 1.31 ms).  Many items per warp: dealt
-      // round-robin -- same-address atomics complete about one per 90 ns and would cap the kernel (131 k items: 11.7 ms).
-      // Claims of several consecutive items at a time are worse than either (2 / 4 / 8 / 16 per claim: C3 1.49 / 1.80 /
-      // 2.28 / 4.38 ms): neighbouring tiles must run on neighbouring warps at the same time, not one after another.
-      P.col_chunk = P.col_n_items <= uint64_t(8) * wgrid * (COL_THREADS / 32) ? 1u : 0u;
+      // A warp's first item is its own number, the global ticket hands out the rest: a warp that finishes early takes
+      // the next tile (C3: 4.1 items per warp ran 5 static rounds, 1.47 -> 1.32 ms; C2 forced to warp-wide tiles, 131 k
+      // items: 1.66 -> 1.43 ms).  Claims of several consecutive items at a time are worse than either (2 / 4 / 8 / 16 per
+      // claim: C3 1.49 / 1.80 / 2.28 / 4.38 ms): neighbouring tiles must run on neighbouring warps at the same time.
+      P.col_chunk = 1u;
       if (MASKS && P.mask_fwd) {
         if (dyn > 40 * 1024) CU_TRY(cudaFuncSetAttribute(optcc_wcolumn_kernel<MODE, MASKS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
         optcc_wcolumn_kernel<MODE, MASKS><<<wgrid, COL_THREADS, dyn, stream>>>(P);
