@@ -785,12 +785,11 @@ __device__ __forceinline__ DFlow load_record(const DFlow* p) {
 template <class PolX>
 __device__ __forceinline__ void lean_item_f32(const ExecParams& P, unsigned int fb, unsigned int fe, unsigned long long tile_off,
                                               unsigned int lane, char* stage, const PolX& pol, unsigned long long bulk_pol,
-                                              unsigned long long v0, unsigned long long vend) {
+                                              unsigned long long v0, unsigned long long vend, uint4 (&acc)[4]) {
   const bool elide = (P.data_fwd & 2u) != 0u, bulk = P.col_bulk != 0u, pf = P.col_pf_dist != 0u;
   const unsigned long long lane_off = tile_off + lane * 16ull;
   const uint4* const rec = reinterpret_cast<const uint4*>(P.flows + fb) + 1;     // second 16 bytes of record fb
   uint4 cur = __ldg(rec);
-  uint4 acc[4];
   auto first_touches = [&](const uint4& r) {     // the raw operands of a flow are DRAM accesses: requested a flow ahead
     if (r.z & DFLOW_SRC_INIT) { const char* q = rank_ptr(P, r.x & 0xFFFFu) + lane_off; for (int k = 0; k < 4; ++k) prefetch_l1(q + k * 512); }
     if ((r.y & 0xFFu) == 0u && (r.z & DFLOW_DST_INIT)) { const char* q = rank_ptr(P, r.x >> 16) + lane_off; for (int k = 0; k < 4; ++k) prefetch_l1(q + k * 512); }
@@ -887,7 +886,8 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel
     if (MASK_FWD && MODE == MODE_F32 && item.w == 128u && (ubeg + 128u) * P.unit_elems <= cur.len) {
       // (a full tile inside the region: no ragged end, four vectors per lane.  The bf16 counterpart -- 32 carried
       // registers per lane -- spilled 1 KB and was slower than the generic path, C3 1.47 vs 1.25 ms: not kept)
-      lean_item_f32(P, fb, fe, cur.off * 4 + ubeg * 16, lane, stage, pol, bulk_pol, ubeg + lane, ubeg + 128u);
+      lean_item_f32(P, fb, fe, cur.off * 4 + ubeg * 16, lane, stage, pol, bulk_pol, ubeg + lane, ubeg + 128u,
+                    reinterpret_cast<uint4 (&)[4]>(carry));
       continue;
     }
     if (pf) prefetch_raw<MODE, 32>(P, cur, ubeg, item.w);
