@@ -845,6 +845,113 @@ __device__ __forceinline__ void lean_item_f32(const ExecParams& P, unsigned int 
   }
 }
 
+// The same for bf16 plans: a unit is 8 elements -- 16 bytes of bf16 in a rank buffer (kind 0) or 32 bytes of fp32
+// partials in the shadow (kind 1) -- four units per lane, the running sum as 8 fp32 values per unit in `acc` (the
+// kernel's carried registers).  A flow's kinds (source, destination before, destination after) are in its record; the
+// sum is rounded to bf16 once, when the flow that completes it stores it to the rank buffer (R12).
+template <class PolX>
+__device__ __forceinline__ void lean_item_bf16(const ExecParams& P, unsigned int fb, unsigned int fe, unsigned long long off,
+                                               unsigned long long tile_unit0, unsigned int lane, char* stage, const PolX& pol,
+                                               unsigned long long bulk_pol, uint4 (&acc)[8]) {
+  const bool elide = (P.data_fwd & 2u) != 0u, bulk = P.col_bulk != 0u, pf = P.col_pf_dist != 0u;
+  const unsigned long long u0 = tile_unit0 + lane, uend = tile_unit0 + 128u;
+  // the lane's first unit of rank r's range, in the rank buffer and in the shadow
+  auto buf_ptr = [&](unsigned int r) { return rank_ptr(P, r) + off * 2 + u0 * 16; };
+  auto sh_ptr = [&](unsigned int r) { return reinterpret_cast<char*>(P.shadow + (unsigned long long)r * P.padded_n + off) + u0 * 32; };
+  const uint4* const rec = reinterpret_cast<const uint4*>(P.flows + fb) + 1;
+  uint4 cur = __ldg(rec);
+  auto first_touches = [&](const uint4& r) {     // raw inputs live in the rank buffers: requested a flow ahead
+    if (r.z & DFLOW_SRC_INIT) { const char* q = buf_ptr(r.x & 0xFFFFu); for (int k = 0; k < 4; ++k) prefetch_l1(q + k * 512); }
+    if ((r.y & 0xFFu) == 0u && (r.z & DFLOW_DST_INIT)) { const char* q = buf_ptr(r.x >> 16); for (int k = 0; k < 4; ++k) prefetch_l1(q + k * 512); }
+  };
+  if (pf) first_touches(cur);
+  for (unsigned int j = fb; j < fe; ++j) {
+    const uint4 nxt = __ldg(rec + 2 * ((j + 1 < fe ? j + 1 : j) - fb));
+    const unsigned int src = cur.x & 0xFFFFu, dst = cur.x >> 16, fl = cur.z;
+    const unsigned int ksrc = (cur.y >> 8) & 0xFFu, kdin = (cur.y >> 16) & 0xFFu, kdout = cur.y >> 24;
+    if (pf && j + 1 < fe) first_touches(nxt);
+    if ((cur.y & 0xFFu) != 0u) {       // copy
+      if (bulk && (fl & DFLOW_FROM_STAGE)) {
+        if (lane == 0) bulk_s2g_hint(rank_ptr(P, dst) + off * 2 + tile_unit0 * 16, stage, 128u * 16u, bulk_pol);
+      } else if (ksrc == 0u) {         // bf16 -> bf16: one vector per unit
+        const char* sp = buf_ptr(src);
+        char* dp = buf_ptr(dst);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) st16(dp + k * 512, ld16(sp + k * 512, pol.lds, pol.l1), pol);
+        __syncwarp();
+      } else {                         // fp32 partials -> fp32 partials: two vectors per unit
+        const char* sp = sh_ptr(src);
+        char* dp = sh_ptr(dst);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const uint4 x0 = ld16(sp + k * 1024, pol.lds, pol.l1), x1 = ld16(sp + k * 1024 + 16, pol.lds, pol.l1);
+          st16(dp + k * 1024, x0, pol);
+          st16(dp + k * 1024 + 16, x1, pol);
+        }
+        __syncwarp();
+      }
+    } else {                           // reduce
+      if (!(fl & DFLOW_SRC_REG)) {     // the source operand: raw bf16 or fp32 partials
+        if (ksrc == 0u) {
+          const char* sp = buf_ptr(src);
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const uint4 r = ld16(sp + k * 512, pol.lds, pol.l1);
+            acc[2 * k] = make_uint4(r.x << 16, r.x & 0xFFFF0000u, r.y << 16, r.y & 0xFFFF0000u);
+            acc[2 * k + 1] = make_uint4(r.z << 16, r.z & 0xFFFF0000u, r.w << 16, r.w & 0xFFFF0000u);
+          }
+        } else {
+          const char* sp = sh_ptr(src);
+#pragma unroll
+          for (int k = 0; k < 4; ++k) { acc[2 * k] = ld16(sp + k * 1024, pol.lds, pol.l1); acc[2 * k + 1] = ld16(sp + k * 1024 + 16, pol.lds, pol.l1); }
+        }
+      }
+      const bool staged = bulk && (fl & DFLOW_STAGE_OUT) != 0u && kdout == 0u;
+      if (staged) {
+        if (lane == 0) bulk_wait_read_all();
+        __syncwarp();
+      }
+      const bool store = !(elide && (fl & DFLOW_NO_STORE));
+      const char* dip = kdin ? sh_ptr(dst) : buf_ptr(dst);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        uint4 b0, b1;                  // the destination operand as 8 fp32 bit patterns
+        if (kdin) {
+          b0 = ld16(dip + k * 1024, pol.ldd, pol.l1);
+          b1 = ld16(dip + k * 1024 + 16, pol.ldd, pol.l1);
+        } else {
+          const uint4 r = ld16(dip + k * 512, pol.ldd, pol.l1);
+          b0 = make_uint4(r.x << 16, r.x & 0xFFFF0000u, r.y << 16, r.y & 0xFFFF0000u);
+          b1 = make_uint4(r.z << 16, r.z & 0xFFFF0000u, r.w << 16, r.w & 0xFFFF0000u);
+        }
+        uint4 c0 = add_f32x4(b0, acc[2 * k]), c1 = add_f32x4(b1, acc[2 * k + 1]);
+        if (kdout) {
+          if (store) { char* dp = sh_ptr(dst); st16(dp + k * 1024, c0, pol); st16(dp + k * 1024 + 16, c1, pol); }
+        } else {                       // complete sum: one RNE rounding, to the rank buffer (and the stage)
+          uint4 o;
+          o.x = f32_to_bf16_rne(__uint_as_float(c0.x)) | (f32_to_bf16_rne(__uint_as_float(c0.y)) << 16);
+          o.y = f32_to_bf16_rne(__uint_as_float(c0.z)) | (f32_to_bf16_rne(__uint_as_float(c0.w)) << 16);
+          o.z = f32_to_bf16_rne(__uint_as_float(c1.x)) | (f32_to_bf16_rne(__uint_as_float(c1.y)) << 16);
+          o.w = f32_to_bf16_rne(__uint_as_float(c1.z)) | (f32_to_bf16_rne(__uint_as_float(c1.w)) << 16);
+          if (store) st16(buf_ptr(dst) + k * 512, o, pol);
+          if (staged) sts16(stage + (lane + k * 32) * 16, o);
+          c0 = make_uint4(o.x << 16, o.x & 0xFFFF0000u, o.y << 16, o.y & 0xFFFF0000u);   // what a load of it would return
+          c1 = make_uint4(o.z << 16, o.z & 0xFFFF0000u, o.w << 16, o.w & 0xFFFF0000u);
+        }
+        acc[2 * k] = c0;
+        acc[2 * k + 1] = c1;
+      }
+      if (staged) fence_proxy_async();
+      if ((fl & DFLOW_DEAD_SRC) && !(elide && (fl & DFLOW_SRC_FWD))) {
+        if (ksrc == 0u) { const char* sp = buf_ptr(src); for (int k = 0; k < 4; ++k) discard_line16(sp + k * 512, u0 + k * 32, uend); }
+        else { const char* sp = sh_ptr(src); for (int k = 0; k < 4; ++k) discard_line32(sp + k * 1024, u0 + k * 32, uend); }
+      }
+      __syncwarp();
+    }
+    cur = nxt;
+  }
+}
+
 template <int MODE, bool MASK_FWD = false>
 __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel(const __grid_constant__ ExecParams P) {
   if (tables_are_stale(P)) return;
@@ -883,11 +990,13 @@ __global__ void __launch_bounds__(COL_THREADS, CTAS_PER_SM) optcc_wcolumn_kernel
     const unsigned int fb = item.x, fe = item.y;
     const unsigned long long ubeg = (unsigned long long)item.z * P.tile_units, uend = ubeg + item.w;
     DFlow cur = load_record(P.flows + fb);
-    if (MASK_FWD && MODE == MODE_F32 && item.w == 128u && (ubeg + 128u) * P.unit_elems <= cur.len) {
-      // (a full tile inside the region: no ragged end, four vectors per lane.  The bf16 counterpart -- 32 carried
-      // registers per lane -- spilled 1 KB and was slower than the generic path, C3 1.47 vs 1.25 ms: not kept)
-      lean_item_f32(P, fb, fe, cur.off * 4 + ubeg * 16, lane, stage, pol, bulk_pol, ubeg + lane, ubeg + 128u,
-                    reinterpret_cast<uint4 (&)[4]>(carry));
+    if (MASK_FWD && !is_mask_mode(MODE) && item.w == 128u && (ubeg + 128u) * P.unit_elems <= cur.len) {
+      // (a full tile inside the region: no ragged end, four vectors / units per lane)
+      if (MODE == MODE_F32)
+        lean_item_f32(P, fb, fe, cur.off * 4 + ubeg * 16, lane, stage, pol, bulk_pol, ubeg + lane, ubeg + 128u,
+                      reinterpret_cast<uint4 (&)[4]>(carry));
+      else
+        lean_item_bf16(P, fb, fe, cur.off, ubeg, lane, stage, pol, bulk_pol, reinterpret_cast<uint4 (&)[8]>(carry));
       continue;
     }
     if (pf) prefetch_raw<MODE, 32>(P, cur, ubeg, item.w);
